@@ -1,0 +1,559 @@
+// ia_oracle.cpp - the ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+//
+// A plain, slow, obviously-correct CPU implementation of the interval-arithmetic helix vote of
+// arxiv 2401.04576, written from the paper before any CUDA kernel existed.  It shares
+// no code, header, table or constant with the CUDA path under paper_2401_04576_b200/csrc and is
+// never called by it.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference leg may load this library.
+//
+// What it computes (citations are PAPER.md line numbers; "S<n>"/"G<n>" are the step and reading
+// numbers of DESIGN.md, which restate SURVEY.md 8(c)):
+//   for every 5-D box  (xc, yc, R, z0, lambda)  and every hit (wire, |drift|):
+//     the interval extension of the stereo-generalised Apollonius residual, eq. (2)/(A.5a) L55,L180,
+//         f = (x_Ax - xc)^2 + (y_Ax - yc)^2 - (R + d_Ax)^2 ,   (R + d_Ax)^2 = radicand of (A.5b) L183
+//     with the angle Phi of (A.3b) taken from the second-order series (A.8a-d) L209-218,
+//     evaluated for both drift signs; the hit votes for the box iff 0 is in the enclosure for
+//     either sign (condition (4), L74-78).  votes[box] = number of hits that vote.
+//   top-K by (votes desc, index asc); refinement by 2^5 midpoint subdivision of the top-K boxes.
+//
+// Rounding: every interval primitive returns the tightest enclosure IEEE-754 allows: lower
+// endpoints rounded toward -inf, upper endpoints toward +inf.  The thread keeps the FPU in
+// FE_UPWARD while interval code runs and obtains round-down results through the identity
+//     RD(x op y) = -RU((-x) op y)            (op in {+, *, /};  x - y = x + (-y))
+// sqrt toward -inf switches the mode for that one instruction.  libm calls (sin, cos, atan2) are
+// made in FE_TONEAREST and widened by ELEM_PAD_ULPS ulps on each side with nextafter (glibc
+// documents <= 1 ulp for these; 4 leaves margin), then clamped to the mathematical range.
+// Build flags: -O2 -frounding-math -ffp-contract=off -fno-fast-math -fno-math-errno  (see build.py)
+//
+// Pins (tests/test_oracle_*.py, all -m "not gpu"):  P1 identity at the generated truth,
+// P3 containment, P4 axial closed form, P5 brute-force sampling, P6 inclusion isotonicity,
+// P8 series order, P9 independent round-to-nearest DAG anchor; primitives against exact
+// rational arithmetic.  Parity status: pinned (none of the functions here is "parity unpinned").
+
+#include <algorithm>
+#include <cfenv>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr int ELEM_PAD_ULPS = 4;
+
+// keep the optimiser from moving or folding a rounded operation
+template <class T> inline T opaque(T x) { asm volatile("" : "+x"(x)); return x; }
+
+struct UpMode {       // RAII: FE_UPWARD for the lifetime of the object
+  int saved;
+  UpMode() : saved(fegetround()) { fesetround(FE_UPWARD); }
+  ~UpMode() { fesetround(saved); }
+};
+struct NearestInUp {  // RAII: FE_TONEAREST inside an UpMode region
+  NearestInUp() { fesetround(FE_TONEAREST); }
+  ~NearestInUp() { fesetround(FE_UPWARD); }
+};
+
+// ---- directed scalar operations (mode must be FE_UPWARD) -------------------------------------
+template <class T> inline T up_add(T a, T b) { return opaque(opaque(a) + opaque(b)); }
+template <class T> inline T dn_add(T a, T b) { return -opaque(opaque(-a) - opaque(b)); }
+template <class T> inline T up_mul(T a, T b) { return opaque(opaque(a) * opaque(b)); }
+template <class T> inline T dn_mul(T a, T b) { return -opaque(opaque(-a) * opaque(b)); }
+template <class T> inline T up_div(T a, T b) { return opaque(opaque(a) / opaque(b)); }
+template <class T> inline T dn_div(T a, T b) { return -opaque(opaque(-a) / opaque(b)); }
+template <class T> inline T up_sqrt(T a) { return opaque(std::sqrt(opaque(a))); }
+template <class T> inline T dn_sqrt(T a) {
+  fesetround(FE_DOWNWARD);
+  T r = opaque(std::sqrt(opaque(a)));
+  fesetround(FE_UPWARD);
+  return r;
+}
+
+// ---- intervals ------------------------------------------------------------------------------
+template <class T> struct Iv { T lo, hi; };
+template <class T> inline Iv<T> thin(T x) { return {x, x}; }
+
+template <class T> inline Iv<T> iadd(Iv<T> a, Iv<T> b) { return {dn_add(a.lo, b.lo), up_add(a.hi, b.hi)}; }
+template <class T> inline Iv<T> isub(Iv<T> a, Iv<T> b) { return {dn_add(a.lo, -b.hi), up_add(a.hi, -b.lo)}; }
+template <class T> inline Iv<T> ineg(Iv<T> a) { return {-a.hi, -a.lo}; }
+template <class T> inline Iv<T> imul(Iv<T> a, Iv<T> b) {
+  T l = std::min(std::min(dn_mul(a.lo, b.lo), dn_mul(a.lo, b.hi)), std::min(dn_mul(a.hi, b.lo), dn_mul(a.hi, b.hi)));
+  T h = std::max(std::max(up_mul(a.lo, b.lo), up_mul(a.lo, b.hi)), std::max(up_mul(a.hi, b.lo), up_mul(a.hi, b.hi)));
+  return {l, h};
+}
+// exact scalar times interval
+template <class T> inline Iv<T> iscale(T c, Iv<T> a) {
+  if (c >= 0) return {dn_mul(c, a.lo), up_mul(c, a.hi)};
+  return {dn_mul(c, a.hi), up_mul(c, a.lo)};
+}
+template <class T> inline Iv<T> isqr(Iv<T> a) {
+  if (a.lo >= 0) return {dn_mul(a.lo, a.lo), up_mul(a.hi, a.hi)};
+  if (a.hi <= 0) return {dn_mul(a.hi, a.hi), up_mul(a.lo, a.lo)};
+  return {T(0), std::max(up_mul(a.lo, a.lo), up_mul(a.hi, a.hi))};
+}
+// a / b with b.lo > 0
+template <class T> inline Iv<T> idiv_pos(Iv<T> a, Iv<T> b) {
+  T l = a.lo >= 0 ? dn_div(a.lo, b.hi) : dn_div(a.lo, b.lo);
+  T h = a.hi >= 0 ? up_div(a.hi, b.lo) : up_div(a.hi, b.hi);
+  return {l, h};
+}
+template <class T> inline Iv<T> irecip_pos(Iv<T> b) { return {dn_div(T(1), b.hi), up_div(T(1), b.lo)}; }
+// sqrt of the non-negative part
+template <class T> inline Iv<T> isqrt(Iv<T> a) {
+  return {dn_sqrt(std::max(a.lo, T(0))), up_sqrt(std::max(a.hi, T(0)))};
+}
+template <class T> inline Iv<T> iclamp(Iv<T> a, T lo, T hi) { return {std::max(a.lo, lo), std::min(a.hi, hi)}; }
+
+// ---- elementary functions --------------------------------------------------------------------
+template <class T> inline T pad_dn(T x) {
+  for (int i = 0; i < ELEM_PAD_ULPS; ++i) x = std::nextafter(x, -std::numeric_limits<T>::infinity());
+  return x;
+}
+template <class T> inline T pad_up(T x) {
+  for (int i = 0; i < ELEM_PAD_ULPS; ++i) x = std::nextafter(x, std::numeric_limits<T>::infinity());
+  return x;
+}
+// libm in double, round-to-nearest; in FP32 mode the double result is converted (rn) to float
+template <class T> inline T el_sin(T x) { return T(std::sin(double(x))); }
+template <class T> inline T el_cos(T x) { return T(std::cos(double(x))); }
+template <class T> inline T el_atan2(T y, T x) { return T(std::atan2(double(y), double(x))); }
+
+template <class T> struct PiC;   // outward-rounded bounds of pi and pi/2 in T
+template <> struct PiC<double> {
+  static constexpr double PI_LO = 0x1.921fb54442d18p+1, PI_HI = 0x1.921fb54442d19p+1;
+  static constexpr double PIO2_LO = 0x1.921fb54442d18p+0, PIO2_HI = 0x1.921fb54442d19p+0;
+};
+template <> struct PiC<float> {
+  static constexpr float PI_LO = 0x1.921fb4p+1f, PI_HI = 0x1.921fb6p+1f;
+  static constexpr float PIO2_LO = 0x1.921fb4p+0f, PIO2_HI = 0x1.921fb6p+0f;
+};
+
+// enclosure of sin over e.  Outside [-4,4] (or NaN) -> [-1,1].  Inside [-4,4] the only interior
+// critical points are +pi/2 (max) and -pi/2 (min).
+template <class T> inline Iv<T> isin(Iv<T> e) {
+  if (!(e.lo >= T(-4) && e.hi <= T(4))) return {T(-1), T(1)};
+  NearestInUp rn;
+  T a = el_sin(e.lo), b = el_sin(e.hi);
+  Iv<T> r = {pad_dn(std::min(a, b)), pad_up(std::max(a, b))};
+  if (e.lo <= PiC<T>::PIO2_HI && e.hi >= PiC<T>::PIO2_LO) r.hi = T(1);
+  if (e.lo <= -PiC<T>::PIO2_LO && e.hi >= -PiC<T>::PIO2_HI) r.lo = T(-1);
+  return iclamp(r, T(-1), T(1));
+}
+// enclosure of cos over e: interior critical points in [-4,4] are 0 (max) and +-pi (min).
+template <class T> inline Iv<T> icos(Iv<T> e) {
+  if (!(e.lo >= T(-4) && e.hi <= T(4))) return {T(-1), T(1)};
+  NearestInUp rn;
+  T a = el_cos(e.lo), b = el_cos(e.hi);
+  Iv<T> r = {pad_dn(std::min(a, b)), pad_up(std::max(a, b))};
+  if (e.lo <= T(0) && e.hi >= T(0)) r.hi = T(1);
+  if (e.lo <= PiC<T>::PI_HI && e.hi >= PiC<T>::PI_LO) r.lo = T(-1);
+  if (e.lo <= -PiC<T>::PI_LO && e.hi >= -PiC<T>::PI_HI) r.lo = T(-1);
+  return iclamp(r, T(-1), T(1));
+}
+// enclosure of atan2(y, x) over the rectangle y x x.  The angle is monotone along every edge of a
+// rectangle that avoids the cut (negative x axis) and the origin, so the extremes are at corners.
+template <class T> inline Iv<T> iatan2(Iv<T> y, Iv<T> x) {
+  if (x.lo <= T(0) && y.lo <= T(0) && y.hi >= T(0)) return {-PiC<T>::PI_HI, PiC<T>::PI_HI};
+  NearestInUp rn;
+  T c0 = el_atan2(y.lo, x.lo), c1 = el_atan2(y.lo, x.hi), c2 = el_atan2(y.hi, x.lo), c3 = el_atan2(y.hi, x.hi);
+  Iv<T> r = {pad_dn(std::min(std::min(c0, c1), std::min(c2, c3))), pad_up(std::max(std::max(c0, c1), std::max(c2, c3)))};
+  return iclamp(r, -PiC<T>::PI_HI, PiC<T>::PI_HI);
+}
+
+// ---- inputs ---------------------------------------------------------------------------------
+struct OrcWire { double x0, y0, sin_phi_s, cos_phi_s, tan_tau; };   // (A.1a,b) L147-152
+struct OrcHit { int32_t wire; int32_t pad; double drift; };         // |d_St| measured, L88
+struct OrcParams { double tol, x_ref, y_ref, z_ref; int32_t precision; uint32_t flags; };
+
+// per-hit scalars, computed once in round-to-nearest and then taken as exact (G-scalars)
+template <class T> struct HitC {
+  T xA, yA;        // (A.4d,e) L174-176: wire point in the plane z = z_ref
+  T sphi, cphi, Tn;
+  T k0, kx, ky;    // S3: cross term  k0 + ky*X + kx*Y
+  T mx, my, h2;    // S3: dot term   (X-mx)^2 + (Y-my)^2 - h2
+  T d, tol, zref;
+};
+
+template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const OrcParams& p) {
+  // round-to-nearest, unfused.  In FP32 mode every scalar input is first converted to float.
+  HitC<T> c;
+  T x0 = T(w.x0), y0 = T(w.y0), s = T(w.sin_phi_s), co = T(w.cos_phi_s), t = T(w.tan_tau);
+  T xr = T(p.x_ref), yr = T(p.y_ref), zr = T(p.z_ref);
+  c.sphi = s; c.cphi = co; c.Tn = t;
+  c.xA = opaque(x0 + opaque(opaque(zr * s) * t));
+  c.yA = opaque(y0 - opaque(opaque(zr * co) * t));
+  c.k0 = opaque(opaque(xr * c.yA) - opaque(yr * c.xA));
+  c.ky = opaque(yr - c.yA);
+  c.kx = opaque(c.xA - xr);
+  c.mx = opaque(T(0.5) * opaque(xr + c.xA));
+  c.my = opaque(T(0.5) * opaque(yr + c.yA));
+  T hx = opaque(T(0.5) * opaque(c.xA - xr)), hy = opaque(T(0.5) * opaque(c.yA - yr));
+  c.h2 = opaque(opaque(hx * hx) + opaque(hy * hy));
+  c.d = T(h.drift); c.tol = T(p.tol); c.zref = zr;
+  return c;
+}
+
+template <class T> struct Box { Iv<T> X, Y, R, Z, L; };
+
+struct Resid { double flo, fhi, scale; bool decided_vote; };   // decided_vote: domain rule forced a vote
+
+// S1-S8 for one (box, hit, drift sign).  Mode must be FE_UPWARD.  sign = +1 / -1.
+template <class T> Resid residual(const Box<T>& b, const HitC<T>& c, int sign) {
+  const T one = T(1), two = T(2), half = T(0.5);
+  // S1 drift interval, tolerance applied on d_St before delta = d/u (G6)
+  Iv<T> D = {std::max(dn_add(c.d, -c.tol), T(0)), up_add(c.d, c.tol)};
+  if (sign < 0) D = ineg(D);
+  // S2 transverse part (A.7a,d,e) L191-201
+  Iv<T> A = isub(thin(c.xA), b.X), B = isub(thin(c.yA), b.Y);
+  Iv<T> Q = iadd(isqr(A), isqr(B));
+  Iv<T> cA = isub(iscale(c.sphi, A), iscale(c.cphi, B));
+  Iv<T> sA = iadd(iscale(c.cphi, A), iscale(c.sphi, B));
+  // S3' domain rule: the xy cell may contain the wire point -> cannot exclude (G15)
+  if (!(Q.lo > T(0))) return {0.0, 0.0, double(Q.hi), true};
+  // S3 turning angle phi_Ax - phi0 (1d) L49, (A.7f) L203, as one atan2(cross, dot) (G8)
+  Iv<T> cr = iadd(iadd(thin(c.k0), iscale(c.ky, b.X)), iscale(c.kx, b.Y));
+  Iv<T> dt = isub(iadd(isqr(isub(b.X, thin(c.mx))), isqr(isub(b.Y, thin(c.my)))), thin(c.h2));
+  Iv<T> dphi = iatan2(cr, dt);
+  // S3' (A.7a,g)
+  Iv<T> iQ = irecip_pos(Q);
+  Iv<T> RA = isqrt(Q);
+  Iv<T> iR = irecip_pos(RA);
+  Iv<T> c2 = imul(isub(isqr(cA), isqr(sA)), iQ);        // cos 2Phi_Ax
+  Iv<T> s2 = imul(iscale(two, imul(sA, cA)), iQ);       // sin 2Phi_Ax
+  // S4 series (A.8a-d) L211-218
+  Iv<T> Zr = isub(b.Z, thin(c.zref));
+  Iv<T> LR = imul(b.L, b.R);
+  Iv<T> zA = iadd(Zr, imul(LR, dphi));                  // (A.8d)
+  Iv<T> LD = imul(b.L, D);
+  Iv<T> P1 = ineg(imul(iadd(imul(zA, sA), imul(LD, cA)), iQ));                         // (A.8b)
+  Iv<T> t1 = imul(LR, zA);
+  Iv<T> t2 = imul(imul(imul(b.L, zA), isub(b.R, iscale(two, D))), c2);
+  Iv<T> t3 = imul(iadd(isqr(zA), imul(D, iadd(RA, imul(isqr(b.L), isub(iadd(b.R, RA), D))))), s2);
+  Iv<T> P2 = iscale(half, imul(iadd(isub(t1, t2), t3), iQ));                           // (A.8c)
+  Iv<T> T2 = isqr(thin(c.Tn));
+  Iv<T> e = iadd(iscale(c.Tn, P1), imul(T2, P2));       // Phi - Phi_Ax  (A.8a)
+  // S5 trig of Phi = Phi_Ax + e  (A.3b), (A.7g)
+  Iv<T> se = isin(e), ce = icos(e);
+  Iv<T> sinP = iclamp(imul(iadd(imul(sA, ce), imul(cA, se)), iR), T(-1), one);
+  Iv<T> cosP = iclamp(imul(isub(imul(cA, ce), imul(sA, se)), iR), T(-1), one);
+  // S6 drift-line norm (A.3a) L160 and delta = d_St / u_d
+  Iv<T> u2 = iadd(iadd(iadd(thin(one), iscale(opaque(two * c.Tn), imul(b.L, sinP))), imul(T2, isqr(b.L))),
+                  imul(T2, isqr(cosP)));
+  Iv<T> u = isqrt(u2);
+  if (!(u.lo > T(0))) return {0.0, 0.0, double(Q.hi), true};
+  Iv<T> dl = idiv_pos(D, u);
+  // S7 z of the wire point (A.4c) L172 with s_perp = R (dphi + e);  c^tau (A.7b) L194
+  Iv<T> z = isub(iadd(Zr, imul(LR, iadd(dphi, e))), iscale(c.Tn, imul(dl, cosP)));
+  Iv<T> Ld = imul(b.L, dl);
+  Iv<T> ct = isub(imul(z, cA), imul(Ld, sA));
+  // S8 (R + d_Ax)^2 = radicand of (A.5b) L183;  f = R_Ax^2 - (R + d_Ax)^2  (A.5a) L180
+  Iv<T> rad = isub(isub(isub(isqr(iadd(b.R, dl)), iscale(opaque(two * c.Tn), ct)), isqr(iscale(c.Tn, z))),
+                   isqr(iscale(c.Tn, Ld)));
+  Iv<T> f = isub(Q, rad);
+  double sc = std::max(double(Q.hi), std::max(std::fabs(double(rad.lo)), std::fabs(double(rad.hi))));
+  return {double(f.lo), double(f.hi), sc, false};
+}
+
+inline bool votes_yes(const Resid& r) { return r.decided_vote || !(r.flo > 0.0 || r.fhi < 0.0); }
+
+// one hit, one box: vote iff either drift sign cannot be excluded (G7: at most one vote per hit)
+template <class T> bool hit_votes(const Box<T>& b, const HitC<T>& c) {
+  return votes_yes(residual(b, c, +1)) || votes_yes(residual(b, c, -1));
+}
+
+// outward conversion of a double box edge to T
+template <class T> inline T cvt_dn(double x);
+template <class T> inline T cvt_up(double x);
+template <> inline double cvt_dn<double>(double x) { return x; }
+template <> inline double cvt_up<double>(double x) { return x; }
+template <> inline float cvt_dn<float>(double x) {
+  float f = float(x);   // any mode: fix up explicitly
+  if (double(f) > x) f = std::nextafter(f, -std::numeric_limits<float>::infinity());
+  return f;
+}
+template <> inline float cvt_up<float>(double x) {
+  float f = float(x);
+  if (double(f) < x) f = std::nextafter(f, std::numeric_limits<float>::infinity());
+  return f;
+}
+template <class T> Box<T> make_box(const double lo[5], const double hi[5]) {
+  Box<T> b;
+  b.X = {cvt_dn<T>(lo[0]), cvt_up<T>(hi[0])};
+  b.Y = {cvt_dn<T>(lo[1]), cvt_up<T>(hi[1])};
+  b.R = {cvt_dn<T>(lo[2]), cvt_up<T>(hi[2])};
+  b.Z = {cvt_dn<T>(lo[3]), cvt_up<T>(hi[3])};
+  b.L = {cvt_dn<T>(lo[4]), cvt_up<T>(hi[4])};
+  return b;
+}
+
+// cell edges e_k = lo + k*((hi-lo)/n), e_n = hi : round-to-nearest, unfused (S9, G14)
+std::vector<double> edges(double lo, double hi, int n) {
+  std::vector<double> e(n + 1);
+  double w = opaque(opaque(hi - lo) / double(n));
+  for (int k = 0; k < n; ++k) e[k] = opaque(lo + opaque(double(k) * w));
+  e[n] = hi;
+  return e;
+}
+
+enum { ORC_OK = 0, ORC_ERR_ARG = -1, ORC_ERR_GEOMETRY = -2, ORC_ERR_DOMAIN = -3 };
+
+int check_domain(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, double Rlo, double Llo, double Lhi) {
+  double tmax = 0;
+  for (int i = 0; i < n_hits; ++i) {
+    if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+    if (!(hits[i].drift >= 0)) return ORC_ERR_ARG;
+    tmax = std::max(tmax, std::fabs(wires[hits[i].wire].tan_tau));
+  }
+  if (!(Rlo > 0)) return ORC_ERR_DOMAIN;
+  if (!(std::max(std::fabs(Llo), std::fabs(Lhi)) * tmax < 0.5)) return ORC_ERR_DOMAIN;
+  return ORC_OK;
+}
+
+template <class T> std::vector<HitC<T>> stage_hits(const OrcWire* wires, const OrcHit* hits, int n_hits, const OrcParams& p) {
+  std::vector<HitC<T>> hc(n_hits);
+  for (int i = 0; i < n_hits; ++i) hc[i] = make_hitc<T>(wires[hits[i].wire], hits[i], p);
+  return hc;
+}
+
+template <class T>
+void vote_boxes_T(const std::vector<HitC<T>>& hc, const double* blo, const double* bhi, int64_t n_boxes, uint16_t* out) {
+#pragma omp parallel
+  {
+    UpMode up;
+#pragma omp for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n_boxes; ++i) {
+      Box<T> b = make_box<T>(blo + 5 * i, bhi + 5 * i);
+      unsigned v = 0;
+      for (const auto& c : hc) v += hit_votes(b, c) ? 1u : 0u;
+      out[i] = uint16_t(v);
+    }
+  }
+}
+
+struct Grid {
+  std::vector<double> e[5];
+  int n[5];
+  Grid(const double lo[5], const double hi[5], const int32_t dims[5]) {
+    for (int d = 0; d < 5; ++d) { n[d] = dims[d]; e[d] = edges(lo[d], hi[d], dims[d]); }
+  }
+  int64_t cells() const { int64_t c = 1; for (int d = 0; d < 5; ++d) c *= n[d]; return c; }
+  // linear index ((((ix*ny+iy)*nR+iR)*nz+iz)*nl+il): lambda fastest (S9)
+  void cell(int64_t idx, double lo[5], double hi[5]) const {
+    for (int d = 4; d >= 0; --d) { int k = int(idx % n[d]); idx /= n[d]; lo[d] = e[d][k]; hi[d] = e[d][k + 1]; }
+  }
+};
+
+template <class T>
+void vote_cells_T(const std::vector<HitC<T>>& hc, const Grid& g, const int64_t* cell_idx, int64_t n, uint16_t* out) {
+#pragma omp parallel
+  {
+    UpMode up;
+#pragma omp for schedule(dynamic, 256)
+    for (int64_t i = 0; i < n; ++i) {
+      double lo[5], hi[5];
+      g.cell(cell_idx ? cell_idx[i] : i, lo, hi);
+      Box<T> b = make_box<T>(lo, hi);
+      unsigned v = 0;
+      for (const auto& c : hc) v += hit_votes(b, c) ? 1u : 0u;
+      out[i] = uint16_t(v);
+    }
+  }
+}
+
+// key order: votes descending, index ascending (S9, G16)
+void topk_plain(const uint16_t* votes, int64_t n, int k, int64_t* idx_out, uint16_t* votes_out) {
+  std::vector<int64_t> idx(n);
+  for (int64_t i = 0; i < n; ++i) idx[i] = i;
+  auto better = [&](int64_t a, int64_t b) { return votes[a] != votes[b] ? votes[a] > votes[b] : a < b; };
+  std::partial_sort(idx.begin(), idx.begin() + k, idx.end(), better);
+  for (int i = 0; i < k; ++i) { idx_out[i] = idx[i]; votes_out[i] = votes[idx[i]]; }
+}
+
+struct OrcBox { double lo[5], hi[5]; uint16_t votes; uint16_t pad[3]; };
+
+template <class T>
+int refine_T(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams& p,
+             const double lo[5], const double hi[5], const int32_t grid0[5], int levels, int k,
+             OrcBox* boxes_out, double* params_out) {
+  auto hc = stage_hits<T>(wires, hits, n_hits, p);
+  Grid g(lo, hi, grid0);
+  int64_t n0 = g.cells();
+  if (k > n0) return ORC_ERR_ARG;
+  std::vector<uint16_t> votes(n0);
+  vote_cells_T<T>(hc, g, nullptr, n0, votes.data());
+  std::vector<int64_t> idx(k);
+  std::vector<uint16_t> kv(k);
+  topk_plain(votes.data(), n0, k, idx.data(), kv.data());
+  std::vector<OrcBox> cur(k);
+  for (int r = 0; r < k; ++r) { g.cell(idx[r], cur[r].lo, cur[r].hi); cur[r].votes = kv[r]; std::memset(cur[r].pad, 0, sizeof cur[r].pad); }
+  std::copy(cur.begin(), cur.end(), boxes_out);
+  for (int lev = 1; lev < levels; ++lev) {
+    // children: list index rank*32 + c; bit (4-dim) of c set -> upper half [mid, hi]; mid = 0.5*(lo+hi) rn (S9, G18)
+    int64_t nc = int64_t(k) * 32;
+    std::vector<double> clo(nc * 5), chi(nc * 5);
+    for (int r = 0; r < k; ++r)
+      for (int c = 0; c < 32; ++c)
+        for (int d = 0; d < 5; ++d) {
+          double mid = opaque(0.5 * opaque(cur[r].lo[d] + cur[r].hi[d]));
+          bool upper = (c >> (4 - d)) & 1;
+          clo[(r * 32 + c) * 5 + d] = upper ? mid : cur[r].lo[d];
+          chi[(r * 32 + c) * 5 + d] = upper ? cur[r].hi[d] : mid;
+        }
+    std::vector<uint16_t> cv(nc);
+    vote_boxes_T<T>(hc, clo.data(), chi.data(), nc, cv.data());
+    topk_plain(cv.data(), nc, k, idx.data(), kv.data());
+    for (int r = 0; r < k; ++r) {
+      for (int d = 0; d < 5; ++d) { cur[r].lo[d] = clo[idx[r] * 5 + d]; cur[r].hi[d] = chi[idx[r] * 5 + d]; }
+      cur[r].votes = kv[r];
+    }
+    // idx refers to the previous cur; write after all reads (clo/chi are copies, so this is safe)
+    std::copy(cur.begin(), cur.end(), boxes_out + int64_t(lev) * k);
+  }
+  // value = centre, error = half-width of the rank-0 box of the last pass (L94, G19)
+  for (int d = 0; d < 5; ++d) {
+    params_out[d] = opaque(0.5 * opaque(cur[0].lo[d] + cur[0].hi[d]));
+    params_out[5 + d] = opaque(0.5 * opaque(cur[0].hi[d] - cur[0].lo[d]));
+  }
+  return ORC_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI (ctypes)
+// =============================================================================================
+extern "C" {
+
+int orc_pad_ulps() { return ELEM_PAD_ULPS; }
+int orc_max_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#endif
+}
+
+// interval primitive on doubles or floats (prec 64/32), for the primitive pins.
+// op: 0 add 1 sub 2 mul 3 sqr(a) 4 div_pos 5 sqrt(a) 6 sin(a) 7 cos(a) 8 atan2(a=y,b=x) 9 recip_pos(a) 10 scale(c=b.lo, a)
+int orc_prim(int op, int prec, double alo, double ahi, double blo, double bhi, double* out) {
+  UpMode up;
+  auto run = [&](auto tag) -> int {
+    using T = decltype(tag);
+    Iv<T> a = {T(alo), T(ahi)}, b = {T(blo), T(bhi)}, r{};
+    switch (op) {
+      case 0: r = iadd(a, b); break;
+      case 1: r = isub(a, b); break;
+      case 2: r = imul(a, b); break;
+      case 3: r = isqr(a); break;
+      case 4: r = idiv_pos(a, b); break;
+      case 5: r = isqrt(a); break;
+      case 6: r = isin(a); break;
+      case 7: r = icos(a); break;
+      case 8: r = iatan2(a, b); break;
+      case 9: r = irecip_pos(a); break;
+      case 10: r = iscale(T(blo), a); break;
+      default: return ORC_ERR_ARG;
+    }
+    out[0] = double(r.lo); out[1] = double(r.hi);
+    return int(ORC_OK);
+  };
+  return prec == 32 ? run(float()) : run(double());
+}
+
+// f enclosure for every (box, hit, sign): out[((i*n_hits + h)*2 + s)*4 + {0,1,2,3}] = f.lo, f.hi, scale, decided
+// sign index 0 = +, 1 = -.
+int orc_residual(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p,
+                 const double* blo, const double* bhi, int64_t n_boxes, double* out) {
+  if (!wires || !hits || !p || !blo || !bhi || !out || n_hits < 0 || n_boxes < 0) return ORC_ERR_ARG;
+  for (int i = 0; i < n_hits; ++i) if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+  auto run = [&](auto tag) {
+    using T = decltype(tag);
+    auto hc = stage_hits<T>(wires, hits, n_hits, *p);
+    UpMode up;
+    for (int64_t i = 0; i < n_boxes; ++i) {
+      Box<T> b = make_box<T>(blo + 5 * i, bhi + 5 * i);
+      for (int h = 0; h < n_hits; ++h)
+        for (int s = 0; s < 2; ++s) {
+          Resid r = residual(b, hc[h], s == 0 ? +1 : -1);
+          double* o = out + ((i * n_hits + h) * 2 + s) * 4;
+          o[0] = r.flo; o[1] = r.fhi; o[2] = r.scale; o[3] = r.decided_vote ? 1.0 : 0.0;
+        }
+    }
+  };
+  if (p->precision == 32) run(float()); else run(double());
+  return ORC_OK;
+}
+
+int orc_vote_boxes(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p,
+                   const double* blo, const double* bhi, int64_t n_boxes, uint16_t* votes_out) {
+  if (!wires || !hits || !p || !blo || !bhi || !votes_out || n_hits < 0 || n_boxes < 0) return ORC_ERR_ARG;
+  for (int i = 0; i < n_hits; ++i) if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+  if (p->precision == 32) vote_boxes_T<float>(stage_hits<float>(wires, hits, n_hits, *p), blo, bhi, n_boxes, votes_out);
+  else vote_boxes_T<double>(stage_hits<double>(wires, hits, n_hits, *p), blo, bhi, n_boxes, votes_out);
+  return ORC_OK;
+}
+
+// dense grid; cell_idx == NULL: all prod(dims) cells in linear order, else the listed cells only
+int orc_vote(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p,
+             const double* lo, const double* hi, const int32_t* dims, const int64_t* cell_idx, int64_t n_idx,
+             uint16_t* votes_out) {
+  if (!wires || !hits || !p || !lo || !hi || !dims || !votes_out || n_hits < 0) return ORC_ERR_ARG;
+  for (int d = 0; d < 5; ++d) if (dims[d] <= 0 || !(hi[d] > lo[d])) return ORC_ERR_ARG;
+  int rc = check_domain(wires, n_wires, hits, n_hits, lo[2], lo[4], hi[4]);
+  if (rc) return rc;
+  Grid g(lo, hi, dims);
+  int64_t n = cell_idx ? n_idx : g.cells();
+  if (cell_idx) for (int64_t i = 0; i < n; ++i) if (cell_idx[i] < 0 || cell_idx[i] >= g.cells()) return ORC_ERR_ARG;
+  if (p->precision == 32) vote_cells_T<float>(stage_hits<float>(wires, hits, n_hits, *p), g, cell_idx, n, votes_out);
+  else vote_cells_T<double>(stage_hits<double>(wires, hits, n_hits, *p), g, cell_idx, n, votes_out);
+  return ORC_OK;
+}
+
+// boxes of listed dense cells (host plumbing for tests)
+int orc_cell_boxes(const double* lo, const double* hi, const int32_t* dims, const int64_t* cell_idx, int64_t n,
+                   double* blo, double* bhi) {
+  Grid g(lo, hi, dims);
+  for (int64_t i = 0; i < n; ++i) g.cell(cell_idx[i], blo + 5 * i, bhi + 5 * i);
+  return ORC_OK;
+}
+
+int orc_topk(const uint16_t* votes, int64_t n, int k, int64_t* idx_out, uint16_t* votes_out) {
+  if (!votes || !idx_out || !votes_out || k <= 0 || k > n) return ORC_ERR_ARG;
+  topk_plain(votes, n, k, idx_out, votes_out);
+  return ORC_OK;
+}
+
+int orc_refine(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p,
+               const double* lo, const double* hi, const int32_t* grid0, int levels, int k,
+               OrcBox* boxes_out, double* params_out) {
+  if (!wires || !hits || !p || !lo || !hi || !grid0 || !boxes_out || !params_out || levels < 1 || k < 1) return ORC_ERR_ARG;
+  for (int d = 0; d < 5; ++d) if (grid0[d] <= 0 || !(hi[d] > lo[d])) return ORC_ERR_ARG;
+  int rc = check_domain(wires, n_wires, hits, n_hits, lo[2], lo[4], hi[4]);
+  if (rc) return rc;
+  if (p->precision == 32) return refine_T<float>(wires, n_wires, hits, n_hits, *p, lo, hi, grid0, levels, k, boxes_out, params_out);
+  return refine_T<double>(wires, n_wires, hits, n_hits, *p, lo, hi, grid0, levels, k, boxes_out, params_out);
+}
+
+// events in CSR: hits of event e are hits[hit_offsets[e] .. hit_offsets[e+1])
+int orc_refine_batch(const OrcWire* wires, int n_wires, const OrcHit* hits, const int32_t* hit_offsets, int n_events,
+                     const OrcParams* p, const double* lo, const double* hi, const int32_t* grid0, int levels, int k,
+                     OrcBox* boxes_out, double* params_out) {
+  if (!hit_offsets || n_events < 0) return ORC_ERR_ARG;
+  for (int e = 0; e < n_events; ++e) {
+    int rc = orc_refine(wires, n_wires, hits + hit_offsets[e], hit_offsets[e + 1] - hit_offsets[e], p, lo, hi, grid0,
+                        levels, k, boxes_out + int64_t(e) * levels * k, params_out + int64_t(e) * 10);
+    if (rc) return rc;
+  }
+  return ORC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,159 @@
+"""ctypes binding of the oracle library (TEST INFRASTRUCTURE ONLY - see ia_oracle.cpp).
+
+Argument marshalling only; every computation is in ia_oracle.cpp.  Arrays are numpy on the host.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+WIRE_DT = np.dtype([("x0", "f8"), ("y0", "f8"), ("sin_phi_s", "f8"), ("cos_phi_s", "f8"), ("tan_tau", "f8")])
+HIT_DT = np.dtype([("wire", "i4"), ("pad", "i4"), ("drift", "f8")])
+BOX_DT = np.dtype([("lo", "f8", (5,)), ("hi", "f8", (5,)), ("votes", "u2"), ("pad", "u2", (3,))])
+
+
+class Params(C.Structure):
+    _fields_ = [("tol", C.c_double), ("x_ref", C.c_double), ("y_ref", C.c_double), ("z_ref", C.c_double),
+                ("precision", C.c_int32), ("flags", C.c_uint32)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        _lib = C.CDLL(path)
+        for name in ("orc_prim", "orc_residual", "orc_vote_boxes", "orc_vote", "orc_cell_boxes", "orc_topk",
+                     "orc_refine", "orc_refine_batch", "orc_pad_ulps", "orc_max_threads"):
+            getattr(_lib, name).restype = C.c_int
+        _lib.orc_set_threads.restype = None
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed: rc={rc}")
+
+
+def make_params(tol, x_ref=0.0, y_ref=0.0, z_ref=0.0, precision=64) -> Params:
+    return Params(tol, x_ref, y_ref, z_ref, precision, 0)
+
+
+def wires_of(chamber) -> np.ndarray:
+    w = np.zeros(chamber.n_wires, WIRE_DT)
+    w["x0"], w["y0"] = chamber.x0, chamber.y0
+    w["sin_phi_s"], w["cos_phi_s"], w["tan_tau"] = chamber.sin_phi_s, chamber.cos_phi_s, chamber.tan_tau
+    return w
+
+
+def hits_of(wire_ids, drifts) -> np.ndarray:
+    h = np.zeros(len(wire_ids), HIT_DT)
+    h["wire"], h["drift"] = wire_ids, drifts
+    return h
+
+
+def set_threads(n: int):
+    lib().orc_set_threads(int(n))
+
+
+def max_threads() -> int:
+    return lib().orc_max_threads()
+
+
+def pad_ulps() -> int:
+    return lib().orc_pad_ulps()
+
+
+def prim(op: int, a, b=(0.0, 0.0), prec: int = 64):
+    out = (C.c_double * 2)()
+    _chk(lib().orc_prim(op, prec, C.c_double(a[0]), C.c_double(a[1]), C.c_double(b[0]), C.c_double(b[1]), out), "prim")
+    return out[0], out[1]
+
+
+def residual(wires, hits, params: Params, blo, bhi) -> np.ndarray:
+    """f enclosures [n_boxes, n_hits, 2 signs (+,-), 4 = (f.lo, f.hi, scale, decided)]."""
+    blo = np.ascontiguousarray(blo, np.float64).reshape(-1, 5)
+    bhi = np.ascontiguousarray(bhi, np.float64).reshape(-1, 5)
+    out = np.zeros((blo.shape[0], len(hits), 2, 4))
+    _chk(lib().orc_residual(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), _p(blo), _p(bhi),
+                            C.c_int64(blo.shape[0]), _p(out)), "residual")
+    return out
+
+
+def vote_boxes(wires, hits, params: Params, blo, bhi) -> np.ndarray:
+    blo = np.ascontiguousarray(blo, np.float64).reshape(-1, 5)
+    bhi = np.ascontiguousarray(bhi, np.float64).reshape(-1, 5)
+    out = np.zeros(blo.shape[0], np.uint16)
+    _chk(lib().orc_vote_boxes(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), _p(blo), _p(bhi),
+                              C.c_int64(blo.shape[0]), _p(out)), "vote_boxes")
+    return out
+
+
+def vote(wires, hits, params: Params, lo, hi, dims, cell_idx=None) -> np.ndarray:
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    if cell_idx is None:
+        n = int(np.prod(dims.astype(np.int64)))
+        idx_p, n_idx = None, 0
+    else:
+        cell_idx = np.ascontiguousarray(cell_idx, np.int64)
+        n = len(cell_idx)
+        idx_p, n_idx = _p(cell_idx), n
+    out = np.zeros(n, np.uint16)
+    _chk(lib().orc_vote(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), _p(lo), _p(hi), _p(dims),
+                        idx_p, C.c_int64(n_idx), _p(out)), "vote")
+    return out
+
+
+def cell_boxes(lo, hi, dims, cell_idx):
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    cell_idx = np.ascontiguousarray(cell_idx, np.int64)
+    blo = np.zeros((len(cell_idx), 5))
+    bhi = np.zeros((len(cell_idx), 5))
+    _chk(lib().orc_cell_boxes(_p(lo), _p(hi), _p(dims), _p(cell_idx), C.c_int64(len(cell_idx)), _p(blo), _p(bhi)),
+         "cell_boxes")
+    return blo, bhi
+
+
+def topk(votes, k: int):
+    votes = np.ascontiguousarray(votes, np.uint16)
+    idx = np.zeros(k, np.int64)
+    v = np.zeros(k, np.uint16)
+    _chk(lib().orc_topk(_p(votes), C.c_int64(len(votes)), k, _p(idx), _p(v)), "topk")
+    return idx, v
+
+
+def refine(wires, hits, params: Params, lo, hi, grid0, levels: int, k: int):
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    grid0 = np.ascontiguousarray(grid0, np.int32)
+    boxes = np.zeros((levels, k), BOX_DT)
+    par = np.zeros(10)
+    _chk(lib().orc_refine(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), _p(lo), _p(hi), _p(grid0),
+                          levels, k, _p(boxes), _p(par)), "refine")
+    return boxes, par
+
+
+def refine_batch(wires, hits, hit_offsets, params: Params, lo, hi, grid0, levels: int, k: int):
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    grid0 = np.ascontiguousarray(grid0, np.int32)
+    hit_offsets = np.ascontiguousarray(hit_offsets, np.int32)
+    n_ev = len(hit_offsets) - 1
+    boxes = np.zeros((n_ev, levels, k), BOX_DT)
+    par = np.zeros((n_ev, 10))
+    _chk(lib().orc_refine_batch(_p(wires), len(wires), _p(hits), _p(hit_offsets), n_ev, C.byref(params), _p(lo),
+                                _p(hi), _p(grid0), levels, k, _p(boxes), _p(par)), "refine_batch")
+    return boxes, par
