@@ -1,0 +1,170 @@
+/* ia.h - C ABI of libia_b200: the interval-arithmetic helix vote of arxiv 2401.04576 on one B200.
+ *
+ * Citations "L<n>" are line numbers of the paper text; "S<n>"/"G<n>" are the step and
+ * reading numbers of DESIGN.md.
+ *
+ * The method (section 3.1): the 5-D helix parameter space (xc, yc, R, z0, lambda)
+ * is tiled into interval boxes; a drift-distance hit votes for a box iff 0 lies in the interval
+ * extension of the stereo-generalised Apollonius residual, eq. (2)/(A.5a) with d_Ax of (A.5b) and
+ * Phi from the series (A.8a-d), for either drift sign (condition (4), L74-78).  The boxes with the
+ * most votes are kept (L94) and, per BASELINE, subdivided into 2^5 children and voted again.
+ *
+ * Conventions
+ *   - extern "C"; no exception crosses the boundary; every call returns IA_OK (0) or a negative
+ *     IA_ERR_* code; ia_strerror() names it, ia_last_cuda_error() gives the CUDA error behind
+ *     IA_ERR_CUDA.
+ *   - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors'
+ *     data_ptr()); pointers named *_host, the 5-element box/grid arrays, ia_wire[] and ia_params
+ *     are HOST memory.  Nothing is retained after the call returns except what the context copies.
+ *   - Calls enqueue work on the context's CUDA stream and do NOT synchronise; results are valid
+ *     after the caller synchronises that stream.  The *_host entry points copy in and out with
+ *     cudaMemcpyAsync on the same stream and DO synchronise before returning.
+ *   - Errors that only the device can see (a hit naming an unknown wire) do not fail the call:
+ *     the hit is dropped (it never votes) and a sticky flag is raised that ia_device_status()
+ *     reads (it synchronises).  The *_host entry points validate hits on the host instead.
+ *   - The library allocates device memory only inside the context (geometry, staged hits, child
+ *     boxes, partial top-K lists, vote scratch) and frees it in ia_destroy().  No global state,
+ *     no CPU fallback: every step below runs in CUDA kernels compiled for sm_100a.
+ *   - Units: cm and rad.  Order of the five axes everywhere: xc, yc, R, z0, lambda.
+ */
+#ifndef IA_B200_H
+#define IA_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  IA_OK = 0,
+  IA_ERR_ARG = -1,      /* null pointer, non-positive size, hi <= lo, k > number of cells ...       */
+  IA_ERR_GEOMETRY = -2, /* no geometry loaded, or (host entry points) a hit names an unknown wire  */
+  IA_ERR_DOMAIN = -3,   /* R.lo <= 0, or max|lambda| * max|tan tau| >= 0.5: u_d^2 > 0 and R+delta>0 */
+                        /* of (A.3a)/(A.5b) cannot be guaranteed (G9)                               */
+  IA_ERR_CAPACITY = -4, /* n_hits per event > IA_MAX_HITS, k > IA_MAX_K, too many cells             */
+  IA_ERR_CUDA = -5      /* a CUDA runtime call failed; see ia_last_cuda_error()                     */
+};
+
+#define IA_MAX_HITS 1024 /* per event: staged hits must fit one CTA's shared memory                */
+#define IA_MAX_K 32      /* top-K list = one key per lane of a warp                                */
+
+typedef struct ia_ctx ia_ctx; /* opaque: device geometry, parameters, stream, scratch */
+
+/* One sense wire, eq. (A.1a,b) L147-152: point (x0,y0) of the wire in the plane z=0, projection
+ * angle phi_s (given as sin/cos, computed by the caller in double), signed tan of the stereo
+ * angle tau.  half_len and layer are carried for the caller's benefit; the vote does not use
+ * them.  40 bytes + 16. */
+typedef struct {
+  double x0, y0;
+  double sin_phi_s, cos_phi_s;
+  double tan_tau;
+  double half_len;
+  int32_t layer;
+  int32_t _pad;
+} ia_wire;
+
+/* One hit, L88: "a hit is defined by this drift distance and the ... wire".  drift = |d_St| >= 0. */
+typedef struct {
+  int32_t wire; /* index into the loaded geometry */
+  int32_t _pad;
+  double drift; /* cm */
+} ia_hit;
+
+/* tol: vote tolerance on the drift distance, D = [max(d-tol,0), d+tol] (S1, G6).
+ * (x_ref, y_ref): reference point of eq. (1d); z_ref: reference plane of (A.4c-e) L172-176.
+ * precision: 64 or 32 = type of the interval endpoints (G22).  flags: reserved, must be 0. */
+typedef struct {
+  double tol;
+  double x_ref, y_ref, z_ref;
+  int32_t precision;
+  uint32_t flags;
+} ia_params;
+
+/* A box with its vote count: 88 bytes. */
+typedef struct {
+  double lo[5], hi[5];
+  uint16_t votes;
+  uint16_t _pad[3];
+} ia_box;
+
+/* Create a context on CUDA device `device` that enqueues on `cuda_stream` (a cudaStream_t cast
+ * to void*; NULL = the legacy default stream).  Parameters default to tol=0.045, ref=(0,0,0),
+ * precision=64. */
+int ia_create(ia_ctx** ctx_out, int device, void* cuda_stream);
+void ia_destroy(ia_ctx* ctx);
+
+/* a1 - copy the wires (HOST array, n_wires > 0) to a device SoA x0,y0,sin,cos,tan.  Replaces any
+ * geometry loaded before.  Synchronises the stream. */
+int ia_load_geometry(ia_ctx* ctx, const ia_wire* wires_host, int n_wires);
+int ia_set_params(ia_ctx* ctx, const ia_params* params_host);
+
+/* a2-a6 - dense single-level vote, condition (4) L74-78.  The box [box_lo, box_hi] is cut into
+ * grid_dims[0..4] cells per axis, edges e_k = lo + k*((hi-lo)/n), e_n = hi (S9, G14);
+ * votes_out_dev[((((ix*ny+iy)*nR+iR)*nz+iz)*nl+il)] = number of hits whose enclosure contains 0
+ * for either drift sign (uint16, lambda fastest; prod(grid_dims) entries, at most 2^40). */
+int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
+            const int32_t grid_dims[5], uint16_t* votes_out_dev);
+
+/* Same vote on an explicit list of boxes: lo_dev/hi_dev are [n_boxes][5] doubles. */
+int ia_vote_boxes(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
+                  int64_t n_boxes, uint16_t* votes_out_dev);
+
+/* a7 - the k largest entries by key (votes descending, index ascending) (L94, G16):
+ * idx_out_dev[k] (int64 linear indices), votes_out_dev[k].  1 <= k <= min(n_cells, IA_MAX_K). */
+int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t* idx_out_dev,
+            uint16_t* votes_out_dev);
+
+/* a8-a9 - adaptive refinement of one event, entirely on the device: vote the dense grid0, keep the
+ * top k, then (levels-1) times: cut every kept box at its per-axis midpoints into 2^5 children
+ * (child c of rank r at list index r*32+c, bit (4-dim) of c set = upper half), vote the 32k
+ * children, keep the top k.  boxes_out_dev[level][rank] (levels*k ia_box); params_out_dev[10] =
+ * centre (5) and half-width (5) of the rank-0 box of the last pass (L94, G19). */
+int ia_refine(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
+              const int32_t grid0[5], int levels, int k, ia_box* boxes_out_dev, double* params_out_dev);
+
+/* a10 - the same for n_events independent events in one launch sequence.  Hits in CSR form:
+ * event e owns hits_dev[hit_offsets_dev[e] .. hit_offsets_dev[e+1]); max_hits_per_event bounds
+ * every event's count (<= IA_MAX_HITS).  boxes_out_dev[n_events][levels][k], params_out_dev
+ * [n_events][10]. */
+int ia_refine_batch(ia_ctx* ctx, const ia_hit* hits_dev, const int32_t* hit_offsets_dev, int n_events,
+                    int max_hits_per_event, const double box_lo[5], const double box_hi[5], const int32_t grid0[5],
+                    int levels, int k, ia_box* boxes_out_dev, double* params_out_dev);
+
+/* End-to-end variants: every pointer is HOST memory (pinned for full copy speed).  They validate
+ * the hits, copy them to the device, run the call above and copy the result back, then
+ * synchronise the stream. */
+int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double box_lo[5], const double box_hi[5],
+                 const int32_t grid_dims[5], uint16_t* votes_out_host);
+int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hit_offsets_host, int n_events,
+                         const double box_lo[5], const double box_hi[5], const int32_t grid0[5], int levels, int k,
+                         ia_box* boxes_out_host, double* params_out_host);
+
+/* Diagnostics for parity tracing (G25): the enclosure f = R_Ax^2 - (R + d_Ax)^2 of every
+ * (box, hit, drift sign): out_dev[((b*n_hits + h)*2 + s)*4 + {0,1,2,3}] = f.lo, f.hi,
+ * scale = max(Q.hi, |rad|), forced (1 if a domain rule forced the vote, G15); s = 0 for +d. */
+int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
+                int64_t n_boxes, double* out_dev);
+
+/* Device interval primitives exposed for unit tests: n independent operations
+ * out_dev[i] = op(a_dev[i], b_dev[i]) on intervals stored as (lo, hi) pairs of doubles; prec = 64 or 32.
+ * op: 0 add 1 sub 2 mul 3 sqr(a) 4 div(a, b>0) 5 sqrt(a) 6 sin(a) 7 cos(a) 8 atan2(y=a, x=b)
+ *     9 recip(a>0) 10 scale(b.lo, a) */
+int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev);
+
+/* Synchronise the stream and return IA_OK, IA_ERR_GEOMETRY (a hit named an unknown wire since
+ * the last call of this function) or IA_ERR_CUDA. */
+int ia_device_status(ia_ctx* ctx);
+
+/* Number of kernels this context has launched so far (for the bench's gpu_launches). */
+int64_t ia_launch_count(const ia_ctx* ctx);
+
+const char* ia_strerror(int code);
+const char* ia_last_cuda_error(const ia_ctx* ctx);
+/* Outward padding of the sin/cos/atan2 enclosures, in ulps (lower bound of the relative pad). */
+int ia_pad_ulps(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IA_B200_H */

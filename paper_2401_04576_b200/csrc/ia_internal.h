@@ -1,0 +1,86 @@
+// ia_internal.h - host-side context and the launcher interface between ia_api.cu and the kernel files.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ia.h"
+
+namespace ia {
+
+// dense grid descriptor (S9, G14): cell k of axis d is [edge(k), edge(k+1)], edge(k) = lo + k*w, edge(n) = hi
+struct GridDesc {
+  double lo[5], hi[5], w[5];
+  int32_t n[5];
+  int64_t cells;      // prod(n)
+  int64_t col_cells;  // n[2]*n[3]*n[4]: cells of one (xc, yc) column
+};
+
+// where the hits of event e live: staged[e*max_hits + i], i < count(e)
+struct HitSpan {
+  const ia_hit* hits;          // device
+  const int32_t* offsets;      // device, n_events+1 entries, or nullptr: one event of n_hits_single hits
+  int32_t n_hits_single;
+  int32_t max_hits;            // slots per event in the staged array
+  int32_t n_events;
+};
+
+struct Scratch {
+  void* p = nullptr;
+  size_t cap = 0;
+};
+
+}  // namespace ia
+
+struct ia_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  ia_params params{};
+  // geometry SoA (a1)
+  int n_wires = 0;
+  double* wires = nullptr;   // 5 * n_wires doubles: x0 | y0 | sin | cos | tan
+  double max_abs_tan = 0.0;
+  // scratch, grown on demand, freed in ia_destroy
+  ia::Scratch staged;        // HitC<T>[n_events * max_hits]
+  ia::Scratch votes;         // uint16 dense votes of the refinement start grid
+  ia::Scratch partial;       // uint16 partial child votes / uint64 partial top-K keys
+  ia::Scratch keys;          // uint64 top-K keys
+  ia::Scratch misc;          // idx / votes of internal top-K, host-variant device buffers
+  ia::Scratch io_a, io_b, io_c, io_d;   // *_host entry points: device mirrors of host buffers
+  int* status = nullptr;     // device: sticky error flag
+  int64_t launches = 0;
+  cudaError_t last_err = cudaSuccess;
+};
+
+namespace ia {
+
+// All launchers enqueue on ctx->stream, bump ctx->launches and return the launch's cudaError_t.
+// prec selects the endpoint type (64: double, 32: float).
+
+cudaError_t launch_stage_hits(ia_ctx* ctx, const HitSpan& span);
+
+cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& span, const GridDesc& g, uint16_t* votes_out);
+
+// explicit boxes, one event: lo/hi [n_boxes][5]
+cudaError_t launch_vote_boxes(ia_ctx* ctx, const HitSpan& span, const double* lo, const double* hi, int64_t n_boxes,
+                              uint16_t* votes_out);
+
+cudaError_t launch_residual(ia_ctx* ctx, const HitSpan& span, const double* lo, const double* hi, int64_t n_boxes,
+                            double* out);
+
+cudaError_t launch_prim(ia_ctx* ctx, int op, int prec, const double* a, const double* b, int64_t n, double* out);
+
+// top-K of n_events independent arrays of n entries each (stride n): idx_out/votes_out [n_events][k]
+cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_events, int k, int64_t* idx_out,
+                        uint16_t* votes_out);
+
+// refinement steps (a8-a9)
+cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* idx, const uint16_t* v, int n_events,
+                                int k, int levels, ia_box* boxes_out);
+// one level: children of boxes_out[e][lev-1][*] voted, top-k written to boxes_out[e][lev][*]
+cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& span, int lev, int levels, int k, ia_box* boxes_out);
+cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out);
+
+// scratch helper: grow-only device buffer
+cudaError_t scratch_reserve(Scratch& s, size_t bytes);
+
+}  // namespace ia

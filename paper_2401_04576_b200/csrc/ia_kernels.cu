@@ -1,0 +1,352 @@
+// ia_kernels.cu - hit staging (a2), explicit-box vote, refinement level (a8-a9), diagnostics.
+#include "ia_internal.h"
+#include "ia_residual.cuh"
+#include "ia_topk.cuh"
+
+namespace ia {
+
+cudaError_t scratch_reserve(Scratch& s, size_t bytes) {
+  if (bytes <= s.cap) return cudaSuccess;
+  if (s.p) cudaFree(s.p);
+  s.p = nullptr;
+  s.cap = 0;
+  size_t want = bytes + bytes / 4 + 256;
+  cudaError_t err = cudaMalloc(&s.p, want);
+  if (err == cudaSuccess) s.cap = want;
+  return err;
+}
+
+namespace {
+
+// ---- a2: staging ------------------------------------------------------------------------------
+// per-hit scalars of S1-S3 in round-to-nearest, unfused (__dmul_rn/__dadd_rn are never contracted).
+// FP32 mode converts every scalar input to float first and then computes in float.
+template <class T>
+__device__ HitC<T> make_hitc(const double* __restrict__ wires, int n_wires, ia_hit h, ia_params p, int* status) {
+  using R = Rnd<T>;
+  HitC<T> c;
+  int w = h.wire;
+  c.valid = (w >= 0 && w < n_wires && h.drift >= 0.0);
+  if (!c.valid) {
+    if (status) atomicOr(status, 1);
+    w = 0;
+    h.drift = 0.0;
+  }
+  const T x0 = R::from_rn(wires[w]), y0 = R::from_rn(wires[n_wires + w]);
+  const T s = R::from_rn(wires[2 * n_wires + w]), co = R::from_rn(wires[3 * n_wires + w]);
+  const T t = R::from_rn(wires[4 * n_wires + w]);
+  const T xr = R::from_rn(p.x_ref), yr = R::from_rn(p.y_ref), zr = R::from_rn(p.z_ref);
+  c.sphi = s; c.cphi = co; c.Tn = t;
+  c.xA = R::add_rn(x0, R::mul_rn(R::mul_rn(zr, s), t));          // (A.4d) L174
+  c.yA = R::add_rn(y0, -R::mul_rn(R::mul_rn(zr, co), t));        // (A.4e) L176
+  c.k0 = R::add_rn(R::mul_rn(xr, c.yA), -R::mul_rn(yr, c.xA));
+  c.ky = R::add_rn(yr, -c.yA);
+  c.kx = R::add_rn(c.xA, -xr);
+  c.mx = R::mul_rn(T(0.5), R::add_rn(xr, c.xA));
+  c.my = R::mul_rn(T(0.5), R::add_rn(yr, c.yA));
+  const T hx = R::mul_rn(T(0.5), R::add_rn(c.xA, -xr)), hy = R::mul_rn(T(0.5), R::add_rn(c.yA, -yr));
+  c.h2 = R::add_rn(R::mul_rn(hx, hx), R::mul_rn(hy, hy));
+  const T d = R::from_rn(h.drift), tol = R::from_rn(p.tol);
+  c.Dlo = mx(R::add_dn(d, -tol), T(0));                          // S1 (G6)
+  c.Dhi = R::add_up(d, tol);
+  c.zref = zr;
+  c._pad = 0;
+  return c;
+}
+
+__device__ __forceinline__ void event_hits(const HitSpan& sp, int e, int& first, int& count) {
+  if (sp.offsets) {
+    first = sp.offsets[e];
+    count = sp.offsets[e + 1] - first;
+    if (count > sp.max_hits) count = sp.max_hits;
+    if (count < 0) count = 0;
+  } else {
+    first = 0;
+    count = sp.n_hits_single;
+  }
+}
+
+template <class T>
+__global__ void stage_hits_kernel(HitSpan sp, const double* __restrict__ wires, int n_wires, ia_params p,
+                                  HitC<T>* __restrict__ staged, int* status) {
+  const int e = blockIdx.x;
+  int first, count;
+  event_hits(sp, e, first, count);
+  for (int i = threadIdx.x; i < count; i += blockDim.x)
+    staged[int64_t(e) * sp.max_hits + i] = make_hitc<T>(wires, n_wires, sp.hits[first + i], p, status);
+}
+
+// ---- explicit-box vote: one thread per box, hits broadcast from shared memory --------------------
+template <class T>
+__global__ void __launch_bounds__(128)
+vote_boxes_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const double* __restrict__ lo,
+                  const double* __restrict__ hi, int64_t n_boxes, uint16_t* __restrict__ votes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  HitC<T>* sh = reinterpret_cast<HitC<T>*>(smem_raw);
+  int first, count;
+  event_hits(sp, 0, first, count);
+  for (int i = threadIdx.x; i < count; i += blockDim.x) sh[i] = staged[i];
+  __syncthreads();
+  const int64_t b = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (b >= n_boxes) return;
+  const Iv<T> X = box_iv<T>(lo[5 * b + 0], hi[5 * b + 0]), Y = box_iv<T>(lo[5 * b + 1], hi[5 * b + 1]);
+  Box3<T> bx = {box_iv<T>(lo[5 * b + 2], hi[5 * b + 2]), box_iv<T>(lo[5 * b + 3], hi[5 * b + 3]),
+                box_iv<T>(lo[5 * b + 4], hi[5 * b + 4])};
+  unsigned v = 0;
+  for (int h = 0; h < count; ++h) {
+    const HitC<T> c = sh[h];
+    const XYInv<T> inv = xy_invariants(X, Y, c);
+    v += hit_votes_general(bx, inv, hit_small(c), c.zref) ? 1u : 0u;
+  }
+  votes[b] = uint16_t(v);
+}
+
+// ---- diagnostics: f enclosure per (box, hit, sign) -----------------------------------------------
+template <class T>
+__global__ void residual_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const double* __restrict__ lo,
+                                const double* __restrict__ hi, int64_t n_boxes, double* __restrict__ out) {
+  const int n_hits = sp.n_hits_single;
+  const int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (t >= n_boxes * n_hits) return;
+  const int64_t b = t / n_hits;
+  const int h = int(t - b * n_hits);
+  const HitC<T> c = staged[h];
+  const Iv<T> X = box_iv<T>(lo[5 * b + 0], hi[5 * b + 0]), Y = box_iv<T>(lo[5 * b + 1], hi[5 * b + 1]);
+  Box3<T> bx = {box_iv<T>(lo[5 * b + 2], hi[5 * b + 2]), box_iv<T>(lo[5 * b + 3], hi[5 * b + 3]),
+                box_iv<T>(lo[5 * b + 4], hi[5 * b + 4])};
+  const XYInv<T> inv = xy_invariants(X, Y, c);
+  for (int s = 0; s < 2; ++s) {
+    Resid r = residual_general(bx, inv, hit_small(c), c.zref, s == 0 ? +1 : -1);
+    double* o = out + (t * 2 + s) * 4;
+    o[0] = r.flo; o[1] = r.fhi; o[2] = r.scale; o[3] = r.forced ? 1.0 : 0.0;
+  }
+}
+
+// ---- primitives exposed for unit tests ---------------------------------------------------------
+template <class T>
+__global__ void prim_kernel(int op, const double* __restrict__ a, const double* __restrict__ b, int64_t n,
+                            double* __restrict__ out) {
+  const int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Iv<T> x = {T(a[2 * i]), T(a[2 * i + 1])}, y = {T(0), T(0)}, r = {T(0), T(0)};
+  if (b) y = {T(b[2 * i]), T(b[2 * i + 1])};
+  switch (op) {
+    case 0: r = iadd(x, y); break;
+    case 1: r = isub(x, y); break;
+    case 2: r = imul(x, y); break;
+    case 3: r = isqr(x); break;
+    case 4: r = idiv_pos(x, y); break;
+    case 5: r = isqrt(x); break;
+    case 6: r = isin(x); break;
+    case 7: r = icos(x); break;
+    case 8: r = iatan2(x, y); break;
+    case 9: r = irecip_pos(x); break;
+    case 10: r = iscale(y.lo, x); break;
+    default: break;
+  }
+  out[2 * i] = double(r.lo);
+  out[2 * i + 1] = double(r.hi);
+}
+
+// ---- refinement ---------------------------------------------------------------------------------
+// dense cell index -> box (S9): linear index ((((ix*ny+iy)*nR+iR)*nz+iz)*nl+il), lambda fastest
+__global__ void gather_dense_kernel(GridDesc g, const int64_t* __restrict__ idx, const uint16_t* __restrict__ v,
+                                    int k, int levels, ia_box* __restrict__ boxes) {
+  const int e = blockIdx.x, r = threadIdx.x;
+  if (r >= k) return;
+  int64_t c = idx[int64_t(e) * k + r];
+  ia_box bx;
+  for (int d = 4; d >= 0; --d) {
+    const int kk = int(c % g.n[d]);
+    c /= g.n[d];
+    bx.lo[d] = cell_edge(g.lo[d], g.hi[d], g.w[d], kk, g.n[d]);
+    bx.hi[d] = cell_edge(g.lo[d], g.hi[d], g.w[d], kk + 1, g.n[d]);
+  }
+  bx.votes = v[int64_t(e) * k + r];
+  bx._pad[0] = bx._pad[1] = bx._pad[2] = 0;
+  boxes[(int64_t(e) * levels + 0) * k + r] = bx;
+}
+
+// child c of a box: bit (4-d) of c set -> upper half [mid, hi], mid = 0.5*(lo+hi) rn (S9, G18)
+__device__ __forceinline__ void child_axis(double lo, double hi, int upper, double& clo, double& chi) {
+  const double mid = __dmul_rn(0.5, __dadd_rn(lo, hi));
+  clo = upper ? mid : lo;
+  chi = upper ? hi : mid;
+}
+
+// One refinement pass, stage 1: block (split, e, chunk) owns the children t = chunk*256 + thread of
+// event e (rank t/32, child t%32); each thread computes its child from the parent on the fly and
+// counts the votes of the hits [split*per_split, ...) - the hit range is split across blocks so
+// that a single event still fills the chip; partial[e][split][t].
+template <class T>
+__global__ void __launch_bounds__(256)
+vote_children_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
+                     int levels, int k, int per_split, uint16_t* __restrict__ partial) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  HitC<T>* sh = reinterpret_cast<HitC<T>*>(smem_raw);
+  const int e = blockIdx.y, split = blockIdx.x;
+  int first, count;
+  event_hits(sp, e, first, count);
+  const int h0 = split * per_split;
+  int h1 = h0 + per_split;
+  if (h1 > count) h1 = count;
+  for (int i = h0 + threadIdx.x; i < h1; i += blockDim.x) sh[i - h0] = staged[int64_t(e) * sp.max_hits + i];
+  __syncthreads();
+  const int t = blockIdx.z * blockDim.x + threadIdx.x;
+  if (t >= k * 32) return;
+  const ia_box par = boxes[(int64_t(e) * levels + (lev - 1)) * k + (t >> 5)];
+  const int c = t & 31;
+  double lo[5], hi[5];
+#pragma unroll
+  for (int d = 0; d < 5; ++d) child_axis(par.lo[d], par.hi[d], (c >> (4 - d)) & 1, lo[d], hi[d]);
+  const Iv<T> X = box_iv<T>(lo[0], hi[0]), Y = box_iv<T>(lo[1], hi[1]);
+  Box3<T> bx = {box_iv<T>(lo[2], hi[2]), box_iv<T>(lo[3], hi[3]), box_iv<T>(lo[4], hi[4])};
+  unsigned v = 0;
+  for (int h = 0; h < h1 - h0; ++h) {
+    const HitC<T> hc = sh[h];
+    const XYInv<T> inv = xy_invariants(X, Y, hc);
+    v += hit_votes_general(bx, inv, hit_small(hc), hc.zref) ? 1u : 0u;
+  }
+  partial[(int64_t(e) * gridDim.x + split) * (k * 32) + t] = uint16_t(v);
+}
+
+// stage 2: one block per event sums the partial counts, selects the top k of the 32k children
+// (warp = one parent's 32 children: sort, then merge across warps) and writes their boxes.
+__global__ void __launch_bounds__(1024)
+select_children_kernel(const uint16_t* __restrict__ partial, int n_splits, int lev, int levels, int k,
+                       ia_box* __restrict__ boxes) {
+  __shared__ u64 smem_keys[32 * 32];
+  const int e = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  unsigned v = 0;
+  for (int s = 0; s < n_splits; ++s) v += partial[(int64_t(e) * n_splits + s) * (k * 32) + t];
+  u64 mine = warp_sort_desc(make_key(v, t));
+  mine = block_merge(mine, smem_keys);
+  if (warp == 0 && lane < k) {
+    const int child = int(key_index(mine));
+    const ia_box par = boxes[(int64_t(e) * levels + (lev - 1)) * k + (child >> 5)];
+    const int c = child & 31;
+    ia_box bx;
+#pragma unroll
+    for (int d = 0; d < 5; ++d) child_axis(par.lo[d], par.hi[d], (c >> (4 - d)) & 1, bx.lo[d], bx.hi[d]);
+    bx.votes = key_votes(mine);
+    bx._pad[0] = bx._pad[1] = bx._pad[2] = 0;
+    boxes[(int64_t(e) * levels + lev) * k + lane] = bx;
+  }
+}
+
+// value = centre, error = half-width of the rank-0 box of the last pass (L94, G19)
+__global__ void params_kernel(int n_events, int levels, int k, const ia_box* __restrict__ boxes,
+                              double* __restrict__ params) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_events) return;
+  const ia_box b = boxes[(int64_t(e) * levels + (levels - 1)) * k];
+  for (int d = 0; d < 5; ++d) {
+    params[int64_t(e) * 10 + d] = __dmul_rn(0.5, __dadd_rn(b.lo[d], b.hi[d]));
+    params[int64_t(e) * 10 + 5 + d] = __dmul_rn(0.5, __dadd_rn(b.hi[d], -b.lo[d]));
+  }
+}
+
+template <class T> size_t staged_bytes(const HitSpan& sp) { return size_t(sp.n_events) * sp.max_hits * sizeof(HitC<T>); }
+
+}  // namespace
+
+#define IA_DISPATCH_PREC(ctx, CALL_D, CALL_F) \
+  do {                                        \
+    if ((ctx)->params.precision == 32) {      \
+      CALL_F;                                 \
+    } else {                                  \
+      CALL_D;                                 \
+    }                                         \
+  } while (0)
+
+cudaError_t launch_stage_hits(ia_ctx* ctx, const HitSpan& sp) {
+  const bool f32 = ctx->params.precision == 32;
+  cudaError_t err = scratch_reserve(ctx->staged, f32 ? staged_bytes<float>(sp) : staged_bytes<double>(sp));
+  if (err != cudaSuccess) return err;
+  if (sp.n_events <= 0 || sp.max_hits <= 0) return cudaSuccess;
+  IA_DISPATCH_PREC(ctx,
+    (stage_hits_kernel<double><<<sp.n_events, 64, 0, ctx->stream>>>(sp, ctx->wires, ctx->n_wires, ctx->params,
+                                                                    static_cast<HitC<double>*>(ctx->staged.p), ctx->status)),
+    (stage_hits_kernel<float><<<sp.n_events, 64, 0, ctx->stream>>>(sp, ctx->wires, ctx->n_wires, ctx->params,
+                                                                   static_cast<HitC<float>*>(ctx->staged.p), ctx->status)));
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_vote_boxes(ia_ctx* ctx, const HitSpan& sp, const double* lo, const double* hi, int64_t n_boxes,
+                              uint16_t* votes_out) {
+  if (n_boxes <= 0) return cudaSuccess;
+  const unsigned blocks = unsigned((n_boxes + 127) / 128);
+  IA_DISPATCH_PREC(ctx,
+    (vote_boxes_kernel<double><<<blocks, 128, sp.max_hits * sizeof(HitC<double>), ctx->stream>>>(
+        sp, static_cast<const HitC<double>*>(ctx->staged.p), lo, hi, n_boxes, votes_out)),
+    (vote_boxes_kernel<float><<<blocks, 128, sp.max_hits * sizeof(HitC<float>), ctx->stream>>>(
+        sp, static_cast<const HitC<float>*>(ctx->staged.p), lo, hi, n_boxes, votes_out)));
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_residual(ia_ctx* ctx, const HitSpan& sp, const double* lo, const double* hi, int64_t n_boxes,
+                            double* out) {
+  const int64_t n = n_boxes * sp.n_hits_single;
+  if (n <= 0) return cudaSuccess;
+  const unsigned blocks = unsigned((n + 127) / 128);
+  IA_DISPATCH_PREC(ctx,
+    (residual_kernel<double><<<blocks, 128, 0, ctx->stream>>>(sp, static_cast<const HitC<double>*>(ctx->staged.p), lo, hi,
+                                                              n_boxes, out)),
+    (residual_kernel<float><<<blocks, 128, 0, ctx->stream>>>(sp, static_cast<const HitC<float>*>(ctx->staged.p), lo, hi,
+                                                             n_boxes, out)));
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prim(ia_ctx* ctx, int op, int prec, const double* a, const double* b, int64_t n, double* out) {
+  if (n <= 0) return cudaSuccess;
+  const unsigned blocks = unsigned((n + 127) / 128);
+  if (prec == 32) prim_kernel<float><<<blocks, 128, 0, ctx->stream>>>(op, a, b, n, out);
+  else prim_kernel<double><<<blocks, 128, 0, ctx->stream>>>(op, a, b, n, out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* idx, const uint16_t* v, int n_events,
+                                int k, int levels, ia_box* boxes_out) {
+  gather_dense_kernel<<<n_events, 32, 0, ctx->stream>>>(g, idx, v, k, levels, boxes_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, ia_box* boxes_out) {
+  int sm = 148;
+  cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, ctx->device);
+  // split the hit range when there are too few events to fill the chip
+  int n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
+  if (n_splits > sp.max_hits) n_splits = sp.max_hits;
+  if (n_splits < 1) n_splits = 1;
+  const int per_split = (sp.max_hits + n_splits - 1) / n_splits;
+  n_splits = (sp.max_hits + per_split - 1) / per_split;
+  cudaError_t err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
+  if (err != cudaSuccess) return err;
+  uint16_t* partial = static_cast<uint16_t*>(ctx->partial.p);
+  const int threads = k * 32;
+  dim3 grid(n_splits, sp.n_events, (threads + 255) / 256);
+  IA_DISPATCH_PREC(ctx,
+    (vote_children_kernel<double><<<grid, 256, per_split * sizeof(HitC<double>), ctx->stream>>>(
+        sp, static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),
+    (vote_children_kernel<float><<<grid, 256, per_split * sizeof(HitC<float>), ctx->stream>>>(
+        sp, static_cast<const HitC<float>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)));
+  ctx->launches++;
+  err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  select_children_kernel<<<sp.n_events, threads, 0, ctx->stream>>>(partial, n_splits, lev, levels, k, boxes_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out) {
+  params_kernel<<<(n_events + 127) / 128, 128, 0, ctx->stream>>>(n_events, levels, k, boxes, params_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+}  // namespace ia

@@ -1,0 +1,347 @@
+"""-m gpu: the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bars (BASELINE.json north_star): top-K boxes and recovered parameters identical at every level;
+vote accumulator equal in >= 99.99 % of cells with every mismatch traced to a residual endpoint
+within 1e-12 relative of zero; integer/index work bit-exact.
+"""
+import numpy as np
+import pytest
+
+from paper_2401_04576_b200 import binding as b
+from paper_2401_04576_b200 import eventgen as g
+from oracle import oracle as o
+
+from gpu_common import HI, LO, Rig, compare_votes
+
+pytestmark = pytest.mark.gpu
+
+ADD, SUB, MUL, SQR, DIV, SQRT, SIN, COS, ATAN2, RECIP, SCALE = range(11)
+
+
+@pytest.fixture(scope="module")
+def rig0():
+    r = Rig(g.chamber_c0())
+    yield r
+    r.close()
+
+
+@pytest.fixture(scope="module")
+def rig1():
+    r = Rig(g.chamber_c1())
+    yield r
+    r.close()
+
+
+def _rand_iv(rng, n, positive=False, prec=64):
+    m = rng.choice([1e-3, 1.0, 37.0, 450.0, 1e5], size=n)
+    a, c = rng.uniform(-m, m), rng.uniform(-m, m)
+    lo, hi = np.minimum(a, c), np.maximum(a, c)
+    thin = rng.random(n) < 0.15
+    hi = np.where(thin, lo, hi)
+    if positive:
+        lo, hi = np.abs(lo) + 1e-3, np.abs(hi) + 1e-3
+        lo, hi = np.minimum(lo, hi), np.maximum(lo, hi)
+    if prec == 32:
+        lo, hi = lo.astype(np.float32).astype(np.float64), hi.astype(np.float32).astype(np.float64)
+        lo, hi = np.minimum(lo, hi), np.maximum(lo, hi)
+    return np.stack([lo, hi], 1)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_arithmetic_primitives_bit_exact(rig0, prec):
+    """Both sides return the tightest enclosure, so + - * sqr / sqrt recip scale agree bit for bit."""
+    rng = np.random.default_rng(prec)
+    n = 3000
+    a, bb, bp = _rand_iv(rng, n, prec=prec), _rand_iv(rng, n, prec=prec), _rand_iv(rng, n, True, prec)
+    # sign cases with zeros and signed zeros
+    pts = [-3.5, -1.25, -0.0, 0.0, 0.75, 2.5]
+    ivs = np.array([(x, y) for x in pts for y in pts if x <= y])
+    a[: len(ivs) ** 2] = np.repeat(ivs, len(ivs), 0)
+    bb[: len(ivs) ** 2] = np.tile(ivs, (len(ivs), 1))
+    ctx = rig0.ctx
+    for op, x, y in ((ADD, a, bb), (SUB, a, bb), (MUL, a, bb), (SQR, a, None), (DIV, a, bp), (SQRT, bp, None),
+                     (RECIP, bp, None), (SCALE, a, bb)):
+        got = ctx.ia_prim(op, prec, rig0.dev(x), None if y is None else rig0.dev(y)).cpu().numpy()
+        for i in range(n):
+            yy = (0.0, 0.0) if y is None else tuple(y[i])
+            if op == SCALE:
+                yy = (y[i, 0], y[i, 0])
+            exp = o.prim(op, tuple(x[i]), yy, prec)
+            assert (got[i, 0] == exp[0] and got[i, 1] == exp[1]) or (np.isnan(exp[0]) and np.isnan(got[i, 0])), (op, x[i], yy, got[i], exp)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_elementary_enclosures(rig0, prec):
+    """sin/cos/atan2: the GPU enclosure overlaps the oracle's everywhere, both within their pads:
+    |gpu - oracle| <= (pad_gpu + pad_oracle + 2) ulps at each endpoint, same special cases."""
+    rng = np.random.default_rng(3)
+    n = 4000
+    eps = 2.0 ** -52 if prec == 64 else 2.0 ** -23
+    w = rng.choice([0.0, 1e-9, 1e-3, 0.1, 1.0, 3.0], size=n)
+    c = rng.uniform(-4.5, 4.5, n)
+    e = np.stack([c - w, c + w], 1)
+    if prec == 32:
+        e = e.astype(np.float32).astype(np.float64)
+    y, x = _rand_iv(rng, n, prec=prec), _rand_iv(rng, n, prec=prec)
+    ctx = rig0.ctx
+    tol_ulps = 8 + o.pad_ulps() + 2
+    for op, A, B, mag in ((SIN, e, None, 1.0), (COS, e, None, 1.0), (ATAN2, y, x, 4.0)):
+        got = ctx.ia_prim(op, prec, rig0.dev(A), None if B is None else rig0.dev(B)).cpu().numpy()
+        for i in range(n):
+            exp = o.prim(op, tuple(A[i]), (0.0, 0.0) if B is None else tuple(B[i]), prec)
+            assert abs(got[i, 0] - exp[0]) <= tol_ulps * eps * mag and abs(got[i, 1] - exp[1]) <= tol_ulps * eps * mag, \
+                (op, A[i], got[i], exp)
+            assert got[i, 0] <= exp[1] and exp[0] <= got[i, 1]
+            if exp in ((-1.0, 1.0),) or abs(exp[1]) == 1.0 or abs(exp[0]) == 1.0:
+                pass
+        # exact special values
+    sp = np.array([[-5.0, 0.0], [0.0, 4.5], [1.0, 2.0], [-2.0, -1.0], [-0.5, 0.25], [3.0, 3.5]])
+    s = ctx.ia_prim(SIN, prec, rig0.dev(sp)).cpu().numpy()
+    cc = ctx.ia_prim(COS, prec, rig0.dev(sp)).cpu().numpy()
+    assert tuple(s[0]) == (-1.0, 1.0) and tuple(cc[1]) == (-1.0, 1.0)
+    assert s[2, 1] == 1.0 and s[3, 0] == -1.0 and cc[4, 1] == 1.0 and cc[5, 0] == -1.0
+    cut = ctx.ia_prim(ATAN2, prec, rig0.dev(np.array([[-1.0, 1.0]])), rig0.dev(np.array([[-2.0, -1.0]]))).cpu().numpy()
+    assert tuple(cut[0]) == o.prim(ATAN2, (-1.0, 1.0), (-2.0, -1.0), prec)
+
+
+def _random_boxes(rng, n, min_log2=2, max_log2=12):
+    c = rng.uniform(LO * 0.9 + HI * 0.1, LO * 0.1 + HI * 0.9, size=(n, 5))
+    w = (HI - LO) * 2.0 ** -rng.integers(min_log2, max_log2, size=(n, 1))
+    blo, bhi = c - w / 2, c + w / 2
+    blo[:, 2] = np.maximum(blo[:, 2], 20.0)
+    blo[:, 4], bhi[:, 4] = np.maximum(blo[:, 4], -0.6), np.minimum(bhi[:, 4], 0.6)
+    return blo, bhi
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("ref", [(0.0, 0.0, 0.0), (1.5, -2.0, 3.0)])
+def test_residual_enclosures_match(precision, ref):
+    """f enclosures of random (box, hit, sign): endpoints agree to a few ulps of the residual's scale."""
+    rng = np.random.default_rng(11)
+    rig = Rig(g.chamber_c1(), precision=precision, x_ref=ref[0], y_ref=ref[1], z_ref=ref[2])
+    try:
+        ev = g.make_event(rig.ch, 5, n_noise=12)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        blo, bhi = _random_boxes(rng, 600)
+        # boxes around the truth as well, where the enclosures are tight and straddle zero
+        par = np.array(ev.track.params)
+        for i in range(0, 200):
+            half = (HI - LO) * 2.0 ** -rng.integers(6, 14) / 2
+            cc = par + rng.uniform(-1, 1, 5) * half
+            blo[i], bhi[i] = cc - half, cc + half
+        rg = rig.gpu_residual(hd, len(oh), blo, bhi)
+        ro = o.residual(rig.owires, oh, rig.oparams, blo, bhi)
+        assert (rg[..., 3] == ro[..., 3]).all()
+        live = ro[..., 3] == 0
+        tol = (1e-13 if precision == 64 else 2e-4) * ro[..., 2]
+        assert (np.abs(rg[..., 0] - ro[..., 0])[live] <= tol[live]).all()
+        assert (np.abs(rg[..., 1] - ro[..., 1])[live] <= tol[live]).all()
+        assert np.allclose(rg[..., 2][live], ro[..., 2][live], rtol=1e-6 if precision == 64 else 1e-3)
+        vg = (rg[..., 3] == 1) | ((rg[..., 0] <= 0) & (rg[..., 1] >= 0))
+        vo = (ro[..., 3] == 1) | ((ro[..., 0] <= 0) & (ro[..., 1] >= 0))
+        assert (vg == vo).mean() > 0.9999 and vg.any() and not vg.all()
+    finally:
+        rig.close()
+
+
+def test_c0_dense_vote_full_parity(rig0):
+    """configs[0]: 16^5 cells x 8 hits, every cell compared."""
+    cfg = g.config(0)
+    ev = cfg.events[0]
+    hd, oh = rig0.hits(ev.wire, ev.drift)
+    vg = rig0.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
+    rig0.ctx.synchronize()
+    vg = vg.cpu().numpy()
+    vo = o.vote(rig0.owires, oh, rig0.oparams, LO, HI, cfg.grid)
+    n_bad = compare_votes(rig0, hd, oh, vg, vo, lambda idx: o.cell_boxes(LO, HI, cfg.grid, idx))
+    assert vg.max() == 8 and n_bad <= len(vg) // 10000
+    truth = g.truth_cell(ev.track.params, LO, HI, cfg.grid)
+    assert vg[truth] >= (~ev.clipped).sum() - 1       # smeared hits: 3-sigma tolerance, allow one miss
+
+
+@pytest.mark.parametrize("dims", [(3, 5, 7, 2, 9), (1, 1, 1, 1, 1), (2, 2, 33, 17, 6), (6, 4, 3, 130, 5)])
+def test_ragged_grids(rig0, dims):
+    """Grid shapes that do not divide the block tiling, with a lambda cell straddling 0 (odd n)."""
+    ev = g.make_event(rig0.ch, 7, n_noise=3)
+    hd, oh = rig0.hits(ev.wire, ev.drift)
+    vg = rig0.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+    rig0.ctx.synchronize()
+    vo = o.vote(rig0.owires, oh, rig0.oparams, LO, HI, dims)
+    compare_votes(rig0, hd, oh, vg.cpu().numpy(), vo, lambda idx: o.cell_boxes(LO, HI, dims, idx), min_equal=0.999)
+
+
+def test_small_window_grid_around_truth(rig1):
+    """A fine grid around the truth (cells of range/2048): votes vary cell to cell here."""
+    ev = g.make_event(rig1.ch, 21, n_noise=5)
+    hd, oh = rig1.hits(ev.wire, ev.drift)
+    par = np.array(ev.track.params)
+    half = (HI - LO) / 256
+    lo, hi = par - half, par + half
+    dims = (8, 8, 8, 8, 8)
+    vg = rig1.ctx.ia_vote(hd, ev.n_hits, lo, hi, dims)
+    rig1.ctx.synchronize()
+    vg = vg.cpu().numpy()
+    vo = o.vote(rig1.owires, oh, rig1.oparams, lo, hi, dims)
+    compare_votes(rig1, hd, oh, vg, vo, lambda idx: o.cell_boxes(lo, hi, dims, idx))
+    assert len(np.unique(vg)) > 4
+
+
+def test_vote_boxes_and_empty_inputs(rig1):
+    rng = np.random.default_rng(2)
+    ev = g.make_event(rig1.ch, 9, n_noise=20)
+    hd, oh = rig1.hits(ev.wire, ev.drift)
+    blo, bhi = _random_boxes(rng, 1000, 2, 10)
+    vg = rig1.ctx.ia_vote_boxes(hd, ev.n_hits, rig1.dev(blo), rig1.dev(bhi))
+    rig1.ctx.synchronize()
+    vo = o.vote_boxes(rig1.owires, oh, rig1.oparams, blo, bhi)
+    compare_votes(rig1, hd, oh, vg.cpu().numpy(), vo, lambda idx: (blo[idx], bhi[idx]), min_equal=0.999)
+    # no hits: all zero
+    v0 = rig1.ctx.ia_vote(None, 0, LO, HI, (4, 4, 4, 4, 4))
+    rig1.ctx.synchronize()
+    assert int(v0.cpu().numpy().astype(np.int64).sum()) == 0
+
+
+@pytest.mark.parametrize("n,k", [(1, 1), (31, 5), (32, 32), (257, 10), (4096, 16), (100003, 8), (1 << 21, 10)])
+def test_topk_bit_exact(rig0, n, k):
+    import torch
+    rng = np.random.default_rng(n)
+    for mode in ("random", "plateau", "zeros", "late_peak"):
+        if mode == "random":
+            v = rng.integers(0, 41, n)
+        elif mode == "plateau":
+            v = np.where(rng.random(n) < 0.4, 40, rng.integers(0, 40, n))
+        elif mode == "zeros":
+            v = np.zeros(n, np.int64)
+        else:
+            v = rng.integers(0, 5, n)
+            v[-min(n, 3):] = 60
+        v = v.astype(np.uint16)
+        vd = torch.from_numpy(v.view(np.int16)).cuda().view(torch.uint16)
+        idx, vv = rig0.ctx.ia_topk(vd, k)
+        rig0.ctx.synchronize()
+        eidx, ev = o.topk(v, k)
+        assert (idx.cpu().numpy() == eidx).all() and (vv.cpu().numpy() == ev).all(), (n, k, mode)
+    # unaligned view: the 16-byte path must not be taken blindly
+    if n > 64:
+        v = rng.integers(0, 41, n).astype(np.uint16)
+        vd = torch.from_numpy(v.view(np.int16)).cuda().view(torch.uint16)
+        idx, vv = rig0.ctx.ia_topk(vd[3:], k, n_cells=n - 3)
+        rig0.ctx.synchronize()
+        eidx, ev = o.topk(v[3:], k)
+        assert (idx.cpu().numpy() == eidx).all() and (vv.cpu().numpy() == ev).all()
+
+
+def _assert_boxes_equal(gb, ob):
+    assert (gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all(), "boxes differ"
+    assert (gb["votes"] == ob["votes"]).all(), "votes differ"
+
+
+def test_c2_refine_identical_at_every_level(rig1):
+    """configs[2]: 8^5 start, K=16, 10 passes: the kept boxes and the parameters are identical."""
+    cfg = g.config(2)
+    ev = cfg.events[0]
+    hd, oh = rig1.hits(ev.wire, ev.drift)
+    boxes, par = rig1.ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, cfg.levels, cfg.k)
+    rig1.ctx.synchronize()
+    gb = b.boxes_to_numpy(boxes, (cfg.levels, cfg.k))
+    ob, opar = o.refine(rig1.owires, oh, rig1.oparams, LO, HI, cfg.grid, cfg.levels, cfg.k)
+    _assert_boxes_equal(gb, ob)
+    assert (par.cpu().numpy() == opar).all()
+    assert np.all(opar[5:] * 2 < (HI - LO) * 1e-3)            # final box width < 1e-3 of the range
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_c3_refine_batch_identical(precision):
+    """configs[3] shape (8^5 start, K=8, 8 passes) on a handful of events, FP64 and FP32 intervals."""
+    rig = Rig(g.chamber_c1(), precision=precision)
+    try:
+        cfg = g.config(3, n_events=5)
+        wire = np.concatenate([e.wire for e in cfg.events])
+        drift = np.concatenate([e.drift for e in cfg.events])
+        off = np.cumsum([0] + [e.n_hits for e in cfg.events]).astype(np.int32)
+        hd, oh = rig.hits(wire, drift)
+        boxes, par = rig.ctx.ia_refine_batch(hd, rig.dev(off), len(cfg.events), 30, LO, HI, cfg.grid, cfg.levels, cfg.k)
+        rig.ctx.synchronize()
+        gb = b.boxes_to_numpy(boxes, (len(cfg.events), cfg.levels, cfg.k))
+        ob, opar = o.refine_batch(rig.owires, oh, off, rig.oparams, LO, HI, cfg.grid, cfg.levels, cfg.k)
+        _assert_boxes_equal(gb, ob)
+        assert (par.cpu().numpy().reshape(-1, 10) == opar).all()
+        # host-buffer entry point gives the same answer
+        hb, hp = rig.ctx.ia_refine_batch_host(b.hits_of(wire, drift), off, LO, HI, cfg.grid, cfg.levels, cfg.k)
+        _assert_boxes_equal(hb, ob)
+        assert (hp == opar).all()
+    finally:
+        rig.close()
+
+
+def test_c1_dense_vote_sampled_and_top10(rig1):
+    """configs[1]: 32^5 x 40 hits at full size; 30000 sampled cells + the GPU's top-10 cells against
+    the oracle, and the top-10 selection itself bit-exact on the GPU's accumulator."""
+    cfg = g.config(1)
+    ev = cfg.events[0]
+    hd, oh = rig1.hits(ev.wire, ev.drift)
+    votes = rig1.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
+    idx, vv = rig1.ctx.ia_topk(votes, cfg.k)
+    rig1.ctx.synchronize()
+    vg = votes.cpu().numpy()
+    eidx, evv = o.topk(vg, cfg.k)
+    assert (idx.cpu().numpy() == eidx).all() and (vv.cpu().numpy() == evv).all()
+    rng = np.random.default_rng(1)
+    sample = np.unique(np.concatenate([rng.integers(0, cfg.n_cells, 30000), eidx,
+                                       [g.truth_cell(ev.track.params, LO, HI, cfg.grid)],
+                                       np.nonzero(vg == vg.max())[0][:2000]]))
+    vo = o.vote(rig1.owires, oh, rig1.oparams, LO, HI, cfg.grid, cell_idx=sample)
+    compare_votes(rig1, hd, oh, vg[sample], vo, lambda i: o.cell_boxes(LO, HI, cfg.grid, sample[i]))
+    assert vg.max() <= ev.n_hits
+
+
+def test_errors_and_device_status(rig0):
+    ctx = rig0.ctx
+    ev = g.make_event(rig0.ch, 1)
+    hd, _ = rig0.hits(ev.wire, ev.drift)
+    lo = LO.copy()
+    lo[2] = 0.0
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_vote(hd, ev.n_hits, lo, HI, (2,) * 5)
+    assert ei.value.code == -3
+    hi = HI.copy()
+    hi[4] = 6.0
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_vote(hd, ev.n_hits, LO, hi, (2,) * 5)
+    assert ei.value.code == -3
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_vote(hd, ev.n_hits, HI, LO, (2,) * 5)
+    assert ei.value.code == -1
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_refine(hd, ev.n_hits, LO, HI, (2,) * 5, 2, b.IA_MAX_K + 1)
+    assert ei.value.code in (-1, -4)
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_vote_host(b.hits_of([99999], [0.3]), LO, HI, (2,) * 5)
+    assert ei.value.code == -2
+    # a bad wire on the device path: the hit is dropped and the sticky status reports it once
+    bad, _ = rig0.hits(np.append(ev.wire, 99999).astype(np.int32), np.append(ev.drift, 0.2))
+    v = ctx.ia_vote(bad, ev.n_hits + 1, LO, HI, (4,) * 5)
+    with pytest.raises(b.IaError) as ei:
+        ctx.ia_device_status()
+    assert ei.value.code == -2
+    ctx.ia_device_status()
+    good = ctx.ia_vote(hd, ev.n_hits, LO, HI, (4,) * 5)
+    ctx.synchronize()
+    assert (v.cpu().numpy() == good.cpu().numpy()).all()
+    # a context without geometry refuses to vote
+    c2 = b.Context(0)
+    with pytest.raises(b.IaError) as ei:
+        c2.ia_vote(hd, ev.n_hits, LO, HI, (2,) * 5)
+    assert ei.value.code == -2
+    c2.close()
+
+
+def test_host_entry_point_matches_device_path(rig0):
+    ev = g.make_event(rig0.ch, 3, n_noise=2)
+    hd, _ = rig0.hits(ev.wire, ev.drift)
+    dims = (6, 6, 6, 6, 6)
+    vd = rig0.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+    rig0.ctx.synchronize()
+    vh = rig0.ctx.ia_vote_host(b.hits_of(ev.wire, ev.drift), LO, HI, dims)
+    assert (vd.cpu().numpy() == vh).all()
+    assert rig0.ctx.ia_launch_count() > 0
