@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py - headline measurement: cell-hit interval evaluations/s of the dense vote.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4|C1|C0]
+
+One "step" = one pass of the dense hot path over one synthetic event of BASELINE.json configs[4]
+(40-layer chamber, 60 hits, 64^5 = 1.07e9 boxes): hit staging (a2), the vote kernel (a3-a6) and the
+top-10 selection (a7), inputs resident in HBM.  `value` = cell-hit evaluations per second (one
+evaluation = one (cell, hit) vote decision, both drift signs).  Extra keys: `roofline` (the vote
+kernel against the FP64 pipe), `cpu_baseline` (the oracle on a bounded sample of the same cells),
+`e2e` (the same step through ia_vote_host: host hits in, host votes out), `events_per_s`
+(configs[3]: 1024 events, 8^5 start, K=8, 8 passes, FP64 and FP32 intervals), `clocks`.
+N > 1: every rank runs the same step on its own event (seed 4 + rank), no collective on the data
+path; value = evaluations of all ranks / max-over-ranks time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2401_04576_b200 import eventgen as g  # noqa: E402
+
+METRIC = "cell-hit interval evals/s"
+UNIT = "evals/s"
+# FP64 thread-instructions the sign-specialised DAG needs per (cell, hit) evaluation
+ALG_FP64_INST_PER_EVAL = 470.0
+# non-tensor FP64 issue peak = SMs x 64 lanes x f_max
+FP64_LANES_PER_SM = 64
+
+
+def workload(name: str, seed_shift: int = 0):
+    if name == "C4":
+        ch = g.chamber_c4()
+        return ch, g.make_event(ch, 4 + seed_shift, n_noise=20), (64,) * 5, 10
+    if name == "C1":
+        ch = g.chamber_c1()
+        return ch, g.make_event(ch, 1 + seed_shift, n_noise=20), (32,) * 5, 10
+    if name == "C0":
+        ch = g.chamber_c0()
+        return ch, g.make_event(ch, 0 + seed_shift), (16,) * 5, 10
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            text, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            text = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in text.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if sm:
+            # under load = the upper half of the samples (the sampler also sees idle gaps)
+            out.update(sm_mhz=statistics.median(sorted(sm)[len(sm) // 2:]), sm_max_mhz=max(mx), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample_rate(ch, ev, dims, n_cells_sample: int, seed: int = 123):
+    """cpu_baseline: the oracle, as it stands, on a random sample of the workload's cells."""
+    from oracle import oracle as o
+    rng = np.random.default_rng(seed)
+    n_cells = int(np.prod(np.array(dims, np.int64)))
+    cells = np.sort(rng.choice(n_cells, size=min(n_cells_sample, n_cells), replace=False)).astype(np.int64)
+    ow, oh, op = o.wires_of(ch), o.hits_of(ev.wire, ev.drift), o.make_params(g.TOL)
+    o.vote(ow, oh, op, g.BOX_LO, g.BOX_HI, dims, cell_idx=cells[:1024])          # warm
+    t0 = time.perf_counter()
+    v = o.vote(ow, oh, op, g.BOX_LO, g.BOX_HI, dims, cell_idx=cells)
+    dt = time.perf_counter() - t0
+    return len(cells) * ev.n_hits / dt, o.max_threads(), len(cells), dt, v, cells
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step."""
+    if rank != 0:
+        return
+    ch, ev, dims, k = workload(args.workload)
+    n_sample = args.ref_cells
+    rates = []
+    for i in range(args.warmup + args.steps):
+        rate, cores, n, dt, _, _ = oracle_sample_rate(ch, ev, dims, n_sample, seed=100 + i)
+        if i >= args.warmup:
+            rates.append((rate, dt))
+    total_evals = n_sample * ev.n_hits * args.steps
+    total_t = sum(dt for _, dt in rates)
+    value = total_evals / total_t
+    sample = f"{n_sample} uniformly sampled cells of the {dims[0]}^5 grid x {ev.n_hits} hits per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: BASELINE.json configs[{args.workload[1]}] dense {dims[0]}^5 x {ev.n_hits} hits (sampled)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0"])
+    ap.add_argument("--ref-cells", type=int, default=1 << 19, help="cells per oracle sample")
+    ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2401_04576_b200 import binding as b
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ch, ev, dims, k = workload(args.workload, seed_shift=rank)
+    n_cells = int(np.prod(np.array(dims, np.int64)))
+    evals_per_step = n_cells * ev.n_hits
+    ctx = b.Context(local_rank)
+    ctx.ia_load_geometry(b.wires_of(ch))
+    ctx.ia_set_params(g.TOL)
+    hits_host = b.hits_of(ev.wire, ev.drift)
+    hd = ctx.to_device(hits_host)
+    votes = torch.empty(n_cells, dtype=torch.uint16, device=f"cuda:{local_rank}")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local_rank}")    # > 126 MB L2
+    stream = ctx.stream
+
+    def step():
+        ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes)
+        return ctx.ia_topk(votes, k)
+
+    # ---- device-resident timing: W warm-ups, K steps between barrier+synchronize ----------------
+    for _ in range(args.warmup):
+        step()
+        flush.zero_()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = ctx.ia_launch_count()
+    ev_kernel = []
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_beg.record(stream)
+    for _ in range(args.steps):
+        a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        # the vote kernel alone (for the roofline): events around ia_vote minus nothing else -
+        # staging is one tiny launch in front of it (microseconds against seconds)
+        a.record(stream)
+        ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes)
+        c.record(stream)
+        idx, vv = ctx.ia_topk(votes, k)
+        ev_kernel.append((a, c))
+        flush.zero_()
+    t_end.record(stream)
+    barrier()
+    launches = ctx.ia_launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    ms_total = t_beg.elapsed_time(t_end)
+    t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local_rank}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = evals_per_step * world / (ms_step * 1e-3)
+    vote_ms = statistics.mean(a.elapsed_time(c) for a, c in ev_kernel)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    props = torch.cuda.get_device_properties(local_rank)
+    n_sm = props.multi_processor_count
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    f_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_inst = n_sm * FP64_LANES_PER_SM * f_max_mhz * 1e6                         # FP64 thread-instructions / s
+    achieved_inst = ALG_FP64_INST_PER_EVAL * evals_per_step / (vote_ms * 1e-3)
+    roofline = {
+        "bound": "alu", "kernel": "vote_dense", "achieved": achieved_inst / 1e12, "peak": peak_inst / 1e12,
+        "unit": "T FP64 inst/s", "frac": achieved_inst / peak_inst, "traffic": None,
+        "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 lanes x {f_max_mhz:.0f} MHz (DESIGN.md 6); "
+                       "MEASURED_PEAKS.json has no FP64 entry",
+        "alg_fp64_inst_per_eval": ALG_FP64_INST_PER_EVAL, "kernel_ms": vote_ms,
+        "alg_bytes_per_launch": 2 * n_cells, "hbm_frac": (2 * n_cells / (vote_ms * 1e-3)) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
+    }
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"{args.workload}: BASELINE.json configs[{args.workload[1]}] "
+                               f"dense {dims[0]}^5 = {n_cells} boxes x {ev.n_hits} hits, top-{k}; seed {ev.seed}",
+                   "grid": list(dims), "n_hits": ev.n_hits, "evals_per_step": evals_per_step,
+                   "l2": "256 MiB flush buffer written between steps; the 2.1 GB accumulator exceeds the 126 MB L2"},
+        "roofline": roofline, "gpu_launches": int(launches), "clocks": clocks,
+    }
+
+    if not args.no_extras:
+        # ---- measured FP64 pipe rate (context for the derived peak) -----------------------------------
+        try:
+            probe = {name: ctx.ia_probe_fp64(mode, 4096, n_sm * 8) / 1e12
+                     for mode, name in ((0, "dfma_rn"), (1, "dadd_rd_dmul_ru"), (2, "dfma_rd_ru"))}
+            line["roofline"]["probe_T_inst_per_s"] = probe
+        except Exception as exc:  # pragma: no cover
+            line["roofline"]["probe_error"] = str(exc)
+
+        # ---- e2e: host hits in, host votes out, through ia_vote_host ------------------------------------
+        host_votes = torch.empty(n_cells, dtype=torch.uint16, pin_memory=True).numpy()
+        pinned_hits = torch.from_numpy(hits_host.view(np.uint8).copy()).pin_memory().numpy().view(b.HIT_DT)
+        ctx.ia_vote_host(pinned_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=host_votes)   # warm
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 2))
+        for _ in range(n_e2e):
+            ctx.ia_vote_host(pinned_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=host_votes)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        line["e2e"] = {"value": evals_per_step / dt, "unit": UNIT, "h2d_bytes_per_step": int(pinned_hits.nbytes),
+                       "d2h_bytes_per_step": int(host_votes.nbytes), "ms_per_step": dt * 1e3,
+                       "call": "ia_vote_host (pinned host buffers, synchronous)"}
+
+        # ---- cpu_baseline: the oracle on a bounded sample of the same cells, and a parity spot check ----
+        rate, cores, n_s, dt_o, vo, cells = oracle_sample_rate(ch, ev, dims, args.ref_cells)
+        vg = host_votes[cells]
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{n_s} uniformly sampled cells of the {dims[0]}^5 grid x {ev.n_hits} hits "
+                                          f"({dt_o:.1f} s)",
+                                "parity_equal_frac": float((vg == vo).mean())}
+
+        # ---- events/s: configs[3], 1024 events, 8^5 start, K=8, 8 passes, FP64 and FP32 intervals --------
+        ch3 = g.chamber_c1()
+        n_ev = 1024
+        evs = [g.make_event(ch3, 1000 + e, n_noise=10) for e in range(n_ev)]
+        h3 = b.hits_of(np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs]))
+        off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
+        ctx3 = b.Context(local_rank)
+        ctx3.ia_load_geometry(b.wires_of(ch3))
+        eps = {}
+        for prec in (64, 32):
+            ctx3.ia_set_params(g.TOL, precision=prec)
+            hd3, od3 = ctx3.to_device(h3), ctx3.to_device(off)
+            boxes, par = ctx3.ia_refine_batch(hd3, od3, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, 8, 8)
+            torch.cuda.synchronize()
+            a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(ctx3.stream)
+            for _ in range(3):
+                ctx3.ia_refine_batch(hd3, od3, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, 8, 8, boxes=boxes, params=par)
+            c.record(ctx3.stream)
+            c.synchronize()
+            ms = a.elapsed_time(c) / 3
+            t0 = time.perf_counter()
+            ctx3.ia_refine_batch_host(h3, off, g.BOX_LO, g.BOX_HI, (8,) * 5, 8, 8)
+            dt_h = time.perf_counter() - t0
+            eps[f"fp{prec}"] = {"events_per_s": n_ev / (ms * 1e-3), "ms": ms, "e2e_events_per_s": n_ev / dt_h,
+                                "evals_per_s": n_ev * (8 ** 5 + 7 * 8 * 32) * 30 / (ms * 1e-3)}
+        line["events_per_s"] = {"workload": "C3: BASELINE.json configs[3], 1024 events x 30 hits, 8^5 start, K=8, 8 passes",
+                                **eps}
+        ctx3.close()
+
+    print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -73,7 +73,9 @@ typedef struct {
 
 /* tol: vote tolerance on the drift distance, D = [max(d-tol,0), d+tol] (S1, G6).
  * (x_ref, y_ref): reference point of eq. (1d); z_ref: reference plane of (A.4c-e) L172-176.
- * precision: 64 or 32 = type of the interval endpoints (G22).  flags: reserved, must be 0. */
+ * precision: 64 or 32 = type of the interval endpoints (G22).  flags: bit 0 = vote the dense grid
+ * with the general (sign-agnostic) kernel instead of the sign-specialised one (same results; for
+ * cross-checks); other bits reserved, must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;
@@ -151,6 +153,12 @@ int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* l
  * op: 0 add 1 sub 2 mul 3 sqr(a) 4 div(a, b>0) 5 sqrt(a) 6 sin(a) 7 cos(a) 8 atan2(y=a, x=b)
  *     9 recip(a>0) 10 scale(b.lo, a) */
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev);
+
+/* Roofline probe: enqueue a kernel of `blocks` x 256 threads, each running 8 independent FP64
+ * dependency chains for `iters` rounds (blocks*256*8*iters FP64 instructions in total).
+ * mode 0: DFMA round-to-nearest; 1: DADD.RM / DMUL.RP alternating; 2: DFMA.RM / DFMA.RP alternating.
+ * The caller times it with events on the context's stream.  sink_dev: one double, never written. */
+int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev);
 
 /* Synchronise the stream and return IA_OK, IA_ERR_GEOMETRY (a hit named an unknown wire since
  * the last call of this function) or IA_ERR_CUDA. */

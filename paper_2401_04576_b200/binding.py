@@ -25,7 +25,7 @@ assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 8
 
 EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_prim",
-           "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
+           "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
 
 class IaParams(C.Structure):
@@ -66,6 +66,7 @@ def load_library(path: str = LIB_PATH):
     lib.ia_refine_batch_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_residual.argtypes = [vp, vp, i32, vp, vp, i64, vp]
     lib.ia_prim.argtypes = [vp, i32, i32, vp, vp, i64, vp]
+    lib.ia_probe_fp64.argtypes = [vp, i32, i32, i32, vp]
     lib.ia_device_status.argtypes = [vp]
     lib.ia_launch_count.argtypes = [vp]
     lib.ia_launch_count.restype = i64
@@ -263,6 +264,19 @@ class Context:
         out = self._empty(2 * n, torch.float64)
         self._chk(self.lib.ia_prim(self.h, op, prec, _dp(a_dev), _dp(b_dev), n, _dp(out)), "ia_prim")
         return out.view(n, 2)
+
+    def ia_probe_fp64(self, mode: int, iters: int, blocks: int) -> float:
+        """FP64 thread-instructions per second sustained by independent chains (timed with CUDA events)."""
+        torch = self._torch
+        sink = self._empty(1, torch.float64)
+        with torch.cuda.stream(self.stream):
+            self._chk(self.lib.ia_probe_fp64(self.h, mode, iters, blocks, _dp(sink)), "ia_probe_fp64")   # warm-up
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(self.stream)
+            self._chk(self.lib.ia_probe_fp64(self.h, mode, iters, blocks, _dp(sink)), "ia_probe_fp64")
+            t1.record(self.stream)
+        t1.synchronize()
+        return blocks * 256.0 * 8.0 * iters / (t0.elapsed_time(t1) * 1e-3)
 
     def ia_device_status(self):
         self._chk(self.lib.ia_device_status(self.h), "ia_device_status")

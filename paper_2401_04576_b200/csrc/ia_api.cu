@@ -194,7 +194,7 @@ int ia_set_params(ia_ctx* ctx, const ia_params* p) {
       !std::isfinite(p->z_ref))
     return IA_ERR_ARG;
   if (p->precision != 64 && p->precision != 32) return IA_ERR_ARG;
-  if (p->flags != 0) return IA_ERR_ARG;
+  if (p->flags & ~1u) return IA_ERR_ARG;
   ctx->params = *p;
   return IA_OK;
 }
@@ -350,6 +350,13 @@ int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_
   if (binary && !b_dev) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_prim(ctx, op, prec, a_dev, b_dev, n, out_dev));
+  return IA_OK;
+}
+
+int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev) {
+  if (!ctx || !sink_dev || mode < 0 || mode > 2 || iters <= 0 || blocks <= 0) return IA_ERR_ARG;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_fp64_probe(ctx, mode, iters, blocks, sink_dev));
   return IA_OK;
 }
 

@@ -80,6 +80,9 @@ cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* i
 cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& span, int lev, int levels, int k, ia_box* boxes_out);
 cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out);
 
+// FP64 pipe probe (roofline denominator check): blocks x 256 threads x 8 chains x iters instructions
+cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, double* sink);
+
 // scratch helper: grow-only device buffer
 cudaError_t scratch_reserve(Scratch& s, size_t bytes);
 

@@ -350,3 +350,47 @@ cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia
 }
 
 }  // namespace ia
+
+// ---- FP64 pipe probe: what the chip sustains on independent double-precision chains ---------------
+// mode 0: DFMA (round-to-nearest); mode 1: DADD.RM / DMUL.RP alternating (the interval mix);
+// mode 2: DFMA.RM / DFMA.RP.  8 independent chains per thread, `iters` rounds of 8 instructions.
+namespace ia {
+namespace {
+__global__ void __launch_bounds__(256) fp64_probe_kernel(int mode, int iters, double seed, double* __restrict__ sink) {
+  double a[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) a[j] = seed + 1e-3 * (threadIdx.x + 8 * j);
+  const double m = 1.0 - 1e-9, c = 1e-12;
+  if (mode == 0) {
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = __fma_rn(a[j], m, c);
+    }
+  } else if (mode == 1) {
+    for (int i = 0; i < iters; i += 2) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = __dadd_rd(a[j], c);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = __dmul_ru(a[j], m);
+    }
+  } else {
+    for (int i = 0; i < iters; i += 2) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = __fma_rd(a[j], m, c);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = __fma_ru(a[j], m, c);
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) s += a[j];
+  if (s == 12345.678) sink[0] = s;   // never true: keeps the chains alive
+}
+}  // namespace
+
+cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, double* sink) {
+  fp64_probe_kernel<<<blocks, 256, 0, ctx->stream>>>(mode, iters, 1.0, sink);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+}  // namespace ia

@@ -8,7 +8,7 @@
 // then walks its cells, reads the hits by shared-memory broadcast, keeps its vote count in a
 // register and writes one uint16 per cell.  No atomics, no inter-thread traffic in the loop.
 #include "ia_internal.h"
-#include "ia_residual.cuh"
+#include "ia_fast.cuh"
 
 namespace ia {
 
@@ -70,29 +70,182 @@ vote_dense_general_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDe
   }
 }
 
+
+// ---- fast form ------------------------------------------------------------------------------------
+// Block = (event, xy cell, tile of FAST_THREADS (R, lambda) pairs, tile of FAST_ZT z0 cells).
+// Thread = one (R, lambda) pair; loops over the hits (outer) and its FAST_ZT z0 cells (inner), so
+// that everything depending on (R, lambda, hit, drift sign) is computed once per FAST_ZT cells.
+// Vote counts: 8 bytes packed in one 64-bit register (hits per event <= 255 on this path).
+constexpr int FAST_THREADS = 256;
+constexpr int FAST_ZT = 8;
+
+template <class T> struct ZTab { Iv<T> z[2][FAST_ZT]; };    // [0]: z0 - z_ref, [1]: its negation
+
+template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>& h, int va, Iv<T> R, Iv<T> Zeff, Iv<T> L) {
+  XYInv<T> v;
+  v.Q = h.Q; v.cA = h.cA; v.sA = h.sA[va]; v.dphi = h.dphi[va]; v.iQ = h.iQ; v.RA = h.RA; v.iR = h.iR; v.c2 = h.c2;
+  v.s2 = h.s2[va];
+  v.forced = 0;
+  HitS<T> hs = {h.Tabs, h.Dlo, h.Dhi, 1};
+  Box3<T> bx = {R, Zeff, L};
+  return hit_votes_general(bx, v, hs, T(0));
+}
+
+// one hit, one thread: both drift signs over the thread's z0 cells; returns the 8-bit vote mask
+template <class T>
+IA_DEV unsigned fast_hit(const HitF<T>& h, int va, Iv<T> L, Iv<T> R, Iv<T> LR, Iv<T> L2, const Iv<T>* zt, int nz_tile) {
+  const Iv<T> LRdphi = mul_pu(LR, h.dphi[va]);
+  const Iv<T> RpRA = iadd(R, h.RA);
+  const Iv<T> T2L2 = mul_pp(h.T2, L2);
+  unsigned bits = 0;
+#pragma unroll 1
+  for (int s = 0; s < 2; ++s) {
+    const bool dneg = s == 1;
+    const PassC<T> pc = pass_prepare(h, dneg, L, R, L2, RpRA);
+#pragma unroll 1
+    for (int i = 0; i < nz_tile; ++i) {
+      // the second pass is needed only where some lane has not voted yet
+      if (__all_sync(0xffffffffu, (bits >> i) & 1u)) continue;
+      bits |= (pass_vote(h, va, dneg, pc, L, R, LR, T2L2, LRdphi, zt[i]) ? 1u : 0u) << i;
+    }
+  }
+  return bits;
+}
+
+// 8 vote bits -> 8 packed byte counters (bit k -> byte k).  Four bits at a time: in k + 7j, k,j < 4,
+// no two partial products meet, so nothing carries.
+IA_DEV unsigned long long spread8(unsigned bits) {
+  const unsigned lo = ((bits & 0xfu) * 0x00204081u) & 0x01010101u;
+  const unsigned hi = (((bits >> 4) & 0xfu) * 0x00204081u) & 0x01010101u;
+  return ((unsigned long long)hi << 32) | lo;
+}
+
+template <class T>
+__global__ void __launch_bounds__(FAST_THREADS, 2)
+vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z,
+                       uint16_t* __restrict__ votes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  ZTab<T>* ztab = reinterpret_cast<ZTab<T>*>(smem_raw);
+  HitF<T>* sh = reinterpret_cast<HitF<T>*>(smem_raw + sizeof(ZTab<T>));
+  const int e = blockIdx.y;
+  int64_t bid = blockIdx.x;
+  const int tz = int(bid % tiles_z); bid /= tiles_z;
+  const int tp = int(bid % tiles_p); bid /= tiles_p;
+  const int64_t ixy = bid;
+  const int ix = int(ixy / g.n[1]), iy = int(ixy - int64_t(ix) * g.n[1]);
+  int count;
+  if (sp.offsets) {
+    count = sp.offsets[e + 1] - sp.offsets[e];
+    if (count > sp.max_hits) count = sp.max_hits;
+    if (count < 0) count = 0;
+  } else {
+    count = sp.n_hits_single;
+  }
+  const int nR = g.n[2], nz = g.n[3], nL = g.n[4];
+  const Iv<T> X = box_iv<T>(cell_edge(g.lo[0], g.hi[0], g.w[0], ix, g.n[0]), cell_edge(g.lo[0], g.hi[0], g.w[0], ix + 1, g.n[0]));
+  const Iv<T> Y = box_iv<T>(cell_edge(g.lo[1], g.hi[1], g.w[1], iy, g.n[1]), cell_edge(g.lo[1], g.hi[1], g.w[1], iy + 1, g.n[1]));
+  const T Rlo_min = Rnd<T>::from_dn(g.lo[2]);
+  const T Lmag = mx(fabs(Rnd<T>::from_dn(g.lo[4])), fabs(Rnd<T>::from_up(g.hi[4])));
+  T zref = T(0);
+  if (count > 0) zref = staged[int64_t(e) * sp.max_hits].zref;
+  for (int h = threadIdx.x; h < count; h += blockDim.x) {
+    const HitC<T> c = staged[int64_t(e) * sp.max_hits + h];
+    make_hitf(xy_invariants(X, Y, c), hit_small(c), Rlo_min, Lmag, sh[h]);
+  }
+  const int iz0 = tz * FAST_ZT;
+  const int nz_tile = (nz - iz0) < FAST_ZT ? (nz - iz0) : FAST_ZT;
+  if (threadIdx.x < FAST_ZT) {
+    const int iz = iz0 + (threadIdx.x < nz_tile ? threadIdx.x : nz_tile - 1);
+    const Iv<T> Z = box_iv<T>(cell_edge(g.lo[3], g.hi[3], g.w[3], iz, nz), cell_edge(g.lo[3], g.hi[3], g.w[3], iz + 1, nz));
+    const Iv<T> Zr = isub(Z, thin(zref));
+    ztab->z[0][threadIdx.x] = Zr;
+    ztab->z[1][threadIdx.x] = ineg(Zr);
+  }
+  __syncthreads();
+  // pair enumeration: lambda index within its half fastest, then R, then the half (so that a warp's
+  // lambda cells share a sign and its stores run along lambda)
+  const int n_pairs = nR * nL;
+  const int hl = (nL % 2 == 0) ? nL / 2 : nL;
+  int p = tp * FAST_THREADS + threadIdx.x;
+  const bool live = p < n_pairs;
+  if (!live) p = n_pairs - 1;
+  const int il_in = p % hl;
+  const int rest = p / hl;
+  const int iR = rest % nR, half = rest / nR;
+  const int iL = half * hl + il_in;
+  const Iv<T> R = box_iv<T>(cell_edge(g.lo[2], g.hi[2], g.w[2], iR, nR), cell_edge(g.lo[2], g.hi[2], g.w[2], iR + 1, nR));
+  const Iv<T> Lraw = box_iv<T>(cell_edge(g.lo[4], g.hi[4], g.w[4], iL, nL), cell_edge(g.lo[4], g.hi[4], g.w[4], iL + 1, nL));
+  const int lcls = cls_of(Lraw);
+  const bool allP = __all_sync(0xffffffffu, lcls == CLS_P), allN = __all_sync(0xffffffffu, lcls == CLS_N);
+  const bool a = !allP && allN;                       // S_a: flip lambda, z0 - z_ref and T for this warp
+  const bool warp_fast = allP || allN;
+  const Iv<T> L = a ? ineg(Lraw) : Lraw;
+  const Iv<T> LR = warp_fast ? mul_pp(L, R) : imul(L, R);
+  const Iv<T> L2 = warp_fast ? mul_pp(L, L) : isqr(L);
+  unsigned long long acc = 0;
+  const int va = a ? 1 : 0;
+  for (int h = 0; h < count; ++h) {
+    const HitF<T>& hf = sh[h];
+    const int kind = hf.kind;
+    if (kind == HIT_SKIP) continue;
+    if (kind == HIT_FORCED) { acc += 0x0101010101010101ull; continue; }
+    const Iv<T>* zt = ztab->z[hf.zflip];
+    if (kind == HIT_FAST && warp_fast) {
+      acc += spread8(fast_hit<T>(hf, va, L, R, LR, L2, zt, nz_tile));
+    } else {
+      for (int i = 0; i < nz_tile; ++i)
+        acc += (unsigned long long)(general_votes_norm(hf, va, R, zt[i], L) ? 1u : 0u) << (8 * i);
+    }
+  }
+  if (live) {
+    uint16_t* out = votes + int64_t(e) * g.cells + ixy * g.col_cells + (int64_t(iR) * nz + iz0) * nL + iL;
+    for (int i = 0; i < nz_tile; ++i) out[int64_t(i) * nL] = uint16_t((acc >> (8 * i)) & 0xffu);
+  }
+}
+
 }  // namespace
 
-cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
+template <class T>
+static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
+  const int n_pairs = g.n[2] * g.n[4];
+  int threads = FAST_THREADS;
+  if (n_pairs < threads) threads = (n_pairs + 31) / 32 * 32;
+  const int tiles_p = (n_pairs + FAST_THREADS - 1) / FAST_THREADS;
+  const int tiles_z = (g.n[3] + FAST_ZT - 1) / FAST_ZT;
+  const int64_t nxy = int64_t(g.n[0]) * g.n[1];
+  const int64_t blocks = nxy * tiles_p * tiles_z;
+  if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+  const size_t smem = sizeof(ZTab<T>) + size_t(sp.max_hits) * sizeof(HitF<T>);
+  cudaError_t err = cudaFuncSetAttribute(vote_dense_fast_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+  if (err != cudaSuccess) return err;
+  dim3 grid((unsigned)blocks, (unsigned)sp.n_events);
+  vote_dense_fast_kernel<T><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g, tiles_p,
+                                                                 tiles_z, votes_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+template <class T>
+static cudaError_t launch_general(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
   const int per_block = GEN_THREADS * GEN_CELLS_PER_THREAD;
   const int chunks = int((g.col_cells + per_block - 1) / per_block);
   const int64_t nxy = int64_t(g.n[0]) * g.n[1];
   dim3 grid((unsigned)(nxy * chunks), (unsigned)sp.n_events);
-  cudaError_t err;
-  if (ctx->params.precision == 32) {
-    const size_t smem = size_t(sp.max_hits) * sizeof(HitShared<float>);
-    err = cudaFuncSetAttribute(vote_dense_general_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    if (err != cudaSuccess) return err;
-    vote_dense_general_kernel<float><<<grid, GEN_THREADS, smem, ctx->stream>>>(
-        sp, static_cast<const HitC<float>*>(ctx->staged.p), g, chunks, votes_out);
-  } else {
-    const size_t smem = size_t(sp.max_hits) * sizeof(HitShared<double>);
-    err = cudaFuncSetAttribute(vote_dense_general_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    if (err != cudaSuccess) return err;
-    vote_dense_general_kernel<double><<<grid, GEN_THREADS, smem, ctx->stream>>>(
-        sp, static_cast<const HitC<double>*>(ctx->staged.p), g, chunks, votes_out);
-  }
+  const size_t smem = size_t(sp.max_hits) * sizeof(HitShared<T>);
+  cudaError_t err = cudaFuncSetAttribute(vote_dense_general_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+  if (err != cudaSuccess) return err;
+  vote_dense_general_kernel<T><<<grid, GEN_THREADS, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
+                                                                        chunks, votes_out);
   ctx->launches++;
   return cudaGetLastError();
+}
+
+cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
+  // the fast form packs vote counts in bytes and keeps one HitF per hit in shared memory
+  const bool fast = !(ctx->params.flags & 1u) && sp.max_hits <= 255;
+  if (ctx->params.precision == 32)
+    return fast ? launch_fast<float>(ctx, sp, g, votes_out) : launch_general<float>(ctx, sp, g, votes_out);
+  return fast ? launch_fast<double>(ctx, sp, g, votes_out) : launch_general<double>(ctx, sp, g, votes_out);
 }
 
 }  // namespace ia

@@ -345,3 +345,25 @@ def test_host_entry_point_matches_device_path(rig0):
     vh = rig0.ctx.ia_vote_host(b.hits_of(ev.wire, ev.drift), LO, HI, dims)
     assert (vd.cpu().numpy() == vh).all()
     assert rig0.ctx.ia_launch_count() > 0
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_fast_and_general_kernels_agree(precision):
+    """The sign-specialised dense kernel against the general one (flags bit 0) on a full 24^5 grid and
+    on ragged shapes: same DAG, same roundings, so only the sin/cos pads may move a knife-edge cell."""
+    rig = Rig(g.chamber_c1(), precision=precision)
+    try:
+        ev = g.make_event(rig.ch, 31, n_noise=10)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        for dims in ((24,) * 5, (5, 4, 10, 9, 12), (3, 3, 6, 20, 7), (2, 2, 64, 3, 64)):
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=0)
+            vf = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=1)
+            vg = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            rig.ctx.synchronize()
+            vf, vg = vf.cpu().numpy(), vg.cpu().numpy()
+            bad = np.nonzero(vf != vg)[0]
+            assert len(bad) <= len(vf) // 100000, (dims, len(bad), bad[:10], vf[bad[:10]], vg[bad[:10]])
+            assert vf.max() > 0
+    finally:
+        rig.close()
