@@ -33,8 +33,9 @@ from paper_2401_04576_b200 import eventgen as g  # noqa: E402
 
 METRIC = "cell-hit interval evals/s"
 UNIT = "evals/s"
-# FP64 thread-instructions the sign-specialised DAG needs per (cell, hit) evaluation
-ALG_FP64_INST_PER_EVAL = 470.0
+# FP64 arithmetic thread-instructions (DADD/DMUL/DFMA, comparisons not counted) that the
+# sign-specialised DAG S4-S8 needs per (cell, hit) evaluation = both drift signs; counted op by op there
+ALG_FP64_INST_PER_EVAL = 366.0
 # non-tensor FP64 issue peak = SMs x 64 lanes x f_max
 FP64_LANES_PER_SM = 64
 
@@ -146,7 +147,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0"])
-    ap.add_argument("--ref-cells", type=int, default=1 << 19, help="cells per oracle sample")
+    ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
