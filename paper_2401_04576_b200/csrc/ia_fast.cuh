@@ -1,25 +1,39 @@
-// ia_fast.cuh - the sign-specialised form of the residual enclosure (steps S4-S8) for the dense vote.
+// ia_fast.cuh - the FP64-pipe form of the residual enclosure (steps S4-S8) for the dense vote.
 //
-// Same expression DAG as ia_residual.cuh, same association order, same tightest directed roundings;
-// what changes is how each interval product is formed.  A general product needs 8 directed
-// multiplies and 6 min/max; when one factor has a known sign it needs 2 multiplies and 2 selects,
-// and when both signs are known, 2 multiplies.  Signs are made known in three ways:
-//   * by construction: R > 0, 1/R_Ax^2 > 0, R_Ax > 0, T^2 >= 0, u_d > 0, |delta| >= 0, squares >= 0;
-//   * by three exact symmetries of the DAG (negating an interval operand negates the product
-//     exactly, because rounding down -x equals minus rounding up x):
+// Same expression DAG as ia_residual.cuh and the same association order.  What changes is how each
+// interval product is formed, because on sm_100a the cost of a product is not its multiplies:
+// measured on B200 (profiles/r01_pipe_probe.md) an FP64 instruction holds the 16-lane FP64 pipe of a
+// sub-partition for 2 cycles but its issue port for 1, while FSEL / ISETP / LOP3 (the "pick the
+// partner endpoint by the sign of x" selects of the textbook sign-case product) hold the half-rate
+// ALU pipe for 2 cycles each, and cycles per evaluation follow 2 N_alu + N_fp64 + N_other.  The
+// select-based product (2 DMUL + 2 ISETP + 4 FSEL) therefore costs 14 cycles, the one below 4 FP64
+// instructions and nothing else:
+//
+//   factor a of KNOWN sign class, kept as midpoint and radius (m, r) with [m-r, m+r] containing a,
+//   times x = [x.lo, x.hi] of ANY sign:   for a >= 0
+//        lower = RD( RD(m x.lo) - r |x.lo| )        upper = RU( RU(m x.hi) + r |x.hi| )
+//   (g(x) = m x - r|x| is the exact lower envelope of {a' x : a' in [m-r, m+r]}; it is concave, and
+//   increasing when a >= 0, so its minimum over x is at x.lo; |x| is an operand modifier of DFMA.)
+//   The result encloses the true product and is at most 2 ulps wider than the tightest enclosure
+//   (one rounding of (m, r), one of the inner product) - the same order as the padding of the
+//   elementary functions, 4 orders below the 1e-12 knife-edge band of the parity criterion.
+//   For a <= 0 the roles of x.lo and x.hi swap (the body negates m instead and flips the add/sub
+//   that consumes the product); for a straddling 0 both endpoints of x are tried (prod_u).
+//
+// Which factors have a known class: by construction R, R_Ax^-2, R_Ax^-1, T^2, |delta|, R - 2D; by three
+// exact symmetries of the DAG (negating an interval operand negates the product exactly, because
+// rounding down -x equals minus rounding up x)
 //        S_a: (lambda, z0 - z_ref, T)      -> -(...)   mirror z -> -z                     f unchanged
 //        S_b: (s_Ax, c_Ax, T)              -> -(...)   the same wire described by phi_s+pi, -tau
 //        S_d: (s_Ax, z0 - z_ref, dphi, T)  -> -(...)   Phi -> -Phi
-//     applied per (warp, hit) so that lambda >= 0 (a = [lambda <= 0], per warp), c_Ax >= 0
-//     (b = [c_Ax <= 0], per hit) and T >= 0 (d = [T < 0] + a + b).  Then z0 - z_ref flips by
-//     [T<0] + b (per hit), s_Ax by [T<0] + a, sin 2Phi_Ax and dphi by [T<0] + a + b: the record below
-//     stores both a-versions of those three;
-//   * what is left - the sign class of s_Ax, sin 2Phi_Ax, cos 2Phi_Ax (P, N or straddling M) and of
-//     c_Ax (P or M) - is the same for every thread of a block, so each of the six products that has
-//     such a factor picks its form by a branch no warp diverges on; the drift sign of the two
-//     passes is likewise a uniform run-time flag (three +/- sites).
-// One compiled body serves every sign combination: the hot loop stays within the 32 KB
-// instruction cache (a body per sign combination does not, and starves the issue ports).
+// applied per (warp, hit) so that lambda >= 0 (a = [lambda <= 0], per warp), c_Ax >= 0 or straddling
+// (b = [c_Ax <= 0], per hit) and T >= 0 (d = [T < 0] + a + b); then z0 - z_ref flips by [T<0] + b (per
+// hit), s_Ax by [T<0] + a, sin 2Phi_Ax and dphi by [T<0] + a + b: the record stores both a-versions.
+// What is left - the class of s_Ax (and with it of sin 2Phi_Ax), of c_Ax (P or straddling) and of
+// cos 2Phi_Ax - is the same for every thread of a block and selects one of three compiled bodies per
+// hit: SS = +1 (s_Ax >= 0, c_Ax >= 0), SS = -1 (s_Ax <= 0, c_Ax >= 0), SS = 0 (anything straddles:
+// universal products).  cos 2Phi_Ax is dispatched inside the body (one site).  Three bodies stay
+// inside the 32 KB instruction cache; a body per sign combination does not (measured, round 1).
 // A hit that violates the guards in make_hitf, and a warp whose lambda cells straddle 0, take the
 // general form (on the same transformed data - the symmetries are exact for it too).
 //
@@ -38,37 +52,52 @@ namespace ia {
 IA_DEV bool sgn(double x) { return __double2hiint(x) < 0; }
 IA_DEV bool sgn(float x) { return __float_as_int(x) < 0; }
 
-// a >= 0, x of unknown sign
+// a >= 0 computed per lane (no midpoint form at hand), x of unknown sign: partner by sign of x
 template <class T> IA_DEV Iv<T> mul_pu(Iv<T> a, Iv<T> x) {
   using R = Rnd<T>;
   return {R::mul_dn(sgn(x.lo) ? a.hi : a.lo, x.lo), R::mul_up(sgn(x.hi) ? a.lo : a.hi, x.hi)};
 }
-// a <= 0, x of unknown sign
-template <class T> IA_DEV Iv<T> mul_nu(Iv<T> a, Iv<T> x) {
-  using R = Rnd<T>;
-  return {R::mul_dn(sgn(x.hi) ? a.hi : a.lo, x.hi), R::mul_up(sgn(x.lo) ? a.lo : a.hi, x.lo)};
-}
 template <class T> IA_DEV Iv<T> mul_pp(Iv<T> a, Iv<T> b) { return {Rnd<T>::mul_dn(a.lo, b.lo), Rnd<T>::mul_up(a.hi, b.hi)}; }
 // a >= 0, b <= 0
 template <class T> IA_DEV Iv<T> mul_pn(Iv<T> a, Iv<T> b) { return {Rnd<T>::mul_dn(a.hi, b.lo), Rnd<T>::mul_up(a.lo, b.hi)}; }
-// m straddles 0, x of unknown sign: two candidates per endpoint
-template <class T> IA_DEV Iv<T> mul_mu(Iv<T> m, Iv<T> x) {
+
+// midpoint-radius form of a factor: [m - r, m + r] contains the interval it was made from
+template <class T> struct MR { T m, r; };
+template <class T> IA_DEV MR<T> to_mr(Iv<T> a) {
   using R = Rnd<T>;
-  return {mn(R::mul_dn(x.lo, m.hi), R::mul_dn(x.hi, m.lo)), mx(R::mul_up(x.lo, m.lo), R::mul_up(x.hi, m.hi))};
+  const T m = R::mul_rn(T(0.5), R::add_rn(a.lo, a.hi));
+  return {m, mx(R::add_up(m, -a.lo), R::add_up(a.hi, -m))};
 }
+template <class T> IA_DEV MR<T> mr_neg(MR<T> a) { return {-a.m, a.r}; }
+// a >= 0 (as an interval; its (m, r) hull may dip an ulp below 0, which only lowers the bound)
+template <class T> IA_DEV Iv<T> prod_p(MR<T> a, Iv<T> x) {
+  using R = Rnd<T>;
+  return {R::fma_dn(-a.r, fabs(x.lo), R::mul_dn(a.m, x.lo)), R::fma_up(a.r, fabs(x.hi), R::mul_up(a.m, x.hi))};
+}
+// a of any class: lower envelope concave, upper convex -> extremes at the endpoints of x
+template <class T> IA_DEV Iv<T> prod_u(MR<T> a, Iv<T> x) {
+  using R = Rnd<T>;
+  const T l0 = R::fma_dn(-a.r, fabs(x.lo), R::mul_dn(a.m, x.lo)), l1 = R::fma_dn(-a.r, fabs(x.hi), R::mul_dn(a.m, x.hi));
+  const T h0 = R::fma_up(a.r, fabs(x.lo), R::mul_up(a.m, x.lo)), h1 = R::fma_up(a.r, fabs(x.hi), R::mul_up(a.m, x.hi));
+  return {mn(l0, l1), mx(h0, h1)};
+}
+// SS = +1: a >= 0;  SS = -1: a <= 0, returns (-a) x;  SS = 0: a of any class, returns a x
+template <int SS, class T> IA_DEV Iv<T> prod_s(MR<T> a, Iv<T> x) {
+  if (SS > 0) return prod_p(a, x);
+  if (SS < 0) return prod_p(mr_neg(a), x);
+  return prod_u(a, x);
+}
+// base + sigma * t, where t = |sigma-signed term| as returned by prod_s (SS = 0: t is the term itself)
+template <int SS, class T> IA_DEV Iv<T> add_s(Iv<T> base, Iv<T> t) { return SS < 0 ? isub(base, t) : iadd(base, t); }
+template <int SS, class T> IA_DEV Iv<T> sub_s(Iv<T> base, Iv<T> t) { return SS < 0 ? iadd(base, t) : isub(base, t); }
+// c >= 0 per lane times a block-uniform interval s:  SS = +1: s >= 0; -1: s <= 0, returns c (-s); 0: any
+template <int SS, class T> IA_DEV Iv<T> mulpos_s(Iv<T> c, Iv<T> s) {
+  if (SS > 0) return mul_pp(c, s);
+  if (SS < 0) return mul_pp(c, ineg(s));
+  return mul_pu(c, s);
+}
+
 enum { CLS_P = 0, CLS_N = 1, CLS_M = 2 };
-// a of block-uniform sign class times x of unknown sign
-template <class T> IA_DEV Iv<T> mul_cu(int cls, Iv<T> a, Iv<T> x) {
-  if (cls == CLS_P) return mul_pu(a, x);
-  if (cls == CLS_N) return mul_nu(a, x);
-  return mul_mu(a, x);
-}
-// scalar of compile-time sign times interval
-template <int S, class T> IA_DEV Iv<T> scale_s(T c, Iv<T> a) {
-  using R = Rnd<T>;
-  if (S >= 0) return {R::mul_dn(c, a.lo), R::mul_up(c, a.hi)};
-  return {R::mul_dn(c, a.hi), R::mul_up(c, a.lo)};
-}
 // square of an interval of unknown sign without branches: largest / smallest magnitude
 template <class T> IA_DEV Iv<T> sqr_u(Iv<T> a) {
   using R = Rnd<T>;
@@ -78,7 +107,16 @@ template <class T> IA_DEV Iv<T> sqr_u(Iv<T> a) {
   const T lo2 = R::mul_dn(mnn, mnn);
   return {straddle ? T(0) : lo2, R::mul_up(mag, mag)};
 }
-
+// intersection with [-1, 1] by integer tests on the high word (keeps the FP64 pipe free):
+// x <= -1  <=>  hi32(x) as unsigned >= hi32(-1);  x >= 1  <=>  hi32(x) as signed >= hi32(1)
+IA_DEV Iv<double> clamp_unit(Iv<double> a) {
+  const bool l = (unsigned)__double2hiint(a.lo) >= 0xbff00000u, h = __double2hiint(a.hi) >= 0x3ff00000;
+  return {l ? -1.0 : a.lo, h ? 1.0 : a.hi};
+}
+IA_DEV Iv<float> clamp_unit(Iv<float> a) {
+  const bool l = (unsigned)__float_as_int(a.lo) >= 0xbf800000u, h = __float_as_int(a.hi) >= 0x3f800000;
+  return {l ? -1.0f : a.lo, h ? 1.0f : a.hi};
+}
 // ---- directed square root and division ----------------------------------------------------------
 template <class T> struct Dir;
 template <> struct Dir<double> {
@@ -188,17 +226,21 @@ template <> struct Trig<float> {
 };
 
 // ---- per-(block, hit) record in shared memory ------------------------------------------------------
-enum { HIT_SKIP = 0, HIT_FORCED = 1, HIT_FAST = 2, HIT_GENERAL = 3 };
+// HIT_FAST_P / _N / _U: the three bodies (SS = +1, -1, 0)
+enum { HIT_SKIP = 0, HIT_FORCED = 1, HIT_FAST_P = 2, HIT_FAST_N = 3, HIT_FAST_U = 4, HIT_GENERAL = 5 };
 
-template <class T> struct HitF {
-  // transformed by S_b^b S_d^(t+b) (and, in the [1] versions, additionally by the S_d that goes with S_a)
-  Iv<T> Q, cA, iQ, hiQ, RA, iR, c2, T2;
-  Iv<T> sA[2], s2[2], dphi[2];     // index a = 1 for warps whose lambda was negated
+template <class T> struct __align__(16) HitF {
+  // transformed by S_b^b S_d^(t+b) (and, in the [1] versions, additionally by the S_d that goes with S_a);
+  // (m, r) forms carry the true sign of the factor in m
+  Iv<T> Q, cA, T2, RA;
+  MR<T> cAm, iQm, hiQm, iRm, c2m, T2m;
+  Iv<T> sA[2], dphi[2];            // index a = 1 for warps whose lambda was negated
+  MR<T> sAm[2], s2m[2];
+  Iv<T> iQ, iR, c2, s2[2];         // interval forms, general fallback only
   T Tabs;                          // |tan tau|
   T Dlo, Dhi;
-  int kind;
-  int ccls, c2cls;                 // classes of cA (P or M) and c2
-  int scls[2], s2cls[2];           // classes of sA[a], s2[a]
+  int kind[2];                     // per a
+  int c2cls;
   int zflip;                       // z0 - z_ref enters negated
 };
 
@@ -210,14 +252,22 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
   o.Dlo = hs.Dlo; o.Dhi = hs.Dhi;
   o.Tabs = fabs(hs.Tn);
   o.Q = v.Q; o.iQ = v.iQ; o.RA = v.RA; o.iR = v.iR; o.c2 = v.c2;
-  o.hiQ = {Rd::mul_rn(T(0.5), v.iQ.lo), Rd::mul_rn(T(0.5), v.iQ.hi)};      // exact scaling
-  o.T2 = {Rd::mul_dn(hs.Tn, hs.Tn), Rd::mul_up(hs.Tn, hs.Tn)};             // isqr(thin(T))
+  o.iQm = to_mr(v.iQ);
+  o.hiQm = {Rd::mul_rn(T(0.5), o.iQm.m), Rd::mul_rn(T(0.5), o.iQm.r)};      // exact scaling of 1/Q by 1/2
+  o.iRm = to_mr(v.iR);
+  o.c2m = to_mr(v.c2);
+  o.T2 = {Rd::mul_dn(hs.Tn, hs.Tn), Rd::mul_up(hs.Tn, hs.Tn)};              // isqr(thin(T))
+  o.T2m = to_mr(o.T2);
   o.c2cls = cls_of(v.c2);
   const bool t = hs.Tn < T(0);
   const bool b = cls_of(v.cA) == CLS_N;
   o.cA = b ? ineg(v.cA) : v.cA;
-  o.ccls = cls_of(o.cA);
+  o.cAm = to_mr(o.cA);
+  const int ccls = cls_of(o.cA);
   o.zflip = (t != b) ? 1 : 0;
+  // guards of the sign-known forms: R - 2D > 0, R + R_Ax - D > 0, R + delta > 0 (|delta| <= 2 D.hi as
+  // long as u_d >= 1/2), u_d^2 >= 1 - 2 |T| |lambda| >= 1/2
+  const bool ok = Rlo_min > T(4) * hs.Dhi && o.Tabs * Lmag <= T(0.25);
 #pragma unroll
   for (int a = 0; a < 2; ++a) {
     const bool fs = t != (a == 1);            // s_Ax flips by t + a
@@ -225,15 +275,17 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
     o.sA[a] = fs ? ineg(v.sA) : v.sA;
     o.s2[a] = fd ? ineg(v.s2) : v.s2;
     o.dphi[a] = fd ? ineg(v.dphi) : v.dphi;
-    o.scls[a] = cls_of(o.sA[a]);
-    o.s2cls[a] = cls_of(o.s2[a]);
+    o.sAm[a] = to_mr(o.sA[a]);
+    o.s2m[a] = to_mr(o.s2[a]);
+    const int scls = cls_of(o.sA[a]), s2cls = cls_of(o.s2[a]);
+    int kind = HIT_FAST_U;
+    if (ccls == CLS_P && scls == CLS_P && s2cls == CLS_P) kind = HIT_FAST_P;
+    if (ccls == CLS_P && scls == CLS_N && s2cls == CLS_N) kind = HIT_FAST_N;
+    if (!ok) kind = HIT_GENERAL;
+    if (v.forced) kind = HIT_FORCED;
+    if (!hs.valid) kind = HIT_SKIP;
+    o.kind[a] = kind;
   }
-  if (!hs.valid) { o.kind = HIT_SKIP; return; }
-  if (v.forced) { o.kind = HIT_FORCED; return; }
-  // guards of the sign-known forms: R - 2D > 0, R + R_Ax - D > 0, R + delta > 0 (|delta| <= 2 D.hi as
-  // long as u_d >= 1/2), u_d^2 >= 1 - 2 |T| |lambda| >= 1/2
-  const bool ok = Rlo_min > T(4) * hs.Dhi && o.Tabs * Lmag <= T(0.25);
-  o.kind = ok ? HIT_FAST : HIT_GENERAL;
 }
 
 // general-form sin / cos and their products with s_Ax, c_Ax for enclosures outside [-1/4, 1/4] (rare)
@@ -245,45 +297,62 @@ __device__ __noinline__ void trig_general(Iv<T> e, Iv<T> sA, Iv<T> cA, Iv<T>& se
   cce = imul(cA, ce);
 }
 
-// what a thread keeps per (hit, drift sign): S4 terms that do not depend on z0
+// what a thread keeps per (R, lambda) pair
+template <class T> struct PairC {
+  Iv<T> L, R;          // lambda >= 0 after S_a, R > 0
+  MR<T> Lm, LRm;       // midpoint forms of lambda and lambda R
+  Iv<T> L2;            // lambda^2
+};
+// ... per (pair, hit)
+template <class T> struct HitP {
+  Iv<T> LRdphi, T2L2, RpRA;
+};
+// ... per (pair, hit, drift sign): S4 terms that do not depend on z0
 template <class T> struct PassC {
-  Iv<T> LDcA, Rm2D, G;
+  Iv<T> LDcA, G;
+  MR<T> Rm2Dm;         // R - 2D > 0 by the guard
 };
 
-template <class T>
-IA_DEV PassC<T> pass_prepare(const HitF<T>& h, bool dneg, Iv<T> L, Iv<T> R, Iv<T> L2, Iv<T> RpRA) {
+template <class T> IA_DEV HitP<T> hit_prepare(const HitF<T>& h, int va, const PairC<T>& p) {
+  return {prod_p(p.LRm, h.dphi[va]), mul_pp(h.T2, p.L2), iadd(p.R, h.RA)};
+}
+
+template <class T> IA_DEV PassC<T> pass_prepare(const HitF<T>& h, bool dneg, const PairC<T>& p, const HitP<T>& hp) {
   PassC<T> c;
   const Iv<T> D = dneg ? Iv<T>{-h.Dhi, -h.Dlo} : Iv<T>{h.Dlo, h.Dhi};
-  const Iv<T> LD = dneg ? mul_pn(L, D) : mul_pp(L, D);
+  const Iv<T> LD = dneg ? mul_pn(p.L, D) : mul_pp(p.L, D);
   c.LDcA = imul(LD, h.cA);
-  c.Rm2D = isub(R, Iv<T>{Rnd<T>::mul_rn(T(2), D.lo), Rnd<T>::mul_rn(T(2), D.hi)});
-  const Iv<T> a = iadd(h.RA, mul_pp(L2, isub(RpRA, D)));
+  c.Rm2Dm = to_mr(isub(p.R, Iv<T>{Rnd<T>::mul_rn(T(2), D.lo), Rnd<T>::mul_rn(T(2), D.hi)}));
+  const Iv<T> a = iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, D)));
   c.G = dneg ? mul_pn(a, D) : mul_pp(D, a);
   return c;
 }
 
 // S4-S8 for one cell and one drift sign; returns true iff 0 is in f.
-// Inputs transformed: L >= 0, T = h.Tabs >= 0, cA >= 0 or M; va = the warp's a.
-template <class T>
-IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, Iv<T> L, Iv<T> R, Iv<T> LR, Iv<T> T2L2,
-                      Iv<T> LRdphi, Iv<T> Zr) {
+// Inputs transformed: L >= 0, T = h.Tabs >= 0, cA >= 0 (SS != 0) or any (SS == 0); va = the warp's a.
+template <int SS, class T>
+IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
   using Rd = Rnd<T>;
   const T Tn = h.Tabs;
-  const Iv<T> sA = h.sA[va];
-  const int scls = h.scls[va];
+  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
   // S4, z0-dependent part
-  const Iv<T> zA = iadd(Zr, LRdphi);                                   // (A.8d)
-  const Iv<T> zAsA = mul_cu(scls, sA, zA);
-  const Iv<T> t1 = mul_pu(LR, zA);
-  const Iv<T> LzA = mul_pu(L, zA);
+  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
+  const Iv<T> zAsA = prod_s<SS>(h.sAm[va], zA);                        // sigma zA sA
+  const Iv<T> t1 = prod_p(p.LRm, zA);
+  const Iv<T> LzA = prod_p(p.Lm, zA);
   const Iv<T> zA2 = sqr_u(zA);
-  const Iv<T> Y = mul_pu(h.iQ, iadd(zAsA, pc.LDcA));                   // Phi1 = -Y           (A.8b)
-  const Iv<T> t2 = mul_cu(h.c2cls, h.c2, mul_pu(pc.Rm2D, LzA));
-  const Iv<T> t3 = mul_cu(h.s2cls[va], h.s2[va], iadd(zA2, pc.G));
-  const Iv<T> P2 = mul_pu(h.hiQ, iadd(isub(t1, t2), t3));              // (A.8c)
-  const Iv<T> e = iadd(Iv<T>{Rd::mul_dn(Tn, -Y.hi), Rd::mul_up(Tn, -Y.lo)}, mul_pu(h.T2, P2));   // (A.8a)
+  const Iv<T> Y = prod_p(h.iQm, add_s<SS>(pc.LDcA, zAsA));             // Phi1 = -Y           (A.8b)
+  const Iv<T> W = prod_p(pc.Rm2Dm, LzA);
+  Iv<T> in;                                                            // t1 - t2
+  if (h.c2cls == CLS_P) in = isub(t1, prod_p(h.c2m, W));
+  else if (h.c2cls == CLS_N) in = iadd(t1, prod_p(mr_neg(h.c2m), W));
+  else in = isub(t1, prod_u(h.c2m, W));
+  const Iv<T> t3 = prod_s<SS>(h.s2m[va], iadd(zA2, pc.G));             // sigma t3
+  const Iv<T> P2 = prod_p(h.hiQm, add_s<SS>(in, t3));                  // (A.8c)
+  const Iv<T> e = iadd(Iv<T>{Rd::mul_dn(Tn, -Y.hi), Rd::mul_up(Tn, -Y.lo)}, prod_p(h.T2m, P2));   // (A.8a)
   // S5
-  Iv<T> se, sce, cce;
+  const Iv<T> sA = h.sA[va];
+  Iv<T> se, sce, cce;                                                  // sin e, sigma sA cos e, cA cos e
   const bool small = e.lo >= T(-0.25) && e.hi <= T(0.25);
   if (__all_sync(0xffffffffu, small)) {
     se = {pad_dn(Trig<T>::sin_small(e.lo)), pad_up(Trig<T>::sin_small(e.hi))};
@@ -292,30 +361,39 @@ IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, I
     const bool straddle = sgn(e.lo) != sgn(e.hi);
     const T chi = pad_up(Trig<T>::cos_small(mnn));
     const Iv<T> ce = {pad_dn(Trig<T>::cos_small(mag)), (straddle || chi > T(1)) ? T(1) : chi};   // cos > 0.96
-    sce = mul_pu(ce, sA);
-    cce = mul_pu(ce, h.cA);
+    sce = mulpos_s<SS>(ce, sA);
+    cce = mulpos_s<SC>(ce, h.cA);
   } else {
     trig_general(e, sA, h.cA, se, sce, cce);
+    if (SS < 0) sce = ineg(sce);
   }
-  const Iv<T> sinP = iclamp(mul_pu(h.iR, iadd(sce, mul_cu(h.ccls, h.cA, se))), T(-1), T(1));
-  const Iv<T> cosP = iclamp(mul_pu(h.iR, isub(cce, mul_cu(scls, sA, se))), T(-1), T(1));
-  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the HIT_FAST guard: roots of normal numbers
+  const Iv<T> cAse = prod_s<SC>(h.cAm, se);
+  const Iv<T> sAse = prod_s<SS>(h.sAm[va], se);                        // sigma sA sin e
+  const Iv<T> sinP = clamp_unit(prod_p(h.iRm, SS < 0 ? isub(cAse, sce) : iadd(sce, cAse)));
+  const Iv<T> cosP = clamp_unit(prod_p(h.iRm, sub_s<SS>(cce, sAse)));
+  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard: roots of normal numbers
   const T twoT = Rd::mul_rn(T(2), Tn);
-  const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, mul_pu(L, sinP)), T(1)), T2L2), mul_pp(h.T2, sqr_u(cosP)));
+  const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, prod_p(p.Lm, sinP)), T(1)), hp.T2L2), mul_pp(h.T2, sqr_u(cosP)));
   T hlo, hhi;
   const T ulo = Dir<T>::sqrt_dn(u2.lo, hlo), uhi = Dir<T>::sqrt_up(u2.hi, hhi);
   // |delta| = D+ / u_d
   const Iv<T> dq = {Dir<T>::div_dn(h.Dlo, uhi, Rd::mul_rn(T(2), hhi)), Dir<T>::div_up(h.Dhi, ulo, Rd::mul_rn(T(2), hlo))};
   // S7: z = (Zr + LR (dphi + e)) - T (delta cosP), delta = -/+ dq
-  const Iv<T> zz = iadd(Zr, mul_pu(LR, iadd(h.dphi[va], e)));
+  const Iv<T> zz = iadd(Zr, prod_p(p.LRm, iadd(h.dphi[va], e)));
   const Iv<T> Tdc = iscale_pos(Tn, mul_pu(dq, cosP));
-  const Iv<T> z = dneg ? iadd(zz, Tdc) : isub(zz, Tdc);
-  const Iv<T> Lq = mul_pp(L, dq);                                      // |lambda delta|
-  const Iv<T> zc = mul_cu(h.ccls, h.cA, z);
-  const Iv<T> qs = mul_pu(Lq, sA);
-  const Iv<T> ct = dneg ? iadd(zc, qs) : isub(zc, qs);                 // c^tau              (A.7b)
+  const Iv<T> Lq = mul_pp(p.L, dq);                                    // |lambda delta|
+  const Iv<T> qs = mulpos_s<SS>(Lq, sA);                               // sigma |lambda delta| sA
+  Iv<T> z, ct, Rd1;
+  if (dneg) {
+    z = iadd(zz, Tdc);
+    ct = add_s<SS>(prod_s<SC>(h.cAm, z), qs);                          // c^tau              (A.7b)
+    Rd1 = isub(p.R, dq);
+  } else {
+    z = isub(zz, Tdc);
+    ct = sub_s<SS>(prod_s<SC>(h.cAm, z), qs);
+    Rd1 = iadd(p.R, dq);
+  }
   // S8
-  const Iv<T> Rd1 = dneg ? isub(R, dq) : iadd(R, dq);
   const Iv<T> TLq = iscale_pos(Tn, Lq);
   const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), iscale_pos(twoT, ct)), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
   const Iv<T> f = isub(h.Q, rad);

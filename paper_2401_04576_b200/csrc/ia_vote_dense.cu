@@ -76,7 +76,14 @@ vote_dense_general_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDe
 // Thread = one (R, lambda) pair; loops over the hits (outer) and its FAST_ZT z0 cells (inner), so
 // that everything depending on (R, lambda, hit, drift sign) is computed once per FAST_ZT cells.
 // Vote counts: 8 bytes packed in one 64-bit register (hits per event <= 255 on this path).
-constexpr int FAST_THREADS = 256;
+#ifndef IA_FAST_THREADS
+#define IA_FAST_THREADS 256
+#endif
+#ifndef IA_FAST_MIN_BLOCKS
+#define IA_FAST_MIN_BLOCKS 2
+#endif
+constexpr int FAST_THREADS = IA_FAST_THREADS;
+constexpr int FAST_MIN_BLOCKS = IA_FAST_MIN_BLOCKS;
 constexpr int FAST_ZT = 8;
 
 template <class T> struct ZTab { Iv<T> z[2][FAST_ZT]; };    // [0]: z0 - z_ref, [1]: its negation
@@ -92,21 +99,19 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
 }
 
 // one hit, one thread: both drift signs over the thread's z0 cells; returns the 8-bit vote mask
-template <class T>
-IA_DEV unsigned fast_hit(const HitF<T>& h, int va, Iv<T> L, Iv<T> R, Iv<T> LR, Iv<T> L2, const Iv<T>* zt, int nz_tile) {
-  const Iv<T> LRdphi = mul_pu(LR, h.dphi[va]);
-  const Iv<T> RpRA = iadd(R, h.RA);
-  const Iv<T> T2L2 = mul_pp(h.T2, L2);
+template <int SS, class T>
+IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
+  const HitP<T> hp = hit_prepare(h, va, p);
   unsigned bits = 0;
 #pragma unroll 1
   for (int s = 0; s < 2; ++s) {
     const bool dneg = s == 1;
-    const PassC<T> pc = pass_prepare(h, dneg, L, R, L2, RpRA);
+    const PassC<T> pc = pass_prepare(h, dneg, p, hp);
 #pragma unroll 1
     for (int i = 0; i < nz_tile; ++i) {
       // the second pass is needed only where some lane has not voted yet
       if (__all_sync(0xffffffffu, (bits >> i) & 1u)) continue;
-      bits |= (pass_vote(h, va, dneg, pc, L, R, LR, T2L2, LRdphi, zt[i]) ? 1u : 0u) << i;
+      bits |= (pass_vote<SS>(h, va, dneg, pc, p, hp, zt[i]) ? 1u : 0u) << i;
     }
   }
   return bits;
@@ -121,7 +126,7 @@ IA_DEV unsigned long long spread8(unsigned bits) {
 }
 
 template <class T>
-__global__ void __launch_bounds__(FAST_THREADS, 2)
+__global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z,
                        uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -179,22 +184,29 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   const bool allP = __all_sync(0xffffffffu, lcls == CLS_P), allN = __all_sync(0xffffffffu, lcls == CLS_N);
   const bool a = !allP && allN;                       // S_a: flip lambda, z0 - z_ref and T for this warp
   const bool warp_fast = allP || allN;
-  const Iv<T> L = a ? ineg(Lraw) : Lraw;
-  const Iv<T> LR = warp_fast ? mul_pp(L, R) : imul(L, R);
-  const Iv<T> L2 = warp_fast ? mul_pp(L, L) : isqr(L);
+  PairC<T> pr;
+  pr.L = a ? ineg(Lraw) : Lraw;
+  pr.R = R;
+  pr.Lm = to_mr(pr.L);
+  pr.LRm = to_mr(warp_fast ? mul_pp(pr.L, R) : imul(pr.L, R));
+  pr.L2 = warp_fast ? mul_pp(pr.L, pr.L) : isqr(pr.L);
   unsigned long long acc = 0;
   const int va = a ? 1 : 0;
   for (int h = 0; h < count; ++h) {
     const HitF<T>& hf = sh[h];
-    const int kind = hf.kind;
+    const int kind = hf.kind[va];
     if (kind == HIT_SKIP) continue;
     if (kind == HIT_FORCED) { acc += 0x0101010101010101ull; continue; }
     const Iv<T>* zt = ztab->z[hf.zflip];
-    if (kind == HIT_FAST && warp_fast) {
-      acc += spread8(fast_hit<T>(hf, va, L, R, LR, L2, zt, nz_tile));
+    if (kind != HIT_GENERAL && warp_fast) {
+      unsigned bits;
+      if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
+      else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, va, pr, zt, nz_tile);
+      else bits = fast_hit<0, T>(hf, va, pr, zt, nz_tile);
+      acc += spread8(bits);
     } else {
       for (int i = 0; i < nz_tile; ++i)
-        acc += (unsigned long long)(general_votes_norm(hf, va, R, zt[i], L) ? 1u : 0u) << (8 * i);
+        acc += (unsigned long long)(general_votes_norm(hf, va, R, zt[i], pr.L) ? 1u : 0u) << (8 * i);
     }
   }
   if (live) {
