@@ -151,7 +151,12 @@ int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* l
 /* Device interval primitives exposed for unit tests: n independent operations
  * out_dev[i] = op(a_dev[i], b_dev[i]) on intervals stored as (lo, hi) pairs of doubles; prec = 64 or 32.
  * op: 0 add 1 sub 2 mul 3 sqr(a) 4 div(a, b>0) 5 sqrt(a) 6 sin(a) 7 cos(a) 8 atan2(y=a, x=b)
- *     9 recip(a>0) 10 scale(b.lo, a) */
+ *     9 recip(a>0) 10 scale(b.lo, a)
+ *     primitives of the dense fast path (enclosures at most a few ulps wider than the tightest):
+ *     11 a*b with a >= 0 taken in midpoint-radius form  12 the same for a of any sign
+ *     13 a / sqrt(b) for a >= 0 and b in [1/4, 4] (delta = d_St/u_d of S6, one fused enclosure)
+ *     14 sqr(a) branch-free  15 sin(a), 16 cos(a) for a inside [-1/4, 1/4] (Taylor, padded)
+ *     17 a intersected with [-1, 1] */
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev);
 
 /* Roofline probe: enqueue a kernel of `blocks` x 256 threads, each running 8 independent FP64

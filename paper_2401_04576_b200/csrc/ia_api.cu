@@ -345,8 +345,8 @@ int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* l
 }
 
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev) {
-  if (!ctx || !a_dev || !out_dev || n < 0 || op < 0 || op > 10 || (prec != 64 && prec != 32)) return IA_ERR_ARG;
-  const bool binary = (op == 0 || op == 1 || op == 2 || op == 4 || op == 8 || op == 10);
+  if (!ctx || !a_dev || !out_dev || n < 0 || op < 0 || op > 17 || (prec != 64 && prec != 32)) return IA_ERR_ARG;
+  const bool binary = (op == 0 || op == 1 || op == 2 || op == 4 || op == 8 || op == 10 || op == 11 || op == 12 || op == 13);
   if (binary && !b_dev) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_prim(ctx, op, prec, a_dev, b_dev, n, out_dev));

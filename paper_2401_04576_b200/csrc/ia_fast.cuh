@@ -171,8 +171,29 @@ template <> struct Dir<double> {
     const double d = __fma_rn(-b, q, a);
     return (d > 0.0) ? (q > 0.0 ? next_up(q) : 4.9406564584124654e-324) : q;
   }
+  // 1/sqrt(x) for x in [2^-2, 2^2], relative error below 2^-51.  y0 = MUFU.RSQ64H (relative error e0
+  // < 2^-20: 1 - x y0^2 = r, |r| < 2^-19); 1/sqrt(x) = y0 (1-r)^(-1/2) = y0 (1 + r/2 + 3r^2/8 + 5r^3/16 ...):
+  // truncation after r^2 leaves 5/16 |r|^3 < 2^-58; rounding: t = x y0 (2^-53 relative, carried into r
+  // as 2^-53 absolute, halved), the final FMA (2^-53): together < 2^-52 + 2^-58.
+  static IA_DEV double rsqrt_near(double x) {
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    const double t = __dmul_rn(x, y0);
+    const double r = __fma_rn(-t, y0, 1.0);
+    const double p = __fma_rn(0.375, r, 0.5);
+    return __fma_rn(__dmul_rn(y0, r), p, y0);
+  }
+  // enclosure of D+ / sqrt(u2): 1/sqrt is decreasing; the relative 2^-50 padding of D+ (DloP, DhiP)
+  // covers the 2^-51 of rsqrt_near, the product is rounded outward
+  template <class H> static IA_DEV Iv<double> d_over_sqrt(const H& h, Iv<double> u2) {
+    return {__dmul_rd(h.DloP, rsqrt_near(u2.hi)), __dmul_ru(h.DhiP, rsqrt_near(u2.lo))};
+  }
 };
 template <> struct Dir<float> {
+  // [DloP, DhiP] are not used in float: correctly rounded sqrt and division are single instructions' worth
+  template <class H> static IA_DEV Iv<float> d_over_sqrt(const H& h, Iv<float> u2) {
+    return {__fdiv_rd(h.Dlo, __fsqrt_ru(u2.hi)), __fdiv_ru(h.Dhi, __fsqrt_rd(u2.lo))};
+  }
   static IA_DEV float sqrt_dn(float x, float& h) { h = 0.f; return __fsqrt_rd(x); }
   static IA_DEV float sqrt_up(float x, float& h) { h = 0.f; return __fsqrt_ru(x); }
   static IA_DEV float div_dn(float a, float b, float) { return __fdiv_rd(a, b); }
@@ -187,8 +208,8 @@ template <> struct Dir<float> {
 // Float: terms to x^7 / x^8, truncation < 1e-11, pad 2^-21.
 template <class T> struct Trig;
 template <> struct Trig<double> {
-  static IA_DEV double sin_small(double x) {
-    const double s = __dmul_rn(x, x);
+  static IA_DEV double sqr(double x) { return __dmul_rn(x, x); }
+  static IA_DEV double sin_small(double x, double s) {
     double q = -2.5052108385441720e-08;               // -1/11!
     q = __fma_rn(q, s, 2.7557319223985893e-06);       //  1/9!
     q = __fma_rn(q, s, -1.9841269841269841e-04);      // -1/7!
@@ -196,8 +217,7 @@ template <> struct Trig<double> {
     q = __fma_rn(q, s, -1.6666666666666666e-01);      // -1/3!
     return __fma_rn(__dmul_rn(x, s), q, x);
   }
-  static IA_DEV double cos_small(double x) {
-    const double s = __dmul_rn(x, x);
+  static IA_DEV double cos_small(double s) {
     double q = 2.0876756987868100e-09;                //  1/12!
     q = __fma_rn(q, s, -2.7557319223985888e-07);      // -1/10!
     q = __fma_rn(q, s, 2.4801587301587302e-05);       //  1/8!
@@ -208,15 +228,14 @@ template <> struct Trig<double> {
   }
 };
 template <> struct Trig<float> {
-  static IA_DEV float sin_small(float x) {
-    const float s = __fmul_rn(x, x);
+  static IA_DEV float sqr(float x) { return __fmul_rn(x, x); }
+  static IA_DEV float sin_small(float x, float s) {
     float q = -1.9841270e-04f;
     q = __fmaf_rn(q, s, 8.3333338e-03f);
     q = __fmaf_rn(q, s, -1.6666667e-01f);
     return __fmaf_rn(__fmul_rn(x, s), q, x);
   }
-  static IA_DEV float cos_small(float x) {
-    const float s = __fmul_rn(x, x);
+  static IA_DEV float cos_small(float s) {
     float q = 2.4801588e-05f;
     q = __fmaf_rn(q, s, -1.3888889e-03f);
     q = __fmaf_rn(q, s, 4.1666668e-02f);
@@ -224,6 +243,18 @@ template <> struct Trig<float> {
     return __fmaf_rn(q, s, 1.0f);
   }
 };
+
+// sin and cos over e inside [-1/4, 1/4]: sin is increasing there, cos decreases in |e|.  The squares
+// serve both polynomials; |e.lo| > |e.hi| is read off them (equal squares give equal cosines).
+template <class T> IA_DEV void trig_small(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
+  const T s0 = Trig<T>::sqr(e.lo), s1 = Trig<T>::sqr(e.hi);
+  se = {pad_dn(Trig<T>::sin_small(e.lo, s0)), pad_up(Trig<T>::sin_small(e.hi, s1))};
+  const T c0 = Trig<T>::cos_small(s0), c1 = Trig<T>::cos_small(s1);
+  const bool c = s0 > s1;
+  const bool straddle = sgn(e.lo) != sgn(e.hi);
+  const T chi = pad_up(c ? c1 : c0);
+  ce = {pad_dn(c ? c0 : c1), (straddle || chi > T(1)) ? T(1) : chi};   // cos > 0.96
+}
 
 // ---- per-(block, hit) record in shared memory ------------------------------------------------------
 // HIT_FAST_P / _N / _U: the three bodies (SS = +1, -1, 0)
@@ -233,12 +264,15 @@ template <class T> struct __align__(16) HitF {
   // transformed by S_b^b S_d^(t+b) (and, in the [1] versions, additionally by the S_d that goes with S_a);
   // (m, r) forms carry the true sign of the factor in m
   Iv<T> Q, cA, T2, RA;
-  MR<T> cAm, iQm, hiQm, iRm, c2m, T2m;
+  MR<T> cAm, iRm, c2m;
+  MR<T> TiQm, T2hiQm, cA2Tm;       // T/Q, T^2/(2Q), 2T c_Ax: the thin scalar folded into the block constant
   Iv<T> sA[2], dphi[2];            // index a = 1 for warps whose lambda was negated
+  Iv<T> sA2T[2];                   // 2T s_Ax
   MR<T> sAm[2], s2m[2];
   Iv<T> iQ, iR, c2, s2[2];         // interval forms, general fallback only
   T Tabs;                          // |tan tau|
   T Dlo, Dhi;
+  T DloP, DhiP;                    // D+ padded outward by 2^-50 (2^-21): absorbs the error of rsqrt_near
   int kind[2];                     // per a
   int c2cls;
   int zflip;                       // z0 - z_ref enters negated
@@ -252,17 +286,20 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
   o.Dlo = hs.Dlo; o.Dhi = hs.Dhi;
   o.Tabs = fabs(hs.Tn);
   o.Q = v.Q; o.iQ = v.iQ; o.RA = v.RA; o.iR = v.iR; o.c2 = v.c2;
-  o.iQm = to_mr(v.iQ);
-  o.hiQm = {Rd::mul_rn(T(0.5), o.iQm.m), Rd::mul_rn(T(0.5), o.iQm.r)};      // exact scaling of 1/Q by 1/2
   o.iRm = to_mr(v.iR);
   o.c2m = to_mr(v.c2);
   o.T2 = {Rd::mul_dn(hs.Tn, hs.Tn), Rd::mul_up(hs.Tn, hs.Tn)};              // isqr(thin(T))
-  o.T2m = to_mr(o.T2);
+  o.TiQm = to_mr(iscale_pos(o.Tabs, v.iQ));
+  o.T2hiQm = to_mr(mul_pp(o.T2, Iv<T>{Rd::mul_rn(T(0.5), v.iQ.lo), Rd::mul_rn(T(0.5), v.iQ.hi)}));
+  o.DloP = Rd::fma_dn(-hs.Dlo, Rd::pad_rel(), hs.Dlo);
+  o.DhiP = Rd::fma_up(hs.Dhi, Rd::pad_rel(), hs.Dhi);
   o.c2cls = cls_of(v.c2);
   const bool t = hs.Tn < T(0);
   const bool b = cls_of(v.cA) == CLS_N;
   o.cA = b ? ineg(v.cA) : v.cA;
   o.cAm = to_mr(o.cA);
+  const T twoT = Rd::mul_rn(T(2), o.Tabs);
+  o.cA2Tm = to_mr(iscale_pos(twoT, o.cA));
   const int ccls = cls_of(o.cA);
   o.zflip = (t != b) ? 1 : 0;
   // guards of the sign-known forms: R - 2D > 0, R + R_Ax - D > 0, R + delta > 0 (|delta| <= 2 D.hi as
@@ -276,6 +313,7 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
     o.s2[a] = fd ? ineg(v.s2) : v.s2;
     o.dphi[a] = fd ? ineg(v.dphi) : v.dphi;
     o.sAm[a] = to_mr(o.sA[a]);
+    o.sA2T[a] = iscale_pos(twoT, o.sA[a]);
     o.s2m[a] = to_mr(o.s2[a]);
     const int scls = cls_of(o.sA[a]), s2cls = cls_of(o.s2[a]);
     int kind = HIT_FAST_U;
@@ -341,26 +379,22 @@ IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, c
   const Iv<T> t1 = prod_p(p.LRm, zA);
   const Iv<T> LzA = prod_p(p.Lm, zA);
   const Iv<T> zA2 = sqr_u(zA);
-  const Iv<T> Y = prod_p(h.iQm, add_s<SS>(pc.LDcA, zAsA));             // Phi1 = -Y           (A.8b)
+  const Iv<T> TY = prod_p(h.TiQm, add_s<SS>(pc.LDcA, zAsA));           // T Phi1 = -TY        (A.8b)
   const Iv<T> W = prod_p(pc.Rm2Dm, LzA);
   Iv<T> in;                                                            // t1 - t2
   if (h.c2cls == CLS_P) in = isub(t1, prod_p(h.c2m, W));
   else if (h.c2cls == CLS_N) in = iadd(t1, prod_p(mr_neg(h.c2m), W));
   else in = isub(t1, prod_u(h.c2m, W));
   const Iv<T> t3 = prod_s<SS>(h.s2m[va], iadd(zA2, pc.G));             // sigma t3
-  const Iv<T> P2 = prod_p(h.hiQm, add_s<SS>(in, t3));                  // (A.8c)
-  const Iv<T> e = iadd(Iv<T>{Rd::mul_dn(Tn, -Y.hi), Rd::mul_up(Tn, -Y.lo)}, prod_p(h.T2m, P2));   // (A.8a)
+  const Iv<T> T2P2 = prod_p(h.T2hiQm, add_s<SS>(in, t3));              // T^2 Phi2            (A.8c)
+  const Iv<T> e = isub(T2P2, TY);                                      // (A.8a)
   // S5
   const Iv<T> sA = h.sA[va];
   Iv<T> se, sce, cce;                                                  // sin e, sigma sA cos e, cA cos e
   const bool small = e.lo >= T(-0.25) && e.hi <= T(0.25);
   if (__all_sync(0xffffffffu, small)) {
-    se = {pad_dn(Trig<T>::sin_small(e.lo)), pad_up(Trig<T>::sin_small(e.hi))};
-    const bool c = fabs(e.lo) > fabs(e.hi);
-    const T mag = c ? e.lo : e.hi, mnn = c ? e.hi : e.lo;
-    const bool straddle = sgn(e.lo) != sgn(e.hi);
-    const T chi = pad_up(Trig<T>::cos_small(mnn));
-    const Iv<T> ce = {pad_dn(Trig<T>::cos_small(mag)), (straddle || chi > T(1)) ? T(1) : chi};   // cos > 0.96
+    Iv<T> ce;
+    trig_small(e, se, ce);
     sce = mulpos_s<SS>(ce, sA);
     cce = mulpos_s<SC>(ce, h.cA);
   } else {
@@ -374,28 +408,25 @@ IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, c
   // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard: roots of normal numbers
   const T twoT = Rd::mul_rn(T(2), Tn);
   const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, prod_p(p.Lm, sinP)), T(1)), hp.T2L2), mul_pp(h.T2, sqr_u(cosP)));
-  T hlo, hhi;
-  const T ulo = Dir<T>::sqrt_dn(u2.lo, hlo), uhi = Dir<T>::sqrt_up(u2.hi, hhi);
-  // |delta| = D+ / u_d
-  const Iv<T> dq = {Dir<T>::div_dn(h.Dlo, uhi, Rd::mul_rn(T(2), hhi)), Dir<T>::div_up(h.Dhi, ulo, Rd::mul_rn(T(2), hlo))};
+  const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                         // |delta| = D+ / u_d
   // S7: z = (Zr + LR (dphi + e)) - T (delta cosP), delta = -/+ dq
   const Iv<T> zz = iadd(Zr, prod_p(p.LRm, iadd(h.dphi[va], e)));
   const Iv<T> Tdc = iscale_pos(Tn, mul_pu(dq, cosP));
   const Iv<T> Lq = mul_pp(p.L, dq);                                    // |lambda delta|
-  const Iv<T> qs = mulpos_s<SS>(Lq, sA);                               // sigma |lambda delta| sA
-  Iv<T> z, ct, Rd1;
+  const Iv<T> qs = mulpos_s<SS>(Lq, h.sA2T[va]);                       // sigma 2T |lambda delta| sA
+  Iv<T> z, ct, Rd1;                                                    // ct = 2T c^tau       (A.7b)
   if (dneg) {
     z = iadd(zz, Tdc);
-    ct = add_s<SS>(prod_s<SC>(h.cAm, z), qs);                          // c^tau              (A.7b)
+    ct = add_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
     Rd1 = isub(p.R, dq);
   } else {
     z = isub(zz, Tdc);
-    ct = sub_s<SS>(prod_s<SC>(h.cAm, z), qs);
+    ct = sub_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
     Rd1 = iadd(p.R, dq);
   }
   // S8
   const Iv<T> TLq = iscale_pos(Tn, Lq);
-  const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), iscale_pos(twoT, ct)), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
+  const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), ct), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
   const Iv<T> f = isub(h.Q, rad);
   return !(f.lo > T(0) || f.hi < T(0));
 }

@@ -1,6 +1,7 @@
 // ia_kernels.cu - hit staging (a2), explicit-box vote, refinement level (a8-a9), diagnostics.
 #include "ia_internal.h"
 #include "ia_residual.cuh"
+#include "ia_fast.cuh"
 #include "ia_topk.cuh"
 
 namespace ia {
@@ -142,6 +143,19 @@ __global__ void prim_kernel(int op, const double* __restrict__ a, const double* 
     case 8: r = iatan2(x, y); break;
     case 9: r = irecip_pos(x); break;
     case 10: r = iscale(y.lo, x); break;
+    // primitives of the dense fast path (ia_fast.cuh)
+    case 11: r = prod_p(to_mr(x), y); break;                 // x >= 0 as (m, r), y any
+    case 12: r = prod_u(to_mr(x), y); break;                 // x any class as (m, r), y any
+    case 13: {                                               // x = D+ >= 0, y = u_d^2 in [1/4, 4]
+      struct { T Dlo, Dhi, DloP, DhiP; } h = {x.lo, x.hi, Rnd<T>::fma_dn(-x.lo, Rnd<T>::pad_rel(), x.lo),
+                                              Rnd<T>::fma_up(x.hi, Rnd<T>::pad_rel(), x.hi)};
+      r = Dir<T>::d_over_sqrt(h, y);
+      break;
+    }
+    case 14: r = sqr_u(x); break;
+    case 15: { Iv<T> c; trig_small(x, r, c); break; }        // sin over x inside [-1/4, 1/4]
+    case 16: { Iv<T> s; trig_small(x, s, r); break; }        // cos
+    case 17: r = clamp_unit(x); break;
     default: break;
   }
   out[2 * i] = double(r.lo);

@@ -367,3 +367,71 @@ def test_fast_and_general_kernels_agree(precision):
             assert vf.max() > 0
     finally:
         rig.close()
+
+
+PROD_P, PROD_U, D_OVER_SQRT, SQR_U, SIN_SMALL, COS_SMALL, CLAMP_UNIT = 11, 12, 13, 14, 15, 16, 17
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_fast_path_primitives(rig0, prec):
+    """The primitives of the dense fast path (ia_fast.cuh) against exact arithmetic: every result
+    contains the exact range and is at most a few ulps wider than the tightest enclosure."""
+    from fractions import Fraction as Fr
+    import mpmath as mp
+    mp.mp.dps = 60
+    rng = np.random.default_rng(100 + prec)
+    n = 1500
+    eps = 2.0 ** -52 if prec == 64 else 2.0 ** -23
+    ctx = rig0.ctx
+    x, ap, au = _rand_iv(rng, n, prec=prec), _rand_iv(rng, n, True, prec), _rand_iv(rng, n, prec=prec)
+    ap[:50, 0] = 0.0                                   # factors touching zero (the first lambda cell)
+    x[:25] = np.stack([np.zeros(25), np.abs(x[:25, 1])], 1)
+    x[25:50] = np.stack([-np.abs(x[25:50, 0]), -np.zeros(25)], 1)
+    for op, a in ((PROD_P, ap), (PROD_U, au)):
+        got = ctx.ia_prim(op, prec, rig0.dev(a), rig0.dev(x)).cpu().numpy()
+        for i in range(n):
+            prods = [Fr(p) * Fr(q) for p in a[i] for q in x[i]]
+            lo, hi = min(prods), max(prods)
+            scale = max(abs(lo), abs(hi), Fr(1, 10 ** 300))
+            assert Fr(got[i, 0]) <= lo and hi <= Fr(got[i, 1]), (op, a[i], x[i], got[i])
+            assert lo - Fr(got[i, 0]) <= 4 * Fr(eps) * scale and Fr(got[i, 1]) - hi <= 4 * Fr(eps) * scale, (op, a[i], x[i], got[i])
+    # D / sqrt(u2)
+    d = np.sort(rng.uniform(0.0, 1.6, size=(n, 2)), axis=1)
+    d[:20, 0] = 0.0
+    u2 = np.sort(rng.uniform(0.3, 3.0, size=(n, 2)), axis=1)
+    u2[:200, 1] = u2[:200, 0]
+    if prec == 32:
+        d, u2 = d.astype(np.float32).astype(np.float64), u2.astype(np.float32).astype(np.float64)
+    got = ctx.ia_prim(D_OVER_SQRT, prec, rig0.dev(d), rig0.dev(u2)).cpu().numpy()
+    for i in range(n):
+        lo, hi = mp.mpf(d[i, 0]) / mp.sqrt(mp.mpf(u2[i, 1])), mp.mpf(d[i, 1]) / mp.sqrt(mp.mpf(u2[i, 0]))
+        assert mp.mpf(got[i, 0]) <= lo and hi <= mp.mpf(got[i, 1]), (d[i], u2[i], got[i])
+        assert lo - mp.mpf(got[i, 0]) <= 8 * eps * hi and mp.mpf(got[i, 1]) - hi <= 8 * eps * hi, (d[i], u2[i], got[i])
+    # branch-free square and the clamp: bit-exact
+    got = ctx.ia_prim(SQR_U, prec, rig0.dev(au)).cpu().numpy()
+    for i in range(n):
+        assert tuple(got[i]) == o.prim(SQR, tuple(au[i]), (0.0, 0.0), prec)
+    cl = np.concatenate([_rand_iv(rng, 300, prec=prec) * 1e-2, np.array([[-1.0, 1.0], [-1.0 - 4 * eps, 1.0 + 4 * eps], [-0.0, 0.0], [1.0 - eps, 1.0 + eps]])])
+    if prec == 32:
+        cl = cl.astype(np.float32).astype(np.float64)
+    got = ctx.ia_prim(CLAMP_UNIT, prec, rig0.dev(cl)).cpu().numpy()
+    assert (got[:, 0] == np.maximum(cl[:, 0], -1.0)).all() and (got[:, 1] == np.minimum(cl[:, 1], 1.0)).all()
+    # sin / cos inside [-1/4, 1/4]
+    c = rng.uniform(-0.25, 0.25, n)
+    w = rng.choice([0.0, 1e-12, 1e-6, 1e-3, 0.05, 0.5], size=n) * rng.random(n)
+    e = np.clip(np.stack([c - w, c + w], 1), -0.25, 0.25)
+    e[:10] = [[-0.25, 0.25]] * 10
+    e[10:20] = np.stack([np.zeros(10), np.abs(e[10:20, 1])], 1)
+    e[20:30] = np.stack([-np.abs(e[20:30, 0]), -np.zeros(10)], 1)
+    if prec == 32:
+        e = e.astype(np.float32).astype(np.float64)
+    s = ctx.ia_prim(SIN_SMALL, prec, rig0.dev(e)).cpu().numpy()
+    cc = ctx.ia_prim(COS_SMALL, prec, rig0.dev(e)).cpu().numpy()
+    for i in range(n):
+        lo, hi = mp.mpf(e[i, 0]), mp.mpf(e[i, 1])
+        assert mp.mpf(s[i, 0]) <= mp.sin(lo) and mp.sin(hi) <= mp.mpf(s[i, 1]), (e[i], s[i])
+        assert mp.sin(lo) - mp.mpf(s[i, 0]) <= 10 * eps * 0.25 and mp.mpf(s[i, 1]) - mp.sin(hi) <= 10 * eps * 0.25, (e[i], s[i])
+        cmin = mp.cos(max(abs(lo), abs(hi)))
+        cmax = mp.mpf(1) if lo <= 0 <= hi else mp.cos(min(abs(lo), abs(hi)))
+        assert mp.mpf(cc[i, 0]) <= cmin and cmax <= mp.mpf(cc[i, 1]) and cc[i, 1] <= 1.0, (e[i], cc[i])
+        assert cmin - mp.mpf(cc[i, 0]) <= 10 * eps and mp.mpf(cc[i, 1]) - cmax <= 10 * eps, (e[i], cc[i])
