@@ -97,11 +97,39 @@ template <int SS, class T> IA_DEV Iv<T> mulpos_s(Iv<T> c, Iv<T> s) {
   return mul_pu(c, s);
 }
 
+// ---- comparisons kept off the FP64 pipe -----------------------------------------------------------
+// The FP64 pipe is the bottleneck of the dense kernel and the ALU pipe has room (profiles/), so the
+// comparisons whose operands are finite by construction are done on the bit patterns: for
+// non-negative doubles the order of the values is the order of the 64-bit integers.
+#ifndef IA_INT_CMP
+#define IA_INT_CMP 1
+#endif
+#if IA_INT_CMP
+IA_DEV bool abs_gt(double a, double b) {           // |a| > |b|
+  return (__double_as_longlong(a) & 0x7fffffffffffffffLL) > (__double_as_longlong(b) & 0x7fffffffffffffffLL);
+}
+IA_DEV bool nn_gt(double a, double b) { return __double_as_longlong(a) > __double_as_longlong(b); }   // a, b >= 0
+IA_DEV bool is_pos(double x) { return __double_as_longlong(x) > 0; }                                 // x > 0
+IA_DEV bool ge_one(double x) { return __double2hiint(x) >= 0x3ff00000; }                              // x >= 1
+IA_DEV bool abs_lt_quarter(double x) { return (__double2hiint(x) & 0x7fffffff) < 0x3fd00000; }        // |x| < 1/4
+#else
+IA_DEV bool abs_gt(double a, double b) { return fabs(a) > fabs(b); }
+IA_DEV bool nn_gt(double a, double b) { return a > b; }
+IA_DEV bool is_pos(double x) { return x > 0.0; }
+IA_DEV bool ge_one(double x) { return x >= 1.0; }
+IA_DEV bool abs_lt_quarter(double x) { return fabs(x) < 0.25; }
+#endif
+IA_DEV bool abs_gt(float a, float b) { return fabsf(a) > fabsf(b); }
+IA_DEV bool nn_gt(float a, float b) { return a > b; }
+IA_DEV bool is_pos(float x) { return x > 0.f; }
+IA_DEV bool ge_one(float x) { return x >= 1.f; }
+IA_DEV bool abs_lt_quarter(float x) { return fabsf(x) < 0.25f; }
+
 enum { CLS_P = 0, CLS_N = 1, CLS_M = 2 };
 // square of an interval of unknown sign without branches: largest / smallest magnitude
 template <class T> IA_DEV Iv<T> sqr_u(Iv<T> a) {
   using R = Rnd<T>;
-  const bool c = fabs(a.lo) > fabs(a.hi);
+  const bool c = abs_gt(a.lo, a.hi);
   const T mag = c ? a.lo : a.hi, mnn = c ? a.hi : a.lo;
   const bool straddle = sgn(a.lo) != sgn(a.hi);
   const T lo2 = R::mul_dn(mnn, mnn);
@@ -250,10 +278,10 @@ template <class T> IA_DEV void trig_small(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
   const T s0 = Trig<T>::sqr(e.lo), s1 = Trig<T>::sqr(e.hi);
   se = {pad_dn(Trig<T>::sin_small(e.lo, s0)), pad_up(Trig<T>::sin_small(e.hi, s1))};
   const T c0 = Trig<T>::cos_small(s0), c1 = Trig<T>::cos_small(s1);
-  const bool c = s0 > s1;
+  const bool c = nn_gt(s0, s1);
   const bool straddle = sgn(e.lo) != sgn(e.hi);
   const T chi = pad_up(c ? c1 : c0);
-  ce = {pad_dn(c ? c0 : c1), (straddle || chi > T(1)) ? T(1) : chi};   // cos > 0.96
+  ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? T(1) : chi};   // cos > 0.96
 }
 
 // ---- per-(block, hit) record in shared memory ------------------------------------------------------
@@ -348,7 +376,9 @@ template <class T> struct HitP {
 // ... per (pair, hit, drift sign): S4 terms that do not depend on z0
 template <class T> struct PassC {
   Iv<T> LDcA, G;
-  MR<T> Rm2Dm;         // R - 2D > 0 by the guard
+  MR<T> Km;            // K = (lambda (R - 2D)) cos 2Phi_Ax, class of cos 2Phi_Ax (R - 2D > 0 by the guard):
+                       // t2 = ((lambda zA)(R - 2D)) c2 = K zA - interval multiplication is associative and
+                       // commutative, so only the roundings differ from the order of S4
 };
 
 template <class T> IA_DEV HitP<T> hit_prepare(const HitF<T>& h, int va, const PairC<T>& p) {
@@ -360,75 +390,95 @@ template <class T> IA_DEV PassC<T> pass_prepare(const HitF<T>& h, bool dneg, con
   const Iv<T> D = dneg ? Iv<T>{-h.Dhi, -h.Dlo} : Iv<T>{h.Dlo, h.Dhi};
   const Iv<T> LD = dneg ? mul_pn(p.L, D) : mul_pp(p.L, D);
   c.LDcA = imul(LD, h.cA);
-  c.Rm2Dm = to_mr(isub(p.R, Iv<T>{Rnd<T>::mul_rn(T(2), D.lo), Rnd<T>::mul_rn(T(2), D.hi)}));
+  const Iv<T> LRm2D = mul_pp(p.L, isub(p.R, Iv<T>{Rnd<T>::mul_rn(T(2), D.lo), Rnd<T>::mul_rn(T(2), D.hi)}));
+  c.Km = to_mr(mul_pu(LRm2D, h.c2));
   const Iv<T> a = iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, D)));
   c.G = dneg ? mul_pn(a, D) : mul_pp(D, a);
   return c;
 }
 
-// S4-S8 for one cell and one drift sign; returns true iff 0 is in f.
+// S4-S8 for NC cells (same (R, lambda) pair, hit and drift sign; NC different z0 cells) at once; bit c
+// of the result is set iff 0 is in f for cell c.  The NC cells are independent dependency chains
+// written side by side, which is what keeps the FP64 pipe fed at 16 warps per SM (its dependent-issue
+// latency is about 12 cycles).
 // Inputs transformed: L >= 0, T = h.Tabs >= 0, cA >= 0 (SS != 0) or any (SS == 0); va = the warp's a.
-template <int SS, class T>
-IA_DEV bool pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
+template <int SS, int NC, class T>
+IA_DEV unsigned pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp,
+                          const Iv<T>* Zr) {
   using Rd = Rnd<T>;
   const T Tn = h.Tabs;
   constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
+  Iv<T> e[NC];
+  bool small = true;
   // S4, z0-dependent part
-  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
-  const Iv<T> zAsA = prod_s<SS>(h.sAm[va], zA);                        // sigma zA sA
-  const Iv<T> t1 = prod_p(p.LRm, zA);
-  const Iv<T> LzA = prod_p(p.Lm, zA);
-  const Iv<T> zA2 = sqr_u(zA);
-  const Iv<T> TY = prod_p(h.TiQm, add_s<SS>(pc.LDcA, zAsA));           // T Phi1 = -TY        (A.8b)
-  const Iv<T> W = prod_p(pc.Rm2Dm, LzA);
-  Iv<T> in;                                                            // t1 - t2
-  if (h.c2cls == CLS_P) in = isub(t1, prod_p(h.c2m, W));
-  else if (h.c2cls == CLS_N) in = iadd(t1, prod_p(mr_neg(h.c2m), W));
-  else in = isub(t1, prod_u(h.c2m, W));
-  const Iv<T> t3 = prod_s<SS>(h.s2m[va], iadd(zA2, pc.G));             // sigma t3
-  const Iv<T> T2P2 = prod_p(h.T2hiQm, add_s<SS>(in, t3));              // T^2 Phi2            (A.8c)
-  const Iv<T> e = isub(T2P2, TY);                                      // (A.8a)
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    const Iv<T> zA = iadd(Zr[c], hp.LRdphi);                           // (A.8d)
+    const Iv<T> zAsA = prod_s<SS>(h.sAm[va], zA);                      // sigma zA sA
+    const Iv<T> t1 = prod_p(p.LRm, zA);
+    const Iv<T> zA2 = sqr_u(zA);
+    const Iv<T> TY = prod_p(h.TiQm, add_s<SS>(pc.LDcA, zAsA));         // T Phi1 = -TY        (A.8b)
+    Iv<T> in;                                                          // t1 - t2
+    if (h.c2cls == CLS_P) in = isub(t1, prod_p(pc.Km, zA));
+    else if (h.c2cls == CLS_N) in = iadd(t1, prod_p(mr_neg(pc.Km), zA));
+    else in = isub(t1, prod_u(pc.Km, zA));
+    const Iv<T> t3 = prod_s<SS>(h.s2m[va], iadd(zA2, pc.G));           // sigma t3
+    const Iv<T> T2P2 = prod_p(h.T2hiQm, add_s<SS>(in, t3));            // T^2 Phi2            (A.8c)
+    e[c] = isub(T2P2, TY);                                             // (A.8a)
+    small = small && abs_lt_quarter(e[c].lo) && abs_lt_quarter(e[c].hi);
+  }
   // S5
   const Iv<T> sA = h.sA[va];
-  Iv<T> se, sce, cce;                                                  // sin e, sigma sA cos e, cA cos e
-  const bool small = e.lo >= T(-0.25) && e.hi <= T(0.25);
+  Iv<T> se[NC], sce[NC], cce[NC];                                      // sin e, sigma sA cos e, cA cos e
   if (__all_sync(0xffffffffu, small)) {
-    Iv<T> ce;
-    trig_small(e, se, ce);
-    sce = mulpos_s<SS>(ce, sA);
-    cce = mulpos_s<SC>(ce, h.cA);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      Iv<T> ce;
+      trig_small(e[c], se[c], ce);
+      sce[c] = mulpos_s<SS>(ce, sA);
+      cce[c] = mulpos_s<SC>(ce, h.cA);
+    }
   } else {
-    trig_general(e, sA, h.cA, se, sce, cce);
-    if (SS < 0) sce = ineg(sce);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      trig_general(e[c], sA, h.cA, se[c], sce[c], cce[c]);
+      if (SS < 0) sce[c] = ineg(sce[c]);
+    }
   }
-  const Iv<T> cAse = prod_s<SC>(h.cAm, se);
-  const Iv<T> sAse = prod_s<SS>(h.sAm[va], se);                        // sigma sA sin e
-  const Iv<T> sinP = clamp_unit(prod_p(h.iRm, SS < 0 ? isub(cAse, sce) : iadd(sce, cAse)));
-  const Iv<T> cosP = clamp_unit(prod_p(h.iRm, sub_s<SS>(cce, sAse)));
-  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard: roots of normal numbers
+  unsigned bits = 0;
   const T twoT = Rd::mul_rn(T(2), Tn);
-  const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, prod_p(p.Lm, sinP)), T(1)), hp.T2L2), mul_pp(h.T2, sqr_u(cosP)));
-  const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                         // |delta| = D+ / u_d
-  // S7: z = (Zr + LR (dphi + e)) - T (delta cosP), delta = -/+ dq
-  const Iv<T> zz = iadd(Zr, prod_p(p.LRm, iadd(h.dphi[va], e)));
-  const Iv<T> Tdc = iscale_pos(Tn, mul_pu(dq, cosP));
-  const Iv<T> Lq = mul_pp(p.L, dq);                                    // |lambda delta|
-  const Iv<T> qs = mulpos_s<SS>(Lq, h.sA2T[va]);                       // sigma 2T |lambda delta| sA
-  Iv<T> z, ct, Rd1;                                                    // ct = 2T c^tau       (A.7b)
-  if (dneg) {
-    z = iadd(zz, Tdc);
-    ct = add_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
-    Rd1 = isub(p.R, dq);
-  } else {
-    z = isub(zz, Tdc);
-    ct = sub_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
-    Rd1 = iadd(p.R, dq);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    const Iv<T> cAse = prod_s<SC>(h.cAm, se[c]);
+    const Iv<T> sAse = prod_s<SS>(h.sAm[va], se[c]);                   // sigma sA sin e
+    const Iv<T> sinP = clamp_unit(prod_p(h.iRm, SS < 0 ? isub(cAse, sce[c]) : iadd(sce[c], cAse)));
+    const Iv<T> cosP = clamp_unit(prod_p(h.iRm, sub_s<SS>(cce[c], sAse)));
+    // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
+    const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, prod_p(p.Lm, sinP)), T(1)), hp.T2L2), mul_pp(h.T2, sqr_u(cosP)));
+    const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                       // |delta| = D+ / u_d
+    // S7: z = (Zr + LR (dphi + e)) - T (delta cosP), delta = -/+ dq
+    const Iv<T> zz = iadd(Zr[c], prod_p(p.LRm, iadd(h.dphi[va], e[c])));
+    const Iv<T> Tdc = iscale_pos(Tn, mul_pu(dq, cosP));
+    const Iv<T> Lq = mul_pp(p.L, dq);                                  // |lambda delta|
+    const Iv<T> qs = mulpos_s<SS>(Lq, h.sA2T[va]);                     // sigma 2T |lambda delta| sA
+    Iv<T> z, ct, Rd1;                                                  // ct = 2T c^tau       (A.7b)
+    if (dneg) {
+      z = iadd(zz, Tdc);
+      ct = add_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
+      Rd1 = isub(p.R, dq);
+    } else {
+      z = isub(zz, Tdc);
+      ct = sub_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
+      Rd1 = iadd(p.R, dq);
+    }
+    // S8
+    const Iv<T> TLq = iscale_pos(Tn, Lq);
+    const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), ct), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
+    const Iv<T> f = isub(h.Q, rad);
+    // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
+    bits |= (!(is_pos(f.lo) || f.hi < T(0)) ? 1u : 0u) << c;
   }
-  // S8
-  const Iv<T> TLq = iscale_pos(Tn, Lq);
-  const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), ct), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
-  const Iv<T> f = isub(h.Q, rad);
-  return !(f.lo > T(0) || f.hi < T(0));
+  return bits;
 }
 
 }  // namespace ia
