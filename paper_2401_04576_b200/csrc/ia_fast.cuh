@@ -90,6 +90,37 @@ template <int SS, class T> IA_DEV Iv<T> prod_s(MR<T> a, Iv<T> x) {
 // base + sigma * t, where t = |sigma-signed term| as returned by prod_s (SS = 0: t is the term itself)
 template <int SS, class T> IA_DEV Iv<T> add_s(Iv<T> base, Iv<T> t) { return SS < 0 ? isub(base, t) : iadd(base, t); }
 template <int SS, class T> IA_DEV Iv<T> sub_s(Iv<T> base, Iv<T> t) { return SS < 0 ? iadd(base, t) : isub(base, t); }
+// ---- fused product-and-add forms ---------------------------------------------------------------------
+// base + a x and base - a x in ONE directed FMA per rounding step: RD(base.lo + m x.lo) is below the
+// exact base.lo + m x.lo, and the radius term is subtracted from that, so the result is below every
+// base' + a' x' - an enclosure by the same argument as prod_p, one rounding tighter than product
+// followed by sum.  Operand negations and |x| are instruction modifiers.
+template <class T> IA_DEV Iv<T> fma_p(MR<T> a, Iv<T> x, Iv<T> base) {            // base + a x, a >= 0
+  using R = Rnd<T>;
+  return {R::fma_dn(-a.r, fabs(x.lo), R::fma_dn(a.m, x.lo, base.lo)), R::fma_up(a.r, fabs(x.hi), R::fma_up(a.m, x.hi, base.hi))};
+}
+template <class T> IA_DEV Iv<T> fms_p(MR<T> a, Iv<T> x, Iv<T> base) {            // base - a x, a >= 0
+  using R = Rnd<T>;
+  return {R::fma_dn(-a.r, fabs(x.hi), R::fma_dn(-a.m, x.hi, base.lo)), R::fma_up(a.r, fabs(x.lo), R::fma_up(-a.m, x.lo, base.hi))};
+}
+template <class T> IA_DEV Iv<T> fma_u(MR<T> a, Iv<T> x, Iv<T> base) {            // base + a x, a of any class
+  using R = Rnd<T>;
+  const T l0 = R::fma_dn(-a.r, fabs(x.lo), R::fma_dn(a.m, x.lo, base.lo)), l1 = R::fma_dn(-a.r, fabs(x.hi), R::fma_dn(a.m, x.hi, base.lo));
+  const T h0 = R::fma_up(a.r, fabs(x.lo), R::fma_up(a.m, x.lo, base.hi)), h1 = R::fma_up(a.r, fabs(x.hi), R::fma_up(a.m, x.hi, base.hi));
+  return {mn(l0, l1), mx(h0, h1)};
+}
+template <class T> IA_DEV Iv<T> fms_u(MR<T> a, Iv<T> x, Iv<T> base) { return fma_u(mr_neg(a), x, base); }
+// base + a x for a of class SS (+1: a >= 0, -1: a <= 0, 0: any); base - a x
+template <int SS, class T> IA_DEV Iv<T> fma_s(MR<T> a, Iv<T> x, Iv<T> base) {
+  if (SS > 0) return fma_p(a, x, base);
+  if (SS < 0) return fms_p(mr_neg(a), x, base);
+  return fma_u(a, x, base);
+}
+template <int SS, class T> IA_DEV Iv<T> fms_s(MR<T> a, Iv<T> x, Iv<T> base) {
+  if (SS > 0) return fms_p(a, x, base);
+  if (SS < 0) return fma_p(mr_neg(a), x, base);
+  return fms_u(a, x, base);
+}
 // c >= 0 per lane times a block-uniform interval s:  SS = +1: s >= 0; -1: s <= 0, returns c (-s); 0: any
 template <int SS, class T> IA_DEV Iv<T> mulpos_s(Iv<T> c, Iv<T> s) {
   if (SS > 0) return mul_pp(c, s);
@@ -134,6 +165,21 @@ template <class T> IA_DEV Iv<T> sqr_u(Iv<T> a) {
   const bool straddle = sgn(a.lo) != sgn(a.hi);
   const T lo2 = R::mul_dn(mnn, mnn);
   return {straddle ? T(0) : lo2, R::mul_up(mag, mag)};
+}
+// largest / smallest magnitude endpoint and the straddle flag of an interval of unknown sign
+template <class T> struct Mag { T mag, mnn; bool straddle; };
+template <class T> IA_DEV Mag<T> mag_of(Iv<T> a) {
+  const bool c = abs_gt(a.lo, a.hi);
+  return {c ? a.lo : a.hi, c ? a.hi : a.lo, sgn(a.lo) != sgn(a.hi)};
+}
+// base + s a^2 and base - a^2, one FMA per endpoint (s = [s.lo, s.hi] >= 0)
+template <class T> IA_DEV Iv<T> add_sqr(Iv<T> base, Iv<T> a) {
+  const Mag<T> g = mag_of(a);
+  return {g.straddle ? base.lo : Rnd<T>::fma_dn(g.mnn, g.mnn, base.lo), Rnd<T>::fma_up(g.mag, g.mag, base.hi)};
+}
+template <class T> IA_DEV Iv<T> sub_sqr(Iv<T> base, Iv<T> a) {
+  const Mag<T> g = mag_of(a);
+  return {Rnd<T>::fma_dn(-g.mag, g.mag, base.lo), g.straddle ? base.hi : Rnd<T>::fma_up(-g.mnn, g.mnn, base.hi)};
 }
 // intersection with [-1, 1] by integer tests on the high word (keeps the FP64 pipe free):
 // x <= -1  <=>  hi32(x) as unsigned >= hi32(-1);  x >= 1  <=>  hi32(x) as signed >= hi32(1)
@@ -296,6 +342,8 @@ template <class T> struct __align__(16) HitF {
   MR<T> TiQm, T2hiQm, cA2Tm;       // T/Q, T^2/(2Q), 2T c_Ax: the thin scalar folded into the block constant
   Iv<T> sA[2], dphi[2];            // index a = 1 for warps whose lambda was negated
   Iv<T> sA2T[2];                   // 2T s_Ax
+  Iv<T> sA2[2];                    // 2 s_Ax (exact)
+  T twoT;                          // 2 |tan tau| (exact)
   MR<T> sAm[2], s2m[2];
   Iv<T> iQ, iR, c2, s2[2];         // interval forms, general fallback only
   T Tabs;                          // |tan tau|
@@ -328,6 +376,7 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
   o.cAm = to_mr(o.cA);
   const T twoT = Rd::mul_rn(T(2), o.Tabs);
   o.cA2Tm = to_mr(iscale_pos(twoT, o.cA));
+  o.twoT = twoT;
   const int ccls = cls_of(o.cA);
   o.zflip = (t != b) ? 1 : 0;
   // guards of the sign-known forms: R - 2D > 0, R + R_Ax - D > 0, R + delta > 0 (|delta| <= 2 D.hi as
@@ -342,6 +391,7 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
     o.dphi[a] = fd ? ineg(v.dphi) : v.dphi;
     o.sAm[a] = to_mr(o.sA[a]);
     o.sA2T[a] = iscale_pos(twoT, o.sA[a]);
+    o.sA2[a] = {Rd::mul_rn(T(2), o.sA[a].lo), Rd::mul_rn(T(2), o.sA[a].hi)};
     o.s2m[a] = to_mr(o.s2[a]);
     const int scls = cls_of(o.sA[a]), s2cls = cls_of(o.s2[a]);
     int kind = HIT_FAST_U;
@@ -370,8 +420,14 @@ template <class T> struct PairC {
   Iv<T> L2;            // lambda^2
 };
 // ... per (pair, hit)
+#ifndef IA_FUSE
+#define IA_FUSE 1
+#endif
 template <class T> struct HitP {
   Iv<T> LRdphi, T2L2, RpRA;
+#if IA_FUSE
+  MR<T> TL2m;          // (2T) lambda in midpoint form; T2L2 holds 1 + T^2 lambda^2
+#endif
 };
 // ... per (pair, hit, drift sign): S4 terms that do not depend on z0
 template <class T> struct PassC {
@@ -382,7 +438,11 @@ template <class T> struct PassC {
 };
 
 template <class T> IA_DEV HitP<T> hit_prepare(const HitF<T>& h, int va, const PairC<T>& p) {
+#if IA_FUSE
+  return {prod_p(p.LRm, h.dphi[va]), iadd_s(mul_pp(h.T2, p.L2), T(1)), iadd(p.R, h.RA), to_mr(iscale_pos(h.twoT, p.L))};
+#else
   return {prod_p(p.LRm, h.dphi[va]), mul_pp(h.T2, p.L2), iadd(p.R, h.RA)};
+#endif
 }
 
 template <class T> IA_DEV PassC<T> pass_prepare(const HitF<T>& h, bool dneg, const PairC<T>& p, const HitP<T>& hp) {
@@ -479,6 +539,177 @@ IA_DEV unsigned pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& p
     bits |= (!(is_pos(f.lo) || f.hi < T(0)) ? 1u : 0u) << c;
   }
   return bits;
+}
+
+// The same S4-S8 with every product-then-sum written as directed FMAs (fma_p / fms_p / add_sqr ...):
+// the expression DAG and its association order are those of DESIGN.md section 2 except for three
+// re-associations of pure products, (2T)(lambda sin Phi) = ((2T) lambda) sin Phi,
+// T (delta cos Phi) = (T delta) cos Phi and (lambda delta)(2T s_Ax) = (lambda (T delta))(2 s_Ax), which
+// move a factor that is constant over the z0 loop out of it.  Only roundings differ.
+template <int SS, class T>
+IA_DEV unsigned pass_vote_fused(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp,
+                                Iv<T> Zr) {
+  using Rd = Rnd<T>;
+  const T Tn = h.Tabs;
+  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
+  // S4, z0-dependent part
+  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
+  const Iv<T> W = fma_s<SS>(h.sAm[va], zA, pc.LDcA);                   // lambda D cA + zA sA
+  const Iv<T> TY = prod_p(h.TiQm, W);                                  // T Phi1 = -TY        (A.8b)
+  const Iv<T> t1 = prod_p(p.LRm, zA);
+  Iv<T> in;                                                            // t1 - t2
+  if (h.c2cls == CLS_P) in = fms_p(pc.Km, zA, t1);
+  else if (h.c2cls == CLS_N) in = fma_p(mr_neg(pc.Km), zA, t1);
+  else in = fms_u(pc.Km, zA, t1);
+  const Iv<T> V = fma_s<SS>(h.s2m[va], add_sqr(pc.G, zA), in);         // (t1 - t2) + t3
+  const Iv<T> e = fma_p(h.T2hiQm, V, ineg(TY));                        // T^2 Phi2 + T Phi1   (A.8a,c)
+  const bool small = abs_lt_quarter(e.lo) && abs_lt_quarter(e.hi);
+  // S5
+  Iv<T> se, sce, cce;                                                  // sin e, sigma sA cos e, cA cos e
+  if (__all_sync(0xffffffffu, small)) {
+    Iv<T> ce;
+    trig_small(e, se, ce);
+    sce = mulpos_s<SS>(ce, h.sA[va]);
+    cce = mulpos_s<SC>(ce, h.cA);
+  } else {
+    trig_general(e, h.sA[va], h.cA, se, sce, cce);
+    if (SS < 0) sce = ineg(sce);
+  }
+  const Iv<T> sinP = clamp_unit(prod_p(h.iRm, fma_s<SC>(h.cAm, se, SS < 0 ? ineg(sce) : sce)));
+  const Iv<T> cosP = clamp_unit(prod_p(h.iRm, fms_s<SS>(h.sAm[va], se, cce)));
+  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
+  const Iv<T> u2a = fma_p(hp.TL2m, sinP, hp.T2L2);
+  const Mag<T> gc = mag_of(cosP);
+  const Iv<T> u2 = {gc.straddle ? u2a.lo : Rd::fma_dn(h.T2.lo, Rd::mul_dn(gc.mnn, gc.mnn), u2a.lo),
+                    Rd::fma_up(h.T2.hi, Rd::mul_up(gc.mag, gc.mag), u2a.hi)};
+  const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                         // |delta| = D+ / u_d
+  // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = -/+ dq
+  const Iv<T> zz = fma_p(p.LRm, iadd(h.dphi[va], e), Zr);
+  const Iv<T> Tdq = iscale_pos(Tn, dq);                                // |T delta|
+  const Iv<T> TLq = mul_pp(p.L, Tdq);                                  // |T lambda delta|
+  const Iv<T> qs = mulpos_s<SS>(TLq, h.sA2[va]);                       // sigma 2T |lambda delta| sA
+  const T plo = sgn(cosP.lo) ? Tdq.hi : Tdq.lo, phi = sgn(cosP.hi) ? Tdq.lo : Tdq.hi;   // partners of cosP.lo / .hi
+  Iv<T> z, ct, Rd1;                                                    // ct = 2T c^tau       (A.7b)
+  if (dneg) {
+    z = {Rd::fma_dn(plo, cosP.lo, zz.lo), Rd::fma_up(phi, cosP.hi, zz.hi)};
+    ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? ineg(qs) : qs);
+    Rd1 = isub(p.R, dq);
+  } else {
+    z = {Rd::fma_dn(-phi, cosP.hi, zz.lo), Rd::fma_up(-plo, cosP.lo, zz.hi)};
+    ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? qs : ineg(qs));
+    Rd1 = iadd(p.R, dq);
+  }
+  // S8
+  const Iv<T> r1 = {Rd::fma_dn(Rd1.lo, Rd1.lo, -ct.hi), Rd::fma_up(Rd1.hi, Rd1.hi, -ct.lo)};
+  const Iv<T> r2 = sub_sqr(r1, iscale_pos(Tn, z));
+  const Iv<T> rad = {Rd::fma_dn(-TLq.hi, TLq.hi, r2.lo), Rd::fma_up(-TLq.lo, TLq.lo, r2.hi)};
+  const Iv<T> f = isub(h.Q, rad);
+  // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
+  return !(is_pos(f.lo) || f.hi < T(0)) ? 1u : 0u;
+}
+
+// ---- both drift signs side by side ------------------------------------------------------------------
+// The two signs of one (cell, hit) are independent dependency chains that share zA, t1 and the
+// magnitude sort of zA.  Written side by side they give the FP64 pipe four independent instructions
+// per step (two endpoints x two signs): measured on B200, threads with 2 independent DFMA chains keep
+// the pipe 79 % busy whatever the number of resident warps, threads with 4 chains 92 %.
+// D- = -D+ exactly, hence lambda D- c_Ax = -(lambda D+ c_Ax) exactly (negation commutes with directed
+// rounding); G and K differ between the signs and are kept for both.
+template <class T> struct Pass2 {
+  Iv<T> LDcA;          // lambda D+ c_Ax
+  Iv<T> G[2];          // D (R_Ax + lambda^2 (R + R_Ax - D)) for D+, D-
+  MR<T> Km[2];         // (lambda (R - 2D)) cos 2Phi_Ax for D+, D-
+};
+template <class T> IA_DEV Pass2<T> pass_prepare2(const HitF<T>& h, const PairC<T>& p, const HitP<T>& hp) {
+  using Rd = Rnd<T>;
+  Pass2<T> c;
+  const Iv<T> D = {h.Dlo, h.Dhi}, Dn = {-h.Dhi, -h.Dlo};
+  c.LDcA = imul(mul_pp(p.L, D), h.cA);
+  const Iv<T> D2 = {Rd::mul_rn(T(2), D.lo), Rd::mul_rn(T(2), D.hi)};
+  c.Km[0] = to_mr(mul_pu(mul_pp(p.L, isub(p.R, D2)), h.c2));
+  c.Km[1] = to_mr(mul_pu(mul_pp(p.L, iadd(p.R, D2)), h.c2));
+  c.G[0] = mul_pp(D, iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, D))));
+  c.G[1] = mul_pn(iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, Dn))), Dn);
+  return c;
+}
+
+template <int SS, class T>
+IA_DEV unsigned pass_vote2(const HitF<T>& h, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
+  using Rd = Rnd<T>;
+  const T Tn = h.Tabs;
+  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
+  // S4: shared part
+  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
+  const Iv<T> t1 = prod_p(p.LRm, zA);
+  const Mag<T> gz = mag_of(zA);
+  Iv<T> e[2];
+  bool small = true;
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const Iv<T> W = fma_s<SS>(h.sAm[va], zA, s ? ineg(pc.LDcA) : pc.LDcA);   // lambda D cA + zA sA
+    const Iv<T> TY = prod_p(h.TiQm, W);                                // T Phi1 = -TY        (A.8b)
+    Iv<T> in;                                                          // t1 - t2
+    if (h.c2cls == CLS_P) in = fms_p(pc.Km[s], zA, t1);
+    else if (h.c2cls == CLS_N) in = fma_p(mr_neg(pc.Km[s]), zA, t1);
+    else in = fms_u(pc.Km[s], zA, t1);
+    const Iv<T> zG = {gz.straddle ? pc.G[s].lo : Rd::fma_dn(gz.mnn, gz.mnn, pc.G[s].lo), Rd::fma_up(gz.mag, gz.mag, pc.G[s].hi)};
+    const Iv<T> V = fma_s<SS>(h.s2m[va], zG, in);                      // (t1 - t2) + t3
+    e[s] = fma_p(h.T2hiQm, V, ineg(TY));                               // T^2 Phi2 + T Phi1   (A.8a,c)
+    small = small && abs_lt_quarter(e[s].lo) && abs_lt_quarter(e[s].hi);
+  }
+  // S5
+  Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
+  if (__all_sync(0xffffffffu, small)) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      Iv<T> ce;
+      trig_small(e[s], se[s], ce);
+      sce[s] = mulpos_s<SS>(ce, h.sA[va]);
+      cce[s] = mulpos_s<SC>(ce, h.cA);
+    }
+  } else {
+#pragma unroll 1
+    for (int s = 0; s < 2; ++s) {
+      trig_general(e[s], h.sA[va], h.cA, se[s], sce[s], cce[s]);
+      if (SS < 0) sce[s] = ineg(sce[s]);
+    }
+  }
+  bool vote = false;
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const Iv<T> sinP = clamp_unit(prod_p(h.iRm, fma_s<SC>(h.cAm, se[s], SS < 0 ? ineg(sce[s]) : sce[s])));
+    const Iv<T> cosP = clamp_unit(prod_p(h.iRm, fms_s<SS>(h.sAm[va], se[s], cce[s])));
+    // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
+    const Iv<T> u2a = fma_p(hp.TL2m, sinP, hp.T2L2);
+    const Mag<T> gc = mag_of(cosP);
+    const Iv<T> u2 = {gc.straddle ? u2a.lo : Rd::fma_dn(h.T2.lo, Rd::mul_dn(gc.mnn, gc.mnn), u2a.lo),
+                      Rd::fma_up(h.T2.hi, Rd::mul_up(gc.mag, gc.mag), u2a.hi)};
+    const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                       // |delta| = D+ / u_d
+    // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (s = 0), -dq (s = 1)
+    const Iv<T> zz = fma_p(p.LRm, iadd(h.dphi[va], e[s]), Zr);
+    const Iv<T> Tdq = iscale_pos(Tn, dq);                              // |T delta|
+    const Iv<T> TLq = mul_pp(p.L, Tdq);                                // |T lambda delta|
+    const Iv<T> qs = mulpos_s<SS>(TLq, h.sA2[va]);                     // sigma 2T |lambda delta| sA
+    const T plo = sgn(cosP.lo) ? Tdq.hi : Tdq.lo, phi = sgn(cosP.hi) ? Tdq.lo : Tdq.hi;   // partners of cosP.lo / .hi
+    Iv<T> z, ct, Rd1;                                                  // ct = 2T c^tau       (A.7b)
+    if (s) {
+      z = {Rd::fma_dn(plo, cosP.lo, zz.lo), Rd::fma_up(phi, cosP.hi, zz.hi)};
+      ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? ineg(qs) : qs);
+      Rd1 = isub(p.R, dq);
+    } else {
+      z = {Rd::fma_dn(-phi, cosP.hi, zz.lo), Rd::fma_up(-plo, cosP.lo, zz.hi)};
+      ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? qs : ineg(qs));
+      Rd1 = iadd(p.R, dq);
+    }
+    // S8
+    const Iv<T> r1 = {Rd::fma_dn(Rd1.lo, Rd1.lo, -ct.hi), Rd::fma_up(Rd1.hi, Rd1.hi, -ct.lo)};
+    const Iv<T> r2 = sub_sqr(r1, iscale_pos(Tn, z));
+    const Iv<T> rad = {Rd::fma_dn(-TLq.hi, TLq.hi, r2.lo), Rd::fma_up(-TLq.lo, TLq.lo, r2.hi)};
+    const Iv<T> f = isub(h.Q, rad);
+    // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
+    vote = vote || !(is_pos(f.lo) || f.hi < T(0));
+  }
+  return vote ? 1u : 0u;
 }
 
 }  // namespace ia

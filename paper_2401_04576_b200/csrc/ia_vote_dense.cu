@@ -8,7 +8,7 @@
 // then walks its cells, reads the hits by shared-memory broadcast, keeps its vote count in a
 // register and writes one uint16 per cell.  No atomics, no inter-thread traffic in the loop.
 #include "ia_internal.h"
-#include "ia_fast.cuh"
+#include "ia_fastq.cuh"
 
 namespace ia {
 
@@ -104,10 +104,19 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
 #define IA_FAST_NC 1
 #endif
 constexpr int FAST_NC = IA_FAST_NC;
+#ifndef IA_DUAL
+#define IA_DUAL 1
+#endif
 template <int SS, class T>
 IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
   unsigned bits = 0;
+#if IA_DUAL
+  const Pass2<T> pc2 = pass_prepare2(h, p, hp);
+#pragma unroll 1
+  for (int i = 0; i < nz_tile; ++i) bits |= pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]) << i;
+  return bits;
+#endif
   const unsigned full = (1u << nz_tile) - 1u;
 #pragma unroll 1
   for (int s = 0; s < 2; ++s) {
@@ -116,12 +125,17 @@ IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T
     if (__all_sync(0xffffffffu, bits == full)) break;
     const PassC<T> pc = pass_prepare(h, dneg, p, hp);
     int i = 0;
+#if IA_FUSE
+#pragma unroll 1
+    for (; i < nz_tile; ++i) bits |= pass_vote_fused<SS>(h, va, dneg, pc, p, hp, zt[i]) << i;
+#else
 #pragma unroll 1
     for (; i + FAST_NC <= nz_tile; i += FAST_NC) bits |= pass_vote<SS, FAST_NC>(h, va, dneg, pc, p, hp, zt + i) << i;
     if (FAST_NC > 1) {
 #pragma unroll 1
       for (; i < nz_tile; ++i) bits |= pass_vote<SS, 1>(h, va, dneg, pc, p, hp, zt + i) << i;
     }
+#endif
   }
   return bits;
 }
