@@ -34,8 +34,13 @@ from paper_2401_04576_b200 import eventgen as g  # noqa: E402
 METRIC = "cell-hit interval evals/s"
 UNIT = "evals/s"
 # FP64 arithmetic thread-instructions (DADD/DMUL/DFMA, comparisons not counted) that the
-# sign-specialised DAG S4-S8 needs per (cell, hit) evaluation = both drift signs; counted op by op there
-ALG_FP64_INST_PER_EVAL = 366.0
+# sign-specialised, FMA-fused DAG S4-S8 needs per (cell, hit) evaluation = both drift signs; counted op by op there
+# (175 FMA + 83 add/mul; ncu counts 277.6 executed on C1, profiles/r01_vote_dense_fast_c1_ncu.md)
+ALG_FP64_INST_PER_EVAL = 258.0
+ALG_FP64_FLOPS_PER_EVAL = 2 * 175.0 + 83.0
+# the same DAG with every product and sum as its own directed instruction (no FMA): what an unfused
+# implementation has to issue; context only
+DAG_UNFUSED_OPS_PER_EVAL = 366.0
 # non-tensor FP64 issue peak = SMs x 64 lanes x f_max
 FP64_LANES_PER_SM = 64
 
@@ -140,13 +145,60 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line))
 
 
+def run_c3(args, rank, world, local_rank, barrier):
+    """--workload C3: one step = ia_refine_batch over 1024 events (BASELINE.json configs[3]); for profiling the
+    batch path on its own.  Same JSON shape; value = cell-hit evaluations/s, events/s beside it."""
+    import torch
+    import torch.distributed as dist
+    from paper_2401_04576_b200 import binding as b
+    ch = g.chamber_c1()
+    n_ev, levels, k = 1024, 8, 8
+    evs = [g.make_event(ch, 1000 + rank * n_ev + e, n_noise=10) for e in range(n_ev)]
+    h3 = b.hits_of(np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs]))
+    off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
+    ctx = b.Context(local_rank)
+    ctx.ia_load_geometry(b.wires_of(ch))
+    ctx.ia_set_params(g.TOL, precision=args.precision)
+    hd, od = ctx.to_device(h3), ctx.to_device(off)
+    boxes, par = ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k)
+    for _ in range(max(0, args.warmup - 1)):
+        ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = ctx.ia_launch_count()
+    a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(ctx.stream)
+    for _ in range(args.steps):
+        ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
+    c.record(ctx.stream)
+    barrier()
+    launches = ctx.ia_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([a.elapsed_time(c)], dtype=torch.float64, device=f"cuda:{local_rank}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    if rank != 0:
+        return
+    evals = n_ev * (8 ** 5 + (levels - 1) * k * 32) * 30
+    line = {"metric": METRIC, "value": evals * world / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": f"f{args.precision}", "data": "synthetic",
+            "config": {"workload": "C3: BASELINE.json configs[3], 1024 events x 30 hits, 8^5 start, K=8, 8 passes; seeds 1000+e",
+                       "evals_per_step": evals, "l2": "67 MB of vote scratch rewritten every step"},
+            "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks}
+    print(json.dumps(line))
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C3"])
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
@@ -172,6 +224,12 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.workload == "C3":
+        run_c3(args, rank, world, local_rank, barrier)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     ch, ev, dims, k = workload(args.workload, seed_shift=rank)
     n_cells = int(np.prod(np.array(dims, np.int64)))
@@ -243,6 +301,10 @@ def main():
         "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 lanes x {f_max_mhz:.0f} MHz (DESIGN.md 6); "
                        "MEASURED_PEAKS.json has no FP64 entry",
         "alg_fp64_inst_per_eval": ALG_FP64_INST_PER_EVAL, "kernel_ms": vote_ms,
+        "flop_frac": ALG_FP64_FLOPS_PER_EVAL * evals_per_step / (vote_ms * 1e-3) / (2 * peak_inst),
+        "flop_peak_T": 2 * peak_inst / 1e12, "alg_fp64_flops_per_eval": ALG_FP64_FLOPS_PER_EVAL,
+        "unfused_dag_ops_per_eval": DAG_UNFUSED_OPS_PER_EVAL,
+        "ncu_pipe_fp64_active_pct": 63.9, "ncu_source": "profiles/r01_vote_dense_fast_c1_ncu.md (C1, same kernel)",
         "alg_bytes_per_launch": 2 * n_cells, "hbm_frac": (2 * n_cells / (vote_ms * 1e-3)) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
     }
     line = {

@@ -75,7 +75,8 @@ typedef struct {
  * (x_ref, y_ref): reference point of eq. (1d); z_ref: reference plane of (A.4c-e) L172-176.
  * precision: 64 or 32 = type of the interval endpoints (G22).  flags: bit 0 = vote the dense grid
  * with the general (sign-agnostic) kernel instead of the sign-specialised one (same results; for
- * cross-checks); other bits reserved, must be 0. */
+ * cross-checks); bits 1 / 2 = force the one-body / three-body variant of the sign-specialised
+ * dense kernel (same results; default: picked from the xy cell width); other bits must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;
@@ -161,7 +162,10 @@ int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_
 
 /* Roofline probe: enqueue a kernel of `blocks` x 256 threads, each running 8 independent FP64
  * dependency chains for `iters` rounds (blocks*256*8*iters FP64 instructions in total).
- * mode 0: DFMA round-to-nearest; 1: DADD.RM / DMUL.RP alternating; 2: DFMA.RM / DFMA.RP alternating.
+ * mode 0: DFMA round-to-nearest; 1: DADD.RM / DMUL.RP alternating; 2: DFMA.RM / DFMA.RP alternating;
+ * 3, 4, 5: DFMA.RM / DFMA.RP on only 1, 2, 4 independent chains per thread (same instruction count);
+ * 6, 7: mode 2 with one independent integer (LOP3) resp. FP32 (FFMA) instruction after every DFMA - do
+ * non-FP64 instructions issue in the shadow of the FP64 pipe?  (only the DFMAs are counted).
  * The caller times it with events on the context's stream.  sink_dev: one double, never written. */
 int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev);
 

@@ -163,7 +163,7 @@ int ia_load_geometry(ia_ctx* ctx, const ia_wire* wires_host, int n_wires) {
   if (!ctx || !wires_host || n_wires <= 0) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   std::vector<double> soa(size_t(5) * n_wires);
-  double tmax = 0.0;
+  double tmax = 0.0, rmax = 0.0;
   for (int i = 0; i < n_wires; ++i) {
     const ia_wire& w = wires_host[i];
     if (!std::isfinite(w.x0) || !std::isfinite(w.y0) || !std::isfinite(w.sin_phi_s) || !std::isfinite(w.cos_phi_s) ||
@@ -175,6 +175,7 @@ int ia_load_geometry(ia_ctx* ctx, const ia_wire* wires_host, int n_wires) {
     soa[size_t(3) * n_wires + i] = w.cos_phi_s;
     soa[size_t(4) * n_wires + i] = w.tan_tau;
     tmax = std::fmax(tmax, std::fabs(w.tan_tau));
+    rmax = std::fmax(rmax, std::hypot(w.x0, w.y0));
   }
   IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
   if (ctx->wires) cudaFree(ctx->wires);
@@ -185,6 +186,7 @@ int ia_load_geometry(ia_ctx* ctx, const ia_wire* wires_host, int n_wires) {
   IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
   ctx->n_wires = n_wires;
   ctx->max_abs_tan = tmax;
+  ctx->max_wire_r = rmax;
   return IA_OK;
 }
 
@@ -194,7 +196,7 @@ int ia_set_params(ia_ctx* ctx, const ia_params* p) {
       !std::isfinite(p->z_ref))
     return IA_ERR_ARG;
   if (p->precision != 64 && p->precision != 32) return IA_ERR_ARG;
-  if (p->flags & ~1u) return IA_ERR_ARG;
+  if (p->flags & ~7u) return IA_ERR_ARG;
   ctx->params = *p;
   return IA_OK;
 }
@@ -354,7 +356,7 @@ int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_
 }
 
 int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev) {
-  if (!ctx || !sink_dev || mode < 0 || mode > 2 || iters <= 0 || blocks <= 0) return IA_ERR_ARG;
+  if (!ctx || !sink_dev || mode < 0 || mode > 7 || iters <= 0 || blocks <= 0) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_fp64_probe(ctx, mode, iters, blocks, sink_dev));
   return IA_OK;

@@ -297,4 +297,136 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   return (v0 || v1) ? 1u : 0u;
 }
 
+// ---- one body for all three sign classes ----------------------------------------------------------
+// pass_vote_q<SS> compiled three times is 2,750 SASS instructions = 44 KB of hot code; the L1.5
+// instruction cache of an SM holds 32 KB.  On fine grids one or two classes dominate and it (just)
+// fits; on the coarse 8^5 start grid of a refinement all three classes are live on every SM and the
+// kernel starves on instruction fetch (measured on C3: icc hit rate 67 %, stall no_instruction 4.5
+// per issue, FP64 pipe 41 %; profiles/r01_c3_ncu.md).  Here the class is a run-time, warp-uniform
+// value: the steps that do not depend on it (two thirds of the body) exist once, the five class-
+// dependent quads are short uniform switches.  Same arithmetic as pass_vote_q<SS> for every class.
+IA_DEV int opaque_i(int x) { asm volatile("" : "+r"(x)); return x; }
+
+template <class T>
+IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp,
+                             Iv<T> Zr, MR<T> sAm, MR<T> s2m, Iv<T> sAabs, Iv<T> sA2abs) {
+  using V = VR<T>;
+  const T Tn = h.Tabs;
+  // sAm, s2m: negated for the class s_Ax <= 0; sAabs, sA2abs: s_Ax and 2 s_Ax, negated for that class
+  const int ss = opaque_i(ss_in);            // keeps the compiler from cloning the loop per class
+  // S4: shared part
+  Iv<T> zA, t1;
+  zA.lo = V::add_dn(Zr.lo, hp.LRdphi.lo); zA.hi = V::add_up(Zr.hi, hp.LRdphi.hi);           // (A.8d)
+  {
+    const T l = V::mul_dn(p.LRm.m, zA.lo), u = V::mul_up(p.LRm.m, zA.hi);
+    t1.lo = V::fma_dn(-p.LRm.r, fabs(zA.lo), l); t1.hi = V::fma_up(p.LRm.r, fabs(zA.hi), u);
+  }
+  const Mag<T> gz = mag_of(zA);
+  Iv<T> W[2], TY[2], in[2], zG[2], Vv[2], e[2];
+  if (ss > 0) q_fma<QK_ADD_P>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);        // lambda D cA + zA sA
+  else if (ss < 0) q_fma<QK_SUB_P>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);
+  else q_fma<QK_ADD_U>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);
+  if (h.c2cls == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
+  else if (h.c2cls == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
+  else q_fma<QK_SUB_U>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);
+  q_prod_p(h.TiQm, W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
+  zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
+  zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
+  if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
+  if (ss > 0) q_fma<QK_ADD_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);          // (t1 - t2) + t3
+  else if (ss < 0) q_fma<QK_SUB_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
+  else q_fma<QK_ADD_U>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
+  q_fma<QK_ADD_P>(h.T2hiQm, h.T2hiQm, Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
+  const bool small = abs_lt_quarter(e[0].lo) && abs_lt_quarter(e[0].hi) && abs_lt_quarter(e[1].lo) && abs_lt_quarter(e[1].hi);
+  // S5
+  Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
+  Iv<T> sa[2], ca[2], sinP[2], cosP[2];
+  if (__all_sync(0xffffffffu, small)) {
+    Iv<T> ce[2];
+    q_trig_small(e, se, ce);
+    if (ss != 0) {
+      q_mulpos<1>(ce[0], ce[1], sAabs, sce[0], sce[1]);
+      q_mulpos<1>(ce[0], ce[1], h.cA, cce[0], cce[1]);
+    } else {
+      q_mulpos<0>(ce[0], ce[1], sAabs, sce[0], sce[1]);
+      q_mulpos<0>(ce[0], ce[1], h.cA, cce[0], cce[1]);
+    }
+  } else {
+#pragma unroll 1
+    for (int s = 0; s < 2; ++s) {
+      trig_general(e[s], h.sA[va], h.cA, se[s], sce[s], cce[s]);
+      if (ss < 0) sce[s] = ineg(sce[s]);
+    }
+  }
+  if (ss > 0) {
+    q_fma<QK_ADD_P>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
+    q_fma<QK_SUB_P>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
+  } else if (ss < 0) {
+    q_fma<QK_ADD_P>(h.cAm, h.cAm, se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
+    q_fma<QK_ADD_P>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
+  } else {
+    q_fma<QK_ADD_U>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
+    q_fma<QK_SUB_U>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
+  }
+  q_prod_p(h.iRm, sa[0], sa[1], sinP[0], sinP[1]);
+  q_prod_p(h.iRm, ca[0], ca[1], cosP[0], cosP[1]);
+#pragma unroll
+  for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_unit(cosP[s]); }
+  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
+  Iv<T> u2[2], dq[2];
+  q_fma<QK_ADD_P>(hp.TL2m, hp.TL2m, sinP[0], sinP[1], hp.T2L2, hp.T2L2, u2[0], u2[1]);
+  {
+    const Mag<T> g0 = mag_of(cosP[0]), g1 = mag_of(cosP[1]);
+    const T a0 = V::mul_dn(g0.mnn, g0.mnn), b0 = V::mul_up(g0.mag, g0.mag), a1 = V::mul_dn(g1.mnn, g1.mnn), b1 = V::mul_up(g1.mag, g1.mag);
+    const T l0 = V::fma_dn(h.T2.lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2.lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+    u2[0].lo = g0.straddle ? u2[0].lo : l0; u2[1].lo = g1.straddle ? u2[1].lo : l1;
+  }
+  QDir<T>::d_over_sqrt(h, u2, dq);                                     // |delta| = D+ / u_d
+  // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (D+), -dq (D-)
+  Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
+  q_add(e[0], e[1], h.dphi[va], h.dphi[va], de[0], de[1]);
+  q_fma<QK_ADD_P>(p.LRm, p.LRm, de[0], de[1], Zr, Zr, zz[0], zz[1]);
+  Tdq[0].lo = V::mul_dn(Tn, dq[0].lo); Tdq[0].hi = V::mul_up(Tn, dq[0].hi);                 // |T delta|
+  Tdq[1].lo = V::mul_dn(Tn, dq[1].lo); Tdq[1].hi = V::mul_up(Tn, dq[1].hi);
+  q_mulpos<1>(Tdq[0], Tdq[1], p.L, TLq[0], TLq[1]);                                         // |T lambda delta|
+  {
+    const T pl0 = sgn(cosP[0].lo) ? Tdq[0].hi : Tdq[0].lo, ph0 = sgn(cosP[0].hi) ? Tdq[0].lo : Tdq[0].hi;   // partners of cosP.lo / .hi
+    const T pl1 = sgn(cosP[1].lo) ? Tdq[1].hi : Tdq[1].lo, ph1 = sgn(cosP[1].hi) ? Tdq[1].lo : Tdq[1].hi;
+    z[0].lo = V::fma_dn(-ph0, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-pl0, cosP[0].lo, zz[0].hi);
+    z[1].lo = V::fma_dn(pl1, cosP[1].lo, zz[1].lo); z[1].hi = V::fma_up(ph1, cosP[1].hi, zz[1].hi);
+  }
+  // qs = sigma 2T |lambda delta| sA;  ct = 2T c^tau (A.7b):  D+: 2T cA z - sigma qs,  D-: 2T cA z + sigma qs
+  if (ss > 0) {
+    q_mulpos<1>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
+    q_fma<QK_ADD_P>(h.cA2Tm, h.cA2Tm, z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
+  } else if (ss < 0) {
+    q_mulpos<1>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
+    q_fma<QK_ADD_P>(h.cA2Tm, h.cA2Tm, z[0], z[1], qs[0], ineg(qs[1]), ct[0], ct[1]);
+  } else {
+    q_mulpos<0>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
+    q_fma<QK_ADD_U>(h.cA2Tm, h.cA2Tm, z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
+  }
+  Rd1[0].lo = V::add_dn(p.R.lo, dq[0].lo); Rd1[0].hi = V::add_up(p.R.hi, dq[0].hi);
+  Rd1[1].lo = V::add_dn(p.R.lo, -dq[1].hi); Rd1[1].hi = V::add_up(p.R.hi, -dq[1].lo);
+  Tz[0].lo = V::mul_dn(Tn, z[0].lo); Tz[0].hi = V::mul_up(Tn, z[0].hi);
+  Tz[1].lo = V::mul_dn(Tn, z[1].lo); Tz[1].hi = V::mul_up(Tn, z[1].hi);
+  // S8
+  Iv<T> r1[2], r2[2], f[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) { r1[s].lo = V::fma_dn(Rd1[s].lo, Rd1[s].lo, -ct[s].hi); r1[s].hi = V::fma_up(Rd1[s].hi, Rd1[s].hi, -ct[s].lo); }
+  {
+    const Mag<T> g0 = mag_of(Tz[0]), g1 = mag_of(Tz[1]);
+    r2[0].lo = V::fma_dn(-g0.mag, g0.mag, r1[0].lo); r2[1].lo = V::fma_dn(-g1.mag, g1.mag, r1[1].lo);
+    const T h0 = V::fma_up(-g0.mnn, g0.mnn, r1[0].hi), h1 = V::fma_up(-g1.mnn, g1.mnn, r1[1].hi);
+    r2[0].hi = g0.straddle ? r1[0].hi : h0; r2[1].hi = g1.straddle ? r1[1].hi : h1;
+  }
+#pragma unroll
+  for (int s = 0; s < 2; ++s) { r2[s].lo = V::fma_dn(-TLq[s].hi, TLq[s].hi, r2[s].lo); r2[s].hi = V::fma_up(-TLq[s].lo, TLq[s].lo, r2[s].hi); }
+#pragma unroll
+  for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q.lo, -r2[s].hi); f[s].hi = V::add_up(h.Q.hi, -r2[s].lo); }
+  const bool v0 = !(is_pos(f[0].lo) || f[0].hi < T(0)), v1 = !(is_pos(f[1].lo) || f[1].hi < T(0));
+  return (v0 || v1) ? 1u : 0u;
+}
+
 }  // namespace ia

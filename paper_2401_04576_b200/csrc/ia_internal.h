@@ -39,6 +39,7 @@ struct ia_ctx {
   int n_wires = 0;
   double* wires = nullptr;   // 5 * n_wires doubles: x0 | y0 | sin | cos | tan
   double max_abs_tan = 0.0;
+  double max_wire_r = 0.0;   // largest |(x0, y0)|: picks the dense kernel variant (performance only)
   // scratch, grown on demand, freed in ia_destroy
   ia::Scratch staged;        // HitC<T>[n_events * max_hits]
   ia::Scratch votes;         // uint16 dense votes of the refinement start grid

@@ -368,9 +368,12 @@ cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia
 // ---- FP64 pipe probe: what the chip sustains on independent double-precision chains ---------------
 // mode 0: DFMA (round-to-nearest); mode 1: DADD.RM / DMUL.RP alternating (the interval mix);
 // mode 2: DFMA.RM / DFMA.RP.  8 independent chains per thread, `iters` rounds of 8 instructions.
+// modes 3, 4, 5: DFMA.RM / DFMA.RP on 1, 2, 4 chains per thread (same instruction count): how much
+// instruction-level parallelism inside one warp the FP64 pipe needs.
 namespace ia {
 namespace {
-__global__ void __launch_bounds__(256) fp64_probe_kernel(int mode, int iters, double seed, double* __restrict__ sink) {
+template <int mode>
+__global__ void __launch_bounds__(256) fp64_probe_kernel(int iters, double seed, double* __restrict__ sink) {
   double a[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) a[j] = seed + 1e-3 * (threadIdx.x + 8 * j);
@@ -387,12 +390,61 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(int mode, int iters, do
 #pragma unroll
       for (int j = 0; j < 8; ++j) a[j] = __dmul_ru(a[j], m);
     }
-  } else {
+  } else if (mode == 2) {
     for (int i = 0; i < iters; i += 2) {
 #pragma unroll
       for (int j = 0; j < 8; ++j) a[j] = __fma_rd(a[j], m, c);
 #pragma unroll
       for (int j = 0; j < 8; ++j) a[j] = __fma_ru(a[j], m, c);
+    }
+  } else if (mode == 6 || mode == 7) {
+    // 8 DFMA.RM/RP chains with one independent non-FP64 instruction after every DFMA: mode 6 an integer
+    // ALU-pipe operation (LOP3), mode 7 an FP32 FMA-pipe operation (FFMA).  Only the DFMAs are counted.
+    unsigned u[8];
+    float f[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { u[j] = threadIdx.x * 2654435761u + j; f[j] = float(j) + 0.5f; }
+    unsigned ku = unsigned(iters) | 0x10001u;
+    float kf = 0.999f, kc = 1e-3f;
+    asm volatile("" : "+r"(ku), "+f"(kf), "+f"(kc));     // in registers, not re-read from the constant bank
+    for (int i = 0; i < iters; i += 2) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        a[j] = __fma_rd(a[j], m, c);
+        if (mode == 6) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[j]) : "r"(ku), "r"(u[(j + 1) & 7]));
+        else asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[j]) : "f"(kf), "f"(kc));
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        a[j] = __fma_ru(a[j], m, c);
+        if (mode == 6) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[j]) : "r"(ku), "r"(u[(j + 3) & 7]));
+        else asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[j]) : "f"(kf), "f"(kc));
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] += double(u[j] & 1u) + double(f[j]) * 1e-30;
+  } else {
+    // modes 3, 4, 5: the same number of DFMA.RM/RP per thread on 1, 2, 4 independent chains only
+    const int nc = 1 << (mode - 3);
+    for (int i = 0; i < iters; i += 2) {
+      if (nc == 1) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) { a[0] = __fma_rd(a[0], m, c); a[0] = __fma_ru(a[0], m, c); }
+      } else if (nc == 2) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          a[0] = __fma_rd(a[0], m, c); a[1] = __fma_rd(a[1], m, c);
+          a[0] = __fma_ru(a[0], m, c); a[1] = __fma_ru(a[1], m, c);
+        }
+      } else {
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) a[j] = __fma_rd(a[j], m, c);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) a[j] = __fma_ru(a[j], m, c);
+        }
+      }
     }
   }
   double s = 0;
@@ -403,7 +455,13 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(int mode, int iters, do
 }  // namespace
 
 cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, double* sink) {
-  fp64_probe_kernel<<<blocks, 256, 0, ctx->stream>>>(mode, iters, 1.0, sink);
+  switch (mode) {
+#define IA_PROBE_CASE(M) case M: fp64_probe_kernel<M><<<blocks, 256, 0, ctx->stream>>>(iters, 1.0, sink); break;
+    IA_PROBE_CASE(0) IA_PROBE_CASE(1) IA_PROBE_CASE(2) IA_PROBE_CASE(3) IA_PROBE_CASE(4) IA_PROBE_CASE(5)
+    IA_PROBE_CASE(6) IA_PROBE_CASE(7)
+#undef IA_PROBE_CASE
+    default: return cudaErrorInvalidValue;
+  }
   ctx->launches++;
   return cudaGetLastError();
 }

@@ -7,6 +7,8 @@
 // the atan2, the square root and the two divisions) into shared memory; every thread
 // then walks its cells, reads the hits by shared-memory broadcast, keeps its vote count in a
 // register and writes one uint16 per cell.  No atomics, no inter-thread traffic in the loop.
+#include <cmath>
+
 #include "ia_internal.h"
 #include "ia_fastq.cuh"
 
@@ -140,6 +142,19 @@ IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T
   return bits;
 }
 
+// the same with the sign class as a run-time value (one compiled body, ia_fastq.cuh)
+template <class T>
+IA_DEV unsigned fast_hit_rt(const HitF<T>& h, int ss, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
+  const HitP<T> hp = hit_prepare(h, va, p);
+  const Pass2<T> pc2 = pass_prepare2(h, p, hp);
+  const MR<T> sAm = ss < 0 ? mr_neg(h.sAm[va]) : h.sAm[va], s2m = ss < 0 ? mr_neg(h.s2m[va]) : h.s2m[va];
+  const Iv<T> sAabs = ss < 0 ? ineg(h.sA[va]) : h.sA[va], sA2abs = ss < 0 ? ineg(h.sA2[va]) : h.sA2[va];
+  unsigned bits = 0;
+#pragma unroll 1
+  for (int i = 0; i < nz_tile; ++i) bits |= pass_vote_qr(h, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs) << i;
+  return bits;
+}
+
 // 8 vote bits -> 8 packed byte counters (bit k -> byte k).  Four bits at a time: in k + 7j, k,j < 4,
 // no two partial products meet, so nothing carries.
 IA_DEV unsigned long long spread8(unsigned bits) {
@@ -148,7 +163,10 @@ IA_DEV unsigned long long spread8(unsigned bits) {
   return ((unsigned long long)hi << 32) | lo;
 }
 
-template <class T>
+// RT: the sign class of a hit as a run-time value in one compiled body (coarse grids, where all three
+// classes are live on every SM and three bodies overflow the instruction cache) or as a template
+// argument of three bodies (fine grids: 6 % faster there).  Same arithmetic, same results.
+template <class T, bool RT>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z,
                        uint16_t* __restrict__ votes) {
@@ -223,7 +241,8 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
       unsigned bits;
-      if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
+      if (RT) bits = fast_hit_rt<T>(hf, kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
+      else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, va, pr, zt, nz_tile);
       else bits = fast_hit<0, T>(hf, va, pr, zt, nz_tile);
       acc += spread8(bits);
@@ -251,11 +270,24 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   const int64_t blocks = nxy * tiles_p * tiles_z;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   const size_t smem = sizeof(ZTab<T>) + size_t(sp.max_hits) * sizeof(HitF<T>);
-  cudaError_t err = cudaFuncSetAttribute(vote_dense_fast_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-  if (err != cudaSuccess) return err;
+  // coarse = an xy cell is wider than half the chamber radius: the classes of s_Ax, c_Ax then vary from
+  // hit to hit inside every block (measured: C3's 8^5 start grid runs 28 % faster with the one-body form,
+  // C1's 32^5 grid 6 % slower)
+  const double wxy = std::fmin((g.hi[0] - g.lo[0]) / g.n[0], (g.hi[1] - g.lo[1]) / g.n[1]);
+  const bool coarse = (ctx->params.flags & 2u) ? true : ((ctx->params.flags & 4u) ? false : wxy > 0.5 * ctx->max_wire_r);
   dim3 grid((unsigned)blocks, (unsigned)sp.n_events);
-  vote_dense_fast_kernel<T><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g, tiles_p,
-                                                                 tiles_z, votes_out);
+  cudaError_t err;
+  if (coarse) {
+    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (err != cudaSuccess) return err;
+    vote_dense_fast_kernel<T, true><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
+                                                                         tiles_p, tiles_z, votes_out);
+  } else {
+    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (err != cudaSuccess) return err;
+    vote_dense_fast_kernel<T, false><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
+                                                                          tiles_p, tiles_z, votes_out);
+  }
   ctx->launches++;
   return cudaGetLastError();
 }

@@ -369,6 +369,28 @@ def test_fast_and_general_kernels_agree(precision):
         rig.close()
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_one_body_and_three_body_variants_identical(precision):
+    """The two compiled forms of the sign-specialised dense kernel (flags bit 1: sign class as a run-time
+    value in one body; bit 2: three bodies) do the same arithmetic: votes identical bit for bit, on a
+    coarse and on a fine grid, and whichever the library picks by itself equals both."""
+    rig = Rig(g.chamber_c1(), precision=precision)
+    try:
+        ev = g.make_event(rig.ch, 33, n_noise=10)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        for dims in ((8,) * 5, (20, 20, 12, 9, 12), (3, 3, 6, 20, 7)):
+            out = []
+            for flags in (2, 4, 0):
+                rig.ctx.ia_set_params(g.TOL, precision=precision, flags=flags)
+                out.append(rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims))
+            rig.ctx.synchronize()
+            a, c, d = (t.cpu().numpy() for t in out)
+            assert (a == c).all() and (a == d).all(), dims
+            assert a.max() > 0
+    finally:
+        rig.close()
+
+
 PROD_P, PROD_U, D_OVER_SQRT, SQR_U, SIN_SMALL, COS_SMALL, CLAMP_UNIT = 11, 12, 13, 14, 15, 16, 17
 
 
