@@ -1,13 +1,11 @@
 // ia_fast.cuh - the FP64-pipe form of the residual enclosure (steps S4-S8) for the dense vote.
 //
 // Same expression DAG as ia_residual.cuh and the same association order.  What changes is how each
-// interval product is formed, because on sm_100a the cost of a product is not its multiplies:
-// measured on B200 (profiles/r01_pipe_probe.md) an FP64 instruction holds the 16-lane FP64 pipe of a
-// sub-partition for 2 cycles but its issue port for 1, while FSEL / ISETP / LOP3 (the "pick the
-// partner endpoint by the sign of x" selects of the textbook sign-case product) hold the half-rate
-// ALU pipe for 2 cycles each, and cycles per evaluation follow 2 N_alu + N_fp64 + N_other.  The
-// select-based product (2 DMUL + 2 ISETP + 4 FSEL) therefore costs 14 cycles, the one below 4 FP64
-// instructions and nothing else:
+// interval product is formed.  The dense kernel is bound by the FP64 pipe and by the dependency
+// latency around it (profiles/r01_pipe_probe.md: a dependent FP64 instruction issues 8 cycles after
+// its producer; profiles/r01_vote_dense_fast_c1_ncu.md), and the textbook sign-case product - pick the
+// partner endpoint by the sign of x, then multiply (2 DMUL + 2 ISETP + 4 FSEL) - puts a compare and a
+// select between every pair of FP64 instructions.  The form below is 4 FP64 instructions and nothing else:
 //
 //   factor a of KNOWN sign class, kept as midpoint and radius (m, r) with [m-r, m+r] containing a,
 //   times x = [x.lo, x.hi] of ANY sign:   for a >= 0
@@ -611,8 +609,8 @@ IA_DEV unsigned pass_vote_fused(const HitF<T>& h, int va, bool dneg, const PassC
 // ---- both drift signs side by side ------------------------------------------------------------------
 // The two signs of one (cell, hit) are independent dependency chains that share zA, t1 and the
 // magnitude sort of zA.  Written side by side they give the FP64 pipe four independent instructions
-// per step (two endpoints x two signs): measured on B200, threads with 2 independent DFMA chains keep
-// the pipe 79 % busy whatever the number of resident warps, threads with 4 chains 92 %.
+// per step (two endpoints x two signs), which covers its 8-cycle dependent-issue latency from inside
+// one warp (profiles/r01_pipe_probe.md).
 // D- = -D+ exactly, hence lambda D- c_Ax = -(lambda D+ c_Ax) exactly (negation commutes with directed
 // rounding); G and K differ between the signs and are kept for both.
 template <class T> struct Pass2 {

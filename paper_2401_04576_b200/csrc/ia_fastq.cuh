@@ -1,16 +1,15 @@
 // ia_fastq.cuh - S4-S8 for both drift signs of one (cell, hit), scheduled for the FP64 pipe of sm_100a.
 //
-// Why this file exists (measured on B200): a sub-partition issues an FP64
-// instruction every 2 cycles when it follows an FP64 instruction of the SAME warp, every 3 cycles
-// when it follows one of another warp, and a dependent FP64 instruction 8 cycles after its producer.
-// Threads with one dependency chain keep the pipe 66 % busy however many warps are resident, two
-// chains 79 %, four chains 92 % - with a single warp per sub-partition.  Occupancy does not help;
-// only runs of independent FP64 instructions inside one warp do.  The two endpoints of an interval
-// and the two drift signs of an evaluation are four such chains, so every step of the DAG is written
-// here as a "quad": the four first-stage instructions, then the four second-stage ones.  The
-// directed operations are volatile inline PTX so that the compiler keeps that order (it otherwise
-// serialises each endpoint chain to save registers: 4 dependent DFMA in a row, the other endpoint 60
-// instructions later).
+// Why this file exists (measured on B200, profiles/r01_pipe_probe.md and DESIGN.md section 6.1): a
+// sub-partition issues one FP64 warp instruction per 2 cycles, a dependent one 8 cycles after its
+// producer, and the dense kernel runs 4 warps per sub-partition (128 registers per thread), each of
+// which stalls on FP64 -> compare/select -> FP64 dependencies.  Four independent FP64 instructions in a
+// row from ONE warp keep the pipe busy through such a stall of the other warps.  The two endpoints of
+// an interval and the two drift signs of an evaluation are four independent chains, so every step of
+// the DAG is written here as a "quad": the four first-stage instructions, then the four second-stage
+// ones.  The directed operations are volatile inline PTX so that the compiler keeps that order (it
+// otherwise serialises each endpoint chain to save registers: 4 dependent DFMA in a row, the other
+// endpoint 60 instructions later).  Measured: C1 37.5 -> 32.4 ms.
 //
 // The arithmetic is that of ia_fast.cuh (fused forms, same DAG, same association order): only the
 // instruction order differs.

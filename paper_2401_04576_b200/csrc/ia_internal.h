@@ -79,6 +79,10 @@ cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* i
                                 int k, int levels, ia_box* boxes_out);
 // one level: children of boxes_out[e][lev-1][*] voted, top-k written to boxes_out[e][lev][*]
 cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& span, int lev, int levels, int k, ia_box* boxes_out);
+// sign-specialised vote of the 32k children of every event (ia_vote_dense.cu); returns where the partial
+// counts are and how many hit splits were used
+cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& span, int lev, int levels, int k, int n_sm,
+                                      ia_box* boxes, int* n_splits_out, uint16_t** partial_out);
 cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out);
 
 // FP64 pipe probe (roofline denominator check): blocks x 256 threads x 8 chains x iters instructions

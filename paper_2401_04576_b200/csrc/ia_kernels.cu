@@ -333,25 +333,34 @@ cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* i
 cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, ia_box* boxes_out) {
   int sm = 148;
   cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, ctx->device);
-  // split the hit range when there are too few events to fill the chip
-  int n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
-  if (n_splits > sp.max_hits) n_splits = sp.max_hits;
-  if (n_splits < 1) n_splits = 1;
-  const int per_split = (sp.max_hits + n_splits - 1) / n_splits;
-  n_splits = (sp.max_hits + per_split - 1) / per_split;
-  cudaError_t err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
-  if (err != cudaSuccess) return err;
-  uint16_t* partial = static_cast<uint16_t*>(ctx->partial.p);
   const int threads = k * 32;
-  dim3 grid(n_splits, sp.n_events, (threads + 255) / 256);
-  IA_DISPATCH_PREC(ctx,
-    (vote_children_kernel<double><<<grid, 256, per_split * sizeof(HitC<double>), ctx->stream>>>(
-        sp, static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),
-    (vote_children_kernel<float><<<grid, 256, per_split * sizeof(HitC<float>), ctx->stream>>>(
-        sp, static_cast<const HitC<float>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)));
-  ctx->launches++;
-  err = cudaGetLastError();
-  if (err != cudaSuccess) return err;
+  int n_splits = 1;
+  uint16_t* partial = nullptr;
+  cudaError_t err;
+  if (!(ctx->params.flags & 1u)) {
+    // sign-specialised form, a4 shared by the children of an xy sub-cell (ia_vote_dense.cu)
+    err = launch_vote_children_fast(ctx, sp, lev, levels, k, sm, boxes_out, &n_splits, &partial);
+    if (err != cudaSuccess) return err;
+  } else {
+    // general form (flags bit 0): split the hit range when there are too few events to fill the chip
+    n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
+    if (n_splits > sp.max_hits) n_splits = sp.max_hits;
+    if (n_splits < 1) n_splits = 1;
+    const int per_split = (sp.max_hits + n_splits - 1) / n_splits;
+    n_splits = (sp.max_hits + per_split - 1) / per_split;
+    err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
+    if (err != cudaSuccess) return err;
+    partial = static_cast<uint16_t*>(ctx->partial.p);
+    dim3 grid(n_splits, sp.n_events, (threads + 255) / 256);
+    IA_DISPATCH_PREC(ctx,
+      (vote_children_kernel<double><<<grid, 256, per_split * sizeof(HitC<double>), ctx->stream>>>(
+          sp, static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),
+      (vote_children_kernel<float><<<grid, 256, per_split * sizeof(HitC<float>), ctx->stream>>>(
+          sp, static_cast<const HitC<float>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)));
+    ctx->launches++;
+    err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+  }
   select_children_kernel<<<sp.n_events, threads, 0, ctx->stream>>>(partial, n_splits, lev, levels, k, boxes_out);
   ctx->launches++;
   return cudaGetLastError();

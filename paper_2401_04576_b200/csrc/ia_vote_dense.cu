@@ -257,6 +257,112 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   }
 }
 
+// ---- refinement children, sign-specialised form ------------------------------------------------------
+// One refinement pass votes the 32 children of each of the k kept boxes (a8-a9).  The 32 children of a
+// parent are 4 (xc, yc) sub-cells x 4 (R, lambda) pairs x 2 z0 halves: a4 is computed once per (parent,
+// xy sub-cell, hit) into shared memory (the general children kernel recomputes it in every child: 8 x),
+// a thread owns one (parent, xy sub-cell, pair) and votes its two z0 children with the one-body fast
+// form.  Block = (hit split, event), k*16 threads; the hit range is split so that the records of a split
+// fit CHILD_SMEM bytes and a single event still fills the chip; partial[e][split][rank*32 + c].
+// A warp holds two parents and four xy sub-cells, so the class of a hit is a per-lane value: the warp
+// takes the body of the class all its lanes share, else the universal one (valid for every class).
+constexpr int CHILD_SMEM = 48 * 1024;
+template <class T> struct ZTab2 { Iv<T> z[2][2]; };           // [negated][z half]
+
+__device__ __forceinline__ void child_half(double lo, double hi, int upper, double& clo, double& chi) {
+  const double mid = __dmul_rn(0.5, __dadd_rn(lo, hi));       // S9, G18: same midpoint as select_children_kernel
+  clo = upper ? mid : lo;
+  chi = upper ? hi : mid;
+}
+
+template <class T>
+__global__ void __launch_bounds__(512, 1)
+vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
+                          int levels, int k, int per_split, uint16_t* __restrict__ partial) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  ZTab2<T>* ztab = reinterpret_cast<ZTab2<T>*>(smem_raw);
+  HitF<T>* rec = reinterpret_cast<HitF<T>*>(smem_raw + size_t(k) * sizeof(ZTab2<T>));
+  const int e = blockIdx.y, split = blockIdx.x;
+  int count;
+  if (sp.offsets) {
+    count = sp.offsets[e + 1] - sp.offsets[e];
+    if (count > sp.max_hits) count = sp.max_hits;
+    if (count < 0) count = 0;
+  } else {
+    count = sp.n_hits_single;
+  }
+  const int h0 = split * per_split;
+  int nh = count - h0;
+  if (nh > per_split) nh = per_split;
+  if (nh < 0) nh = 0;
+  const ia_box* par = boxes + (int64_t(e) * levels + (lev - 1)) * k;
+  const HitC<T>* hits = staged + int64_t(e) * sp.max_hits + h0;
+  T zref = T(0);
+  if (count > 0) zref = staged[int64_t(e) * sp.max_hits].zref;
+  // a4 per (parent, xy sub-cell, hit)
+  for (int i = threadIdx.x; i < k * 4 * nh; i += blockDim.x) {
+    const int h = i % nh, rx = i / nh, xy = rx & 3, r = rx >> 2;
+    double xl, xh, yl, yh;
+    child_half(par[r].lo[0], par[r].hi[0], (xy >> 1) & 1, xl, xh);
+    child_half(par[r].lo[1], par[r].hi[1], xy & 1, yl, yh);
+    const T Rlo_min = Rnd<T>::from_dn(par[r].lo[2]);
+    const T Lmag = mx(fabs(Rnd<T>::from_dn(par[r].lo[4])), fabs(Rnd<T>::from_up(par[r].hi[4])));
+    const HitC<T> c = hits[h];
+    make_hitf(xy_invariants(box_iv<T>(xl, xh), box_iv<T>(yl, yh), c), hit_small(c), Rlo_min, Lmag, rec[rx * per_split + h]);
+  }
+  for (int i = threadIdx.x; i < k * 2; i += blockDim.x) {
+    double zl, zh;
+    child_half(par[i >> 1].lo[3], par[i >> 1].hi[3], i & 1, zl, zh);
+    const Iv<T> Zr = isub(box_iv<T>(zl, zh), thin(zref));
+    ztab[i >> 1].z[0][i & 1] = Zr;
+    ztab[i >> 1].z[1][i & 1] = ineg(Zr);
+  }
+  __syncthreads();
+  const bool live = int(threadIdx.x) < k * 16;
+  const int t = live ? threadIdx.x : k * 16 - 1;
+  const int r = t >> 4, xy = (t >> 2) & 3, rb = (t >> 1) & 1, lb = t & 1;
+  double rl, rh, ll, lh;
+  child_half(par[r].lo[2], par[r].hi[2], rb, rl, rh);
+  child_half(par[r].lo[4], par[r].hi[4], lb, ll, lh);
+  const Iv<T> R = box_iv<T>(rl, rh), Lraw = box_iv<T>(ll, lh);
+  const int lcls = cls_of(Lraw);
+  const bool warp_fast = __all_sync(0xffffffffu, lcls != CLS_M);
+  const bool a = lcls == CLS_N;                       // S_a for this lane: flip lambda, z0 - z_ref and T
+  const int va = a ? 1 : 0;
+  PairC<T> pr;
+  pr.L = a ? ineg(Lraw) : Lraw;
+  pr.R = R;
+  pr.Lm = to_mr(pr.L);
+  pr.LRm = to_mr(lcls != CLS_M ? mul_pp(pr.L, R) : imul(pr.L, R));
+  pr.L2 = lcls != CLS_M ? mul_pp(pr.L, pr.L) : isqr(pr.L);
+  unsigned v0 = 0, v1 = 0;
+  const HitF<T>* myrec = rec + (r * 4 + xy) * per_split;
+  for (int h = 0; h < nh; ++h) {
+    const HitF<T>& hf = myrec[h];
+    const int kind = hf.kind[va];
+    const bool need = kind >= HIT_FAST_P;
+    const Iv<T>* zt = ztab[r].z[hf.zflip];
+    if (kind == HIT_FORCED) { v0 += 1; v1 += 1; }
+    if (!warp_fast || __any_sync(0xffffffffu, kind == HIT_GENERAL)) {
+      if (need) {
+        v0 += general_votes_norm(hf, va, R, zt[0], pr.L) ? 1u : 0u;
+        v1 += general_votes_norm(hf, va, R, zt[1], pr.L) ? 1u : 0u;
+      }
+    } else {
+      const bool allP = __all_sync(0xffffffffu, kind == HIT_FAST_P || !need);
+      const bool allN = __all_sync(0xffffffffu, kind == HIT_FAST_N || !need);
+      // lanes that do not need the hit (forced, skipped) run along on their record and drop the result
+      const unsigned bits = fast_hit_rt<T>(hf, allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
+      if (need) { v0 += bits & 1u; v1 += (bits >> 1) & 1u; }
+    }
+  }
+  if (live) {
+    uint16_t* out = partial + (int64_t(e) * gridDim.x + split) * (k * 32) + r * 32 + ((xy << 3) | (rb << 2) | lb);
+    out[0] = uint16_t(v0);
+    out[2] = uint16_t(v1);
+  }
+}
+
 }  // namespace
 
 template <class T>
@@ -305,6 +411,41 @@ static cudaError_t launch_general(ia_ctx* ctx, const HitSpan& sp, const GridDesc
                                                                         chunks, votes_out);
   ctx->launches++;
   return cudaGetLastError();
+}
+
+template <class T>
+static cudaError_t launch_children_fast_t(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, int n_sm,
+                                          ia_box* boxes, int* n_splits_out, uint16_t** partial_out) {
+  int per_split = int(CHILD_SMEM / (size_t(k) * 4 * sizeof(HitF<T>)));
+  if (per_split < 1) per_split = 1;
+  // few events: split further so that about two blocks per SM exist
+  const int want = (2 * n_sm + sp.n_events - 1) / sp.n_events;
+  if (want > 1) {
+    const int ps = (sp.max_hits + want - 1) / want;
+    if (ps < per_split) per_split = ps < 1 ? 1 : ps;
+  }
+  if (per_split > sp.max_hits) per_split = sp.max_hits;
+  const int n_splits = (sp.max_hits + per_split - 1) / per_split;
+  cudaError_t err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
+  if (err != cudaSuccess) return err;
+  uint16_t* partial = static_cast<uint16_t*>(ctx->partial.p);
+  const size_t smem = size_t(k) * sizeof(ZTab2<T>) + size_t(k) * 4 * per_split * sizeof(HitF<T>);
+  err = cudaFuncSetAttribute(vote_children_fast_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+  if (err != cudaSuccess) return err;
+  const int threads = (k * 16 + 31) / 32 * 32;
+  dim3 grid(n_splits, sp.n_events);
+  vote_children_fast_kernel<T><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), boxes, lev,
+                                                                    levels, k, per_split, partial);
+  ctx->launches++;
+  *n_splits_out = n_splits;
+  *partial_out = partial;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, int n_sm, ia_box* boxes,
+                                      int* n_splits_out, uint16_t** partial_out) {
+  if (ctx->params.precision == 32) return launch_children_fast_t<float>(ctx, sp, lev, levels, k, n_sm, boxes, n_splits_out, partial_out);
+  return launch_children_fast_t<double>(ctx, sp, lev, levels, k, n_sm, boxes, n_splits_out, partial_out);
 }
 
 cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {

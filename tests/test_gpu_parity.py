@@ -274,6 +274,35 @@ def test_c3_refine_batch_identical(precision):
         rig.close()
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("grid,levels,k", [((8,) * 5, 6, 8), ((4, 4, 4, 4, 5), 5, 3), ((6, 5, 4, 3, 2), 4, 32),
+                                           ((3, 3, 3, 3, 3), 7, 1)])
+def test_children_fast_and_general_kernels_agree(precision, grid, levels, k):
+    """The sign-specialised children kernel against the general one (flags bit 0) and against the oracle:
+    K = 3 and 1 leave warps partly filled, an odd lambda grid makes parents whose children straddle 0,
+    K = 32 is the largest list."""
+    rig = Rig(g.chamber_c1(), precision=precision)
+    try:
+        evs = [g.make_event(rig.ch, 2000 + e, n_noise=6) for e in range(3)]
+        wire = np.concatenate([e.wire for e in evs])
+        drift = np.concatenate([e.drift for e in evs])
+        off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
+        hd, oh = rig.hits(wire, drift)
+        mh = max(e.n_hits for e in evs)
+        out = []
+        for flags in (0, 1):
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=flags)
+            boxes, par = rig.ctx.ia_refine_batch(hd, rig.dev(off), len(evs), mh, LO, HI, grid, levels, k)
+            rig.ctx.synchronize()
+            out.append((b.boxes_to_numpy(boxes, (len(evs), levels, k)), par.cpu().numpy().reshape(-1, 10)))
+        ob, opar = o.refine_batch(rig.owires, oh, off, rig.oparams, LO, HI, grid, levels, k)
+        _assert_boxes_equal(out[0][0], out[1][0])
+        _assert_boxes_equal(out[0][0], ob)
+        assert (out[0][1] == opar).all() and (out[1][1] == opar).all()
+    finally:
+        rig.close()
+
+
 def test_c1_dense_vote_sampled_and_top10(rig1):
     """configs[1]: 32^5 x 40 hits at full size; 30000 sampled cells + the GPU's top-10 cells against
     the oracle, and the top-10 selection itself bit-exact on the GPU's accumulator."""
