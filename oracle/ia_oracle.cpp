@@ -424,6 +424,135 @@ int refine_T(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, 
 }  // namespace
 
 // =============================================================================================
+// Paper-mode vote: the configuration the paper ran.
+//   M1  voxel = 4-D interval  xc x yc x R x z0  (L64); its mid-point m = 0.5*(lo+hi) per axis.
+//   M2  "The momentum of the particle is fixed to its true value" (L64): |p| enters as the length
+//       P = R sqrt(1 + lambda^2) (the radius a track of that momentum would have at lambda = 0), so
+//       |lambda| = sqrt((P/R_m)^2 - 1) at the voxel's mid radius; "The sign of lambda remains unknown
+//       ... This procedure is applied for each sign of the lambda value, so two 4D accumulators are
+//       used" (L64, L78): accumulator 0 takes +|lambda|, accumulator 1 takes -|lambda|.  A voxel
+//       with R_m > P has no lambda and gets no vote (reading M2 of DESIGN.md).
+//   M3  "the variables appearing in the expression of d_Ax, given in the equation (A.5b), are not
+//       considered as interval.  Their values are taken in the middle of the voxel" (L82):
+//       d_Ax = sqrt(radicand of (A.5b)) - R_m from steps S2-S8 evaluated at the point
+//       (xc_m, yc_m, R_m, z0_m, +-|lambda|) in plain round-to-nearest double arithmetic, same
+//       association order as the interval form.  A negative radicand or a NaN: that drift sign
+//       does not vote (no virtual circle exists).
+//   M4  tolerance (not in the paper, L88; BASELINE's +-tol): d_Ax is evaluated at d - tol (clamped
+//       at 0) and d + tol and the hull of the two values is used; tol = 0 is the paper's literal form.
+//   M5  condition (4) L74-76:  0 in (x_Ax - xc)^2 + (y_Ax - yc)^2 - (R + d_Ax)^2  in interval
+//       arithmetic (outward rounding), for the two drift signs; one count per hit (G7).
+// The property "false => the solution is not in the voxel" is lost in this mode, as L80-82 says.
+// =============================================================================================
+struct PointEval { bool ok; double rad, dax; };
+
+// S2-S8 at a point.  The caller holds FE_TONEAREST.  D is the signed drift distance.
+__attribute__((noinline)) PointEval dax_point(const HitC<double>& c, double xc, double yc, double R, double z0, double lam, double D) {
+  const double Tn = c.Tn;
+  // S2
+  const double A = c.xA - xc, B = c.yA - yc;
+  const double Q = A * A + B * B;
+  const double cA = A * c.sphi - B * c.cphi;
+  const double sA = A * c.cphi + B * c.sphi;
+  // S3
+  const double cr = (c.k0 + c.ky * xc) + c.kx * yc;
+  const double dx = xc - c.mx, dy = yc - c.my;
+  const double dt = (dx * dx + dy * dy) - c.h2;
+  const double dphi = std::atan2(cr, dt);
+  // S3'
+  const double iQ = 1.0 / Q, RA = std::sqrt(Q), iR = 1.0 / RA;
+  const double c2 = (cA * cA - sA * sA) * iQ;
+  const double s2 = (2.0 * (sA * cA)) * iQ;
+  // S4
+  const double Zr = z0 - c.zref;
+  const double LR = lam * R;
+  const double zA = Zr + LR * dphi;
+  const double LD = lam * D;
+  const double P1 = -((zA * sA + LD * cA) * iQ);
+  const double t1 = LR * zA;
+  const double t2 = ((lam * zA) * (R - 2.0 * D)) * c2;
+  const double t3 = (zA * zA + D * (RA + (lam * lam) * ((R + RA) - D))) * s2;
+  const double P2 = 0.5 * (((t1 - t2) + t3) * iQ);
+  const double T2 = Tn * Tn;
+  const double e = Tn * P1 + T2 * P2;
+  // S5
+  const double se = std::sin(e), ce = std::cos(e);
+  double sinP = (sA * ce + cA * se) * iR, cosP = (cA * ce - sA * se) * iR;
+  sinP = std::min(1.0, std::max(-1.0, sinP));
+  cosP = std::min(1.0, std::max(-1.0, cosP));
+  // S6
+  const double u2 = ((1.0 + (2.0 * Tn) * (lam * sinP)) + T2 * (lam * lam)) + T2 * (cosP * cosP);
+  const double u = std::sqrt(u2);
+  const double dl = D / u;
+  // S7
+  const double z = (Zr + LR * (dphi + e)) - Tn * (dl * cosP);
+  const double Ld = lam * dl;
+  const double ct = z * cA - Ld * sA;
+  // S8
+  const double Rd = R + dl, Tz = Tn * z, TLd = Tn * Ld;
+  const double rad = ((Rd * Rd - (2.0 * Tn) * ct) - Tz * Tz) - TLd * TLd;
+  if (!(rad >= 0.0)) return {false, rad, 0.0};
+  return {true, rad, std::sqrt(rad) - R};
+}
+
+struct PaperResid { double flo, fhi, scale; bool has; };   // has = false: no d_Ax for this sign -> no vote
+
+// M3-M4: hull of d_Ax at d - tol and d + tol, at the voxel's mid-point.  Switches to FE_TONEAREST for
+// its own duration; noinline and fenced so that no operation drifts across the mode switches.
+__attribute__((noinline)) bool paper_dax_hull(const double lo[4], const double hi[4], const HitC<double>& c, double lam,
+                                              int dsign, double* dax0, double* dax1) {
+  NearestInUp rn;
+  asm volatile("" ::: "memory");
+  double m[4];
+  for (int d = 0; d < 4; ++d) m[d] = opaque(0.5 * opaque(lo[d] + hi[d]));
+  const double dlo = std::max(opaque(c.d - c.tol), 0.0), dhi = opaque(c.d + c.tol);
+  const PointEval a = dax_point(c, m[0], m[1], m[2], m[3], lam, dsign > 0 ? dlo : -dlo);
+  const PointEval b = dax_point(c, m[0], m[1], m[2], m[3], lam, dsign > 0 ? dhi : -dhi);
+  bool ok = a.ok && b.ok;
+  *dax0 = opaque(std::min(a.dax, b.dax));
+  *dax1 = opaque(std::max(a.dax, b.dax));
+  asm volatile("" ::: "memory");
+  return ok;
+}
+
+// M3-M5 for one (voxel, hit, lambda sign, drift sign).  Mode must be FE_UPWARD.
+PaperResid paper_residual(const double lo[4], const double hi[4], const HitC<double>& c, double lam, int dsign) {
+  double dax0, dax1;
+  if (!paper_dax_hull(lo, hi, c, lam, dsign, &dax0, &dax1)) return {0.0, 0.0, 0.0, false};
+  const Iv<double> X = {lo[0], hi[0]}, Y = {lo[1], hi[1]}, R = {lo[2], hi[2]}, Dax = {dax0, dax1};
+  const Iv<double> Q = iadd(isqr(isub(thin(c.xA), X)), isqr(isub(thin(c.yA), Y)));
+  const Iv<double> S = isqr(iadd(R, Dax));
+  const Iv<double> f = isub(Q, S);
+  return {f.lo, f.hi, std::max(Q.hi, S.hi), true};
+}
+
+// |lambda| of the voxel from the fixed momentum (M2); false if R_m > P
+__attribute__((noinline)) bool paper_lambda(double Rlo, double Rhi, double P, double* lam) {
+  NearestInUp rn;
+  asm volatile("" ::: "memory");
+  const double Rm = opaque(0.5 * opaque(Rlo + Rhi));
+  const double q = opaque(P / Rm);
+  const double l2 = opaque(opaque(q * q) - 1.0);
+  const bool ok = l2 >= 0.0;
+  *lam = ok ? opaque(std::sqrt(l2)) : 0.0;
+  asm volatile("" ::: "memory");
+  return ok;
+}
+
+struct Grid4 {
+  std::vector<double> e[4];
+  int n[4];
+  Grid4(const double lo[4], const double hi[4], const int32_t dims[4]) {
+    for (int d = 0; d < 4; ++d) { n[d] = dims[d]; e[d] = edges(lo[d], hi[d], dims[d]); }
+  }
+  int64_t cells() const { int64_t c = 1; for (int d = 0; d < 4; ++d) c *= n[d]; return c; }
+  // linear index (((ix*ny+iy)*nR+iR)*nz+iz): z0 fastest
+  void cell(int64_t idx, double lo[4], double hi[4]) const {
+    for (int d = 3; d >= 0; --d) { int k = int(idx % n[d]); idx /= n[d]; lo[d] = e[d][k]; hi[d] = e[d][k + 1]; }
+  }
+};
+
+// =============================================================================================
 // C ABI (ctypes)
 // =============================================================================================
 extern "C" {
@@ -553,6 +682,98 @@ int orc_refine_batch(const OrcWire* wires, int n_wires, const OrcHit* hits, cons
                         levels, k, boxes_out + int64_t(e) * levels * k, params_out + int64_t(e) * 10);
     if (rc) return rc;
   }
+  return ORC_OK;
+}
+
+// ---- paper mode (f1) ------------------------------------------------------------------------------
+// point evaluation for the pins: out[0] = radicand of (A.5b), out[1] = d_Ax, returns 1 if no d_Ax exists
+int orc_dax_point(const OrcWire* wire, const OrcParams* p, const double pt[5], double D_signed, double* out) {
+  if (!wire || !p || !pt || !out) return ORC_ERR_ARG;
+  OrcHit h = {0, 0, std::fabs(D_signed)};
+  HitC<double> c = make_hitc<double>(*wire, h, *p);
+  UpMode up;
+  PointEval r;
+  {
+    NearestInUp rn;
+    asm volatile("" ::: "memory");
+    r = dax_point(c, pt[0], pt[1], pt[2], pt[3], pt[4], D_signed);
+    asm volatile("" ::: "memory");
+  }
+  out[0] = r.rad; out[1] = r.dax;
+  return r.ok ? 0 : 1;
+}
+
+// f enclosure of condition (4) for every (voxel, hit, lambda sign, drift sign):
+// out[(((i*n_hits + h)*2 + ls)*2 + ds)*4 + {0,1,2,3}] = f.lo, f.hi, scale, has (0: no d_Ax or no lambda -> no vote)
+int orc_residual_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
+                       const double* blo, const double* bhi, int64_t n_boxes, double* out) {
+  if (!wires || !hits || !p || !blo || !bhi || !out || n_hits < 0 || !(P > 0)) return ORC_ERR_ARG;
+  for (int i = 0; i < n_hits; ++i) if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+  std::vector<HitC<double>> hc = stage_hits<double>(wires, hits, n_hits, *p);
+  UpMode up;
+  for (int64_t i = 0; i < n_boxes; ++i) {
+    const double* lo = blo + 4 * i; const double* hi = bhi + 4 * i;
+    double lam = 0;
+    const bool has_l = paper_lambda(lo[2], hi[2], P, &lam);
+    for (int h = 0; h < n_hits; ++h)
+      for (int ls = 0; ls < 2; ++ls)
+        for (int ds = 0; ds < 2; ++ds) {
+          PaperResid r = {0, 0, 0, false};
+          if (has_l) r = paper_residual(lo, hi, hc[h], ls == 0 ? lam : -lam, ds == 0 ? +1 : -1);
+          double* o = out + ((((i * n_hits + h) * 2 + ls) * 2 + ds) * 4);
+          o[0] = r.flo; o[1] = r.fhi; o[2] = r.scale; o[3] = r.has ? 1.0 : 0.0;
+        }
+  }
+  return ORC_OK;
+}
+
+// dense 4-D grid, two accumulators: votes_out[ls*n + i], ls = 0 for lambda >= 0, 1 for lambda < 0;
+// cell_idx == NULL: all prod(dims) voxels in linear order (z0 fastest), else the listed voxels
+int orc_vote_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
+                   const double* lo, const double* hi, const int32_t* dims, const int64_t* cell_idx, int64_t n_idx,
+                   uint16_t* votes_out) {
+  if (!wires || !hits || !p || !lo || !hi || !dims || !votes_out || n_hits < 0 || !(P > 0)) return ORC_ERR_ARG;
+  for (int d = 0; d < 4; ++d) if (dims[d] <= 0 || !(hi[d] > lo[d])) return ORC_ERR_ARG;
+  if (!(lo[2] > 0)) return ORC_ERR_DOMAIN;
+  for (int i = 0; i < n_hits; ++i) {
+    if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+    if (!(hits[i].drift >= 0)) return ORC_ERR_ARG;
+  }
+  Grid4 g(lo, hi, dims);
+  const int64_t n = cell_idx ? n_idx : g.cells();
+  if (cell_idx) for (int64_t i = 0; i < n; ++i) if (cell_idx[i] < 0 || cell_idx[i] >= g.cells()) return ORC_ERR_ARG;
+  std::vector<HitC<double>> hc = stage_hits<double>(wires, hits, n_hits, *p);
+#pragma omp parallel
+  {
+    UpMode up;
+#pragma omp for schedule(dynamic, 256)
+    for (int64_t i = 0; i < n; ++i) {
+      double clo[4], chi[4];
+      g.cell(cell_idx ? cell_idx[i] : i, clo, chi);
+      double lam = 0;
+      const bool has_l = paper_lambda(clo[2], chi[2], P, &lam);
+      for (int ls = 0; ls < 2; ++ls) {
+        unsigned v = 0;
+        if (has_l)
+          for (const auto& c : hc) {
+            bool yes = false;
+            for (int ds = 0; ds < 2 && !yes; ++ds) {
+              const PaperResid r = paper_residual(clo, chi, c, ls == 0 ? lam : -lam, ds == 0 ? +1 : -1);
+              yes = r.has && !(r.flo > 0.0 || r.fhi < 0.0);
+            }
+            v += yes ? 1u : 0u;
+          }
+        votes_out[int64_t(ls) * n + i] = uint16_t(v);
+      }
+    }
+  }
+  return ORC_OK;
+}
+
+int orc_cell_boxes4(const double* lo, const double* hi, const int32_t* dims, const int64_t* cell_idx, int64_t n,
+                    double* blo, double* bhi) {
+  Grid4 g(lo, hi, dims);
+  for (int64_t i = 0; i < n; ++i) g.cell(cell_idx[i], blo + 4 * i, bhi + 4 * i);
   return ORC_OK;
 }
 

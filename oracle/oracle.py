@@ -29,7 +29,8 @@ def lib():
         path = _build.build()
         _lib = C.CDLL(path)
         for name in ("orc_prim", "orc_residual", "orc_vote_boxes", "orc_vote", "orc_cell_boxes", "orc_topk",
-                     "orc_refine", "orc_refine_batch", "orc_pad_ulps", "orc_max_threads"):
+                     "orc_refine", "orc_refine_batch", "orc_pad_ulps", "orc_max_threads", "orc_dax_point",
+                     "orc_residual_paper", "orc_vote_paper", "orc_cell_boxes4"):
             getattr(_lib, name).restype = C.c_int
         _lib.orc_set_threads.restype = None
     return _lib
@@ -157,3 +158,56 @@ def refine_batch(wires, hits, hit_offsets, params: Params, lo, hi, grid0, levels
     _chk(lib().orc_refine_batch(_p(wires), len(wires), _p(hits), _p(hit_offsets), n_ev, C.byref(params), _p(lo),
                                 _p(hi), _p(grid0), levels, k, _p(boxes), _p(par)), "refine_batch")
     return boxes, par
+
+
+# ---- paper mode (ia_oracle.cpp "Paper-mode vote") --------------------------------------------
+def dax_point(wire_row, params: Params, point, d_signed: float):
+    """(ok, radicand of (A.5b), d_Ax) of steps S2-S8 at the point (xc, yc, R, z0, lambda), plain double."""
+    w = np.zeros(1, WIRE_DT)
+    w[0] = wire_row
+    pt = np.ascontiguousarray(point, np.float64)
+    out = np.zeros(2)
+    rc = lib().orc_dax_point(_p(w), C.byref(params), _p(pt), C.c_double(d_signed), _p(out))
+    if rc < 0:
+        raise RuntimeError(f"oracle dax_point failed: rc={rc}")
+    return rc == 0, out[0], out[1]
+
+
+def residual_paper(wires, hits, params: Params, P: float, blo, bhi) -> np.ndarray:
+    """condition (4) enclosures [n_boxes, n_hits, 2 lambda signs (+,-), 2 drift signs (+,-), 4 = (f.lo, f.hi, scale, has)]."""
+    blo = np.ascontiguousarray(blo, np.float64).reshape(-1, 4)
+    bhi = np.ascontiguousarray(bhi, np.float64).reshape(-1, 4)
+    out = np.zeros((blo.shape[0], len(hits), 2, 2, 4))
+    _chk(lib().orc_residual_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P), _p(blo),
+                                  _p(bhi), C.c_int64(blo.shape[0]), _p(out)), "residual_paper")
+    return out
+
+
+def vote_paper(wires, hits, params: Params, P: float, lo, hi, dims, cell_idx=None) -> np.ndarray:
+    """two 4-D accumulators [2, n]: [0] for lambda >= 0, [1] for lambda < 0; voxel index z0 fastest."""
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    if cell_idx is None:
+        n = int(np.prod(dims.astype(np.int64)))
+        idx_p, n_idx = None, 0
+    else:
+        cell_idx = np.ascontiguousarray(cell_idx, np.int64)
+        n = len(cell_idx)
+        idx_p, n_idx = _p(cell_idx), n
+    out = np.zeros((2, n), np.uint16)
+    _chk(lib().orc_vote_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P), _p(lo), _p(hi),
+                              _p(dims), idx_p, C.c_int64(n_idx), _p(out)), "vote_paper")
+    return out
+
+
+def cell_boxes4(lo, hi, dims, cell_idx):
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    cell_idx = np.ascontiguousarray(cell_idx, np.int64)
+    blo = np.zeros((len(cell_idx), 4))
+    bhi = np.zeros((len(cell_idx), 4))
+    _chk(lib().orc_cell_boxes4(_p(lo), _p(hi), _p(dims), _p(cell_idx), C.c_int64(len(cell_idx)), _p(blo), _p(bhi)),
+         "cell_boxes4")
+    return blo, bhi
