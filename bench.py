@@ -380,6 +380,37 @@ def main():
                                 **eps}
         ctx3.close()
 
+        # ---- paper mode: the paper's own configuration on a Table-1-shaped grid ------------
+        # 50 x 50 x 40 x 20 voxels (iteration 1) x the C1 event's 40 hits; one evaluation =
+        # one (voxel, hit) decision = 2 lambda signs x 2 drift signs x 2 tolerance ends of the mid-voxel d_Ax
+        try:
+            ch1 = g.chamber_c1()
+            ev1 = g.make_event(ch1, 1, n_noise=20)
+            ctxp = b.Context(local_rank)
+            ctxp.ia_load_geometry(b.wires_of(ch1))
+            ctxp.ia_set_params(g.TOL)
+            hdp = ctxp.to_device(b.hits_of(ev1.wire, ev1.drift))
+            xc, yc, R, z0, lam = ev1.track.params
+            P = R * (1.0 + lam * lam) ** 0.5
+            pdims = (50, 50, 40, 20)
+            nvox = int(np.prod(pdims))
+            vp = ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims)
+            torch.cuda.synchronize()
+            a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(ctxp.stream)
+            for _ in range(5):
+                ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims, votes_out=vp.view(-1))
+            c.record(ctxp.stream)
+            c.synchronize()
+            ms = a.elapsed_time(c) / 5
+            line["paper_mode"] = {"workload": "f1: 4-D 50x50x40x20 voxels (Table 1 iteration-1 shape) x 40 hits (C1 event), "
+                                              "momentum fixed, 2 lambda-sign accumulators, mid-voxel d_Ax, tol 0.045",
+                                  "ms": ms, "voxel_hit_evals_per_s": nvox * ev1.n_hits / (ms * 1e-3),
+                                  "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
+            ctxp.close()
+        except Exception as exc:  # pragma: no cover
+            line["paper_mode"] = {"error": str(exc)}
+
     print(json.dumps(line))
     ctx.close()
     if world > 1:

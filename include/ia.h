@@ -113,6 +113,21 @@ int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo
 int ia_vote_boxes(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
                   int64_t n_boxes, uint16_t* votes_out_dev);
 
+/* f1 - the paper's own configuration of the vote (readings M1-M5 of DESIGN.md):
+ * 4-D voxels xc x yc x R x z0 (L64), the momentum fixed to its true value - given as the length
+ * momentum_radius = R sqrt(1 + lambda^2) (cm), so that |lambda| = sqrt((P/R_m)^2 - 1) at a voxel's mid
+ * radius - and one accumulator per sign of lambda (L78).  d_Ax of (A.5b) is a NUMBER evaluated at the
+ * voxel's mid-point in round-to-nearest double arithmetic (L82); only condition (4), L74-76,
+ * 0 in (x_Ax - xc)^2 + (y_Ax - yc)^2 - (R + d_Ax)^2, is evaluated in intervals, for both drift signs,
+ * one count per hit.  With tol > 0, d_Ax is the hull of its values at d - tol and d + tol; tol = 0 is
+ * the paper's literal form.  Voxels whose mid radius exceeds momentum_radius have no lambda and get 0.
+ * The guarantee "no vote => no solution in the voxel" does not hold in this mode (L80-82).
+ * votes_out_dev[s*N + (((ix*ny+iy)*nR+iR)*nz+iz)], N = prod(grid_dims), s = 0: lambda >= 0, 1: lambda < 0
+ * (2*N uint16, z0 fastest).  Always double precision (params.precision is not consulted).
+ * Errors: IA_ERR_ARG (null, sizes, momentum_radius <= 0), IA_ERR_DOMAIN (box_lo[2] <= 0). */
+int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const double box_lo[4],
+                  const double box_hi[4], const int32_t grid_dims[4], uint16_t* votes_out_dev);
+
 /* a7 - the k largest entries by key (votes descending, index ascending) (L94, G16):
  * idx_out_dev[k] (int64 linear indices), votes_out_dev[k].  1 <= k <= min(n_cells, IA_MAX_K). */
 int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t* idx_out_dev,

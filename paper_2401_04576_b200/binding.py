@@ -23,7 +23,7 @@ HIT_DT = np.dtype([("wire", "i4"), ("_pad", "i4"), ("drift", "f8")])
 BOX_DT = np.dtype([("lo", "f8", (5,)), ("hi", "f8", (5,)), ("votes", "u2"), ("_pad", "u2", (3,))])
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88
 
-EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_topk",
+EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
@@ -59,6 +59,7 @@ def load_library(path: str = LIB_PATH):
     lib.ia_set_params.argtypes = [vp, C.POINTER(IaParams)]
     lib.ia_vote.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_vote_boxes.argtypes = [vp, vp, i32, vp, vp, i64, vp]
+    lib.ia_vote_paper.argtypes = [vp, vp, i32, dbl, vp, vp, vp, vp]
     lib.ia_topk.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.ia_refine.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_refine_batch.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, i32, i32, vp, vp]
@@ -184,6 +185,19 @@ class Context:
             votes_out = self._empty(n, torch.uint16)
         self._chk(self.lib.ia_vote(self.h, _dp(hits_dev), n_hits, _hp(lo), _hp(hi), _hp(dims), _dp(votes_out)), "ia_vote")
         return votes_out
+
+    # ---- f1: the paper's own configuration (4-D voxels, mid-voxel d_Ax, two lambda-sign accumulators)
+    def ia_vote_paper(self, hits_dev, n_hits, momentum_radius, box_lo, box_hi, grid_dims, votes_out=None):
+        torch = self._torch
+        lo = np.ascontiguousarray(box_lo, np.float64).reshape(4)
+        hi = np.ascontiguousarray(box_hi, np.float64).reshape(4)
+        dims = np.ascontiguousarray(grid_dims, np.int32).reshape(4)
+        n = int(np.prod(dims.astype(np.int64)))
+        if votes_out is None:
+            votes_out = self._empty(2 * n, torch.uint16)
+        self._chk(self.lib.ia_vote_paper(self.h, _dp(hits_dev), n_hits, float(momentum_radius), _hp(lo), _hp(hi), _hp(dims),
+                                         _dp(votes_out)), "ia_vote_paper")
+        return votes_out.view(2, n)
 
     def ia_vote_boxes(self, hits_dev, n_hits, lo_dev, hi_dev, votes_out=None):
         torch = self._torch

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libia_b200.so")
-SOURCES = ["ia_api.cu", "ia_kernels.cu", "ia_topk.cu", "ia_vote_dense.cu"]
+SOURCES = ["ia_api.cu", "ia_kernels.cu", "ia_topk.cu", "ia_vote_dense.cu", "ia_vote_paper.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=false",
          "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-Xptxas", "-v"]

@@ -219,6 +219,27 @@ int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo
   return IA_OK;
 }
 
+int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const double box_lo[4],
+                  const double box_hi[4], const int32_t grid_dims[4], uint16_t* votes_out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits < 0 || (n_hits > 0 && !hits_dev) || !votes_out_dev || !box_lo || !box_hi || !grid_dims) return IA_ERR_ARG;
+  if (!(momentum_radius > 0.0) || !std::isfinite(momentum_radius)) return IA_ERR_ARG;
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  const double lo5[5] = {box_lo[0], box_lo[1], box_lo[2], box_lo[3], 0.0};
+  const double hi5[5] = {box_hi[0], box_hi[1], box_hi[2], box_hi[3], 1.0};
+  const int32_t n5[5] = {grid_dims[0], grid_dims[1], grid_dims[2], grid_dims[3], 1};
+  GridDesc g;
+  rc = make_grid(lo5, hi5, n5, g);
+  if (rc) return rc;
+  if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
+  if (int64_t(grid_dims[0]) * grid_dims[1] > 0x7fffffffLL || int64_t(grid_dims[2]) * grid_dims[3] > 0x7fffffffLL)
+    return IA_ERR_CAPACITY;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, momentum_radius, g, votes_out_dev));
+  return IA_OK;
+}
+
 int ia_vote_boxes(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
                   int64_t n_boxes, uint16_t* votes_out_dev) {
   int rc = check_ready(ctx);

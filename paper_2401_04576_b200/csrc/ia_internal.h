@@ -85,6 +85,9 @@ cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& span, int lev,
                                       ia_box* boxes, int* n_splits_out, uint16_t** partial_out);
 cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out);
 
+// paper-mode vote (ia_vote_paper.cu): 4-D grid in g (axis 4 unused, n = 1), votes_out [2][cells]
+cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const GridDesc& g, uint16_t* votes_out);
+
 // FP64 pipe probe (roofline denominator check): blocks x 256 threads x 8 chains x iters instructions
 cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, double* sink);
 

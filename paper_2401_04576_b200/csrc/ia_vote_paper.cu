@@ -1,0 +1,195 @@
+// ia_vote_paper.cu - the paper's own vote configuration.
+//
+//   M1  voxel = 4-D interval xc x yc x R x z0 (L64); mid-point m = 0.5*(lo+hi) per axis.
+//   M2  momentum fixed to its true value (L64), given as P = R sqrt(1 + lambda^2): |lambda| =
+//       sqrt((P/R_m)^2 - 1); two accumulators for the two signs of lambda (L78); R_m > P: no vote.
+//   M3  d_Ax of (A.5b) is a NUMBER: steps S2-S8 at the voxel's mid-point in round-to-nearest double
+//       arithmetic (L82: "Their values are taken in the middle of the voxel").  Negative radicand or
+//       NaN: that drift sign does not vote.
+//   M4  tolerance: hull of d_Ax at d - tol (clamped at 0) and d + tol; tol = 0 is the paper's form.
+//   M5  condition (4) L74-76 in interval arithmetic: 0 in (x_Ax-xc)^2 + (y_Ax-yc)^2 - (R + d_Ax)^2,
+//       either drift sign, one count per hit.
+// The point arithmetic keeps the association order of the interval form and is
+// never contracted into FMAs (explicit __dmul_rn/__dadd_rn), so it differs from a plain host evaluation
+// only through sin, cos and atan2.
+//
+// Block = one (xc, yc) cell: its threads compute once per hit what depends on (xc_m, yc_m, hit) only
+// (the point values of S2, S3, S3' and the interval (x_Ax-xc)^2 + (y_Ax-yc)^2) into shared memory, then
+// every thread walks (R, z0) voxels of the column, keeps the two vote counts in registers and stores
+// two uint16 per voxel.  No atomics.
+#include "ia_internal.h"
+#include "ia_fast.cuh"
+
+namespace ia {
+namespace {
+
+struct PHit {
+  double Qlo, Qhi;                            // interval (x_Ax - X)^2 + (y_Ax - Y)^2
+  double cA, sA, dphi, iQ, RA, iR, c2, s2;    // point values at (xc_m, yc_m)
+  double Tn, T2, twoT, dlo, dhi, zref;
+  int valid, _pad;
+};
+
+IA_DEV double mul(double a, double b) { return __dmul_rn(a, b); }
+IA_DEV double add(double a, double b) { return __dadd_rn(a, b); }
+IA_DEV double sub(double a, double b) { return __dadd_rn(a, -b); }
+
+// per-hit scalars (round to nearest, unfused: the same operations as stage_hits_kernel) and the
+// (xc_m, yc_m)-dependent point values of S2, S3, S3'
+__device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit h, const ia_params& p, Iv<double> X,
+                          Iv<double> Y, int* status, PHit& o) {
+  int w = h.wire;
+  o.valid = (w >= 0 && w < n_wires && h.drift >= 0.0);
+  if (!o.valid) {
+    if (status) atomicOr(status, 1);
+    w = 0;
+    h.drift = 0.0;
+  }
+  const double x0 = wires[w], y0 = wires[n_wires + w], s = wires[2 * n_wires + w], co = wires[3 * n_wires + w];
+  const double t = wires[4 * n_wires + w];
+  const double xr = p.x_ref, yr = p.y_ref, zr = p.z_ref;
+  const double xA = add(x0, mul(mul(zr, s), t));                       // (A.4d)
+  const double yA = sub(y0, mul(mul(zr, co), t));                      // (A.4e)
+  const double k0 = sub(mul(xr, yA), mul(yr, xA)), ky = sub(yr, yA), kx = sub(xA, xr);
+  const double mx_ = mul(0.5, add(xr, xA)), my_ = mul(0.5, add(yr, yA));
+  const double hx = mul(0.5, sub(xA, xr)), hy = mul(0.5, sub(yA, yr));
+  const double h2 = add(mul(hx, hx), mul(hy, hy));
+  o.Tn = t; o.T2 = mul(t, t); o.twoT = mul(2.0, t); o.zref = zr;
+  o.dlo = fmax(sub(h.drift, p.tol), 0.0);                              // M4
+  o.dhi = add(h.drift, p.tol);
+  // M5, xy part: every variable occurs once
+  const Iv<double> Q = iadd(isqr(isub(thin(xA), X)), isqr(isub(thin(yA), Y)));
+  o.Qlo = Q.lo; o.Qhi = Q.hi;
+  // S2, S3, S3' at the mid-point
+  const double xc = mul(0.5, add(X.lo, X.hi)), yc = mul(0.5, add(Y.lo, Y.hi));
+  const double A = sub(xA, xc), B = sub(yA, yc);
+  const double Qp = add(mul(A, A), mul(B, B));
+  o.cA = sub(mul(A, s), mul(B, co));
+  o.sA = add(mul(A, co), mul(B, s));
+  const double cr = add(add(k0, mul(ky, xc)), mul(kx, yc));
+  const double dx = sub(xc, mx_), dy = sub(yc, my_);
+  const double dt = sub(add(mul(dx, dx), mul(dy, dy)), h2);
+  o.dphi = atan2(cr, dt);
+  o.iQ = __ddiv_rn(1.0, Qp);
+  o.RA = __dsqrt_rn(Qp);
+  o.iR = __ddiv_rn(1.0, o.RA);
+  o.c2 = mul(sub(mul(o.cA, o.cA), mul(o.sA, o.sA)), o.iQ);
+  o.s2 = mul(mul(2.0, mul(o.sA, o.cA)), o.iQ);
+}
+
+// sin and cos of e = Phi - Phi_Ax: Taylor forms of ia_fast.cuh inside [-1/4, 1/4] (error below 1 ulp),
+// the library functions outside
+IA_DEV void sincos_e(double e, double& se, double& ce) {
+  if (fabs(e) < 0.25) {
+    const double s = mul(e, e);
+    se = Trig<double>::sin_small(e, s);
+    ce = Trig<double>::cos_small(s);
+  } else {
+    se = sin(e);
+    ce = cos(e);
+  }
+}
+
+// S4-S8 at a point; D is the signed drift distance.  false: no d_Ax (M3)
+IA_DEV bool dax_point(const PHit& h, double R, double Zr, double lam, double D, double& dax) {
+  const double LR = mul(lam, R);
+  const double zA = add(Zr, mul(LR, h.dphi));
+  const double LD = mul(lam, D);
+  const double P1 = -mul(add(mul(zA, h.sA), mul(LD, h.cA)), h.iQ);
+  const double t1 = mul(LR, zA);
+  const double t2 = mul(mul(mul(lam, zA), sub(R, mul(2.0, D))), h.c2);
+  const double t3 = mul(add(mul(zA, zA), mul(D, add(h.RA, mul(mul(lam, lam), sub(add(R, h.RA), D))))), h.s2);
+  const double P2 = mul(0.5, mul(add(sub(t1, t2), t3), h.iQ));
+  const double e = add(mul(h.Tn, P1), mul(h.T2, P2));
+  double se, ce;
+  sincos_e(e, se, ce);
+  double sinP = mul(add(mul(h.sA, ce), mul(h.cA, se)), h.iR);
+  double cosP = mul(sub(mul(h.cA, ce), mul(h.sA, se)), h.iR);
+  sinP = fmin(1.0, fmax(-1.0, sinP));
+  cosP = fmin(1.0, fmax(-1.0, cosP));
+  const double u2 = add(add(add(1.0, mul(h.twoT, mul(lam, sinP))), mul(h.T2, mul(lam, lam))), mul(h.T2, mul(cosP, cosP)));
+  const double u = __dsqrt_rn(u2);
+  const double dl = __ddiv_rn(D, u);
+  const double z = sub(add(Zr, mul(LR, add(h.dphi, e))), mul(h.Tn, mul(dl, cosP)));
+  const double Ld = mul(lam, dl);
+  const double ct = sub(mul(z, h.cA), mul(Ld, h.sA));
+  const double Rd = add(R, dl), Tz = mul(h.Tn, z), TLd = mul(h.Tn, Ld);
+  const double rad = sub(sub(sub(mul(Rd, Rd), mul(h.twoT, ct)), mul(Tz, Tz)), mul(TLd, TLd));
+  if (!(rad >= 0.0)) return false;
+  dax = sub(__dsqrt_rn(rad), R);
+  return true;
+}
+
+constexpr int PAPER_THREADS = 256;
+
+__global__ void __launch_bounds__(PAPER_THREADS)
+vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const double* __restrict__ wires, int n_wires, ia_params p,
+                  double P, GridDesc g, int* status, uint16_t* __restrict__ votes) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  PHit* sh = reinterpret_cast<PHit*>(smem_raw);
+  const int ixy = blockIdx.x;
+  const int ix = ixy / g.n[1], iy = ixy - ix * g.n[1];
+  const Iv<double> X = {cell_edge(g.lo[0], g.hi[0], g.w[0], ix, g.n[0]), cell_edge(g.lo[0], g.hi[0], g.w[0], ix + 1, g.n[0])};
+  const Iv<double> Y = {cell_edge(g.lo[1], g.hi[1], g.w[1], iy, g.n[1]), cell_edge(g.lo[1], g.hi[1], g.w[1], iy + 1, g.n[1])};
+  for (int h = threadIdx.x; h < n_hits; h += blockDim.x) make_phit(wires, n_wires, hits[h], p, X, Y, status, sh[h]);
+  __syncthreads();
+  const int nR = g.n[2], nz = g.n[3];
+  const int64_t n_cells = g.cells;                       // nx*ny*nR*nz
+  const bool two_ends = p.tol > 0.0;
+  for (int j = threadIdx.x; j < nR * nz; j += blockDim.x) {
+    const int iR = j / nz, iz = j - iR * nz;
+    const Iv<double> R = {cell_edge(g.lo[2], g.hi[2], g.w[2], iR, nR), cell_edge(g.lo[2], g.hi[2], g.w[2], iR + 1, nR)};
+    const double zlo = cell_edge(g.lo[3], g.hi[3], g.w[3], iz, nz), zhi = cell_edge(g.lo[3], g.hi[3], g.w[3], iz + 1, nz);
+    const double Rm = mul(0.5, add(R.lo, R.hi)), zm = mul(0.5, add(zlo, zhi));
+    // M2
+    const double q = __ddiv_rn(P, Rm);
+    const double l2 = sub(mul(q, q), 1.0);
+    const bool has_l = l2 >= 0.0;
+    const double lam = has_l ? __dsqrt_rn(l2) : 0.0;
+    unsigned v[2] = {0u, 0u};
+    if (has_l) {
+      for (int h = 0; h < n_hits; ++h) {
+        const PHit& ph = sh[h];
+        if (!ph.valid) continue;
+        const double Zr = sub(zm, ph.zref);
+#pragma unroll
+        for (int ls = 0; ls < 2; ++ls) {
+          const double l = ls == 0 ? lam : -lam;
+          bool yes = false;
+#pragma unroll
+          for (int ds = 0; ds < 2; ++ds) {
+            double a = 0.0, b;
+            bool ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dlo : -ph.dlo, a);
+            b = a;
+            if (two_ends) ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dhi : -ph.dhi, b) && ok;
+            const Iv<double> Dax = {fmin(a, b), fmax(a, b)};
+            const Iv<double> S = isqr(iadd(R, Dax));
+            const Iv<double> f = isub(Iv<double>{ph.Qlo, ph.Qhi}, S);
+            yes = yes || (ok && !(f.lo > 0.0 || f.hi < 0.0));
+          }
+          v[ls] += yes ? 1u : 0u;
+        }
+      }
+    }
+    const int64_t cell = int64_t(ixy) * (nR * nz) + j;
+    votes[cell] = uint16_t(v[0]);
+    votes[n_cells + cell] = uint16_t(v[1]);
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const GridDesc& g, uint16_t* votes_out) {
+  const size_t smem = size_t(n_hits) * sizeof(PHit);
+  cudaError_t err = cudaFuncSetAttribute(vote_paper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+  if (err != cudaSuccess) return err;
+  const int col = g.n[2] * g.n[3];
+  int threads = PAPER_THREADS;
+  if (col < threads) threads = (col + 31) / 32 * 32;
+  vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, ctx->wires, ctx->n_wires, ctx->params,
+                                                                              P, g, ctx->status, votes_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+}  // namespace ia
