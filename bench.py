@@ -145,6 +145,41 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line))
 
 
+def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
+    """SURVEY 8(f) f1 on 50 x 50 x 40 x 20 voxels (iteration 1) x the C1 event's 40 hits; one
+    evaluation = one (voxel, hit) decision = 2 lambda signs x 2 drift signs x 2 tolerance ends of the mid-voxel d_Ax."""
+    import torch
+    from paper_2401_04576_b200 import binding as b
+    ch1 = g.chamber_c1()
+    ev1 = g.make_event(ch1, 1, n_noise=20)
+    ctxp = b.Context(local_rank)
+    ctxp.ia_load_geometry(b.wires_of(ch1))
+    ctxp.ia_set_params(g.TOL)
+    hdp = ctxp.to_device(b.hits_of(ev1.wire, ev1.drift))
+    xc, yc, R, z0, lam = ev1.track.params
+    P = R * (1.0 + lam * lam) ** 0.5
+    pdims = (50, 50, 40, 20)
+    nvox = int(np.prod(pdims))
+    vp = ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims)
+    for _ in range(warmup):
+        ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims, votes_out=vp.view(-1))
+    torch.cuda.synchronize()
+    a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(ctxp.stream)
+    for _ in range(steps):
+        ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims, votes_out=vp.view(-1))
+    c.record(ctxp.stream)
+    c.synchronize()
+    ms = a.elapsed_time(c) / steps
+    launches = ctxp.ia_launch_count()
+    ctxp.close()
+    return {"workload": "f1: 4-D 50x50x40x20 voxels (Table 1 iteration-1 shape) x 40 hits (C1 event), "
+                        "momentum fixed, 2 lambda-sign accumulators, mid-voxel d_Ax, tol 0.045",
+            "ms": ms, "voxel_hit_evals_per_s": nvox * ev1.n_hits / (ms * 1e-3), "evals_per_step": nvox * ev1.n_hits,
+            "gpu_launches": int(launches),
+            "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
+
+
 def run_c3(args, rank, world, local_rank, barrier):
     """--workload C3: one step = ia_refine_batch over 1024 events (BASELINE.json configs[3]); for profiling the
     batch path on its own.  Same JSON shape; value = cell-hit evaluations/s, events/s beside it."""
@@ -152,24 +187,28 @@ def run_c3(args, rank, world, local_rank, barrier):
     import torch.distributed as dist
     from paper_2401_04576_b200 import binding as b
     ch = g.chamber_c1()
-    n_ev, levels, k = 1024, 8, 8
-    evs = [g.make_event(ch, 1000 + rank * n_ev + e, n_noise=10) for e in range(n_ev)]
+    if args.workload == "C2":      # configs[2]: one event, 1 track + 20 noise, K=16, 10 passes (latency-bound)
+        n_ev, levels, k, mh = 1, 10, 16, 40
+        evs = [g.make_event(ch, 2 + rank, n_noise=20)]
+    else:                          # configs[3]
+        n_ev, levels, k, mh = 1024, 8, 8, 30
+        evs = [g.make_event(ch, 1000 + rank * n_ev + e, n_noise=10) for e in range(n_ev)]
     h3 = b.hits_of(np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs]))
     off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
     ctx = b.Context(local_rank)
     ctx.ia_load_geometry(b.wires_of(ch))
     ctx.ia_set_params(g.TOL, precision=args.precision)
     hd, od = ctx.to_device(h3), ctx.to_device(off)
-    boxes, par = ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k)
+    boxes, par = ctx.ia_refine_batch(hd, od, n_ev, mh, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k)
     for _ in range(max(0, args.warmup - 1)):
-        ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
+        ctx.ia_refine_batch(hd, od, n_ev, mh, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = ctx.ia_launch_count()
     a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(ctx.stream)
     for _ in range(args.steps):
-        ctx.ia_refine_batch(hd, od, n_ev, 30, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
+        ctx.ia_refine_batch(hd, od, n_ev, mh, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
     c.record(ctx.stream)
     barrier()
     launches = ctx.ia_launch_count() - l0
@@ -180,13 +219,28 @@ def run_c3(args, rank, world, local_rank, barrier):
     ms_step = float(t.item()) / args.steps
     if rank != 0:
         return
-    evals = n_ev * (8 ** 5 + (levels - 1) * k * 32) * 30
+    evals = n_ev * (8 ** 5 + (levels - 1) * k * 32) * mh
+    # cpu_baseline: the oracle's refine on a bounded sample of the same events
+    from oracle import oracle as o
+    n_s = min(n_ev, 16)
+    off_s = off[:n_s + 1]
+    oh = o.hits_of(h3["wire"][:off_s[-1]], h3["drift"][:off_s[-1]])
+    t0 = time.perf_counter()
+    ob, opar = o.refine_batch(o.wires_of(ch), oh, off_s, o.make_params(g.TOL, precision=args.precision), g.BOX_LO, g.BOX_HI,
+                              (8,) * 5, levels, k)
+    dt_o = time.perf_counter() - t0
+    gb = b.boxes_to_numpy(boxes, (n_ev, levels, k))[:n_s]
+    same = bool((gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all())
     line = {"metric": METRIC, "value": evals * world / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": f"f{args.precision}", "data": "synthetic",
-            "config": {"workload": "C3: BASELINE.json configs[3], 1024 events x 30 hits, 8^5 start, K=8, 8 passes; seeds 1000+e",
-                       "evals_per_step": evals, "l2": "67 MB of vote scratch rewritten every step"},
-            "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks}
+            "config": {"workload": f"{args.workload}: BASELINE.json configs[{args.workload[1]}], {n_ev} event(s) x {mh} hits, "
+                                   f"8^5 start, K={k}, {levels} passes",
+                       "evals_per_step": evals, "l2": "vote scratch (64 KB per event) rewritten every step"},
+            "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks,
+            "cpu_baseline": {"value": n_s * evals / n_ev / dt_o, "unit": UNIT, "cores": o.max_threads(), "kind": "oracle",
+                             "sample": f"orc_refine_batch on the first {n_s} event(s) ({dt_o:.2f} s)",
+                             "events_per_s": n_s / dt_o, "boxes_identical": same}}
     print(json.dumps(line))
     ctx.close()
 
@@ -197,7 +251,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C3"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
@@ -225,7 +279,20 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.workload == "C3":
+    if args.workload == "F1":
+        # paper mode alone (for profiling): same JSON shape, value = voxel-hit evaluations/s
+        barrier()
+        r = paper_mode_leg(local_rank, steps=args.steps, warmup=args.warmup)
+        if rank == 0:
+            print(json.dumps({"metric": "voxel-hit paper-mode evals/s", "value": r["voxel_hit_evals_per_s"] * world,
+                              "unit": "evals/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                              "ms_per_step": r["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                              "dtype": "f64", "data": "synthetic", "config": {"workload": r["workload"]},
+                              "gpu_launches": r["gpu_launches"]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    if args.workload in ("C2", "C3"):
         run_c3(args, rank, world, local_rank, barrier)
         if world > 1:
             dist.destroy_process_group()
@@ -381,33 +448,8 @@ def main():
         ctx3.close()
 
         # ---- paper mode: the paper's own configuration on a Table-1-shaped grid ------------
-        # 50 x 50 x 40 x 20 voxels (iteration 1) x the C1 event's 40 hits; one evaluation =
-        # one (voxel, hit) decision = 2 lambda signs x 2 drift signs x 2 tolerance ends of the mid-voxel d_Ax
         try:
-            ch1 = g.chamber_c1()
-            ev1 = g.make_event(ch1, 1, n_noise=20)
-            ctxp = b.Context(local_rank)
-            ctxp.ia_load_geometry(b.wires_of(ch1))
-            ctxp.ia_set_params(g.TOL)
-            hdp = ctxp.to_device(b.hits_of(ev1.wire, ev1.drift))
-            xc, yc, R, z0, lam = ev1.track.params
-            P = R * (1.0 + lam * lam) ** 0.5
-            pdims = (50, 50, 40, 20)
-            nvox = int(np.prod(pdims))
-            vp = ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims)
-            torch.cuda.synchronize()
-            a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(ctxp.stream)
-            for _ in range(5):
-                ctxp.ia_vote_paper(hdp, ev1.n_hits, P, g.BOX_LO[:4], g.BOX_HI[:4], pdims, votes_out=vp.view(-1))
-            c.record(ctxp.stream)
-            c.synchronize()
-            ms = a.elapsed_time(c) / 5
-            line["paper_mode"] = {"workload": "f1: 4-D 50x50x40x20 voxels (Table 1 iteration-1 shape) x 40 hits (C1 event), "
-                                              "momentum fixed, 2 lambda-sign accumulators, mid-voxel d_Ax, tol 0.045",
-                                  "ms": ms, "voxel_hit_evals_per_s": nvox * ev1.n_hits / (ms * 1e-3),
-                                  "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
-            ctxp.close()
+            line["paper_mode"] = paper_mode_leg(local_rank, steps=5)
         except Exception as exc:  # pragma: no cover
             line["paper_mode"] = {"error": str(exc)}
 
