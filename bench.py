@@ -364,7 +364,9 @@ def main():
     achieved_inst = ALG_FP64_INST_PER_EVAL * evals_per_step / (vote_ms * 1e-3)
     roofline = {
         "bound": "alu", "kernel": "vote_dense", "achieved": achieved_inst / 1e12, "peak": peak_inst / 1e12,
-        "unit": "T FP64 inst/s", "frac": achieved_inst / peak_inst, "traffic": None,
+        "unit": "T FP64 inst/s", "frac": achieved_inst / peak_inst,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from profiles/r01_traffic_c4.md (C4 only)
+        "traffic": 2361204736 if args.workload == "C4" else None,
         "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 lanes x {f_max_mhz:.0f} MHz (DESIGN.md 6); "
                        "MEASURED_PEAKS.json has no FP64 entry",
         "alg_fp64_inst_per_eval": ALG_FP64_INST_PER_EVAL, "kernel_ms": vote_ms,

@@ -168,7 +168,7 @@ IA_DEV unsigned long long spread8(unsigned bits) {
 // argument of three bodies (fine grids: 6 % faster there).  Same arithmetic, same results.
 template <class T, bool RT>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
-vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z,
+vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z, int zt,
                        uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ZTab<T>* ztab = reinterpret_cast<ZTab<T>*>(smem_raw);
@@ -198,8 +198,8 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     const HitC<T> c = staged[int64_t(e) * sp.max_hits + h];
     make_hitf(xy_invariants(X, Y, c), hit_small(c), Rlo_min, Lmag, sh[h]);
   }
-  const int iz0 = tz * FAST_ZT;
-  const int nz_tile = (nz - iz0) < FAST_ZT ? (nz - iz0) : FAST_ZT;
+  const int iz0 = tz * zt;                              // zt <= FAST_ZT z0 cells per block (launcher's choice)
+  const int nz_tile = (nz - iz0) < zt ? (nz - iz0) : zt;
   if (threadIdx.x < FAST_ZT) {
     const int iz = iz0 + (threadIdx.x < nz_tile ? threadIdx.x : nz_tile - 1);
     const Iv<T> Z = box_iv<T>(cell_edge(g.lo[3], g.hi[3], g.w[3], iz, nz), cell_edge(g.lo[3], g.hi[3], g.w[3], iz + 1, nz));
@@ -371,7 +371,16 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   int threads = FAST_THREADS;
   if (n_pairs < threads) threads = (n_pairs + 31) / 32 * 32;
   const int tiles_p = (n_pairs + FAST_THREADS - 1) / FAST_THREADS;
-  const int tiles_z = (g.n[3] + FAST_ZT - 1) / FAST_ZT;
+  // z0 cells per block: FAST_ZT amortises the per-(pair, hit) terms best; small launches (one event on a
+  // coarse grid) take fewer so that the chip still gets about 8 blocks per SM
+  int n_sm = 148;
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
+  int zt = FAST_ZT;
+  {
+    const int64_t base = int64_t(g.n[0]) * g.n[1] * ((n_pairs + FAST_THREADS - 1) / FAST_THREADS) * sp.n_events;
+    while (zt > 1 && base * ((g.n[3] + zt - 1) / zt) < int64_t(8) * n_sm) zt >>= 1;
+  }
+  const int tiles_z = (g.n[3] + zt - 1) / zt;
   const int64_t nxy = int64_t(g.n[0]) * g.n[1];
   const int64_t blocks = nxy * tiles_p * tiles_z;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
@@ -387,12 +396,12 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
     err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (err != cudaSuccess) return err;
     vote_dense_fast_kernel<T, true><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
-                                                                         tiles_p, tiles_z, votes_out);
+                                                                         tiles_p, tiles_z, zt, votes_out);
   } else {
     err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (err != cudaSuccess) return err;
     vote_dense_fast_kernel<T, false><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
-                                                                          tiles_p, tiles_z, votes_out);
+                                                                          tiles_p, tiles_z, zt, votes_out);
   }
   ctx->launches++;
   return cudaGetLastError();
