@@ -552,6 +552,35 @@ struct Grid4 {
   }
 };
 
+// ---- paper's iteration scheme, pieces -----------
+// F2a  disk pre-filter, conditions (3a),(3b) L66-70: a voxel is considered only if
+//        0 in xc^2 + yc^2 - (R + R_Disk)^2,   R_Disk = [-r_disk, +r_disk]
+//      (the particle is emitted within r_disk of the origin).  Interval arithmetic, outward rounding;
+//      every variable occurs once, so the enclosure is the exact range.  Mode must be FE_UPWARD.
+bool disk_passes(const double lo[4], const double hi[4], double r_disk) {
+  const Iv<double> X = {lo[0], hi[0]}, Y = {lo[1], hi[1]}, R = {lo[2], hi[2]}, D = {-r_disk, r_disk};
+  const Iv<double> f = isub(iadd(isqr(X), isqr(Y)), isqr(iadd(R, D)));
+  return !(f.lo > 0.0 || f.hi < 0.0);
+}
+
+// F2b  selection, L94 ("voxels corresponding to selected cells where the maximum of votes in the
+//      accumulator are found.  The central values and the size of the selected voxels are used to
+//      calculate the parameter values with their errors") and L121 (the sign of lambda from the two
+//      accumulators).  Reading (F2b): vmax = largest count in either accumulator; the sign of
+//      lambda = the accumulator that holds it (both: lambda >= 0 wins); selected = the voxels of that
+//      accumulator with count == vmax; value_d = centre of the mean cell index, error_d = half the extent
+//      of the selected voxels along axis d.  Integer sums, so the result does not depend on any order:
+//        mean index  m_d = (2 sum(k_d) + n_sel) / (2 n_sel)   (one correctly rounded division)
+//        value_d = lo_d + m_d * w_d,  w_d = (hi_d - lo_d)/n_d   (rn, unfused)
+//        error_d = 0.5 * ((kmax_d - kmin_d + 1) * w_d)
+struct OrcPaperFit {
+  double value[4], error[4];
+  double lambda;          // signed, from the fixed momentum at value[2]; 0 if value[2] > P
+  int32_t lambda_sign;    // +1 / -1
+  int32_t vmax;
+  int64_t n_sel;
+};
+
 // =============================================================================================
 // C ABI (ctypes)
 // =============================================================================================
@@ -729,7 +758,10 @@ int orc_residual_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, in
 
 // dense 4-D grid, two accumulators: votes_out[ls*n + i], ls = 0 for lambda >= 0, 1 for lambda < 0;
 // cell_idx == NULL: all prod(dims) voxels in linear order (z0 fastest), else the listed voxels
-int orc_vote_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
+// hit_mask (may be NULL): hits with mask 0 are not used (L96: "Only the selected hits are used for the next
+// iteration"); r_disk >= 0: voxels failing the disk pre-filter (3a,b) get no vote; r_disk < 0: no filter
+int orc_vote_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const uint8_t* hit_mask,
+                   const OrcParams* p, double P, double r_disk,
                    const double* lo, const double* hi, const int32_t* dims, const int64_t* cell_idx, int64_t n_idx,
                    uint16_t* votes_out) {
   if (!wires || !hits || !p || !lo || !hi || !dims || !votes_out || n_hits < 0 || !(P > 0)) return ORC_ERR_ARG;
@@ -751,11 +783,13 @@ int orc_vote_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_
       double clo[4], chi[4];
       g.cell(cell_idx ? cell_idx[i] : i, clo, chi);
       double lam = 0;
-      const bool has_l = paper_lambda(clo[2], chi[2], P, &lam);
+      const bool has_l = paper_lambda(clo[2], chi[2], P, &lam) && (r_disk < 0.0 || disk_passes(clo, chi, r_disk));
       for (int ls = 0; ls < 2; ++ls) {
         unsigned v = 0;
         if (has_l)
-          for (const auto& c : hc) {
+          for (int h = 0; h < n_hits; ++h) {
+            if (hit_mask && !hit_mask[h]) continue;
+            const auto& c = hc[h];
             bool yes = false;
             for (int ds = 0; ds < 2 && !yes; ++ds) {
               const PaperResid r = paper_residual(clo, chi, c, ls == 0 ? lam : -lam, ds == 0 ? +1 : -1);
@@ -774,6 +808,77 @@ int orc_cell_boxes4(const double* lo, const double* hi, const int32_t* dims, con
                     double* blo, double* bhi) {
   Grid4 g(lo, hi, dims);
   for (int64_t i = 0; i < n; ++i) g.cell(cell_idx[i], blo + 4 * i, bhi + 4 * i);
+  return ORC_OK;
+}
+
+int orc_disk_filter(const double* lo, const double* hi, const int32_t* dims, double r_disk, const int64_t* cell_idx,
+                    int64_t n_idx, uint8_t* out) {
+  if (!lo || !hi || !dims || !out || !(r_disk >= 0)) return ORC_ERR_ARG;
+  Grid4 g(lo, hi, dims);
+  const int64_t n = cell_idx ? n_idx : g.cells();
+  UpMode up;
+  for (int64_t i = 0; i < n; ++i) {
+    double clo[4], chi[4];
+    g.cell(cell_idx ? cell_idx[i] : i, clo, chi);
+    out[i] = disk_passes(clo, chi, r_disk) ? 1 : 0;
+  }
+  return ORC_OK;
+}
+
+int orc_select_max_paper(const uint16_t* votes, const double* lo, const double* hi, const int32_t* dims, double P,
+                         OrcPaperFit* out) {
+  if (!votes || !lo || !hi || !dims || !out || !(P > 0)) return ORC_ERR_ARG;
+  int64_t n = 1;
+  for (int d = 0; d < 4; ++d) { if (dims[d] <= 0 || !(hi[d] > lo[d])) return ORC_ERR_ARG; n *= dims[d]; }
+  int vmax[2] = {0, 0};
+  for (int s = 0; s < 2; ++s) for (int64_t i = 0; i < n; ++i) vmax[s] = std::max(vmax[s], int(votes[s * n + i]));
+  const int s = vmax[1] > vmax[0] ? 1 : 0;
+  int64_t sum[4] = {0, 0, 0, 0}, kmin[4], kmax[4], cnt = 0;
+  for (int d = 0; d < 4; ++d) { kmin[d] = dims[d]; kmax[d] = -1; }
+  for (int64_t i = 0; i < n; ++i) {
+    if (votes[s * n + i] != vmax[s]) continue;
+    int64_t idx = i;
+    for (int d = 3; d >= 0; --d) {
+      const int64_t k = idx % dims[d]; idx /= dims[d];
+      sum[d] += k; kmin[d] = std::min(kmin[d], k); kmax[d] = std::max(kmax[d], k);
+    }
+    ++cnt;
+  }
+  for (int d = 0; d < 4; ++d) {
+    const double w = opaque(opaque(hi[d] - lo[d]) / double(dims[d]));
+    const double m = opaque(double(2 * sum[d] + cnt) / double(2 * cnt));
+    out->value[d] = opaque(lo[d] + opaque(m * w));
+    out->error[d] = opaque(0.5 * opaque(double(kmax[d] - kmin[d] + 1) * w));
+  }
+  const double q = opaque(P / out->value[2]);
+  const double l2 = opaque(opaque(q * q) - 1.0);
+  out->lambda = l2 >= 0.0 ? (s == 0 ? std::sqrt(l2) : -std::sqrt(l2)) : 0.0;
+  out->lambda_sign = s == 0 ? +1 : -1;
+  out->vmax = vmax[s];
+  out->n_sel = cnt;
+  return ORC_OK;
+}
+
+// F2c  hit finding, L96: one multidimensional interval [lo, hi] (the caller builds it: value -/+ 5 error);
+//      "One hit is selected when the condition (4) is true for this multidimensional interval": paper-mode
+//      condition (4) with d_Ax at the interval's mid-point, the given sign of lambda, either drift sign.
+int orc_find_hits_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
+                        int lambda_sign, const double* lo, const double* hi, uint8_t* flags_out) {
+  if (!wires || !hits || !p || !lo || !hi || !flags_out || n_hits < 0 || !(P > 0)) return ORC_ERR_ARG;
+  for (int d = 0; d < 4; ++d) if (!(hi[d] > lo[d])) return ORC_ERR_ARG;
+  for (int i = 0; i < n_hits; ++i) if (hits[i].wire < 0 || hits[i].wire >= n_wires) return ORC_ERR_GEOMETRY;
+  std::vector<HitC<double>> hc = stage_hits<double>(wires, hits, n_hits, *p);
+  UpMode up;
+  double lam = 0;
+  const bool has_l = paper_lambda(lo[2], hi[2], P, &lam);
+  for (int h = 0; h < n_hits; ++h) {
+    bool yes = false;
+    for (int ds = 0; ds < 2 && has_l && !yes; ++ds) {
+      const PaperResid r = paper_residual(lo, hi, hc[h], lambda_sign >= 0 ? lam : -lam, ds == 0 ? +1 : -1);
+      yes = r.has && !(r.flo > 0.0 || r.fhi < 0.0);
+    }
+    flags_out[h] = yes ? 1 : 0;
+  }
   return ORC_OK;
 }
 

@@ -30,7 +30,8 @@ def lib():
         _lib = C.CDLL(path)
         for name in ("orc_prim", "orc_residual", "orc_vote_boxes", "orc_vote", "orc_cell_boxes", "orc_topk",
                      "orc_refine", "orc_refine_batch", "orc_pad_ulps", "orc_max_threads", "orc_dax_point",
-                     "orc_residual_paper", "orc_vote_paper", "orc_cell_boxes4"):
+                     "orc_residual_paper", "orc_vote_paper", "orc_cell_boxes4", "orc_disk_filter",
+                     "orc_select_max_paper", "orc_find_hits_paper"):
             getattr(_lib, name).restype = C.c_int
         _lib.orc_set_threads.restype = None
     return _lib
@@ -183,8 +184,9 @@ def residual_paper(wires, hits, params: Params, P: float, blo, bhi) -> np.ndarra
     return out
 
 
-def vote_paper(wires, hits, params: Params, P: float, lo, hi, dims, cell_idx=None) -> np.ndarray:
-    """two 4-D accumulators [2, n]: [0] for lambda >= 0, [1] for lambda < 0; voxel index z0 fastest."""
+def vote_paper(wires, hits, params: Params, P: float, lo, hi, dims, cell_idx=None, hit_mask=None, r_disk=-1.0) -> np.ndarray:
+    """two 4-D accumulators [2, n]: [0] for lambda >= 0, [1] for lambda < 0; voxel index z0 fastest.
+    hit_mask: uint8 per hit (0 = not used); r_disk >= 0: disk pre-filter (3a,b)."""
     lo = np.ascontiguousarray(lo, np.float64)
     hi = np.ascontiguousarray(hi, np.float64)
     dims = np.ascontiguousarray(dims, np.int32)
@@ -196,8 +198,12 @@ def vote_paper(wires, hits, params: Params, P: float, lo, hi, dims, cell_idx=Non
         n = len(cell_idx)
         idx_p, n_idx = _p(cell_idx), n
     out = np.zeros((2, n), np.uint16)
-    _chk(lib().orc_vote_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P), _p(lo), _p(hi),
-                              _p(dims), idx_p, C.c_int64(n_idx), _p(out)), "vote_paper")
+    mask_p = None
+    if hit_mask is not None:
+        hit_mask = np.ascontiguousarray(hit_mask, np.uint8)
+        mask_p = _p(hit_mask)
+    _chk(lib().orc_vote_paper(_p(wires), len(wires), _p(hits), len(hits), mask_p, C.byref(params), C.c_double(P),
+                              C.c_double(r_disk), _p(lo), _p(hi), _p(dims), idx_p, C.c_int64(n_idx), _p(out)), "vote_paper")
     return out
 
 
@@ -211,3 +217,42 @@ def cell_boxes4(lo, hi, dims, cell_idx):
     _chk(lib().orc_cell_boxes4(_p(lo), _p(hi), _p(dims), _p(cell_idx), C.c_int64(len(cell_idx)), _p(blo), _p(bhi)),
          "cell_boxes4")
     return blo, bhi
+
+
+# ---- pieces of the paper's iteration scheme ------------------------------------------------------
+class PaperFit(C.Structure):
+    _fields_ = [("value", C.c_double * 4), ("error", C.c_double * 4), ("lam", C.c_double), ("lambda_sign", C.c_int32),
+                ("vmax", C.c_int32), ("n_sel", C.c_int64)]
+
+
+def disk_filter(lo, hi, dims, r_disk: float, cell_idx=None) -> np.ndarray:
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    if cell_idx is None:
+        n, idx_p, n_idx = int(np.prod(dims.astype(np.int64))), None, 0
+    else:
+        cell_idx = np.ascontiguousarray(cell_idx, np.int64)
+        n, idx_p, n_idx = len(cell_idx), _p(cell_idx), len(cell_idx)
+    out = np.zeros(n, np.uint8)
+    _chk(lib().orc_disk_filter(_p(lo), _p(hi), _p(dims), C.c_double(r_disk), idx_p, C.c_int64(n_idx), _p(out)), "disk_filter")
+    return out
+
+
+def select_max_paper(votes, lo, hi, dims, P: float) -> PaperFit:
+    votes = np.ascontiguousarray(votes, np.uint16)
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    dims = np.ascontiguousarray(dims, np.int32)
+    fit = PaperFit()
+    _chk(lib().orc_select_max_paper(_p(votes), _p(lo), _p(hi), _p(dims), C.c_double(P), C.byref(fit)), "select_max_paper")
+    return fit
+
+
+def find_hits_paper(wires, hits, params: Params, P: float, lambda_sign: int, lo, hi) -> np.ndarray:
+    lo = np.ascontiguousarray(lo, np.float64)
+    hi = np.ascontiguousarray(hi, np.float64)
+    out = np.zeros(len(hits), np.uint8)
+    _chk(lib().orc_find_hits_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P),
+                                   int(lambda_sign), _p(lo), _p(hi), _p(out)), "find_hits_paper")
+    return out

@@ -1,0 +1,135 @@
+"""Pins of the oracle's pieces of the paper's iteration scheme.
+
+F2a  disk pre-filter (3a,b): every variable occurs once => exact range; compared with the closed form in exact
+     rational arithmetic, and with the defining property (a voxel that holds a circle passing within r_disk of the
+     origin is kept) by brute force.
+F2b  selection of the maximum-vote voxels: special cases whose answer the definition fixes - a single voxel (its
+     centre, its half-size), a rectangular block (its centre, its half-extent), a set symmetric about a point, the
+     accumulator choice for the sign of lambda, order independence.
+F2c  hit finding = condition (4) on one multidimensional interval: equals the (pinned) paper-mode vote of a 1-voxel
+     grid hit by hit; an interval around the generated truth finds every genuine hit and rejects far noise.
+--   hit mask: masked hits do not vote (vote with mask = vote of the sub-list).
+"""
+from fractions import Fraction as Fr
+
+import numpy as np
+
+from paper_2401_04576_b200 import eventgen as g
+from oracle import oracle as o
+
+LO4, HI4 = np.array(g.BOX_LO[:4]), np.array(g.BOX_HI[:4])
+
+
+def _disk_exact(lo, hi, r):
+    F = Fr
+    def sq_minmax(l, h):
+        l, h = F(l), F(h)
+        mn = F(0) if l <= 0 <= h else min(l * l, h * h)
+        return mn, max(l * l, h * h)
+    xmn, xmx = sq_minmax(lo[0], hi[0])
+    ymn, ymx = sq_minmax(lo[1], hi[1])
+    smn, smx = sq_minmax(F(lo[2]) - F(r), F(hi[2]) + F(r))
+    return (xmn + ymn - smx) <= 0 <= (xmx + ymx - smn)
+
+
+def test_f2a_disk_filter_is_the_exact_range_test():
+    rng = np.random.default_rng(3)
+    dims = (9, 8, 7, 2)
+    for trial in range(6):
+        lo = np.array([rng.uniform(-450, -50), rng.uniform(-450, -50), rng.uniform(5, 60), -10.0])
+        hi = np.array([rng.uniform(50, 450), rng.uniform(50, 450), rng.uniform(100, 450), 10.0])
+        r = [10.0, 0.0, 3.5, 25.0, 10.0, 1.0][trial]
+        keep = o.disk_filter(lo, hi, dims, r)
+        n = int(np.prod(dims))
+        blo, bhi = o.cell_boxes4(lo, hi, dims, np.arange(n))
+        exact = np.array([_disk_exact(blo[i], bhi[i], r) for i in range(n)])
+        # the enclosure is the exact range up to outward rounding: it may only add knife-edge voxels
+        assert (keep[exact] == 1).all()
+        extra = np.nonzero((keep == 1) & ~exact)[0]
+        assert len(extra) <= 2
+        assert 0 < keep.sum() < n or r == 25.0
+        # defining property by brute force: a circle through a point within r of the origin
+        for _ in range(300):
+            i = int(rng.integers(n))
+            xc, yc = rng.uniform(blo[i, 0], bhi[i, 0]), rng.uniform(blo[i, 1], bhi[i, 1])
+            R = rng.uniform(blo[i, 2], bhi[i, 2])
+            if abs(np.hypot(xc, yc) - R) <= r * (1 - 1e-12):
+                assert keep[i] == 1
+
+
+def _votes_with(dims, cells, acc, vmax=7, base=3):
+    n = int(np.prod(dims))
+    v = np.full((2, n), base, np.uint16)
+    for c in cells:
+        idx = ((c[0] * dims[1] + c[1]) * dims[2] + c[2]) * dims[3] + c[3]
+        v[acc, idx] = vmax
+    return v
+
+
+def test_f2b_selection_special_cases():
+    dims = (10, 8, 6, 4)
+    lo, hi = np.array([-100.0, -80.0, 60.0, -8.0]), np.array([100.0, 80.0, 120.0, 8.0])
+    w = (hi - lo) / np.array(dims)
+    P = 200.0
+    # one voxel: its centre and half-size
+    f = o.select_max_paper(_votes_with(dims, [(3, 5, 2, 1)], 0), lo, hi, dims, P)
+    assert f.n_sel == 1 and f.vmax == 7 and f.lambda_sign == 1
+    assert np.allclose(list(f.value), lo + (np.array([3, 5, 2, 1]) + 0.5) * w, rtol=0, atol=1e-12)
+    assert np.allclose(list(f.error), 0.5 * w, rtol=0, atol=1e-12)
+    assert abs(f.lam - np.sqrt((P / f.value[2]) ** 2 - 1)) < 1e-12
+    # a rectangular block in the other accumulator: its centre, its half-extent, lambda < 0
+    block = [(i, j, k, l) for i in (2, 3, 4) for j in (1, 2) for k in (0, 1, 2, 3) for l in (3,)]
+    f = o.select_max_paper(_votes_with(dims, block, 1), lo, hi, dims, P)
+    assert f.n_sel == len(block) and f.lambda_sign == -1 and f.lam < 0
+    assert np.allclose(list(f.value), lo + np.array([3.5, 2.0, 2.0, 3.5]) * w, rtol=0, atol=1e-12)
+    assert np.allclose(list(f.error), 0.5 * np.array([3, 2, 4, 1]) * w, rtol=0, atol=1e-12)
+    # a set symmetric about a voxel centre (an L-shape and its mirror image): value = that centre
+    sym = [(5, 4, 3, 2), (6, 4, 3, 2), (4, 4, 3, 2), (5, 5, 3, 2), (5, 3, 3, 2), (7, 6, 3, 2), (3, 2, 3, 2)]
+    f = o.select_max_paper(_votes_with(dims, sym, 0), lo, hi, dims, P)
+    assert np.allclose(list(f.value), lo + (np.array([5, 4, 3, 2]) + 0.5) * w, rtol=0, atol=1e-12)
+    assert np.allclose(list(f.error), 0.5 * np.array([5, 5, 1, 1]) * w, rtol=0, atol=1e-12)
+    # equal maxima in both accumulators: lambda >= 0 wins; a larger maximum in accumulator 1 wins
+    v = _votes_with(dims, [(1, 1, 1, 1)], 0)
+    v[1] = _votes_with(dims, [(8, 6, 4, 2)], 1)[1]
+    f = o.select_max_paper(v, lo, hi, dims, P)
+    assert f.lambda_sign == 1 and np.isclose(f.value[0], lo[0] + 1.5 * w[0])
+    v[1, 5] = 9
+    f = o.select_max_paper(v, lo, hi, dims, P)
+    assert f.lambda_sign == -1 and f.vmax == 9 and f.n_sel == 1
+    # R value above P: no lambda
+    f = o.select_max_paper(_votes_with(dims, [(3, 5, 5, 1)], 0), lo, hi, dims, 100.0)
+    assert f.lam == 0.0
+
+
+def test_f2c_hit_finding_and_hit_mask():
+    ch = g.chamber_c1()
+    wires = o.wires_of(ch)
+    p = o.make_params(g.TOL)
+    for seed in (41, 42, 43, 44):
+        ev = g.make_event(ch, seed, n_noise=12)
+        hits = o.hits_of(ev.wire, ev.drift)
+        xc, yc, R, z0, lam = ev.track.params
+        P = R * np.sqrt(1 + lam * lam)
+        c = np.array([xc, yc, R, z0])
+        sgn = 1 if lam >= 0 else -1
+        for hw in (np.array([0.3, 0.3, 0.3, 1.0]), np.array([5.0, 5.0, 3.0, 4.0])):
+            fl = o.find_hits_paper(wires, hits, p, P, sgn, c - hw, c + hw)
+            # definition: the paper-mode vote of the 1-voxel grid, hit by hit
+            for h in range(ev.n_hits):
+                v = o.vote_paper(wires, hits[h:h + 1], p, P, c - hw, c + hw, (1, 1, 1, 1))
+                assert fl[h] == v[0 if sgn > 0 else 1, 0]
+            genuine = ~ev.is_noise & ~ev.clipped
+            assert fl[genuine].all()
+        # the small interval rejects most noise hits
+        fl = o.find_hits_paper(wires, hits, p, P, sgn, c - 0.3, c + 0.3)
+        assert fl[ev.is_noise].sum() <= 3
+        # hit mask = vote of the sub-list; disk filter only removes voxels
+        mask = (np.arange(ev.n_hits) % 3 != 0).astype(np.uint8)
+        dims = (5, 4, 6, 3)
+        vm = o.vote_paper(wires, hits, p, P, LO4, HI4, dims, hit_mask=mask)
+        vs = o.vote_paper(wires, hits[mask == 1], p, P, LO4, HI4, dims)
+        assert (vm == vs).all()
+        vd = o.vote_paper(wires, hits, p, P, LO4, HI4, dims, r_disk=10.0)
+        vf = o.vote_paper(wires, hits, p, P, LO4, HI4, dims)
+        keep = o.disk_filter(LO4, HI4, dims, 10.0)
+        assert (vd[:, keep == 1] == vf[:, keep == 1]).all() and (vd[:, keep == 0] == 0).all()
