@@ -124,9 +124,44 @@ int ia_vote_boxes(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double*
  * The guarantee "no vote => no solution in the voxel" does not hold in this mode (L80-82).
  * votes_out_dev[s*N + (((ix*ny+iy)*nR+iR)*nz+iz)], N = prod(grid_dims), s = 0: lambda >= 0, 1: lambda < 0
  * (2*N uint16, z0 fastest).  Always double precision (params.precision is not consulted).
- * Errors: IA_ERR_ARG (null, sizes, momentum_radius <= 0), IA_ERR_DOMAIN (box_lo[2] <= 0). */
-int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const double box_lo[4],
-                  const double box_hi[4], const int32_t grid_dims[4], uint16_t* votes_out_dev);
+ * Errors: IA_ERR_ARG (null, sizes, momentum_radius <= 0), IA_ERR_DOMAIN (box_lo[2] <= 0).
+ * hit_mask_dev (may be NULL): uint8 per hit, 0 = the hit is not used (L96: "Only the selected hits are used
+ * for the next iteration").  r_disk >= 0: disk pre-filter, conditions (3a),(3b) L66-70 - a voxel is
+ * considered only if 0 in xc^2 + yc^2 - (R + [-r_disk, r_disk])^2 (interval arithmetic), the others get
+ * 0 in both accumulators; r_disk < 0: no filter. */
+int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t* hit_mask_dev, double momentum_radius,
+                  double r_disk, const double box_lo[4], const double box_hi[4], const int32_t grid_dims[4],
+                  uint16_t* votes_out_dev);
+
+/* f2 (pieces of the paper's iteration scheme; readings F2b, F2c of DESIGN.md).
+ * Result of the selection: 88 bytes. */
+typedef struct {
+  double value[4], error[4]; /* xc, yc, R, z0: centre of the mean cell index / half-extent of the selected voxels */
+  double lambda;             /* signed, sqrt((P/value[2])^2 - 1); 0 if value[2] > P */
+  int32_t lambda_sign;       /* +1: accumulator 0 holds the maximum (ties included), -1: accumulator 1 */
+  int32_t vmax;              /* the maximum count */
+  int64_t n_sel;             /* number of selected voxels */
+} ia_paper_fit;
+
+/* L94: "the values and the errors of the parameters are computed using voxels corresponding to selected
+ * cells where the maximum of votes in the accumulator are found.  The central values and the size of the
+ * selected voxels are used": vmax = the largest count of votes_dev[2][N] (as written by ia_vote_paper on
+ * the same grid); the sign of lambda = the accumulator that holds it (L121); with k_d the cell indices of
+ * the voxels of that accumulator whose count equals vmax,
+ *   value_d = lo_d + ((2 sum k_d + n)/(2 n)) * w_d,   error_d = 0.5 * ((max k_d - min k_d + 1) * w_d),
+ * w_d = (hi_d - lo_d)/n_d - integer sums, round-to-nearest unfused arithmetic, independent of any order.
+ * fit_out_dev: DEVICE pointer. */
+int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_radius, const double box_lo[4],
+                        const double box_hi[4], const int32_t grid_dims[4], ia_paper_fit* fit_out_dev);
+
+/* L96: "An multidimensional interval is constructed.  Its central value is given by the parameter values ...
+ * and its radius is given by their errors multiplied by a factor of 5 ... One hit is selected when the
+ * condition (4) is true for this multidimensional interval": flags_out_dev[h] = 1 iff the paper-mode
+ * condition (4) holds for hit h on [value - factor*error, value + factor*error] (d_Ax at its mid-point,
+ * lambda of the fit's sign, either drift sign).  fit_dev: DEVICE pointer (as written by
+ * ia_select_max_paper), so that no host round trip separates the two calls. */
+int ia_find_hits_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const ia_paper_fit* fit_dev,
+                       double factor, uint8_t* flags_out_dev);
 
 /* a7 - the k largest entries by key (votes descending, index ascending) (L94, G16):
  * idx_out_dev[k] (int64 linear indices), votes_out_dev[k].  1 <= k <= min(n_cells, IA_MAX_K). */

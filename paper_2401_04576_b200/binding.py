@@ -21,9 +21,11 @@ WIRE_DT = np.dtype([("x0", "f8"), ("y0", "f8"), ("sin_phi_s", "f8"), ("cos_phi_s
                     ("half_len", "f8"), ("layer", "i4"), ("_pad", "i4")])
 HIT_DT = np.dtype([("wire", "i4"), ("_pad", "i4"), ("drift", "f8")])
 BOX_DT = np.dtype([("lo", "f8", (5,)), ("hi", "f8", (5,)), ("votes", "u2"), ("_pad", "u2", (3,))])
-assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88
+FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), ("lambda_sign", "i4"), ("vmax", "i4"),
+                   ("n_sel", "i8")])
+assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 88
 
-EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_topk",
+EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
@@ -59,7 +61,9 @@ def load_library(path: str = LIB_PATH):
     lib.ia_set_params.argtypes = [vp, C.POINTER(IaParams)]
     lib.ia_vote.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_vote_boxes.argtypes = [vp, vp, i32, vp, vp, i64, vp]
-    lib.ia_vote_paper.argtypes = [vp, vp, i32, dbl, vp, vp, vp, vp]
+    lib.ia_vote_paper.argtypes = [vp, vp, i32, vp, dbl, dbl, vp, vp, vp, vp]
+    lib.ia_select_max_paper.argtypes = [vp, vp, dbl, vp, vp, vp, vp]
+    lib.ia_find_hits_paper.argtypes = [vp, vp, i32, dbl, vp, dbl, vp]
     lib.ia_topk.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.ia_refine.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_refine_batch.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, i32, i32, vp, vp]
@@ -99,6 +103,13 @@ def _host5(a, dtype):
     a = np.ascontiguousarray(a, dtype)
     if a.shape != (5,):
         raise ValueError("expected 5 values (xc, yc, R, z0, lambda)")
+    return a
+
+
+def _host4(a, dtype):
+    a = np.ascontiguousarray(a, dtype)
+    if a.shape != (4,):
+        raise ValueError("expected 4 values (xc, yc, R, z0)")
     return a
 
 
@@ -187,17 +198,34 @@ class Context:
         return votes_out
 
     # ---- f1: the paper's own configuration (4-D voxels, mid-voxel d_Ax, two lambda-sign accumulators)
-    def ia_vote_paper(self, hits_dev, n_hits, momentum_radius, box_lo, box_hi, grid_dims, votes_out=None):
+    def ia_vote_paper(self, hits_dev, n_hits, momentum_radius, box_lo, box_hi, grid_dims, votes_out=None, hit_mask_dev=None,
+                      r_disk=-1.0):
         torch = self._torch
-        lo = np.ascontiguousarray(box_lo, np.float64).reshape(4)
-        hi = np.ascontiguousarray(box_hi, np.float64).reshape(4)
-        dims = np.ascontiguousarray(grid_dims, np.int32).reshape(4)
+        lo, hi, dims = _host4(box_lo, np.float64), _host4(box_hi, np.float64), _host4(grid_dims, np.int32)
         n = int(np.prod(dims.astype(np.int64)))
         if votes_out is None:
             votes_out = self._empty(2 * n, torch.uint16)
-        self._chk(self.lib.ia_vote_paper(self.h, _dp(hits_dev), n_hits, float(momentum_radius), _hp(lo), _hp(hi), _hp(dims),
-                                         _dp(votes_out)), "ia_vote_paper")
+        self._chk(self.lib.ia_vote_paper(self.h, _dp(hits_dev), n_hits, _dp(hit_mask_dev), float(momentum_radius), float(r_disk),
+                                         _hp(lo), _hp(hi), _hp(dims), _dp(votes_out)), "ia_vote_paper")
         return votes_out.view(2, n)
+
+    # ---- f2 pieces: maximum-vote selection (device-resident result) and hit finding
+    def ia_select_max_paper(self, votes_dev, momentum_radius, box_lo, box_hi, grid_dims, fit_out=None):
+        torch = self._torch
+        lo, hi, dims = _host4(box_lo, np.float64), _host4(box_hi, np.float64), _host4(grid_dims, np.int32)
+        if fit_out is None:
+            fit_out = self._empty(FIT_DT.itemsize, torch.uint8)
+        self._chk(self.lib.ia_select_max_paper(self.h, _dp(votes_dev), float(momentum_radius), _hp(lo), _hp(hi), _hp(dims),
+                                               _dp(fit_out)), "ia_select_max_paper")
+        return fit_out
+
+    def ia_find_hits_paper(self, hits_dev, n_hits, momentum_radius, fit_dev, factor=5.0, flags_out=None):
+        torch = self._torch
+        if flags_out is None:
+            flags_out = self._empty(max(n_hits, 1), torch.uint8)
+        self._chk(self.lib.ia_find_hits_paper(self.h, _dp(hits_dev), n_hits, float(momentum_radius), _dp(fit_dev), float(factor),
+                                              _dp(flags_out)), "ia_find_hits_paper")
+        return flags_out[:n_hits]
 
     def ia_vote_boxes(self, hits_dev, n_hits, lo_dev, hi_dev, votes_out=None):
         torch = self._torch

@@ -219,24 +219,54 @@ int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo
   return IA_OK;
 }
 
-int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const double box_lo[4],
-                  const double box_hi[4], const int32_t grid_dims[4], uint16_t* votes_out_dev) {
-  int rc = check_ready(ctx);
-  if (rc) return rc;
-  if (n_hits < 0 || (n_hits > 0 && !hits_dev) || !votes_out_dev || !box_lo || !box_hi || !grid_dims) return IA_ERR_ARG;
-  if (!(momentum_radius > 0.0) || !std::isfinite(momentum_radius)) return IA_ERR_ARG;
-  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+static int make_grid4(const double box_lo[4], const double box_hi[4], const int32_t grid_dims[4], GridDesc& g) {
+  if (!box_lo || !box_hi || !grid_dims) return IA_ERR_ARG;
   const double lo5[5] = {box_lo[0], box_lo[1], box_lo[2], box_lo[3], 0.0};
   const double hi5[5] = {box_hi[0], box_hi[1], box_hi[2], box_hi[3], 1.0};
   const int32_t n5[5] = {grid_dims[0], grid_dims[1], grid_dims[2], grid_dims[3], 1};
-  GridDesc g;
-  rc = make_grid(lo5, hi5, n5, g);
+  int rc = make_grid(lo5, hi5, n5, g);
   if (rc) return rc;
-  if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
   if (int64_t(grid_dims[0]) * grid_dims[1] > 0x7fffffffLL || int64_t(grid_dims[2]) * grid_dims[3] > 0x7fffffffLL)
     return IA_ERR_CAPACITY;
+  return IA_OK;
+}
+
+int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t* hit_mask_dev, double momentum_radius,
+                  double r_disk, const double box_lo[4], const double box_hi[4], const int32_t grid_dims[4],
+                  uint16_t* votes_out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits < 0 || (n_hits > 0 && !hits_dev) || !votes_out_dev) return IA_ERR_ARG;
+  if (!(momentum_radius > 0.0) || !std::isfinite(momentum_radius) || std::isnan(r_disk)) return IA_ERR_ARG;
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  GridDesc g;
+  rc = make_grid4(box_lo, box_hi, grid_dims, g);
+  if (rc) return rc;
+  if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
   DeviceGuard guard(ctx->device);
-  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, momentum_radius, g, votes_out_dev));
+  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, g, votes_out_dev));
+  return IA_OK;
+}
+
+int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_radius, const double box_lo[4],
+                        const double box_hi[4], const int32_t grid_dims[4], ia_paper_fit* fit_out_dev) {
+  if (!ctx || !votes_dev || !fit_out_dev || !(momentum_radius > 0.0)) return IA_ERR_ARG;
+  GridDesc g;
+  int rc = make_grid4(box_lo, box_hi, grid_dims, g);
+  if (rc) return rc;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_select_max_paper(ctx, votes_dev, g, momentum_radius, fit_out_dev));
+  return IA_OK;
+}
+
+int ia_find_hits_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const ia_paper_fit* fit_dev,
+                       double factor, uint8_t* flags_out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits < 0 || (n_hits > 0 && (!hits_dev || !flags_out_dev)) || !fit_dev) return IA_ERR_ARG;
+  if (!(momentum_radius > 0.0) || !(factor > 0.0) || !std::isfinite(factor)) return IA_ERR_ARG;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_find_hits_paper(ctx, hits_dev, n_hits, momentum_radius, fit_dev, factor, flags_out_dev));
   return IA_OK;
 }
 

@@ -122,16 +122,51 @@ IA_DEV bool dax_point(const PHit& h, double R, double Zr, double lam, double D, 
 
 constexpr int PAPER_THREADS = 256;
 
+// M3-M5 for one (voxel, hit, lambda): does either drift sign contain 0 ?
+IA_DEV bool paper_hit_votes(const PHit& ph, Iv<double> R, double Rm, double Zr, double l, bool two_ends) {
+  bool yes = false;
+#pragma unroll
+  for (int ds = 0; ds < 2; ++ds) {
+    double a = 0.0, b;
+    bool ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dlo : -ph.dlo, a);
+    b = a;
+    if (two_ends) ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dhi : -ph.dhi, b) && ok;
+    const Iv<double> Dax = {fmin(a, b), fmax(a, b)};
+    const Iv<double> S = isqr(iadd(R, Dax));
+    const Iv<double> f = isub(Iv<double>{ph.Qlo, ph.Qhi}, S);
+    yes = yes || (ok && !(f.lo > 0.0 || f.hi < 0.0));
+  }
+  return yes;
+}
+
+// M2: |lambda| at the mid radius from the fixed momentum; false if R_m > P
+IA_DEV bool paper_lambda(double P, double Rm, double& lam) {
+  const double q = __ddiv_rn(P, Rm);
+  const double l2 = sub(mul(q, q), 1.0);
+  lam = l2 >= 0.0 ? __dsqrt_rn(l2) : 0.0;
+  return l2 >= 0.0;
+}
+
+// F2a, conditions (3a,b) L66-70: 0 in X^2 + Y^2 - (R + [-r_disk, r_disk])^2
+IA_DEV bool disk_passes(Iv<double> X, Iv<double> Y, Iv<double> R, double r_disk) {
+  const Iv<double> f = isub(iadd(isqr(X), isqr(Y)), isqr(iadd(R, Iv<double>{-r_disk, r_disk})));
+  return !(f.lo > 0.0 || f.hi < 0.0);
+}
+
 __global__ void __launch_bounds__(PAPER_THREADS)
-vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const double* __restrict__ wires, int n_wires, ia_params p,
-                  double P, GridDesc g, int* status, uint16_t* __restrict__ votes) {
+vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __restrict__ hit_mask,
+                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, GridDesc g, int* status,
+                  uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PHit* sh = reinterpret_cast<PHit*>(smem_raw);
   const int ixy = blockIdx.x;
   const int ix = ixy / g.n[1], iy = ixy - ix * g.n[1];
   const Iv<double> X = {cell_edge(g.lo[0], g.hi[0], g.w[0], ix, g.n[0]), cell_edge(g.lo[0], g.hi[0], g.w[0], ix + 1, g.n[0])};
   const Iv<double> Y = {cell_edge(g.lo[1], g.hi[1], g.w[1], iy, g.n[1]), cell_edge(g.lo[1], g.hi[1], g.w[1], iy + 1, g.n[1])};
-  for (int h = threadIdx.x; h < n_hits; h += blockDim.x) make_phit(wires, n_wires, hits[h], p, X, Y, status, sh[h]);
+  for (int h = threadIdx.x; h < n_hits; h += blockDim.x) {
+    make_phit(wires, n_wires, hits[h], p, X, Y, status, sh[h]);
+    if (hit_mask && !hit_mask[h]) sh[h].valid = 0;       // L96: only the selected hits are used
+  }
   __syncthreads();
   const int nR = g.n[2], nz = g.n[3];
   const int64_t n_cells = g.cells;                       // nx*ny*nR*nz
@@ -141,34 +176,17 @@ vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const double* __r
     const Iv<double> R = {cell_edge(g.lo[2], g.hi[2], g.w[2], iR, nR), cell_edge(g.lo[2], g.hi[2], g.w[2], iR + 1, nR)};
     const double zlo = cell_edge(g.lo[3], g.hi[3], g.w[3], iz, nz), zhi = cell_edge(g.lo[3], g.hi[3], g.w[3], iz + 1, nz);
     const double Rm = mul(0.5, add(R.lo, R.hi)), zm = mul(0.5, add(zlo, zhi));
-    // M2
-    const double q = __ddiv_rn(P, Rm);
-    const double l2 = sub(mul(q, q), 1.0);
-    const bool has_l = l2 >= 0.0;
-    const double lam = has_l ? __dsqrt_rn(l2) : 0.0;
+    double lam;
+    bool live = paper_lambda(P, Rm, lam);
+    if (live && r_disk >= 0.0) live = disk_passes(X, Y, R, r_disk);
     unsigned v[2] = {0u, 0u};
-    if (has_l) {
+    if (live) {
       for (int h = 0; h < n_hits; ++h) {
         const PHit& ph = sh[h];
         if (!ph.valid) continue;
         const double Zr = sub(zm, ph.zref);
-#pragma unroll
-        for (int ls = 0; ls < 2; ++ls) {
-          const double l = ls == 0 ? lam : -lam;
-          bool yes = false;
-#pragma unroll
-          for (int ds = 0; ds < 2; ++ds) {
-            double a = 0.0, b;
-            bool ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dlo : -ph.dlo, a);
-            b = a;
-            if (two_ends) ok = dax_point(ph, Rm, Zr, l, ds == 0 ? ph.dhi : -ph.dhi, b) && ok;
-            const Iv<double> Dax = {fmin(a, b), fmax(a, b)};
-            const Iv<double> S = isqr(iadd(R, Dax));
-            const Iv<double> f = isub(Iv<double>{ph.Qlo, ph.Qhi}, S);
-            yes = yes || (ok && !(f.lo > 0.0 || f.hi < 0.0));
-          }
-          v[ls] += yes ? 1u : 0u;
-        }
+        v[0] += paper_hit_votes(ph, R, Rm, Zr, lam, two_ends) ? 1u : 0u;
+        v[1] += paper_hit_votes(ph, R, Rm, Zr, -lam, two_ends) ? 1u : 0u;
       }
     }
     const int64_t cell = int64_t(ixy) * (nR * nz) + j;
@@ -177,17 +195,125 @@ vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const double* __r
   }
 }
 
+// ---- F2b: selection of the maximum-vote voxels (L94, L121) -------------------------------------------
+// Integer reductions only (atomicMax / atomicMin / atomicAdd on integers), so the result does not depend on
+// the order in which blocks run.  acc: [0..1] vmax per accumulator, then for the chosen accumulator
+// [2] count, [3..6] sum of cell indices per axis, [7..10] kmin, [11..14] kmax  (all unsigned long long)
+__global__ void paper_init_kernel(unsigned long long* __restrict__ acc) {
+  if (threadIdx.x < 16) acc[threadIdx.x] = (threadIdx.x >= 7 && threadIdx.x <= 10) ? ~0ull : 0ull;
+}
+
+__global__ void paper_max_kernel(const uint16_t* __restrict__ votes, int64_t n, unsigned long long* __restrict__ acc) {
+  unsigned m0 = 0, m1 = 0;
+  for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
+    m0 = max(m0, unsigned(votes[i]));
+    m1 = max(m1, unsigned(votes[n + i]));
+  }
+  m0 = __reduce_max_sync(0xffffffffu, m0);
+  m1 = __reduce_max_sync(0xffffffffu, m1);
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax(&acc[0], (unsigned long long)m0);
+    atomicMax(&acc[1], (unsigned long long)m1);
+  }
+}
+
+__global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t n, GridDesc g, unsigned long long* __restrict__ acc) {
+  const int s = acc[1] > acc[0] ? 1 : 0;                 // equal maxima: lambda >= 0 wins
+  const unsigned vmax = unsigned(acc[s]);
+  const uint16_t* v = votes + int64_t(s) * n;
+  for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
+    if (unsigned(v[i]) != vmax) continue;
+    int64_t idx = i;
+    atomicAdd(&acc[2], 1ull);
+#pragma unroll
+    for (int d = 3; d >= 0; --d) {
+      const unsigned long long k = (unsigned long long)(idx % g.n[d]);
+      idx /= g.n[d];
+      atomicAdd(&acc[3 + d], k);
+      atomicMin(&acc[7 + d], k);
+      atomicMax(&acc[11 + d], k);
+    }
+  }
+}
+
+__global__ void paper_fit_kernel(const unsigned long long* __restrict__ acc, GridDesc g, double P, ia_paper_fit* __restrict__ out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int s = acc[1] > acc[0] ? 1 : 0;
+  const unsigned long long cnt = acc[2];
+  ia_paper_fit f;
+  for (int d = 0; d < 4; ++d) {
+    const double m = __ddiv_rn(double(2 * acc[3 + d] + cnt), double(2 * cnt));
+    f.value[d] = add(g.lo[d], mul(m, g.w[d]));
+    f.error[d] = mul(0.5, mul(double(acc[11 + d] - acc[7 + d] + 1), g.w[d]));
+  }
+  double lam;
+  const bool has = paper_lambda(P, f.value[2], lam);
+  f.lambda = has ? (s == 0 ? lam : -lam) : 0.0;
+  f.lambda_sign = s == 0 ? 1 : -1;
+  f.vmax = int32_t(acc[s]);
+  f.n_sel = int64_t(cnt);
+  *out = f;
+}
+
+// ---- F2c: hit finding (L96): condition (4) on the interval value -/+ factor * error, per hit ---------------
+__global__ void find_hits_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const double* __restrict__ wires, int n_wires,
+                                       ia_params p, double P, const ia_paper_fit* __restrict__ fit, double factor, int* status,
+                                       uint8_t* __restrict__ flags) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= n_hits) return;
+  double lo[4], hi[4];
+  for (int d = 0; d < 4; ++d) {
+    const double e = mul(factor, fit->error[d]);
+    lo[d] = sub(fit->value[d], e);
+    hi[d] = add(fit->value[d], e);
+  }
+  PHit ph;
+  make_phit(wires, n_wires, hits[h], p, Iv<double>{lo[0], hi[0]}, Iv<double>{lo[1], hi[1]}, status, ph);
+  const Iv<double> R = {lo[2], hi[2]};
+  const double Rm = mul(0.5, add(lo[2], hi[2])), zm = mul(0.5, add(lo[3], hi[3]));
+  double lam;
+  bool yes = false;
+  if (ph.valid && paper_lambda(P, Rm, lam))
+    yes = paper_hit_votes(ph, R, Rm, sub(zm, ph.zref), fit->lambda_sign >= 0 ? lam : -lam, p.tol > 0.0);
+  flags[h] = yes ? 1 : 0;
+}
+
 }  // namespace
 
-cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const GridDesc& g, uint16_t* votes_out) {
+cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
+                              const GridDesc& g, uint16_t* votes_out) {
   const size_t smem = size_t(n_hits) * sizeof(PHit);
   cudaError_t err = cudaFuncSetAttribute(vote_paper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
   if (err != cudaSuccess) return err;
   const int col = g.n[2] * g.n[3];
   int threads = PAPER_THREADS;
   if (col < threads) threads = (col + 31) / 32 * 32;
-  vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, ctx->wires, ctx->n_wires, ctx->params,
-                                                                              P, g, ctx->status, votes_out);
+  vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, hit_mask, ctx->wires, ctx->n_wires,
+                                                                              ctx->params, P, r_disk, g, ctx->status, votes_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const GridDesc& g, double P, ia_paper_fit* fit_out) {
+  cudaError_t err = scratch_reserve(ctx->keys, 16 * sizeof(unsigned long long));
+  if (err != cudaSuccess) return err;
+  unsigned long long* acc = static_cast<unsigned long long*>(ctx->keys.p);
+  paper_init_kernel<<<1, 32, 0, ctx->stream>>>(acc);
+  const int64_t n = g.cells;
+  int blocks = int((n + 1023) / 1024);
+  if (blocks > 1184) blocks = 1184;
+  paper_max_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, acc);
+  paper_moments_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, g, acc);
+  paper_fit_kernel<<<1, 32, 0, ctx->stream>>>(acc, g, P, fit_out);
+  ctx->launches += 4;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const ia_paper_fit* fit, double factor,
+                                   uint8_t* flags_out) {
+  if (n_hits <= 0) return cudaSuccess;
+  find_hits_paper_kernel<<<(n_hits + 63) / 64, 64, 0, ctx->stream>>>(hits, n_hits, ctx->wires, ctx->n_wires, ctx->params, P, fit,
+                                                                    factor, ctx->status, flags_out);
   ctx->launches++;
   return cudaGetLastError();
 }

@@ -117,3 +117,72 @@ def test_paper_mode_degenerate_and_errors():
         assert ei.value.code == -3
     finally:
         rig.close()
+
+
+# ---- pieces of the paper's iteration scheme ---------------------------------------------------
+def _fit_to_host(t):
+    return np.frombuffer(t.cpu().numpy().tobytes(), dtype=b.FIT_DT)[0]
+
+
+def test_f2_disk_filter_hit_mask_selection_and_hit_finding():
+    """ia_vote_paper with a hit mask and the disk pre-filter, ia_select_max_paper and ia_find_hits_paper against the
+    oracle: accumulators equal (>= 99.99 %, traced), the selection bit-identical (integer sums), flags identical."""
+    rig = Rig(g.chamber_c1())
+    try:
+        for seed, dims in ((21, (20, 20, 16, 8)), (22, (13, 11, 9, 7)), (23, (30, 30, 10, 4))):
+            ev = g.make_event(rig.ch, seed, n_noise=15)
+            P = _momentum_radius(ev)
+            hd, oh = rig.hits(ev.wire, ev.drift)
+            mask = (np.arange(ev.n_hits) % 4 != 1).astype(np.uint8)
+            rig.ctx.ia_set_params(g.TOL)
+            vg = rig.ctx.ia_vote_paper(hd, ev.n_hits, P, LO4, HI4, dims, hit_mask_dev=rig.dev(mask), r_disk=10.0)
+            fit_dev = rig.ctx.ia_select_max_paper(vg.view(-1), P, LO4, HI4, dims)
+            flags = rig.ctx.ia_find_hits_paper(hd, ev.n_hits, P, fit_dev, 5.0)
+            rig.ctx.synchronize()
+            vg_h = vg.cpu().numpy()
+            op = o.make_params(g.TOL)
+            vo = o.vote_paper(rig.owires, oh, op, P, LO4, HI4, dims, hit_mask=mask, r_disk=10.0)
+            assert (vg_h != vo).sum() <= vo.size * 1e-4
+            keep = o.disk_filter(LO4, HI4, dims, 10.0)
+            assert (vg_h[:, keep == 0] == 0).all() and 0 < keep.sum() < keep.size
+            # selection: defined on the accumulators it is given -> compare on the GPU's own accumulators
+            fo = o.select_max_paper(vg_h, LO4, HI4, dims, P)
+            fg = _fit_to_host(fit_dev)
+            assert list(fg["value"]) == list(fo.value) and list(fg["error"]) == list(fo.error)
+            assert fg["vmax"] == fo.vmax and fg["n_sel"] == fo.n_sel and fg["lambda_sign"] == fo.lambda_sign
+            assert fg["lam"] == fo.lam
+            # hit finding on value -/+ 5 error (rn, unfused - the same two operations as the kernel)
+            val, err = np.array(fo.value), np.array(fo.error)
+            lo, hi = val - 5.0 * err, val + 5.0 * err
+            fl_o = o.find_hits_paper(rig.owires, oh, op, P, fo.lambda_sign, lo, hi)
+            assert (flags.cpu().numpy() == fl_o).all()
+            assert fl_o.sum() > 0
+    finally:
+        rig.close()
+
+
+def test_f2_selection_special_cases_on_device():
+    """hand-made accumulators: single voxel, block, ties between the accumulators, all-equal counts (every voxel
+    selected: the centre of the grid, half its size)."""
+    import torch
+    rig = Rig(g.chamber_c0())
+    try:
+        dims = (10, 8, 6, 4)
+        lo, hi = np.array([-100.0, -80.0, 60.0, -8.0]), np.array([100.0, 80.0, 120.0, 8.0])
+        n = int(np.prod(dims))
+        rng = np.random.default_rng(9)
+        cases = []
+        v = np.full((2, n), 3, np.uint16); v[0, 777] = 9; cases.append(v)
+        v = np.full((2, n), 3, np.uint16); v[1, 100:140] = 5; cases.append(v)
+        v = np.full((2, n), 2, np.uint16); cases.append(v)
+        v = rng.integers(0, 4, (2, n)).astype(np.uint16); cases.append(v)
+        v = rng.integers(0, 30, (2, n)).astype(np.uint16); v[1, 5] = 40; v[0, 6] = 40; cases.append(v)
+        for v in cases:
+            fit_dev = rig.ctx.ia_select_max_paper(torch.from_numpy(v.view(np.int16).copy()).view(torch.uint16).cuda().view(-1),
+                                                  150.0, lo, hi, dims)
+            rig.ctx.synchronize()
+            fg, fo = _fit_to_host(fit_dev), o.select_max_paper(v, lo, hi, dims, 150.0)
+            assert list(fg["value"]) == list(fo.value) and list(fg["error"]) == list(fo.error)
+            assert (fg["vmax"], fg["n_sel"], fg["lambda_sign"], fg["lam"]) == (fo.vmax, fo.n_sel, fo.lambda_sign, fo.lam)
+    finally:
+        rig.close()
