@@ -76,7 +76,9 @@ typedef struct {
  * precision: 64 or 32 = type of the interval endpoints (G22).  flags: bit 0 = vote the dense grid
  * with the general (sign-agnostic) kernel instead of the sign-specialised one (same results; for
  * cross-checks); bits 1 / 2 = force the one-body / three-body variant of the sign-specialised
- * dense kernel (same results; default: picked from the xy cell width); other bits must be 0. */
+ * dense kernel (same results; default: picked from the xy cell width); bit 3 (paper-mode calls only):
+ * the turning angle phi_Ax - phi0 of (A.8d) is taken in [0, 2 pi) instead of (-pi, pi] - tracks of more
+ * than half a turn, PAPER.md L88 (reading M6); other bits must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;

@@ -176,6 +176,7 @@ template <class T> struct HitC {
   T k0, kx, ky;    // S3: cross term  k0 + ky*X + kx*Y
   T mx, my, h2;    // S3: dot term   (X-mx)^2 + (Y-my)^2 - h2
   T d, tol, zref;
+  int full_turn;   // params.flags bit 3 (paper mode only): phi_Ax - phi0 taken in [0, 2 pi) instead of (-pi, pi]
 };
 
 template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const OrcParams& p) {
@@ -194,6 +195,7 @@ template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const Or
   T hx = opaque(T(0.5) * opaque(c.xA - xr)), hy = opaque(T(0.5) * opaque(c.yA - yr));
   c.h2 = opaque(opaque(hx * hx) + opaque(hy * hy));
   c.d = T(h.drift); c.tol = T(p.tol); c.zref = zr;
+  c.full_turn = (p.flags & 8u) ? 1 : 0;
   return c;
 }
 
@@ -458,7 +460,10 @@ __attribute__((noinline)) PointEval dax_point(const HitC<double>& c, double xc, 
   const double cr = (c.k0 + c.ky * xc) + c.kx * yc;
   const double dx = xc - c.mx, dy = yc - c.my;
   const double dt = (dx * dx + dy * dy) - c.h2;
-  const double dphi = std::atan2(cr, dt);
+  double dphi = std::atan2(cr, dt);
+  // reading M6: a counter-clockwise track of less than one turn (L88) has turned by an angle in [0, 2 pi)
+  // when it passes the wire; the principal value is moved there when the caller asks for it
+  if (c.full_turn && dphi < 0.0) dphi = dphi + 6.283185307179586;
   // S3'
   const double iQ = 1.0 / Q, RA = std::sqrt(Q), iR = 1.0 / RA;
   const double c2 = (cA * cA - sA * sA) * iQ;
@@ -825,14 +830,15 @@ int orc_disk_filter(const double* lo, const double* hi, const int32_t* dims, dou
   return ORC_OK;
 }
 
+// which: 0 = the accumulator holding the larger maximum (ties: lambda >= 0); +1 / -1 = that accumulator
 int orc_select_max_paper(const uint16_t* votes, const double* lo, const double* hi, const int32_t* dims, double P,
-                         OrcPaperFit* out) {
+                         int which, OrcPaperFit* out) {
   if (!votes || !lo || !hi || !dims || !out || !(P > 0)) return ORC_ERR_ARG;
   int64_t n = 1;
   for (int d = 0; d < 4; ++d) { if (dims[d] <= 0 || !(hi[d] > lo[d])) return ORC_ERR_ARG; n *= dims[d]; }
   int vmax[2] = {0, 0};
   for (int s = 0; s < 2; ++s) for (int64_t i = 0; i < n; ++i) vmax[s] = std::max(vmax[s], int(votes[s * n + i]));
-  const int s = vmax[1] > vmax[0] ? 1 : 0;
+  const int s = which > 0 ? 0 : (which < 0 ? 1 : (vmax[1] > vmax[0] ? 1 : 0));
   int64_t sum[4] = {0, 0, 0, 0}, kmin[4], kmax[4], cnt = 0;
   for (int d = 0; d < 4; ++d) { kmin[d] = dims[d]; kmax[d] = -1; }
   for (int64_t i = 0; i < n; ++i) {
@@ -879,6 +885,61 @@ int orc_find_hits_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, i
     }
     flags_out[h] = yes ? 1 : 0;
   }
+  return ORC_OK;
+}
+
+// F2e  the iteration scheme, L92-106: n_passes vote passes; pass i votes its grid with the hits found by the
+//      previous pass (L96), selects the maximum-vote voxels (L94) and finds the hits of the next pass on
+//      value -/+ factor*error.  A pass is either a fixed grid [lo, hi] x dims (Table 1, iterations 1-2) or
+//      a window of half-widths `lo` (sic) around the previous pass's value (iteration 3).
+//      "This procedure is applied for each sign of the lambda value" (L78): reading F2e - one chain per
+//      sign of lambda (accumulator s of every pass, hits found with that sign); the sign is decided by
+//      comparing the maxima of the last pass (L121; ties: lambda >= 0).  The reference point stays where
+//      params put it (the update of L98 is the caller's: DESIGN.md).
+struct OrcPaperPass { double lo[4], hi[4]; int32_t dims[4]; int32_t windowed; int32_t pad; };
+
+int orc_track_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
+                    double r_disk, double factor, const OrcPaperPass* passes, int n_passes, OrcPaperFit* fits_out,
+                    int32_t* sign_out) {
+  if (!passes || n_passes < 1 || !fits_out || !sign_out || !(factor > 0)) return ORC_ERR_ARG;
+  if (passes[0].windowed) return ORC_ERR_ARG;
+  for (int s = 0; s < 2; ++s) {
+    std::vector<uint8_t> mask(n_hits, 1);
+    OrcPaperFit prev{};
+    for (int i = 0; i < n_passes; ++i) {
+      double lo[4], hi[4];
+      for (int d = 0; d < 4; ++d) {
+        if (passes[i].windowed) {
+          lo[d] = opaque(prev.value[d] - passes[i].lo[d]);
+          hi[d] = opaque(prev.value[d] + passes[i].lo[d]);
+        } else {
+          lo[d] = passes[i].lo[d];
+          hi[d] = passes[i].hi[d];
+        }
+      }
+      int64_t n = 1;
+      for (int d = 0; d < 4; ++d) n *= passes[i].dims[d];
+      std::vector<uint16_t> votes(2 * n);
+      int rc = orc_vote_paper(wires, n_wires, hits, n_hits, mask.data(), p, P, r_disk, lo, hi, passes[i].dims, nullptr, 0,
+                              votes.data());
+      if (rc) return rc;
+      OrcPaperFit fit;
+      rc = orc_select_max_paper(votes.data(), lo, hi, passes[i].dims, P, s == 0 ? +1 : -1, &fit);
+      if (rc) return rc;
+      fits_out[i * 2 + s] = fit;
+      double blo[4], bhi[4];
+      for (int d = 0; d < 4; ++d) {
+        const double e = opaque(factor * fit.error[d]);
+        blo[d] = opaque(fit.value[d] - e);
+        bhi[d] = opaque(fit.value[d] + e);
+      }
+      rc = orc_find_hits_paper(wires, n_wires, hits, n_hits, p, P, s == 0 ? +1 : -1, blo, bhi, mask.data());
+      if (rc) return rc;
+      prev = fit;
+    }
+  }
+  const OrcPaperFit* last = fits_out + (n_passes - 1) * 2;
+  *sign_out = last[1].vmax > last[0].vmax ? -1 : +1;
   return ORC_OK;
 }
 

@@ -31,7 +31,7 @@ def lib():
         for name in ("orc_prim", "orc_residual", "orc_vote_boxes", "orc_vote", "orc_cell_boxes", "orc_topk",
                      "orc_refine", "orc_refine_batch", "orc_pad_ulps", "orc_max_threads", "orc_dax_point",
                      "orc_residual_paper", "orc_vote_paper", "orc_cell_boxes4", "orc_disk_filter",
-                     "orc_select_max_paper", "orc_find_hits_paper"):
+                     "orc_select_max_paper", "orc_find_hits_paper", "orc_track_paper"):
             getattr(_lib, name).restype = C.c_int
         _lib.orc_set_threads.restype = None
     return _lib
@@ -46,8 +46,8 @@ def _chk(rc, what):
         raise RuntimeError(f"oracle {what} failed: rc={rc}")
 
 
-def make_params(tol, x_ref=0.0, y_ref=0.0, z_ref=0.0, precision=64) -> Params:
-    return Params(tol, x_ref, y_ref, z_ref, precision, 0)
+def make_params(tol, x_ref=0.0, y_ref=0.0, z_ref=0.0, precision=64, flags=0) -> Params:
+    return Params(tol, x_ref, y_ref, z_ref, precision, flags)
 
 
 def wires_of(chamber) -> np.ndarray:
@@ -239,13 +239,13 @@ def disk_filter(lo, hi, dims, r_disk: float, cell_idx=None) -> np.ndarray:
     return out
 
 
-def select_max_paper(votes, lo, hi, dims, P: float) -> PaperFit:
+def select_max_paper(votes, lo, hi, dims, P: float, which: int = 0) -> PaperFit:
     votes = np.ascontiguousarray(votes, np.uint16)
     lo = np.ascontiguousarray(lo, np.float64)
     hi = np.ascontiguousarray(hi, np.float64)
     dims = np.ascontiguousarray(dims, np.int32)
     fit = PaperFit()
-    _chk(lib().orc_select_max_paper(_p(votes), _p(lo), _p(hi), _p(dims), C.c_double(P), C.byref(fit)), "select_max_paper")
+    _chk(lib().orc_select_max_paper(_p(votes), _p(lo), _p(hi), _p(dims), C.c_double(P), int(which), C.byref(fit)), "select_max_paper")
     return fit
 
 
@@ -256,3 +256,28 @@ def find_hits_paper(wires, hits, params: Params, P: float, lambda_sign: int, lo,
     _chk(lib().orc_find_hits_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P),
                                    int(lambda_sign), _p(lo), _p(hi), _p(out)), "find_hits_paper")
     return out
+
+
+PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("pad", "i4")])
+FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), ("lambda_sign", "i4"), ("vmax", "i4"),
+                   ("n_sel", "i8")])
+
+
+def make_passes(spec) -> np.ndarray:
+    """spec: list of ("grid", lo4, hi4, dims4) or ("window", half4, dims4)."""
+    ps = np.zeros(len(spec), PASS_DT)
+    for i, s in enumerate(spec):
+        if s[0] == "grid":
+            ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[2], s[3], 0
+        else:
+            ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[1], s[2], 1
+    return ps
+
+
+def track_paper(wires, hits, params: Params, P: float, r_disk: float, factor: float, passes: np.ndarray):
+    """the paper's iteration scheme, one chain per sign of lambda: (fits [n_passes, 2] of FIT_DT, final sign)."""
+    fits = np.zeros((len(passes), 2), FIT_DT)
+    sign = C.c_int32(0)
+    _chk(lib().orc_track_paper(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), C.c_double(P), C.c_double(r_disk),
+                               C.c_double(factor), _p(passes), len(passes), _p(fits), C.byref(sign)), "track_paper")
+    return fits, int(sign.value)

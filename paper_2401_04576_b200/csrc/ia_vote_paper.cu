@@ -69,7 +69,10 @@ __device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit 
   const double cr = add(add(k0, mul(ky, xc)), mul(kx, yc));
   const double dx = sub(xc, mx_), dy = sub(yc, my_);
   const double dt = sub(add(mul(dx, dx), mul(dy, dy)), h2);
-  o.dphi = atan2(cr, dt);
+  double dphi = atan2(cr, dt);
+  // reading M6 (flags bit 3): turning angle of a counter-clockwise track of less than one turn, in [0, 2 pi)
+  if ((p.flags & 8u) && dphi < 0.0) dphi = add(dphi, 6.283185307179586);
+  o.dphi = dphi;
   o.iQ = __ddiv_rn(1.0, Qp);
   o.RA = __dsqrt_rn(Qp);
   o.iR = __ddiv_rn(1.0, o.RA);

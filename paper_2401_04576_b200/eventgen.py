@@ -325,3 +325,99 @@ def truth_cell(params, lo, hi, dims) -> int:
         k = min(max(k, 0), n - 1)
         idx = idx * n + k
     return idx
+
+
+# ---------------------------------------------------------------------------------------------
+# Paper-shaped workload.  The paper's COMET-like toy chamber is
+# not published; this one has its stated shape: 20 layers between r = 49.6 and 83.7 cm, |tau| = 0.1 rad
+# alternating, length 153.6 cm, 250 wires per layer (5,000 against the paper's 4,986), 1 T.
+# Electrons of 105 MeV/c from the origin: momentum radius P = p/(0.3 B) = 35 cm, R = P/sqrt(1+lambda^2);
+# |lambda| ~ U[0.45, 0.85], random sign (reaches the first three layers, leaves the chamber before one
+# turn: L88), phi ~ U[0, 2 pi), z0 = 0.  A hit = every wire whose 3-D distance of closest approach to
+# the helix, over the arc inside the chamber, is <= 0.8 cm (L88); drift = that distance (+ optional smear).
+# ---------------------------------------------------------------------------------------------
+PAPER_P = 35.0                      # cm: 105 MeV/c in 1 T
+PAPER_DRIFT_MAX = 0.8               # cm
+PAPER_BOX_LO = (-45.0, -45.0, 22.5, -75.0)      # Table 1 (L100-106) in cm: xc, yc, R, z0
+PAPER_BOX_HI = (45.0, 45.0, 37.5, 75.0)
+PAPER_HALF_LEN = 76.8
+
+
+def chamber_paper() -> Chamber:
+    return make_chamber(20, 49.6, (83.7 - 49.6) / 19.0, 250, 0.1, half_len=PAPER_HALF_LEN)
+
+
+def make_track_paper(rng: SplitMix64) -> Track:
+    lam = 0.45 + 0.40 * rng.uniform()
+    if rng.uniform() < 0.5:
+        lam = -lam
+    phi = 2.0 * math.pi * rng.uniform()
+    R = PAPER_P / math.sqrt(1.0 + lam * lam)
+    return Track(R, phi, 0.0, lam)
+
+
+def track_hits_all_wires(trk: Track, ch: Chamber, d_max: float = PAPER_DRIFT_MAX, ds: float = 0.25):
+    """Every wire whose distance of closest approach to the helix, over the arc from the origin to the end
+    plate (or one full turn), is <= d_max.  Coarse scan of the arc in steps of `ds`, then the exact
+    stationarity solve of helix_wire_dca around the best sample of each candidate wire; a wire approached
+    on both the outgoing and the returning arc keeps the smaller distance (the first drift electrons)."""
+    half = float(ch.half_len[0])
+    s_end = 2.0 * math.pi * trk.R
+    if abs(trk.lam) > 0:
+        s_end = min(s_end, (half - math.copysign(trk.z0, trk.lam)) / abs(trk.lam))
+    s = np.arange(0.0, s_end + ds, ds)
+    th = s / trk.R + trk.phi
+    hx, hy, hz = trk.xc + trk.R * np.sin(th), trk.yc - trk.R * np.cos(th), trk.z0 + trk.lam * s
+    T = ch.tan_tau
+    wx, wy = ch.sin_phi_s * T, -ch.cos_phi_s * T
+    wn = np.sqrt(wx * wx + wy * wy + 1.0)
+    ux, uy, uz = wx / wn, wy / wn, 1.0 / wn
+    best_d = np.full(ch.n_wires, np.inf)
+    best_s = np.zeros(ch.n_wires)
+    for i0 in range(0, len(s), 128):                      # chunks keep the temporary at n_wires x 128
+        sl = slice(i0, i0 + 128)
+        qx = hx[None, sl] - ch.x0[:, None]
+        qy = hy[None, sl] - ch.y0[:, None]
+        qz = np.broadcast_to(hz[None, sl], qx.shape)
+        a = qx * ux[:, None] + qy * uy[:, None] + qz * uz[:, None]
+        d2 = qx * qx + qy * qy + qz * qz - a * a
+        k = np.argmin(d2, axis=1)
+        dmin = np.sqrt(np.maximum(d2[np.arange(ch.n_wires), k], 0.0))
+        upd = dmin < best_d
+        best_d[upd] = dmin[upd]
+        best_s[upd] = s[i0 + k[upd]]
+    cand = np.nonzero(best_d < d_max + 2.0 * ds)[0]
+    if len(cand) == 0:
+        return (np.zeros(0, np.int32),) + (np.zeros(0),) * 3
+    d, sp, zw, res, dist = helix_wire_dca(trk, ch, cand, best_s[cand], window=2.0 * ds + 1.0)
+    ok = (dist <= d_max) & (res < 1e-9) & (np.abs(zw) <= half) & (sp >= 0.0) & (sp <= s_end)
+    order = np.argsort(sp[ok], kind="stable")
+    return cand[ok][order].astype(np.int32), d[ok][order], sp[ok][order], zw[ok][order]
+
+
+def make_event_paper(ch: Chamber, seed: int, n_noise: int = 0, smear: float = 0.0, track: Track | None = None) -> Event:
+    """Paper-shaped event: the paper simulates no measurement error (L88: smear = 0 by default) and no noise."""
+    rng = SplitMix64(seed)
+    trk = track if track is not None else make_track_paper(rng)
+    wires, d_true, s_perp, z_wire = track_hits_all_wires(trk, ch)
+    drift = np.empty(len(wires))
+    clipped = np.zeros(len(wires), bool)
+    for i in range(len(wires)):
+        meas = abs(d_true[i]) + (smear * rng.normal() if smear > 0 else 0.0)
+        clipped[i] = meas < 0.0
+        drift[i] = max(meas, 0.0)
+    nz_w, nz_d = [], []
+    for _ in range(n_noise):
+        lay = rng.randint(ch.n_layers)
+        j = rng.randint(ch.wires_per_layer)
+        nz_w.append(lay * ch.wires_per_layer + j)
+        nz_d.append(PAPER_DRIFT_MAX * rng.uniform())
+    nan = np.full(n_noise, np.nan)
+    return Event(
+        chamber=ch, track=trk,
+        wire=np.concatenate([wires, np.array(nz_w, np.int32)]).astype(np.int32),
+        drift=np.concatenate([drift, np.array(nz_d, np.float64)]),
+        is_noise=np.concatenate([np.zeros(len(wires), bool), np.ones(n_noise, bool)]),
+        clipped=np.concatenate([clipped, np.zeros(n_noise, bool)]),
+        d_true=np.concatenate([d_true, nan]), s_perp=np.concatenate([s_perp, nan]),
+        z_wire=np.concatenate([z_wire, nan]), seed=seed)
