@@ -180,6 +180,50 @@ def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
             "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
 
 
+def paper_track_leg(local_rank: int, n_tracks: int = 16):
+    """SURVEY 8(f) f2 + f4: the paper's three-pass scheme (Table 1 in cm) as one ia_track_paper call per track on
+    paper-shaped events (5,000-wire chamber, 105 MeV/c, 19-57 hits); time per track with the hits resident."""
+    import torch
+    from paper_2401_04576_b200 import binding as b
+    ch = g.chamber_paper()
+    ctx = b.Context(local_rank)
+    ctx.ia_load_geometry(b.wires_of(ch))
+    ctx.ia_set_params(0.0, flags=8)
+    lo, hi = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
+    ps = np.zeros(3, b.PASS_DT)
+    ps[0]["lo"], ps[0]["hi"], ps[0]["dims"] = lo, hi, (50, 50, 40, 20)
+    ps[1]["lo"], ps[1]["hi"], ps[1]["dims"] = lo, hi, (90, 90, 40, 20)
+    ps[2]["lo"], ps[2]["hi"], ps[2]["dims"], ps[2]["windowed"] = (2.5, 2.5, 2.5, 40.0), (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20), 1
+    evs = [g.make_event_paper(ch, 500 + i) for i in range(n_tracks)]
+    hds = [ctx.to_device(b.hits_of(e.wire, e.drift)) for e in evs]
+    outs = [ctx.ia_track_paper(hds[0], evs[0].n_hits, g.PAPER_P, ps)]            # warm-up
+    torch.cuda.synchronize()
+    a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.ia_launch_count()
+    a.record(ctx.stream)
+    outs = [ctx.ia_track_paper(hd, e.n_hits, g.PAPER_P, ps) for hd, e in zip(hds, evs)]
+    c.record(ctx.stream)
+    c.synchronize()
+    ms = a.elapsed_time(c) / n_tracks
+    launches = (ctx.ia_launch_count() - l0) // n_tracks
+    dev, sign_ok = [], 0
+    for (fits, sign), e in zip(outs, evs):
+        f = np.frombuffer(fits.cpu().numpy().tobytes(), dtype=b.FIT_DT).reshape(3, 2)
+        s = int(sign.cpu().numpy()[0])
+        sign_ok += s == (1 if e.track.lam >= 0 else -1)
+        dev.append(np.abs(np.array(f[2, 0 if s > 0 else 1]["value"]) - np.array(e.track.params[:4])))
+    dev = np.array(dev)
+    ctx.close()
+    return {"workload": "f2/f4: paper-shaped chamber (20 layers x 250 wires, r 49.6-83.7 cm, tau +/-0.1), 105 MeV/c tracks from the "
+                        "origin, noise-free hits (L88); passes 50x50x40x20, 90x90x40x20 (global), 50x50x50x20 (window), both "
+                        "lambda-sign chains",
+            "ms_per_track": ms, "tracks_per_s": 1e3 / ms, "launches_per_track": int(launches), "n_tracks": n_tracks,
+            "lambda_sign_correct": sign_ok / n_tracks,
+            "median_abs_dev_cm": {"xc": float(np.median(dev[:, 0])), "yc": float(np.median(dev[:, 1])),
+                                  "R": float(np.median(dev[:, 2])), "z0": float(np.median(dev[:, 3]))},
+            "context": "paper: about 1.2 s per track on 4 x K80, about 0.2 s on V100 (L117)"}
+
+
 def run_c3(args, rank, world, local_rank, barrier):
     """--workload C3: one step = ia_refine_batch over 1024 events (BASELINE.json configs[3]); for profiling the
     batch path on its own.  Same JSON shape; value = cell-hit evaluations/s, events/s beside it."""
@@ -251,7 +295,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1", "F2"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
@@ -279,6 +323,18 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.workload == "F2":
+        barrier()
+        r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1))
+        if rank == 0:
+            print(json.dumps({"metric": "paper-scheme tracks/s", "value": r["tracks_per_s"] * world, "unit": "tracks/s",
+                              "n_gpus": world, "steps": args.steps, "warmup": 1, "ms_per_step": r["ms_per_track"],
+                              "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                              "data": "synthetic", "config": {"workload": r["workload"]},
+                              "gpu_launches": r["launches_per_track"] * r["n_tracks"], "paper_track": r}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if args.workload == "F1":
         # paper mode alone (for profiling): same JSON shape, value = voxel-hit evaluations/s
         barrier()
@@ -454,6 +510,10 @@ def main():
             line["paper_mode"] = paper_mode_leg(local_rank, steps=5)
         except Exception as exc:  # pragma: no cover
             line["paper_mode"] = {"error": str(exc)}
+        try:
+            line["paper_track"] = paper_track_leg(local_rank)
+        except Exception as exc:  # pragma: no cover
+            line["paper_track"] = {"error": str(exc)}
 
     print(json.dumps(line))
     ctx.close()

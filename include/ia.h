@@ -152,9 +152,10 @@ typedef struct {
  * the voxels of that accumulator whose count equals vmax,
  *   value_d = lo_d + ((2 sum k_d + n)/(2 n)) * w_d,   error_d = 0.5 * ((max k_d - min k_d + 1) * w_d),
  * w_d = (hi_d - lo_d)/n_d - integer sums, round-to-nearest unfused arithmetic, independent of any order.
- * fit_out_dev: DEVICE pointer. */
+ * fit_out_dev: DEVICE pointer.
+ * which: 0 = the accumulator holding the larger maximum (ties: lambda >= 0), +1 / -1 = that accumulator. */
 int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_radius, const double box_lo[4],
-                        const double box_hi[4], const int32_t grid_dims[4], ia_paper_fit* fit_out_dev);
+                        const double box_hi[4], const int32_t grid_dims[4], int which, ia_paper_fit* fit_out_dev);
 
 /* L96: "An multidimensional interval is constructed.  Its central value is given by the parameter values ...
  * and its radius is given by their errors multiplied by a factor of 5 ... One hit is selected when the
@@ -164,6 +165,26 @@ int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_
  * ia_select_max_paper), so that no host round trip separates the two calls. */
 int ia_find_hits_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, const ia_paper_fit* fit_dev,
                        double factor, uint8_t* flags_out_dev);
+
+/* f2 - the paper's iteration scheme as one call, nothing returning to the host in between.
+ * A pass is a fixed grid [lo, hi] x dims (Table 1, iterations 1-2) or, windowed != 0, a window of half-widths
+ * lo[0..3] around the value found by the previous pass (iteration 3; hi is ignored).  Pass i votes its grid
+ * (ia_vote_paper, disk pre-filter r_disk) with the hits found by pass i-1 - all hits for the first pass -,
+ * selects the maximum-vote voxels (ia_select_max_paper) and finds the hits for the next pass on
+ * value -/+ factor*error (ia_find_hits_paper; "all hits are always considered for the hit finding", L96).
+ * "This procedure is applied for each sign of the lambda value" (L78): one chain per sign (reading F2e) -
+ * fits_out_dev[pass][s], s = 0: lambda >= 0, 1: lambda < 0 - and sign_out_dev = +1 / -1 = the sign whose last
+ * pass has the larger maximum (L121; ties: +1).  The reference point is the one of ia_set_params throughout
+ * (the update of L98 is left to the caller).  passes_host: HOST; fits_out_dev (2*n_passes), sign_out_dev: DEVICE.
+ * Windows are expected to stay inside R > 0.  The first pass must be a fixed grid. */
+typedef struct {
+  double lo[4], hi[4];
+  int32_t dims[4];
+  int32_t windowed;
+  int32_t _pad;
+} ia_paper_pass;
+int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, double r_disk, double factor,
+                   const ia_paper_pass* passes_host, int n_passes, ia_paper_fit* fits_out_dev, int32_t* sign_out_dev);
 
 /* a7 - the k largest entries by key (votes descending, index ascending) (L94, G16):
  * idx_out_dev[k] (int64 linear indices), votes_out_dev[k].  1 <= k <= min(n_cells, IA_MAX_K). */

@@ -23,9 +23,10 @@ HIT_DT = np.dtype([("wire", "i4"), ("_pad", "i4"), ("drift", "f8")])
 BOX_DT = np.dtype([("lo", "f8", (5,)), ("hi", "f8", (5,)), ("votes", "u2"), ("_pad", "u2", (3,))])
 FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), ("lambda_sign", "i4"), ("vmax", "i4"),
                    ("n_sel", "i8")])
+PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("_pad", "i4")])
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 88
 
-EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_topk",
+EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
@@ -62,7 +63,8 @@ def load_library(path: str = LIB_PATH):
     lib.ia_vote.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_vote_boxes.argtypes = [vp, vp, i32, vp, vp, i64, vp]
     lib.ia_vote_paper.argtypes = [vp, vp, i32, vp, dbl, dbl, vp, vp, vp, vp]
-    lib.ia_select_max_paper.argtypes = [vp, vp, dbl, vp, vp, vp, vp]
+    lib.ia_select_max_paper.argtypes = [vp, vp, dbl, vp, vp, vp, i32, vp]
+    lib.ia_track_paper.argtypes = [vp, vp, i32, dbl, dbl, dbl, vp, i32, vp, vp]
     lib.ia_find_hits_paper.argtypes = [vp, vp, i32, dbl, vp, dbl, vp]
     lib.ia_topk.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.ia_refine.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
@@ -210,14 +212,28 @@ class Context:
         return votes_out.view(2, n)
 
     # ---- f2 pieces: maximum-vote selection (device-resident result) and hit finding
-    def ia_select_max_paper(self, votes_dev, momentum_radius, box_lo, box_hi, grid_dims, fit_out=None):
+    def ia_select_max_paper(self, votes_dev, momentum_radius, box_lo, box_hi, grid_dims, fit_out=None, which=0):
         torch = self._torch
         lo, hi, dims = _host4(box_lo, np.float64), _host4(box_hi, np.float64), _host4(grid_dims, np.int32)
         if fit_out is None:
             fit_out = self._empty(FIT_DT.itemsize, torch.uint8)
         self._chk(self.lib.ia_select_max_paper(self.h, _dp(votes_dev), float(momentum_radius), _hp(lo), _hp(hi), _hp(dims),
-                                               _dp(fit_out)), "ia_select_max_paper")
+                                               int(which), _dp(fit_out)), "ia_select_max_paper")
         return fit_out
+
+    def ia_track_paper(self, hits_dev, n_hits, momentum_radius, passes: np.ndarray, r_disk=10.0, factor=5.0, fits_out=None,
+                       sign_out=None):
+        """passes: PASS_DT array (host).  Returns (fits uint8 tensor holding [n_passes][2] FIT_DT, sign int32 tensor),
+        both on the device; nothing is synchronised."""
+        torch = self._torch
+        passes = np.ascontiguousarray(passes, PASS_DT)
+        if fits_out is None:
+            fits_out = self._empty(2 * len(passes) * FIT_DT.itemsize, torch.uint8)
+        if sign_out is None:
+            sign_out = self._empty(1, torch.int32)
+        self._chk(self.lib.ia_track_paper(self.h, _dp(hits_dev), n_hits, float(momentum_radius), float(r_disk), float(factor),
+                                          _hp(passes), len(passes), _dp(fits_out), _dp(sign_out)), "ia_track_paper")
+        return fits_out, sign_out
 
     def ia_find_hits_paper(self, hits_dev, n_hits, momentum_radius, fit_dev, factor=5.0, flags_out=None):
         torch = self._torch

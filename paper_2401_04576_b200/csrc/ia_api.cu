@@ -244,18 +244,20 @@ int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t
   if (rc) return rc;
   if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
   DeviceGuard guard(ctx->device);
-  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, g, votes_out_dev));
+  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}};
+  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, pg, votes_out_dev));
   return IA_OK;
 }
 
 int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_radius, const double box_lo[4],
-                        const double box_hi[4], const int32_t grid_dims[4], ia_paper_fit* fit_out_dev) {
-  if (!ctx || !votes_dev || !fit_out_dev || !(momentum_radius > 0.0)) return IA_ERR_ARG;
+                        const double box_hi[4], const int32_t grid_dims[4], int which, ia_paper_fit* fit_out_dev) {
+  if (!ctx || !votes_dev || !fit_out_dev || !(momentum_radius > 0.0) || which < -1 || which > 1) return IA_ERR_ARG;
   GridDesc g;
   int rc = make_grid4(box_lo, box_hi, grid_dims, g);
   if (rc) return rc;
   DeviceGuard guard(ctx->device);
-  IA_CUDA(ctx, launch_select_max_paper(ctx, votes_dev, g, momentum_radius, fit_out_dev));
+  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}};
+  IA_CUDA(ctx, launch_select_max_paper(ctx, votes_dev, pg, momentum_radius, which, fit_out_dev));
   return IA_OK;
 }
 
@@ -267,6 +269,54 @@ int ia_find_hits_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double m
   if (!(momentum_radius > 0.0) || !(factor > 0.0) || !std::isfinite(factor)) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_find_hits_paper(ctx, hits_dev, n_hits, momentum_radius, fit_dev, factor, flags_out_dev));
+  return IA_OK;
+}
+
+int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, double r_disk, double factor,
+                   const ia_paper_pass* passes_host, int n_passes, ia_paper_fit* fits_out_dev, int32_t* sign_out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits <= 0 || !hits_dev || !passes_host || n_passes < 1 || !fits_out_dev || !sign_out_dev) return IA_ERR_ARG;
+  if (!(momentum_radius > 0.0) || !(factor > 0.0) || std::isnan(r_disk) || passes_host[0].windowed) return IA_ERR_ARG;
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  std::vector<PaperGrid> grids(n_passes);
+  int64_t max_cells = 0;
+  for (int i = 0; i < n_passes; ++i) {
+    const ia_paper_pass& ps = passes_host[i];
+    if (ps.windowed) {
+      // dims only; lo/hi are placeholders that make_grid4 accepts, the kernels rebuild them from the centre
+      const double zero[4] = {0, 0, 0, 0}, one[4] = {1, 1, 1, 1};
+      rc = make_grid4(zero, one, ps.dims, grids[i].g);
+      for (int d = 0; d < 4; ++d) {
+        if (!(ps.lo[d] > 0.0) || !std::isfinite(ps.lo[d])) return IA_ERR_ARG;
+        grids[i].half[d] = ps.lo[d];
+      }
+    } else {
+      rc = make_grid4(ps.lo, ps.hi, ps.dims, grids[i].g);
+      if (!rc && !(ps.lo[2] > 0.0)) rc = IA_ERR_DOMAIN;
+    }
+    if (rc) return rc;
+    grids[i].centre = nullptr;
+    max_cells = std::max(max_cells, grids[i].g.cells);
+  }
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, scratch_reserve(ctx->votes, size_t(2) * max_cells * sizeof(uint16_t)));
+  IA_CUDA(ctx, scratch_reserve(ctx->misc, size_t(2) * n_hits));
+  uint16_t* votes = static_cast<uint16_t*>(ctx->votes.p);
+  uint8_t* mask[2] = {static_cast<uint8_t*>(ctx->misc.p), static_cast<uint8_t*>(ctx->misc.p) + n_hits};
+  for (int i = 0; i < n_passes; ++i) {
+    for (int s = 0; s < 2; ++s) {
+      PaperGrid pg = grids[i];
+      if (passes_host[i].windowed) pg.centre = fits_out_dev + (i - 1) * 2 + s;
+      ia_paper_fit* fit = fits_out_dev + i * 2 + s;
+      // the first pass is the same vote for both chains (all hits, fixed grid): voted once
+      if (i > 0 || s == 0)
+        IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, i == 0 ? nullptr : mask[s], momentum_radius, r_disk, pg, votes));
+      IA_CUDA(ctx, launch_select_max_paper(ctx, votes, pg, momentum_radius, s == 0 ? +1 : -1, fit));
+      IA_CUDA(ctx, launch_find_hits_paper(ctx, hits_dev, n_hits, momentum_radius, fit, factor, mask[s]));
+    }
+  }
+  IA_CUDA(ctx, launch_paper_sign(ctx, fits_out_dev + (n_passes - 1) * 2, sign_out_dev));
   return IA_OK;
 }
 

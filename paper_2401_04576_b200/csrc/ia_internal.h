@@ -85,13 +85,20 @@ cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& span, int lev,
                                       ia_box* boxes, int* n_splits_out, uint16_t** partial_out);
 cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out);
 
-// paper-mode vote (ia_vote_paper.cu): 4-D grid in g (axis 4 unused, n = 1), votes_out [2][cells]
+// paper mode (ia_vote_paper.cu).  PaperGrid: a fixed 4-D grid in g (axis 4 unused, n = 1), or - centre != nullptr -
+// a window of half-widths `half` around a fit on the device (g then carries only the dims)
+struct PaperGrid {
+  GridDesc g;
+  const ia_paper_fit* centre;
+  double half[4];
+};
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const GridDesc& g, uint16_t* votes_out);
-// pieces of the paper's iteration scheme (f2): maximum-vote selection and hit finding
-cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const GridDesc& g, double P, ia_paper_fit* fit_out);
+                              const PaperGrid& pg, uint16_t* votes_out);          // votes_out [2][cells]
+cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const PaperGrid& pg, double P, int which,
+                                    ia_paper_fit* fit_out);
 cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const ia_paper_fit* fit, double factor,
                                    uint8_t* flags_out);
+cudaError_t launch_paper_sign(ia_ctx* ctx, const ia_paper_fit* last, int32_t* sign_out);
 
 // FP64 pipe probe (roofline denominator check): blocks x 256 threads x 8 chains x iters instructions
 cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, double* sink);

@@ -125,6 +125,22 @@ IA_DEV bool dax_point(const PHit& h, double R, double Zr, double lam, double D, 
 
 constexpr int PAPER_THREADS = 256;
 
+// a fixed grid, or (centre != nullptr) a window of half-widths `half` around a fit that lives on the device:
+// lo = value - half, hi = value + half, w = (hi - lo)/n - the operations of make_grid, done by every kernel
+// that needs the grid, so that a pass can be enqueued before the previous one has produced its centre
+IA_DEV GridDesc resolve_grid(const PaperGrid& pg) {
+  GridDesc g = pg.g;
+  if (pg.centre) {
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      g.lo[d] = sub(pg.centre->value[d], pg.half[d]);
+      g.hi[d] = add(pg.centre->value[d], pg.half[d]);
+      g.w[d] = __ddiv_rn(sub(g.hi[d], g.lo[d]), double(g.n[d]));
+    }
+  }
+  return g;
+}
+
 // M3-M5 for one (voxel, hit, lambda): does either drift sign contain 0 ?
 IA_DEV bool paper_hit_votes(const PHit& ph, Iv<double> R, double Rm, double Zr, double l, bool two_ends) {
   bool yes = false;
@@ -158,10 +174,11 @@ IA_DEV bool disk_passes(Iv<double> X, Iv<double> Y, Iv<double> R, double r_disk)
 
 __global__ void __launch_bounds__(PAPER_THREADS)
 vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __restrict__ hit_mask,
-                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, GridDesc g, int* status,
+                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, PaperGrid pg, int* status,
                   uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PHit* sh = reinterpret_cast<PHit*>(smem_raw);
+  const GridDesc g = resolve_grid(pg);
   const int ixy = blockIdx.x;
   const int ix = ixy / g.n[1], iy = ixy - ix * g.n[1];
   const Iv<double> X = {cell_edge(g.lo[0], g.hi[0], g.w[0], ix, g.n[0]), cell_edge(g.lo[0], g.hi[0], g.w[0], ix + 1, g.n[0])};
@@ -220,8 +237,12 @@ __global__ void paper_max_kernel(const uint16_t* __restrict__ votes, int64_t n, 
   }
 }
 
-__global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t n, GridDesc g, unsigned long long* __restrict__ acc) {
-  const int s = acc[1] > acc[0] ? 1 : 0;                 // equal maxima: lambda >= 0 wins
+// which: 0 = the accumulator with the larger maximum (equal maxima: lambda >= 0 wins), +1 / -1 = that accumulator
+IA_DEV int pick_acc(const unsigned long long* acc, int which) { return which > 0 ? 0 : (which < 0 ? 1 : (acc[1] > acc[0] ? 1 : 0)); }
+
+__global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t n, GridDesc g, int which,
+                                     unsigned long long* __restrict__ acc) {
+  const int s = pick_acc(acc, which);
   const unsigned vmax = unsigned(acc[s]);
   const uint16_t* v = votes + int64_t(s) * n;
   for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
@@ -239,9 +260,11 @@ __global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t
   }
 }
 
-__global__ void paper_fit_kernel(const unsigned long long* __restrict__ acc, GridDesc g, double P, ia_paper_fit* __restrict__ out) {
+__global__ void paper_fit_kernel(const unsigned long long* __restrict__ acc, PaperGrid pg, double P, int which,
+                                 ia_paper_fit* __restrict__ out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  const int s = acc[1] > acc[0] ? 1 : 0;
+  const GridDesc g = resolve_grid(pg);
+  const int s = pick_acc(acc, which);
   const unsigned long long cnt = acc[2];
   ia_paper_fit f;
   for (int d = 0; d < 4; ++d) {
@@ -284,7 +307,8 @@ __global__ void find_hits_paper_kernel(const ia_hit* __restrict__ hits, int n_hi
 }  // namespace
 
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const GridDesc& g, uint16_t* votes_out) {
+                              const PaperGrid& pg, uint16_t* votes_out) {
+  const GridDesc& g = pg.g;
   const size_t smem = size_t(n_hits) * sizeof(PHit);
   cudaError_t err = cudaFuncSetAttribute(vote_paper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
   if (err != cudaSuccess) return err;
@@ -292,22 +316,23 @@ cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const
   int threads = PAPER_THREADS;
   if (col < threads) threads = (col + 31) / 32 * 32;
   vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, hit_mask, ctx->wires, ctx->n_wires,
-                                                                              ctx->params, P, r_disk, g, ctx->status, votes_out);
+                                                                              ctx->params, P, r_disk, pg, ctx->status, votes_out);
   ctx->launches++;
   return cudaGetLastError();
 }
 
-cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const GridDesc& g, double P, ia_paper_fit* fit_out) {
+cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const PaperGrid& pg, double P, int which,
+                                    ia_paper_fit* fit_out) {
   cudaError_t err = scratch_reserve(ctx->keys, 16 * sizeof(unsigned long long));
   if (err != cudaSuccess) return err;
   unsigned long long* acc = static_cast<unsigned long long*>(ctx->keys.p);
   paper_init_kernel<<<1, 32, 0, ctx->stream>>>(acc);
-  const int64_t n = g.cells;
+  const int64_t n = pg.g.cells;
   int blocks = int((n + 1023) / 1024);
   if (blocks > 1184) blocks = 1184;
   paper_max_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, acc);
-  paper_moments_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, g, acc);
-  paper_fit_kernel<<<1, 32, 0, ctx->stream>>>(acc, g, P, fit_out);
+  paper_moments_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, pg.g, which, acc);   // cell indices only: dims suffice
+  paper_fit_kernel<<<1, 32, 0, ctx->stream>>>(acc, pg, P, which, fit_out);
   ctx->launches += 4;
   return cudaGetLastError();
 }
@@ -317,6 +342,18 @@ cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, 
   if (n_hits <= 0) return cudaSuccess;
   find_hits_paper_kernel<<<(n_hits + 63) / 64, 64, 0, ctx->stream>>>(hits, n_hits, ctx->wires, ctx->n_wires, ctx->params, P, fit,
                                                                     factor, ctx->status, flags_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+namespace {
+__global__ void paper_sign_kernel(const ia_paper_fit* __restrict__ last, int32_t* __restrict__ sign_out) {
+  if (threadIdx.x == 0) *sign_out = last[1].vmax > last[0].vmax ? -1 : 1;      // L121; ties: lambda >= 0
+}
+}  // namespace
+
+cudaError_t launch_paper_sign(ia_ctx* ctx, const ia_paper_fit* last, int32_t* sign_out) {
+  paper_sign_kernel<<<1, 32, 0, ctx->stream>>>(last, sign_out);
   ctx->launches++;
   return cudaGetLastError();
 }

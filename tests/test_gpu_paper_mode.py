@@ -186,3 +186,75 @@ def test_f2_selection_special_cases_on_device():
             assert (fg["vmax"], fg["n_sel"], fg["lambda_sign"], fg["lam"]) == (fo.vmax, fo.n_sel, fo.lambda_sign, fo.lam)
     finally:
         rig.close()
+
+
+# ---- the iteration scheme as one call (f2) on the paper-shaped workload (f4) ------------------------------------------
+PLO, PHI = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
+
+
+def _passes(spec):
+    ps = np.zeros(len(spec), b.PASS_DT)
+    for i, s in enumerate(spec):
+        if s[0] == "grid":
+            ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[2], s[3], 0
+        else:
+            ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[1], s[2], 1
+    return ps
+
+
+def _fits_to_host(t, n_passes):
+    return np.frombuffer(t.cpu().numpy().tobytes(), dtype=b.FIT_DT).reshape(n_passes, 2)
+
+
+def test_track_paper_matches_the_oracle_chain():
+    """ia_track_paper against orc_track_paper on reduced grids (the oracle needs seconds per pass): every fit of every
+    pass and both chains identical, same final sign.  Tracks of more than half a turn (flags bit 3)."""
+    ch = g.chamber_paper()
+    rig = Rig(ch)
+    try:
+        spec = [("grid", PLO, PHI, (24, 24, 16, 10)), ("grid", PLO, PHI, (36, 36, 16, 10)),
+                ("window", (3.0, 3.0, 2.0, 30.0), (20, 20, 16, 10))]
+        for seed in (300, 301, 302):
+            ev = g.make_event_paper(ch, seed, n_noise=3)
+            hd, oh = rig.hits(ev.wire, ev.drift)
+            rig.ctx.ia_set_params(0.01, flags=8)
+            fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec), r_disk=10.0, factor=5.0)
+            rig.ctx.synchronize()
+            fg = _fits_to_host(fits_dev, len(spec))
+            fo, so = o.track_paper(rig.owires, oh, o.make_params(0.01, flags=8), g.PAPER_P, 10.0, 5.0, o.make_passes(spec))
+            assert int(sign_dev.cpu().numpy()[0]) == so
+            for name in ("value", "error", "lam", "lambda_sign", "vmax", "n_sel"):
+                assert (fg[name] == fo[name]).all(), (seed, name, fg[name], fo[name])
+    finally:
+        rig.close()
+
+
+def test_track_paper_recovers_the_generated_helix():
+    """Table 1 of the paper in cm (L100-106): two global passes (voxels 1.8 x 1.8 x 0.375 x 7.5 and 1.0 x 1.0 x 0.375 x 7.5
+    cm) and a window of +/-2.5, 2.5, 2.5, 40 cm with voxels 0.1 x 0.1 x 0.1 x 4 cm, on noise-free paper-shaped events
+    (L88).  Measured, then asserted loosely: the sign of lambda and the helix within a few final voxels."""
+    ch = g.chamber_paper()
+    rig = Rig(ch)
+    try:
+        spec = [("grid", PLO, PHI, (50, 50, 40, 20)), ("grid", PLO, PHI, (90, 90, 40, 20)),
+                ("window", (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20))]
+        rig.ctx.ia_set_params(0.0, flags=8)
+        ok_sign, dev = 0, []
+        seeds = range(400, 424)
+        for seed in seeds:
+            ev = g.make_event_paper(ch, seed)
+            hd, _ = rig.hits(ev.wire, ev.drift)
+            fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec))
+            rig.ctx.synchronize()
+            fg = _fits_to_host(fits_dev, 3)
+            s = int(sign_dev.cpu().numpy()[0])
+            ok_sign += s == (1 if ev.track.lam >= 0 else -1)
+            f = fg[2, 0 if s > 0 else 1]
+            dev.append(np.abs(np.array(f["value"]) - np.array(ev.track.params[:4])))
+        dev = np.array(dev)
+        assert ok_sign >= len(seeds) - 1, ok_sign
+        good = (dev[:, :3] < 0.3).all(axis=1) & (dev[:, 3] < 4.0)
+        assert good.mean() >= 0.9, (good.mean(), np.median(dev, axis=0))
+        assert (np.median(dev, axis=0) < np.array([0.1, 0.1, 0.1, 2.0])).all(), np.median(dev, axis=0)
+    finally:
+        rig.close()
