@@ -133,3 +133,89 @@ def test_f2c_hit_finding_and_hit_mask():
         vf = o.vote_paper(wires, hits, p, P, LO4, HI4, dims)
         keep = o.disk_filter(LO4, HI4, dims, 10.0)
         assert (vd[:, keep == 1] == vf[:, keep == 1]).all() and (vd[:, keep == 0] == 0).all()
+
+
+# ---- paper-shaped workload (8(f) f4), full-turn branch (M6) and the chain (F2e) ----------------------------------------
+def test_paper_shaped_generator_against_brute_force():
+    """every hit of make_event_paper is a stationary point of the wire-helix distance with DCA <= 0.8 cm, and a dense
+    scan of the arc (independent of the generator's candidate search) finds no wire it missed and no closer approach."""
+    ch = g.chamber_paper()
+    assert ch.n_wires == 5000 and abs(ch.radius[0] - 49.6) < 1e-12 and abs(ch.radius[-1] - 83.7) < 1e-9
+    counts = []
+    for seed in (0, 1, 2, 3):
+        ev = g.make_event_paper(ch, seed)
+        trk = ev.track
+        assert abs(trk.R * np.sqrt(1 + trk.lam ** 2) - g.PAPER_P) < 1e-12 and trk.z0 == 0.0
+        assert 0.45 <= abs(trk.lam) <= 0.85
+        counts.append(ev.n_hits)
+        assert (ev.drift <= g.PAPER_DRIFT_MAX).all() and (np.abs(ev.z_wire) <= g.PAPER_HALF_LEN).all()
+        assert len(set(ev.wire.tolist())) == ev.n_hits
+        # dense scan, 0.02 cm steps
+        s_end = min(2 * np.pi * trk.R, g.PAPER_HALF_LEN / abs(trk.lam))
+        s = np.arange(0.0, s_end, 0.02)
+        th = s / trk.R + trk.phi
+        hx, hy, hz = trk.xc + trk.R * np.sin(th), trk.yc - trk.R * np.cos(th), trk.lam * s
+        T = ch.tan_tau
+        wx, wy = ch.sin_phi_s * T, -ch.cos_phi_s * T
+        wn = np.sqrt(wx * wx + wy * wy + 1)
+        dmin = np.full(ch.n_wires, np.inf)
+        for i0 in range(0, len(s), 500):
+            sl = slice(i0, i0 + 500)
+            qx, qy = hx[None, sl] - ch.x0[:, None], hy[None, sl] - ch.y0[:, None]
+            qz = np.broadcast_to(hz[None, sl], qx.shape)
+            a = (qx * wx[:, None] + qy * wy[:, None] + qz) / wn[:, None]
+            dmin = np.minimum(dmin, np.sqrt(np.maximum(qx * qx + qy * qy + qz * qz - a * a, 0)).min(axis=1))
+        hit = np.zeros(ch.n_wires, bool)
+        hit[ev.wire] = True
+        # the scan (step 0.02 cm along the arc) can only be above the DCA, by at most the half step in quadrature
+        assert (dmin[ev.wire] >= ev.drift - 1e-9).all()
+        assert (dmin[ev.wire] <= np.sqrt(ev.drift ** 2 + 0.011 ** 2)).all()
+        missed = np.nonzero(~hit & (dmin < g.PAPER_DRIFT_MAX - 5e-3))[0]
+        # a wire can be missed only if its closest approach lies beyond the end plate (|z on the wire| > half length)
+        assert len(missed) <= 2, (seed, missed, dmin[missed])
+    assert 15 <= min(counts) and max(counts) <= 65
+
+
+def test_m6_full_turn_branch_truth_voxel():
+    """tracks of more than half a turn (paper-shaped): with the turning angle in [0, 2 pi) (flags bit 3) the truth voxel
+    (+-0.5 mm) receives every hit, tol = 0; with the principal value it loses the hits of the returning arc."""
+    ch = g.chamber_paper()
+    wires = o.wires_of(ch)
+    got = {0: 0, 8: 0}
+    tot = 0
+    for seed in range(8):
+        ev = g.make_event_paper(ch, seed)
+        xc, yc, R, z0, lam = ev.track.params
+        c, hw = np.array([xc, yc, R, z0]), np.array([0.05, 0.05, 0.05, 0.5])
+        hits = o.hits_of(ev.wire, ev.drift)
+        tot += ev.n_hits
+        assert (ev.s_perp / R).max() > np.pi                     # the workload does reach beyond half a turn
+        for flags in (0, 8):
+            v = o.vote_paper(wires, hits, o.make_params(0.0, flags=flags), g.PAPER_P, c - hw, c + hw, (1, 1, 1, 1))
+            got[flags] += int(v[0 if lam >= 0 else 1, 0])
+    assert got[8] == tot and got[0] < 0.8 * tot
+
+
+def test_f2e_chain_is_the_composition_of_its_pinned_pieces():
+    """orc_track_paper = vote (masked, disk filter) -> select (per sign) -> find hits -> next pass, recomputed here from the
+    individually pinned calls on a small schedule; final sign = larger last maximum."""
+    ch = g.chamber_paper()
+    wires = o.wires_of(ch)
+    p = o.make_params(0.01, flags=8)
+    ev = g.make_event_paper(ch, 5, n_noise=4)
+    hits = o.hits_of(ev.wire, ev.drift)
+    lo, hi = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
+    spec = [("grid", lo, hi, (12, 12, 8, 6)), ("window", (8.0, 8.0, 3.0, 30.0), (10, 10, 8, 6))]
+    fits, sign = o.track_paper(wires, hits, p, g.PAPER_P, 10.0, 5.0, o.make_passes(spec))
+    for s, which in ((0, +1), (1, -1)):
+        v = o.vote_paper(wires, hits, p, g.PAPER_P, lo, hi, spec[0][3], r_disk=10.0)
+        f0 = o.select_max_paper(v, lo, hi, spec[0][3], g.PAPER_P, which)
+        assert list(f0.value) == list(fits[0, s]["value"]) and f0.vmax == fits[0, s]["vmax"] and f0.n_sel == fits[0, s]["n_sel"]
+        val, err = np.array(f0.value), np.array(f0.error)
+        mask = o.find_hits_paper(wires, hits, p, g.PAPER_P, which, val - 5.0 * err, val + 5.0 * err)
+        half = np.array(spec[1][1])
+        v1 = o.vote_paper(wires, hits, p, g.PAPER_P, val - half, val + half, spec[1][2], hit_mask=mask, r_disk=10.0)
+        f1 = o.select_max_paper(v1, val - half, val + half, spec[1][2], g.PAPER_P, which)
+        assert list(f1.value) == list(fits[1, s]["value"]) and list(f1.error) == list(fits[1, s]["error"])
+        assert f1.vmax == fits[1, s]["vmax"] and f1.lambda_sign == which
+    assert sign == (-1 if fits[1, 1]["vmax"] > fits[1, 0]["vmax"] else 1)
