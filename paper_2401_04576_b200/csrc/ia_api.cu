@@ -245,7 +245,7 @@ int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t
   if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
   DeviceGuard guard(ctx->device);
   PaperGrid pg = {g, nullptr, {0, 0, 0, 0}};
-  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, pg, votes_out_dev));
+  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, pg, 3, votes_out_dev));
   return IA_OK;
 }
 
@@ -311,7 +311,8 @@ int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momen
       ia_paper_fit* fit = fits_out_dev + i * 2 + s;
       // the first pass is the same vote for both chains (all hits, fixed grid): voted once
       if (i > 0 || s == 0)
-        IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, i == 0 ? nullptr : mask[s], momentum_radius, r_disk, pg, votes));
+        IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, i == 0 ? nullptr : mask[s], momentum_radius, r_disk, pg,
+                                       i == 0 ? 3 : (s == 0 ? 1 : 2), votes));
       IA_CUDA(ctx, launch_select_max_paper(ctx, votes, pg, momentum_radius, s == 0 ? +1 : -1, fit));
       IA_CUDA(ctx, launch_find_hits_paper(ctx, hits_dev, n_hits, momentum_radius, fit, factor, mask[s]));
     }

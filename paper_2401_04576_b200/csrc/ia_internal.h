@@ -93,7 +93,7 @@ struct PaperGrid {
   double half[4];
 };
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const PaperGrid& pg, uint16_t* votes_out);          // votes_out [2][cells]
+                              const PaperGrid& pg, int signs, uint16_t* votes_out);   // votes_out [2][cells]; signs: bit 0 / 1
 cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const PaperGrid& pg, double P, int which,
                                     ia_paper_fit* fit_out);
 cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const ia_paper_fit* fit, double factor,

@@ -174,8 +174,8 @@ IA_DEV bool disk_passes(Iv<double> X, Iv<double> Y, Iv<double> R, double r_disk)
 
 __global__ void __launch_bounds__(PAPER_THREADS)
 vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __restrict__ hit_mask,
-                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, PaperGrid pg, int* status,
-                  uint16_t* __restrict__ votes) {
+                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, PaperGrid pg, int signs,
+                  int* status, uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PHit* sh = reinterpret_cast<PHit*>(smem_raw);
   const GridDesc g = resolve_grid(pg);
@@ -205,8 +205,10 @@ vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __
         const PHit& ph = sh[h];
         if (!ph.valid) continue;
         const double Zr = sub(zm, ph.zref);
-        v[0] += paper_hit_votes(ph, R, Rm, Zr, lam, two_ends) ? 1u : 0u;
-        v[1] += paper_hit_votes(ph, R, Rm, Zr, -lam, two_ends) ? 1u : 0u;
+        // signs: bit 0 = the lambda >= 0 accumulator is wanted, bit 1 = the lambda < 0 one (a chain of
+        // ia_track_paper needs one; the other is written as 0)
+        if (signs & 1) v[0] += paper_hit_votes(ph, R, Rm, Zr, lam, two_ends) ? 1u : 0u;
+        if (signs & 2) v[1] += paper_hit_votes(ph, R, Rm, Zr, -lam, two_ends) ? 1u : 0u;
       }
     }
     const int64_t cell = int64_t(ixy) * (nR * nz) + j;
@@ -307,7 +309,7 @@ __global__ void find_hits_paper_kernel(const ia_hit* __restrict__ hits, int n_hi
 }  // namespace
 
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const PaperGrid& pg, uint16_t* votes_out) {
+                              const PaperGrid& pg, int signs, uint16_t* votes_out) {
   const GridDesc& g = pg.g;
   const size_t smem = size_t(n_hits) * sizeof(PHit);
   cudaError_t err = cudaFuncSetAttribute(vote_paper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
@@ -316,7 +318,7 @@ cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const
   int threads = PAPER_THREADS;
   if (col < threads) threads = (col + 31) / 32 * 32;
   vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, hit_mask, ctx->wires, ctx->n_wires,
-                                                                              ctx->params, P, r_disk, pg, ctx->status, votes_out);
+                                                                              ctx->params, P, r_disk, pg, signs, ctx->status, votes_out);
   ctx->launches++;
   return cudaGetLastError();
 }
