@@ -176,6 +176,7 @@ template <class T> struct HitC {
   T k0, kx, ky;    // S3: cross term  k0 + ky*X + kx*Y
   T mx, my, h2;    // S3: dot term   (X-mx)^2 + (Y-my)^2 - h2
   T d, tol, zref;
+  int rigorous;    // params.flags bit 4: Phi from a verified enclosure of the fixed point of (A.6) (reading f3)
   int full_turn;   // params.flags bit 3 (paper mode only): phi_Ax - phi0 taken in [0, 2 pi) instead of (-pi, pi]
 };
 
@@ -196,6 +197,7 @@ template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const Or
   c.h2 = opaque(opaque(hx * hx) + opaque(hy * hy));
   c.d = T(h.drift); c.tol = T(p.tol); c.zref = zr;
   c.full_turn = (p.flags & 8u) ? 1 : 0;
+  c.rigorous = (p.flags & 16u) ? 1 : 0;
   return c;
 }
 
@@ -238,20 +240,62 @@ template <class T> Resid residual(const Box<T>& b, const HitC<T>& c, int sign) {
   Iv<T> P2 = iscale(half, imul(iadd(isub(t1, t2), t3), iQ));                           // (A.8c)
   Iv<T> T2 = isqr(thin(c.Tn));
   Iv<T> e = iadd(iscale(c.Tn, P1), imul(T2, P2));       // Phi - Phi_Ax  (A.8a)
-  // S5 trig of Phi = Phi_Ax + e  (A.3b), (A.7g)
-  Iv<T> se = isin(e), ce = icos(e);
-  Iv<T> sinP = iclamp(imul(iadd(imul(sA, ce), imul(cA, se)), iR), T(-1), one);
-  Iv<T> cosP = iclamp(imul(isub(imul(cA, ce), imul(sA, se)), iR), T(-1), one);
-  // S6 drift-line norm (A.3a) L160 and delta = d_St / u_d
-  Iv<T> u2 = iadd(iadd(iadd(thin(one), iscale(opaque(two * c.Tn), imul(b.L, sinP))), imul(T2, isqr(b.L))),
-                  imul(T2, isqr(cosP)));
-  Iv<T> u = isqrt(u2);
-  if (!(u.lo > T(0))) return {0.0, 0.0, double(Q.hi), true};
-  Iv<T> dl = idiv_pos(D, u);
-  // S7 z of the wire point (A.4c) L172 with s_perp = R (dphi + e);  c^tau (A.7b) L194
-  Iv<T> z = isub(iadd(Zr, imul(LR, iadd(dphi, e))), iscale(c.Tn, imul(dl, cosP)));
-  Iv<T> Ld = imul(b.L, dl);
-  Iv<T> ct = isub(imul(z, cA), imul(Ld, sA));
+  // S5-S7 as a function of e = Phi - Phi_Ax (they are evaluated once with the series value, or - rigorous mode -
+  // several times inside the verification of the fixed point of (A.6))
+  Iv<T> sinP, cosP, dl, z, Ld, ct;
+  bool u_ok = true;
+  auto s5_to_s7 = [&](Iv<T> ee) {
+    // S5 trig of Phi = Phi_Ax + e  (A.3b), (A.7g)
+    Iv<T> se = isin(ee), ce = icos(ee);
+    sinP = iclamp(imul(iadd(imul(sA, ce), imul(cA, se)), iR), T(-1), one);
+    cosP = iclamp(imul(isub(imul(cA, ce), imul(sA, se)), iR), T(-1), one);
+    // S6 drift-line norm (A.3a) L160 and delta = d_St / u_d
+    Iv<T> u2 = iadd(iadd(iadd(thin(one), iscale(opaque(two * c.Tn), imul(b.L, sinP))), imul(T2, isqr(b.L))),
+                    imul(T2, isqr(cosP)));
+    Iv<T> u = isqrt(u2);
+    if (!(u.lo > T(0))) { u_ok = false; return; }
+    dl = idiv_pos(D, u);
+    // S7 z of the wire point (A.4c) L172 with s_perp = R (dphi + e);  c^tau (A.7b) L194
+    z = isub(iadd(Zr, imul(LR, iadd(dphi, ee))), iscale(c.Tn, imul(dl, cosP)));
+    Ld = imul(b.L, dl);
+    ct = isub(imul(z, cA), imul(Ld, sA));
+  };
+  if (c.rigorous) {
+    // Reading f3 (PAPER.md L187 eq. (A.6) "solved numerically"): e is a fixed point of
+    //   g(e) = atan2( T s^tau(e), R_Ax^2 + T c^tau(e) ),  s^tau = -z s_Ax - lambda delta c_Ax   (A.6), (A.7b,c)
+    // Verification by inflation: start from the series enclosure; if g(E) is inside E, g has a fixed point in
+    // g(E) (Brouwer) - taken as THE solution of (A.6) on this branch - and E := g(E), then once more
+    // E := g(E) meet E.  Otherwise E := hull(E, g(E)) widened by a tenth of its width (+ a small absolute
+    // amount) and again, at most RIG_ROUNDS times; no verification: the hit votes (cannot exclude).
+    const int RIG_ROUNDS = 6;
+    const T tiny = std::is_same<T, float>::value ? T(1e-6) : T(1e-12);
+    auto g_of = [&](Iv<T> ee, Iv<T>& out) -> bool {
+      s5_to_s7(ee);
+      if (!u_ok) return false;
+      Iv<T> st = ineg(iadd(imul(z, sA), imul(Ld, cA)));
+      out = iatan2(iscale(c.Tn, st), iadd(Q, iscale(c.Tn, ct)));
+      return true;
+    };
+    Iv<T> E = e, G;
+    bool verified = false;
+    for (int k = 0; k < RIG_ROUNDS && !verified; ++k) {
+      if (!g_of(E, G)) return {0.0, 0.0, double(Q.hi), true};
+      if (G.lo >= E.lo && G.hi <= E.hi) {
+        verified = true;
+        E = G;
+      } else {
+        const T lo_h = std::min(E.lo, G.lo), hi_h = std::max(E.hi, G.hi);
+        const T pad = up_add(up_mul(T(0.1), up_add(hi_h, -lo_h)), tiny);
+        E = {dn_add(lo_h, -pad), up_add(hi_h, pad)};
+      }
+    }
+    if (!verified) return {0.0, 0.0, double(Q.hi), true};
+    if (!g_of(E, G)) return {0.0, 0.0, double(Q.hi), true};
+    e = {std::max(E.lo, G.lo), std::min(E.hi, G.hi)};
+    if (!(e.lo <= e.hi)) return {0.0, 0.0, double(Q.hi), true};
+  }
+  s5_to_s7(e);
+  if (!u_ok) return {0.0, 0.0, double(Q.hi), true};
   // S8 (R + d_Ax)^2 = radicand of (A.5b) L183;  f = R_Ax^2 - (R + d_Ax)^2  (A.5a) L180
   Iv<T> rad = isub(isub(isub(isqr(iadd(b.R, dl)), iscale(opaque(two * c.Tn), ct)), isqr(iscale(c.Tn, z))),
                    isqr(iscale(c.Tn, Ld)));
