@@ -78,7 +78,10 @@ typedef struct {
  * cross-checks); bits 1 / 2 = force the one-body / three-body variant of the sign-specialised
  * dense kernel (same results; default: picked from the xy cell width); bit 3 (paper-mode calls only):
  * the turning angle phi_Ax - phi0 of (A.8d) is taken in [0, 2 pi) instead of (-pi, pi] - tracks of more
- * than half a turn, PAPER.md L88 (reading M6); other bits must be 0. */
+ * than half a turn, PAPER.md L88 (reading M6); bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
+ * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
+ * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; runs in the
+ * general (sign-agnostic) kernels, about 3 x the arithmetic; other bits must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;

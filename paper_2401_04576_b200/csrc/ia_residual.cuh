@@ -31,8 +31,9 @@ template <class T> struct HitC {
 template <class T> struct HitS {
   T Tn, Dlo, Dhi;
   int valid;
+  int rig;           // params.flags bit 4: rigorous enclosure of Phi (reading f3), carried in HitC::_pad
 };
-template <class T> IA_DEV HitS<T> hit_small(const HitC<T>& c) { return {c.Tn, c.Dlo, c.Dhi, c.valid}; }
+template <class T> IA_DEV HitS<T> hit_small(const HitC<T>& c) { return {c.Tn, c.Dlo, c.Dhi, c.valid, c._pad}; }
 
 // what depends on (xc, yc, hit) only: S2, S3, S3'
 template <class T> struct XYInv {
@@ -88,20 +89,60 @@ template <class T> IA_DEV Resid residual_general(const Box3<T>& b, const XYInv<T
   Iv<T> P2 = iscale(T(0.5), imul(iadd(isub(t1, t2), t3), v.iQ));                    // (A.8c)
   Iv<T> T2 = isqr(thin(Tn));
   Iv<T> e = iadd(iscale(Tn, P1), imul(T2, P2));                                     // (A.8a)
-  // S5 sin/cos of Phi = Phi_Ax + e, (A.3b) and (A.7g)
-  Iv<T> se = isin(e), ce = icos(e);
-  Iv<T> sinP = iclamp(imul(iadd(imul(v.sA, ce), imul(v.cA, se)), v.iR), T(-1), T(1));
-  Iv<T> cosP = iclamp(imul(isub(imul(v.cA, ce), imul(v.sA, se)), v.iR), T(-1), T(1));
-  // S6 (A.3a) L160 and delta = d_St/u_d
+  // S5-S7 as a function of e = Phi - Phi_Ax: evaluated once with the series value, or - rigorous mode - several
+  // times inside the verification of the fixed point of (A.6)
   const T twoT = Rd::mul_rn(T(2), Tn);
-  Iv<T> u2 = iadd(iadd(iadd(thin(T(1)), iscale(twoT, imul(b.L, sinP))), imul(T2, isqr(b.L))), imul(T2, isqr(cosP)));
-  Iv<T> u = isqrt(u2);
-  if (!(u.lo > T(0))) return {0.0, 0.0, double(v.Q.hi), 1};
-  Iv<T> dl = idiv_pos(D, u);
-  // S7 (A.4c) L172 with s_perp = R (dphi + e);  c^tau of (A.7b) L194
-  Iv<T> z = isub(iadd(Zr, imul(LR, iadd(v.dphi, e))), iscale(Tn, imul(dl, cosP)));
-  Iv<T> Ld = imul(b.L, dl);
-  Iv<T> ct = isub(imul(z, v.cA), imul(Ld, v.sA));
+  Iv<T> sinP, cosP, dl, z, Ld, ct;
+  bool u_ok = true;
+  auto s5_to_s7 = [&](Iv<T> ee) {
+    // S5 sin/cos of Phi = Phi_Ax + e, (A.3b) and (A.7g)
+    Iv<T> se = isin(ee), ce = icos(ee);
+    sinP = iclamp(imul(iadd(imul(v.sA, ce), imul(v.cA, se)), v.iR), T(-1), T(1));
+    cosP = iclamp(imul(isub(imul(v.cA, ce), imul(v.sA, se)), v.iR), T(-1), T(1));
+    // S6 (A.3a) L160 and delta = d_St/u_d
+    Iv<T> u2 = iadd(iadd(iadd(thin(T(1)), iscale(twoT, imul(b.L, sinP))), imul(T2, isqr(b.L))), imul(T2, isqr(cosP)));
+    Iv<T> u = isqrt(u2);
+    if (!(u.lo > T(0))) { u_ok = false; return; }
+    dl = idiv_pos(D, u);
+    // S7 (A.4c) L172 with s_perp = R (dphi + e);  c^tau of (A.7b) L194
+    z = isub(iadd(Zr, imul(LR, iadd(v.dphi, ee))), iscale(Tn, imul(dl, cosP)));
+    Ld = imul(b.L, dl);
+    ct = isub(imul(z, v.cA), imul(Ld, v.sA));
+  };
+  if (c.rig) {
+    // Reading f3 (PAPER.md L187 eq. (A.6)): e is a fixed point of
+    //   g(e) = atan2(T s^tau(e), R_Ax^2 + T c^tau(e)),  s^tau = -z s_Ax - lambda delta c_Ax     (A.6), (A.7b,c)
+    // Verification by inflation from the series enclosure: g(E) inside E => a fixed point lies in g(E); then
+    // E := g(E), and once more E := g(E) meet E.  Otherwise E := hull(E, g(E)) widened by a tenth of its width
+    // (+ a small absolute amount), at most 6 rounds; not verified: the hit votes (cannot exclude).
+    const T tiny = sizeof(T) == 4 ? T(1e-6) : T(1e-12);
+    auto g_of = [&](Iv<T> ee, Iv<T>& out) -> bool {
+      s5_to_s7(ee);
+      if (!u_ok) return false;
+      Iv<T> st = ineg(iadd(imul(z, v.sA), imul(Ld, v.cA)));
+      out = iatan2(iscale(Tn, st), iadd(v.Q, iscale(Tn, ct)));
+      return true;
+    };
+    Iv<T> E = e, G;
+    bool verified = false;
+    for (int k = 0; k < 6 && !verified; ++k) {
+      if (!g_of(E, G)) return {0.0, 0.0, double(v.Q.hi), 1};
+      if (G.lo >= E.lo && G.hi <= E.hi) {
+        verified = true;
+        E = G;
+      } else {
+        const T lo_h = mn(E.lo, G.lo), hi_h = mx(E.hi, G.hi);
+        const T pad = Rd::add_up(Rd::mul_up(T(0.1), Rd::add_up(hi_h, -lo_h)), tiny);
+        E = {Rd::add_dn(lo_h, -pad), Rd::add_up(hi_h, pad)};
+      }
+    }
+    if (!verified) return {0.0, 0.0, double(v.Q.hi), 1};
+    if (!g_of(E, G)) return {0.0, 0.0, double(v.Q.hi), 1};
+    e = {mx(E.lo, G.lo), mn(E.hi, G.hi)};
+    if (!(e.lo <= e.hi)) return {0.0, 0.0, double(v.Q.hi), 1};
+  }
+  s5_to_s7(e);
+  if (!u_ok) return {0.0, 0.0, double(v.Q.hi), 1};
   // S8 radicand of (A.5b) L183 and f of (A.5a) L180
   Iv<T> rad = isub(isub(isub(isqr(iadd(b.R, dl)), iscale(twoT, ct)), isqr(iscale(Tn, z))), isqr(iscale(Tn, Ld)));
   Iv<T> f = isub(v.Q, rad);

@@ -95,7 +95,7 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
   v.Q = h.Q; v.cA = h.cA; v.sA = h.sA[va]; v.dphi = h.dphi[va]; v.iQ = h.iQ; v.RA = h.RA; v.iR = h.iR; v.c2 = h.c2;
   v.s2 = h.s2[va];
   v.forced = 0;
-  HitS<T> hs = {h.Tabs, h.Dlo, h.Dhi, 1};
+  HitS<T> hs = {h.Tabs, h.Dlo, h.Dhi, 1, 0};
   Box3<T> bx = {R, Zeff, L};
   return hit_votes_general(bx, v, hs, T(0));
 }
@@ -459,7 +459,7 @@ cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& sp, int lev, i
 
 cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
   // the fast form packs vote counts in bytes and keeps one HitF per hit in shared memory
-  const bool fast = !(ctx->params.flags & 1u) && sp.max_hits <= 255;
+  const bool fast = !(ctx->params.flags & 17u) && sp.max_hits <= 255;   // bit 4 (rigorous Phi) lives in the general form
   if (ctx->params.precision == 32)
     return fast ? launch_fast<float>(ctx, sp, g, votes_out) : launch_general<float>(ctx, sp, g, votes_out);
   return fast ? launch_fast<double>(ctx, sp, g, votes_out) : launch_general<double>(ctx, sp, g, votes_out);

@@ -13,15 +13,15 @@ LO, HI = np.array(g.BOX_LO), np.array(g.BOX_HI)
 class Rig:
     """A chamber loaded on both sides."""
 
-    def __init__(self, chamber, tol=g.TOL, precision=64, x_ref=0.0, y_ref=0.0, z_ref=0.0):
+    def __init__(self, chamber, tol=g.TOL, precision=64, x_ref=0.0, y_ref=0.0, z_ref=0.0, flags=0):
         import torch
         self.torch = torch
         self.ch = chamber
         self.ctx = b.Context(0)
         self.ctx.ia_load_geometry(b.wires_of(chamber))
-        self.ctx.ia_set_params(tol, x_ref, y_ref, z_ref, precision)
+        self.ctx.ia_set_params(tol, x_ref, y_ref, z_ref, precision, flags)
         self.owires = o.wires_of(chamber)
-        self.oparams = o.make_params(tol, x_ref, y_ref, z_ref, precision)
+        self.oparams = o.make_params(tol, x_ref, y_ref, z_ref, precision, flags)
 
     def hits(self, wire, drift):
         """(device hits tensor, oracle hits array)"""

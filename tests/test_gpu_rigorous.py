@@ -1,0 +1,91 @@
+"""-m gpu parity of the rigorous-Phi mode (flags bit 4) against the oracle's.
+
+Same algorithm on both sides (verification of the fixed point of (A.6) by inflation from the series enclosure, then
+S5-S8); they differ only in the padding of sin, cos and atan2, a few ulps per round of the verification.
+"""
+import numpy as np
+import pytest
+
+from paper_2401_04576_b200 import binding as b
+from paper_2401_04576_b200 import eventgen as g
+from oracle import oracle as o
+
+from gpu_common import HI, LO, Rig, compare_votes
+
+pytestmark = pytest.mark.gpu
+RIG = 16
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_rigorous_residual_enclosures_match(precision):
+    rng = np.random.default_rng(23)
+    rig = Rig(g.chamber_c1(), precision=precision, flags=RIG)
+    try:
+        ev = g.make_event(rig.ch, 6, n_noise=10)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        par = np.array(ev.track.params)
+        n = 500
+        c = np.stack([rng.uniform(LO, HI) for _ in range(n)])
+        half = (HI - LO)[None, :] * 2.0 ** -rng.integers(3, 12, (n, 1)).astype(np.float64) / 2
+        for i in range(200):
+            c[i] = par + rng.uniform(-1, 1, 5) * half[i]
+        blo, bhi = c - half, c + half
+        blo[:, 2] = np.maximum(blo[:, 2], 20.0)
+        blo[:, 4], bhi[:, 4] = np.maximum(blo[:, 4], -0.6), np.minimum(bhi[:, 4], 0.6)
+        rg = rig.gpu_residual(hd, len(oh), blo, bhi)
+        ro = o.residual(rig.owires, oh, rig.oparams, blo, bhi)
+        same_forced = rg[..., 3] == ro[..., 3]
+        assert same_forced.mean() > 0.9995                  # "verified in round k" can flip on an ulp
+        live = (ro[..., 3] == 0) & same_forced
+        tol = (1e-12 if precision == 64 else 5e-4) * ro[..., 2]
+        assert (np.abs(rg[..., 0] - ro[..., 0])[live] <= tol[live]).mean() > 0.9995
+        assert (np.abs(rg[..., 1] - ro[..., 1])[live] <= tol[live]).mean() > 0.9995
+        vg = (rg[..., 3] == 1) | ((rg[..., 0] <= 0) & (rg[..., 1] >= 0))
+        vo = (ro[..., 3] == 1) | ((ro[..., 0] <= 0) & (ro[..., 1] >= 0))
+        assert (vg == vo).mean() > 0.9995 and vg.any() and not vg.all()
+    finally:
+        rig.close()
+
+
+def test_rigorous_dense_vote_refine_and_truth_with_no_tolerance():
+    """dense 12^5 vote (every cell, mismatches traced), a 4-level refinement (boxes identical), and the strict
+    guarantee: with tol = 0 the cell holding the generated parameters keeps every noise-free hit at every size."""
+    rig = Rig(g.chamber_c1(), flags=RIG)
+    try:
+        ev = g.make_event(rig.ch, 1, n_noise=20)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        dims = (12,) * 5
+        vg = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+        rig.ctx.synchronize()
+        vg = vg.cpu().numpy()
+        vo = o.vote(rig.owires, oh, rig.oparams, LO, HI, dims)
+        compare_votes(rig, hd, oh, vg, vo, lambda idx: o.cell_boxes(LO, HI, dims, idx))
+        # the mode is really on: it differs from the series mode in thousands of cells
+        rig.ctx.ia_set_params(g.TOL, flags=0)
+        vs = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+        rig.ctx.synchronize()
+        assert (vs.cpu().numpy() != vg).sum() > 1000
+        rig.ctx.ia_set_params(g.TOL, flags=RIG)
+        boxes, par = rig.ctx.ia_refine(hd, ev.n_hits, LO, HI, (8,) * 5, 4, 8)
+        rig.ctx.synchronize()
+        gb = b.boxes_to_numpy(boxes, (4, 8))
+        ob, opar = o.refine(rig.owires, oh, rig.oparams, LO, HI, (8,) * 5, 4, 8)
+        assert (gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all()
+        assert (par.cpu().numpy() == opar).all()
+    finally:
+        rig.close()
+    rig = Rig(g.chamber_c1(), tol=0.0, flags=RIG)
+    try:
+        for seed in range(4):
+            ev = g.make_event(rig.ch, 960 + seed, smear=0.0)
+            keep = ~ev.clipped
+            hd, oh = rig.hits(ev.wire[keep], np.abs(ev.d_true[keep]))
+            for n in (8, 100, 4096):
+                dims = (n,) * 5
+                tc = g.truth_cell(ev.track.params, LO, HI, dims)
+                blo, bhi = o.cell_boxes(LO, HI, dims, [tc])
+                v = rig.ctx.ia_vote_boxes(hd, int(keep.sum()), rig.dev(blo), rig.dev(bhi))
+                rig.ctx.synchronize()
+                assert int(v.cpu().numpy()[0]) == keep.sum(), (seed, n)
+    finally:
+        rig.close()
