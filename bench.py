@@ -510,6 +510,35 @@ def main():
             line["paper_mode"] = paper_mode_leg(local_rank, steps=5)
         except Exception as exc:  # pragma: no cover
             line["paper_mode"] = {"error": str(exc)}
+        # ---- f3: rigorous-Phi mode (flags bit 4) against the series mode, both in the general-form kernel ----------
+        try:
+            ch1 = g.chamber_c1()
+            ev1 = g.make_event(ch1, 1, n_noise=20)
+            ctxr = b.Context(local_rank)
+            ctxr.ia_load_geometry(b.wires_of(ch1))
+            hdr = ctxr.to_device(b.hits_of(ev1.wire, ev1.drift))
+            rdims = (16,) * 5
+            nr = int(np.prod(rdims))
+            vr = torch.empty(nr, dtype=torch.uint16, device=f"cuda:{local_rank}")
+            rr = {}
+            for name, fl in (("general_series", 1), ("rigorous", 16)):
+                ctxr.ia_set_params(g.TOL, flags=fl)
+                ctxr.ia_vote(hdr, ev1.n_hits, g.BOX_LO, g.BOX_HI, rdims, votes_out=vr)
+                torch.cuda.synchronize()
+                a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(ctxr.stream)
+                for _ in range(3):
+                    ctxr.ia_vote(hdr, ev1.n_hits, g.BOX_LO, g.BOX_HI, rdims, votes_out=vr)
+                c.record(ctxr.stream)
+                c.synchronize()
+                ms = a.elapsed_time(c) / 3
+                rr[name] = {"ms": ms, "evals_per_s": nr * ev1.n_hits / (ms * 1e-3), "sum_votes": int(vr.to(torch.int64).sum().item())}
+            rr["workload"] = "f3: dense 16^5 x 40 hits (C1 event), general-form kernel: series (A.8) vs verified fixed point of (A.6)"
+            rr["cost_ratio"] = rr["rigorous"]["ms"] / rr["general_series"]["ms"]
+            line["rigorous_phi"] = rr
+            ctxr.close()
+        except Exception as exc:  # pragma: no cover
+            line["rigorous_phi"] = {"error": str(exc)}
         try:
             line["paper_track"] = paper_track_leg(local_rank)
         except Exception as exc:  # pragma: no cover
