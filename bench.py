@@ -429,6 +429,9 @@ def main():
         "flop_frac": ALG_FP64_FLOPS_PER_EVAL * evals_per_step / (vote_ms * 1e-3) / (2 * peak_inst),
         "flop_peak_T": 2 * peak_inst / 1e12, "alg_fp64_flops_per_eval": ALG_FP64_FLOPS_PER_EVAL,
         "unfused_dag_ops_per_eval": DAG_UNFUSED_OPS_PER_EVAL,
+        "operand_note": "a DFMA with 3 distinct vector-register operands issues every 3 cycles (2.25 with operand reuse): 107 of "
+                        "the kernel's 284 FP64-pipe instructions per evaluation; the pipe demand is 611-675 cycles per "
+                        "warp-evaluation against 896 measured (profiles/r01_pipe_probe.md)",
         "ncu_pipe_fp64_active_pct": 63.9, "ncu_source": "profiles/r01_vote_dense_fast_c1_ncu.md (C1, same kernel)",
         "alg_bytes_per_launch": 2 * n_cells, "hbm_frac": (2 * n_cells / (vote_ms * 1e-3)) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
     }

@@ -241,7 +241,10 @@ int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_
  * mode 0: DFMA round-to-nearest; 1: DADD.RM / DMUL.RP alternating; 2: DFMA.RM / DFMA.RP alternating;
  * 3, 4, 5: DFMA.RM / DFMA.RP on only 1, 2, 4 independent chains per thread (same instruction count);
  * 6, 7: mode 2 with one independent integer (LOP3) resp. FP32 (FFMA) instruction after every DFMA - do
- * non-FP64 instructions issue in the shadow of the FP64 pipe?  (only the DFMAs are counted).
+ * non-FP64 instructions issue in the shadow of the FP64 pipe?  (only the DFMAs are counted);
+ * 8, 9: DFMA.RM/RP with three distinct register operands, DMUL.RM/DADD.RP with two (the modes above take
+ * the multiplier and the addend from uniform registers) - is operand fetch a limit?
+ * 10, 11: mode 8 with the multiplier register shared by 4 resp. 2 consecutive DFMAs (operand reuse cache).
  * The caller times it with events on the context's stream.  sink_dev: one double, never written. */
 int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev);
 

@@ -458,7 +458,7 @@ int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_
 }
 
 int ia_probe_fp64(ia_ctx* ctx, int mode, int iters, int blocks, double* sink_dev) {
-  if (!ctx || !sink_dev || mode < 0 || mode > 7 || iters <= 0 || blocks <= 0) return IA_ERR_ARG;
+  if (!ctx || !sink_dev || mode < 0 || mode > 11 || iters <= 0 || blocks <= 0) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_fp64_probe(ctx, mode, iters, blocks, sink_dev));
   return IA_OK;

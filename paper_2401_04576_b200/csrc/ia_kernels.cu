@@ -432,6 +432,43 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(int iters, double seed,
     }
 #pragma unroll
     for (int j = 0; j < 8; ++j) a[j] += double(u[j] & 1u) + double(f[j]) * 1e-30;
+  } else if (mode == 10 || mode == 11) {
+    // three register operands, one of them shared by consecutive instructions (the operand reuse cache):
+    // mode 10 shares the multiplier among 4 consecutive DFMAs, mode 11 among 2
+    double bb[8], cc[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { bb[j] = 1.0 - 1e-9 * (threadIdx.x + j + 1); cc[j] = 1e-12 * (threadIdx.x + 3 * j + 1); }
+    asm volatile("" : "+d"(bb[0]), "+d"(bb[1]), "+d"(bb[2]), "+d"(bb[3]), "+d"(bb[4]), "+d"(bb[5]), "+d"(bb[6]), "+d"(bb[7]));
+    asm volatile("" : "+d"(cc[0]), "+d"(cc[1]), "+d"(cc[2]), "+d"(cc[3]), "+d"(cc[4]), "+d"(cc[5]), "+d"(cc[6]), "+d"(cc[7]));
+    const int sh = mode == 10 ? 2 : 1;
+    for (int i = 0; i < iters; i += 2) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) asm volatile("fma.rm.f64 %0, %1, %0, %2;" : "+d"(a[j]) : "d"(bb[j >> sh]), "d"(cc[j]));
+#pragma unroll
+      for (int j = 0; j < 8; ++j) asm volatile("fma.rp.f64 %0, %1, %0, %2;" : "+d"(a[j]) : "d"(bb[4 + (j >> sh)]), "d"(cc[(j + 1) & 7]));
+    }
+  } else if (mode == 8 || mode == 9) {
+    // register operands: mode 8 DFMA.RM/RP with three distinct per-thread register operands (the probes above
+    // multiply by and add uniform values), mode 9 DMUL.RM / DADD.RP with two - does operand fetch from the
+    // register file hold the pipe below one instruction per two cycles?
+    double bb[8], cc[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { bb[j] = 1.0 - 1e-9 * (threadIdx.x + j + 1); cc[j] = 1e-12 * (threadIdx.x + 3 * j + 1); }
+    asm volatile("" : "+d"(bb[0]), "+d"(bb[1]), "+d"(bb[2]), "+d"(bb[3]), "+d"(bb[4]), "+d"(bb[5]), "+d"(bb[6]), "+d"(bb[7]));
+    asm volatile("" : "+d"(cc[0]), "+d"(cc[1]), "+d"(cc[2]), "+d"(cc[3]), "+d"(cc[4]), "+d"(cc[5]), "+d"(cc[6]), "+d"(cc[7]));
+    for (int i = 0; i < iters; i += 2) {
+      if (mode == 8) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = __fma_rd(a[j], bb[j], cc[(j + 1) & 7]);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = __fma_ru(a[j], bb[(j + 3) & 7], cc[j]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = __dmul_rd(a[j], bb[j]);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = __dadd_ru(a[j], cc[j]);
+      }
+    }
   } else {
     // modes 3, 4, 5: the same number of DFMA.RM/RP per thread on 1, 2, 4 independent chains only
     const int nc = 1 << (mode - 3);
@@ -467,7 +504,7 @@ cudaError_t launch_fp64_probe(ia_ctx* ctx, int mode, int iters, int blocks, doub
   switch (mode) {
 #define IA_PROBE_CASE(M) case M: fp64_probe_kernel<M><<<blocks, 256, 0, ctx->stream>>>(iters, 1.0, sink); break;
     IA_PROBE_CASE(0) IA_PROBE_CASE(1) IA_PROBE_CASE(2) IA_PROBE_CASE(3) IA_PROBE_CASE(4) IA_PROBE_CASE(5)
-    IA_PROBE_CASE(6) IA_PROBE_CASE(7)
+    IA_PROBE_CASE(6) IA_PROBE_CASE(7) IA_PROBE_CASE(8) IA_PROBE_CASE(9) IA_PROBE_CASE(10) IA_PROBE_CASE(11)
 #undef IA_PROBE_CASE
     default: return cudaErrorInvalidValue;
   }

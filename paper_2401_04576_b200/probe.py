@@ -16,7 +16,9 @@ from . import binding as b
 
 MODES = {0: "DFMA rn, 8 chains", 1: "DADD.RM/DMUL.RP, 8 chains", 2: "DFMA.RM/RP, 8 chains",
          3: "DFMA.RM/RP, 1 chain", 4: "DFMA.RM/RP, 2 chains", 5: "DFMA.RM/RP, 4 chains",
-         6: "DFMA.RM/RP + 1 LOP3 each", 7: "DFMA.RM/RP + 1 FFMA each"}
+         6: "DFMA.RM/RP + 1 LOP3 each", 7: "DFMA.RM/RP + 1 FFMA each",
+         8: "DFMA.RM/RP, 3 register operands", 9: "DMUL.RM/DADD.RP, 2 register operands",
+         10: "DFMA 3 reg, multiplier shared by 4", 11: "DFMA 3 reg, multiplier shared by 2"}
 
 
 def main():
