@@ -418,193 +418,19 @@ template <class T> struct PairC {
   Iv<T> L2;            // lambda^2
 };
 // ... per (pair, hit)
-#ifndef IA_FUSE
-#define IA_FUSE 1
-#endif
 template <class T> struct HitP {
-  Iv<T> LRdphi, T2L2, RpRA;
-#if IA_FUSE
-  MR<T> TL2m;          // (2T) lambda in midpoint form; T2L2 holds 1 + T^2 lambda^2
-#endif
-};
-// ... per (pair, hit, drift sign): S4 terms that do not depend on z0
-template <class T> struct PassC {
-  Iv<T> LDcA, G;
-  MR<T> Km;            // K = (lambda (R - 2D)) cos 2Phi_Ax, class of cos 2Phi_Ax (R - 2D > 0 by the guard):
-                       // t2 = ((lambda zA)(R - 2D)) c2 = K zA - interval multiplication is associative and
-                       // commutative, so only the roundings differ from the order of S4
+  Iv<T> LRdphi, T2L2, RpRA;      // lambda R dphi;  1 + T^2 lambda^2;  R + R_Ax
+  MR<T> TL2m;                    // (2T) lambda in midpoint form
 };
 
 template <class T> IA_DEV HitP<T> hit_prepare(const HitF<T>& h, int va, const PairC<T>& p) {
-#if IA_FUSE
   return {prod_p(p.LRm, h.dphi[va]), iadd_s(mul_pp(h.T2, p.L2), T(1)), iadd(p.R, h.RA), to_mr(iscale_pos(h.twoT, p.L))};
-#else
-  return {prod_p(p.LRm, h.dphi[va]), mul_pp(h.T2, p.L2), iadd(p.R, h.RA)};
-#endif
 }
 
-template <class T> IA_DEV PassC<T> pass_prepare(const HitF<T>& h, bool dneg, const PairC<T>& p, const HitP<T>& hp) {
-  PassC<T> c;
-  const Iv<T> D = dneg ? Iv<T>{-h.Dhi, -h.Dlo} : Iv<T>{h.Dlo, h.Dhi};
-  const Iv<T> LD = dneg ? mul_pn(p.L, D) : mul_pp(p.L, D);
-  c.LDcA = imul(LD, h.cA);
-  const Iv<T> LRm2D = mul_pp(p.L, isub(p.R, Iv<T>{Rnd<T>::mul_rn(T(2), D.lo), Rnd<T>::mul_rn(T(2), D.hi)}));
-  c.Km = to_mr(mul_pu(LRm2D, h.c2));
-  const Iv<T> a = iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, D)));
-  c.G = dneg ? mul_pn(a, D) : mul_pp(D, a);
-  return c;
-}
-
-// S4-S8 for NC cells (same (R, lambda) pair, hit and drift sign; NC different z0 cells) at once; bit c
-// of the result is set iff 0 is in f for cell c.  The NC cells are independent dependency chains
-// written side by side, which is what keeps the FP64 pipe fed at 16 warps per SM (its dependent-issue
-// latency is about 12 cycles).
-// Inputs transformed: L >= 0, T = h.Tabs >= 0, cA >= 0 (SS != 0) or any (SS == 0); va = the warp's a.
-template <int SS, int NC, class T>
-IA_DEV unsigned pass_vote(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp,
-                          const Iv<T>* Zr) {
-  using Rd = Rnd<T>;
-  const T Tn = h.Tabs;
-  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
-  Iv<T> e[NC];
-  bool small = true;
-  // S4, z0-dependent part
-#pragma unroll
-  for (int c = 0; c < NC; ++c) {
-    const Iv<T> zA = iadd(Zr[c], hp.LRdphi);                           // (A.8d)
-    const Iv<T> zAsA = prod_s<SS>(h.sAm[va], zA);                      // sigma zA sA
-    const Iv<T> t1 = prod_p(p.LRm, zA);
-    const Iv<T> zA2 = sqr_u(zA);
-    const Iv<T> TY = prod_p(h.TiQm, add_s<SS>(pc.LDcA, zAsA));         // T Phi1 = -TY        (A.8b)
-    Iv<T> in;                                                          // t1 - t2
-    if (h.c2cls == CLS_P) in = isub(t1, prod_p(pc.Km, zA));
-    else if (h.c2cls == CLS_N) in = iadd(t1, prod_p(mr_neg(pc.Km), zA));
-    else in = isub(t1, prod_u(pc.Km, zA));
-    const Iv<T> t3 = prod_s<SS>(h.s2m[va], iadd(zA2, pc.G));           // sigma t3
-    const Iv<T> T2P2 = prod_p(h.T2hiQm, add_s<SS>(in, t3));            // T^2 Phi2            (A.8c)
-    e[c] = isub(T2P2, TY);                                             // (A.8a)
-    small = small && abs_lt_quarter(e[c].lo) && abs_lt_quarter(e[c].hi);
-  }
-  // S5
-  const Iv<T> sA = h.sA[va];
-  Iv<T> se[NC], sce[NC], cce[NC];                                      // sin e, sigma sA cos e, cA cos e
-  if (__all_sync(0xffffffffu, small)) {
-#pragma unroll
-    for (int c = 0; c < NC; ++c) {
-      Iv<T> ce;
-      trig_small(e[c], se[c], ce);
-      sce[c] = mulpos_s<SS>(ce, sA);
-      cce[c] = mulpos_s<SC>(ce, h.cA);
-    }
-  } else {
-#pragma unroll
-    for (int c = 0; c < NC; ++c) {
-      trig_general(e[c], sA, h.cA, se[c], sce[c], cce[c]);
-      if (SS < 0) sce[c] = ineg(sce[c]);
-    }
-  }
-  unsigned bits = 0;
-  const T twoT = Rd::mul_rn(T(2), Tn);
-#pragma unroll
-  for (int c = 0; c < NC; ++c) {
-    const Iv<T> cAse = prod_s<SC>(h.cAm, se[c]);
-    const Iv<T> sAse = prod_s<SS>(h.sAm[va], se[c]);                   // sigma sA sin e
-    const Iv<T> sinP = clamp_unit(prod_p(h.iRm, SS < 0 ? isub(cAse, sce[c]) : iadd(sce[c], cAse)));
-    const Iv<T> cosP = clamp_unit(prod_p(h.iRm, sub_s<SS>(cce[c], sAse)));
-    // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
-    const Iv<T> u2 = iadd(iadd(iadd_s(iscale_pos(twoT, prod_p(p.Lm, sinP)), T(1)), hp.T2L2), mul_pp(h.T2, sqr_u(cosP)));
-    const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                       // |delta| = D+ / u_d
-    // S7: z = (Zr + LR (dphi + e)) - T (delta cosP), delta = -/+ dq
-    const Iv<T> zz = iadd(Zr[c], prod_p(p.LRm, iadd(h.dphi[va], e[c])));
-    const Iv<T> Tdc = iscale_pos(Tn, mul_pu(dq, cosP));
-    const Iv<T> Lq = mul_pp(p.L, dq);                                  // |lambda delta|
-    const Iv<T> qs = mulpos_s<SS>(Lq, h.sA2T[va]);                     // sigma 2T |lambda delta| sA
-    Iv<T> z, ct, Rd1;                                                  // ct = 2T c^tau       (A.7b)
-    if (dneg) {
-      z = iadd(zz, Tdc);
-      ct = add_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
-      Rd1 = isub(p.R, dq);
-    } else {
-      z = isub(zz, Tdc);
-      ct = sub_s<SS>(prod_s<SC>(h.cA2Tm, z), qs);
-      Rd1 = iadd(p.R, dq);
-    }
-    // S8
-    const Iv<T> TLq = iscale_pos(Tn, Lq);
-    const Iv<T> rad = isub(isub(isub(mul_pp(Rd1, Rd1), ct), sqr_u(iscale_pos(Tn, z))), mul_pp(TLq, TLq));
-    const Iv<T> f = isub(h.Q, rad);
-    // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
-    bits |= (!(is_pos(f.lo) || f.hi < T(0)) ? 1u : 0u) << c;
-  }
-  return bits;
-}
-
-// The same S4-S8 with every product-then-sum written as directed FMAs (fma_p / fms_p / add_sqr ...):
-// the expression DAG and its association order are those of DESIGN.md section 2 except for three
-// re-associations of pure products, (2T)(lambda sin Phi) = ((2T) lambda) sin Phi,
-// T (delta cos Phi) = (T delta) cos Phi and (lambda delta)(2T s_Ax) = (lambda (T delta))(2 s_Ax), which
-// move a factor that is constant over the z0 loop out of it.  Only roundings differ.
-template <int SS, class T>
-IA_DEV unsigned pass_vote_fused(const HitF<T>& h, int va, bool dneg, const PassC<T>& pc, const PairC<T>& p, const HitP<T>& hp,
-                                Iv<T> Zr) {
-  using Rd = Rnd<T>;
-  const T Tn = h.Tabs;
-  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
-  // S4, z0-dependent part
-  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
-  const Iv<T> W = fma_s<SS>(h.sAm[va], zA, pc.LDcA);                   // lambda D cA + zA sA
-  const Iv<T> TY = prod_p(h.TiQm, W);                                  // T Phi1 = -TY        (A.8b)
-  const Iv<T> t1 = prod_p(p.LRm, zA);
-  Iv<T> in;                                                            // t1 - t2
-  if (h.c2cls == CLS_P) in = fms_p(pc.Km, zA, t1);
-  else if (h.c2cls == CLS_N) in = fma_p(mr_neg(pc.Km), zA, t1);
-  else in = fms_u(pc.Km, zA, t1);
-  const Iv<T> V = fma_s<SS>(h.s2m[va], add_sqr(pc.G, zA), in);         // (t1 - t2) + t3
-  const Iv<T> e = fma_p(h.T2hiQm, V, ineg(TY));                        // T^2 Phi2 + T Phi1   (A.8a,c)
-  const bool small = abs_lt_quarter(e.lo) && abs_lt_quarter(e.hi);
-  // S5
-  Iv<T> se, sce, cce;                                                  // sin e, sigma sA cos e, cA cos e
-  if (__all_sync(0xffffffffu, small)) {
-    Iv<T> ce;
-    trig_small(e, se, ce);
-    sce = mulpos_s<SS>(ce, h.sA[va]);
-    cce = mulpos_s<SC>(ce, h.cA);
-  } else {
-    trig_general(e, h.sA[va], h.cA, se, sce, cce);
-    if (SS < 0) sce = ineg(sce);
-  }
-  const Iv<T> sinP = clamp_unit(prod_p(h.iRm, fma_s<SC>(h.cAm, se, SS < 0 ? ineg(sce) : sce)));
-  const Iv<T> cosP = clamp_unit(prod_p(h.iRm, fms_s<SS>(h.sAm[va], se, cce)));
-  // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
-  const Iv<T> u2a = fma_p(hp.TL2m, sinP, hp.T2L2);
-  const Mag<T> gc = mag_of(cosP);
-  const Iv<T> u2 = {gc.straddle ? u2a.lo : Rd::fma_dn(h.T2.lo, Rd::mul_dn(gc.mnn, gc.mnn), u2a.lo),
-                    Rd::fma_up(h.T2.hi, Rd::mul_up(gc.mag, gc.mag), u2a.hi)};
-  const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                         // |delta| = D+ / u_d
-  // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = -/+ dq
-  const Iv<T> zz = fma_p(p.LRm, iadd(h.dphi[va], e), Zr);
-  const Iv<T> Tdq = iscale_pos(Tn, dq);                                // |T delta|
-  const Iv<T> TLq = mul_pp(p.L, Tdq);                                  // |T lambda delta|
-  const Iv<T> qs = mulpos_s<SS>(TLq, h.sA2[va]);                       // sigma 2T |lambda delta| sA
-  const T plo = sgn(cosP.lo) ? Tdq.hi : Tdq.lo, phi = sgn(cosP.hi) ? Tdq.lo : Tdq.hi;   // partners of cosP.lo / .hi
-  Iv<T> z, ct, Rd1;                                                    // ct = 2T c^tau       (A.7b)
-  if (dneg) {
-    z = {Rd::fma_dn(plo, cosP.lo, zz.lo), Rd::fma_up(phi, cosP.hi, zz.hi)};
-    ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? ineg(qs) : qs);
-    Rd1 = isub(p.R, dq);
-  } else {
-    z = {Rd::fma_dn(-phi, cosP.hi, zz.lo), Rd::fma_up(-plo, cosP.lo, zz.hi)};
-    ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? qs : ineg(qs));
-    Rd1 = iadd(p.R, dq);
-  }
-  // S8
-  const Iv<T> r1 = {Rd::fma_dn(Rd1.lo, Rd1.lo, -ct.hi), Rd::fma_up(Rd1.hi, Rd1.hi, -ct.lo)};
-  const Iv<T> r2 = sub_sqr(r1, iscale_pos(Tn, z));
-  const Iv<T> rad = {Rd::fma_dn(-TLq.hi, TLq.hi, r2.lo), Rd::fma_up(-TLq.lo, TLq.lo, r2.hi)};
-  const Iv<T> f = isub(h.Q, rad);
-  // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
-  return !(is_pos(f.lo) || f.hi < T(0)) ? 1u : 0u;
-}
+// The evaluation itself (S4-S8 for both drift signs of one cell) is pass_vote_q / pass_vote_qr of ia_fastq.cuh.
+// Round 1 went through four earlier forms of it - products followed by sums, several z0 cells side by side, fused
+// directed FMAs one sign at a time, both signs without instruction ordering - which the git history keeps
+// (commits 94cbacd ... d7c361e); the measured steps are in DESIGN.md section 12.
 
 // ---- both drift signs side by side ------------------------------------------------------------------
 // The two signs of one (cell, hit) are independent dependency chains that share zA, t1 and the
@@ -629,85 +455,6 @@ template <class T> IA_DEV Pass2<T> pass_prepare2(const HitF<T>& h, const PairC<T
   c.G[0] = mul_pp(D, iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, D))));
   c.G[1] = mul_pn(iadd(h.RA, mul_pp(p.L2, isub(hp.RpRA, Dn))), Dn);
   return c;
-}
-
-template <int SS, class T>
-IA_DEV unsigned pass_vote2(const HitF<T>& h, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
-  using Rd = Rnd<T>;
-  const T Tn = h.Tabs;
-  constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
-  // S4: shared part
-  const Iv<T> zA = iadd(Zr, hp.LRdphi);                                // (A.8d)
-  const Iv<T> t1 = prod_p(p.LRm, zA);
-  const Mag<T> gz = mag_of(zA);
-  Iv<T> e[2];
-  bool small = true;
-#pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    const Iv<T> W = fma_s<SS>(h.sAm[va], zA, s ? ineg(pc.LDcA) : pc.LDcA);   // lambda D cA + zA sA
-    const Iv<T> TY = prod_p(h.TiQm, W);                                // T Phi1 = -TY        (A.8b)
-    Iv<T> in;                                                          // t1 - t2
-    if (h.c2cls == CLS_P) in = fms_p(pc.Km[s], zA, t1);
-    else if (h.c2cls == CLS_N) in = fma_p(mr_neg(pc.Km[s]), zA, t1);
-    else in = fms_u(pc.Km[s], zA, t1);
-    const Iv<T> zG = {gz.straddle ? pc.G[s].lo : Rd::fma_dn(gz.mnn, gz.mnn, pc.G[s].lo), Rd::fma_up(gz.mag, gz.mag, pc.G[s].hi)};
-    const Iv<T> V = fma_s<SS>(h.s2m[va], zG, in);                      // (t1 - t2) + t3
-    e[s] = fma_p(h.T2hiQm, V, ineg(TY));                               // T^2 Phi2 + T Phi1   (A.8a,c)
-    small = small && abs_lt_quarter(e[s].lo) && abs_lt_quarter(e[s].hi);
-  }
-  // S5
-  Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
-  if (__all_sync(0xffffffffu, small)) {
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      Iv<T> ce;
-      trig_small(e[s], se[s], ce);
-      sce[s] = mulpos_s<SS>(ce, h.sA[va]);
-      cce[s] = mulpos_s<SC>(ce, h.cA);
-    }
-  } else {
-#pragma unroll 1
-    for (int s = 0; s < 2; ++s) {
-      trig_general(e[s], h.sA[va], h.cA, se[s], sce[s], cce[s]);
-      if (SS < 0) sce[s] = ineg(sce[s]);
-    }
-  }
-  bool vote = false;
-#pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    const Iv<T> sinP = clamp_unit(prod_p(h.iRm, fma_s<SC>(h.cAm, se[s], SS < 0 ? ineg(sce[s]) : sce[s])));
-    const Iv<T> cosP = clamp_unit(prod_p(h.iRm, fms_s<SS>(h.sAm[va], se[s], cce[s])));
-    // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
-    const Iv<T> u2a = fma_p(hp.TL2m, sinP, hp.T2L2);
-    const Mag<T> gc = mag_of(cosP);
-    const Iv<T> u2 = {gc.straddle ? u2a.lo : Rd::fma_dn(h.T2.lo, Rd::mul_dn(gc.mnn, gc.mnn), u2a.lo),
-                      Rd::fma_up(h.T2.hi, Rd::mul_up(gc.mag, gc.mag), u2a.hi)};
-    const Iv<T> dq = Dir<T>::d_over_sqrt(h, u2);                       // |delta| = D+ / u_d
-    // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (s = 0), -dq (s = 1)
-    const Iv<T> zz = fma_p(p.LRm, iadd(h.dphi[va], e[s]), Zr);
-    const Iv<T> Tdq = iscale_pos(Tn, dq);                              // |T delta|
-    const Iv<T> TLq = mul_pp(p.L, Tdq);                                // |T lambda delta|
-    const Iv<T> qs = mulpos_s<SS>(TLq, h.sA2[va]);                     // sigma 2T |lambda delta| sA
-    const T plo = sgn(cosP.lo) ? Tdq.hi : Tdq.lo, phi = sgn(cosP.hi) ? Tdq.lo : Tdq.hi;   // partners of cosP.lo / .hi
-    Iv<T> z, ct, Rd1;                                                  // ct = 2T c^tau       (A.7b)
-    if (s) {
-      z = {Rd::fma_dn(plo, cosP.lo, zz.lo), Rd::fma_up(phi, cosP.hi, zz.hi)};
-      ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? ineg(qs) : qs);
-      Rd1 = isub(p.R, dq);
-    } else {
-      z = {Rd::fma_dn(-phi, cosP.hi, zz.lo), Rd::fma_up(-plo, cosP.lo, zz.hi)};
-      ct = fma_s<SC>(h.cA2Tm, z, SS < 0 ? qs : ineg(qs));
-      Rd1 = iadd(p.R, dq);
-    }
-    // S8
-    const Iv<T> r1 = {Rd::fma_dn(Rd1.lo, Rd1.lo, -ct.hi), Rd::fma_up(Rd1.hi, Rd1.hi, -ct.lo)};
-    const Iv<T> r2 = sub_sqr(r1, iscale_pos(Tn, z));
-    const Iv<T> rad = {Rd::fma_dn(-TLq.hi, TLq.hi, r2.lo), Rd::fma_up(-TLq.lo, TLq.lo, r2.hi)};
-    const Iv<T> f = isub(h.Q, rad);
-    // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
-    vote = vote || !(is_pos(f.lo) || f.hi < T(0));
-  }
-  return vote ? 1u : 0u;
 }
 
 }  // namespace ia

@@ -100,45 +100,14 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
   return hit_votes_general(bx, v, hs, T(0));
 }
 
-// one hit, one thread: both drift signs over the thread's z0 cells, FAST_NC cells at a time; returns
-// the 8-bit vote mask
-#ifndef IA_FAST_NC
-#define IA_FAST_NC 1
-#endif
-constexpr int FAST_NC = IA_FAST_NC;
-#ifndef IA_DUAL
-#define IA_DUAL 1
-#endif
+// one hit, one thread: both drift signs over the thread's z0 cells; returns the vote mask (bit i = z0 cell i)
 template <int SS, class T>
 IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
-  unsigned bits = 0;
-#if IA_DUAL
   const Pass2<T> pc2 = pass_prepare2(h, p, hp);
+  unsigned bits = 0;
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) bits |= pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]) << i;
-  return bits;
-#endif
-  const unsigned full = (1u << nz_tile) - 1u;
-#pragma unroll 1
-  for (int s = 0; s < 2; ++s) {
-    const bool dneg = s == 1;
-    // the second pass is needed only where some lane has not voted yet
-    if (__all_sync(0xffffffffu, bits == full)) break;
-    const PassC<T> pc = pass_prepare(h, dneg, p, hp);
-    int i = 0;
-#if IA_FUSE
-#pragma unroll 1
-    for (; i < nz_tile; ++i) bits |= pass_vote_fused<SS>(h, va, dneg, pc, p, hp, zt[i]) << i;
-#else
-#pragma unroll 1
-    for (; i + FAST_NC <= nz_tile; i += FAST_NC) bits |= pass_vote<SS, FAST_NC>(h, va, dneg, pc, p, hp, zt + i) << i;
-    if (FAST_NC > 1) {
-#pragma unroll 1
-      for (; i < nz_tile; ++i) bits |= pass_vote<SS, 1>(h, va, dneg, pc, p, hp, zt + i) << i;
-    }
-#endif
-  }
   return bits;
 }
 
