@@ -28,7 +28,9 @@
 // Pins (tests/test_oracle_*.py, all -m "not gpu"):  P1 identity at the generated truth,
 // P3 containment, P4 axial closed form, P5 brute-force sampling, P6 inclusion isotonicity,
 // P8 series order, P9 independent round-to-nearest DAG anchor; primitives against exact
-// rational arithmetic.  Parity status: pinned (none of the functions here is "parity unpinned").
+// rational arithmetic.  Paper mode (orc_vote_paper ...): MP1-MP6; iteration scheme (orc_disk_filter,
+// orc_select_max_paper, orc_find_hits_paper, orc_track_paper): F2a-F2e, M6; rigorous Phi (flags bit 4): R1-R3.
+// Parity status: pinned (none of the functions here is "parity unpinned").
 
 #include <algorithm>
 #include <cfenv>
