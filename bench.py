@@ -298,6 +298,7 @@ def main():
     ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1", "F2"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
+    ap.add_argument("--flags", type=int, default=0, help="ia_params.flags for the dense workloads (1: general kernel, 16: rigorous Phi)")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -359,7 +360,7 @@ def main():
     evals_per_step = n_cells * ev.n_hits
     ctx = b.Context(local_rank)
     ctx.ia_load_geometry(b.wires_of(ch))
-    ctx.ia_set_params(g.TOL)
+    ctx.ia_set_params(g.TOL, flags=args.flags)
     hits_host = b.hits_of(ev.wire, ev.drift)
     hd = ctx.to_device(hits_host)
     votes = torch.empty(n_cells, dtype=torch.uint16, device=f"cuda:{local_rank}")

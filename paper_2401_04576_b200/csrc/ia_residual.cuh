@@ -109,40 +109,39 @@ template <class T> IA_DEV Resid residual_general(const Box3<T>& b, const XYInv<T
     Ld = imul(b.L, dl);
     ct = isub(imul(z, v.cA), imul(Ld, v.sA));
   };
-  if (c.rig) {
-    // Reading f3 (PAPER.md L187 eq. (A.6)): e is a fixed point of
-    //   g(e) = atan2(T s^tau(e), R_Ax^2 + T c^tau(e)),  s^tau = -z s_Ax - lambda delta c_Ax     (A.6), (A.7b,c)
-    // Verification by inflation from the series enclosure: g(E) inside E => a fixed point lies in g(E); then
-    // E := g(E), and once more E := g(E) meet E.  Otherwise E := hull(E, g(E)) widened by a tenth of its width
-    // (+ a small absolute amount), at most 6 rounds; not verified: the hit votes (cannot exclude).
-    const T tiny = sizeof(T) == 4 ? T(1e-6) : T(1e-12);
-    auto g_of = [&](Iv<T> ee, Iv<T>& out) -> bool {
-      s5_to_s7(ee);
-      if (!u_ok) return false;
-      Iv<T> st = ineg(iadd(imul(z, v.sA), imul(Ld, v.cA)));
-      out = iatan2(iscale(Tn, st), iadd(v.Q, iscale(Tn, ct)));
-      return true;
-    };
-    Iv<T> E = e, G;
-    bool verified = false;
-    for (int k = 0; k < 6 && !verified; ++k) {
-      if (!g_of(E, G)) return {0.0, 0.0, double(v.Q.hi), 1};
-      if (G.lo >= E.lo && G.hi <= E.hi) {
-        verified = true;
-        E = G;
+  // Rigorous mode, reading f3 (PAPER.md L187 eq. (A.6)): e is a fixed point of
+  //   g(e) = atan2(T s^tau(e), R_Ax^2 + T c^tau(e)),  s^tau = -z s_Ax - lambda delta c_Ax     (A.6), (A.7b,c)
+  // Verification by inflation from the series enclosure: g(E) inside E => a fixed point lies in g(E); then
+  // E := g(E), and once more E := g(E) meet E.  Otherwise E := hull(E, g(E)) widened by a tenth of its width
+  // (+ a small absolute amount), at most 6 rounds; not verified: the hit votes (cannot exclude).
+  // One loop, one copy of S5-S7 in the binary: state 0 = verifying, 1 = tightening, 2 = the evaluation that S8 uses
+  // (the series mode enters in state 2).  Three inlined copies per drift sign starved the kernel on instruction
+  // fetch (icc hit rate 44 %).
+  const T tiny = sizeof(T) == 4 ? T(1e-6) : T(1e-12);
+  int state = c.rig ? 0 : 2, rounds = 0;
+#pragma unroll 1
+  for (;;) {
+    s5_to_s7(e);
+    if (!u_ok) return {0.0, 0.0, double(v.Q.hi), 1};
+    if (state == 2) break;
+    const Iv<T> st = ineg(iadd(imul(z, v.sA), imul(Ld, v.cA)));
+    const Iv<T> G = iatan2(iscale(Tn, st), iadd(v.Q, iscale(Tn, ct)));
+    if (state == 0) {
+      if (G.lo >= e.lo && G.hi <= e.hi) {
+        e = G;
+        state = 1;
       } else {
-        const T lo_h = mn(E.lo, G.lo), hi_h = mx(E.hi, G.hi);
+        if (++rounds >= 6) return {0.0, 0.0, double(v.Q.hi), 1};
+        const T lo_h = mn(e.lo, G.lo), hi_h = mx(e.hi, G.hi);
         const T pad = Rd::add_up(Rd::mul_up(T(0.1), Rd::add_up(hi_h, -lo_h)), tiny);
-        E = {Rd::add_dn(lo_h, -pad), Rd::add_up(hi_h, pad)};
+        e = {Rd::add_dn(lo_h, -pad), Rd::add_up(hi_h, pad)};
       }
+    } else {
+      e = {mx(e.lo, G.lo), mn(e.hi, G.hi)};
+      if (!(e.lo <= e.hi)) return {0.0, 0.0, double(v.Q.hi), 1};
+      state = 2;
     }
-    if (!verified) return {0.0, 0.0, double(v.Q.hi), 1};
-    if (!g_of(E, G)) return {0.0, 0.0, double(v.Q.hi), 1};
-    e = {mx(E.lo, G.lo), mn(E.hi, G.hi)};
-    if (!(e.lo <= e.hi)) return {0.0, 0.0, double(v.Q.hi), 1};
   }
-  s5_to_s7(e);
-  if (!u_ok) return {0.0, 0.0, double(v.Q.hi), 1};
   // S8 radicand of (A.5b) L183 and f of (A.5a) L180
   Iv<T> rad = isub(isub(isub(isqr(iadd(b.R, dl)), iscale(twoT, ct)), isqr(iscale(Tn, z))), isqr(iscale(Tn, Ld)));
   Iv<T> f = isub(v.Q, rad);
@@ -154,7 +153,11 @@ IA_DEV bool resid_votes(const Resid& r) { return r.forced || !(r.flo > 0.0 || r.
 
 template <class T> IA_DEV bool hit_votes_general(const Box3<T>& b, const XYInv<T>& v, const HitS<T>& c, T zref) {
   if (!c.valid) return false;
-  return resid_votes(residual_general(b, v, c, zref, +1)) || resid_votes(residual_general(b, v, c, zref, -1));
+  // one copy of the residual in the binary for both drift signs (the general kernels are bound by instruction fetch)
+#pragma unroll 1
+  for (int s = 0; s < 2; ++s)
+    if (resid_votes(residual_general(b, v, c, zref, s == 0 ? +1 : -1))) return true;
+  return false;
 }
 
 // outward conversion of a double box [lo, hi] to T endpoints (G22)
