@@ -81,7 +81,9 @@ typedef struct {
  * than half a turn, PAPER.md L88 (reading M6); bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
  * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
  * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; runs in the
- * general (sign-agnostic) kernels, about 3 x the arithmetic; other bits must be 0. */
+ * general (sign-agnostic) kernels, about 4 x the arithmetic; bit 5: ia_refine / ia_refine_batch always enqueue
+ * their launches one by one (default: a call repeated with identical arguments and buffers is replayed as a
+ * CUDA graph from its third occurrence on); other bits must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;

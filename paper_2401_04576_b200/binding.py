@@ -262,11 +262,13 @@ class Context:
         return idx, v
 
     # ---- a8-a10
-    def ia_refine(self, hits_dev, n_hits, box_lo, box_hi, grid0, levels, k):
+    def ia_refine(self, hits_dev, n_hits, box_lo, box_hi, grid0, levels, k, boxes=None, params=None):
         torch = self._torch
         lo, hi, dims = _host5(box_lo, np.float64), _host5(box_hi, np.float64), _host5(grid0, np.int32)
-        boxes = self._empty(max(levels * k, 1) * BOX_DT.itemsize, torch.uint8)
-        params = self._empty(10, torch.float64)
+        if boxes is None:
+            boxes = self._empty(max(levels * k, 1) * BOX_DT.itemsize, torch.uint8)
+        if params is None:
+            params = self._empty(10, torch.float64)
         self._chk(self.lib.ia_refine(self.h, _dp(hits_dev), n_hits, _hp(lo), _hp(hi), _hp(dims), levels, k, _dp(boxes),
                                      _dp(params)), "ia_refine")
         return boxes, params

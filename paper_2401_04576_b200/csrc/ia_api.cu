@@ -91,20 +91,81 @@ int refine_impl(ia_ctx* ctx, const HitSpan& sp, const double lo[5], const double
   if (k > IA_MAX_K || sp.n_events > 65535) return IA_ERR_CAPACITY;
   rc = check_domain(ctx, lo, hi);
   if (rc) return rc;
-  const int ne = sp.n_events;
-  IA_CUDA(ctx, launch_stage_hits(ctx, sp));
-  // level 0: dense start grid -> top k -> boxes
-  IA_CUDA(ctx, scratch_reserve(ctx->votes, size_t(ne) * g.cells * sizeof(uint16_t)));
-  uint16_t* votes = static_cast<uint16_t*>(ctx->votes.p);
-  IA_CUDA(ctx, launch_vote_dense(ctx, sp, g, votes));
-  IA_CUDA(ctx, scratch_reserve(ctx->misc, size_t(ne) * k * (sizeof(int64_t) + sizeof(uint16_t)) + 64));
-  int64_t* idx = static_cast<int64_t*>(ctx->misc.p);
-  uint16_t* kv = reinterpret_cast<uint16_t*>(idx + size_t(ne) * k);
-  IA_CUDA(ctx, launch_topk(ctx, votes, g.cells, ne, k, idx, kv));
-  IA_CUDA(ctx, launch_gather_dense(ctx, g, idx, kv, ne, k, levels, boxes_out));
-  // levels 1..: subdivide, vote the children, keep the top k - all stream-ordered, no host round trip
-  for (int lev = 1; lev < levels; ++lev) IA_CUDA(ctx, launch_refine_level(ctx, sp, lev, levels, k, boxes_out));
-  IA_CUDA(ctx, launch_params(ctx, ne, levels, k, boxes_out, params_out));
+  // the same call again (same buffers, grid, parameters, scratch): replay its CUDA graph
+  RefineKey key;
+  std::memset(&key, 0, sizeof(key));
+  key.sp.hits = sp.hits; key.sp.offsets = sp.offsets; key.sp.n_hits_single = sp.n_hits_single;
+  key.sp.max_hits = sp.max_hits; key.sp.n_events = sp.n_events;          // field by field: no padding bytes copied
+  for (int d = 0; d < 5; ++d) { key.lo[d] = lo[d]; key.hi[d] = hi[d]; key.grid[d] = grid0[d]; }
+  key.levels = levels; key.k = k; key.boxes = boxes_out; key.params_out = params_out;
+  std::memcpy(&key.params, &ctx->params, sizeof(ia_params));
+  key.wires = ctx->wires;
+  key.n_wires = ctx->n_wires;
+  auto fill_scratch = [&](RefineKey& kk) {
+    kk.scratch[0] = ctx->staged.p; kk.scratch[1] = ctx->votes.p; kk.scratch[2] = ctx->partial.p;
+    kk.scratch[3] = ctx->keys.p; kk.scratch[4] = ctx->misc.p;
+  };
+  fill_scratch(key);
+  RefineGraph& rg = ctx->rgraph;
+  const bool use_graphs = !(ctx->params.flags & 32u);
+  const bool same = rg.seen > 0 && std::memcmp(&rg.key, &key, sizeof(key)) == 0;
+  if (use_graphs && same && rg.exec) {
+    IA_CUDA(ctx, cudaGraphLaunch(rg.exec, ctx->stream));
+    ctx->launches += rg.launches;
+    return IA_OK;
+  }
+  auto enqueue = [&]() -> cudaError_t {
+    const int ne = sp.n_events;
+    cudaError_t e = launch_stage_hits(ctx, sp);
+    if (e != cudaSuccess) return e;
+    // level 0: dense start grid -> top k -> boxes
+    if ((e = scratch_reserve(ctx->votes, size_t(ne) * g.cells * sizeof(uint16_t))) != cudaSuccess) return e;
+    uint16_t* votes = static_cast<uint16_t*>(ctx->votes.p);
+    if ((e = launch_vote_dense(ctx, sp, g, votes)) != cudaSuccess) return e;
+    if ((e = scratch_reserve(ctx->misc, size_t(ne) * k * (sizeof(int64_t) + sizeof(uint16_t)) + 64)) != cudaSuccess) return e;
+    int64_t* idx = static_cast<int64_t*>(ctx->misc.p);
+    uint16_t* kv = reinterpret_cast<uint16_t*>(idx + size_t(ne) * k);
+    if ((e = launch_topk(ctx, votes, g.cells, ne, k, idx, kv)) != cudaSuccess) return e;
+    if ((e = launch_gather_dense(ctx, g, idx, kv, ne, k, levels, boxes_out)) != cudaSuccess) return e;
+    // levels 1..: subdivide, vote the children, keep the top k - all stream-ordered, no host round trip
+    for (int lev = 1; lev < levels; ++lev)
+      if ((e = launch_refine_level(ctx, sp, lev, levels, k, boxes_out)) != cudaSuccess) return e;
+    return launch_params(ctx, ne, levels, k, boxes_out, params_out);
+  };
+  if (use_graphs && same && rg.seen == 1) {
+    // second identical call: the scratch buffers have their final sizes (no allocation inside the capture)
+    const int64_t l0 = ctx->launches;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+      const cudaError_t eq = enqueue();
+      e = cudaStreamEndCapture(ctx->stream, &graph);
+      if (eq != cudaSuccess) e = eq;
+    }
+    const int64_t n_launch = ctx->launches - l0;
+    ctx->launches = l0;
+    if (e == cudaSuccess && graph) e = cudaGraphInstantiate(&rg.exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e == cudaSuccess && rg.exec) {
+      rg.launches = n_launch;
+      rg.seen = 2;
+      IA_CUDA(ctx, cudaGraphLaunch(rg.exec, ctx->stream));
+      ctx->launches += rg.launches;
+      return IA_OK;
+    }
+    // capture not possible here (e.g. the caller's stream is already capturing): run directly from now on
+    cudaGetLastError();
+    rg.exec = nullptr;
+    rg.seen = 3;
+  }
+  IA_CUDA(ctx, enqueue());
+  if (!same) {
+    if (rg.exec) cudaGraphExecDestroy(rg.exec);
+    rg.exec = nullptr;
+    rg.seen = 1;
+    fill_scratch(key);           // the pointers after this call's reservations
+    rg.key = key;
+  }
   return IA_OK;
 }
 
@@ -154,6 +215,7 @@ void ia_destroy(ia_ctx* ctx) {
                     &ctx->io_a,   &ctx->io_b,  &ctx->io_c,    &ctx->io_d};
   for (Scratch* s : all)
     if (s->p) cudaFree(s->p);
+  if (ctx->rgraph.exec) cudaGraphExecDestroy(ctx->rgraph.exec);
   if (ctx->wires) cudaFree(ctx->wires);
   if (ctx->status) cudaFree(ctx->status);
   delete ctx;
@@ -196,7 +258,7 @@ int ia_set_params(ia_ctx* ctx, const ia_params* p) {
       !std::isfinite(p->z_ref))
     return IA_ERR_ARG;
   if (p->precision != 64 && p->precision != 32) return IA_ERR_ARG;
-  if (p->flags & ~31u) return IA_ERR_ARG;
+  if (p->flags & ~63u) return IA_ERR_ARG;
   ctx->params = *p;
   return IA_OK;
 }

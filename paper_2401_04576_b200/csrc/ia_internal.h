@@ -31,6 +31,30 @@ struct Scratch {
 
 }  // namespace ia
 
+namespace ia {
+// Cached CUDA graph of one refinement call (ia_refine / ia_refine_batch).  A refinement is a fixed sequence of
+// small launches (C2: 38 of them for one event): the second call with the same arguments - same buffers, grid,
+// parameters and scratch - is captured, later ones are one cudaGraphLaunch.  Any difference re-records.
+struct RefineKey {
+  HitSpan sp;
+  double lo[5], hi[5];
+  int32_t grid[5];
+  int32_t levels, k;
+  const void* boxes;
+  const void* params_out;
+  ia_params params;
+  const void* wires;
+  int64_t n_wires;
+  const void* scratch[5];     // staged, votes, partial, keys, misc: the kernels of the graph point into them
+};
+struct RefineGraph {
+  RefineKey key;
+  int seen = 0;               // calls seen with this key (1: ran directly, 2+: graph)
+  cudaGraphExec_t exec = nullptr;
+  int64_t launches = 0;       // kernels inside the graph (for ia_launch_count)
+};
+}  // namespace ia
+
 struct ia_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
@@ -50,6 +74,7 @@ struct ia_ctx {
   int* status = nullptr;     // device: sticky error flag
   int64_t launches = 0;
   cudaError_t last_err = cudaSuccess;
+  ia::RefineGraph rgraph;
 };
 
 namespace ia {

@@ -486,3 +486,45 @@ def test_fast_path_primitives(rig0, prec):
         cmax = mp.mpf(1) if lo <= 0 <= hi else mp.cos(min(abs(lo), abs(hi)))
         assert mp.mpf(cc[i, 0]) <= cmin and cmax <= mp.mpf(cc[i, 1]) and cc[i, 1] <= 1.0, (e[i], cc[i])
         assert cmin - mp.mpf(cc[i, 0]) <= 10 * eps and mp.mpf(cc[i, 1]) - cmax <= 10 * eps, (e[i], cc[i])
+
+
+def test_refine_graph_replay_gives_the_same_boxes(rig1):
+    """ia_refine repeated with identical arguments is replayed as a CUDA graph from the third call on: results
+    identical to the direct path (flags bit 5), also after the hits in the same buffer change, after another call
+    in between, and with new output buffers."""
+    cfg = g.config(2)
+    ev = cfg.events[0]
+    hd, oh = rig1.hits(ev.wire, ev.drift)
+    ctx = rig1.ctx
+    ctx.ia_set_params(g.TOL, flags=32)
+    b0, p0 = ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k)
+    ctx.synchronize()
+    ref = (b.boxes_to_numpy(b0, (5, cfg.k)).copy(), p0.cpu().numpy().copy())
+    ctx.ia_set_params(g.TOL, flags=0)
+    boxes, par = ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k)
+    n_direct = None
+    for i in range(5):
+        l0 = ctx.ia_launch_count()
+        ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k, boxes=boxes, params=par)
+        ctx.synchronize()
+        n = ctx.ia_launch_count() - l0
+        n_direct = n if n_direct is None else n_direct
+        assert n == n_direct                                   # the launch count is the same on every path
+        gb = b.boxes_to_numpy(boxes, (5, cfg.k))
+        assert (gb["lo"] == ref[0]["lo"]).all() and (gb["votes"] == ref[0]["votes"]).all() and (par.cpu().numpy() == ref[1]).all()
+    # new content in the same hit buffer: the replayed graph reads it
+    ev2 = g.make_event(rig1.ch, 77, n_noise=20)
+    assert ev2.n_hits == ev.n_hits
+    hd.copy_(ctx.to_device(b.hits_of(ev2.wire, ev2.drift)))
+    ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k, boxes=boxes, params=par)
+    ctx.synchronize()
+    ob, opar = o.refine(rig1.owires, o.hits_of(ev2.wire, ev2.drift), rig1.oparams, LO, HI, cfg.grid, 5, cfg.k)
+    _assert_boxes_equal(b.boxes_to_numpy(boxes, (5, cfg.k)), ob)
+    # a different call in between (grows scratch, changes the key), then back
+    ctx.ia_vote(hd, ev.n_hits, LO, HI, (12,) * 5)
+    ctx.ia_refine(hd, ev.n_hits, LO, HI, (6,) * 5, 3, 4)
+    for _ in range(3):
+        ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k, boxes=boxes, params=par)
+    ctx.synchronize()
+    _assert_boxes_equal(b.boxes_to_numpy(boxes, (5, cfg.k)), ob)
+    assert (par.cpu().numpy() == opar).all()
