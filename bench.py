@@ -436,6 +436,11 @@ def main():
         "ncu_pipe_fp64_active_pct": 63.9, "ncu_source": "profiles/r01_vote_dense_fast_c1_ncu.md (C1, same kernel)",
         "alg_bytes_per_launch": 2 * n_cells, "hbm_frac": (2 * n_cells / (vote_ms * 1e-3)) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
     }
+    if clocks and clocks.get("sm_mhz"):
+        # the same fraction against the peak at the SM clock sampled during the timed region (the box runs this
+        # kernel under sw_power_cap at 1.87-1.92 GHz); roofline.frac keeps the maximum clock
+        roofline["frac_at_sampled_clock"] = achieved_inst / (n_sm * FP64_LANES_PER_SM * clocks["sm_mhz"] * 1e6)
+        roofline["sampled_sm_mhz"] = clocks["sm_mhz"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
