@@ -7,6 +7,7 @@
 // the atan2, the square root and the two divisions) into shared memory; every thread
 // then walks its cells, reads the hits by shared-memory broadcast, keeps its vote count in a
 // register and writes one uint16 per cell.  No atomics, no inter-thread traffic in the loop.
+#include <algorithm>
 #include <cmath>
 
 #include "ia_internal.h"
@@ -135,10 +136,12 @@ IA_DEV unsigned long long spread8(unsigned bits) {
 // RT: the sign class of a hit as a run-time value in one compiled body (coarse grids, where all three
 // classes are live on every SM and three bodies overflow the instruction cache) or as a template
 // argument of three bodies (fine grids: 6 % faster there).  Same arithmetic, same results.
-template <class T, bool RT>
+// SPLIT: the hit range is divided over blockIdx.z (small launches only; a separate instantiation so that the
+// main path keeps its code: with the split as a run-time case C1 and C3 ran 0.5-0.9 % slower).
+template <class T, bool RT, bool SPLIT>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z, int zt,
-                       uint16_t* __restrict__ votes) {
+                       int per_split, uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ZTab<T>* ztab = reinterpret_cast<ZTab<T>*>(smem_raw);
   HitF<T>* sh = reinterpret_cast<HitF<T>*>(smem_raw + sizeof(ZTab<T>));
@@ -163,7 +166,16 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   const T Lmag = mx(fabs(Rnd<T>::from_dn(g.lo[4])), fabs(Rnd<T>::from_up(g.hi[4])));
   T zref = T(0);
   if (count > 0) zref = staged[int64_t(e) * sp.max_hits].zref;
-  for (int h = threadIdx.x; h < count; h += blockDim.x) {
+  // small launches split the hit range over blockIdx.z (a single event on a coarse grid would otherwise leave every
+  // thread a serial chain of all its hits): block z votes the hits [z*per_split, (z+1)*per_split) into its own
+  // partial accumulator votes + z*(n_events*cells); sum_partial_votes_kernel adds them up - no atomics
+  const int h_begin = SPLIT ? blockIdx.z * per_split : 0;
+  const int h_end = SPLIT ? ((h_begin + per_split < count) ? h_begin + per_split : count) : count;
+  if (SPLIT) {
+    votes += int64_t(blockIdx.z) * (int64_t(gridDim.y) * g.cells);
+    sh -= h_begin;                                      // sh[h] for h in [h_begin, h_end)
+  }
+  for (int h = h_begin + threadIdx.x; h < h_end; h += blockDim.x) {
     const HitC<T> c = staged[int64_t(e) * sp.max_hits + h];
     make_hitf(xy_invariants(X, Y, c), hit_small(c), Rlo_min, Lmag, sh[h]);
   }
@@ -202,7 +214,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   pr.L2 = warp_fast ? mul_pp(pr.L, pr.L) : isqr(pr.L);
   unsigned long long acc = 0;
   const int va = a ? 1 : 0;
-  for (int h = 0; h < count; ++h) {
+  for (int h = h_begin; h < h_end; ++h) {
     const HitF<T>& hf = sh[h];
     const int kind = hf.kind[va];
     if (kind == HIT_SKIP) continue;
@@ -223,6 +235,15 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   if (live) {
     uint16_t* out = votes + int64_t(e) * g.cells + ixy * g.col_cells + (int64_t(iR) * nz + iz0) * nL + iL;
     for (int i = 0; i < nz_tile; ++i) out[int64_t(i) * nL] = uint16_t((acc >> (8 * i)) & 0xffu);
+  }
+}
+
+// partial accumulators of a hit-split launch -> the accumulator (deterministic, no atomics)
+__global__ void sum_partial_votes_kernel(const uint16_t* __restrict__ partial, int n_splits, int64_t n, uint16_t* __restrict__ votes) {
+  for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
+    unsigned v = 0;
+    for (int s = 0; s < n_splits; ++s) v += partial[int64_t(s) * n + i];
+    votes[i] = uint16_t(v);
   }
 }
 
@@ -353,25 +374,52 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   const int64_t nxy = int64_t(g.n[0]) * g.n[1];
   const int64_t blocks = nxy * tiles_p * tiles_z;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-  const size_t smem = sizeof(ZTab<T>) + size_t(sp.max_hits) * sizeof(HitF<T>);
+  // still too few warps to hide the latency of a thread's serial chain over its hits (one event on a coarse grid):
+  // split the hits over blockIdx.z, up to 8 ways, aiming at 32 warps per SM
+  int n_splits = 1;
+  {
+    const int64_t warps = blocks * sp.n_events * ((threads + 31) / 32);
+    const int64_t want = int64_t(32) * n_sm;
+    if (warps < want / 2) n_splits = int(std::min<int64_t>(8, (want + warps - 1) / warps));
+    if (n_splits > sp.max_hits) n_splits = sp.max_hits > 0 ? sp.max_hits : 1;
+  }
+  const int per_split = (sp.max_hits + n_splits - 1) / (n_splits > 0 ? n_splits : 1);
+  n_splits = per_split > 0 ? (sp.max_hits + per_split - 1) / per_split : 1;
+  const size_t smem = sizeof(ZTab<T>) + size_t(per_split) * sizeof(HitF<T>);
+  uint16_t* target = votes_out;
+  const int64_t n_acc = int64_t(sp.n_events) * g.cells;
+  cudaError_t err;
+  if (n_splits > 1) {
+    err = scratch_reserve(ctx->partial, size_t(n_splits) * n_acc * sizeof(uint16_t));
+    if (err != cudaSuccess) return err;
+    target = static_cast<uint16_t*>(ctx->partial.p);
+  }
   // coarse = an xy cell is wider than half the chamber radius: the classes of s_Ax, c_Ax then vary from
   // hit to hit inside every block (measured: C3's 8^5 start grid runs 28 % faster with the one-body form,
-  // C1's 32^5 grid 6 % slower)
+  // C1's 32^5 grid about the same, C4's 64^5 grid 0.7 % slower)
   const double wxy = std::fmin((g.hi[0] - g.lo[0]) / g.n[0], (g.hi[1] - g.lo[1]) / g.n[1]);
   const bool coarse = (ctx->params.flags & 2u) ? true : ((ctx->params.flags & 4u) ? false : wxy > 0.5 * ctx->max_wire_r);
-  dim3 grid((unsigned)blocks, (unsigned)sp.n_events);
-  cudaError_t err;
-  if (coarse) {
-    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    if (err != cudaSuccess) return err;
-    vote_dense_fast_kernel<T, true><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
-                                                                         tiles_p, tiles_z, zt, votes_out);
+  dim3 grid((unsigned)blocks, (unsigned)sp.n_events, (unsigned)n_splits);
+  const HitC<T>* staged = static_cast<const HitC<T>*>(ctx->staged.p);
+#define IA_LAUNCH_FAST(RT_, SPLIT_)                                                                                          \
+  do {                                                                                                                       \
+    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
+    if (err != cudaSuccess) return err;                                                                                      \
+    vote_dense_fast_kernel<T, RT_, SPLIT_><<<grid, threads, smem, ctx->stream>>>(sp, staged, g, tiles_p, tiles_z, zt, per_split, \
+                                                                                  target);                                      \
+  } while (0)
+  if (n_splits > 1) {
+    if (coarse) IA_LAUNCH_FAST(true, true); else IA_LAUNCH_FAST(false, true);
   } else {
-    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-    if (err != cudaSuccess) return err;
-    vote_dense_fast_kernel<T, false><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
-                                                                          tiles_p, tiles_z, zt, votes_out);
+    if (coarse) IA_LAUNCH_FAST(true, false); else IA_LAUNCH_FAST(false, false);
   }
+#undef IA_LAUNCH_FAST
+  ctx->launches++;
+  err = cudaGetLastError();
+  if (err != cudaSuccess || n_splits == 1) return err;
+  int sum_blocks = int((n_acc + 1023) / 1024);
+  if (sum_blocks > 8 * n_sm) sum_blocks = 8 * n_sm;
+  sum_partial_votes_kernel<<<sum_blocks, 256, 0, ctx->stream>>>(target, n_splits, n_acc, votes_out);
   ctx->launches++;
   return cudaGetLastError();
 }
