@@ -247,17 +247,41 @@ __global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t
   const int s = pick_acc(acc, which);
   const unsigned vmax = unsigned(acc[s]);
   const uint16_t* v = votes + int64_t(s) * n;
+  // per-thread, then per-warp partial results; 13 atomics per warp at the end (a plateau can hold every voxel)
+  unsigned long long cnt = 0, sum[4] = {0, 0, 0, 0};
+  unsigned kmin[4] = {~0u, ~0u, ~0u, ~0u}, kmax[4] = {0, 0, 0, 0};
   for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
     if (unsigned(v[i]) != vmax) continue;
     int64_t idx = i;
-    atomicAdd(&acc[2], 1ull);
+    ++cnt;
 #pragma unroll
     for (int d = 3; d >= 0; --d) {
-      const unsigned long long k = (unsigned long long)(idx % g.n[d]);
+      const unsigned k = unsigned(idx % g.n[d]);
       idx /= g.n[d];
-      atomicAdd(&acc[3 + d], k);
-      atomicMin(&acc[7 + d], k);
-      atomicMax(&acc[11 + d], k);
+      sum[d] += k;
+      kmin[d] = min(kmin[d], k);
+      kmax[d] = max(kmax[d], k);
+    }
+  }
+  const bool lead = (threadIdx.x & 31) == 0;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    cnt += __shfl_down_sync(0xffffffffu, cnt, off);
+#pragma unroll
+    for (int d = 0; d < 4; ++d) sum[d] += __shfl_down_sync(0xffffffffu, sum[d], off);
+  }
+#pragma unroll
+  for (int d = 0; d < 4; ++d) {
+    kmin[d] = __reduce_min_sync(0xffffffffu, kmin[d]);
+    kmax[d] = __reduce_max_sync(0xffffffffu, kmax[d]);
+  }
+  if (lead && cnt != 0) {
+    atomicAdd(&acc[2], cnt);
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      atomicAdd(&acc[3 + d], sum[d]);
+      atomicMin(&acc[7 + d], (unsigned long long)kmin[d]);
+      atomicMax(&acc[11 + d], (unsigned long long)kmax[d]);
     }
   }
 }

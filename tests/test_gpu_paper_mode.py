@@ -258,3 +258,22 @@ def test_track_paper_recovers_the_generated_helix():
         assert (np.median(dev, axis=0) < np.array([0.1, 0.1, 0.1, 2.0])).all(), np.median(dev, axis=0)
     finally:
         rig.close()
+
+
+def test_f2_selection_when_every_voxel_is_selected():
+    """a plateau that holds the whole grid (all counts equal): the centre of the grid and half its size, also on a
+    grid of millions of voxels (the reduction aggregates per warp before its atomics)."""
+    import torch
+    rig = Rig(g.chamber_c0())
+    try:
+        dims = (64, 64, 32, 16)
+        n = int(np.prod(dims))
+        v = torch.full((2 * n,), 5, dtype=torch.int16, device="cuda").view(torch.uint16)
+        fit_dev = rig.ctx.ia_select_max_paper(v, 300.0, PLO, PHI, dims)
+        rig.ctx.synchronize()
+        f = _fit_to_host(fit_dev)
+        assert f["n_sel"] == n and f["vmax"] == 5 and f["lambda_sign"] == 1
+        assert np.allclose(f["value"], 0.5 * (PLO + PHI), rtol=0, atol=1e-9)
+        assert np.allclose(f["error"], 0.5 * (PHI - PLO), rtol=0, atol=1e-9)
+    finally:
+        rig.close()
