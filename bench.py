@@ -219,6 +219,12 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16):
                         "lambda-sign chains",
             "ms_per_track": ms, "tracks_per_s": 1e3 / ms, "launches_per_track": int(launches), "n_tracks": n_tracks,
             "lambda_sign_correct": sign_ok / n_tracks,
+            # the paper's efficiency criterion (L123): |d xc|, |d yc|, |d R| < 1 mm and |d z0| < 10 mm; and a looser one at
+            # the size of the last pass's voxels (1 mm x 40 mm): 3 mm and 40 mm
+            "frac_within_1mm_10mm": float(np.mean((dev[:, :3] < 0.1).all(axis=1) & (dev[:, 3] < 1.0))),
+            "frac_within_3mm_40mm": float(np.mean((dev[:, :3] < 0.3).all(axis=1) & (dev[:, 3] < 4.0))),
+            "rms_dev_cm": {"xc": float(np.sqrt(np.mean(dev[:, 0] ** 2))), "yc": float(np.sqrt(np.mean(dev[:, 1] ** 2))),
+                           "R": float(np.sqrt(np.mean(dev[:, 2] ** 2))), "z0": float(np.sqrt(np.mean(dev[:, 3] ** 2)))},
             "median_abs_dev_cm": {"xc": float(np.median(dev[:, 0])), "yc": float(np.median(dev[:, 1])),
                                   "R": float(np.median(dev[:, 2])), "z0": float(np.median(dev[:, 3]))},
             "context": "paper: about 1.2 s per track on 4 x K80, about 0.2 s on V100 (L117)"}
