@@ -180,7 +180,7 @@ def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
             "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
 
 
-def paper_track_leg(local_rank: int, n_tracks: int = 16):
+def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0):
     """SURVEY 8(f) f2 + f4: the paper's three-pass scheme (Table 1 in cm) as one ia_track_paper call per track on
     paper-shaped events (5,000-wire chamber, 105 MeV/c, 19-57 hits); time per track with the hits resident."""
     import torch
@@ -190,7 +190,11 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16):
     ctx.ia_load_geometry(b.wires_of(ch))
     ctx.ia_set_params(0.0, flags=8)
     lo, hi = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
-    ps = np.zeros(3, b.PASS_DT)
+    # beyond Table 1 (--f2-extra-passes): finer windows around the third pass's value - 0.2 mm voxels, then 0.05 mm
+    extra = [((0.5, 0.5, 0.5, 8.0), (50, 50, 50, 16)), ((0.1, 0.1, 0.1, 2.0), (40, 40, 40, 16))][:extra_passes]
+    ps = np.zeros(3 + len(extra), b.PASS_DT)
+    for j, (half, dims) in enumerate(extra):
+        ps[3 + j]["lo"], ps[3 + j]["hi"], ps[3 + j]["dims"], ps[3 + j]["windowed"] = half, half, dims, 1
     ps[0]["lo"], ps[0]["hi"], ps[0]["dims"] = lo, hi, (50, 50, 40, 20)
     ps[1]["lo"], ps[1]["hi"], ps[1]["dims"] = lo, hi, (90, 90, 40, 20)
     ps[2]["lo"], ps[2]["hi"], ps[2]["dims"], ps[2]["windowed"] = (2.5, 2.5, 2.5, 40.0), (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20), 1
@@ -208,15 +212,16 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16):
     launches = (ctx.ia_launch_count() - l0) // n_tracks
     dev, sign_ok = [], 0
     for (fits, sign), e in zip(outs, evs):
-        f = np.frombuffer(fits.cpu().numpy().tobytes(), dtype=b.FIT_DT).reshape(3, 2)
+        f = np.frombuffer(fits.cpu().numpy().tobytes(), dtype=b.FIT_DT).reshape(len(ps), 2)
         s = int(sign.cpu().numpy()[0])
         sign_ok += s == (1 if e.track.lam >= 0 else -1)
-        dev.append(np.abs(np.array(f[2, 0 if s > 0 else 1]["value"]) - np.array(e.track.params[:4])))
+        dev.append(np.abs(np.array(f[-1, 0 if s > 0 else 1]["value"]) - np.array(e.track.params[:4])))
     dev = np.array(dev)
     ctx.close()
     return {"workload": "f2/f4: paper-shaped chamber (20 layers x 250 wires, r 49.6-83.7 cm, tau +/-0.1), 105 MeV/c tracks from the "
                         "origin, noise-free hits (L88); passes 50x50x40x20, 90x90x40x20 (global), 50x50x50x20 (window), both "
                         "lambda-sign chains",
+            "extra_window_passes": len(extra),
             "ms_per_track": ms, "tracks_per_s": 1e3 / ms, "launches_per_track": int(launches), "n_tracks": n_tracks,
             "lambda_sign_correct": sign_ok / n_tracks,
             # the paper's efficiency criterion (L123): |d xc|, |d yc|, |d R| < 1 mm and |d z0| < 10 mm; and a looser one at
@@ -304,6 +309,8 @@ def main():
     ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1", "F2"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
+    ap.add_argument("--f2-extra-passes", type=int, default=0, choices=[0, 1, 2],
+                    help="workload F2: finer window passes after the paper's three (0.2 mm voxels, then 0.05 mm)")
     ap.add_argument("--flags", type=int, default=0, help="ia_params.flags for the dense workloads (1: general kernel, 16: rigorous Phi)")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
@@ -332,7 +339,7 @@ def main():
 
     if args.workload == "F2":
         barrier()
-        r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1))
+        r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1), extra_passes=args.f2_extra_passes)
         if rank == 0:
             print(json.dumps({"metric": "paper-scheme tracks/s", "value": r["tracks_per_s"] * world, "unit": "tracks/s",
                               "n_gpus": world, "steps": args.steps, "warmup": 1, "ms_per_step": r["ms_per_track"],
