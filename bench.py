@@ -180,7 +180,8 @@ def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
             "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
 
 
-def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0):
+def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0, n_noise: int = 0, smear: float = 0.0,
+                    tol: float = 0.0):
     """SURVEY 8(f) f2 + f4: the paper's three-pass scheme (Table 1 in cm) as one ia_track_paper call per track on
     paper-shaped events (5,000-wire chamber, 105 MeV/c, 19-57 hits); time per track with the hits resident."""
     import torch
@@ -188,7 +189,7 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0):
     ch = g.chamber_paper()
     ctx = b.Context(local_rank)
     ctx.ia_load_geometry(b.wires_of(ch))
-    ctx.ia_set_params(0.0, flags=8)
+    ctx.ia_set_params(tol, flags=8)
     lo, hi = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
     # beyond Table 1 (--f2-extra-passes): finer windows around the third pass's value - 0.2 mm voxels, then 0.05 mm
     extra = [((0.5, 0.5, 0.5, 8.0), (50, 50, 50, 16)), ((0.1, 0.1, 0.1, 2.0), (40, 40, 40, 16))][:extra_passes]
@@ -198,7 +199,7 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0):
     ps[0]["lo"], ps[0]["hi"], ps[0]["dims"] = lo, hi, (50, 50, 40, 20)
     ps[1]["lo"], ps[1]["hi"], ps[1]["dims"] = lo, hi, (90, 90, 40, 20)
     ps[2]["lo"], ps[2]["hi"], ps[2]["dims"], ps[2]["windowed"] = (2.5, 2.5, 2.5, 40.0), (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20), 1
-    evs = [g.make_event_paper(ch, 500 + i) for i in range(n_tracks)]
+    evs = [g.make_event_paper(ch, 500 + i, n_noise=n_noise, smear=smear) for i in range(n_tracks)]
     hds = [ctx.to_device(b.hits_of(e.wire, e.drift)) for e in evs]
     outs = [ctx.ia_track_paper(hds[0], evs[0].n_hits, g.PAPER_P, ps)]            # warm-up
     torch.cuda.synchronize()
@@ -221,7 +222,7 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0):
     return {"workload": "f2/f4: paper-shaped chamber (20 layers x 250 wires, r 49.6-83.7 cm, tau +/-0.1), 105 MeV/c tracks from the "
                         "origin, noise-free hits (L88); passes 50x50x40x20, 90x90x40x20 (global), 50x50x50x20 (window), both "
                         "lambda-sign chains",
-            "extra_window_passes": len(extra),
+            "extra_window_passes": len(extra), "noise_hits": n_noise, "smear_cm": smear, "tol_cm": tol,
             "ms_per_track": ms, "tracks_per_s": 1e3 / ms, "launches_per_track": int(launches), "n_tracks": n_tracks,
             "lambda_sign_correct": sign_ok / n_tracks,
             # the paper's efficiency criterion (L123): |d xc|, |d yc|, |d R| < 1 mm and |d z0| < 10 mm; and a looser one at
@@ -311,6 +312,9 @@ def main():
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--f2-extra-passes", type=int, default=0, choices=[0, 1, 2],
                     help="workload F2: finer window passes after the paper's three (0.2 mm voxels, then 0.05 mm)")
+    ap.add_argument("--f2-noise", type=int, default=0, help="workload F2: noise hits per event (the paper has none)")
+    ap.add_argument("--f2-smear", type=float, default=0.0, help="workload F2: drift-distance smearing, cm (the paper has none)")
+    ap.add_argument("--f2-tol", type=float, default=0.0, help="workload F2: vote tolerance, cm")
     ap.add_argument("--flags", type=int, default=0, help="ia_params.flags for the dense workloads (1: general kernel, 16: rigorous Phi)")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
@@ -339,7 +343,8 @@ def main():
 
     if args.workload == "F2":
         barrier()
-        r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1), extra_passes=args.f2_extra_passes)
+        r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1), extra_passes=args.f2_extra_passes,
+                            n_noise=args.f2_noise, smear=args.f2_smear, tol=args.f2_tol)
         if rank == 0:
             print(json.dumps({"metric": "paper-scheme tracks/s", "value": r["tracks_per_s"] * world, "unit": "tracks/s",
                               "n_gpus": world, "steps": args.steps, "warmup": 1, "ms_per_step": r["ms_per_track"],
