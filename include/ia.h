@@ -46,7 +46,11 @@ enum {
   IA_ERR_CUDA = -5      /* a CUDA runtime call failed; see ia_last_cuda_error()                     */
 };
 
-#define IA_MAX_HITS 1024 /* per event: staged hits must fit one CTA's shared memory                */
+/* Hits per event.  SURVEY 8(b) proposed 65,535 (the range of the uint16 accumulator); the bound built is 1,024:
+ * every vote kernel stages one event's hits in the shared memory of a CTA and reads them by broadcast
+ * (120 B per hit in the explicit-box kernels, 184 B in the general dense kernel: 1,024 hits = 188 KB of the
+ * 227 KB a CTA can have), and the paper's events hold 25-62 hits (L88).  More hits return IA_ERR_CAPACITY. */
+#define IA_MAX_HITS 1024
 #define IA_MAX_K 32      /* top-K list = one key per lane of a warp                                */
 
 typedef struct ia_ctx ia_ctx; /* opaque: device geometry, parameters, stream, scratch */
@@ -227,6 +231,14 @@ int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hi
 int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
                 int64_t n_boxes, double* out_dev);
 
+/* The same record from the sign-specialised ("fast") form that the dense and children kernels run, for the cell
+ * [lo, hi] taken as a one-cell grid: slot 3 = form (0: fast form, scale = R_Ax^2.hi; 1: forced vote; 2: this
+ * (box, hit) takes the general form - guards of the fast form, lambda straddling 0 - whose enclosure is written;
+ * 3: invalid hit).  The two forms enclose the same function f of eq. (2) with different roundings; the tests bound
+ * their difference (the FP32 variant uses the fast form as a filter in front of the general one). */
+int ia_residual_fast(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
+                     int64_t n_boxes, double* out_dev);
+
 /* Device interval primitives exposed for unit tests: n independent operations
  * out_dev[i] = op(a_dev[i], b_dev[i]) on intervals stored as (lo, hi) pairs of doubles; prec = 64 or 32.
  * op: 0 add 1 sub 2 mul 3 sqr(a) 4 div(a, b>0) 5 sqrt(a) 6 sin(a) 7 cos(a) 8 atan2(y=a, x=b)
@@ -256,6 +268,10 @@ int ia_device_status(ia_ctx* ctx);
 
 /* Number of kernels this context has launched so far (for the bench's gpu_launches). */
 int64_t ia_launch_count(const ia_ctx* ctx);
+
+/* Number of ia_refine / ia_refine_batch calls of this context that were served by replaying the cached CUDA graph of
+ * the call (third identical call on; needs a capturable stream, i.e. not the legacy default stream). */
+int64_t ia_graph_replays(const ia_ctx* ctx);
 
 const char* ia_strerror(int code);
 const char* ia_last_cuda_error(const ia_ctx* ctx);

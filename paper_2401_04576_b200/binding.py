@@ -27,8 +27,8 @@ PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,))
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 88
 
 EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
-           "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_prim",
-           "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
+           "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_residual_fast", "ia_prim",
+           "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_graph_replays", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
 
 class IaParams(C.Structure):
@@ -72,11 +72,14 @@ def load_library(path: str = LIB_PATH):
     lib.ia_vote_host.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_refine_batch_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_residual.argtypes = [vp, vp, i32, vp, vp, i64, vp]
+    lib.ia_residual_fast.argtypes = [vp, vp, i32, vp, vp, i64, vp]
     lib.ia_prim.argtypes = [vp, i32, i32, vp, vp, i64, vp]
     lib.ia_probe_fp64.argtypes = [vp, i32, i32, i32, vp]
     lib.ia_device_status.argtypes = [vp]
     lib.ia_launch_count.argtypes = [vp]
     lib.ia_launch_count.restype = i64
+    lib.ia_graph_replays.argtypes = [vp]
+    lib.ia_graph_replays.restype = i64
     lib.ia_strerror.argtypes = [i32]
     lib.ia_strerror.restype = C.c_char_p
     lib.ia_last_cuda_error.argtypes = [vp]
@@ -318,6 +321,13 @@ class Context:
         self._chk(self.lib.ia_residual(self.h, _dp(hits_dev), n_hits, _dp(lo_dev), _dp(hi_dev), n, _dp(out)), "ia_residual")
         return out.view(n, n_hits, 2, 4)
 
+    def ia_residual_fast(self, hits_dev, n_hits, lo_dev, hi_dev):
+        torch = self._torch
+        n = lo_dev.numel() // 5
+        out = self._empty(n * n_hits * 2 * 4, torch.float64)
+        self._chk(self.lib.ia_residual_fast(self.h, _dp(hits_dev), n_hits, _dp(lo_dev), _dp(hi_dev), n, _dp(out)), "ia_residual_fast")
+        return out.view(n, n_hits, 2, 4)
+
     def ia_prim(self, op, prec, a_dev, b_dev=None):
         torch = self._torch
         n = a_dev.numel() // 2
@@ -343,6 +353,9 @@ class Context:
 
     def ia_launch_count(self) -> int:
         return int(self.lib.ia_launch_count(self.h))
+
+    def ia_graph_replays(self) -> int:
+        return int(self.lib.ia_graph_replays(self.h))
 
     def synchronize(self):
         self.stream.synchronize()

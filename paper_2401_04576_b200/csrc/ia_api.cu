@@ -111,6 +111,7 @@ int refine_impl(ia_ctx* ctx, const HitSpan& sp, const double lo[5], const double
   const bool same = rg.seen > 0 && std::memcmp(&rg.key, &key, sizeof(key)) == 0;
   if (use_graphs && same && rg.exec) {
     IA_CUDA(ctx, cudaGraphLaunch(rg.exec, ctx->stream));
+    ctx->graph_replays++;
     ctx->launches += rg.launches;
     return IA_OK;
   }
@@ -150,6 +151,7 @@ int refine_impl(ia_ctx* ctx, const HitSpan& sp, const double lo[5], const double
       rg.launches = n_launch;
       rg.seen = 2;
       IA_CUDA(ctx, cudaGraphLaunch(rg.exec, ctx->stream));
+      ctx->graph_replays++;
       ctx->launches += rg.launches;
       return IA_OK;
     }
@@ -510,6 +512,19 @@ int ia_residual(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* l
   return IA_OK;
 }
 
+int ia_residual_fast(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
+                     int64_t n_boxes, double* out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits <= 0 || !hits_dev || n_boxes <= 0 || !lo_dev || !hi_dev || !out_dev) return IA_ERR_ARG;
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  DeviceGuard guard(ctx->device);
+  HitSpan sp = single_span(hits_dev, n_hits);
+  IA_CUDA(ctx, launch_stage_hits(ctx, sp));
+  IA_CUDA(ctx, launch_residual_fast(ctx, sp, lo_dev, hi_dev, n_boxes, out_dev));
+  return IA_OK;
+}
+
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev) {
   if (!ctx || !a_dev || !out_dev || n < 0 || op < 0 || op > 17 || (prec != 64 && prec != 32)) return IA_ERR_ARG;
   const bool binary = (op == 0 || op == 1 || op == 2 || op == 4 || op == 8 || op == 10 || op == 11 || op == 12 || op == 13);
@@ -537,6 +552,8 @@ int ia_device_status(ia_ctx* ctx) {
 }
 
 int64_t ia_launch_count(const ia_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int64_t ia_graph_replays(const ia_ctx* ctx) { return ctx ? ctx->graph_replays : 0; }
 
 const char* ia_strerror(int code) {
   switch (code) {

@@ -338,6 +338,32 @@ template <class T> IA_DEV void trig_small(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
   ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? T(1) : chi};   // cos > 0.96
 }
 
+// ---- the FP32 fast form as a floating-point filter ---------------------------------------------------
+// The sign-specialised form and the general form enclose the same function but round differently (fused FMAs, midpoint-
+// radius products, re-associated constants): their endpoints of f differ by a few ulps of the residual's scale
+// (max(R_Ax^2, (R + d_Ax)^2); at a sign change of f both are equal).  In double that is 1e-15 relative, 3 orders inside
+// the 1e-12 knife-edge band of the parity criterion, and changes no decision in practice.  In float it is 1e-6 of f's
+// scale against cells whose f varies by 1e-3 of it at the deep refinement levels: one vote in 10^4 flipped, and C3's
+// kept boxes differed from the oracle's in 1 event of 1,024.  So the float fast form only DECIDES when both endpoints of
+// one sign's f are further than `band` = 2^-20 * R_Ax^2.hi (8 ulps of the scale; the two forms differ by at most
+// 5 roundings of scale-sized terms, tests/test_gpu_parity.py checks <= 4 ulps on 10^6 evaluations) from zero, or
+// when both signs exclude by that margin; anything closer is re-evaluated in the general form, which does the
+// oracle's arithmetic operation for operation.
+template <class T> struct Filter;
+template <> struct Filter<double> { static constexpr bool on = false; static IA_DEV double rel() { return 0.0; } };
+template <> struct Filter<float> { static constexpr bool on = true; static IA_DEV float rel() { return 0x1p-20f; } };
+// bit 0: the vote; bit 1: ambiguous (float only) - the caller re-takes the decision in the general form
+template <class T> IA_DEV unsigned decide(const Iv<T> (&f)[2], T band) {
+  const bool v0 = !(is_pos(f[0].lo) || f[0].hi < T(0)), v1 = !(is_pos(f[1].lo) || f[1].hi < T(0));
+  unsigned r = (v0 || v1) ? 1u : 0u;
+  if (Filter<T>::on) {
+    const bool in0 = f[0].lo < -band && f[0].hi > band, in1 = f[1].lo < -band && f[1].hi > band;
+    const bool out0 = f[0].lo > band || f[0].hi < -band, out1 = f[1].lo > band || f[1].hi < -band;
+    if (!(in0 || in1 || (out0 && out1))) r |= 2u;
+  }
+  return r;
+}
+
 // ---- per-(block, hit) record in shared memory ------------------------------------------------------
 // HIT_FAST_P / _N / _U: the three bodies (SS = +1, -1, 0)
 enum { HIT_SKIP = 0, HIT_FORCED = 1, HIT_FAST_P = 2, HIT_FAST_N = 3, HIT_FAST_U = 4, HIT_GENERAL = 5 };
@@ -357,6 +383,7 @@ template <class T> struct __align__(16) HitF {
   T Tabs;                          // |tan tau|
   T Dlo, Dhi;
   T DloP, DhiP;                    // D+ padded outward by 2^-50 (2^-21): absorbs the error of rsqrt_near
+  T band;                          // FP32 filter: decisions with an endpoint of f within +-band of 0 are re-taken in the general form
   int kind[2];                     // per a
   int c2cls;
   int zflip;                       // z0 - z_ref enters negated
@@ -378,6 +405,7 @@ template <class T> IA_DEV void make_hitf(const XYInv<T>& v, const HitS<T>& hs, T
   o.DloP = Rd::fma_dn(-hs.Dlo, Rd::pad_rel(), hs.Dlo);
   o.DhiP = Rd::fma_up(hs.Dhi, Rd::pad_rel(), hs.Dhi);
   o.c2cls = cls_of(v.c2);
+  o.band = Rd::mul_up(v.Q.hi, Filter<T>::rel());
   const bool t = hs.Tn < T(0);
   const bool b = cls_of(v.cA) == CLS_N;
   o.cA = b ? ineg(v.cA) : v.cA;

@@ -216,6 +216,7 @@ template <> struct QDir<float> {
 // Inputs transformed as in ia_fast.cuh: L >= 0, T = h.Tabs >= 0, cA >= 0 (SS != 0) or any (SS == 0).
 template <int SS, class T>
 IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
+  // returns decide(): bit 0 the vote, bit 1 (float only) "too close to call in this form"
   using V = VR<T>;
   const T Tn = h.Tabs;
   constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
@@ -309,8 +310,7 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
 #pragma unroll
   for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q.lo, -r2[s].hi); f[s].hi = V::add_up(h.Q.hi, -r2[s].lo); }
   // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
-  const bool v0 = !(is_pos(f[0].lo) || f[0].hi < T(0)), v1 = !(is_pos(f[1].lo) || f[1].hi < T(0));
-  return (v0 || v1) ? 1u : 0u;
+  return decide(f, h.band);
 }
 
 // ---- one body for all three sign classes ----------------------------------------------------------
@@ -325,7 +325,7 @@ IA_DEV int opaque_i(int x) { asm volatile("" : "+r"(x)); return x; }
 
 template <class T>
 IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp,
-                             Iv<T> Zr, MR<T> sAm, MR<T> s2m, Iv<T> sAabs, Iv<T> sA2abs) {
+                             Iv<T> Zr, MR<T> sAm, MR<T> s2m, Iv<T> sAabs, Iv<T> sA2abs, Iv<T>* fout = nullptr) {
   using V = VR<T>;
   const T Tn = h.Tabs;
   // sAm, s2m: negated for the class s_Ax <= 0; sAabs, sA2abs: s_Ax and 2 s_Ax, negated for that class
@@ -441,8 +441,8 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   for (int s = 0; s < 2; ++s) { r2[s].lo = V::fma_dn(-TLq[s].hi, TLq[s].hi, r2[s].lo); r2[s].hi = V::fma_up(-TLq[s].lo, TLq[s].lo, r2[s].hi); }
 #pragma unroll
   for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q.lo, -r2[s].hi); f[s].hi = V::add_up(h.Q.hi, -r2[s].lo); }
-  const bool v0 = !(is_pos(f[0].lo) || f[0].hi < T(0)), v1 = !(is_pos(f[1].lo) || f[1].hi < T(0));
-  return (v0 || v1) ? 1u : 0u;
+  if (fout) { fout[0] = f[0]; fout[1] = f[1]; }       // diagnostics (ia_residual_fast); nullptr in the vote kernels
+  return decide(f, h.band);
 }
 
 }  // namespace ia

@@ -73,6 +73,7 @@ struct ia_ctx {
   ia::Scratch io_a, io_b, io_c, io_d;   // *_host entry points: device mirrors of host buffers
   int* status = nullptr;     // device: sticky error flag
   int64_t launches = 0;
+  int64_t graph_replays = 0;  // refinement calls served by cudaGraphLaunch
   cudaError_t last_err = cudaSuccess;
   ia::RefineGraph rgraph;
 };
@@ -92,6 +93,10 @@ cudaError_t launch_vote_boxes(ia_ctx* ctx, const HitSpan& span, const double* lo
 
 cudaError_t launch_residual(ia_ctx* ctx, const HitSpan& span, const double* lo, const double* hi, int64_t n_boxes,
                             double* out);
+
+// the same record from the sign-specialised form of the dense kernel (ia_vote_dense.cu)
+cudaError_t launch_residual_fast(ia_ctx* ctx, const HitSpan& span, const double* lo, const double* hi, int64_t n_boxes,
+                                 double* out);
 
 cudaError_t launch_prim(ia_ctx* ctx, int op, int prec, const double* a, const double* b, int64_t n, double* out);
 

@@ -291,6 +291,14 @@ cudaError_t launch_vote_boxes(ia_ctx* ctx, const HitSpan& sp, const double* lo, 
                               uint16_t* votes_out) {
   if (n_boxes <= 0) return cudaSuccess;
   const unsigned blocks = unsigned((n_boxes + 127) / 128);
+  // up to IA_MAX_HITS staged hits (120 B each in double) exceed the 48 KB default of dynamic shared memory
+  cudaError_t aerr = cudaSuccess;
+  IA_DISPATCH_PREC(ctx,
+    (aerr = cudaFuncSetAttribute(vote_boxes_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 int(sp.max_hits * sizeof(HitC<double>)))),
+    (aerr = cudaFuncSetAttribute(vote_boxes_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 int(sp.max_hits * sizeof(HitC<float>)))));
+  if (aerr != cudaSuccess) return aerr;
   IA_DISPATCH_PREC(ctx,
     (vote_boxes_kernel<double><<<blocks, 128, sp.max_hits * sizeof(HitC<double>), ctx->stream>>>(
         sp, static_cast<const HitC<double>*>(ctx->staged.p), lo, hi, n_boxes, votes_out)),
@@ -346,12 +354,19 @@ cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int lev
     n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
     if (n_splits > sp.max_hits) n_splits = sp.max_hits;
     if (n_splits < 1) n_splits = 1;
-    const int per_split = (sp.max_hits + n_splits - 1) / n_splits;
-    n_splits = (sp.max_hits + per_split - 1) / per_split;
+    int per_split = (sp.max_hits + n_splits - 1) / n_splits;
+    if (per_split < 1) per_split = 1;                   // no hits at all: one split that votes nothing
+    n_splits = sp.max_hits > 0 ? (sp.max_hits + per_split - 1) / per_split : 1;
     err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
     if (err != cudaSuccess) return err;
     partial = static_cast<uint16_t*>(ctx->partial.p);
     dim3 grid(n_splits, sp.n_events, (threads + 255) / 256);
+    IA_DISPATCH_PREC(ctx,
+      (err = cudaFuncSetAttribute(vote_children_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  int(per_split * sizeof(HitC<double>)))),
+      (err = cudaFuncSetAttribute(vote_children_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  int(per_split * sizeof(HitC<float>)))));
+    if (err != cudaSuccess) return err;
     IA_DISPATCH_PREC(ctx,
       (vote_children_kernel<double><<<grid, 256, per_split * sizeof(HitC<double>), ctx->stream>>>(
           sp, static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),

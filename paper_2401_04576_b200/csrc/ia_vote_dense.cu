@@ -102,13 +102,32 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
 }
 
 // one hit, one thread: both drift signs over the thread's z0 cells; returns the vote mask (bit i = z0 cell i)
+// (float: bit 8 + i set = cell i is too close to call in this form, see Filter in ia_fast.cuh)
 template <int SS, class T>
 IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
   const Pass2<T> pc2 = pass_prepare2(h, p, hp);
   unsigned bits = 0;
 #pragma unroll 1
-  for (int i = 0; i < nz_tile; ++i) bits |= pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]) << i;
+  for (int i = 0; i < nz_tile; ++i) {
+    const unsigned r = pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]);
+    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << 7)) << i : r << i;
+  }
+  return bits;
+}
+
+// float: the cells the fast form could not decide are re-taken in the general form (which does the oracle's arithmetic)
+template <class T>
+IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L, const Iv<T>* zt) {
+  if (Filter<T>::on) {
+    unsigned amb = bits >> 8;
+    bits &= 0xffu;
+    while (amb) {
+      const int i = __ffs(amb) - 1;
+      amb &= amb - 1;
+      bits = (bits & ~(1u << i)) | (general_votes_norm(h, va, R, zt[i], L) ? 1u << i : 0u);
+    }
+  }
   return bits;
 }
 
@@ -121,7 +140,10 @@ IA_DEV unsigned fast_hit_rt(const HitF<T>& h, int ss, int va, const PairC<T>& p,
   const Iv<T> sAabs = ss < 0 ? ineg(h.sA[va]) : h.sA[va], sA2abs = ss < 0 ? ineg(h.sA2[va]) : h.sA2[va];
   unsigned bits = 0;
 #pragma unroll 1
-  for (int i = 0; i < nz_tile; ++i) bits |= pass_vote_qr(h, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs) << i;
+  for (int i = 0; i < nz_tile; ++i) {
+    const unsigned r = pass_vote_qr(h, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
+    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << 7)) << i : r << i;
+  }
   return bits;
 }
 
@@ -226,7 +248,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
       else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, va, pr, zt, nz_tile);
       else bits = fast_hit<0, T>(hf, va, pr, zt, nz_tile);
-      acc += spread8(bits);
+      acc += spread8(settle(bits, hf, va, R, pr.L, zt));
     } else {
       for (int i = 0; i < nz_tile; ++i)
         acc += (unsigned long long)(general_votes_norm(hf, va, R, zt[i], pr.L) ? 1u : 0u) << (8 * i);
@@ -342,8 +364,11 @@ vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const 
       const bool allP = __all_sync(0xffffffffu, kind == HIT_FAST_P || !need);
       const bool allN = __all_sync(0xffffffffu, kind == HIT_FAST_N || !need);
       // lanes that do not need the hit (forced, skipped) run along on their record and drop the result
-      const unsigned bits = fast_hit_rt<T>(hf, allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
-      if (need) { v0 += bits & 1u; v1 += (bits >> 1) & 1u; }
+      unsigned bits = fast_hit_rt<T>(hf, allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
+      if (need) {
+        bits = settle(bits, hf, va, R, pr.L, zt);
+        v0 += bits & 1u; v1 += (bits >> 1) & 1u;
+      }
     }
   }
   if (live) {
@@ -353,7 +378,69 @@ vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const 
   }
 }
 
+// ---- diagnostics: the f enclosures of the sign-specialised form, per (box, hit, drift sign) -------------------
+// What the dense fast kernel computes for the cell [lo, hi] (one-body variant: same arithmetic as the three-body one),
+// next to residual_kernel's general form: out[(box*n_hits + hit)*2 + sign][4] = f.lo, f.hi, scale (R_Ax^2.hi), form
+// (0: fast form; 1: forced vote, G15; 2: this (box, hit) takes the general form - guards, lambda straddling 0 - whose
+// enclosure is written instead; 3: invalid hit).
+template <class T>
+__global__ void residual_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const double* __restrict__ lo,
+                                     const double* __restrict__ hi, int64_t n_boxes, double* __restrict__ out) {
+  const int n_hits = sp.n_hits_single;
+  const int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (t >= n_boxes * n_hits) return;
+  const int64_t b = t / n_hits;
+  const HitC<T> c = staged[int(t - b * n_hits)];
+  const Iv<T> X = box_iv<T>(lo[5 * b + 0], hi[5 * b + 0]), Y = box_iv<T>(lo[5 * b + 1], hi[5 * b + 1]);
+  const Iv<T> R = box_iv<T>(lo[5 * b + 2], hi[5 * b + 2]), Z = box_iv<T>(lo[5 * b + 3], hi[5 * b + 3]);
+  const Iv<T> Lraw = box_iv<T>(lo[5 * b + 4], hi[5 * b + 4]);
+  const XYInv<T> inv = xy_invariants(X, Y, c);
+  HitF<T> hf;
+  make_hitf(inv, hit_small(c), R.lo, mx(fabs(Lraw.lo), fabs(Lraw.hi)), hf);
+  const int lcls = cls_of(Lraw);
+  const int va = lcls == CLS_N ? 1 : 0;
+  const int kind = hf.kind[va];
+  double* o = out + t * 8;
+  if (kind == HIT_SKIP || kind == HIT_FORCED || kind == HIT_GENERAL || lcls == CLS_M) {
+    const Box3<T> bx = {R, Z, Lraw};
+    for (int s = 0; s < 2; ++s) {
+      const Resid r = residual_general(bx, inv, hit_small(c), c.zref, s == 0 ? +1 : -1);
+      o[4 * s] = r.flo; o[4 * s + 1] = r.fhi; o[4 * s + 2] = r.scale;
+      o[4 * s + 3] = kind == HIT_SKIP ? 3.0 : (r.forced ? 1.0 : 2.0);
+    }
+    return;
+  }
+  PairC<T> pr;
+  pr.L = va ? ineg(Lraw) : Lraw;
+  pr.R = R;
+  pr.Lm = to_mr(pr.L);
+  pr.LRm = to_mr(mul_pp(pr.L, R));
+  pr.L2 = mul_pp(pr.L, pr.L);
+  const HitP<T> hp = hit_prepare(hf, va, pr);
+  const Pass2<T> pc2 = pass_prepare2(hf, pr, hp);
+  const int ss = kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0);
+  const MR<T> sAm = ss < 0 ? mr_neg(hf.sAm[va]) : hf.sAm[va], s2m = ss < 0 ? mr_neg(hf.s2m[va]) : hf.s2m[va];
+  const Iv<T> sAabs = ss < 0 ? ineg(hf.sA[va]) : hf.sA[va], sA2abs = ss < 0 ? ineg(hf.sA2[va]) : hf.sA2[va];
+  const Iv<T> Zr = isub(Z, thin(c.zref));
+  Iv<T> f[2];
+  pass_vote_qr(hf, ss, va, pc2, pr, hp, hf.zflip ? ineg(Zr) : Zr, sAm, s2m, sAabs, sA2abs, f);
+  for (int s = 0; s < 2; ++s) { o[4 * s] = f[s].lo; o[4 * s + 1] = f[s].hi; o[4 * s + 2] = hf.Q.hi; o[4 * s + 3] = 0.0; }
+}
+
 }  // namespace
+
+cudaError_t launch_residual_fast(ia_ctx* ctx, const HitSpan& sp, const double* lo, const double* hi, int64_t n_boxes,
+                                 double* out) {
+  const int64_t n = n_boxes * sp.n_hits_single;
+  if (n <= 0) return cudaSuccess;
+  const unsigned blocks = unsigned((n + 63) / 64);
+  if (ctx->params.precision == 32)
+    residual_fast_kernel<float><<<blocks, 64, 0, ctx->stream>>>(sp, static_cast<const HitC<float>*>(ctx->staged.p), lo, hi, n_boxes, out);
+  else
+    residual_fast_kernel<double><<<blocks, 64, 0, ctx->stream>>>(sp, static_cast<const HitC<double>*>(ctx->staged.p), lo, hi, n_boxes, out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
 
 template <class T>
 static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
@@ -451,7 +538,8 @@ static cudaError_t launch_children_fast_t(ia_ctx* ctx, const HitSpan& sp, int le
     if (ps < per_split) per_split = ps < 1 ? 1 : ps;
   }
   if (per_split > sp.max_hits) per_split = sp.max_hits;
-  const int n_splits = (sp.max_hits + per_split - 1) / per_split;
+  if (per_split < 1) per_split = 1;                     // no hits at all: one split that votes nothing
+  const int n_splits = sp.max_hits > 0 ? (sp.max_hits + per_split - 1) / per_split : 1;
   cudaError_t err = scratch_reserve(ctx->partial, size_t(sp.n_events) * n_splits * k * 32 * sizeof(uint16_t));
   if (err != cudaSuccess) return err;
   uint16_t* partial = static_cast<uint16_t*>(ctx->partial.p);

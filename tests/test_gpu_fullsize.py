@@ -1,0 +1,94 @@
+"""-m gpu: parity at BASELINE.json's full sizes, in the launch configuration bench.py times (SURVEY 8(d) "Parity protocol").
+
+  C1  every one of the 32^5 cells x 40 hits against the oracle, top-10 identical
+  C3  all 1,024 events, FP64 and FP32 intervals: the kept boxes of all 8 passes, their votes and the parameters
+      bit-identical to orc_refine_batch (north_star clause 1)
+  C4  a stratified sample of the 64^5 grid: 2^22 uniformly drawn cells, the GPU's top-10 cells, the truth cell and two
+      complete (R, z0, lambda) columns (the truth's and a random one)
+
+The oracle runs on the host cores (about a minute each on 16 cores), so these are the slow tests of the suite; every
+vote mismatch is traced per hit (G25, gpu_common.trace_mismatches).
+"""
+import numpy as np
+import pytest
+
+from paper_2401_04576_b200 import binding as b
+from paper_2401_04576_b200 import eventgen as g
+from oracle import oracle as o
+
+from gpu_common import HI, LO, Rig, compare_votes
+
+pytestmark = pytest.mark.gpu
+
+
+def _dense(cfg_idx, sample):
+    cfg = g.config(cfg_idx)
+    ev = cfg.events[0]
+    rig = Rig(cfg.chamber)
+    try:
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        votes = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
+        idx, vv = rig.ctx.ia_topk(votes, 10)
+        rig.ctx.synchronize()
+        vg = votes.cpu().numpy()
+        idx, vv = idx.cpu().numpy(), vv.cpu().numpy()
+        n = vg.size
+        truth = g.truth_cell(ev.track.params, LO, HI, cfg.grid)
+        if sample is None:
+            cells = None
+            vo = o.vote(rig.owires, oh, rig.oparams, LO, HI, cfg.grid)
+            vgs = vg
+            oi, ov = o.topk(vo, 10)
+            assert (oi == idx).all() and (ov == vv).all(), "top-10 of the oracle's accumulator differs from the GPU's"
+        else:
+            rng = np.random.default_rng(2024)
+            col = int(np.prod(cfg.grid[2:]))
+            cols = [truth // col, int(rng.integers(n // col))]
+            extra = np.concatenate([idx, [truth]] + [np.arange(c * col, (c + 1) * col) for c in cols])
+            cells = np.unique(np.concatenate([rng.integers(0, n, size=sample), extra])).astype(np.int64)
+            vo = o.vote(rig.owires, oh, rig.oparams, LO, HI, cfg.grid, cell_idx=cells)
+            vgs = vg[cells]
+            # the GPU's top-10 is the exact top-10 of its own accumulator, and the oracle agrees on those cells' counts
+            ei, evv = o.topk(vg, 10)
+            assert (ei == idx).all() and (evv == vv).all()
+            assert (vo[np.searchsorted(cells, idx)] == vv).all()
+        where = (lambda i: o.cell_boxes(LO, HI, cfg.grid, i)) if cells is None else (lambda i: o.cell_boxes(LO, HI, cfg.grid, cells[i]))
+        n_bad = compare_votes(rig, hd, oh, vgs, vo, where)
+        assert vg.max() <= ev.n_hits
+        return n_bad, vo.size, int(vg[truth])
+    finally:
+        rig.close()
+
+
+def test_c1_every_cell():
+    n_bad, n, _ = _dense(1, None)
+    assert n == 32 ** 5 and n_bad <= n // 10000
+
+
+def test_c4_stratified_sample():
+    n_bad, n, v_truth = _dense(4, 1 << 22)
+    assert n >= (1 << 22) and n_bad <= n // 10000
+    assert v_truth >= 38            # 40 genuine hits, 3-sigma tolerance on smeared drifts
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_c3_all_1024_events_identical(precision):
+    n_events = 1024
+    cfg = g.config(3, n_events=n_events)
+    rig = Rig(cfg.chamber, precision=precision)
+    try:
+        wire = np.concatenate([e.wire for e in cfg.events])
+        drift = np.concatenate([e.drift for e in cfg.events])
+        off = np.cumsum([0] + [e.n_hits for e in cfg.events]).astype(np.int32)
+        hd, oh = rig.hits(wire, drift)
+        boxes, par = rig.ctx.ia_refine_batch(hd, rig.dev(off), n_events, 30, LO, HI, cfg.grid, cfg.levels, cfg.k)
+        rig.ctx.synchronize()
+        gb = b.boxes_to_numpy(boxes, (n_events, cfg.levels, cfg.k))
+        ob, opar = o.refine_batch(rig.owires, oh, off, rig.oparams, LO, HI, cfg.grid, cfg.levels, cfg.k)
+        same = [(gb["lo"][e] == ob["lo"][e]).all() and (gb["hi"][e] == ob["hi"][e]).all() and (gb["votes"][e] == ob["votes"][e]).all()
+                for e in range(n_events)]
+        bad = [e for e in range(n_events) if not same[e]]
+        assert not bad, f"events whose kept boxes differ from the oracle's: {bad[:20]}"
+        assert (par.cpu().numpy().reshape(-1, 10) == opar).all()
+    finally:
+        rig.close()
