@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - headline measurement: cell-hit interval evaluations/s of the dense vote.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4|C1|C0]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4|C1|C0|C2|C3|F1|F2|PROBE]
 
 One "step" = one pass of the dense hot path over one synthetic event of BASELINE.json configs[4]
 (40-layer chamber, 60 hits, 64^5 = 1.07e9 boxes): hit staging (a2), the vote kernel (a3-a6) and the
@@ -43,6 +43,32 @@ ALG_FP64_FLOPS_PER_EVAL = 2 * 175.0 + 83.0
 DAG_UNFUSED_OPS_PER_EVAL = 366.0
 # non-tensor FP64 issue peak = SMs x 64 lanes x f_max
 FP64_LANES_PER_SM = 64
+
+
+# Values that only a profiler can give (ncu counters of the vote kernel) are NOT measured by a bench run; they are read
+# from this committed file, which names the capture each row comes from, and reported under roofline.profile_refs.
+PROFILE_REFS = os.path.join("profiles", "vote_dense_refs.csv")
+
+
+def profile_refs(workload_name: str):
+    """rows `workload,metric,value,source` of profiles/vote_dense_refs.csv -> {metric: value} for this workload"""
+    out, src = {}, set()
+    try:
+        with open(os.path.join(ROOT, PROFILE_REFS)) as f:
+            for line in f:
+                if line.startswith("#") or not line.strip() or line.startswith("workload,"):
+                    continue
+                w, metric, value, source = [x.strip() for x in line.split(",", 3)]
+                if w == workload_name:
+                    out[metric] = float(value)
+                    src.add(source)
+    except OSError:
+        return None
+    if not out:
+        return None
+    out["file"] = PROFILE_REFS
+    out["captures"] = sorted(src)
+    return out
 
 
 def workload(name: str, seed_shift: int = 0):
@@ -236,6 +262,98 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0, 
             "context": "paper: about 1.2 s per track on 4 x K80, about 0.2 s on V100 (L117)"}
 
 
+def truth_boxes(params, lo, hi, grid0, levels):
+    """The cell of the start grid that contains the generated parameters and its descendant at every deeper level (S9: a
+    box is cut at its per-axis midpoints 0.5*(lo+hi)): lo[levels][5], hi[levels][5].  Host bookkeeping for the statistics
+    below; no residual arithmetic."""
+    blo, bhi = np.zeros((levels, 5)), np.zeros((levels, 5))
+    for d in range(5):
+        e = g.cell_edges(lo[d], hi[d], grid0[d])
+        kk = min(max(int(np.searchsorted(e, params[d], side="right") - 1), 0), grid0[d] - 1)
+        a, c = e[kk], e[kk + 1]
+        for lev in range(levels):
+            blo[lev, d], bhi[lev, d] = a, c
+            mid = 0.5 * (a + c)
+            if params[d] >= mid:
+                a = mid
+            else:
+                c = mid
+    return blo, bhi
+
+
+def refine_truth_stats(ctx, hd, off, evs, boxes, par, grid0, levels):
+    """SURVEY 8(c) H1 (ii) / north_star clause 3: what the literal top-K policy achieves against the GENERATED helix, level
+    by level - measured, not assumed.  boxes: structured array [n_events][levels][k] (the call's boxes_out), par
+    [n_events][IA_N_PARAMS].  Per level: the fraction of events whose kept boxes still include the truth's box, the votes
+    of rank 0, the votes of the truth's box (one ia_vote_boxes call per event on the truth's boxes of all levels), the
+    distance rank-0 centre -> truth in cell widths of that level (largest of the five axes).  Final: |centre - truth| in
+    finest-cell widths per axis, whether the truth lies inside the G19 hull of the maximum-vote kept boxes."""
+    n_ev = len(evs)
+    lo, hi = np.array(g.BOX_LO), np.array(g.BOX_HI)
+    kept = np.zeros((n_ev, levels), bool)
+    v_truth = np.zeros((n_ev, levels), np.int64)
+    v_rank0 = boxes["votes"][:, :, 0].astype(np.int64)
+    dist = np.zeros((n_ev, levels))
+    fin = np.zeros((n_ev, 5))
+    in_hull = np.zeros(n_ev, bool)
+    n_genuine = np.zeros(n_ev, np.int64)
+    for e, ev in enumerate(evs):
+        t = np.array(ev.track.params)
+        blo, bhi = truth_boxes(t, lo, hi, grid0, levels)
+        vb = ctx.ia_vote_boxes(hd[16 * int(off[e]):16 * int(off[e + 1])], ev.n_hits, ctx.to_device(blo), ctx.to_device(bhi))
+        v_truth[e] = vb.cpu().numpy()
+        n_genuine[e] = int((~ev.is_noise).sum()) if hasattr(ev, "is_noise") else ev.n_hits
+        for lev in range(levels):
+            kept[e, lev] = bool(((boxes["lo"][e, lev] == blo[lev]).all(axis=1) & (boxes["hi"][e, lev] == bhi[lev]).all(axis=1)).any())
+            c0 = 0.5 * (boxes["lo"][e, lev, 0] + boxes["hi"][e, lev, 0])
+            dist[e, lev] = float(np.max(np.abs(c0 - t) / (bhi[lev] - blo[lev])))
+        fin[e] = np.abs(par[e, :5] - t) / (2.0 * par[e, 5:10])
+        in_hull[e] = bool(((par[e, 10:15] <= t) & (t <= par[e, 15:20])).all())
+    return {
+        "what": "generated helix vs the kept boxes, per level (level 0 = start grid); SURVEY 8(c) H1: recovery is not expected "
+                "under the literal top-K policy",
+        "frac_events_truth_box_kept": [float(x) for x in kept.mean(axis=0)],
+        "mean_votes_rank0": [float(x) for x in v_rank0.mean(axis=0)],
+        "mean_votes_truth_box": [float(x) for x in v_truth.mean(axis=0)],
+        "mean_genuine_hits": float(n_genuine.mean()),
+        "median_dist_rank0_centre_to_truth_in_cell_widths": [float(x) for x in np.median(dist, axis=0)],
+        "final_abs_dev_in_finest_cell_widths_median": dict(zip(("xc", "yc", "R", "z0", "lambda"), (float(x) for x in np.median(fin, axis=0)))),
+        "frac_events_within_one_finest_cell": float((fin <= 1.0).all(axis=1).mean()),
+        "frac_events_truth_in_hull_of_max_vote_boxes": float(in_hull.mean()),
+        "n_events": n_ev,
+    }
+
+
+PROBE_MODES = {0: "DFMA rn, 8 chains", 1: "DADD.RM/DMUL.RP, 8 chains", 2: "DFMA.RM/RP, 8 chains",
+               3: "DFMA.RM/RP, 1 chain", 4: "DFMA.RM/RP, 2 chains", 5: "DFMA.RM/RP, 4 chains",
+               6: "DFMA.RM/RP + 1 LOP3 each", 7: "DFMA.RM/RP + 1 FFMA each",
+               8: "DFMA.RM/RP, 3 register operands", 9: "DMUL.RM/DADD.RP, 2 register operands",
+               10: "DFMA 3 reg, multiplier shared by 4", 11: "DFMA 3 reg, multiplier shared by 2"}
+
+
+def probe_leg(local_rank: int):
+    """--workload PROBE: what independent FP64 chains sustain on this device (ia_probe_fp64), per instruction mix and per
+    number of resident warps per SM sub-partition: the measured check of the derived roofline peak."""
+    import torch
+    from paper_2401_04576_b200 import binding as b
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    mhz = 1965.0
+    try:
+        mhz = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("sm_max_mhz", mhz))
+    except Exception:
+        pass
+    peak = n_sm * FP64_LANES_PER_SM * mhz * 1e6
+    ctx = b.Context(local_rank)
+    rows = []
+    for mode, name in PROBE_MODES.items():
+        for per_sm in (1, 2, 4, 8):               # blocks of 256 threads = 2 warps per sub-partition each
+            rate = max(ctx.ia_probe_fp64(mode, 8192, n_sm * per_sm) for _ in range(3))
+            rows.append({"mode": mode, "mix": name, "warps_per_subpartition": 2 * per_sm, "T_inst_per_s": rate / 1e12,
+                         "frac_of_peak": rate / peak})
+    ctx.close()
+    return {"n_sm": n_sm, "sm_max_mhz": mhz, "peak_T_inst_per_s": peak / 1e12, "rows": rows}
+
+
 def run_c3(args, rank, world, local_rank, barrier):
     """--workload C3: one step = ia_refine_batch over 1024 events (BASELINE.json configs[3]); for profiling the
     batch path on its own.  Same JSON shape; value = cell-hit evaluations/s, events/s beside it."""
@@ -285,8 +403,10 @@ def run_c3(args, rank, world, local_rank, barrier):
     ob, opar = o.refine_batch(o.wires_of(ch), oh, off_s, o.make_params(g.TOL, precision=args.precision), g.BOX_LO, g.BOX_HI,
                               (8,) * 5, levels, k)
     dt_o = time.perf_counter() - t0
-    gb = b.boxes_to_numpy(boxes, (n_ev, levels, k))[:n_s]
+    gb_all = b.boxes_to_numpy(boxes, (n_ev, levels, k))
+    gb = gb_all[:n_s]
     same = bool((gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all())
+    truth = refine_truth_stats(ctx, hd, off, evs, gb_all, par.cpu().numpy().reshape(n_ev, -1), (8,) * 5, levels)
     line = {"metric": METRIC, "value": evals * world / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": f"f{args.precision}", "data": "synthetic",
@@ -296,7 +416,8 @@ def run_c3(args, rank, world, local_rank, barrier):
             "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks,
             "cpu_baseline": {"value": n_s * evals / n_ev / dt_o, "unit": UNIT, "cores": o.max_threads(), "kind": "oracle",
                              "sample": f"orc_refine_batch on the first {n_s} event(s) ({dt_o:.2f} s)",
-                             "events_per_s": n_s / dt_o, "boxes_identical": same}}
+                             "events_per_s": n_s / dt_o, "boxes_identical": same},
+            "truth": truth}
     print(json.dumps(line))
     ctx.close()
 
@@ -307,7 +428,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1", "F2"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1", "C0", "C2", "C3", "F1", "F2", "PROBE"])
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="interval endpoint type (C3 only)")
     ap.add_argument("--ref-cells", type=int, default=1 << 22, help="cells per oracle sample")
     ap.add_argument("--f2-extra-passes", type=int, default=0, choices=[0, 1, 2],
@@ -351,6 +472,17 @@ def main():
                               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                               "data": "synthetic", "config": {"workload": r["workload"]},
                               "gpu_launches": r["launches_per_track"] * r["n_tracks"], "paper_track": r}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    if args.workload == "PROBE":
+        r = probe_leg(local_rank) if rank == 0 else None
+        if rank == 0:
+            best = max(x["T_inst_per_s"] for x in r["rows"])
+            print(json.dumps({"metric": "FP64 thread-instructions/s (probe)", "value": best * 1e12, "unit": "inst/s", "n_gpus": 1,
+                              "steps": 3, "warmup": 1, "ms_per_step": None, "higher_is_better": True, "scaling": "weak",
+                              "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                              "config": {"workload": "PROBE: ia_probe_fp64 sweep"}, "gpu_launches": 2 * 3 * len(r["rows"]), "probe": r}))
         if world > 1:
             dist.destroy_process_group()
         return
@@ -436,22 +568,24 @@ def main():
         pass
     f_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_inst = n_sm * FP64_LANES_PER_SM * f_max_mhz * 1e6                         # FP64 thread-instructions / s
+    refs = profile_refs(args.workload)
     achieved_inst = ALG_FP64_INST_PER_EVAL * evals_per_step / (vote_ms * 1e-3)
     roofline = {
         "bound": "alu", "kernel": "vote_dense", "achieved": achieved_inst / 1e12, "peak": peak_inst / 1e12,
         "unit": "T FP64 inst/s", "frac": achieved_inst / peak_inst,
-        # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from profiles/r01_traffic_c4.md (C4 only)
-        "traffic": 2361204736 if args.workload == "C4" else None,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch of this workload: an ncu counter, read from the
+        # committed capture that profile_refs names (null when there is none for this workload)
+        "traffic": (refs or {}).get("dram_bytes_per_launch"),
         "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} FP64 lanes x {f_max_mhz:.0f} MHz (DESIGN.md 6); "
                        "MEASURED_PEAKS.json has no FP64 entry",
         "alg_fp64_inst_per_eval": ALG_FP64_INST_PER_EVAL, "kernel_ms": vote_ms,
         "flop_frac": ALG_FP64_FLOPS_PER_EVAL * evals_per_step / (vote_ms * 1e-3) / (2 * peak_inst),
         "flop_peak_T": 2 * peak_inst / 1e12, "alg_fp64_flops_per_eval": ALG_FP64_FLOPS_PER_EVAL,
         "unfused_dag_ops_per_eval": DAG_UNFUSED_OPS_PER_EVAL,
-        "operand_note": "a DFMA with 3 distinct vector-register operands issues every 3 cycles (2.25 with operand reuse): 107 of "
-                        "the kernel's 284 FP64-pipe instructions per evaluation; the pipe demand is 611-675 cycles per "
-                        "warp-evaluation against 896 measured (profiles/r01_pipe_probe.md)",
-        "ncu_pipe_fp64_active_pct": 63.9, "ncu_source": "profiles/r01_vote_dense_fast_c1_ncu.md (C1, same kernel)",
+        "executed_fp64_inst_per_eval": (refs or {}).get("executed_fp64_inst_per_eval"),
+        "profile_refs": refs,
+        "target_reading": "north_star's '>= 50 % of FP64 non-tensor peak' is claimed on frac (algorithmic FP64 instructions / "
+                          "instruction peak); flop_frac (FMA = 2 flops against 2 x the instruction peak) is the stricter reading",
         "alg_bytes_per_launch": 2 * n_cells, "hbm_frac": (2 * n_cells / (vote_ms * 1e-3)) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
     }
     if clocks and clocks.get("sm_mhz"):
@@ -527,7 +661,9 @@ def main():
             ctx3.ia_refine_batch_host(h3, off, g.BOX_LO, g.BOX_HI, (8,) * 5, 8, 8)
             dt_h = time.perf_counter() - t0
             eps[f"fp{prec}"] = {"events_per_s": n_ev / (ms * 1e-3), "ms": ms, "e2e_events_per_s": n_ev / dt_h,
-                                "evals_per_s": n_ev * (8 ** 5 + 7 * 8 * 32) * 30 / (ms * 1e-3)}
+                                "evals_per_s": n_ev * (8 ** 5 + 7 * 8 * 32) * 30 / (ms * 1e-3),
+                                "truth": refine_truth_stats(ctx3, hd3, off, evs, b.boxes_to_numpy(boxes, (n_ev, 8, 8)),
+                                                            par.cpu().numpy().reshape(n_ev, -1), (8,) * 5, 8)}
         line["events_per_s"] = {"workload": "C3: BASELINE.json configs[3], 1024 events x 30 hits, 8^5 start, K=8, 8 passes",
                                 **eps}
         ctx3.close()

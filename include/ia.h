@@ -52,6 +52,7 @@ enum {
  * 227 KB a CTA can have), and the paper's events hold 25-62 hits (L88).  More hits return IA_ERR_CAPACITY. */
 #define IA_MAX_HITS 1024
 #define IA_MAX_K 32      /* top-K list = one key per lane of a warp                                */
+#define IA_N_PARAMS 20   /* doubles per event in params_out: centre[5], half-width[5], hull lo[5], hull hi[5]       */
 
 typedef struct ia_ctx ia_ctx; /* opaque: device geometry, parameters, stream, scratch */
 
@@ -203,15 +204,17 @@ int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int6
 /* a8-a9 - adaptive refinement of one event, entirely on the device: vote the dense grid0, keep the
  * top k, then (levels-1) times: cut every kept box at its per-axis midpoints into 2^5 children
  * (child c of rank r at list index r*32+c, bit (4-dim) of c set = upper half), vote the 32k
- * children, keep the top k.  boxes_out_dev[level][rank] (levels*k ia_box); params_out_dev[10] =
- * centre (5) and half-width (5) of the rank-0 box of the last pass (L94, G19). */
+ * children, keep the top k.  boxes_out_dev[level][rank] (levels*k ia_box); params_out_dev[IA_N_PARAMS] =
+ * centre (5) and half-width (5) of the rank-0 box of the last pass (L94, G19), then lower (5) and upper (5)
+ * corner of the hull of the last pass's kept boxes whose votes equal rank 0's ("the cells where the maximum of
+ * votes ... are found", L94). */
 int ia_refine(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
               const int32_t grid0[5], int levels, int k, ia_box* boxes_out_dev, double* params_out_dev);
 
 /* a10 - the same for n_events independent events in one launch sequence.  Hits in CSR form:
  * event e owns hits_dev[hit_offsets_dev[e] .. hit_offsets_dev[e+1]); max_hits_per_event bounds
  * every event's count (<= IA_MAX_HITS).  boxes_out_dev[n_events][levels][k], params_out_dev
- * [n_events][10]. */
+ * [n_events][IA_N_PARAMS]. */
 int ia_refine_batch(ia_ctx* ctx, const ia_hit* hits_dev, const int32_t* hit_offsets_dev, int n_events,
                     int max_hits_per_event, const double box_lo[5], const double box_hi[5], const int32_t grid0[5],
                     int levels, int k, ia_box* boxes_out_dev, double* params_out_dev);

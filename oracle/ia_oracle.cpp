@@ -466,6 +466,16 @@ int refine_T(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, 
     params_out[d] = opaque(0.5 * opaque(cur[0].lo[d] + cur[0].hi[d]));
     params_out[5 + d] = opaque(0.5 * opaque(cur[0].hi[d] - cur[0].lo[d]));
   }
+  // G19: "additionally report hull of last-pass boxes with votes == max" - the paper keeps ALL the cells
+  // at the maximum and takes value and error from their centres and sizes (L94); of the K kept boxes those at the
+  // maximum are the ones with the votes of rank 0
+  for (int d = 0; d < 5; ++d) {
+    double hl = cur[0].lo[d], hh = cur[0].hi[d];
+    for (int r = 1; r < k; ++r)
+      if (cur[r].votes == cur[0].votes) { hl = std::min(hl, cur[r].lo[d]); hh = std::max(hh, cur[r].hi[d]); }
+    params_out[10 + d] = hl;
+    params_out[15 + d] = hh;
+  }
   return ORC_OK;
 }
 
@@ -759,7 +769,7 @@ int orc_refine_batch(const OrcWire* wires, int n_wires, const OrcHit* hits, cons
   if (!hit_offsets || n_events < 0) return ORC_ERR_ARG;
   for (int e = 0; e < n_events; ++e) {
     int rc = orc_refine(wires, n_wires, hits + hit_offsets[e], hit_offsets[e + 1] - hit_offsets[e], p, lo, hi, grid0,
-                        levels, k, boxes_out + int64_t(e) * levels * k, params_out + int64_t(e) * 10);
+                        levels, k, boxes_out + int64_t(e) * levels * k, params_out + int64_t(e) * 20);
     if (rc) return rc;
   }
   return ORC_OK;

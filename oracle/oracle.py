@@ -142,7 +142,7 @@ def refine(wires, hits, params: Params, lo, hi, grid0, levels: int, k: int):
     hi = np.ascontiguousarray(hi, np.float64)
     grid0 = np.ascontiguousarray(grid0, np.int32)
     boxes = np.zeros((levels, k), BOX_DT)
-    par = np.zeros(10)
+    par = np.zeros(20)          # centre[5], half-width[5] of the rank-0 box; hull lo[5], hi[5] of the kept boxes at the maximum (G19)
     _chk(lib().orc_refine(_p(wires), len(wires), _p(hits), len(hits), C.byref(params), _p(lo), _p(hi), _p(grid0),
                           levels, k, _p(boxes), _p(par)), "refine")
     return boxes, par
@@ -155,7 +155,7 @@ def refine_batch(wires, hits, hit_offsets, params: Params, lo, hi, grid0, levels
     hit_offsets = np.ascontiguousarray(hit_offsets, np.int32)
     n_ev = len(hit_offsets) - 1
     boxes = np.zeros((n_ev, levels, k), BOX_DT)
-    par = np.zeros((n_ev, 10))
+    par = np.zeros((n_ev, 20))
     _chk(lib().orc_refine_batch(_p(wires), len(wires), _p(hits), _p(hit_offsets), n_ev, C.byref(params), _p(lo),
                                 _p(hi), _p(grid0), levels, k, _p(boxes), _p(par)), "refine_batch")
     return boxes, par

@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "libia_b200.so")
 
 IA_MAX_HITS = 1024
 IA_MAX_K = 32
+IA_N_PARAMS = 20
 
 WIRE_DT = np.dtype([("x0", "f8"), ("y0", "f8"), ("sin_phi_s", "f8"), ("cos_phi_s", "f8"), ("tan_tau", "f8"),
                     ("half_len", "f8"), ("layer", "i4"), ("_pad", "i4")])
@@ -271,7 +272,7 @@ class Context:
         if boxes is None:
             boxes = self._empty(max(levels * k, 1) * BOX_DT.itemsize, torch.uint8)
         if params is None:
-            params = self._empty(10, torch.float64)
+            params = self._empty(IA_N_PARAMS, torch.float64)
         self._chk(self.lib.ia_refine(self.h, _dp(hits_dev), n_hits, _hp(lo), _hp(hi), _hp(dims), levels, k, _dp(boxes),
                                      _dp(params)), "ia_refine")
         return boxes, params
@@ -283,7 +284,7 @@ class Context:
         if boxes is None:
             boxes = self._empty(max(n_events * levels * k, 1) * BOX_DT.itemsize, torch.uint8)
         if params is None:
-            params = self._empty(max(n_events, 1) * 10, torch.float64)
+            params = self._empty(max(n_events, 1) * IA_N_PARAMS, torch.float64)
         self._chk(self.lib.ia_refine_batch(self.h, _dp(hits_dev), _dp(hit_offsets_dev), n_events, max_hits, _hp(lo),
                                            _hp(hi), _hp(dims), levels, k, _dp(boxes), _dp(params)), "ia_refine_batch")
         return boxes, params
@@ -308,7 +309,7 @@ class Context:
         if boxes is None:
             boxes = np.zeros((n_events, levels, k), BOX_DT)
         if params is None:
-            params = np.zeros((n_events, 10))
+            params = np.zeros((n_events, IA_N_PARAMS))
         self._chk(self.lib.ia_refine_batch_host(self.h, _hp(hits), _hp(off), n_events, _hp(lo), _hp(hi), _hp(dims), levels,
                                                 k, _hp(boxes), _hp(params)), "ia_refine_batch_host")
         return boxes, params

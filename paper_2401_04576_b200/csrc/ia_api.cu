@@ -483,7 +483,7 @@ int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hi
   IA_CUDA(ctx, scratch_reserve(ctx->io_a, size_t(total) * sizeof(ia_hit) + 16));
   IA_CUDA(ctx, scratch_reserve(ctx->io_b, size_t(n_events + 1) * sizeof(int32_t)));
   IA_CUDA(ctx, scratch_reserve(ctx->io_c, nb * sizeof(ia_box)));
-  IA_CUDA(ctx, scratch_reserve(ctx->io_d, size_t(n_events) * 10 * sizeof(double)));
+  IA_CUDA(ctx, scratch_reserve(ctx->io_d, size_t(n_events) * IA_N_PARAMS * sizeof(double)));
   if (total > 0)
     IA_CUDA(ctx, cudaMemcpyAsync(ctx->io_a.p, hits_host, size_t(total) * sizeof(ia_hit), cudaMemcpyHostToDevice, ctx->stream));
   IA_CUDA(ctx, cudaMemcpyAsync(ctx->io_b.p, hit_offsets_host, size_t(n_events + 1) * sizeof(int32_t), cudaMemcpyHostToDevice,
@@ -493,7 +493,7 @@ int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hi
                        static_cast<double*>(ctx->io_d.p));
   if (rc) return rc;
   IA_CUDA(ctx, cudaMemcpyAsync(boxes_out_host, ctx->io_c.p, nb * sizeof(ia_box), cudaMemcpyDeviceToHost, ctx->stream));
-  IA_CUDA(ctx, cudaMemcpyAsync(params_out_host, ctx->io_d.p, size_t(n_events) * 10 * sizeof(double), cudaMemcpyDeviceToHost,
+  IA_CUDA(ctx, cudaMemcpyAsync(params_out_host, ctx->io_d.p, size_t(n_events) * IA_N_PARAMS * sizeof(double), cudaMemcpyDeviceToHost,
                                ctx->stream));
   IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
   return IA_OK;

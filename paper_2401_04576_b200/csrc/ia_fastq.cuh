@@ -105,19 +105,17 @@ template <class T> IA_DEV void q_add(Iv<T> a0, Iv<T> a1, Iv<T> b0, Iv<T> b1, Iv<
 }
 
 // sin and cos over e0, e1 inside [-1/4, 1/4] (trig_small of ia_fast.cuh, eight Horner chains abreast)
+// The coefficients sit in constant memory: a DFMA takes c[bank][offset] as an operand directly, whereas literals are
+// rebuilt in uniform registers (two UMOV each) on every evaluation - there are not enough of them to keep 11 doubles.
+static __constant__ double IA_SIN_C[5] = {-2.5052108385441720e-08, 2.7557319223985893e-06, -1.9841269841269841e-04,
+                                          8.3333333333333332e-03, -1.6666666666666666e-01};
+static __constant__ double IA_COS_C[6] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05,
+                                          -1.3888888888888889e-03, 4.1666666666666664e-02, -0.5};
 template <class T> struct TrigC;
 template <> struct TrigC<double> {
   static constexpr int NS = 5, NC = 6;
-  static IA_DEV double s(int k) {
-    const double c[NS] = {-2.5052108385441720e-08, 2.7557319223985893e-06, -1.9841269841269841e-04, 8.3333333333333332e-03,
-                          -1.6666666666666666e-01};
-    return c[k];
-  }
-  static IA_DEV double c(int k) {
-    const double d[NC] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05, -1.3888888888888889e-03,
-                          4.1666666666666664e-02, -0.5};
-    return d[k];
-  }
+  static IA_DEV double s(int k) { return IA_SIN_C[k]; }
+  static IA_DEV double c(int k) { return IA_COS_C[k]; }
 };
 template <> struct TrigC<float> {
   static constexpr int NS = 3, NC = 4;
@@ -249,11 +247,9 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
     q_mulpos<SS>(ce[0], ce[1], SS < 0 ? ineg(h.sA[va]) : h.sA[va], sce[0], sce[1]);
     q_mulpos<SC>(ce[0], ce[1], h.cA, cce[0], cce[1]);
   } else {
-#pragma unroll 1
-    for (int s = 0; s < 2; ++s) {
-      trig_general(e[s], h.sA[va], h.cA, se[s], sce[s], cce[s]);
-      if (SS < 0) sce[s] = ineg(sce[s]);
-    }
+    const Trig3<T> g0 = trig_general(e[0], h.sA[va], h.cA), g1 = trig_general(e[1], h.sA[va], h.cA);
+    se[0] = g0.se; cce[0] = g0.cce; sce[0] = SS < 0 ? ineg(g0.sce) : g0.sce;
+    se[1] = g1.se; cce[1] = g1.cce; sce[1] = SS < 0 ? ineg(g1.sce) : g1.sce;
   }
   Iv<T> sa[2], ca[2], sinP[2], cosP[2];
   if (SS < 0) q_fma<QKind<SC>::add>(h.cAm, h.cAm, se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
@@ -261,12 +257,20 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   q_fma<QKind<SS>::sub>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
   q_prod_p(h.iRm, sa[0], sa[1], sinP[0], sinP[1]);
   q_prod_p(h.iRm, ca[0], ca[1], cosP[0], cosP[1]);
+  // the common case cos Phi >= 0 is decided per warp (cos_nonneg in ia_fast.cuh)
+  const bool plain = __all_sync(0xffffffffu, cos_nonneg(cosP));
 #pragma unroll
-  for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_unit(cosP[s]); }
+  for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_hi(cosP[s]); }
+  if (!plain) { cosP[0] = clamp_lo(cosP[0]); cosP[1] = clamp_lo(cosP[1]); }
   // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
   Iv<T> u2[2], dq[2];
   q_fma<QK_ADD_P>(hp.TL2m, hp.TL2m, sinP[0], sinP[1], hp.T2L2, hp.T2L2, u2[0], u2[1]);
-  {
+  if (plain) {
+    const T a0 = V::mul_dn(cosP[0].lo, cosP[0].lo), b0 = V::mul_up(cosP[0].hi, cosP[0].hi);
+    const T a1 = V::mul_dn(cosP[1].lo, cosP[1].lo), b1 = V::mul_up(cosP[1].hi, cosP[1].hi);
+    u2[0].lo = V::fma_dn(h.T2.lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2.lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+  } else {
     const Mag<T> g0 = mag_of(cosP[0]), g1 = mag_of(cosP[1]);
     const T a0 = V::mul_dn(g0.mnn, g0.mnn), b0 = V::mul_up(g0.mag, g0.mag), a1 = V::mul_dn(g1.mnn, g1.mnn), b1 = V::mul_up(g1.mag, g1.mag);
     const T l0 = V::fma_dn(h.T2.lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2.lo, a1, u2[1].lo);
@@ -282,7 +286,10 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   Tdq[1].lo = V::mul_dn(Tn, dq[1].lo); Tdq[1].hi = V::mul_up(Tn, dq[1].hi);
   q_mulpos<1>(Tdq[0], Tdq[1], p.L, TLq[0], TLq[1]);                                         // |T lambda delta|
   q_mulpos<SS>(TLq[0], TLq[1], SS < 0 ? ineg(h.sA2[va]) : h.sA2[va], qs[0], qs[1]);         // sigma 2T |lambda delta| sA
-  {
+  if (plain) {                                                           // cos Phi >= 0: the partner of .lo is .lo, of .hi is .hi
+    z[0].lo = V::fma_dn(-Tdq[0].hi, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-Tdq[0].lo, cosP[0].lo, zz[0].hi);
+    z[1].lo = V::fma_dn(Tdq[1].lo, cosP[1].lo, zz[1].lo); z[1].hi = V::fma_up(Tdq[1].hi, cosP[1].hi, zz[1].hi);
+  } else {
     const T pl0 = sgn(cosP[0].lo) ? Tdq[0].hi : Tdq[0].lo, ph0 = sgn(cosP[0].hi) ? Tdq[0].lo : Tdq[0].hi;   // partners of cosP.lo / .hi
     const T pl1 = sgn(cosP[1].lo) ? Tdq[1].hi : Tdq[1].lo, ph1 = sgn(cosP[1].hi) ? Tdq[1].lo : Tdq[1].hi;
     z[0].lo = V::fma_dn(-ph0, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-pl0, cosP[0].lo, zz[0].hi);
@@ -368,11 +375,9 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
       q_mulpos<0>(ce[0], ce[1], h.cA, cce[0], cce[1]);
     }
   } else {
-#pragma unroll 1
-    for (int s = 0; s < 2; ++s) {
-      trig_general(e[s], h.sA[va], h.cA, se[s], sce[s], cce[s]);
-      if (ss < 0) sce[s] = ineg(sce[s]);
-    }
+    const Trig3<T> g0 = trig_general(e[0], h.sA[va], h.cA), g1 = trig_general(e[1], h.sA[va], h.cA);
+    se[0] = g0.se; cce[0] = g0.cce; sce[0] = ss < 0 ? ineg(g0.sce) : g0.sce;
+    se[1] = g1.se; cce[1] = g1.cce; sce[1] = ss < 0 ? ineg(g1.sce) : g1.sce;
   }
   if (ss > 0) {
     q_fma<QK_ADD_P>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
@@ -386,12 +391,20 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   }
   q_prod_p(h.iRm, sa[0], sa[1], sinP[0], sinP[1]);
   q_prod_p(h.iRm, ca[0], ca[1], cosP[0], cosP[1]);
+  // the common case cos Phi >= 0 is decided per warp (cos_nonneg in ia_fast.cuh)
+  const bool plain = __all_sync(0xffffffffu, cos_nonneg(cosP));
 #pragma unroll
-  for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_unit(cosP[s]); }
+  for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_hi(cosP[s]); }
+  if (!plain) { cosP[0] = clamp_lo(cosP[0]); cosP[1] = clamp_lo(cosP[1]); }
   // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
   Iv<T> u2[2], dq[2];
   q_fma<QK_ADD_P>(hp.TL2m, hp.TL2m, sinP[0], sinP[1], hp.T2L2, hp.T2L2, u2[0], u2[1]);
-  {
+  if (plain) {
+    const T a0 = V::mul_dn(cosP[0].lo, cosP[0].lo), b0 = V::mul_up(cosP[0].hi, cosP[0].hi);
+    const T a1 = V::mul_dn(cosP[1].lo, cosP[1].lo), b1 = V::mul_up(cosP[1].hi, cosP[1].hi);
+    u2[0].lo = V::fma_dn(h.T2.lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2.lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+  } else {
     const Mag<T> g0 = mag_of(cosP[0]), g1 = mag_of(cosP[1]);
     const T a0 = V::mul_dn(g0.mnn, g0.mnn), b0 = V::mul_up(g0.mag, g0.mag), a1 = V::mul_dn(g1.mnn, g1.mnn), b1 = V::mul_up(g1.mag, g1.mag);
     const T l0 = V::fma_dn(h.T2.lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2.lo, a1, u2[1].lo);
@@ -406,7 +419,10 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   Tdq[0].lo = V::mul_dn(Tn, dq[0].lo); Tdq[0].hi = V::mul_up(Tn, dq[0].hi);                 // |T delta|
   Tdq[1].lo = V::mul_dn(Tn, dq[1].lo); Tdq[1].hi = V::mul_up(Tn, dq[1].hi);
   q_mulpos<1>(Tdq[0], Tdq[1], p.L, TLq[0], TLq[1]);                                         // |T lambda delta|
-  {
+  if (plain) {                                                           // cos Phi >= 0: the partner of .lo is .lo, of .hi is .hi
+    z[0].lo = V::fma_dn(-Tdq[0].hi, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-Tdq[0].lo, cosP[0].lo, zz[0].hi);
+    z[1].lo = V::fma_dn(Tdq[1].lo, cosP[1].lo, zz[1].lo); z[1].hi = V::fma_up(Tdq[1].hi, cosP[1].hi, zz[1].hi);
+  } else {
     const T pl0 = sgn(cosP[0].lo) ? Tdq[0].hi : Tdq[0].lo, ph0 = sgn(cosP[0].hi) ? Tdq[0].lo : Tdq[0].hi;   // partners of cosP.lo / .hi
     const T pl1 = sgn(cosP[1].lo) ? Tdq[1].hi : Tdq[1].lo, ph1 = sgn(cosP[1].hi) ? Tdq[1].lo : Tdq[1].hi;
     z[0].lo = V::fma_dn(-ph0, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-pl0, cosP[0].lo, zz[0].hi);

@@ -248,15 +248,23 @@ select_children_kernel(const uint16_t* __restrict__ partial, int n_splits, int l
   }
 }
 
-// value = centre, error = half-width of the rank-0 box of the last pass (L94, G19)
+// value = centre, error = half-width of the rank-0 box of the last pass (L94, G19); then the hull of the kept boxes of
+// the last pass that share rank 0's vote count (G19: the paper keeps every cell at the maximum, L94)
 __global__ void params_kernel(int n_events, int levels, int k, const ia_box* __restrict__ boxes,
                               double* __restrict__ params) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n_events) return;
-  const ia_box b = boxes[(int64_t(e) * levels + (levels - 1)) * k];
+  const ia_box* last = boxes + (int64_t(e) * levels + (levels - 1)) * k;
+  const ia_box b = last[0];
+  double* out = params + int64_t(e) * IA_N_PARAMS;
   for (int d = 0; d < 5; ++d) {
-    params[int64_t(e) * 10 + d] = __dmul_rn(0.5, __dadd_rn(b.lo[d], b.hi[d]));
-    params[int64_t(e) * 10 + 5 + d] = __dmul_rn(0.5, __dadd_rn(b.hi[d], -b.lo[d]));
+    out[d] = __dmul_rn(0.5, __dadd_rn(b.lo[d], b.hi[d]));
+    out[5 + d] = __dmul_rn(0.5, __dadd_rn(b.hi[d], -b.lo[d]));
+    double hl = b.lo[d], hh = b.hi[d];
+    for (int r = 1; r < k; ++r)
+      if (last[r].votes == b.votes) { hl = fmin(hl, last[r].lo[d]); hh = fmax(hh, last[r].hi[d]); }
+    out[10 + d] = hl;
+    out[15 + d] = hh;
   }
 }
 

@@ -89,6 +89,6 @@ def test_c3_all_1024_events_identical(precision):
                 for e in range(n_events)]
         bad = [e for e in range(n_events) if not same[e]]
         assert not bad, f"events whose kept boxes differ from the oracle's: {bad[:20]}"
-        assert (par.cpu().numpy().reshape(-1, 10) == opar).all()
+        assert (par.cpu().numpy().reshape(-1, 20) == opar).all()
     finally:
         rig.close()

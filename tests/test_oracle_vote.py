@@ -215,8 +215,12 @@ def test_refine_follows_its_definition():
         assert boxes[lev]["votes"].max() <= boxes[lev - 1]["votes"].max()          # P6
         assert (np.diff(boxes[lev]["votes"].astype(int)) <= 0).all()
     last = boxes[-1][0]
-    assert (par[:5] == 0.5 * (last["lo"] + last["hi"])).all() and (par[5:] == 0.5 * (last["hi"] - last["lo"])).all()
-    assert np.allclose(par[5:], (HI - LO) / 4 / 2 ** (levels - 1) / 2)
+    assert (par[:5] == 0.5 * (last["lo"] + last["hi"])).all() and (par[5:10] == 0.5 * (last["hi"] - last["lo"])).all()
+    assert np.allclose(par[5:10], (HI - LO) / 4 / 2 ** (levels - 1) / 2)
+    # G19: hull of the kept boxes of the last pass that share the maximum vote count (written out from its definition)
+    top = boxes[-1][boxes[-1]["votes"] == boxes[-1]["votes"].max()]
+    assert (par[10:15] == top["lo"].min(axis=0)).all() and (par[15:20] == top["hi"].max(axis=0)).all()
+    assert (par[10:15] <= last["lo"]).all() and (par[15:20] >= last["hi"]).all()
 
 
 def test_refine_batch_equals_loop_and_fp32_runs():
