@@ -87,7 +87,11 @@ vote_dense_general_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDe
 #endif
 constexpr int FAST_THREADS = IA_FAST_THREADS;
 constexpr int FAST_MIN_BLOCKS = IA_FAST_MIN_BLOCKS;
-constexpr int FAST_ZT = 8;
+#ifndef IA_FAST_ZT
+#define IA_FAST_ZT 16
+#endif
+constexpr int FAST_ZT = IA_FAST_ZT;                      // 8 or 16: z0 cells per thread (vote bits + filter bits share 32 bits)
+static_assert(FAST_ZT == 8 || FAST_ZT == 16, "FAST_ZT");
 
 template <class T> struct ZTab { Iv<T> z[2][FAST_ZT]; };    // [0]: z0 - z_ref, [1]: its negation
 
@@ -102,7 +106,7 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
 }
 
 // one hit, one thread: both drift signs over the thread's z0 cells; returns the vote mask (bit i = z0 cell i)
-// (float: bit 8 + i set = cell i is too close to call in this form, see Filter in ia_fast.cuh)
+// (float: bit FAST_ZT + i set = cell i is too close to call in this form, see Filter in ia_fast.cuh)
 template <int SS, class T>
 IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
@@ -111,7 +115,7 @@ IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) {
     const unsigned r = pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]);
-    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << 7)) << i : r << i;
+    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : r << i;
   }
   return bits;
 }
@@ -120,8 +124,8 @@ IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T
 template <class T>
 IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L, const Iv<T>* zt) {
   if (Filter<T>::on) {
-    unsigned amb = bits >> 8;
-    bits &= 0xffu;
+    unsigned amb = bits >> FAST_ZT;
+    bits &= (1u << FAST_ZT) - 1u;
     while (amb) {
       const int i = __ffs(amb) - 1;
       amb &= amb - 1;
@@ -142,7 +146,7 @@ IA_DEV unsigned fast_hit_rt(const HitF<T>& h, int ss, int va, const PairC<T>& p,
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) {
     const unsigned r = pass_vote_qr(h, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
-    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << 7)) << i : r << i;
+    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : r << i;
   }
   return bits;
 }
@@ -234,13 +238,19 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   pr.Lm = to_mr(pr.L);
   pr.LRm = to_mr(warp_fast ? mul_pp(pr.L, R) : imul(pr.L, R));
   pr.L2 = warp_fast ? mul_pp(pr.L, pr.L) : isqr(pr.L);
-  unsigned long long acc = 0;
+  unsigned long long acc[FAST_ZT / 8];
+#pragma unroll
+  for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] = 0;
   const int va = a ? 1 : 0;
   for (int h = h_begin; h < h_end; ++h) {
     const HitF<T>& hf = sh[h];
     const int kind = hf.kind[va];
     if (kind == HIT_SKIP) continue;
-    if (kind == HIT_FORCED) { acc += 0x0101010101010101ull; continue; }
+    if (kind == HIT_FORCED) {
+#pragma unroll
+      for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += 0x0101010101010101ull;
+      continue;
+    }
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
       unsigned bits;
@@ -248,15 +258,21 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
       else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, va, pr, zt, nz_tile);
       else bits = fast_hit<0, T>(hf, va, pr, zt, nz_tile);
-      acc += spread8(settle(bits, hf, va, R, pr.L, zt));
+      bits = settle(bits, hf, va, R, pr.L, zt);
+#pragma unroll
+      for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += spread8((bits >> (8 * j)) & 0xffu);
     } else {
-      for (int i = 0; i < nz_tile; ++i)
-        acc += (unsigned long long)(general_votes_norm(hf, va, R, zt[i], pr.L) ? 1u : 0u) << (8 * i);
+      unsigned bits = 0;
+      for (int i = 0; i < nz_tile; ++i) bits |= (general_votes_norm(hf, va, R, zt[i], pr.L) ? 1u : 0u) << i;
+#pragma unroll
+      for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += spread8((bits >> (8 * j)) & 0xffu);
     }
   }
   if (live) {
     uint16_t* out = votes + int64_t(e) * g.cells + ixy * g.col_cells + (int64_t(iR) * nz + iz0) * nL + iL;
-    for (int i = 0; i < nz_tile; ++i) out[int64_t(i) * nL] = uint16_t((acc >> (8 * i)) & 0xffu);
+#pragma unroll
+    for (int i = 0; i < FAST_ZT; ++i)
+      if (i < nz_tile) out[int64_t(i) * nL] = uint16_t((acc[i >> 3] >> (8 * (i & 7))) & 0xffu);
   }
 }
 
