@@ -82,8 +82,9 @@ typedef struct {
  * with the general (sign-agnostic) kernel instead of the sign-specialised one (same results; for
  * cross-checks); bits 1 / 2 = force the one-body / three-body variant of the sign-specialised
  * dense kernel (same results; default: picked from the xy cell width); bit 3 (paper-mode calls only):
- * the turning angle phi_Ax - phi0 of (A.8d) is taken in [0, 2 pi) instead of (-pi, pi] - tracks of more
- * than half a turn, PAPER.md L88 (reading M6); bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
+ * tracks of up to one turn emitted near the z axis (reading M6) - the turning angle
+ * phi_Ax - phi0 of (A.8d) is theta(wire point) - theta(reference point), theta in [-0.3, 2 pi - 0.3) counted from the
+ * point of the base circle closest to the axis, instead of the principal value in (-pi, pi]; bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
  * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
  * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; runs in the
  * general (sign-agnostic) kernels, about 4 x the arithmetic; bit 5: ia_refine / ia_refine_batch always enqueue
@@ -146,13 +147,15 @@ int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t
                   uint16_t* votes_out_dev);
 
 /* f2 (pieces of the paper's iteration scheme; readings F2b, F2c of DESIGN.md).
- * Result of the selection: 88 bytes. */
+ * Result of the selection: 112 bytes. */
 typedef struct {
   double value[4], error[4]; /* xc, yc, R, z0: centre of the mean cell index / half-extent of the selected voxels */
   double lambda;             /* signed, sqrt((P/value[2])^2 - 1); 0 if value[2] > P */
   int32_t lambda_sign;       /* +1: accumulator 0 holds the maximum (ties included), -1: accumulator 1 */
   int32_t vmax;              /* the maximum count */
   int64_t n_sel;             /* number of selected voxels */
+  double x_ref, y_ref;       /* the reference point the pass was voted with: z0 = z where the helix is closest to it */
+  double z0_centre;          /* ia_track_paper: the previous pass's z0 re-expressed for this pass's reference point */
 } ia_paper_fit;
 
 /* L94: "the values and the errors of the parameters are computed using voxels corresponding to selected
@@ -184,14 +187,22 @@ int ia_find_hits_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double m
  * value -/+ factor*error (ia_find_hits_paper; "all hits are always considered for the hit finding", L96).
  * "This procedure is applied for each sign of the lambda value" (L78): one chain per sign (reading F2e) -
  * fits_out_dev[pass][s], s = 0: lambda >= 0, 1: lambda < 0 - and sign_out_dev = +1 / -1 = the sign whose last
- * pass has the larger maximum (L121; ties: +1).  The reference point is the one of ia_set_params throughout
- * (the update of L98 is left to the caller).  passes_host: HOST; fits_out_dev (2*n_passes), sign_out_dev: DEVICE.
- * Windows are expected to stay inside R > 0.  The first pass must be a fixed grid. */
+ * pass has the larger maximum (L121; ties: +1).
+ * Reference point (L98, reading F2d' of DESIGN.md): the first pass is voted with the one of ia_set_params ("The
+ * reference point is set to (0,0)"); a later pass with move_ref != 0 is voted with "the position of measurement point
+ * closest to the recovered circle": of the hits the previous pass of its chain found, the one whose wire point in the
+ * plane z = z_ref, (x_Ax, y_Ax) of (A.4d,e), minimises | |(x_Ax, y_Ax) - (xc, yc)| - R | for that pass's values
+ * (round-to-nearest; ties: lowest hit index; no hit found: the point stays); move_ref == 0 keeps the previous pass's
+ * point.  Every fit records the point of its pass, and its z0 is relative to it; a windowed pass is centred on the
+ * previous pass's value with z0 re-expressed for the new point, z0 + lambda R (theta(new) - theta(old)).  With ia_params.flags bit 3 the turning angles are unwrapped independently of
+ * the reference point (reading M6), which is what lets it move along a track of up to one turn.
+ * passes_host: HOST; fits_out_dev (2*n_passes), sign_out_dev: DEVICE.  Windows are expected to stay inside R > 0.
+ * The first pass must be a fixed grid with move_ref == 0. */
 typedef struct {
   double lo[4], hi[4];
   int32_t dims[4];
   int32_t windowed;
-  int32_t _pad;
+  int32_t move_ref;
 } ia_paper_pass;
 int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momentum_radius, double r_disk, double factor,
                    const ia_paper_pass* passes_host, int n_passes, ia_paper_fit* fits_out_dev, int32_t* sign_out_dev);

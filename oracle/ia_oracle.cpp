@@ -179,7 +179,8 @@ template <class T> struct HitC {
   T mx, my, h2;    // S3: dot term   (X-mx)^2 + (Y-my)^2 - h2
   T d, tol, zref;
   int rigorous;    // params.flags bit 4: Phi from a verified enclosure of the fixed point of (A.6) (reading f3)
-  int full_turn;   // params.flags bit 3 (paper mode only): phi_Ax - phi0 taken in [0, 2 pi) instead of (-pi, pi]
+  int full_turn;   // params.flags bit 3 (paper mode only): turning angles unwrapped for tracks of up to one turn (M6)
+  T xr, yr;        // the reference point (M6 needs it beside the S3 scalars)
 };
 
 template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const OrcParams& p) {
@@ -199,6 +200,7 @@ template <class T> HitC<T> make_hitc(const OrcWire& w, const OrcHit& h, const Or
   c.h2 = opaque(opaque(hx * hx) + opaque(hy * hy));
   c.d = T(h.drift); c.tol = T(p.tol); c.zref = zr;
   c.full_turn = (p.flags & 8u) ? 1 : 0;
+  c.xr = xr; c.yr = yr;
   c.rigorous = (p.flags & 16u) ? 1 : 0;
   return c;
 }
@@ -517,9 +519,26 @@ __attribute__((noinline)) PointEval dax_point(const HitC<double>& c, double xc, 
   const double dx = xc - c.mx, dy = yc - c.my;
   const double dt = (dx * dx + dy * dy) - c.h2;
   double dphi = std::atan2(cr, dt);
-  // reading M6: a counter-clockwise track of less than one turn (L88) has turned by an angle in [0, 2 pi)
-  // when it passes the wire; the principal value is moved there when the caller asks for it
-  if (c.full_turn && dphi < 0.0) dphi = dphi + 6.283185307179586;
+  // reading M6 (flags bit 3): a counter-clockwise track of less than one turn (L88) emitted near the z axis (L88: at the
+  // origin; L123: 5 cm from it) has turned by an angle theta in [-m, 2 pi - m) past the point of its base circle closest
+  // to the axis when it reaches a given point of the circle, m = 0.3 rad.  phi_Ax - phi0 of (A.8d) is taken as
+  // theta(wire point) - theta(reference point): right for every hit of such a track wherever the reference point
+  // lies (it moves along the track between the passes, L98); theta(P) = atan2(cross, dot) of S3 with the reference
+  // replaced by the axis and the wire point by P.  With the reference point at (0, 0) this is the S3 angle moved
+  // from (-pi, pi] to [-m, 2 pi - m).
+  if (c.full_turn) {
+    const double two_pi = 6.283185307179586, m = 0.3;
+    auto theta = [&](double px, double py) {
+      const double hx = 0.5 * px, hy = 0.5 * py;
+      const double cr0 = (0.0 - py) * xc + px * yc;
+      const double ex = xc - hx, ey = yc - hy;
+      const double dt0 = (ex * ex + ey * ey) - (hx * hx + hy * hy);
+      double th = std::atan2(cr0, dt0);
+      if (th < -m) th = th + two_pi;
+      return th;
+    };
+    dphi = theta(c.xA, c.yA) - theta(c.xr, c.yr);
+  }
   // S3'
   const double iQ = 1.0 / Q, RA = std::sqrt(Q), iR = 1.0 / RA;
   const double c2 = (cA * cA - sA * sA) * iQ;
@@ -640,6 +659,8 @@ struct OrcPaperFit {
   int32_t lambda_sign;    // +1 / -1
   int32_t vmax;
   int64_t n_sel;
+  double x_ref, y_ref;    // the reference point the pass was voted with (reading F2d': it moves between passes, L98)
+  double z0_centre;       // the previous pass's z0 re-expressed for this pass's reference point (centre of a z0 window)
 };
 
 // =============================================================================================
@@ -918,6 +939,7 @@ int orc_select_max_paper(const uint16_t* votes, const double* lo, const double* 
   out->lambda_sign = s == 0 ? +1 : -1;
   out->vmax = vmax[s];
   out->n_sel = cnt;
+  out->x_ref = out->y_ref = out->z0_centre = 0.0;   // set by the caller that knows the reference point (orc_track_paper)
   return ORC_OK;
 }
 
@@ -944,30 +966,99 @@ int orc_find_hits_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, i
   return ORC_OK;
 }
 
+// F2d' the reference-point update, L98: "In the second step, the reference point is taken as the position of
+//      measurement point closest to the recovered circle. ... In the third step, a new reference point is defined as
+//      in the previous step."  Reading: measurement points = the hits the previous pass's hit finding
+//      selected (mask != 0; "only the selected hits are used for the next iteration", L96); position of a measurement
+//      point = the wire's point in the transverse plane z = z_ref, (x_Ax, y_Ax) of (A.4d,e) - the transverse position the
+//      vote itself gives the wire; distance to the recovered circle = | sqrt((x_Ax - xc)^2 + (y_Ax - yc)^2) - R | with
+//      (xc, yc, R) the previous pass's values; round-to-nearest double, unfused; ties: the lowest hit index; no
+//      selected hit: the reference point stays.  Returns the chosen hit index (-1: none), out_xy = the new point.
+//      z0 keeps its meaning "z where the helix is closest to the reference point" (eq. (1d)), so after a move
+//      it refers to the new point, and "the value determined by the previous step" on which a window is centred (L98)
+//      is re-expressed for it: z0' = z0 + (lambda R) (theta(new point) - theta(old point)) with the previous pass's
+//      xc, yc, R, lambda (orc_transport_z0 below; the arc between two hits times lambda can exceed the +-40 cm window).
+int orc_move_ref_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const uint8_t* mask,
+                       const OrcParams* p, const OrcPaperFit* prev, double* out_xy) {
+  if (!wires || !hits || !p || !prev || !out_xy || n_hits < 0) return ORC_ERR_ARG;
+  out_xy[0] = p->x_ref; out_xy[1] = p->y_ref;
+  int best = -1;
+  double best_d = 0.0;
+  for (int h = 0; h < n_hits; ++h) {
+    if (mask && !mask[h]) continue;
+    if (hits[h].wire < 0 || hits[h].wire >= n_wires) return ORC_ERR_GEOMETRY;
+    const OrcWire& w = wires[hits[h].wire];
+    const double xA = opaque(w.x0 + opaque(opaque(p->z_ref * w.sin_phi_s) * w.tan_tau));      // (A.4d) L174
+    const double yA = opaque(w.y0 - opaque(opaque(p->z_ref * w.cos_phi_s) * w.tan_tau));      // (A.4e) L176
+    const double dx = opaque(xA - prev->value[0]), dy = opaque(yA - prev->value[1]);
+    const double rho = std::sqrt(opaque(opaque(dx * dx) + opaque(dy * dy)));
+    const double d = std::fabs(opaque(rho - prev->value[2]));
+    if (best < 0 || d < best_d) { best = h; best_d = d; out_xy[0] = xA; out_xy[1] = yA; }
+  }
+  return best;
+}
+
+// z0 of `prev` re-expressed for the reference point (x_new, y_new): turning angles theta as in dax_point - with flags
+// bit 3 counted from the point of the circle closest to the axis in [-0.3, 2 pi - 0.3) (reading M6), else the principal
+// value of eq. (1d)'s phi0, their difference wrapped into (-pi, pi].  Round-to-nearest double, unfused.
+double orc_transport_z0(const OrcParams* p, const OrcPaperFit* prev, double x_new, double y_new) {
+  const double xc = prev->value[0], yc = prev->value[1], two_pi = 6.283185307179586;
+  double dth;
+  if (p->flags & 8u) {
+    auto theta = [&](double px, double py) {
+      const double hx = opaque(0.5 * px), hy = opaque(0.5 * py);
+      const double cr0 = opaque(opaque(opaque(0.0 - py) * xc) + opaque(px * yc));
+      const double ex = opaque(xc - hx), ey = opaque(yc - hy);
+      const double dt0 = opaque(opaque(opaque(ex * ex) + opaque(ey * ey)) - opaque(opaque(hx * hx) + opaque(hy * hy)));
+      double th = std::atan2(cr0, dt0);
+      if (th < -0.3) th = opaque(th + two_pi);
+      return th;
+    };
+    dth = opaque(theta(x_new, y_new) - theta(prev->x_ref, prev->y_ref));
+  } else {
+    dth = opaque(std::atan2(opaque(x_new - xc), opaque(yc - y_new)) - std::atan2(opaque(prev->x_ref - xc), opaque(yc - prev->y_ref)));
+    if (dth > 3.141592653589793) dth = opaque(dth - two_pi);
+    if (dth <= -3.141592653589793) dth = opaque(dth + two_pi);
+  }
+  return opaque(prev->value[3] + opaque(opaque(prev->lambda * prev->value[2]) * dth));
+}
+
 // F2e  the iteration scheme, L92-106: n_passes vote passes; pass i votes its grid with the hits found by the
 //      previous pass (L96), selects the maximum-vote voxels (L94) and finds the hits of the next pass on
 //      value -/+ factor*error.  A pass is either a fixed grid [lo, hi] x dims (Table 1, iterations 1-2) or
 //      a window of half-widths `lo` (sic) around the previous pass's value (iteration 3).
 //      "This procedure is applied for each sign of the lambda value" (L78): reading F2e - one chain per
 //      sign of lambda (accumulator s of every pass, hits found with that sign); the sign is decided by
-//      comparing the maxima of the last pass (L121; ties: lambda >= 0).  The reference point stays where
-//      params put it (the update of L98 is the caller's: DESIGN.md).
-struct OrcPaperPass { double lo[4], hi[4]; int32_t dims[4]; int32_t windowed; int32_t pad; };
+//      comparing the maxima of the last pass (L121; ties: lambda >= 0).  A pass with move_ref != 0 (not the
+//      first) is voted with the reference point of F2d' taken from the previous pass of its chain; every fit
+//      records the reference point of its pass.
+struct OrcPaperPass { double lo[4], hi[4]; int32_t dims[4]; int32_t windowed; int32_t move_ref; };
 
 int orc_track_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n_hits, const OrcParams* p, double P,
                     double r_disk, double factor, const OrcPaperPass* passes, int n_passes, OrcPaperFit* fits_out,
                     int32_t* sign_out) {
   if (!passes || n_passes < 1 || !fits_out || !sign_out || !(factor > 0)) return ORC_ERR_ARG;
-  if (passes[0].windowed) return ORC_ERR_ARG;
+  if (passes[0].windowed || passes[0].move_ref) return ORC_ERR_ARG;
   for (int s = 0; s < 2; ++s) {
     std::vector<uint8_t> mask(n_hits, 1);
     OrcPaperFit prev{};
+    OrcParams pp = *p;                       // the chain's own reference point
     for (int i = 0; i < n_passes; ++i) {
+      if (passes[i].move_ref) {
+        double xy[2];
+        const int rc_m = orc_move_ref_paper(wires, n_wires, hits, n_hits, mask.data(), &pp, &prev, xy);
+        if (rc_m < -1) return rc_m;
+        pp.x_ref = xy[0]; pp.y_ref = xy[1];
+      }
+      // the previous z0 seen from this pass's reference point (unchanged point: unchanged value)
+      const double z0c = i == 0 ? 0.0 : ((pp.x_ref == prev.x_ref && pp.y_ref == prev.y_ref) ? prev.value[3]
+                                                                                             : orc_transport_z0(&pp, &prev, pp.x_ref, pp.y_ref));
       double lo[4], hi[4];
       for (int d = 0; d < 4; ++d) {
         if (passes[i].windowed) {
-          lo[d] = opaque(prev.value[d] - passes[i].lo[d]);
-          hi[d] = opaque(prev.value[d] + passes[i].lo[d]);
+          const double centre = d == 3 ? z0c : prev.value[d];
+          lo[d] = opaque(centre - passes[i].lo[d]);
+          hi[d] = opaque(centre + passes[i].lo[d]);
         } else {
           lo[d] = passes[i].lo[d];
           hi[d] = passes[i].hi[d];
@@ -976,12 +1067,13 @@ int orc_track_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n
       int64_t n = 1;
       for (int d = 0; d < 4; ++d) n *= passes[i].dims[d];
       std::vector<uint16_t> votes(2 * n);
-      int rc = orc_vote_paper(wires, n_wires, hits, n_hits, mask.data(), p, P, r_disk, lo, hi, passes[i].dims, nullptr, 0,
+      int rc = orc_vote_paper(wires, n_wires, hits, n_hits, mask.data(), &pp, P, r_disk, lo, hi, passes[i].dims, nullptr, 0,
                               votes.data());
       if (rc) return rc;
       OrcPaperFit fit;
       rc = orc_select_max_paper(votes.data(), lo, hi, passes[i].dims, P, s == 0 ? +1 : -1, &fit);
       if (rc) return rc;
+      fit.x_ref = pp.x_ref; fit.y_ref = pp.y_ref; fit.z0_centre = z0c;
       fits_out[i * 2 + s] = fit;
       double blo[4], bhi[4];
       for (int d = 0; d < 4; ++d) {
@@ -989,7 +1081,7 @@ int orc_track_paper(const OrcWire* wires, int n_wires, const OrcHit* hits, int n
         blo[d] = opaque(fit.value[d] - e);
         bhi[d] = opaque(fit.value[d] + e);
       }
-      rc = orc_find_hits_paper(wires, n_wires, hits, n_hits, p, P, s == 0 ? +1 : -1, blo, bhi, mask.data());
+      rc = orc_find_hits_paper(wires, n_wires, hits, n_hits, &pp, P, s == 0 ? +1 : -1, blo, bhi, mask.data());
       if (rc) return rc;
       prev = fit;
     }

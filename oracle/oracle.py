@@ -222,7 +222,7 @@ def cell_boxes4(lo, hi, dims, cell_idx):
 # ---- pieces of the paper's iteration scheme ------------------------------------------------------
 class PaperFit(C.Structure):
     _fields_ = [("value", C.c_double * 4), ("error", C.c_double * 4), ("lam", C.c_double), ("lambda_sign", C.c_int32),
-                ("vmax", C.c_int32), ("n_sel", C.c_int64)]
+                ("vmax", C.c_int32), ("n_sel", C.c_int64), ("x_ref", C.c_double), ("y_ref", C.c_double), ("z0_centre", C.c_double)]
 
 
 def disk_filter(lo, hi, dims, r_disk: float, cell_idx=None) -> np.ndarray:
@@ -258,20 +258,45 @@ def find_hits_paper(wires, hits, params: Params, P: float, lambda_sign: int, lo,
     return out
 
 
-PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("pad", "i4")])
+PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("move_ref", "i4")])
 FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), ("lambda_sign", "i4"), ("vmax", "i4"),
-                   ("n_sel", "i8")])
+                   ("n_sel", "i8"), ("x_ref", "f8"), ("y_ref", "f8"), ("z0_centre", "f8")])
 
 
-def make_passes(spec) -> np.ndarray:
-    """spec: list of ("grid", lo4, hi4, dims4) or ("window", half4, dims4)."""
+def make_passes(spec, move_ref=False) -> np.ndarray:
+    """spec: list of ("grid", lo4, hi4, dims4) or ("window", half4, dims4); move_ref: every pass but the first is voted
+    with the reference point of L98 (reading F2d')."""
     ps = np.zeros(len(spec), PASS_DT)
+    ps["move_ref"][1:] = 1 if move_ref else 0
     for i, s in enumerate(spec):
         if s[0] == "grid":
             ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[2], s[3], 0
         else:
             ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[1], s[2], 1
     return ps
+
+
+def move_ref_paper(wires, hits, mask, params: Params, prev_fit):
+    """F2d' (L98): (index of the selected hit whose wire point in the plane z_ref is closest to the circle of prev_fit,
+    or -1; the new reference point (x, y))."""
+    out = np.zeros(2)
+    fit = np.zeros(1, FIT_DT)
+    fit[0] = prev_fit
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    rc = lib().orc_move_ref_paper(_p(wires), len(wires), _p(hits), len(hits), None if m is None else _p(m), C.byref(params),
+                                  _p(fit), _p(out))
+    if rc < -1:
+        _chk(rc, "move_ref_paper")
+    return rc, out
+
+
+def transport_z0(params: Params, prev_fit, x_new: float, y_new: float) -> float:
+    """z0 of prev_fit re-expressed for the reference point (x_new, y_new) (reading F2d')."""
+    fit = np.zeros(1, FIT_DT)
+    fit[0] = prev_fit
+    f = lib().orc_transport_z0
+    f.restype = C.c_double
+    return float(f(C.byref(params), _p(fit), C.c_double(x_new), C.c_double(y_new)))
 
 
 def track_paper(wires, hits, params: Params, P: float, r_disk: float, factor: float, passes: np.ndarray):

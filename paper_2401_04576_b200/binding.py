@@ -23,9 +23,9 @@ WIRE_DT = np.dtype([("x0", "f8"), ("y0", "f8"), ("sin_phi_s", "f8"), ("cos_phi_s
 HIT_DT = np.dtype([("wire", "i4"), ("_pad", "i4"), ("drift", "f8")])
 BOX_DT = np.dtype([("lo", "f8", (5,)), ("hi", "f8", (5,)), ("votes", "u2"), ("_pad", "u2", (3,))])
 FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), ("lambda_sign", "i4"), ("vmax", "i4"),
-                   ("n_sel", "i8")])
-PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("_pad", "i4")])
-assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 88
+                   ("n_sel", "i8"), ("x_ref", "f8"), ("y_ref", "f8"), ("z0_centre", "f8")])
+PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("move_ref", "i4")])
+assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 112
 
 EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_residual_fast", "ia_prim",

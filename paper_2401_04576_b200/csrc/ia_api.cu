@@ -308,8 +308,8 @@ int ia_vote_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const uint8_t
   if (rc) return rc;
   if (!(box_lo[2] > 0.0)) return IA_ERR_DOMAIN;
   DeviceGuard guard(ctx->device);
-  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}};
-  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, pg, 3, votes_out_dev));
+  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}, nullptr};
+  IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, hit_mask_dev, momentum_radius, r_disk, pg, 3, nullptr, votes_out_dev));
   return IA_OK;
 }
 
@@ -320,8 +320,8 @@ int ia_select_max_paper(ia_ctx* ctx, const uint16_t* votes_dev, double momentum_
   int rc = make_grid4(box_lo, box_hi, grid_dims, g);
   if (rc) return rc;
   DeviceGuard guard(ctx->device);
-  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}};
-  IA_CUDA(ctx, launch_select_max_paper(ctx, votes_dev, pg, momentum_radius, which, fit_out_dev));
+  PaperGrid pg = {g, nullptr, {0, 0, 0, 0}, nullptr};
+  IA_CUDA(ctx, launch_select_max_paper(ctx, votes_dev, pg, momentum_radius, which, 0, fit_out_dev));
   return IA_OK;
 }
 
@@ -341,7 +341,8 @@ int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momen
   int rc = check_ready(ctx);
   if (rc) return rc;
   if (n_hits <= 0 || !hits_dev || !passes_host || n_passes < 1 || !fits_out_dev || !sign_out_dev) return IA_ERR_ARG;
-  if (!(momentum_radius > 0.0) || !(factor > 0.0) || std::isnan(r_disk) || passes_host[0].windowed) return IA_ERR_ARG;
+  if (!(momentum_radius > 0.0) || !(factor > 0.0) || std::isnan(r_disk) || passes_host[0].windowed || passes_host[0].move_ref)
+    return IA_ERR_ARG;
   if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
   std::vector<PaperGrid> grids(n_passes);
   int64_t max_cells = 0;
@@ -361,6 +362,7 @@ int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momen
     }
     if (rc) return rc;
     grids[i].centre = nullptr;
+    grids[i].self = nullptr;
     max_cells = std::max(max_cells, grids[i].g.cells);
   }
   DeviceGuard guard(ctx->device);
@@ -371,13 +373,17 @@ int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momen
   for (int i = 0; i < n_passes; ++i) {
     for (int s = 0; s < 2; ++s) {
       PaperGrid pg = grids[i];
-      if (passes_host[i].windowed) pg.centre = fits_out_dev + (i - 1) * 2 + s;
       ia_paper_fit* fit = fits_out_dev + i * 2 + s;
-      // the first pass is the same vote for both chains (all hits, fixed grid): voted once
+      if (passes_host[i].windowed) { pg.centre = fit - 2; pg.self = fit; }
+      // the reference point of this pass goes into its fit slot first: ia_params' for the first pass, then the previous
+      // pass's of the chain, moved along the track where the pass asks for it (F2d', L98)
+      IA_CUDA(ctx, launch_paper_ref(ctx, hits_dev, n_hits, i == 0 ? nullptr : mask[s], i == 0 ? nullptr : fit - 2,
+                                    i > 0 && passes_host[i].move_ref ? 1 : 0, fit));
+      // the first pass is the same vote for both chains (all hits, fixed grid, same reference point): voted once
       if (i > 0 || s == 0)
         IA_CUDA(ctx, launch_vote_paper(ctx, hits_dev, n_hits, i == 0 ? nullptr : mask[s], momentum_radius, r_disk, pg,
-                                       i == 0 ? 3 : (s == 0 ? 1 : 2), votes));
-      IA_CUDA(ctx, launch_select_max_paper(ctx, votes, pg, momentum_radius, s == 0 ? +1 : -1, fit));
+                                       i == 0 ? 3 : (s == 0 ? 1 : 2), fit, votes));
+      IA_CUDA(ctx, launch_select_max_paper(ctx, votes, pg, momentum_radius, s == 0 ? +1 : -1, 1, fit));
       IA_CUDA(ctx, launch_find_hits_paper(ctx, hits_dev, n_hits, momentum_radius, fit, factor, mask[s]));
     }
   }

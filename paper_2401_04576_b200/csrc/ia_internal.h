@@ -119,13 +119,20 @@ cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia
 // a window of half-widths `half` around a fit on the device (g then carries only the dims)
 struct PaperGrid {
   GridDesc g;
-  const ia_paper_fit* centre;
+  const ia_paper_fit* centre;   // previous pass: value[0..2] centre the window
   double half[4];
+  const ia_paper_fit* self;     // this pass's slot: z0_centre (the previous z0 seen from this pass's reference point); may be nullptr
 };
+// ref (device, may be nullptr): the fit slot that holds the reference point of this pass; nullptr: ia_params'
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const PaperGrid& pg, int signs, uint16_t* votes_out);   // votes_out [2][cells]; signs: bit 0 / 1
+                              const PaperGrid& pg, int signs, const ia_paper_fit* ref, uint16_t* votes_out);   // votes_out [2][cells]; signs: bit 0 / 1
+// keep_ref: fit_out already holds the reference point of its pass (ia_track_paper); else ia_params' is written
 cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const PaperGrid& pg, double P, int which,
-                                    ia_paper_fit* fit_out);
+                                    int keep_ref, ia_paper_fit* fit_out);
+// F2d' (L98): next->x_ref, y_ref = the reference point of prev (move == 0; prev == nullptr: ia_params') or the wire point
+// of the selected hit closest to prev's circle (move != 0)
+cudaError_t launch_paper_ref(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* mask, const ia_paper_fit* prev, int move,
+                             ia_paper_fit* next);
 cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, double P, const ia_paper_fit* fit, double factor,
                                    uint8_t* flags_out);
 cudaError_t launch_paper_sign(ia_ctx* ctx, const ia_paper_fit* last, int32_t* sign_out);

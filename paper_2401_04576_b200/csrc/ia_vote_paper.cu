@@ -36,8 +36,9 @@ IA_DEV double sub(double a, double b) { return __dadd_rn(a, -b); }
 
 // per-hit scalars (round to nearest, unfused: the same operations as stage_hits_kernel) and the
 // (xc_m, yc_m)-dependent point values of S2, S3, S3'
-__device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit h, const ia_params& p, Iv<double> X,
-                          Iv<double> Y, int* status, PHit& o) {
+// (xr, yr): the reference point of this pass - ia_params' or, inside ia_track_paper, the one of reading F2d'
+__device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit h, const ia_params& p, double xr, double yr,
+                          Iv<double> X, Iv<double> Y, int* status, PHit& o) {
   int w = h.wire;
   o.valid = (w >= 0 && w < n_wires && h.drift >= 0.0);
   if (!o.valid) {
@@ -47,7 +48,7 @@ __device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit 
   }
   const double x0 = wires[w], y0 = wires[n_wires + w], s = wires[2 * n_wires + w], co = wires[3 * n_wires + w];
   const double t = wires[4 * n_wires + w];
-  const double xr = p.x_ref, yr = p.y_ref, zr = p.z_ref;
+  const double zr = p.z_ref;
   const double xA = add(x0, mul(mul(zr, s), t));                       // (A.4d)
   const double yA = sub(y0, mul(mul(zr, co), t));                      // (A.4e)
   const double k0 = sub(mul(xr, yA), mul(yr, xA)), ky = sub(yr, yA), kx = sub(xA, xr);
@@ -70,8 +71,23 @@ __device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit 
   const double dx = sub(xc, mx_), dy = sub(yc, my_);
   const double dt = sub(add(mul(dx, dx), mul(dy, dy)), h2);
   double dphi = atan2(cr, dt);
-  // reading M6 (flags bit 3): turning angle of a counter-clockwise track of less than one turn, in [0, 2 pi)
-  if ((p.flags & 8u) && dphi < 0.0) dphi = add(dphi, 6.283185307179586);
+  // reading M6 (flags bit 3): a counter-clockwise track of less than one turn emitted near the z axis has turned by
+  // theta in [-m, 2 pi - m), m = 0.3 rad, past the point of its base circle closest to the axis when it reaches a point
+  // P of the circle; phi_Ax - phi0 of (A.8d) = theta(wire point) - theta(reference point), right wherever the
+  // reference point lies along the track (it moves between passes, L98).  theta(P) = the S3 angle with the reference
+  // at the axis and the wire point at P; same operations, same order as the oracle's.
+  if (p.flags & 8u) {
+    auto theta = [&](double px, double py) {
+      const double hx_ = mul(0.5, px), hy_ = mul(0.5, py);
+      const double cr0 = add(mul(sub(0.0, py), xc), mul(px, yc));
+      const double ex = sub(xc, hx_), ey = sub(yc, hy_);
+      const double dt0 = sub(add(mul(ex, ex), mul(ey, ey)), add(mul(hx_, hx_), mul(hy_, hy_)));
+      double th = atan2(cr0, dt0);
+      if (th < -0.3) th = add(th, 6.283185307179586);
+      return th;
+    };
+    dphi = sub(theta(xA, yA), theta(xr, yr));
+  }
   o.dphi = dphi;
   o.iQ = __ddiv_rn(1.0, Qp);
   o.RA = __dsqrt_rn(Qp);
@@ -133,8 +149,9 @@ IA_DEV GridDesc resolve_grid(const PaperGrid& pg) {
   if (pg.centre) {
 #pragma unroll
     for (int d = 0; d < 4; ++d) {
-      g.lo[d] = sub(pg.centre->value[d], pg.half[d]);
-      g.hi[d] = add(pg.centre->value[d], pg.half[d]);
+      const double c = (d == 3 && pg.self) ? pg.self->z0_centre : pg.centre->value[d];
+      g.lo[d] = sub(c, pg.half[d]);
+      g.hi[d] = add(c, pg.half[d]);
       g.w[d] = __ddiv_rn(sub(g.hi[d], g.lo[d]), double(g.n[d]));
     }
   }
@@ -174,8 +191,8 @@ IA_DEV bool disk_passes(Iv<double> X, Iv<double> Y, Iv<double> R, double r_disk)
 
 __global__ void __launch_bounds__(PAPER_THREADS)
 vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __restrict__ hit_mask,
-                  const double* __restrict__ wires, int n_wires, ia_params p, double P, double r_disk, PaperGrid pg, int signs,
-                  int* status, uint16_t* __restrict__ votes) {
+                  const double* __restrict__ wires, int n_wires, ia_params p, const ia_paper_fit* __restrict__ ref, double P,
+                  double r_disk, PaperGrid pg, int signs, int* status, uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PHit* sh = reinterpret_cast<PHit*>(smem_raw);
   const GridDesc g = resolve_grid(pg);
@@ -183,8 +200,10 @@ vote_paper_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __
   const int ix = ixy / g.n[1], iy = ixy - ix * g.n[1];
   const Iv<double> X = {cell_edge(g.lo[0], g.hi[0], g.w[0], ix, g.n[0]), cell_edge(g.lo[0], g.hi[0], g.w[0], ix + 1, g.n[0])};
   const Iv<double> Y = {cell_edge(g.lo[1], g.hi[1], g.w[1], iy, g.n[1]), cell_edge(g.lo[1], g.hi[1], g.w[1], iy + 1, g.n[1])};
+  // ref != nullptr: the reference point of this pass sits on the device (written by paper_ref_kernel just before)
+  const double xr = ref ? ref->x_ref : p.x_ref, yr = ref ? ref->y_ref : p.y_ref;
   for (int h = threadIdx.x; h < n_hits; h += blockDim.x) {
-    make_phit(wires, n_wires, hits[h], p, X, Y, status, sh[h]);
+    make_phit(wires, n_wires, hits[h], p, xr, yr, X, Y, status, sh[h]);
     if (hit_mask && !hit_mask[h]) sh[h].valid = 0;       // L96: only the selected hits are used
   }
   __syncthreads();
@@ -287,7 +306,7 @@ __global__ void paper_moments_kernel(const uint16_t* __restrict__ votes, int64_t
 }
 
 __global__ void paper_fit_kernel(const unsigned long long* __restrict__ acc, PaperGrid pg, double P, int which,
-                                 ia_paper_fit* __restrict__ out) {
+                                 int keep_ref, double x_ref, double y_ref, ia_paper_fit* __restrict__ out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   const GridDesc g = resolve_grid(pg);
   const int s = pick_acc(acc, which);
@@ -304,6 +323,10 @@ __global__ void paper_fit_kernel(const unsigned long long* __restrict__ acc, Pap
   f.lambda_sign = s == 0 ? 1 : -1;
   f.vmax = int32_t(acc[s]);
   f.n_sel = int64_t(cnt);
+  // the reference point of the pass: written into the slot before the vote (ia_track_paper) or the caller's (ia_params)
+  f.x_ref = keep_ref ? out->x_ref : x_ref;
+  f.y_ref = keep_ref ? out->y_ref : y_ref;
+  f.z0_centre = keep_ref ? out->z0_centre : 0.0;
   *out = f;
 }
 
@@ -320,7 +343,7 @@ __global__ void find_hits_paper_kernel(const ia_hit* __restrict__ hits, int n_hi
     hi[d] = add(fit->value[d], e);
   }
   PHit ph;
-  make_phit(wires, n_wires, hits[h], p, Iv<double>{lo[0], hi[0]}, Iv<double>{lo[1], hi[1]}, status, ph);
+  make_phit(wires, n_wires, hits[h], p, fit->x_ref, fit->y_ref, Iv<double>{lo[0], hi[0]}, Iv<double>{lo[1], hi[1]}, status, ph);
   const Iv<double> R = {lo[2], hi[2]};
   const double Rm = mul(0.5, add(lo[2], hi[2])), zm = mul(0.5, add(lo[3], hi[3]));
   double lam;
@@ -333,7 +356,7 @@ __global__ void find_hits_paper_kernel(const ia_hit* __restrict__ hits, int n_hi
 }  // namespace
 
 cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* hit_mask, double P, double r_disk,
-                              const PaperGrid& pg, int signs, uint16_t* votes_out) {
+                              const PaperGrid& pg, int signs, const ia_paper_fit* ref, uint16_t* votes_out) {
   const GridDesc& g = pg.g;
   const size_t smem = size_t(n_hits) * sizeof(PHit);
   cudaError_t err = cudaFuncSetAttribute(vote_paper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
@@ -342,13 +365,14 @@ cudaError_t launch_vote_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, const
   int threads = PAPER_THREADS;
   if (col < threads) threads = (col + 31) / 32 * 32;
   vote_paper_kernel<<<unsigned(g.n[0] * g.n[1]), threads, smem, ctx->stream>>>(hits, n_hits, hit_mask, ctx->wires, ctx->n_wires,
-                                                                              ctx->params, P, r_disk, pg, signs, ctx->status, votes_out);
+                                                                              ctx->params, ref, P, r_disk, pg, signs, ctx->status,
+                                                                              votes_out);
   ctx->launches++;
   return cudaGetLastError();
 }
 
 cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const PaperGrid& pg, double P, int which,
-                                    ia_paper_fit* fit_out) {
+                                    int keep_ref, ia_paper_fit* fit_out) {
   cudaError_t err = scratch_reserve(ctx->keys, 16 * sizeof(unsigned long long));
   if (err != cudaSuccess) return err;
   unsigned long long* acc = static_cast<unsigned long long*>(ctx->keys.p);
@@ -358,7 +382,7 @@ cudaError_t launch_select_max_paper(ia_ctx* ctx, const uint16_t* votes, const Pa
   if (blocks > 1184) blocks = 1184;
   paper_max_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, acc);
   paper_moments_kernel<<<blocks, 256, 0, ctx->stream>>>(votes, n, pg.g, which, acc);   // cell indices only: dims suffice
-  paper_fit_kernel<<<1, 32, 0, ctx->stream>>>(acc, pg, P, which, fit_out);
+  paper_fit_kernel<<<1, 32, 0, ctx->stream>>>(acc, pg, P, which, keep_ref, ctx->params.x_ref, ctx->params.y_ref, fit_out);
   ctx->launches += 4;
   return cudaGetLastError();
 }
@@ -373,10 +397,81 @@ cudaError_t launch_find_hits_paper(ia_ctx* ctx, const ia_hit* hits, int n_hits, 
 }
 
 namespace {
+// F2d' (L98): the reference point of the next pass = the z_ref-plane point (A.4d,e) of the wire of the selected hit
+// (mask != 0) closest to the circle of the previous pass's fit; ties: lowest hit index; none selected: it stays.
+// mode 0: copy the reference point of `prev` (or of ia_params when prev == nullptr) into next; 1: move it.
+__global__ void paper_ref_kernel(const ia_hit* __restrict__ hits, int n_hits, const uint8_t* __restrict__ mask,
+                                 const double* __restrict__ wires, int n_wires, ia_params p, const ia_paper_fit* __restrict__ prev,
+                                 int mode, ia_paper_fit* __restrict__ next) {
+  const double x_old = prev ? prev->x_ref : p.x_ref, y_old = prev ? prev->y_ref : p.y_ref;
+  if (mode == 0) {
+    if (threadIdx.x == 0) { next->x_ref = x_old; next->y_ref = y_old; next->z0_centre = prev ? prev->value[3] : 0.0; }
+    return;
+  }
+  // one warp: every lane keeps the best of its hits (strict <, so the lowest index of equal distances), then a
+  // shuffle reduction on (distance, index).  Distances are non-negative doubles: their bit patterns order like the values.
+  unsigned long long bd = ~0ull;
+  int bh = 0x7fffffff;
+  double bx = x_old, by = y_old;
+  for (int h = threadIdx.x; h < n_hits; h += 32) {
+    if (mask && !mask[h]) continue;
+    const int w = hits[h].wire;
+    if (w < 0 || w >= n_wires) continue;
+    const double x0 = wires[w], y0 = wires[n_wires + w], s = wires[2 * n_wires + w], co = wires[3 * n_wires + w], t = wires[4 * n_wires + w];
+    const double xA = add(x0, mul(mul(p.z_ref, s), t)), yA = sub(y0, mul(mul(p.z_ref, co), t));       // (A.4d,e)
+    const double dx = sub(xA, prev->value[0]), dy = sub(yA, prev->value[1]);
+    const double d = fabs(sub(__dsqrt_rn(add(mul(dx, dx), mul(dy, dy))), prev->value[2]));
+    const unsigned long long db = (unsigned long long)__double_as_longlong(d);
+    if (db < bd) { bd = db; bh = h; bx = xA; by = yA; }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    const unsigned long long od = __shfl_down_sync(0xffffffffu, bd, off);
+    const int oh = __shfl_down_sync(0xffffffffu, bh, off);
+    const double ox = __shfl_down_sync(0xffffffffu, bx, off), oy = __shfl_down_sync(0xffffffffu, by, off);
+    if (od < bd || (od == bd && oh < bh)) { bd = od; bh = oh; bx = ox; by = oy; }
+  }
+  if (threadIdx.x == 0) {
+    next->x_ref = bx;
+    next->y_ref = by;
+    // the previous z0 seen from the new point: z0 + (lambda R) (theta(new) - theta(old)), angles as in make_phit
+    double z0c = prev->value[3];
+    if (!(bx == x_old && by == y_old)) {
+      const double xc = prev->value[0], yc = prev->value[1], two_pi = 6.283185307179586;
+      double dth;
+      if (p.flags & 8u) {
+        auto theta = [&](double px, double py) {
+          const double hx_ = mul(0.5, px), hy_ = mul(0.5, py);
+          const double cr0 = add(mul(sub(0.0, py), xc), mul(px, yc));
+          const double ex = sub(xc, hx_), ey = sub(yc, hy_);
+          const double dt0 = sub(add(mul(ex, ex), mul(ey, ey)), add(mul(hx_, hx_), mul(hy_, hy_)));
+          double th = atan2(cr0, dt0);
+          if (th < -0.3) th = add(th, two_pi);
+          return th;
+        };
+        dth = sub(theta(bx, by), theta(x_old, y_old));
+      } else {
+        dth = sub(atan2(sub(bx, xc), sub(yc, by)), atan2(sub(x_old, xc), sub(yc, y_old)));
+        if (dth > 3.141592653589793) dth = sub(dth, two_pi);
+        if (dth <= -3.141592653589793) dth = add(dth, two_pi);
+      }
+      z0c = add(prev->value[3], mul(mul(prev->lambda, prev->value[2]), dth));
+    }
+    next->z0_centre = z0c;
+  }
+}
+
 __global__ void paper_sign_kernel(const ia_paper_fit* __restrict__ last, int32_t* __restrict__ sign_out) {
   if (threadIdx.x == 0) *sign_out = last[1].vmax > last[0].vmax ? -1 : 1;      // L121; ties: lambda >= 0
 }
 }  // namespace
+
+cudaError_t launch_paper_ref(ia_ctx* ctx, const ia_hit* hits, int n_hits, const uint8_t* mask, const ia_paper_fit* prev, int move,
+                             ia_paper_fit* next) {
+  paper_ref_kernel<<<1, 32, 0, ctx->stream>>>(hits, n_hits, mask, ctx->wires, ctx->n_wires, ctx->params, prev, move, next);
+  ctx->launches++;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_paper_sign(ia_ctx* ctx, const ia_paper_fit* last, int32_t* sign_out) {
   paper_sign_kernel<<<1, 32, 0, ctx->stream>>>(last, sign_out);

@@ -112,24 +112,46 @@ def chamber_c4() -> Chamber:      # configs[4]: 40 layers r=20+1.25l, 256 wires/
 
 @dataclass
 class Track:
-    """Helix of eq. (1a-d) through the reference point (0,0): counter-clockwise, R>0."""
+    """Helix of eq. (1a-d): counter-clockwise, R>0, emitted at (xv, yv, z0) with direction phi in the
+    transverse plane; the emission point is the reference point (0,0) unless stated (PAPER.md L123 also emits at
+    (5 cm, 0) and (0, 5 cm))."""
     R: float
     phi: float
     z0: float
     lam: float
+    xv: float = 0.0
+    yv: float = 0.0
 
     @property
     def xc(self) -> float:
-        return -self.R * math.sin(self.phi)
+        return self.xv - self.R * math.sin(self.phi)
 
     @property
     def yc(self) -> float:
-        return self.R * math.cos(self.phi)
+        return self.yv + self.R * math.cos(self.phi)
 
     @property
     def params(self):
-        """(xc, yc, R, z0, lambda) - the order of the vote's five axes."""
+        """(xc, yc, R, z0, lambda) - the order of the vote's five axes; z0 = z at the emission point."""
         return (self.xc, self.yc, self.R, self.z0, self.lam)
+
+    def z0_at(self, x_ref: float, y_ref: float, unwrap: bool = False) -> float:
+        """z where the helix is closest (in the transverse plane) to the reference point (x_ref, y_ref): the z0 of eq. (1)
+        for that reference point (phi0 = atan2(x_ref - xc, yc - y_ref), L49), on the turn that contains the emission."""
+        phi0 = math.atan2(x_ref - self.xc, self.yc - y_ref)
+        if unwrap:
+            # turning angles counted from the point of the circle closest to the z axis, in [-0.3, 2 pi - 0.3): the
+            # convention of the paper-mode vote for tracks of up to one turn (reading M6)
+            phi00 = math.atan2(-self.xc, self.yc)
+            th_ref = (phi0 - phi00 + 0.3) % (2.0 * math.pi) - 0.3
+            th_v = (self.phi - phi00 + math.pi) % (2.0 * math.pi) - math.pi
+            dphi = th_ref - th_v
+        else:
+            dphi = (phi0 - self.phi + math.pi) % (2.0 * math.pi) - math.pi
+        return self.z0 + self.lam * self.R * dphi
+
+    def params_at(self, x_ref: float, y_ref: float, unwrap: bool = False):
+        return (self.xc, self.yc, self.R, self.z0_at(x_ref, y_ref, unwrap), self.lam)
 
 
 def helix_wire_dca(trk: Track, ch: Chamber, wire_ids: np.ndarray, s_init: np.ndarray,
@@ -347,13 +369,13 @@ def chamber_paper() -> Chamber:
     return make_chamber(20, 49.6, (83.7 - 49.6) / 19.0, 250, 0.1, half_len=PAPER_HALF_LEN)
 
 
-def make_track_paper(rng: SplitMix64) -> Track:
+def make_track_paper(rng: SplitMix64, vertex=(0.0, 0.0)) -> Track:
     lam = 0.45 + 0.40 * rng.uniform()
     if rng.uniform() < 0.5:
         lam = -lam
     phi = 2.0 * math.pi * rng.uniform()
     R = PAPER_P / math.sqrt(1.0 + lam * lam)
-    return Track(R, phi, 0.0, lam)
+    return Track(R, phi, 0.0, lam, float(vertex[0]), float(vertex[1]))
 
 
 def track_hits_all_wires(trk: Track, ch: Chamber, d_max: float = PAPER_DRIFT_MAX, ds: float = 0.25):
@@ -395,10 +417,12 @@ def track_hits_all_wires(trk: Track, ch: Chamber, d_max: float = PAPER_DRIFT_MAX
     return cand[ok][order].astype(np.int32), d[ok][order], sp[ok][order], zw[ok][order]
 
 
-def make_event_paper(ch: Chamber, seed: int, n_noise: int = 0, smear: float = 0.0, track: Track | None = None) -> Event:
-    """Paper-shaped event: the paper simulates no measurement error (L88: smear = 0 by default) and no noise."""
+def make_event_paper(ch: Chamber, seed: int, n_noise: int = 0, smear: float = 0.0, track: Track | None = None,
+                     vertex=(0.0, 0.0)) -> Event:
+    """Paper-shaped event: the paper simulates no measurement error (L88: smear = 0 by default) and no noise.
+    vertex: emission point in the transverse plane (L123: the origin, (5, 0) cm, (0, 5) cm)."""
     rng = SplitMix64(seed)
-    trk = track if track is not None else make_track_paper(rng)
+    trk = track if track is not None else make_track_paper(rng, vertex)
     wires, d_true, s_perp, z_wire = track_hits_all_wires(trk, ch)
     drift = np.empty(len(wires))
     clipped = np.zeros(len(wires), bool)

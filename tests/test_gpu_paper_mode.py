@@ -192,8 +192,9 @@ def test_f2_selection_special_cases_on_device():
 PLO, PHI = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
 
 
-def _passes(spec):
+def _passes(spec, move_ref=False):
     ps = np.zeros(len(spec), b.PASS_DT)
+    ps["move_ref"][1:] = 1 if move_ref else 0          # L98: every pass but the first is voted with the moved reference point
     for i, s in enumerate(spec):
         if s[0] == "grid":
             ps[i]["lo"], ps[i]["hi"], ps[i]["dims"], ps[i]["windowed"] = s[1], s[2], s[3], 0
@@ -214,17 +215,31 @@ def test_track_paper_matches_the_oracle_chain():
     try:
         spec = [("grid", PLO, PHI, (24, 24, 16, 10)), ("grid", PLO, PHI, (36, 36, 16, 10)),
                 ("window", (3.0, 3.0, 2.0, 30.0), (20, 20, 16, 10))]
-        for seed in (300, 301, 302):
-            ev = g.make_event_paper(ch, seed, n_noise=3)
+        # fixed reference point, then the reference point of L98 (reading F2d') on tracks from the origin and from (5, 0) cm
+        for seed, move, vertex in ((300, False, (0.0, 0.0)), (301, False, (0.0, 0.0)), (302, False, (0.0, 0.0)),
+                                   (300, True, (0.0, 0.0)), (301, True, (0.0, 0.0)), (303, True, (5.0, 0.0)), (304, True, (0.0, 5.0))):
+            ev = g.make_event_paper(ch, seed, n_noise=3, vertex=vertex)
             hd, oh = rig.hits(ev.wire, ev.drift)
             rig.ctx.ia_set_params(0.01, flags=8)
-            fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec), r_disk=10.0, factor=5.0)
+            fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec, move), r_disk=10.0, factor=5.0)
             rig.ctx.synchronize()
             fg = _fits_to_host(fits_dev, len(spec))
-            fo, so = o.track_paper(rig.owires, oh, o.make_params(0.01, flags=8), g.PAPER_P, 10.0, 5.0, o.make_passes(spec))
+            fo, so = o.track_paper(rig.owires, oh, o.make_params(0.01, flags=8), g.PAPER_P, 10.0, 5.0, o.make_passes(spec, move))
             assert int(sign_dev.cpu().numpy()[0]) == so
-            for name in ("value", "error", "lam", "lambda_sign", "vmax", "n_sel"):
-                assert (fg[name] == fo[name]).all(), (seed, name, fg[name], fo[name])
+            for name in ("lambda_sign", "vmax", "n_sel", "x_ref", "y_ref"):
+                assert (fg[name] == fo[name]).all(), (seed, move, name, fg[name], fo[name])
+            assert np.allclose(fg["z0_centre"], fo["z0_centre"], rtol=0, atol=1e-9)      # transported with atan2: to rounding
+            for name in ("value", "error", "lam"):
+                # the global passes bit for bit; the window after a moved reference point is centred on a z0 transported
+                # with atan2 (CUDA's against glibc's: an ulp), so its grid - and with it the fit - agrees to rounding
+                assert (fg[name][:2] == fo[name][:2]).all(), (seed, move, name, fg[name], fo[name])
+                if move:
+                    assert np.allclose(fg[name][2], fo[name][2], rtol=0, atol=1e-9), (seed, name, fg[name][2], fo[name][2])
+                else:
+                    assert (fg[name][2] == fo[name][2]).all(), (seed, name, fg[name][2], fo[name][2])
+            assert (fg["x_ref"][0] == 0.0).all() and (fg["y_ref"][0] == 0.0).all()
+            if move:
+                assert (np.hypot(fg["x_ref"][1:], fg["y_ref"][1:]) > 40.0).all()      # on a wire of the chamber (r >= 49.6 cm)
     finally:
         rig.close()
 
@@ -239,23 +254,26 @@ def test_track_paper_recovers_the_generated_helix():
         spec = [("grid", PLO, PHI, (50, 50, 40, 20)), ("grid", PLO, PHI, (90, 90, 40, 20)),
                 ("window", (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20))]
         rig.ctx.ia_set_params(0.0, flags=8)
-        ok_sign, dev = 0, []
-        seeds = range(400, 424)
-        for seed in seeds:
-            ev = g.make_event_paper(ch, seed)
-            hd, _ = rig.hits(ev.wire, ev.drift)
-            fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec))
-            rig.ctx.synchronize()
-            fg = _fits_to_host(fits_dev, 3)
-            s = int(sign_dev.cpu().numpy()[0])
-            ok_sign += s == (1 if ev.track.lam >= 0 else -1)
-            f = fg[2, 0 if s > 0 else 1]
-            dev.append(np.abs(np.array(f["value"]) - np.array(ev.track.params[:4])))
-        dev = np.array(dev)
-        assert ok_sign >= len(seeds) - 1, ok_sign
-        good = (dev[:, :3] < 0.3).all(axis=1) & (dev[:, 3] < 4.0)
-        assert good.mean() >= 0.9, (good.mean(), np.median(dev, axis=0))
-        assert (np.median(dev, axis=0) < np.array([0.1, 0.1, 0.1, 2.0])).all(), np.median(dev, axis=0)
+        for move, vertex in ((False, (0.0, 0.0)), (True, (0.0, 0.0)), (True, (5.0, 0.0))):
+            ok_sign, dev = 0, []
+            seeds = range(400, 424)
+            for seed in seeds:
+                ev = g.make_event_paper(ch, seed, vertex=vertex)
+                hd, _ = rig.hits(ev.wire, ev.drift)
+                fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec, move))
+                rig.ctx.synchronize()
+                fg = _fits_to_host(fits_dev, 3)
+                s = int(sign_dev.cpu().numpy()[0])
+                ok_sign += s == (1 if ev.track.lam >= 0 else -1)
+                f = fg[2, 0 if s > 0 else 1]
+                # z0 of a fit is relative to the reference point of its pass: compare with the generated helix there
+                truth = np.array(ev.track.params_at(float(f["x_ref"]), float(f["y_ref"]), unwrap=True)[:4])
+                dev.append(np.abs(np.array(f["value"]) - truth))
+            dev = np.array(dev)
+            assert ok_sign >= len(seeds) - 1, (move, vertex, ok_sign)
+            good = (dev[:, :3] < 0.3).all(axis=1) & (dev[:, 3] < 4.0)
+            assert good.mean() >= 0.9, (move, vertex, good.mean(), np.median(dev, axis=0))
+            assert (np.median(dev, axis=0) < np.array([0.1, 0.1, 0.1, 2.0])).all(), (move, vertex, np.median(dev, axis=0))
     finally:
         rig.close()
 

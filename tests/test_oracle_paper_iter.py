@@ -219,3 +219,117 @@ def test_f2e_chain_is_the_composition_of_its_pinned_pieces():
         assert list(f1.value) == list(fits[1, s]["value"]) and list(f1.error) == list(fits[1, s]["error"])
         assert f1.vmax == fits[1, s]["vmax"] and f1.lambda_sign == which
     assert sign == (-1 if fits[1, 1]["vmax"] > fits[1, 0]["vmax"] else 1)
+
+
+# ---- F2d': the reference-point update of L98 ------------------------------------------------------------------------
+
+def _fit(xc, yc, R):
+    f = np.zeros(1, o.FIT_DT)
+    f[0]["value"] = (xc, yc, R, 0.0)
+    return f[0]
+
+
+def test_f2d_move_ref_special_cases():
+    """The new reference point is the z_ref-plane point of the wire of the SELECTED hit that lies closest to the recovered
+    circle: cases the definition fixes - a circle drawn through one wire point picks that wire; a masked hit is never
+    picked; of two equal hits the first wins; no selected hit leaves the point where it was; the point is on the wire
+    line at z = z_ref (independent parametrisation of the wire: (x0, y0, 0) + z (sin phi_s tan tau, -cos phi_s tan tau, 1))."""
+    ch = g.chamber_paper()
+    wires = o.wires_of(ch)
+    rng = np.random.default_rng(8)
+    for z_ref in (0.0, 12.5, -30.0):
+        p = o.make_params(0.0, x_ref=0.3, y_ref=-0.2, z_ref=z_ref)
+        wid = rng.choice(ch.n_wires, size=12, replace=False).astype(np.int32)
+        hits = o.hits_of(wid, np.full(12, 0.3))
+        T = ch.tan_tau[wid]
+        px, py = ch.x0[wid] + z_ref * ch.sin_phi_s[wid] * T, ch.y0[wid] - z_ref * ch.cos_phi_s[wid] * T
+        for k in (0, 5, 11):
+            c = np.array([px[k] + 21.0, py[k] - 17.0])                      # a circle through wire point k
+            R = float(np.hypot(px[k] - c[0], py[k] - c[1]))
+            others = np.abs(np.hypot(px - c[0], py - c[1]) - R)
+            others[k] = np.inf
+            assert others.min() > 1e-6
+            idx, xy = o.move_ref_paper(wires, hits, None, p, _fit(c[0], c[1], R))
+            assert idx == k and np.allclose(xy, (px[k], py[k]), rtol=0, atol=1e-12)
+            if z_ref == 0.0:
+                assert xy[0] == ch.x0[wid[k]] and xy[1] == ch.y0[wid[k]]     # no arithmetic at all in the plane z = 0
+            else:
+                assert abs(xy[0] - ch.x0[wid[k]]) + abs(xy[1] - ch.y0[wid[k]]) > 0.5
+            # masked out: the runner-up among the selected hits
+            mask = np.ones(12, np.uint8)
+            mask[k] = 0
+            idx2, xy2 = o.move_ref_paper(wires, hits, mask, p, _fit(c[0], c[1], R))
+            assert idx2 == int(np.argmin(others)) and np.allclose(xy2, (px[idx2], py[idx2]), atol=1e-12)
+        # the same wire twice: the first of the two
+        hits2 = o.hits_of(np.array([wid[3], wid[7], wid[3]], np.int32), np.full(3, 0.1))
+        idx, _ = o.move_ref_paper(wires, hits2, None, p, _fit(px[3] + 10.0, py[3], 10.0))
+        assert idx == 0
+        # nothing selected: the point stays
+        idx, xy = o.move_ref_paper(wires, hits, np.zeros(12, np.uint8), p, _fit(0.0, 0.0, 30.0))
+        assert idx == -1 and tuple(xy) == (0.3, -0.2)
+
+
+def test_f2d_truth_voxel_keeps_every_hit_for_any_reference_point_and_emission_point():
+    """What makes the update legitimate: the residual does not care where the reference point
+    is, as long as z0 is read as "z where the helix is closest to it".  Tracks emitted at the origin, at (5, 0) cm and at
+    (0, 5) cm; reference point (0, 0), then the point orc_move_ref_paper picks for the generated circle: the +-0.5 mm
+    voxel around (xc, yc, R, z0 of that reference point) receives every noise-free hit (tol = 0) in the accumulator of
+    the true sign of lambda - and with z0 NOT re-expressed for the new point it loses hits."""
+    ch = g.chamber_paper()
+    wires = o.wires_of(ch)
+    hw = np.array([0.05, 0.05, 0.05, 0.5])
+    lost = tot = 0
+    for vertex in ((0.0, 0.0), (5.0, 0.0), (0.0, 5.0)):
+        for seed in range(4):
+            ev = g.make_event_paper(ch, 40 + seed, vertex=vertex)
+            t = ev.track
+            hits = o.hits_of(ev.wire, ev.drift)
+            good = 0 if t.lam >= 0 else 1
+            p0 = o.make_params(0.0, flags=8)
+            idx, xy = o.move_ref_paper(wires, hits, None, p0, _fit(t.xc, t.yc, t.R))
+            assert idx >= 0
+            refs = [(0.0, 0.0), (float(xy[0]), float(xy[1])), (-3.0, 2.0)]
+            for xr, yr in refs:
+                p = o.make_params(0.0, x_ref=xr, y_ref=yr, flags=8)
+                c = np.array([t.xc, t.yc, t.R, t.z0_at(xr, yr, unwrap=True)])
+                v = o.vote_paper(wires, hits, p, g.PAPER_P, c - hw, c + hw, (1, 1, 1, 1))
+                assert v[good, 0] == ev.n_hits, (vertex, seed, (xr, yr), v[:, 0], ev.n_hits)
+            # the old z0 with the new reference point is a different helix
+            xr, yr = refs[1]
+            p = o.make_params(0.0, x_ref=xr, y_ref=yr, flags=8)
+            c = np.array([t.xc, t.yc, t.R, t.z0_at(0.0, 0.0, unwrap=True)])
+            v = o.vote_paper(wires, hits, p, g.PAPER_P, c - hw, c + hw, (1, 1, 1, 1))
+            lost += ev.n_hits - int(v[good, 0])
+            tot += ev.n_hits
+    assert lost > 0.5 * tot
+
+
+def test_f2d_transport_of_z0_between_reference_points():
+    """z0 re-expressed for a new reference point (orc_transport_z0) against the generator's own helix: the z of the
+    generated track where it is closest to the new point (eventgen.Track.z0_at: eq. (1d)'s phi0 by atan2 of the point
+    itself, a different route from the oracle's cross/dot form).  Both angle conventions, emission at and off the axis."""
+    ch = g.chamber_paper()
+    rng = np.random.default_rng(12)
+    for vertex in ((0.0, 0.0), (5.0, 0.0), (0.0, 5.0)):
+        for seed in range(6):
+            ev = g.make_event_paper(ch, 60 + seed, vertex=vertex)
+            t = ev.track
+            # reference points on the travelled arc (wire points of hits) for the unwrapped convention ...
+            pts = [(float(ch.x0[w]), float(ch.y0[w])) for w in ev.wire[:: max(1, ev.n_hits // 6)]]
+            for unwrap, flags in ((True, 8), (False, 0)):
+                p = o.make_params(0.0, flags=flags)
+                a = pts[0]
+                for b_ in pts[1:] + [(0.0, 0.0)]:
+                    if not unwrap:
+                        # ... the principal-value convention needs the two points within half a turn of each other
+                        b_ = (a[0] + rng.uniform(-3, 3), a[1] + rng.uniform(-3, 3))
+                    f = _fit(t.xc, t.yc, t.R)
+                    f["value"][3] = t.z0_at(a[0], a[1], unwrap=unwrap)
+                    f["lam"], f["x_ref"], f["y_ref"] = t.lam, a[0], a[1]
+                    got = o.transport_z0(p, f, b_[0], b_[1])
+                    want = t.z0_at(b_[0], b_[1], unwrap=unwrap)
+                    if not unwrap:
+                        # same branch as the start point: compare modulo one turn of z
+                        turn = 2.0 * np.pi * t.R * t.lam
+                        want = want + turn * round((got - want) / turn)
+                    assert abs(got - want) < 1e-9, (vertex, seed, unwrap, a, b_, got, want)
