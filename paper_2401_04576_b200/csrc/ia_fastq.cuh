@@ -104,6 +104,14 @@ template <class T> IA_DEV void q_add(Iv<T> a0, Iv<T> a1, Iv<T> b0, Iv<T> b1, Iv<
   o1.lo = V::add_dn(a1.lo, b1.lo); o1.hi = V::add_up(a1.hi, b1.hi);
 }
 
+// largest magnitude among the four endpoints of e (both drift signs), read off the sign-magnitude bit patterns
+template <class T> struct EMag;
+template <> struct EMag<double> { static constexpr int quarter = 0x3fd00000, sixteenth = 0x3fb00000; };
+template <> struct EMag<float> { static constexpr int quarter = 0x3e800000, sixteenth = 0x3d800000; };
+template <class T> IA_DEV int e_mag(const Iv<T> (&e)[2]) {
+  return max(__vimax3_s32(hiw(e[0].lo) & 0x7fffffff, hiw(e[0].hi) & 0x7fffffff, hiw(e[1].lo) & 0x7fffffff), hiw(e[1].hi) & 0x7fffffff);
+}
+
 // sin and cos over e0, e1 inside [-1/4, 1/4] (trig_small of ia_fast.cuh, eight Horner chains abreast)
 // The coefficients sit in constant memory: a DFMA takes c[bank][offset] as an operand directly, whereas literals are
 // rebuilt in uniform registers (two UMOV each) on every evaluation - there are not enough of them to keep 11 doubles.
@@ -122,15 +130,25 @@ template <> struct TrigC<float> {
   static IA_DEV float s(int k) { const float c[NS] = {-1.9841270e-04f, 8.3333338e-03f, -1.6666667e-01f}; return c[k]; }
   static IA_DEV float c(int k) { const float d[NC] = {2.4801588e-05f, -1.3888889e-03f, 4.1666668e-02f, -0.5f}; return d[k]; }
 };
-template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2], Iv<T> (&ce)[2]) {
+// short (warp-uniform, double only): every |e| < 2^-4 - the leading coefficients 1/11! (sin) and 1/12!, 1/10! (cos) are
+// then below 2^-60 relative (x^10/11! < 2.3e-20; x^10/10! < 2.5e-19 against cos > 0.99) and their three Horner steps
+// per point are skipped: 12 FP64 instructions per evaluation.  Same bound as the long form (below 1 ulp, inside the pad).
+template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2], Iv<T> (&ce)[2], bool short_poly = false) {
   using V = VR<T>;
   using C = TrigC<T>;
   const T x[4] = {e[0].lo, e[0].hi, e[1].lo, e[1].hi};
   T s[4], xs[4], qs[4], qc[4], sn[4], cs[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) s[i] = V::mul_rn(x[i], x[i]);
+  if (sizeof(T) == 8 && short_poly) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::s(0), s[i], C::s(1)); qc[i] = V::fma_rn(C::c(0), s[i], C::c(1)); }
+    for (int i = 0; i < 4; ++i) { qs[i] = C::s(1); qc[i] = C::c(2); }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::s(0), s[i], C::s(1)); qc[i] = V::fma_rn(C::c(0), s[i], C::c(1)); }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) qc[i] = V::fma_rn(qc[i], s[i], C::c(2));
+  }
 #pragma unroll
   for (int i = 0; i < 4; ++i) xs[i] = V::mul_rn(x[i], s[i]);
 #pragma unroll
@@ -138,7 +156,7 @@ template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2],
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       if (k < C::NS) qs[i] = V::fma_rn(qs[i], s[i], C::s(k));
-      qc[i] = V::fma_rn(qc[i], s[i], C::c(k));
+      if (k > 2) qc[i] = V::fma_rn(qc[i], s[i], C::c(k));
     }
   }
 #pragma unroll
@@ -238,12 +256,13 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
   q_fma<QKind<SS>::add>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);                // (t1 - t2) + t3
   q_fma<QK_ADD_P>(h.T2hiQm, h.T2hiQm, Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
-  const bool small = abs_lt_quarter(e[0].lo) && abs_lt_quarter(e[0].hi) && abs_lt_quarter(e[1].lo) && abs_lt_quarter(e[1].hi);
+  const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
+  const bool small = emag < EMag<T>::quarter;
   // S5
   Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
   if (__all_sync(0xffffffffu, small)) {
     Iv<T> ce[2];
-    q_trig_small(e, se, ce);
+    q_trig_small(e, se, ce, __all_sync(0xffffffffu, emag < EMag<T>::sixteenth));
     q_mulpos<SS>(ce[0], ce[1], SS < 0 ? ineg(h.sA[va]) : h.sA[va], sce[0], sce[1]);
     q_mulpos<SC>(ce[0], ce[1], h.cA, cce[0], cce[1]);
   } else {
@@ -360,13 +379,14 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   else if (ss < 0) q_fma<QK_SUB_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
   else q_fma<QK_ADD_U>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
   q_fma<QK_ADD_P>(h.T2hiQm, h.T2hiQm, Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
-  const bool small = abs_lt_quarter(e[0].lo) && abs_lt_quarter(e[0].hi) && abs_lt_quarter(e[1].lo) && abs_lt_quarter(e[1].hi);
+  const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
+  const bool small = emag < EMag<T>::quarter;
   // S5
   Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
   Iv<T> sa[2], ca[2], sinP[2], cosP[2];
   if (__all_sync(0xffffffffu, small)) {
     Iv<T> ce[2];
-    q_trig_small(e, se, ce);
+    q_trig_small(e, se, ce, __all_sync(0xffffffffu, emag < EMag<T>::sixteenth));
     if (ss != 0) {
       q_mulpos<1>(ce[0], ce[1], sAabs, sce[0], sce[1]);
       q_mulpos<1>(ce[0], ce[1], h.cA, cce[0], cce[1]);
