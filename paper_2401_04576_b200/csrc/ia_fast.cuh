@@ -412,9 +412,11 @@ template <class T> struct __align__(16) HitF {
   Iv<T> sA[2], dphi[2];            // index a = 1 for warps whose lambda was negated
   Iv<T> sA2T[2];                   // 2T s_Ax
   Iv<T> sA2[2];                    // 2 s_Ax (exact)
-  T twoT;                          // 2 |tan tau| (exact)
   MR<T> sAm[2], s2m[2];
   Iv<T> iQ, iR, c2, s2[2];         // interval forms, general fallback only
+  // scalars after the pairs: every Iv / MR above sits on a 16-byte (8-byte in float) boundary, which the vector
+  // ld.shared of HitLds (ia_fastq.cuh) needs
+  T twoT;                          // 2 |tan tau| (exact)
   T Tabs;                          // |tan tau|
   T Dlo, Dhi;
   T DloP, DhiP;                    // D+ padded outward by 2^-50 (2^-21): absorbs the error of rsqrt_near

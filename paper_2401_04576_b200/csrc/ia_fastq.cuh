@@ -14,6 +14,8 @@
 // The arithmetic is that of ia_fast.cuh (fused forms, same DAG, same association order): only the
 // instruction order differs.
 #pragma once
+#include <cstddef>
+
 #include "ia_fast.cuh"
 
 namespace ia {
@@ -186,7 +188,7 @@ template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2],
 // |delta| = D+ / sqrt(u2) for both signs: four 1/sqrt chains abreast (Dir<double>::rsqrt_near, same bound)
 template <class T> struct QDir;
 template <> struct QDir<double> {
-  template <class H> static IA_DEV void d_over_sqrt(const H& h, const Iv<double> (&u2)[2], Iv<double> (&dq)[2]) {
+  static IA_DEV void d_over_sqrt(double DloP, double DhiP, const Iv<double> (&u2)[2], Iv<double> (&dq)[2]) {
     using V = VR<double>;
     const double x[4] = {u2[0].hi, u2[0].lo, u2[1].hi, u2[1].lo};
     double y0[4], t[4], r[4], pp[4], yr[4], y[4];
@@ -200,8 +202,8 @@ template <> struct QDir<double> {
     for (int i = 0; i < 4; ++i) { pp[i] = V::fma_rn(0.375, r[i], 0.5); yr[i] = V::mul_rn(y0[i], r[i]); }
 #pragma unroll
     for (int i = 0; i < 4; ++i) y[i] = V::fma_rn(yr[i], pp[i], y0[i]);
-    dq[0].lo = V::mul_dn(h.DloP, y[0]); dq[0].hi = V::mul_up(h.DhiP, y[1]);
-    dq[1].lo = V::mul_dn(h.DloP, y[2]); dq[1].hi = V::mul_up(h.DhiP, y[3]);
+    dq[0].lo = V::mul_dn(DloP, y[0]); dq[0].hi = V::mul_up(DhiP, y[1]);
+    dq[1].lo = V::mul_dn(DloP, y[2]); dq[1].hi = V::mul_up(DhiP, y[3]);
   }
 };
 template <> struct QDir<float> {
@@ -209,7 +211,7 @@ template <> struct QDir<float> {
   // (result within 2^-23 of 1/sqrt), D+ padded outward by the relative 2^-21 of the float elementary pads.
   // Replaces __fdiv_rd(D, __fsqrt_ru(u2)): two library calls with slow paths per endpoint (4 CALL, 17 BSSY/BSYNC
   // per evaluation in the ncu source page of round 1).
-  template <class H> static IA_DEV void d_over_sqrt(const H& h, const Iv<float> (&u2)[2], Iv<float> (&dq)[2]) {
+  static IA_DEV void d_over_sqrt(float DloP, float DhiP, const Iv<float> (&u2)[2], Iv<float> (&dq)[2]) {
     using V = VR<float>;
     const float x[4] = {u2[0].hi, u2[0].lo, u2[1].hi, u2[1].lo};
     float y0[4], t[4], r[4], pp[4], yr[4], y[4];
@@ -223,20 +225,92 @@ template <> struct QDir<float> {
     for (int i = 0; i < 4; ++i) { pp[i] = V::fma_rn(0.375f, r[i], 0.5f); yr[i] = V::mul_rn(y0[i], r[i]); }
 #pragma unroll
     for (int i = 0; i < 4; ++i) y[i] = V::fma_rn(yr[i], pp[i], y0[i]);
-    dq[0].lo = V::mul_dn(h.DloP, y[0]); dq[0].hi = V::mul_up(h.DhiP, y[1]);
-    dq[1].lo = V::mul_dn(h.DloP, y[2]); dq[1].hi = V::mul_up(h.DhiP, y[3]);
+    dq[0].lo = V::mul_dn(DloP, y[0]); dq[0].hi = V::mul_up(DhiP, y[1]);
+    dq[1].lo = V::mul_dn(DloP, y[2]); dq[1].hi = V::mul_up(DhiP, y[3]);
   }
 };
 
+// ---- two ways to read the per-(block, hit) record inside pass_vote_q ---------------------------------------------
+// HitDirect: plain member access (diagnostics, records in local memory).  HitLds: ld.shared from a 32-bit shared-space
+// address held in a register - the compiler otherwise rebuilds the record's address in the uniform datapath for every
+// group of loads (S2UR SR_CgaCtaId, UMOV, ULEA, UIADD3: 19 instructions per evaluation in the round-2 profile), and an
+// instruction that is not an FP64 instruction costs this kernel almost a full issue cycle.  The loads are plain (not
+// volatile) asm: the record is read-only after the block's barrier, and the address they depend on is made opaque AFTER
+// that barrier (hit_address), so none of them can move above it.
+template <class T> struct HitDirect {
+  const HitF<T>& r;
+  IA_DEV T Tabs() const { return r.Tabs; }
+  IA_DEV T DloP() const { return r.DloP; }
+  IA_DEV T DhiP() const { return r.DhiP; }
+  IA_DEV T band() const { return r.band; }
+  IA_DEV int c2cls() const { return r.c2cls; }
+  IA_DEV Iv<T> Q() const { return r.Q; }
+  IA_DEV Iv<T> cA() const { return r.cA; }
+  IA_DEV Iv<T> T2() const { return r.T2; }
+  IA_DEV MR<T> cAm() const { return r.cAm; }
+  IA_DEV MR<T> iRm() const { return r.iRm; }
+  IA_DEV MR<T> TiQm() const { return r.TiQm; }
+  IA_DEV MR<T> T2hiQm() const { return r.T2hiQm; }
+  IA_DEV MR<T> cA2Tm() const { return r.cA2Tm; }
+  IA_DEV Iv<T> sA(int va) const { return r.sA[va]; }
+  IA_DEV Iv<T> dphi(int va) const { return r.dphi[va]; }
+  IA_DEV Iv<T> sA2(int va) const { return r.sA2[va]; }
+  IA_DEV MR<T> sAm(int va) const { return r.sAm[va]; }
+  IA_DEV MR<T> s2m(int va) const { return r.s2m[va]; }
+};
+template <class T> struct LdsOp;
+template <> struct LdsOp<double> {
+  static IA_DEV void v2(unsigned a, double& x, double& y) { asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a)); }
+  static IA_DEV double s(unsigned a) { double x; asm("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(a)); return x; }
+};
+template <> struct LdsOp<float> {
+  static IA_DEV void v2(unsigned a, float& x, float& y) { asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(x), "=f"(y) : "r"(a)); }
+  static IA_DEV float s(unsigned a) { float x; asm("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(a)); return x; }
+};
+#define IA_HOFF(field) unsigned(offsetof(HitF<T>, field))
+static_assert(offsetof(HitF<double>, sAm) % 16 == 0 && offsetof(HitF<double>, s2m) % 16 == 0 && offsetof(HitF<double>, sA2) % 16 == 0 &&
+              offsetof(HitF<double>, cA2Tm) % 16 == 0 && sizeof(HitF<double>) % 16 == 0, "HitF<double>: pairs must be 16-byte aligned");
+static_assert(offsetof(HitF<float>, sAm) % 8 == 0 && offsetof(HitF<float>, s2m) % 8 == 0 && sizeof(HitF<float>) % 16 == 0,
+              "HitF<float>: pairs must be 8-byte aligned");
+template <class T> struct HitLds {
+  unsigned a;            // shared-space address of the record
+  IA_DEV Iv<T> iv(unsigned off) const { Iv<T> v; LdsOp<T>::v2(a + off, v.lo, v.hi); return v; }
+  IA_DEV MR<T> mr(unsigned off) const { MR<T> v; LdsOp<T>::v2(a + off, v.m, v.r); return v; }
+  IA_DEV T Tabs() const { return LdsOp<T>::s(a + IA_HOFF(Tabs)); }
+  IA_DEV T DloP() const { return LdsOp<T>::s(a + IA_HOFF(DloP)); }
+  IA_DEV T DhiP() const { return LdsOp<T>::s(a + IA_HOFF(DhiP)); }
+  IA_DEV T band() const { return LdsOp<T>::s(a + IA_HOFF(band)); }
+  IA_DEV int c2cls() const { int x; asm("ld.shared.s32 %0, [%1];" : "=r"(x) : "r"(a + IA_HOFF(c2cls))); return x; }
+  IA_DEV Iv<T> Q() const { return iv(IA_HOFF(Q)); }
+  IA_DEV Iv<T> cA() const { return iv(IA_HOFF(cA)); }
+  IA_DEV Iv<T> T2() const { return iv(IA_HOFF(T2)); }
+  IA_DEV MR<T> cAm() const { return mr(IA_HOFF(cAm)); }
+  IA_DEV MR<T> iRm() const { return mr(IA_HOFF(iRm)); }
+  IA_DEV MR<T> TiQm() const { return mr(IA_HOFF(TiQm)); }
+  IA_DEV MR<T> T2hiQm() const { return mr(IA_HOFF(T2hiQm)); }
+  IA_DEV MR<T> cA2Tm() const { return mr(IA_HOFF(cA2Tm)); }
+  IA_DEV Iv<T> sA(int va) const { return iv(IA_HOFF(sA) + va * unsigned(sizeof(Iv<T>))); }
+  IA_DEV Iv<T> dphi(int va) const { return iv(IA_HOFF(dphi) + va * unsigned(sizeof(Iv<T>))); }
+  IA_DEV Iv<T> sA2(int va) const { return iv(IA_HOFF(sA2) + va * unsigned(sizeof(Iv<T>))); }
+  IA_DEV MR<T> sAm(int va) const { return mr(IA_HOFF(sAm) + va * unsigned(sizeof(MR<T>))); }
+  IA_DEV MR<T> s2m(int va) const { return mr(IA_HOFF(s2m) + va * unsigned(sizeof(MR<T>))); }
+};
+// shared-space address of a record, opaque to the compiler from here on (call after the barrier that publishes the records)
+template <class T> IA_DEV unsigned hit_address(const HitF<T>* rec) {
+  unsigned a = unsigned(__cvta_generic_to_shared(rec));
+  asm volatile("" : "+r"(a));
+  return a;
+}
+
 // S4-S8 for both drift signs (index 0: D+, 1: D-) of one (cell, hit); returns 1 iff 0 is in f for either.
 // Inputs transformed as in ia_fast.cuh: L >= 0, T = h.Tabs >= 0, cA >= 0 (SS != 0) or any (SS == 0).
-template <int SS, class T>
-IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
+template <int SS, class T, class H>
+IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp, Iv<T> Zr) {
   // returns decide(): bit 0 the vote, bit 1 (float only) "too close to call in this form"
   using V = VR<T>;
-  const T Tn = h.Tabs;
+  const T Tn = h.Tabs();
   constexpr int SC = SS == 0 ? 0 : 1;                                  // class of cA inside this body
-  const MR<T> sAm = q_arg<SS>(h.sAm[va]), s2m = q_arg<SS>(h.s2m[va]);
+  const MR<T> sAm = q_arg<SS>(h.sAm(va)), s2m = q_arg<SS>(h.s2m(va));
   // S4: shared part
   Iv<T> zA, t1;
   zA.lo = V::add_dn(Zr.lo, hp.LRdphi.lo); zA.hi = V::add_up(Zr.hi, hp.LRdphi.hi);           // (A.8d)
@@ -247,15 +321,15 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   const Mag<T> gz = mag_of(zA);
   Iv<T> W[2], TY[2], in[2], zG[2], Vv[2], e[2];
   q_fma<QKind<SS>::add>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);              // lambda D cA + zA sA
-  if (h.c2cls == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
-  else if (h.c2cls == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
+  if (h.c2cls() == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
+  else if (h.c2cls() == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
   else q_fma<QK_SUB_U>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);
-  q_prod_p(h.TiQm, W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
+  q_prod_p(h.TiQm(), W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
   zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
   zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
   if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
   q_fma<QKind<SS>::add>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);                // (t1 - t2) + t3
-  q_fma<QK_ADD_P>(h.T2hiQm, h.T2hiQm, Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
+  q_fma<QK_ADD_P>(h.T2hiQm(), h.T2hiQm(), Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
   const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
   const bool small = emag < EMag<T>::quarter;
   // S5
@@ -263,19 +337,19 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   if (__all_sync(0xffffffffu, small)) {
     Iv<T> ce[2];
     q_trig_small(e, se, ce, __all_sync(0xffffffffu, emag < EMag<T>::sixteenth));
-    q_mulpos<SS>(ce[0], ce[1], SS < 0 ? ineg(h.sA[va]) : h.sA[va], sce[0], sce[1]);
-    q_mulpos<SC>(ce[0], ce[1], h.cA, cce[0], cce[1]);
+    q_mulpos<SS>(ce[0], ce[1], SS < 0 ? ineg(h.sA(va)) : h.sA(va), sce[0], sce[1]);
+    q_mulpos<SC>(ce[0], ce[1], h.cA(), cce[0], cce[1]);
   } else {
-    const Trig3<T> g0 = trig_general(e[0], h.sA[va], h.cA), g1 = trig_general(e[1], h.sA[va], h.cA);
+    const Trig3<T> g0 = trig_general(e[0], h.sA(va), h.cA()), g1 = trig_general(e[1], h.sA(va), h.cA());
     se[0] = g0.se; cce[0] = g0.cce; sce[0] = SS < 0 ? ineg(g0.sce) : g0.sce;
     se[1] = g1.se; cce[1] = g1.cce; sce[1] = SS < 0 ? ineg(g1.sce) : g1.sce;
   }
   Iv<T> sa[2], ca[2], sinP[2], cosP[2];
-  if (SS < 0) q_fma<QKind<SC>::add>(h.cAm, h.cAm, se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
-  else q_fma<QKind<SC>::add>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
+  if (SS < 0) q_fma<QKind<SC>::add>(h.cAm(), h.cAm(), se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
+  else q_fma<QKind<SC>::add>(h.cAm(), h.cAm(), se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
   q_fma<QKind<SS>::sub>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
-  q_prod_p(h.iRm, sa[0], sa[1], sinP[0], sinP[1]);
-  q_prod_p(h.iRm, ca[0], ca[1], cosP[0], cosP[1]);
+  q_prod_p(h.iRm(), sa[0], sa[1], sinP[0], sinP[1]);
+  q_prod_p(h.iRm(), ca[0], ca[1], cosP[0], cosP[1]);
   // the common case cos Phi >= 0 is decided per warp (cos_nonneg in ia_fast.cuh)
   const bool plain = __all_sync(0xffffffffu, cos_nonneg(cosP));
 #pragma unroll
@@ -287,24 +361,24 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
   if (plain) {
     const T a0 = V::mul_dn(cosP[0].lo, cosP[0].lo), b0 = V::mul_up(cosP[0].hi, cosP[0].hi);
     const T a1 = V::mul_dn(cosP[1].lo, cosP[1].lo), b1 = V::mul_up(cosP[1].hi, cosP[1].hi);
-    u2[0].lo = V::fma_dn(h.T2.lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2.lo, a1, u2[1].lo);
-    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+    u2[0].lo = V::fma_dn(h.T2().lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2().lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2().hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2().hi, b1, u2[1].hi);
   } else {
     const Mag<T> g0 = mag_of(cosP[0]), g1 = mag_of(cosP[1]);
     const T a0 = V::mul_dn(g0.mnn, g0.mnn), b0 = V::mul_up(g0.mag, g0.mag), a1 = V::mul_dn(g1.mnn, g1.mnn), b1 = V::mul_up(g1.mag, g1.mag);
-    const T l0 = V::fma_dn(h.T2.lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2.lo, a1, u2[1].lo);
-    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+    const T l0 = V::fma_dn(h.T2().lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2().lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2().hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2().hi, b1, u2[1].hi);
     u2[0].lo = g0.straddle ? u2[0].lo : l0; u2[1].lo = g1.straddle ? u2[1].lo : l1;
   }
-  QDir<T>::d_over_sqrt(h, u2, dq);                                     // |delta| = D+ / u_d
+  QDir<T>::d_over_sqrt(h.DloP(), h.DhiP(), u2, dq);                                     // |delta| = D+ / u_d
   // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (D+), -dq (D-)
   Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
-  q_add(e[0], e[1], h.dphi[va], h.dphi[va], de[0], de[1]);
+  q_add(e[0], e[1], h.dphi(va), h.dphi(va), de[0], de[1]);
   q_fma<QK_ADD_P>(p.LRm, p.LRm, de[0], de[1], Zr, Zr, zz[0], zz[1]);
   Tdq[0].lo = V::mul_dn(Tn, dq[0].lo); Tdq[0].hi = V::mul_up(Tn, dq[0].hi);                 // |T delta|
   Tdq[1].lo = V::mul_dn(Tn, dq[1].lo); Tdq[1].hi = V::mul_up(Tn, dq[1].hi);
   q_mulpos<1>(Tdq[0], Tdq[1], p.L, TLq[0], TLq[1]);                                         // |T lambda delta|
-  q_mulpos<SS>(TLq[0], TLq[1], SS < 0 ? ineg(h.sA2[va]) : h.sA2[va], qs[0], qs[1]);         // sigma 2T |lambda delta| sA
+  q_mulpos<SS>(TLq[0], TLq[1], SS < 0 ? ineg(h.sA2(va)) : h.sA2(va), qs[0], qs[1]);         // sigma 2T |lambda delta| sA
   if (plain) {                                                           // cos Phi >= 0: the partner of .lo is .lo, of .hi is .hi
     z[0].lo = V::fma_dn(-Tdq[0].hi, cosP[0].hi, zz[0].lo); z[0].hi = V::fma_up(-Tdq[0].lo, cosP[0].lo, zz[0].hi);
     z[1].lo = V::fma_dn(Tdq[1].lo, cosP[1].lo, zz[1].lo); z[1].hi = V::fma_up(Tdq[1].hi, cosP[1].hi, zz[1].hi);
@@ -315,8 +389,8 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
     z[1].lo = V::fma_dn(pl1, cosP[1].lo, zz[1].lo); z[1].hi = V::fma_up(ph1, cosP[1].hi, zz[1].hi);
   }
   // ct = 2T c^tau (A.7b):  D+: 2T cA z - sigma qs,  D-: 2T cA z + sigma qs
-  if (SS < 0) q_fma<QKind<SC>::add>(h.cA2Tm, h.cA2Tm, z[0], z[1], qs[0], ineg(qs[1]), ct[0], ct[1]);
-  else q_fma<QKind<SC>::add>(h.cA2Tm, h.cA2Tm, z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
+  if (SS < 0) q_fma<QKind<SC>::add>(h.cA2Tm(), h.cA2Tm(), z[0], z[1], qs[0], ineg(qs[1]), ct[0], ct[1]);
+  else q_fma<QKind<SC>::add>(h.cA2Tm(), h.cA2Tm(), z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
   Rd1[0].lo = V::add_dn(p.R.lo, dq[0].lo); Rd1[0].hi = V::add_up(p.R.hi, dq[0].hi);
   Rd1[1].lo = V::add_dn(p.R.lo, -dq[1].hi); Rd1[1].hi = V::add_up(p.R.hi, -dq[1].lo);
   Tz[0].lo = V::mul_dn(Tn, z[0].lo); Tz[0].hi = V::mul_up(Tn, z[0].hi);
@@ -334,9 +408,9 @@ IA_DEV unsigned pass_vote_q(const HitF<T>& h, int va, const Pass2<T>& pc, const 
 #pragma unroll
   for (int s = 0; s < 2; ++s) { r2[s].lo = V::fma_dn(-TLq[s].hi, TLq[s].hi, r2[s].lo); r2[s].hi = V::fma_up(-TLq[s].lo, TLq[s].lo, r2[s].hi); }
 #pragma unroll
-  for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q.lo, -r2[s].hi); f[s].hi = V::add_up(h.Q.hi, -r2[s].lo); }
+  for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q().lo, -r2[s].hi); f[s].hi = V::add_up(h.Q().hi, -r2[s].lo); }
   // inputs are finite and u_d^2 >= 0.49, so f is never NaN here; f.hi is a round-up sum, never -0
-  return decide(f, h.band);
+  return decide(f, h.band());
 }
 
 // ---- one body for all three sign classes ----------------------------------------------------------
@@ -431,7 +505,7 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
     u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
     u2[0].lo = g0.straddle ? u2[0].lo : l0; u2[1].lo = g1.straddle ? u2[1].lo : l1;
   }
-  QDir<T>::d_over_sqrt(h, u2, dq);                                     // |delta| = D+ / u_d
+  QDir<T>::d_over_sqrt(h.DloP, h.DhiP, u2, dq);                                     // |delta| = D+ / u_d
   // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (D+), -dq (D-)
   Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
   q_add(e[0], e[1], h.dphi[va], h.dphi[va], de[0], de[1]);

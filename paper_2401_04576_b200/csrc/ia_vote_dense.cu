@@ -108,13 +108,14 @@ template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>
 // one hit, one thread: both drift signs over the thread's z0 cells; returns the vote mask (bit i = z0 cell i)
 // (float: bit FAST_ZT + i set = cell i is too close to call in this form, see Filter in ia_fast.cuh)
 template <int SS, class T>
-IA_DEV unsigned fast_hit(const HitF<T>& h, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
+IA_DEV unsigned fast_hit(const HitF<T>& h, unsigned h_addr, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
   const Pass2<T> pc2 = pass_prepare2(h, p, hp);
+  const HitLds<T> hl = {h_addr};
   unsigned bits = 0;
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) {
-    const unsigned r = pass_vote_q<SS>(h, va, pc2, p, hp, zt[i]);
+    const unsigned r = pass_vote_q<SS, T>(hl, va, pc2, p, hp, zt[i]);
     bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : r << i;
   }
   return bits;
@@ -215,6 +216,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     ztab->z[1][threadIdx.x] = ineg(Zr);
   }
   __syncthreads();
+  const unsigned sh_addr = hit_address(sh);             // of record 0 (sh is already shifted by -h_begin in the SPLIT case)
   // pair enumeration: lambda index within its half fastest, then R, then the half (so that a warp's
   // lambda cells share a sign and its stores run along lambda)
   const int n_pairs = nR * nL;
@@ -255,9 +257,9 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     if (kind != HIT_GENERAL && warp_fast) {
       unsigned bits;
       if (RT) bits = fast_hit_rt<T>(hf, kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
-      else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, va, pr, zt, nz_tile);
-      else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, va, pr, zt, nz_tile);
-      else bits = fast_hit<0, T>(hf, va, pr, zt, nz_tile);
+      else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
+      else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
+      else bits = fast_hit<0, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
       bits = settle(bits, hf, va, R, pr.L, zt);
 #pragma unroll
       for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += spread8((bits >> (8 * j)) & 0xffu);
