@@ -423,11 +423,11 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
 // dependent quads are short uniform switches.  Same arithmetic as pass_vote_q<SS> for every class.
 IA_DEV int opaque_i(int x) { asm volatile("" : "+r"(x)); return x; }
 
-template <class T>
-IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp,
+template <class T, class H>
+IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp,
                              Iv<T> Zr, MR<T> sAm, MR<T> s2m, Iv<T> sAabs, Iv<T> sA2abs, Iv<T>* fout = nullptr) {
   using V = VR<T>;
-  const T Tn = h.Tabs;
+  const T Tn = h.Tabs();
   // sAm, s2m: negated for the class s_Ax <= 0; sAabs, sA2abs: s_Ax and 2 s_Ax, negated for that class
   const int ss = opaque_i(ss_in);            // keeps the compiler from cloning the loop per class
   // S4: shared part
@@ -442,17 +442,17 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   if (ss > 0) q_fma<QK_ADD_P>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);        // lambda D cA + zA sA
   else if (ss < 0) q_fma<QK_SUB_P>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);
   else q_fma<QK_ADD_U>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);
-  if (h.c2cls == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
-  else if (h.c2cls == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
+  if (h.c2cls() == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
+  else if (h.c2cls() == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
   else q_fma<QK_SUB_U>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);
-  q_prod_p(h.TiQm, W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
+  q_prod_p(h.TiQm(), W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
   zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
   zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
   if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
   if (ss > 0) q_fma<QK_ADD_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);          // (t1 - t2) + t3
   else if (ss < 0) q_fma<QK_SUB_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
   else q_fma<QK_ADD_U>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
-  q_fma<QK_ADD_P>(h.T2hiQm, h.T2hiQm, Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
+  q_fma<QK_ADD_P>(h.T2hiQm(), h.T2hiQm(), Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
   const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
   const bool small = emag < EMag<T>::quarter;
   // S5
@@ -463,28 +463,28 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
     q_trig_small(e, se, ce, __all_sync(0xffffffffu, emag < EMag<T>::sixteenth));
     if (ss != 0) {
       q_mulpos<1>(ce[0], ce[1], sAabs, sce[0], sce[1]);
-      q_mulpos<1>(ce[0], ce[1], h.cA, cce[0], cce[1]);
+      q_mulpos<1>(ce[0], ce[1], h.cA(), cce[0], cce[1]);
     } else {
       q_mulpos<0>(ce[0], ce[1], sAabs, sce[0], sce[1]);
-      q_mulpos<0>(ce[0], ce[1], h.cA, cce[0], cce[1]);
+      q_mulpos<0>(ce[0], ce[1], h.cA(), cce[0], cce[1]);
     }
   } else {
-    const Trig3<T> g0 = trig_general(e[0], h.sA[va], h.cA), g1 = trig_general(e[1], h.sA[va], h.cA);
+    const Trig3<T> g0 = trig_general(e[0], h.sA(va), h.cA()), g1 = trig_general(e[1], h.sA(va), h.cA());
     se[0] = g0.se; cce[0] = g0.cce; sce[0] = ss < 0 ? ineg(g0.sce) : g0.sce;
     se[1] = g1.se; cce[1] = g1.cce; sce[1] = ss < 0 ? ineg(g1.sce) : g1.sce;
   }
   if (ss > 0) {
-    q_fma<QK_ADD_P>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
+    q_fma<QK_ADD_P>(h.cAm(), h.cAm(), se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
     q_fma<QK_SUB_P>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
   } else if (ss < 0) {
-    q_fma<QK_ADD_P>(h.cAm, h.cAm, se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
+    q_fma<QK_ADD_P>(h.cAm(), h.cAm(), se[0], se[1], ineg(sce[0]), ineg(sce[1]), sa[0], sa[1]);
     q_fma<QK_ADD_P>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
   } else {
-    q_fma<QK_ADD_U>(h.cAm, h.cAm, se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
+    q_fma<QK_ADD_U>(h.cAm(), h.cAm(), se[0], se[1], sce[0], sce[1], sa[0], sa[1]);
     q_fma<QK_SUB_U>(sAm, sAm, se[0], se[1], cce[0], cce[1], ca[0], ca[1]);
   }
-  q_prod_p(h.iRm, sa[0], sa[1], sinP[0], sinP[1]);
-  q_prod_p(h.iRm, ca[0], ca[1], cosP[0], cosP[1]);
+  q_prod_p(h.iRm(), sa[0], sa[1], sinP[0], sinP[1]);
+  q_prod_p(h.iRm(), ca[0], ca[1], cosP[0], cosP[1]);
   // the common case cos Phi >= 0 is decided per warp (cos_nonneg in ia_fast.cuh)
   const bool plain = __all_sync(0xffffffffu, cos_nonneg(cosP));
 #pragma unroll
@@ -496,19 +496,19 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   if (plain) {
     const T a0 = V::mul_dn(cosP[0].lo, cosP[0].lo), b0 = V::mul_up(cosP[0].hi, cosP[0].hi);
     const T a1 = V::mul_dn(cosP[1].lo, cosP[1].lo), b1 = V::mul_up(cosP[1].hi, cosP[1].hi);
-    u2[0].lo = V::fma_dn(h.T2.lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2.lo, a1, u2[1].lo);
-    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+    u2[0].lo = V::fma_dn(h.T2().lo, a0, u2[0].lo); u2[1].lo = V::fma_dn(h.T2().lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2().hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2().hi, b1, u2[1].hi);
   } else {
     const Mag<T> g0 = mag_of(cosP[0]), g1 = mag_of(cosP[1]);
     const T a0 = V::mul_dn(g0.mnn, g0.mnn), b0 = V::mul_up(g0.mag, g0.mag), a1 = V::mul_dn(g1.mnn, g1.mnn), b1 = V::mul_up(g1.mag, g1.mag);
-    const T l0 = V::fma_dn(h.T2.lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2.lo, a1, u2[1].lo);
-    u2[0].hi = V::fma_up(h.T2.hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2.hi, b1, u2[1].hi);
+    const T l0 = V::fma_dn(h.T2().lo, a0, u2[0].lo), l1 = V::fma_dn(h.T2().lo, a1, u2[1].lo);
+    u2[0].hi = V::fma_up(h.T2().hi, b0, u2[0].hi); u2[1].hi = V::fma_up(h.T2().hi, b1, u2[1].hi);
     u2[0].lo = g0.straddle ? u2[0].lo : l0; u2[1].lo = g1.straddle ? u2[1].lo : l1;
   }
-  QDir<T>::d_over_sqrt(h.DloP, h.DhiP, u2, dq);                                     // |delta| = D+ / u_d
+  QDir<T>::d_over_sqrt(h.DloP(), h.DhiP(), u2, dq);                                     // |delta| = D+ / u_d
   // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (D+), -dq (D-)
   Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
-  q_add(e[0], e[1], h.dphi[va], h.dphi[va], de[0], de[1]);
+  q_add(e[0], e[1], h.dphi(va), h.dphi(va), de[0], de[1]);
   q_fma<QK_ADD_P>(p.LRm, p.LRm, de[0], de[1], Zr, Zr, zz[0], zz[1]);
   Tdq[0].lo = V::mul_dn(Tn, dq[0].lo); Tdq[0].hi = V::mul_up(Tn, dq[0].hi);                 // |T delta|
   Tdq[1].lo = V::mul_dn(Tn, dq[1].lo); Tdq[1].hi = V::mul_up(Tn, dq[1].hi);
@@ -525,13 +525,13 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
   // qs = sigma 2T |lambda delta| sA;  ct = 2T c^tau (A.7b):  D+: 2T cA z - sigma qs,  D-: 2T cA z + sigma qs
   if (ss > 0) {
     q_mulpos<1>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
-    q_fma<QK_ADD_P>(h.cA2Tm, h.cA2Tm, z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
+    q_fma<QK_ADD_P>(h.cA2Tm(), h.cA2Tm(), z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
   } else if (ss < 0) {
     q_mulpos<1>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
-    q_fma<QK_ADD_P>(h.cA2Tm, h.cA2Tm, z[0], z[1], qs[0], ineg(qs[1]), ct[0], ct[1]);
+    q_fma<QK_ADD_P>(h.cA2Tm(), h.cA2Tm(), z[0], z[1], qs[0], ineg(qs[1]), ct[0], ct[1]);
   } else {
     q_mulpos<0>(TLq[0], TLq[1], sA2abs, qs[0], qs[1]);
-    q_fma<QK_ADD_U>(h.cA2Tm, h.cA2Tm, z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
+    q_fma<QK_ADD_U>(h.cA2Tm(), h.cA2Tm(), z[0], z[1], ineg(qs[0]), qs[1], ct[0], ct[1]);
   }
   Rd1[0].lo = V::add_dn(p.R.lo, dq[0].lo); Rd1[0].hi = V::add_up(p.R.hi, dq[0].hi);
   Rd1[1].lo = V::add_dn(p.R.lo, -dq[1].hi); Rd1[1].hi = V::add_up(p.R.hi, -dq[1].lo);
@@ -550,9 +550,9 @@ IA_DEV unsigned pass_vote_qr(const HitF<T>& h, int ss_in, int va, const Pass2<T>
 #pragma unroll
   for (int s = 0; s < 2; ++s) { r2[s].lo = V::fma_dn(-TLq[s].hi, TLq[s].hi, r2[s].lo); r2[s].hi = V::fma_up(-TLq[s].lo, TLq[s].lo, r2[s].hi); }
 #pragma unroll
-  for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q.lo, -r2[s].hi); f[s].hi = V::add_up(h.Q.hi, -r2[s].lo); }
+  for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q().lo, -r2[s].hi); f[s].hi = V::add_up(h.Q().hi, -r2[s].lo); }
   if (fout) { fout[0] = f[0]; fout[1] = f[1]; }       // diagnostics (ia_residual_fast); nullptr in the vote kernels
-  return decide(f, h.band);
+  return decide(f, h.band());
 }
 
 }  // namespace ia

@@ -138,15 +138,16 @@ IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L
 
 // the same with the sign class as a run-time value (one compiled body, ia_fastq.cuh)
 template <class T>
-IA_DEV unsigned fast_hit_rt(const HitF<T>& h, int ss, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
+IA_DEV unsigned fast_hit_rt(const HitF<T>& h, unsigned h_addr, int ss, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
   const Pass2<T> pc2 = pass_prepare2(h, p, hp);
+  const HitLds<T> hl = {h_addr};
   const MR<T> sAm = ss < 0 ? mr_neg(h.sAm[va]) : h.sAm[va], s2m = ss < 0 ? mr_neg(h.s2m[va]) : h.s2m[va];
   const Iv<T> sAabs = ss < 0 ? ineg(h.sA[va]) : h.sA[va], sA2abs = ss < 0 ? ineg(h.sA2[va]) : h.sA2[va];
   unsigned bits = 0;
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) {
-    const unsigned r = pass_vote_qr(h, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
+    const unsigned r = pass_vote_qr<T>(hl, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
     bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : r << i;
   }
   return bits;
@@ -256,7 +257,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
       unsigned bits;
-      if (RT) bits = fast_hit_rt<T>(hf, kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
+      if (RT) bits = fast_hit_rt<T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
       else bits = fast_hit<0, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
@@ -367,6 +368,7 @@ vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const 
   pr.L2 = lcls != CLS_M ? mul_pp(pr.L, pr.L) : isqr(pr.L);
   unsigned v0 = 0, v1 = 0;
   const HitF<T>* myrec = rec + (r * 4 + xy) * per_split;
+  const unsigned my_addr = hit_address(myrec);          // after the barrier above
   for (int h = 0; h < nh; ++h) {
     const HitF<T>& hf = myrec[h];
     const int kind = hf.kind[va];
@@ -382,7 +384,7 @@ vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const 
       const bool allP = __all_sync(0xffffffffu, kind == HIT_FAST_P || !need);
       const bool allN = __all_sync(0xffffffffu, kind == HIT_FAST_N || !need);
       // lanes that do not need the hit (forced, skipped) run along on their record and drop the result
-      unsigned bits = fast_hit_rt<T>(hf, allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
+      unsigned bits = fast_hit_rt<T>(hf, my_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
       if (need) {
         bits = settle(bits, hf, va, R, pr.L, zt);
         v0 += bits & 1u; v1 += (bits >> 1) & 1u;
@@ -441,7 +443,7 @@ __global__ void residual_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ sta
   const Iv<T> sAabs = ss < 0 ? ineg(hf.sA[va]) : hf.sA[va], sA2abs = ss < 0 ? ineg(hf.sA2[va]) : hf.sA2[va];
   const Iv<T> Zr = isub(Z, thin(c.zref));
   Iv<T> f[2];
-  pass_vote_qr(hf, ss, va, pc2, pr, hp, hf.zflip ? ineg(Zr) : Zr, sAm, s2m, sAabs, sA2abs, f);
+  pass_vote_qr<T>(HitDirect<T>{hf}, ss, va, pc2, pr, hp, hf.zflip ? ineg(Zr) : Zr, sAm, s2m, sAabs, sA2abs, f);
   for (int s = 0; s < 2; ++s) { o[4 * s] = f[s].lo; o[4 * s + 1] = f[s].hi; o[4 * s + 2] = hf.Q.hi; o[4 * s + 3] = 0.0; }
 }
 
