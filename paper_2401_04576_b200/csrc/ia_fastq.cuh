@@ -142,23 +142,37 @@ template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2],
   T s[4], xs[4], qs[4], qc[4], sn[4], cs[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) s[i] = V::mul_rn(x[i], x[i]);
-  if (sizeof(T) == 8 && short_poly) {
+  if (sizeof(T) == 8) {
+    // both forms start with an FMA on constants (no register initialisation) and meet after the 1/7! and 1/6! steps
+    if (short_poly) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { qs[i] = C::s(1); qc[i] = C::c(2); }
+      for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::s(1), s[i], C::s(2)); qc[i] = V::fma_rn(C::c(2), s[i], C::c(3)); }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::s(0), s[i], C::s(1)); qc[i] = V::fma_rn(C::c(0), s[i], C::c(1)); }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(qs[i], s[i], C::s(2)); qc[i] = V::fma_rn(qc[i], s[i], C::c(2)); }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) qc[i] = V::fma_rn(qc[i], s[i], C::c(3));
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) xs[i] = V::mul_rn(x[i], s[i]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(qs[i], s[i], C::s(3)); qc[i] = V::fma_rn(qc[i], s[i], C::c(4)); }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(qs[i], s[i], C::s(4)); qc[i] = V::fma_rn(qc[i], s[i], C::c(5)); }
   } else {
 #pragma unroll
     for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::s(0), s[i], C::s(1)); qc[i] = V::fma_rn(C::c(0), s[i], C::c(1)); }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) qc[i] = V::fma_rn(qc[i], s[i], C::c(2));
-  }
+    for (int i = 0; i < 4; ++i) xs[i] = V::mul_rn(x[i], s[i]);
 #pragma unroll
-  for (int i = 0; i < 4; ++i) xs[i] = V::mul_rn(x[i], s[i]);
+    for (int k = 2; k < C::NC; ++k) {
 #pragma unroll
-  for (int k = 2; k < C::NC; ++k) {
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      if (k < C::NS) qs[i] = V::fma_rn(qs[i], s[i], C::s(k));
-      if (k > 2) qc[i] = V::fma_rn(qc[i], s[i], C::c(k));
+      for (int i = 0; i < 4; ++i) {
+        if (k < C::NS) qs[i] = V::fma_rn(qs[i], s[i], C::s(k));
+        qc[i] = V::fma_rn(qc[i], s[i], C::c(k));
+      }
     }
   }
 #pragma unroll
