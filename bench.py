@@ -629,6 +629,30 @@ def main():
         except Exception as exc:  # pragma: no cover
             line["roofline"]["probe_error"] = str(exc)
 
+        # ---- prefilter (ia_params.flags bit 6): the same grid with hits skipped that a crude enclosure excludes for a whole
+        # warp and z0 tile; identical accumulator (checked here on the device), NOT the brute-force evaluation the headline
+        # value and the roofline describe
+        try:
+            ctx.ia_set_params(g.TOL, flags=args.flags | 64)
+            votes_pf = torch.empty_like(votes)
+            ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes_pf)
+            torch.cuda.synchronize()
+            a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            n_pf = max(1, min(args.steps, 3))
+            for _ in range(n_pf):
+                ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes_pf)
+            c.record(stream)
+            c.synchronize()
+            ms_pf = a.elapsed_time(c) / n_pf
+            line["prefilter"] = {"flags": 64, "kernel_ms": ms_pf, "evals_per_s": evals_per_step / (ms_pf * 1e-3),
+                                 "speedup_over_brute_force": vote_ms / ms_pf,
+                                 "accumulator_identical": bool(torch.equal(votes.view(torch.int16), votes_pf.view(torch.int16))),
+                                 "note": "extension beyond north_star (default off): a (cell, hit) pair is no longer always evaluated in full"}
+            del votes_pf
+        finally:
+            ctx.ia_set_params(g.TOL, flags=args.flags)
+
         # ---- e2e: host hits in, host votes out, through ia_vote_host ------------------------------------
         host_votes = torch.empty(n_cells, dtype=torch.uint16, pin_memory=True).numpy()
         pinned_hits = torch.from_numpy(hits_host.view(np.uint8).copy()).pin_memory().numpy().view(b.HIT_DT)

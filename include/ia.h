@@ -89,7 +89,12 @@ typedef struct {
  * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; runs in the
  * general (sign-agnostic) kernels, about 4 x the arithmetic; bit 5: ia_refine / ia_refine_batch always enqueue
  * their launches one by one (default: a call repeated with identical arguments and buffers is replayed as a
- * CUDA graph from its third occurrence on); other bits must be 0. */
+ * CUDA graph from its third occurrence on); bit 6 (sign-specialised dense kernel): prefilter - before the fine
+ * evaluation of a hit a warp asks a crude enclosure of the same residual (magnitude bounds of every step of S4-S8, both
+ * drift signs, all the z0 cells of its tile at once) whether 0 can be excluded for all its cells, and skips the hit if
+ * so: the votes are identical (a wider enclosure that excludes 0 implies the finer one does, L80), the kernel no longer
+ * evaluates every (cell, hit) in full - default off: north_star's metric is the brute-force evaluation; other bits
+ * must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;

@@ -93,7 +93,10 @@ constexpr int FAST_MIN_BLOCKS = IA_FAST_MIN_BLOCKS;
 constexpr int FAST_ZT = IA_FAST_ZT;                      // 8 or 16: z0 cells per thread (vote bits + filter bits share 32 bits)
 static_assert(FAST_ZT == 8 || FAST_ZT == 16, "FAST_ZT");
 
-template <class T> struct ZTab { Iv<T> z[2][FAST_ZT]; };    // [0]: z0 - z_ref, [1]: its negation
+template <class T> struct __align__(16) ZTab {
+  Iv<T> z[2][FAST_ZT];        // [0]: z0 - z_ref, [1]: its negation
+  T zeta, _pad;               // largest |z0 - z_ref| of the tile (prefilter)
+};
 
 template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>& h, int va, Iv<T> R, Iv<T> Zeff, Iv<T> L) {
   XYInv<T> v;
@@ -169,7 +172,7 @@ IA_DEV unsigned long long spread8(unsigned bits) {
 template <class T, bool RT, bool SPLIT>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z, int zt,
-                       int per_split, uint16_t* __restrict__ votes) {
+                       int per_split, int prefilter, uint16_t* __restrict__ votes) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ZTab<T>* ztab = reinterpret_cast<ZTab<T>*>(smem_raw);
   HitF<T>* sh = reinterpret_cast<HitF<T>*>(smem_raw + sizeof(ZTab<T>));
@@ -215,6 +218,11 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     const Iv<T> Zr = isub(Z, thin(zref));
     ztab->z[0][threadIdx.x] = Zr;
     ztab->z[1][threadIdx.x] = ineg(Zr);
+    // (threads beyond nz_tile repeat the last cell, so the maximum over all FAST_ZT lanes is the tile's)
+    T zm = mx(fabs(Zr.lo), fabs(Zr.hi));
+#pragma unroll
+    for (int off = FAST_ZT / 2; off > 0; off >>= 1) zm = mx(zm, __shfl_xor_sync((1u << FAST_ZT) - 1u, zm, off));
+    if (threadIdx.x == 0) ztab->zeta = zm;
   }
   __syncthreads();
   const unsigned sh_addr = hit_address(sh);             // of record 0 (sh is already shifted by -h_begin in the SPLIT case)
@@ -256,6 +264,8 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     }
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
+      // flags bit 6: a crude enclosure over the whole z0 tile excludes this hit for every lane -> nobody votes
+      if (prefilter && __all_sync(0xffffffffu, crude_excludes(hf, pr, ztab->zeta))) continue;
       unsigned bits;
       if (RT) bits = fast_hit_rt<T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
@@ -513,7 +523,7 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
     err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
     if (err != cudaSuccess) return err;                                                                                      \
     vote_dense_fast_kernel<T, RT_, SPLIT_><<<grid, threads, smem, ctx->stream>>>(sp, staged, g, tiles_p, tiles_z, zt, per_split, \
-                                                                                  target);                                      \
+                                                                                  (ctx->params.flags & 64u) ? 1 : 0, target);   \
   } while (0)
   if (n_splits > 1) {
     if (coarse) IA_LAUNCH_FAST(true, true); else IA_LAUNCH_FAST(false, true);

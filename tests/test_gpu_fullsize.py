@@ -27,10 +27,17 @@ def _dense(cfg_idx, sample):
     rig = Rig(cfg.chamber)
     try:
         hd, oh = rig.hits(ev.wire, ev.drift)
+        # the prefiltered kernel (flags bit 6) must give the brute-force accumulator bit for bit, at full size
+        rig.ctx.ia_set_params(g.TOL, flags=64)
+        votes_pf = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
+        rig.ctx.ia_set_params(g.TOL, flags=0)
         votes = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
         idx, vv = rig.ctx.ia_topk(votes, 10)
         rig.ctx.synchronize()
         vg = votes.cpu().numpy()
+        vpf = votes_pf.cpu().numpy()
+        assert (vg == vpf).all(), f"prefilter changed {int((vg != vpf).sum())} cells"
+        del votes_pf, vpf
         idx, vv = idx.cpu().numpy(), vv.cpu().numpy()
         n = vg.size
         truth = g.truth_cell(ev.track.params, LO, HI, cfg.grid)

@@ -690,3 +690,32 @@ def test_refine_graph_is_really_replayed_on_a_capturable_stream():
         _assert_boxes_equal(ref, ob)
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_prefilter_gives_identical_votes(precision):
+    """flags bit 6: hits that a crude enclosure (magnitude bounds over a whole z0 tile) excludes for every lane of a warp
+    are skipped.  A wider enclosure that excludes 0 implies the fine one does, so the accumulator must be identical bit for
+    bit to the exhaustive kernel's - on a fine grid (where most hits are skipped), a coarse one, ragged shapes, a window
+    around the truth (where few are), an odd lambda grid, and with the reference plane and point off zero."""
+    import torch
+    for ref in ((0.0, 0.0, 0.0), (1.5, -2.0, 3.0)):
+        rig = Rig(g.chamber_c1(), precision=precision, x_ref=ref[0], y_ref=ref[1], z_ref=ref[2])
+        try:
+            ev = g.make_event(rig.ch, 35, n_noise=10)
+            hd, oh = rig.hits(ev.wire, ev.drift)
+            par = np.array(ev.track.params)
+            half = (HI - LO) / 128
+            grids = [(LO, HI, (24,) * 5), (LO, HI, (8,) * 5), (LO, HI, (5, 4, 10, 37, 12)), (LO, HI, (3, 3, 6, 20, 7)),
+                     (par - half, par + half, (8, 8, 8, 8, 8)), (LO, HI, (40, 40, 8, 4, 8))]
+            for lo, hi, dims in grids:
+                out = []
+                for flags in (0, 64):
+                    rig.ctx.ia_set_params(g.TOL, ref[0], ref[1], ref[2], precision, flags)
+                    out.append(rig.ctx.ia_vote(hd, ev.n_hits, lo, hi, dims))
+                rig.ctx.synchronize()
+                a, c = out[0].cpu().numpy(), out[1].cpu().numpy()
+                assert (a == c).all(), (precision, ref, dims, int((a != c).sum()), np.nonzero(a != c)[0][:10], a[a != c][:10], c[a != c][:10])
+                assert a.max() > 0
+        finally:
+            rig.close()
