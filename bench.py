@@ -34,10 +34,12 @@ from paper_2401_04576_b200 import eventgen as g  # noqa: E402
 METRIC = "cell-hit interval evals/s"
 UNIT = "evals/s"
 # FP64 arithmetic thread-instructions (DADD/DMUL/DFMA, comparisons not counted) that the
-# sign-specialised, FMA-fused DAG S4-S8 needs per (cell, hit) evaluation = both drift signs; counted op by op there
-# (175 FMA + 83 add/mul; ncu counts 277.6 executed on C1, profiles/r01_vote_dense_fast_c1_ncu.md)
-ALG_FP64_INST_PER_EVAL = 258.0
-ALG_FP64_FLOPS_PER_EVAL = 2 * 175.0 + 83.0
+# sign-specialised, FMA-fused DAG S4-S8 needs per (cell, hit) evaluation = both drift signs, counted op by op there in
+# its SHORTEST form (sin/cos polynomials without the three leading steps that |Phi - Phi_Ax| < 1/16 makes negligible):
+# 163 FMA + 83 add/mul.  ncu counts 248.3 executed on C1 (profiles/r02_vote_dense_c1_ncu.md): the numerator is below what
+# the kernel executes, never above.  (Round 1 used the long form, 258 = 175 + 83.)
+ALG_FP64_INST_PER_EVAL = 246.0
+ALG_FP64_FLOPS_PER_EVAL = 2 * 163.0 + 83.0
 # the same DAG with every product and sum as its own directed instruction (no FMA): what an unfused
 # implementation has to issue; context only
 DAG_UNFUSED_OPS_PER_EVAL = 366.0
@@ -382,10 +384,12 @@ def run_c3(args, rank, world, local_rank, barrier):
         evs = [g.make_event(ch, 1000 + rank * n_ev + e, n_noise=10) for e in range(n_ev)]
     h3 = b.hits_of(np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs]))
     off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
-    ctx = b.Context(local_rank)
+    # an explicit stream: the legacy default stream cannot be captured, and a repeated refinement is replayed as a CUDA graph
+    ctx = b.Context(local_rank, stream=torch.cuda.Stream(local_rank))
     ctx.ia_load_geometry(b.wires_of(ch))
-    ctx.ia_set_params(g.TOL, precision=args.precision)
+    ctx.ia_set_params(g.TOL, precision=args.precision, flags=args.flags)
     hd, od = ctx.to_device(h3), ctx.to_device(off)
+    torch.cuda.synchronize()
     boxes, par = ctx.ia_refine_batch(hd, od, n_ev, mh, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k)
     for _ in range(max(0, args.warmup - 1)):
         ctx.ia_refine_batch(hd, od, n_ev, mh, g.BOX_LO, g.BOX_HI, (8,) * 5, levels, k, boxes=boxes, params=par)
@@ -399,6 +403,7 @@ def run_c3(args, rank, world, local_rank, barrier):
     c.record(ctx.stream)
     barrier()
     launches = ctx.ia_launch_count() - l0
+    replays = ctx.ia_graph_replays()
     clocks = sampler.stop() if sampler else None
     t = torch.tensor([a.elapsed_time(c)], dtype=torch.float64, device=f"cuda:{local_rank}")
     if world > 1:
@@ -419,6 +424,7 @@ def run_c3(args, rank, world, local_rank, barrier):
     gb_all = b.boxes_to_numpy(boxes, (n_ev, levels, k))
     gb = gb_all[:n_s]
     same = bool((gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all())
+    ctx.ia_set_params(g.TOL, precision=args.precision, flags=0)
     truth = refine_truth_stats(ctx, hd, off, evs, gb_all, par.cpu().numpy().reshape(n_ev, -1), (8,) * 5, levels)
     line = {"metric": METRIC, "value": evals * world / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -426,7 +432,8 @@ def run_c3(args, rank, world, local_rank, barrier):
             "config": {"workload": f"{args.workload}: BASELINE.json configs[{args.workload[1]}], {n_ev} event(s) x {mh} hits, "
                                    f"8^5 start, K={k}, {levels} passes",
                        "evals_per_step": evals, "l2": "vote scratch (64 KB per event) rewritten every step"},
-            "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks,
+            "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "graph_replays": int(replays),
+            "clocks": clocks,
             "cpu_baseline": {"value": n_s * evals / n_ev / dt_o, "unit": UNIT, "cores": o.max_threads(), "kind": "oracle",
                              "sample": f"orc_refine_batch on the first {n_s} event(s) ({dt_o:.2f} s)",
                              "events_per_s": n_s / dt_o, "boxes_identical": same},
@@ -682,7 +689,7 @@ def main():
         evs = [g.make_event(ch3, 1000 + e, n_noise=10) for e in range(n_ev)]
         h3 = b.hits_of(np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs]))
         off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
-        ctx3 = b.Context(local_rank)
+        ctx3 = b.Context(local_rank, stream=torch.cuda.Stream(local_rank))     # capturable: repeated calls replay a CUDA graph
         ctx3.ia_load_geometry(b.wires_of(ch3))
         eps = {}
         for prec in (64, 32):
@@ -701,6 +708,7 @@ def main():
             ctx3.ia_refine_batch_host(h3, off, g.BOX_LO, g.BOX_HI, (8,) * 5, 8, 8)
             dt_h = time.perf_counter() - t0
             eps[f"fp{prec}"] = {"events_per_s": n_ev / (ms * 1e-3), "ms": ms, "e2e_events_per_s": n_ev / dt_h,
+                                "graph_replays": ctx3.ia_graph_replays(),
                                 "evals_per_s": n_ev * (8 ** 5 + 7 * 8 * 32) * 30 / (ms * 1e-3),
                                 "truth": refine_truth_stats(ctx3, hd3, off, evs, b.boxes_to_numpy(boxes, (n_ev, 8, 8)),
                                                             par.cpu().numpy().reshape(n_ev, -1), (8,) * 5, 8)}
