@@ -322,24 +322,30 @@ template <> struct Dir<float> {
 // rounding: the last operations are x + x^3 q and 1 - x^2 r with |x^3 q| <= |x|/96, |x^2 r| <= 1/32,
 // so the total error stays below 1 ulp of the result - well inside the relative pad 2^-50 (4..8 ulps).
 // Float: terms to x^7 / x^8, truncation < 1e-11, pad 2^-21.
+// The double coefficients sit in constant memory: a DFMA takes c[bank][offset] as an operand directly, whereas literals
+// are rebuilt in uniform registers (two UMOV each) on every evaluation - there are not enough of them to keep 11 doubles.
+//                                        -1/11!                   1/9!                    -1/7!                    1/5!                    -1/3!
+static __constant__ double IA_SIN_C[5] = {-2.5052108385441720e-08, 2.7557319223985893e-06, -1.9841269841269841e-04, 8.3333333333333332e-03,
+                                          -1.6666666666666666e-01};
+//                                        1/12!                   -1/10!                   1/8!                    -1/6!                    1/4!
+static __constant__ double IA_COS_C[6] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05, -1.3888888888888889e-03,
+                                          4.1666666666666664e-02, -0.5};
 template <class T> struct Trig;
 template <> struct Trig<double> {
   static IA_DEV double sqr(double x) { return __dmul_rn(x, x); }
   static IA_DEV double sin_small(double x, double s) {
-    double q = -2.5052108385441720e-08;               // -1/11!
-    q = __fma_rn(q, s, 2.7557319223985893e-06);       //  1/9!
-    q = __fma_rn(q, s, -1.9841269841269841e-04);      // -1/7!
-    q = __fma_rn(q, s, 8.3333333333333332e-03);       //  1/5!
-    q = __fma_rn(q, s, -1.6666666666666666e-01);      // -1/3!
+    double q = __fma_rn(IA_SIN_C[0], s, IA_SIN_C[1]);
+    q = __fma_rn(q, s, IA_SIN_C[2]);
+    q = __fma_rn(q, s, IA_SIN_C[3]);
+    q = __fma_rn(q, s, IA_SIN_C[4]);
     return __fma_rn(__dmul_rn(x, s), q, x);
   }
   static IA_DEV double cos_small(double s) {
-    double q = 2.0876756987868100e-09;                //  1/12!
-    q = __fma_rn(q, s, -2.7557319223985888e-07);      // -1/10!
-    q = __fma_rn(q, s, 2.4801587301587302e-05);       //  1/8!
-    q = __fma_rn(q, s, -1.3888888888888889e-03);      // -1/6!
-    q = __fma_rn(q, s, 4.1666666666666664e-02);       //  1/4!
-    q = __fma_rn(q, s, -0.5);
+    double q = __fma_rn(IA_COS_C[0], s, IA_COS_C[1]);
+    q = __fma_rn(q, s, IA_COS_C[2]);
+    q = __fma_rn(q, s, IA_COS_C[3]);
+    q = __fma_rn(q, s, IA_COS_C[4]);
+    q = __fma_rn(q, s, IA_COS_C[5]);
     return __fma_rn(q, s, 1.0);
   }
 };

@@ -115,12 +115,6 @@ template <class T> IA_DEV int e_mag(const Iv<T> (&e)[2]) {
 }
 
 // sin and cos over e0, e1 inside [-1/4, 1/4] (trig_small of ia_fast.cuh, eight Horner chains abreast)
-// The coefficients sit in constant memory: a DFMA takes c[bank][offset] as an operand directly, whereas literals are
-// rebuilt in uniform registers (two UMOV each) on every evaluation - there are not enough of them to keep 11 doubles.
-static __constant__ double IA_SIN_C[5] = {-2.5052108385441720e-08, 2.7557319223985893e-06, -1.9841269841269841e-04,
-                                          8.3333333333333332e-03, -1.6666666666666666e-01};
-static __constant__ double IA_COS_C[6] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05,
-                                          -1.3888888888888889e-03, 4.1666666666666664e-02, -0.5};
 template <class T> struct TrigC;
 template <> struct TrigC<double> {
   static constexpr int NS = 5, NC = 6;
