@@ -86,8 +86,9 @@ typedef struct {
  * phi_Ax - phi0 of (A.8d) is theta(wire point) - theta(reference point), theta in [-0.3, 2 pi - 0.3) counted from the
  * point of the base circle closest to the axis, instead of the principal value in (-pi, pi]; bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
  * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
- * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; runs in the
- * general (sign-agnostic) kernels, about 4 x the arithmetic; bit 5: ia_refine / ia_refine_batch always enqueue
+ * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; ia_vote runs it in the
+ * sign-specialised dense kernel (about 6 x the series mode), the explicit-box and refinement kernels in the general
+ * form; bit 5: ia_refine / ia_refine_batch always enqueue
  * their launches one by one (default: a call repeated with identical arguments and buffers is replayed as a
  * CUDA graph from its third occurrence on); bit 6 (sign-specialised dense kernel): prefilter - before the fine
  * evaluation of a hit a warp asks a crude enclosure of the same residual (magnitude bounds of every step of S4-S8, both

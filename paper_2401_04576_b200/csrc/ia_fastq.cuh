@@ -431,7 +431,64 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
 // dependent quads are short uniform switches.  Same arithmetic as pass_vote_q<SS> for every class.
 IA_DEV int opaque_i(int x) { asm volatile("" : "+r"(x)); return x; }
 
-template <class T, class H>
+// ---- rigorous Phi in the sign-specialised form (ia_params.flags bit 4; reading f3) ------------------
+// atan on [-1/16, 1/16]: odd Taylor polynomial, round-to-nearest Horner; truncation t^14/15 < 2^-59 relative (double,
+// terms to t^13) resp. t^8/9 < 2^-35 (float, terms to t^7), rounding below 1 ulp: inside the relative pad 2^-50 (2^-21).
+template <class T> struct AtanC;
+template <> struct AtanC<double> {
+  static IA_DEV double poly(double t) {
+    const double s = __dmul_rn(t, t);
+    double q = 1.0 / 13.0;
+    q = __fma_rn(q, s, -1.0 / 11.0);
+    q = __fma_rn(q, s, 1.0 / 9.0);
+    q = __fma_rn(q, s, -1.0 / 7.0);
+    q = __fma_rn(q, s, 1.0 / 5.0);
+    q = __fma_rn(q, s, -1.0 / 3.0);
+    return __fma_rn(__dmul_rn(t, s), q, t);
+  }
+  static constexpr int p4 = 0x3fb00000;            // high word of 2^-4
+  static __device__ __noinline__ double lib(double t) { return atan(t); }
+  static IA_DEV double rcp(double x) {                 // x in [2^-500, 2^500]; relative error below 2^-51
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = __fma_rn(-x, y, 1.0);
+    y = __fma_rn(y, e, y);
+    e = __fma_rn(-x, y, 1.0);
+    return __fma_rn(y, e, y);
+  }
+};
+template <> struct AtanC<float> {
+  static IA_DEV float poly(float t) {
+    const float s = __fmul_rn(t, t);
+    float q = -1.0f / 7.0f;
+    q = __fmaf_rn(q, s, 1.0f / 5.0f);
+    q = __fmaf_rn(q, s, -1.0f / 3.0f);
+    return __fmaf_rn(__fmul_rn(t, s), q, t);
+  }
+  static constexpr int p4 = 0x3d800000;
+  static __device__ __noinline__ float lib(float t) { return atanf(t); }
+  static IA_DEV float rcp(float x) { return __frcp_rn(x); }
+};
+// g(E) = atan2(y, x) of the angular equation (A.6) over the rectangle y x x with x > 0: y/x increases with y, and with
+// x it decreases where y > 0 and increases where y < 0, so the extremes are at two corners.  ok = false: x may touch 0 -
+// the caller re-takes the whole evaluation in the general form (there atan2 on such a rectangle is [-pi, pi]).
+template <class T> IA_DEV Iv<T> atan2_small(Iv<T> y, Iv<T> x, bool& ok) {
+  using R = Rnd<T>;
+  ok = is_pos(x.lo);
+  const T xl = ok ? x.lo : T(1), xh = ok ? x.hi : T(1);
+  // 1/x in [rl, rh]: a reciprocal good to a few ulps (MUFU seed + two Newton steps, resp. the float instruction), pushed
+  // outward by the relative pad - no directed-division subroutine in the loop
+  const T rl = pad_dn(AtanC<T>::rcp(xh)), rh = pad_up(AtanC<T>::rcp(xl));
+  const T tl = R::mul_dn(y.lo, sgn(y.lo) ? rh : rl), th = R::mul_up(y.hi, sgn(y.hi) ? rl : rh);
+  // beyond 1/16 (wide cells): the library's atan, documented maximum error 2 ulp, under the same relative pad
+  const bool in = (hiw(tl) & 0x7fffffff) < AtanC<T>::p4 && (hiw(th) & 0x7fffffff) < AtanC<T>::p4;
+  T al, ah;
+  if (in) { al = AtanC<T>::poly(tl); ah = AtanC<T>::poly(th); }
+  else { al = AtanC<T>::lib(tl); ah = AtanC<T>::lib(th); }
+  return {pad_dn(al), pad_up(ah)};
+}
+
+template <bool RIG = false, class T, class H>
 IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, const PairC<T>& p, const HitP<T>& hp,
                              Iv<T> Zr, MR<T> sAm, MR<T> s2m, Iv<T> sAabs, Iv<T> sA2abs, Iv<T>* fout = nullptr) {
   using V = VR<T>;
@@ -461,11 +518,21 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
   else if (ss < 0) q_fma<QK_SUB_P>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
   else q_fma<QK_ADD_U>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);
   q_fma<QK_ADD_P>(h.T2hiQm(), h.T2hiQm(), Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
+  // RIG: e is not the series value but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
+  // inflation from the series enclosure exactly as in residual_general (ia_residual.cuh; state 0 = verifying, 1 = tightening,
+  // 2 = final, per drift sign and lane); S5-S7 below then run once per round for the whole warp.  bad: x of (A.6) is not
+  // positive on this lane's box (the wire point may lie on the circle's centre) - the caller re-takes it in the general form.
+  int st0 = RIG ? 0 : 2, st1 = RIG ? 0 : 2, rounds0 = 0, rounds1 = 0;
+  bool fail0 = false, fail1 = false, bad = false;
+  Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
+  Iv<T> sa[2], ca[2], sinP[2], cosP[2];
+  Iv<T> u2[2], dq[2];
+  Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
+#pragma unroll 1
+  for (;;) {
   const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
   const bool small = emag < EMag<T>::quarter;
   // S5
-  Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
-  Iv<T> sa[2], ca[2], sinP[2], cosP[2];
   if (__all_sync(0xffffffffu, small)) {
     Iv<T> ce[2];
     q_trig_small(e, se, ce, __all_sync(0xffffffffu, emag < EMag<T>::sixteenth));
@@ -499,7 +566,6 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
   for (int s = 0; s < 2; ++s) { sinP[s] = clamp_unit(sinP[s]); cosP[s] = clamp_hi(cosP[s]); }
   if (!plain) { cosP[0] = clamp_lo(cosP[0]); cosP[1] = clamp_lo(cosP[1]); }
   // S6: u_d^2 >= 1 - 2 T max|lambda| - rounding >= 0.49 by the guard
-  Iv<T> u2[2], dq[2];
   q_fma<QK_ADD_P>(hp.TL2m, hp.TL2m, sinP[0], sinP[1], hp.T2L2, hp.T2L2, u2[0], u2[1]);
   if (plain) {
     const T a0 = V::mul_dn(cosP[0].lo, cosP[0].lo), b0 = V::mul_up(cosP[0].hi, cosP[0].hi);
@@ -515,7 +581,6 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
   }
   QDir<T>::d_over_sqrt(h.DloP(), h.DhiP(), u2, dq);                                     // |delta| = D+ / u_d
   // S7: z = (Zr + LR (dphi + e)) - T delta cosP, delta = dq (D+), -dq (D-)
-  Iv<T> de[2], zz[2], Tdq[2], TLq[2], qs[2], z[2], ct[2], Rd1[2], Tz[2];
   q_add(e[0], e[1], h.dphi(va), h.dphi(va), de[0], de[1]);
   q_fma<QK_ADD_P>(p.LRm, p.LRm, de[0], de[1], Zr, Zr, zz[0], zz[1]);
   Tdq[0].lo = V::mul_dn(Tn, dq[0].lo); Tdq[0].hi = V::mul_up(Tn, dq[0].hi);                 // |T delta|
@@ -545,6 +610,45 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
   Rd1[1].lo = V::add_dn(p.R.lo, -dq[1].hi); Rd1[1].hi = V::add_up(p.R.hi, -dq[1].lo);
   Tz[0].lo = V::mul_dn(Tn, z[0].lo); Tz[0].hi = V::mul_up(Tn, z[0].hi);
   Tz[1].lo = V::mul_dn(Tn, z[1].lo); Tz[1].hi = V::mul_up(Tn, z[1].hi);
+  if (!RIG) break;
+  if (__all_sync(0xffffffffu, (st0 == 2 || fail0 || bad) && (st1 == 2 || fail1 || bad))) break;
+  {
+    // g(E) = atan2(T s^tau, R_Ax^2 + T c^tau), s^tau = -(z s_Ax + lambda delta c_Ax) (A.6), (A.7b,c); here T z = Tz,
+    // T lambda delta = +-TLq (D+ / D-), 2 T c^tau = ct
+    using Rd = Rnd<T>;
+    const T tiny = sizeof(T) == 4 ? T(1e-6) : T(1e-12);
+    const MR<T> sAt = h.sAm(va), cAt = h.cAm();          // true signs (universal products: any class)
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      const Iv<T> zs = prod_u(sAt, Tz[s]), lc = prod_u(cAt, TLq[s]);
+      const Iv<T> sum = s == 0 ? iadd(zs, lc) : isub(zs, lc);
+      const Iv<T> y = ineg(sum);
+      const Iv<T> x = {Rd::add_dn(h.Q().lo, Rd::mul_dn(T(0.5), ct[s].lo)), Rd::add_up(h.Q().hi, Rd::mul_up(T(0.5), ct[s].hi))};
+      bool ok;
+      const Iv<T> G = atan2_small(y, x, ok);
+      int& st = s == 0 ? st0 : st1;
+      int& rounds = s == 0 ? rounds0 : rounds1;
+      bool& fail = s == 0 ? fail0 : fail1;
+      if (!ok) bad = true;
+      if (st == 0) {
+        if (G.lo >= e[s].lo && G.hi <= e[s].hi) {
+          e[s] = G;
+          st = 1;
+        } else {
+          if (++rounds >= 6) { fail = true; st = 2; }
+          const T lo_h = mn(e[s].lo, G.lo), hi_h = mx(e[s].hi, G.hi);
+          const T pad = Rd::add_up(Rd::mul_up(T(0.1), Rd::add_up(hi_h, -lo_h)), tiny);
+          e[s] = {Rd::add_dn(lo_h, -pad), Rd::add_up(hi_h, pad)};
+        }
+      } else if (st == 1) {
+        e[s] = {mx(e[s].lo, G.lo), mn(e[s].hi, G.hi)};
+        if (!(e[s].lo <= e[s].hi)) { fail = true; e[s] = G; }
+        st = 2;
+      }
+    }
+    if (bad) { e[0] = e[1] = Iv<T>{T(0), T(0)}; }
+  }
+  }
   // S8
   Iv<T> r1[2], r2[2], f[2];
 #pragma unroll
@@ -560,7 +664,12 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
 #pragma unroll
   for (int s = 0; s < 2; ++s) { f[s].lo = V::add_dn(h.Q().lo, -r2[s].hi); f[s].hi = V::add_up(h.Q().hi, -r2[s].lo); }
   if (fout) { fout[0] = f[0]; fout[1] = f[1]; }       // diagnostics (ia_residual_fast); nullptr in the vote kernels
-  return decide(f, h.band());
+  unsigned r = decide(f, h.band());
+  if (RIG) {
+    if (fail0 || fail1) r |= 1u;                      // not verified: the hit votes (cannot exclude), as in the general form
+    if (bad) r |= 4u;                                 // outside the fast form's domain: re-take in the general form
+  }
+  return r;
 }
 
 }  // namespace ia

@@ -98,12 +98,12 @@ template <class T> struct __align__(16) ZTab {
   T zeta, _pad;               // largest |z0 - z_ref| of the tile (prefilter)
 };
 
-template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>& h, int va, Iv<T> R, Iv<T> Zeff, Iv<T> L) {
+template <class T> __device__ __noinline__ bool general_votes_norm(const HitF<T>& h, int va, Iv<T> R, Iv<T> Zeff, Iv<T> L, int rig = 0) {
   XYInv<T> v;
   v.Q = h.Q; v.cA = h.cA; v.sA = h.sA[va]; v.dphi = h.dphi[va]; v.iQ = h.iQ; v.RA = h.RA; v.iR = h.iR; v.c2 = h.c2;
   v.s2 = h.s2[va];
   v.forced = 0;
-  HitS<T> hs = {h.Tabs, h.Dlo, h.Dhi, 1, 0};
+  HitS<T> hs = {h.Tabs, h.Dlo, h.Dhi, 1, rig};
   Box3<T> bx = {R, Zeff, L};
   return hit_votes_general(bx, v, hs, T(0));
 }
@@ -126,21 +126,23 @@ IA_DEV unsigned fast_hit(const HitF<T>& h, unsigned h_addr, int va, const PairC<
 
 // float: the cells the fast form could not decide are re-taken in the general form (which does the oracle's arithmetic)
 template <class T>
-IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L, const Iv<T>* zt) {
+IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L, const Iv<T>* zt, int rig = 0) {
   if (Filter<T>::on) {
     unsigned amb = bits >> FAST_ZT;
     bits &= (1u << FAST_ZT) - 1u;
     while (amb) {
       const int i = __ffs(amb) - 1;
       amb &= amb - 1;
-      bits = (bits & ~(1u << i)) | (general_votes_norm(h, va, R, zt[i], L) ? 1u << i : 0u);
+      bits = (bits & ~(1u << i)) | (general_votes_norm(h, va, R, zt[i], L, rig) ? 1u << i : 0u);
     }
   }
   return bits;
 }
 
 // the same with the sign class as a run-time value (one compiled body, ia_fastq.cuh)
-template <class T>
+// RIG: rigorous-Phi mode (flags bit 4); cells whose evaluation leaves the fast form's domain there (bit 2 of the result)
+// are re-taken in the general form at once
+template <class T, bool RIG = false>
 IA_DEV unsigned fast_hit_rt(const HitF<T>& h, unsigned h_addr, int ss, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
   const HitP<T> hp = hit_prepare(h, va, p);
   const Pass2<T> pc2 = pass_prepare2(h, p, hp);
@@ -150,8 +152,9 @@ IA_DEV unsigned fast_hit_rt(const HitF<T>& h, unsigned h_addr, int ss, int va, c
   unsigned bits = 0;
 #pragma unroll 1
   for (int i = 0; i < nz_tile; ++i) {
-    const unsigned r = pass_vote_qr<T>(hl, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
-    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : r << i;
+    unsigned r = pass_vote_qr<RIG, T>(hl, ss, va, pc2, p, hp, zt[i], sAm, s2m, sAabs, sA2abs);
+    if (RIG && (r & 4u)) r = general_votes_norm(h, va, p.R, zt[i], p.L, 1) ? 1u : 0u;
+    bits |= Filter<T>::on ? ((r & 1u) | ((r & 2u) << (FAST_ZT - 1))) << i : (r & 1u) << i;
   }
   return bits;
 }
@@ -169,7 +172,7 @@ IA_DEV unsigned long long spread8(unsigned bits) {
 // argument of three bodies (fine grids: 6 % faster there).  Same arithmetic, same results.
 // SPLIT: the hit range is divided over blockIdx.z (small launches only; a separate instantiation so that the
 // main path keeps its code: with the split as a run-time case C1 and C3 ran 0.5-0.9 % slower).
-template <class T, bool RT, bool SPLIT>
+template <class T, bool RT, bool SPLIT, bool RIG = false>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z, int zt,
                        int per_split, int prefilter, uint16_t* __restrict__ votes) {
@@ -265,18 +268,19 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
       // flags bit 6: a crude enclosure over the whole z0 tile excludes this hit for every lane -> nobody votes
-      if (prefilter && __all_sync(0xffffffffu, crude_excludes(hf, pr, ztab->zeta))) continue;
+      // (not in the rigorous-Phi mode: the bound is built on the series value of Phi - Phi_Ax)
+      if (!RIG && prefilter && __all_sync(0xffffffffu, crude_excludes(hf, pr, ztab->zeta))) continue;
       unsigned bits;
-      if (RT) bits = fast_hit_rt<T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
+      if (RT) bits = fast_hit_rt<T, RIG>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), kind == HIT_FAST_P ? 1 : (kind == HIT_FAST_N ? -1 : 0), va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_P) bits = fast_hit<1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
       else if (kind == HIT_FAST_N) bits = fast_hit<-1, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
       else bits = fast_hit<0, T>(hf, sh_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), va, pr, zt, nz_tile);
-      bits = settle(bits, hf, va, R, pr.L, zt);
+      bits = settle(bits, hf, va, R, pr.L, zt, RIG ? 1 : 0);
 #pragma unroll
       for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += spread8((bits >> (8 * j)) & 0xffu);
     } else {
       unsigned bits = 0;
-      for (int i = 0; i < nz_tile; ++i) bits |= (general_votes_norm(hf, va, R, zt[i], pr.L) ? 1u : 0u) << i;
+      for (int i = 0; i < nz_tile; ++i) bits |= (general_votes_norm(hf, va, R, zt[i], pr.L, RIG ? 1 : 0) ? 1u : 0u) << i;
 #pragma unroll
       for (int j = 0; j < FAST_ZT / 8; ++j) acc[j] += spread8((bits >> (8 * j)) & 0xffu);
     }
@@ -453,7 +457,7 @@ __global__ void residual_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ sta
   const Iv<T> sAabs = ss < 0 ? ineg(hf.sA[va]) : hf.sA[va], sA2abs = ss < 0 ? ineg(hf.sA2[va]) : hf.sA2[va];
   const Iv<T> Zr = isub(Z, thin(c.zref));
   Iv<T> f[2];
-  pass_vote_qr<T>(HitDirect<T>{hf}, ss, va, pc2, pr, hp, hf.zflip ? ineg(Zr) : Zr, sAm, s2m, sAabs, sA2abs, f);
+  pass_vote_qr<false, T>(HitDirect<T>{hf}, ss, va, pc2, pr, hp, hf.zflip ? ineg(Zr) : Zr, sAm, s2m, sAabs, sA2abs, f);
   for (int s = 0; s < 2; ++s) { o[4 * s] = f[s].lo; o[4 * s + 1] = f[s].hi; o[4 * s + 2] = hf.Q.hi; o[4 * s + 3] = 0.0; }
 }
 
@@ -518,17 +522,20 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   const bool coarse = (ctx->params.flags & 2u) ? true : ((ctx->params.flags & 4u) ? false : wxy > 0.5 * ctx->max_wire_r);
   dim3 grid((unsigned)blocks, (unsigned)sp.n_events, (unsigned)n_splits);
   const HitC<T>* staged = static_cast<const HitC<T>*>(ctx->staged.p);
-#define IA_LAUNCH_FAST(RT_, SPLIT_)                                                                                          \
+#define IA_LAUNCH_FAST(RT_, SPLIT_, RIG_)                                                                                    \
   do {                                                                                                                       \
-    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
+    err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
     if (err != cudaSuccess) return err;                                                                                      \
-    vote_dense_fast_kernel<T, RT_, SPLIT_><<<grid, threads, smem, ctx->stream>>>(sp, staged, g, tiles_p, tiles_z, zt, per_split, \
+    vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_><<<grid, threads, smem, ctx->stream>>>(sp, staged, g, tiles_p, tiles_z, zt, per_split, \
                                                                                   (ctx->params.flags & 64u) ? 1 : 0, target);   \
   } while (0)
-  if (n_splits > 1) {
-    if (coarse) IA_LAUNCH_FAST(true, true); else IA_LAUNCH_FAST(false, true);
+  if (ctx->params.flags & 16u) {
+    // rigorous Phi: the one-body variant carries the verification loop (any grid)
+    if (n_splits > 1) IA_LAUNCH_FAST(true, true, true); else IA_LAUNCH_FAST(true, false, true);
+  } else if (n_splits > 1) {
+    if (coarse) IA_LAUNCH_FAST(true, true, false); else IA_LAUNCH_FAST(false, true, false);
   } else {
-    if (coarse) IA_LAUNCH_FAST(true, false); else IA_LAUNCH_FAST(false, false);
+    if (coarse) IA_LAUNCH_FAST(true, false, false); else IA_LAUNCH_FAST(false, false, false);
   }
 #undef IA_LAUNCH_FAST
   ctx->launches++;
@@ -594,7 +601,9 @@ cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& sp, int lev, i
 
 cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
   // the fast form packs vote counts in bytes and keeps one HitF per hit in shared memory
-  const bool fast = !(ctx->params.flags & 17u) && sp.max_hits <= 255;   // bit 4 (rigorous Phi) lives in the general form
+  // bit 4 (rigorous Phi): sign-specialised too since round 2 (one-body variant with the verification loop); bits 0 + 4
+  // together keep the general form
+  const bool fast = !(ctx->params.flags & 1u) && sp.max_hits <= 255;
   if (ctx->params.precision == 32)
     return fast ? launch_fast<float>(ctx, sp, g, votes_out) : launch_general<float>(ctx, sp, g, votes_out);
   return fast ? launch_fast<double>(ctx, sp, g, votes_out) : launch_general<double>(ctx, sp, g, votes_out);
