@@ -728,7 +728,7 @@ def main():
             ctxr = b.Context(local_rank)
             ctxr.ia_load_geometry(b.wires_of(ch1))
             hdr = ctxr.to_device(b.hits_of(ev1.wire, ev1.drift))
-            rdims = (16,) * 5
+            rdims = (24,) * 5
             nr = int(np.prod(rdims))
             vr = torch.empty(nr, dtype=torch.uint16, device=f"cuda:{local_rank}")
             rr = {}
@@ -744,7 +744,7 @@ def main():
                 c.synchronize()
                 ms = a.elapsed_time(c) / 3
                 rr[name] = {"ms": ms, "evals_per_s": nr * ev1.n_hits / (ms * 1e-3), "sum_votes": int(vr.to(torch.int64).sum().item())}
-            rr["workload"] = ("f3: dense 16^5 x 40 hits (C1 event): series (A.8) vs verified fixed point of (A.6), in the "
+            rr["workload"] = ("f3: dense 24^5 x 40 hits (C1 event): series (A.8) vs verified fixed point of (A.6), in the "
                               "sign-specialised kernels (flags 0 / 16) and in the general-form kernel (flags 1 / 17)")
             rr["cost_ratio"] = rr["fast_rigorous"]["ms"] / rr["fast_series"]["ms"]
             rr["cost_ratio_general_form"] = rr["general_rigorous"]["ms"] / rr["general_series"]["ms"]

@@ -89,3 +89,26 @@ def test_rigorous_dense_vote_refine_and_truth_with_no_tolerance():
                 assert int(v.cpu().numpy()[0]) == keep.sum(), (seed, n)
     finally:
         rig.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_sign_specialised_rigorous_kernel_agrees_with_the_general_one(precision):
+    """flags bit 4 in the sign-specialised dense kernel (verification loop inside the one-body form, own atan2 on x > 0)
+    against the general-form kernel (bits 0 + 4: library atan2 at four corners): same algorithm, roundings differ by the
+    pads, so the accumulators agree except at knife edges - on a full 14^5 grid, ragged shapes and an odd lambda grid."""
+    rig = Rig(g.chamber_c1(), precision=precision, flags=RIG)
+    try:
+        ev = g.make_event(rig.ch, 31, n_noise=10)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        for dims in ((14,) * 5, (5, 4, 10, 19, 12), (3, 3, 6, 20, 7)):
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG)
+            vf = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | 1)
+            vg = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            rig.ctx.synchronize()
+            vf, vg = vf.cpu().numpy(), vg.cpu().numpy()
+            bad = np.nonzero(vf != vg)[0]
+            assert len(bad) <= max(1, len(vf) // (100000 if precision == 64 else 2000)), (dims, len(bad), vf[bad[:10]], vg[bad[:10]])
+            assert vf.max() > 0
+    finally:
+        rig.close()
