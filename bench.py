@@ -303,6 +303,7 @@ def refine_truth_stats(ctx, hd, off, evs, boxes, par, grid0, levels):
     of rank 0, the votes of the truth's box (one ia_vote_boxes call per event on the truth's boxes of all levels), the
     distance rank-0 centre -> truth in cell widths of that level (largest of the five axes).  Final: |centre - truth| in
     finest-cell widths per axis, whether the truth lies inside the G19 hull of the maximum-vote kept boxes."""
+    import torch
     n_ev = len(evs)
     lo, hi = np.array(g.BOX_LO), np.array(g.BOX_HI)
     kept = np.zeros((n_ev, levels), bool)
@@ -315,7 +316,10 @@ def refine_truth_stats(ctx, hd, off, evs, boxes, par, grid0, levels):
     for e, ev in enumerate(evs):
         t = np.array(ev.track.params)
         blo, bhi = truth_boxes(t, lo, hi, grid0, levels)
-        vb = ctx.ia_vote_boxes(hd[16 * int(off[e]):16 * int(off[e + 1])], ev.n_hits, ctx.to_device(blo), ctx.to_device(bhi))
+        blo_d, bhi_d = ctx.to_device(blo), ctx.to_device(bhi)
+        torch.cuda.synchronize()          # the copies run on torch's stream, the vote on the context's (an explicit one here)
+        vb = ctx.ia_vote_boxes(hd[16 * int(off[e]):16 * int(off[e + 1])], ev.n_hits, blo_d, bhi_d)
+        ctx.synchronize()                 # ... and .cpu() below would not wait for it
         v_truth[e] = vb.cpu().numpy()
         n_genuine[e] = int((~ev.is_noise).sum()) if hasattr(ev, "is_noise") else ev.n_hits
         for lev in range(levels):
@@ -562,7 +566,9 @@ def main():
         ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes)
         c.record(stream)
         idx, vv = ctx.ia_topk(votes, k)
-        ev_kernel.append((a, c))
+        d = torch.cuda.Event(enable_timing=True)
+        d.record(stream)
+        ev_kernel.append((a, c, d))
         flush.zero_()
     t_end.record(stream)
     barrier()
@@ -575,7 +581,8 @@ def main():
     ms_total = float(t.item())
     ms_step = ms_total / args.steps
     value = evals_per_step * world / (ms_step * 1e-3)
-    vote_ms = statistics.mean(a.elapsed_time(c) for a, c in ev_kernel)
+    vote_ms = statistics.mean(a.elapsed_time(c) for a, c, _ in ev_kernel)
+    topk_ms = statistics.mean(c.elapsed_time(d) for _, c, d in ev_kernel)
 
     if rank != 0:
         if world > 1:
@@ -625,6 +632,10 @@ def main():
                    "grid": list(dims), "n_hits": ev.n_hits, "evals_per_step": evals_per_step,
                    "l2": "256 MiB flush buffer written between steps; the 2.1 GB accumulator exceeds the 126 MB L2"},
         "roofline": roofline, "gpu_launches": int(launches), "clocks": clocks,
+        # a7, the only HBM-bound kernel of the path: 2 B per cell read once (events around ia_topk: two launches)
+        "topk": {"ms": topk_ms, "read_GBps": 2 * n_cells / (topk_ms * 1e-3) / 1e9,
+                 "hbm_frac": 2 * n_cells / (topk_ms * 1e-3) / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9),
+                 "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"},
     }
 
     if not args.no_extras:

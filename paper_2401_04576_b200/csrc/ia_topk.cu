@@ -1,9 +1,9 @@
 // ia_topk.cu - step a7: the K best cells of a vote accumulator (G16).
 //
-// Pass 1 (topk_partial): the accumulator is cut into one contiguous range per warp; each warp streams
-// its range with 16-byte loads (8 votes per lane) and keeps a sorted top-32 in its lanes
-// (ia_topk.cuh).  After the first few chunks the entry bar is high, so the common case per 256
-// votes is one compare per lane and one warp vote - the pass is HBM-bound.  Warps are merged per
+// Pass 1 (topk_partial): the accumulator is read as one stream of 256-vote chunks (16 bytes per lane) dealt
+// round-robin to the warps in groups of eight; each warp keeps a sorted top-32 in its lanes (ia_topk.cuh).
+// After the first few chunks the entry bar is high, so the common case per 256 votes is three packed
+// maxima, one compare per lane and one warp vote - the pass is HBM-bound.  Warps are merged per
 // block through shared memory.  Pass 2 (topk_final): the per-block lists of an event are merged and
 // the first k entries written out.  Ties on votes are broken by index ascending, carried in the key.
 #include "ia_internal.h"
@@ -15,51 +15,66 @@ namespace {
 
 constexpr int TOPK_THREADS = 256;
 
-__device__ __forceinline__ u64 best_of_8(const uint4 q, int64_t idx0) {
-  // the best key among 8 consecutive votes: highest votes, then lowest index
-  unsigned w[4] = {q.x, q.y, q.z, q.w};
-  u64 best = 0;
-#pragma unroll
-  for (int i = 3; i >= 0; --i) {
-    u64 kb = make_key(w[i] >> 16, idx0 + 2 * i + 1);
-    u64 ka = make_key(w[i] & 0xffffu, idx0 + 2 * i);
-    best = umax64(best, umax64(ka, kb));
-  }
-  return best;
+// an upper bound of every key among 8 consecutive votes starting at idx0: their largest vote with the smallest index
+__device__ __forceinline__ u64 bound_of_8(const uint4 q, int64_t idx0) {
+  const unsigned m = __vmaxu2(__vmaxu2(q.x, q.y), __vmaxu2(q.z, q.w));
+  return make_key(max(m >> 16, m & 0xffffu), idx0);
 }
 
-// grid (blocks_per_event, n_events); votes of event e at votes + e*n
+#ifndef IA_TOPK_UNROLL
+#define IA_TOPK_UNROLL 8
+#endif
+#ifndef IA_TOPK_BLOCKS_PER_SM
+#define IA_TOPK_BLOCKS_PER_SM 2
+#endif
+constexpr int TOPK_UNROLL = IA_TOPK_UNROLL;      // 16-byte loads in flight per lane (large accumulators; small ones take 1)
+
+// grid (blocks_per_event, n_events); votes of event e at votes + e*n.
+// The accumulator is read as a stream: chunk c = 256 votes = one 16-byte load per lane; a warp takes TOPK_UNROLL
+// consecutive chunks, consecutive warps consecutive groups, so the warps in flight read one contiguous window of the
+// accumulator (DRAM pages are read whole; one private range per warp, as in round 1, had every warp on a page of its
+// own and reached 37 % of the HBM rate).  All loads of a group are issued before the first is looked at.
+template <int U>
 __global__ void __launch_bounds__(TOPK_THREADS)
-topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, int64_t per_warp, u64* __restrict__ partial,
+topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, u64* __restrict__ partial,
              int64_t* __restrict__ idx_out, uint16_t* __restrict__ votes_out, int write_final) {
   __shared__ u64 smem_keys[(TOPK_THREADS / 32) * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int e = blockIdx.y;
   const uint16_t* v = votes + int64_t(e) * n;
   const int64_t gw = int64_t(blockIdx.x) * (TOPK_THREADS / 32) + warp;
-  int64_t beg = gw * per_warp, end = beg + per_warp;
-  if (end > n) end = n;
+  const int64_t n_warps = int64_t(gridDim.x) * (TOPK_THREADS / 32);
+  // [0, head): votes before the first 16-byte boundary; then n_chunks aligned chunks; then the tail
+  int64_t head = int64_t((16 - (reinterpret_cast<uintptr_t>(v) & 15)) & 15) >> 1;
+  if (head > n) head = n;
+  const int64_t n_chunks = (n - head) / 256;
+  const uint16_t* va = v + head;
   u64 mine = 0, kth = 0;
-  int64_t i = beg;
-  const bool aligned = ((reinterpret_cast<uintptr_t>(v + beg) & 15) == 0);
-  if (aligned) {
-    for (; i + 256 <= end; i += 256) {
-      const int64_t idx0 = i + 8 * lane;
-      const uint4 q = *reinterpret_cast<const uint4*>(v + idx0);
-      if (__any_sync(0xffffffffu, best_of_8(q, idx0) > kth)) {
-        unsigned w[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          unsigned vv = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
-          warp_offer(mine, kth, make_key(vv, idx0 + j), k);
-        }
-      }
+  if (gw == 0) {
+    for (int64_t i = 0; i < head; i += 32) {
+      const int64_t idx = i + lane;
+      warp_offer(mine, kth, idx < head ? make_key(v[idx], idx) : 0, k);
     }
   }
-  for (; i < end; i += 32) {
-    const int64_t idx = i + lane;
-    u64 cand = idx < end ? make_key(v[idx], idx) : 0;
-    warp_offer(mine, kth, cand, k);
+  for (int64_t c0 = gw * U; c0 < n_chunks; c0 += n_warps * U) {
+    uint4 q[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      q[u] = make_uint4(0u, 0u, 0u, 0u);
+      if (c0 + u < n_chunks) q[u] = __ldcs(reinterpret_cast<const uint4*>(va + (c0 + u) * 256 + 8 * lane));
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (c0 + u >= n_chunks) break;
+      const int64_t idx0 = head + (c0 + u) * 256 + 8 * lane;
+      warp_offer_8(mine, kth, q[u], idx0, bound_of_8(q[u], idx0) > kth, k);
+    }
+  }
+  if (gw == n_warps - 1) {
+    for (int64_t i = head + n_chunks * 256; i < n; i += 32) {
+      const int64_t idx = i + lane;
+      warp_offer(mine, kth, idx < n ? make_key(v[idx], idx) : 0, k);
+    }
   }
   mine = block_merge(mine, smem_keys);
   if (warp == 0) {
@@ -95,17 +110,20 @@ topk_final(const u64* __restrict__ partial, int n_lists, int k, int64_t* __restr
 
 cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_events, int k, int64_t* idx_out,
                         uint16_t* votes_out) {
-  // ranges per warp: multiples of 256 votes so that the 16-byte path stays aligned
+  // 2 blocks per SM over all events, never more than there are groups of chunks (measured on the 2.1 GB accumulator of
+  // C4, loads in flight per lane x blocks per SM: 4x8 0.468 ms, 8x4 0.402, 8x2 0.404, 8x3 0.388, 16x2 0.407, 8x1 0.552;
+  // on random votes 8x2 is the fastest, 0.396 ms = 5.4 TB/s)
   int sm = 148;
   cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, ctx->device);
-  const int warps_per_block = TOPK_THREADS / 32;
-  int64_t want_blocks = (int64_t(sm) * 8 + n_events - 1) / n_events;          // fill the chip across events
-  int64_t max_blocks = (n + 256 * warps_per_block - 1) / (256 * warps_per_block);
+  // a chunk whose votes beat the entry bar costs a warp some microseconds (eight sort-and-merge rounds), and every
+  // warp's first chunk does: small accumulators (the start grid of a refinement) take one chunk per warp and turn
+  const int64_t n_chunks = (n + 255) / 256;
+  const int64_t want_blocks = (int64_t(sm) * IA_TOPK_BLOCKS_PER_SM + n_events - 1) / n_events;     // fill the chip across events
+  const int unroll = n_chunks >= want_blocks * (TOPK_THREADS / 32) * TOPK_UNROLL ? TOPK_UNROLL : 1;
+  const int64_t per_block = int64_t(256) * unroll * (TOPK_THREADS / 32);
+  const int64_t max_blocks = (n + per_block - 1) / per_block;
   int64_t blocks = want_blocks < max_blocks ? want_blocks : max_blocks;
   if (blocks < 1) blocks = 1;
-  int64_t per_warp = (n + blocks * warps_per_block - 1) / (blocks * warps_per_block);
-  per_warp = (per_warp + 255) / 256 * 256;
-  blocks = (n + per_warp * warps_per_block - 1) / (per_warp * warps_per_block);
   const int write_final = blocks == 1;
   u64* partial = nullptr;
   if (!write_final) {
@@ -114,7 +132,8 @@ cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_eve
     partial = static_cast<u64*>(ctx->keys.p);
   }
   dim3 grid((unsigned)blocks, (unsigned)n_events);
-  topk_partial<<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, per_warp, partial, idx_out, votes_out, write_final);
+  if (unroll == 1) topk_partial<1><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, partial, idx_out, votes_out, write_final);
+  else topk_partial<TOPK_UNROLL><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, partial, idx_out, votes_out, write_final);
   ctx->launches++;
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess || write_final) return err;

@@ -59,6 +59,57 @@ __device__ __forceinline__ void warp_offer(u64& mine, u64& kth, u64 cand, int k)
   }
 }
 
+// insert ONE key x (the same value in every lane, x > kth) into the sorted list: the entries greater than x are the
+// lanes [0, pos); x goes to lane pos, the rest moves down one lane, the last entry drops out.  One ballot and one
+// 64-bit shuffle instead of a 32-key sort and a merge - the common case of a chunk that beats the entry bar is one
+// or two such keys.
+__device__ __forceinline__ void warp_insert(u64& mine, u64& kth, u64 x, int k) {
+  const int lane = threadIdx.x & 31;
+  const int pos = __popc(__ballot_sync(0xffffffffu, mine > x));
+  const u64 up = __shfl_up_sync(0xffffffffu, mine, 1);
+  if (lane == pos) mine = x;
+  else if (lane > pos) mine = up;
+  kth = __shfl_sync(0xffffffffu, mine, k - 1);
+}
+
+// offer the 8 consecutive votes of every lane (packed in q, first index idx0 per lane).  Few lanes with something above
+// the bar: their keys are inserted one at a time, lowest lane first, each lane walking its votes in index order and
+// skipping what the rising bar has overtaken.  Many lanes (a warp's first chunks, a plateau): eight sort-and-merge rounds.
+__device__ __forceinline__ void warp_offer_8(u64& mine, u64& kth, const uint4 q, int64_t idx0, bool lane_may, int k) {
+  const int lane = threadIdx.x & 31;
+  const unsigned may = __ballot_sync(0xffffffffu, lane_may);
+  if (may == 0u) return;
+  if (__popc(may) > 8) {
+    const unsigned w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const unsigned vv = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+      warp_offer(mine, kth, make_key(vv, idx0 + j), k);
+    }
+    return;
+  }
+  const u64 lo = (u64(q.y) << 32) | q.x, hi = (u64(q.w) << 32) | q.z;
+  int j = 0;
+  u64 c = 0;
+  auto next = [&]() {
+    c = 0;
+    while (j < 8) {
+      const unsigned vv = unsigned(((j < 4 ? lo : hi) >> (16 * (j & 3))) & 0xffffu);
+      const u64 kk = make_key(vv, idx0 + j);
+      ++j;
+      if (kk > kth) { c = kk; break; }
+    }
+  };
+  if (lane_may) next();
+  unsigned m;
+  while ((m = __ballot_sync(0xffffffffu, c != 0)) != 0u) {
+    const int src = __ffs(m) - 1;
+    const u64 x = __shfl_sync(0xffffffffu, c, src);
+    if (x > kth) warp_insert(mine, kth, x, k);
+    if (lane == src) next();
+  }
+}
+
 // block-level merge: every warp deposits its list in shared memory (nwarps*32 keys), warp 0 folds
 // them together and returns the block's list in its lanes (other warps return garbage)
 __device__ __forceinline__ u64 block_merge(u64 mine, u64* smem_keys) {

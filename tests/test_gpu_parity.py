@@ -204,17 +204,27 @@ def test_vote_boxes_and_empty_inputs(rig1):
     assert int(v0.cpu().numpy().astype(np.int64).sum()) == 0
 
 
-@pytest.mark.parametrize("n,k", [(1, 1), (31, 5), (32, 32), (257, 10), (4096, 16), (100003, 8), (1 << 21, 10)])
+# (1 << 23) + 77 cells: beyond the size from which the streaming form (8 loads in flight per lane) is taken
+@pytest.mark.parametrize("n,k", [(1, 1), (31, 5), (32, 32), (257, 10), (4096, 16), (100003, 8), (1 << 21, 10),
+                                 ((1 << 23) + 77, 10), ((1 << 23) + 77, 32)])
 def test_topk_bit_exact(rig0, n, k):
     import torch
     rng = np.random.default_rng(n)
-    for mode in ("random", "plateau", "zeros", "late_peak"):
+    for mode in ("random", "plateau", "zeros", "late_peak", "ramp", "bell", "sparse"):
         if mode == "random":
             v = rng.integers(0, 41, n)
         elif mode == "plateau":
             v = np.where(rng.random(n) < 0.4, 40, rng.integers(0, 40, n))
         elif mode == "zeros":
             v = np.zeros(n, np.int64)
+        elif mode == "ramp":            # rising: every chunk beats the entry bar (single-key insertions all the way)
+            v = (np.arange(n, dtype=np.int64) * 60000) // max(n, 1) + rng.integers(0, 3, n)
+        elif mode == "bell":            # the entry bar rises slowly (many rare records)
+            v = np.clip(rng.normal(12.0, 6.0, n), 0, 60).astype(np.int64)
+        elif mode == "sparse":          # one or two lanes of a chunk above the bar
+            v = np.zeros(n, np.int64)
+            pos = rng.integers(0, n, max(1, n // 997))
+            v[pos] = rng.integers(1, 200, len(pos))
         else:
             v = rng.integers(0, 5, n)
             v[-min(n, 3):] = 60
