@@ -353,12 +353,13 @@ cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int lev
   int n_splits = 1;
   uint16_t* partial = nullptr;
   cudaError_t err;
-  if (!(ctx->params.flags & 17u)) {
-    // sign-specialised form, a4 shared by the children of an xy sub-cell (ia_vote_dense.cu)
+  if (!(ctx->params.flags & 1u)) {
+    // sign-specialised form, a4 shared by the children of an xy sub-cell (ia_vote_dense.cu); with flags bit 4 its
+    // rigorous-Phi instantiation
     err = launch_vote_children_fast(ctx, sp, lev, levels, k, sm, boxes_out, &n_splits, &partial);
     if (err != cudaSuccess) return err;
   } else {
-    // general form (flags bit 0, and the rigorous-Phi mode of bit 4): split the hit range when there are too few events to fill the chip
+    // general form (flags bit 0, alone or with the rigorous-Phi mode of bit 4): split the hit range when there are too few events to fill the chip
     n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
     if (n_splits > sp.max_hits) n_splits = sp.max_hits;
     if (n_splits < 1) n_splits = 1;

@@ -320,7 +320,8 @@ __device__ __forceinline__ void child_half(double lo, double hi, int upper, doub
   chi = upper ? hi : mid;
 }
 
-template <class T>
+// RIG: rigorous-Phi mode (flags bit 4): the verification loop of pass_vote_qr, as in the dense kernel
+template <class T, bool RIG = false>
 __global__ void __launch_bounds__(512, 1)
 vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
                           int levels, int k, int per_split, uint16_t* __restrict__ partial) {
@@ -391,16 +392,16 @@ vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const 
     if (kind == HIT_FORCED) { v0 += 1; v1 += 1; }
     if (!warp_fast || __any_sync(0xffffffffu, kind == HIT_GENERAL)) {
       if (need) {
-        v0 += general_votes_norm(hf, va, R, zt[0], pr.L) ? 1u : 0u;
-        v1 += general_votes_norm(hf, va, R, zt[1], pr.L) ? 1u : 0u;
+        v0 += general_votes_norm(hf, va, R, zt[0], pr.L, RIG ? 1 : 0) ? 1u : 0u;
+        v1 += general_votes_norm(hf, va, R, zt[1], pr.L, RIG ? 1 : 0) ? 1u : 0u;
       }
     } else {
       const bool allP = __all_sync(0xffffffffu, kind == HIT_FAST_P || !need);
       const bool allN = __all_sync(0xffffffffu, kind == HIT_FAST_N || !need);
       // lanes that do not need the hit (forced, skipped) run along on their record and drop the result
-      unsigned bits = fast_hit_rt<T>(hf, my_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
+      unsigned bits = fast_hit_rt<T, RIG>(hf, my_addr + unsigned(h) * unsigned(sizeof(HitF<T>)), allP ? 1 : (allN ? -1 : 0), va, pr, zt, 2);
       if (need) {
-        bits = settle(bits, hf, va, R, pr.L, zt);
+        bits = settle(bits, hf, va, R, pr.L, zt, RIG ? 1 : 0);
         v0 += bits & 1u; v1 += (bits >> 1) & 1u;
       }
     }
@@ -581,12 +582,18 @@ static cudaError_t launch_children_fast_t(ia_ctx* ctx, const HitSpan& sp, int le
   if (err != cudaSuccess) return err;
   uint16_t* partial = static_cast<uint16_t*>(ctx->partial.p);
   const size_t smem = size_t(k) * sizeof(ZTab2<T>) + size_t(k) * 4 * per_split * sizeof(HitF<T>);
-  err = cudaFuncSetAttribute(vote_children_fast_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-  if (err != cudaSuccess) return err;
   const int threads = (k * 16 + 31) / 32 * 32;
   dim3 grid(n_splits, sp.n_events);
-  vote_children_fast_kernel<T><<<grid, threads, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), boxes, lev,
-                                                                    levels, k, per_split, partial);
+  const HitC<T>* staged = static_cast<const HitC<T>*>(ctx->staged.p);
+  if (ctx->params.flags & 16u) {
+    err = cudaFuncSetAttribute(vote_children_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (err != cudaSuccess) return err;
+    vote_children_fast_kernel<T, true><<<grid, threads, smem, ctx->stream>>>(sp, staged, boxes, lev, levels, k, per_split, partial);
+  } else {
+    err = cudaFuncSetAttribute(vote_children_fast_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (err != cudaSuccess) return err;
+    vote_children_fast_kernel<T, false><<<grid, threads, smem, ctx->stream>>>(sp, staged, boxes, lev, levels, k, per_split, partial);
+  }
   ctx->launches++;
   *n_splits_out = n_splits;
   *partial_out = partial;

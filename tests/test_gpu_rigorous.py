@@ -112,3 +112,32 @@ def test_sign_specialised_rigorous_kernel_agrees_with_the_general_one(precision)
             assert vf.max() > 0
     finally:
         rig.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_rigorous_refinement_children_kernel_matches_the_oracle(precision):
+    """flags bit 4 in the sign-specialised CHILDREN kernel (round 2; before, a rigorous refinement took the general-form
+    children kernel): kept boxes, votes and parameters of a batch refinement identical to the oracle's rigorous mode at
+    every level, and to the general-form kernels (bits 0 + 4)."""
+    rig = Rig(g.chamber_c1(), precision=precision, flags=RIG)
+    try:
+        evs = [g.make_event(rig.ch, 700 + e, n_noise=10) for e in range(6)]
+        wire, drift = np.concatenate([e.wire for e in evs]), np.concatenate([e.drift for e in evs])
+        off = np.cumsum([0] + [e.n_hits for e in evs]).astype(np.int32)
+        hd, oh = rig.hits(wire, drift)
+        od = rig.ctx.to_device(off)
+        for levels, k in ((6, 8), (5, 16), (4, 3)):
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG)
+            boxes, par = rig.ctx.ia_refine_batch(hd, od, len(evs), 30, LO, HI, (8,) * 5, levels, k)
+            rig.ctx.synchronize()
+            gb = b.boxes_to_numpy(boxes, (len(evs), levels, k))
+            ob, opar = o.refine_batch(rig.owires, oh, off, rig.oparams, LO, HI, (8,) * 5, levels, k)
+            assert (gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all(), (levels, k)
+            assert (par.cpu().numpy().reshape(opar.shape) == opar).all()
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | 1)
+            boxes2, par2 = rig.ctx.ia_refine_batch(hd, od, len(evs), 30, LO, HI, (8,) * 5, levels, k)
+            rig.ctx.synchronize()
+            g2 = b.boxes_to_numpy(boxes2, (len(evs), levels, k))
+            assert (gb["lo"] == g2["lo"]).all() and (gb["hi"] == g2["hi"]).all() and (gb["votes"] == g2["votes"]).all()
+    finally:
+        rig.close()
