@@ -446,6 +446,64 @@ def run_c3(args, rank, world, local_rank, barrier):
     ctx.close()
 
 
+def run_split(args, rank, world, local_rank, barrier):
+    """--split-event (SURVEY 8(e), strong scaling): ONE event's dense vote over all ranks - every rank votes its slab of xc
+    cells (ia_vote_slab), reduces it to its K best keys (ia_topk_keys), the key lists are all-gathered (NCCL, 256 B per
+    rank: the one exchange of the path) and merged on every rank (ia_merge_keys).  value = the event's evaluations / the
+    slowest rank's time."""
+    import torch
+    import torch.distributed as dist
+    from paper_2401_04576_b200 import binding as b
+    from paper_2401_04576_b200 import shard
+    ch, ev, dims, k = workload(args.workload, seed_shift=0)
+    n_cells = int(np.prod(np.array(dims, np.int64)))
+    evals_per_step = n_cells * ev.n_hits
+    ctx = b.Context(local_rank)
+    ctx.ia_load_geometry(b.wires_of(ch))
+    ctx.ia_set_params(g.TOL, flags=args.flags)
+    hd = ctx.to_device(b.hits_of(ev.wire, ev.drift))
+    b0, e0 = shard.slab_range(dims[0], rank, world)
+    col = n_cells // dims[0]
+    slab = torch.empty(max(e0 - b0, 1) * col, dtype=torch.uint16, device=f"cuda:{local_rank}")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local_rank}")
+    d = dist if world > 1 else None
+
+    def step():
+        return shard.split_vote_topk(ctx, hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, k, rank, world, d, votes_out=slab)
+
+    for _ in range(args.warmup):
+        step()
+        flush.zero_()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = ctx.ia_launch_count()
+    a, c = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(ctx.stream)
+    for _ in range(args.steps):
+        idx, vv, _ = step()
+        flush.zero_()
+    c.record(ctx.stream)
+    barrier()
+    launches = ctx.ia_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([a.elapsed_time(c)], dtype=torch.float64, device=f"cuda:{local_rank}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": evals_per_step / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: one event, dense {dims[0]}^5 x {ev.n_hits} hits, top-{k}, split along xc over "
+                                   f"{world} GPU(s)", "parallelism": f"ix-split x{world}: slab vote, {k} keys per rank all-gathered "
+                                   "(256 B per rank per step), merge on every rank", "evals_per_step": evals_per_step,
+                       "l2": "256 MiB flush buffer written between steps"},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "top": {"idx": [int(x) for x in idx.cpu().numpy()[:3]], "votes": [int(x) for x in vv.cpu().numpy()[:3]]}}))
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -463,6 +521,9 @@ def main():
     ap.add_argument("--f2-fixed-ref", action="store_true", help="workload F2: keep the reference point at (0,0) (no L98 update)")
     ap.add_argument("--f2-vertex", type=float, nargs=2, default=[0.0, 0.0], help="workload F2: emission point (x y) in cm (L123)")
     ap.add_argument("--flags", type=int, default=0, help="ia_params.flags for the dense workloads (1: general kernel, 16: rigorous Phi)")
+    ap.add_argument("--split-event", action="store_true",
+                    help="C0/C1/C4 with --gpus N: one event split along xc over the ranks (strong scaling, SURVEY 8(e)) "
+                         "instead of one event per rank (weak, the default)")
     ap.add_argument("--no-extras", action="store_true", help="skip events/s, e2e and cpu_baseline legs")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -528,6 +589,12 @@ def main():
         return
     if args.workload in ("C2", "C3"):
         run_c3(args, rank, world, local_rank, barrier)
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    if args.split_event:
+        run_split(args, rank, world, local_rank, barrier)
         if world > 1:
             dist.destroy_process_group()
         return

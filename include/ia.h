@@ -128,6 +128,15 @@ int ia_set_params(ia_ctx* ctx, const ia_params* params_host);
 int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
             const int32_t grid_dims[5], uint16_t* votes_out_dev);
 
+/* (e) SURVEY.md 8(e), "Dense vote: split the slowest axis (ix) across GPUs" - the same vote for the xc cells
+ * [ix_begin, ix_end) of the grid only.  Cell edges are those of the FULL grid (e_k = lo + k*w with w = (hi-lo)/n over
+ * all grid_dims[0] cells, G14), so the slabs of several calls - or of several GPUs - tile ia_vote's accumulator
+ * exactly, count for count.  votes_out_dev holds (ix_end - ix_begin)*ny*nR*nz*nl counts: the slab, in the layout of
+ * the full accumulator (a cell's index in it = its full-grid index - ix_begin*ny*nR*nz*nl).  An empty range is a no-op.
+ * Errors as ia_vote; IA_ERR_ARG for a range outside [0, grid_dims[0]]. */
+int ia_vote_slab(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
+                 const int32_t grid_dims[5], int ix_begin, int ix_end, uint16_t* votes_out_dev);
+
 /* Same vote on an explicit list of boxes: lo_dev/hi_dev are [n_boxes][5] doubles. */
 int ia_vote_boxes(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double* lo_dev, const double* hi_dev,
                   int64_t n_boxes, uint16_t* votes_out_dev);
@@ -217,6 +226,17 @@ int ia_track_paper(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, double momen
  * idx_out_dev[k] (int64 linear indices), votes_out_dev[k].  1 <= k <= min(n_cells, IA_MAX_K). */
 int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t* idx_out_dev,
             uint16_t* votes_out_dev);
+
+/* (e) SURVEY.md 8(e), the one exchange of the split dense vote ("all-gather of K (index, votes) pairs and a K-way
+ * merge").  ia_topk_keys: the k best cells of one slab as keys_out_dev[IA_KEY_LIST] (uint64, sorted descending;
+ * entries from k on are 0): key = votes << 48 | (2^48 - 1 - (index_base + index)) - larger key = more votes, then lower
+ * index, the selection order of ia_topk (L94, G16) - with index_base the slab's first cell in the full accumulator
+ * (ix_begin*ny*nR*nz*nl).  ia_merge_keys: n_lists such lists, rank after rank (what an all-gather of the lists
+ * delivers), merged into the k best cells of the whole accumulator, idx_out_dev[k] / votes_out_dev[k] as ia_topk
+ * writes them; entries of empty keys (fewer than k cells in all lists) come back as index 2^48 - 1, votes 0. */
+#define IA_KEY_LIST 32
+int ia_topk_keys(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t index_base, uint64_t* keys_out_dev);
+int ia_merge_keys(ia_ctx* ctx, const uint64_t* keys_dev, int n_lists, int k, int64_t* idx_out_dev, uint16_t* votes_out_dev);
 
 /* a8-a9 - adaptive refinement of one event, entirely on the device: vote the dense grid0, keep the
  * top k, then (levels-1) times: cut every kept box at its per-axis midpoints into 2^5 children

@@ -27,9 +27,11 @@ FIT_DT = np.dtype([("value", "f8", (4,)), ("error", "f8", (4,)), ("lam", "f8"), 
 PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,)), ("windowed", "i4"), ("move_ref", "i4")])
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 112
 
-EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
+EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_slab", "ia_topk_keys", "ia_merge_keys", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_residual_fast", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_graph_replays", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
+
+KEY_LIST = 32      # IA_KEY_LIST
 
 
 class IaParams(C.Structure):
@@ -63,6 +65,9 @@ def load_library(path: str = LIB_PATH):
     lib.ia_set_params.argtypes = [vp, C.POINTER(IaParams)]
     lib.ia_vote.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_vote_boxes.argtypes = [vp, vp, i32, vp, vp, i64, vp]
+    lib.ia_vote_slab.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp]
+    lib.ia_topk_keys.argtypes = [vp, vp, i64, i32, i64, vp]
+    lib.ia_merge_keys.argtypes = [vp, vp, i32, i32, vp, vp]
     lib.ia_vote_paper.argtypes = [vp, vp, i32, vp, dbl, dbl, vp, vp, vp, vp]
     lib.ia_select_max_paper.argtypes = [vp, vp, dbl, vp, vp, vp, i32, vp]
     lib.ia_track_paper.argtypes = [vp, vp, i32, dbl, dbl, dbl, vp, i32, vp, vp]
@@ -202,6 +207,32 @@ class Context:
             votes_out = self._empty(n, torch.uint16)
         self._chk(self.lib.ia_vote(self.h, _dp(hits_dev), n_hits, _hp(lo), _hp(hi), _hp(dims), _dp(votes_out)), "ia_vote")
         return votes_out
+
+    # ---- (e): the dense vote of the xc cells [ix_begin, ix_end) only, and the key lists that cross GPUs
+    def ia_vote_slab(self, hits_dev, n_hits, box_lo, box_hi, grid_dims, ix_begin, ix_end, votes_out=None):
+        torch = self._torch
+        lo, hi, dims = _host5(box_lo, np.float64), _host5(box_hi, np.float64), _host5(grid_dims, np.int32)
+        n = int(ix_end - ix_begin) * int(np.prod(dims[1:].astype(np.int64)))
+        if votes_out is None:
+            votes_out = self._empty(max(n, 0), torch.uint16)
+        self._chk(self.lib.ia_vote_slab(self.h, _dp(hits_dev), n_hits, _hp(lo), _hp(hi), _hp(dims), int(ix_begin), int(ix_end),
+                                        _dp(votes_out)), "ia_vote_slab")
+        return votes_out
+
+    def ia_topk_keys(self, votes_dev, k, index_base=0, n_cells=None, keys_out=None):
+        torch = self._torch
+        n = votes_dev.numel() if n_cells is None else n_cells
+        if keys_out is None:
+            keys_out = self._empty(KEY_LIST, torch.int64)          # uint64 keys carried as int64 bit patterns
+        self._chk(self.lib.ia_topk_keys(self.h, _dp(votes_dev), n, k, int(index_base), _dp(keys_out)), "ia_topk_keys")
+        return keys_out
+
+    def ia_merge_keys(self, keys_dev, n_lists, k):
+        torch = self._torch
+        idx = self._empty(max(k, 1), torch.int64)
+        v = self._empty(max(k, 1), torch.uint16)
+        self._chk(self.lib.ia_merge_keys(self.h, _dp(keys_dev), int(n_lists), k, _dp(idx), _dp(v)), "ia_merge_keys")
+        return idx, v
 
     # ---- f1: the paper's own configuration (4-D voxels, mid-voxel d_Ax, two lambda-sign accumulators)
     def ia_vote_paper(self, hits_dev, n_hits, momentum_radius, box_lo, box_hi, grid_dims, votes_out=None, hit_mask_dev=None,

@@ -53,6 +53,8 @@ int make_grid(const double lo[5], const double hi[5], const int32_t n[5], GridDe
     g.cells *= n[d];
   }
   g.col_cells = int64_t(n[2]) * n[3] * n[4];
+  g.ix0 = 0;
+  g.nx_run = n[0];
   if (int64_t(n[0]) * n[1] * ((g.col_cells + 1023) / 1024) > 0x7fffffffLL) return IA_ERR_CAPACITY;
   return IA_OK;
 }
@@ -283,6 +285,31 @@ int ia_vote(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo
   return IA_OK;
 }
 
+int ia_vote_slab(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const double box_lo[5], const double box_hi[5],
+                 const int32_t grid_dims[5], int ix_begin, int ix_end, uint16_t* votes_out_dev) {
+  int rc = check_ready(ctx);
+  if (rc) return rc;
+  if (n_hits < 0 || (n_hits > 0 && !hits_dev) || !votes_out_dev) return IA_ERR_ARG;
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  GridDesc g;
+  rc = make_grid(box_lo, box_hi, grid_dims, g);
+  if (rc) return rc;
+  if (ix_begin < 0 || ix_end > g.n[0] || ix_begin > ix_end) return IA_ERR_ARG;
+  rc = check_domain(ctx, box_lo, box_hi);
+  if (rc) return rc;
+  if (ix_begin == ix_end) return IA_OK;                   // an empty slab (more ranks than xc cells)
+  // the edges stay those of the full grid (cell_edge with n[0] cells on [lo[0], hi[0]], G14); only the range of xc
+  // cells and the accumulator the blocks write - the slab - change
+  g.ix0 = ix_begin;
+  g.nx_run = ix_end - ix_begin;
+  g.cells = int64_t(g.nx_run) * g.n[1] * g.col_cells;
+  DeviceGuard guard(ctx->device);
+  HitSpan sp = single_span(hits_dev, n_hits);
+  IA_CUDA(ctx, launch_stage_hits(ctx, sp));
+  IA_CUDA(ctx, launch_vote_dense(ctx, sp, g, votes_out_dev));
+  return IA_OK;
+}
+
 static int make_grid4(const double box_lo[4], const double box_hi[4], const int32_t grid_dims[4], GridDesc& g) {
   if (!box_lo || !box_hi || !grid_dims) return IA_ERR_ARG;
   const double lo5[5] = {box_lo[0], box_lo[1], box_lo[2], box_lo[3], 0.0};
@@ -411,6 +438,24 @@ int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int6
   if (k > IA_MAX_K || n_cells > (int64_t(1) << 40)) return IA_ERR_CAPACITY;
   DeviceGuard guard(ctx->device);
   IA_CUDA(ctx, launch_topk(ctx, votes_dev, n_cells, 1, k, idx_out_dev, votes_out_dev));
+  return IA_OK;
+}
+
+int ia_topk_keys(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t index_base, uint64_t* keys_out_dev) {
+  if (!ctx || !votes_dev || !keys_out_dev || n_cells <= 0 || k <= 0 || k > n_cells || index_base < 0) return IA_ERR_ARG;
+  if (k > IA_MAX_K || n_cells > (int64_t(1) << 40) || index_base > (int64_t(1) << 40)) return IA_ERR_CAPACITY;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_topk(ctx, votes_dev, n_cells, 1, k, nullptr, nullptr, index_base,
+                           reinterpret_cast<unsigned long long*>(keys_out_dev)));
+  return IA_OK;
+}
+
+int ia_merge_keys(ia_ctx* ctx, const uint64_t* keys_dev, int n_lists, int k, int64_t* idx_out_dev, uint16_t* votes_out_dev) {
+  if (!ctx || !keys_dev || !idx_out_dev || !votes_out_dev || n_lists <= 0 || k <= 0) return IA_ERR_ARG;
+  if (k > IA_MAX_K || n_lists > 65535) return IA_ERR_CAPACITY;
+  DeviceGuard guard(ctx->device);
+  IA_CUDA(ctx, launch_merge_keys(ctx, reinterpret_cast<const unsigned long long*>(keys_dev), n_lists, k, idx_out_dev,
+                                 votes_out_dev));
   return IA_OK;
 }
 

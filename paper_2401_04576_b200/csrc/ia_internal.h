@@ -11,8 +11,10 @@ namespace ia {
 struct GridDesc {
   double lo[5], hi[5], w[5];
   int32_t n[5];
-  int64_t cells;      // prod(n)
+  int64_t cells;      // prod(n); for a slab (ia_vote_slab): the cells of the slab = the accumulator the vote writes
   int64_t col_cells;  // n[2]*n[3]*n[4]: cells of one (xc, yc) column
+  int32_t ix0;        // dense vote: first xc cell voted and how many (the whole axis: 0, n[0]); edges are always those
+  int32_t nx_run;     // of the full grid (n[0] cells on [lo[0], hi[0]])
 };
 
 // where the hits of event e live: staged[e*max_hits + i], i < count(e)
@@ -101,8 +103,12 @@ cudaError_t launch_residual_fast(ia_ctx* ctx, const HitSpan& span, const double*
 cudaError_t launch_prim(ia_ctx* ctx, int op, int prec, const double* a, const double* b, int64_t n, double* out);
 
 // top-K of n_events independent arrays of n entries each (stride n): idx_out/votes_out [n_events][k]
+// idx_base: added to every index (a slab of a larger accumulator); keys_out != nullptr: write the sorted 32-key list
+// per event (first k entries, the rest 0) instead of idx_out/votes_out
 cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_events, int k, int64_t* idx_out,
-                        uint16_t* votes_out);
+                        uint16_t* votes_out, int64_t idx_base = 0, unsigned long long* keys_out = nullptr);
+cudaError_t launch_merge_keys(ia_ctx* ctx, const unsigned long long* keys, int n_lists, int k, int64_t* idx_out,
+                              uint16_t* votes_out);
 
 // refinement steps (a8-a9)
 cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* idx, const uint16_t* v, int n_events,

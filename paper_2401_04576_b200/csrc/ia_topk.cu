@@ -36,8 +36,8 @@ constexpr int TOPK_UNROLL = IA_TOPK_UNROLL;      // 16-byte loads in flight per 
 // own and reached 37 % of the HBM rate).  All loads of a group are issued before the first is looked at.
 template <int U>
 __global__ void __launch_bounds__(TOPK_THREADS)
-topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, u64* __restrict__ partial,
-             int64_t* __restrict__ idx_out, uint16_t* __restrict__ votes_out, int write_final) {
+topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, int64_t idx_base, u64* __restrict__ partial,
+             int64_t* __restrict__ idx_out, uint16_t* __restrict__ votes_out, u64* __restrict__ keys_out, int write_final) {
   __shared__ u64 smem_keys[(TOPK_THREADS / 32) * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int e = blockIdx.y;
@@ -53,7 +53,7 @@ topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, u64* __restri
   if (gw == 0) {
     for (int64_t i = 0; i < head; i += 32) {
       const int64_t idx = i + lane;
-      warp_offer(mine, kth, idx < head ? make_key(v[idx], idx) : 0, k);
+      warp_offer(mine, kth, idx < head ? make_key(v[idx], idx_base + idx) : 0, k);
     }
   }
   for (int64_t c0 = gw * U; c0 < n_chunks; c0 += n_warps * U) {
@@ -66,20 +66,22 @@ topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, u64* __restri
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       if (c0 + u >= n_chunks) break;
-      const int64_t idx0 = head + (c0 + u) * 256 + 8 * lane;
+      const int64_t idx0 = idx_base + head + (c0 + u) * 256 + 8 * lane;
       warp_offer_8(mine, kth, q[u], idx0, bound_of_8(q[u], idx0) > kth, k);
     }
   }
   if (gw == n_warps - 1) {
     for (int64_t i = head + n_chunks * 256; i < n; i += 32) {
       const int64_t idx = i + lane;
-      warp_offer(mine, kth, idx < n ? make_key(v[idx], idx) : 0, k);
+      warp_offer(mine, kth, idx < n ? make_key(v[idx], idx_base + idx) : 0, k);
     }
   }
   mine = block_merge(mine, smem_keys);
   if (warp == 0) {
     if (write_final) {
-      if (lane < k) {
+      if (keys_out) {
+        keys_out[int64_t(e) * 32 + lane] = lane < k ? mine : 0;       // only the first k of a list are exact
+      } else if (lane < k) {
         idx_out[int64_t(e) * k + lane] = key_index(mine);
         votes_out[int64_t(e) * k + lane] = key_votes(mine);
       }
@@ -92,7 +94,7 @@ topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, u64* __restri
 // grid (n_events); merges n_lists lists of 32 keys
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_final(const u64* __restrict__ partial, int n_lists, int k, int64_t* __restrict__ idx_out,
-           uint16_t* __restrict__ votes_out) {
+           uint16_t* __restrict__ votes_out, u64* __restrict__ keys_out) {
   __shared__ u64 smem_keys[(TOPK_THREADS / 32) * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int e = blockIdx.x;
@@ -100,16 +102,20 @@ topk_final(const u64* __restrict__ partial, int n_lists, int k, int64_t* __restr
   u64 mine = 0;
   for (int l = warp; l < n_lists; l += TOPK_THREADS / 32) mine = warp_merge_desc(mine, p[l * 32 + lane]);
   mine = block_merge(mine, smem_keys);
-  if (warp == 0 && lane < k) {
-    idx_out[int64_t(e) * k + lane] = key_index(mine);
-    votes_out[int64_t(e) * k + lane] = key_votes(mine);
+  if (warp == 0) {
+    if (keys_out) {
+      keys_out[int64_t(e) * 32 + lane] = lane < k ? mine : 0;
+    } else if (lane < k) {
+      idx_out[int64_t(e) * k + lane] = key_index(mine);
+      votes_out[int64_t(e) * k + lane] = key_votes(mine);
+    }
   }
 }
 
 }  // namespace
 
 cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_events, int k, int64_t* idx_out,
-                        uint16_t* votes_out) {
+                        uint16_t* votes_out, int64_t idx_base, unsigned long long* keys_out) {
   // 2 blocks per SM over all events, never more than there are groups of chunks (measured on the 2.1 GB accumulator of
   // C4, loads in flight per lane x blocks per SM: 4x8 0.468 ms, 8x4 0.402, 8x2 0.404, 8x3 0.388, 16x2 0.407, 8x1 0.552;
   // on random votes 8x2 is the fastest, 0.396 ms = 5.4 TB/s)
@@ -132,12 +138,20 @@ cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_eve
     partial = static_cast<u64*>(ctx->keys.p);
   }
   dim3 grid((unsigned)blocks, (unsigned)n_events);
-  if (unroll == 1) topk_partial<1><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, partial, idx_out, votes_out, write_final);
-  else topk_partial<TOPK_UNROLL><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, partial, idx_out, votes_out, write_final);
+  if (unroll == 1) topk_partial<1><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, idx_base, partial, idx_out, votes_out, keys_out, write_final);
+  else topk_partial<TOPK_UNROLL><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, idx_base, partial, idx_out, votes_out, keys_out, write_final);
   ctx->launches++;
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess || write_final) return err;
-  topk_final<<<n_events, TOPK_THREADS, 0, ctx->stream>>>(partial, int(blocks), k, idx_out, votes_out);
+  topk_final<<<n_events, TOPK_THREADS, 0, ctx->stream>>>(partial, int(blocks), k, idx_out, votes_out, keys_out);
+  ctx->launches++;
+  return cudaGetLastError();
+}
+
+// key lists of several accumulators (the slabs of a split vote, gathered from their GPUs) -> the k best of their union
+cudaError_t launch_merge_keys(ia_ctx* ctx, const unsigned long long* keys, int n_lists, int k, int64_t* idx_out,
+                              uint16_t* votes_out) {
+  topk_final<<<1, TOPK_THREADS, 0, ctx->stream>>>(keys, n_lists, k, idx_out, votes_out, nullptr);
   ctx->launches++;
   return cudaGetLastError();
 }

@@ -36,7 +36,8 @@ vote_dense_general_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDe
   const int64_t bid = blockIdx.x;
   const int64_t ixy = bid / chunks_per_col;
   const int chunk = int(bid - ixy * chunks_per_col);
-  const int ix = int(ixy / g.n[1]), iy = int(ixy - int64_t(ix) * g.n[1]);
+  const int ixl = int(ixy / g.n[1]), iy = int(ixy - int64_t(ixl) * g.n[1]);
+  const int ix = g.ix0 + ixl;                                   // ixy counts inside the slab, ix in the full grid
   int count;
   if (sp.offsets) {
     count = sp.offsets[e + 1] - sp.offsets[e];
@@ -184,7 +185,8 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
   const int tz = int(bid % tiles_z); bid /= tiles_z;
   const int tp = int(bid % tiles_p); bid /= tiles_p;
   const int64_t ixy = bid;
-  const int ix = int(ixy / g.n[1]), iy = int(ixy - int64_t(ix) * g.n[1]);
+  const int ixl = int(ixy / g.n[1]), iy = int(ixy - int64_t(ixl) * g.n[1]);
+  const int ix = g.ix0 + ixl;                                   // ixy counts inside the slab, ix in the full grid
   int count;
   if (sp.offsets) {
     count = sp.offsets[e + 1] - sp.offsets[e];
@@ -489,11 +491,11 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
   int zt = FAST_ZT;
   {
-    const int64_t base = int64_t(g.n[0]) * g.n[1] * ((n_pairs + FAST_THREADS - 1) / FAST_THREADS) * sp.n_events;
+    const int64_t base = int64_t(g.nx_run) * g.n[1] * ((n_pairs + FAST_THREADS - 1) / FAST_THREADS) * sp.n_events;
     while (zt > 1 && base * ((g.n[3] + zt - 1) / zt) < int64_t(8) * n_sm) zt >>= 1;
   }
   const int tiles_z = (g.n[3] + zt - 1) / zt;
-  const int64_t nxy = int64_t(g.n[0]) * g.n[1];
+  const int64_t nxy = int64_t(g.nx_run) * g.n[1];
   const int64_t blocks = nxy * tiles_p * tiles_z;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   // still too few warps to hide the latency of a thread's serial chain over its hits (one event on a coarse grid):
@@ -553,7 +555,7 @@ template <class T>
 static cudaError_t launch_general(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g, uint16_t* votes_out) {
   const int per_block = GEN_THREADS * GEN_CELLS_PER_THREAD;
   const int chunks = int((g.col_cells + per_block - 1) / per_block);
-  const int64_t nxy = int64_t(g.n[0]) * g.n[1];
+  const int64_t nxy = int64_t(g.nx_run) * g.n[1];
   dim3 grid((unsigned)(nxy * chunks), (unsigned)sp.n_events);
   const size_t smem = size_t(sp.max_hits) * sizeof(HitShared<T>);
   cudaError_t err = cudaFuncSetAttribute(vote_dense_general_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));

@@ -1,9 +1,11 @@
-"""Host-side sharding of independent events across ranks.
+"""Host-side sharding across ranks.
 
-The path partitions by event: every rank refines its own contiguous range of events with no
-exchange on the data path.  What crosses ranks is bookkeeping only: the results are gathered on
-rank 0 and the step time is the maximum over ranks.  Works with any torch.distributed backend
-(nccl on GPUs, gloo in the CPU tests); holds none of the method's arithmetic.
+Independent events: every rank refines its own contiguous range of events with no exchange on the data path; the results
+are gathered on rank 0 and the step time is the maximum over ranks.
+One event on several GPUs: the dense vote is split along its slowest axis (xc); every rank votes its
+slab (ia_vote_slab), reduces it to its K best keys (ia_topk_keys), the key lists - 256 bytes per rank - are all-gathered
+(the one exchange of the path) and merged by every rank (ia_merge_keys).  Works with any torch.distributed backend (nccl
+on GPUs, gloo in the CPU tests); holds none of the method's arithmetic: votes, keys and the merge are the library's.
 """
 from __future__ import annotations
 
@@ -49,3 +51,43 @@ def gather_results(local: np.ndarray, n_events: int, dist=None):
     if out.shape[0] != n_events:
         raise RuntimeError(f"gathered {out.shape[0]} events, expected {n_events}")
     return out
+
+
+def slab_range(nx: int, rank: int, world: int) -> tuple[int, int]:
+    """xc cells [begin, end) of rank `rank` in a dense vote split over `world` ranks (balanced, contiguous; a rank may get
+    none when world > nx)."""
+    return event_range(nx, rank, world)
+
+
+def gather_key_lists(keys_local, dist=None):
+    """All-gather of the per-rank key lists (ia_topk_keys: IA_KEY_LIST uint64 carried as int64) -> one tensor
+    [world * IA_KEY_LIST] in rank order on every rank.  A rank with an empty slab contributes zeros (empty keys)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return keys_local
+    import torch
+    world = dist.get_world_size()
+    out = torch.empty(world * keys_local.numel(), dtype=keys_local.dtype, device=keys_local.device)
+    dist.all_gather_into_tensor(out, keys_local.contiguous())
+    return out
+
+
+def split_vote_topk(ctx, hits_dev, n_hits, box_lo, box_hi, grid_dims, k, rank=0, world=1, dist=None, votes_out=None):
+    """The K best cells of ONE event's dense vote computed by `world` GPUs: slab vote, local key list, all-gather, merge.
+    Returns (idx[k], votes[k]) - identical on every rank and identical to ia_vote + ia_topk on one GPU - and the rank's
+    slab accumulator.  Every step is a call of the C ABI on ctx's stream; the all-gather runs on torch's current stream,
+    so the caller's streams must be ordered (bench.py and the tests use one stream for both)."""
+    import torch
+    dims = [int(d) for d in grid_dims]
+    b, e = slab_range(dims[0], rank, world)
+    col = 1
+    for d in dims[1:]:
+        col *= d
+    if e > b:
+        votes = ctx.ia_vote_slab(hits_dev, n_hits, box_lo, box_hi, dims, b, e, votes_out=votes_out)
+        keys = ctx.ia_topk_keys(votes, min(k, (e - b) * col), index_base=b * col, n_cells=(e - b) * col)
+    else:
+        votes = None
+        keys = torch.zeros(32, dtype=torch.int64, device=f"cuda:{ctx.device}")
+    all_keys = gather_key_lists(keys, dist)
+    idx, v = ctx.ia_merge_keys(all_keys, all_keys.numel() // 32, k)
+    return idx, v, votes

@@ -729,3 +729,49 @@ def test_prefilter_gives_identical_votes(precision):
                 assert a.max() > 0
         finally:
             rig.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_slab_votes_tile_the_accumulator_and_key_lists_merge_to_the_same_topk(precision):
+    """SURVEY 8(e), one event on several GPUs: the slabs of ia_vote_slab (2, 3, 5 and 8 "ranks", run one after the other on
+    this GPU - no rank waits for another) concatenate to ia_vote's accumulator count for count, the merged key lists of
+    ia_topk_keys give ia_topk's result on the whole accumulator, and that is the oracle's top-K of the oracle's votes."""
+    import torch
+    from paper_2401_04576_b200 import shard
+    rig = Rig(g.chamber_c1(), precision=precision)
+    try:
+        ev = g.make_event(rig.ch, 11, n_noise=20)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        for dims, k in (((12, 10, 12, 12, 12), 10), ((5, 7, 6, 9, 3), 32), ((3, 4, 8, 8, 8), 16)):
+            full = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            idx_f, v_f = rig.ctx.ia_topk(full, k)
+            rig.ctx.synchronize()
+            col = int(np.prod(dims[1:]))
+            for world in (2, 3, 5, 8):
+                slabs, lists = [], []
+                for rank in range(world):
+                    b0, e0 = shard.slab_range(dims[0], rank, world)
+                    if e0 > b0:
+                        vs = rig.ctx.ia_vote_slab(hd, ev.n_hits, LO, HI, dims, b0, e0)
+                        lists.append(rig.ctx.ia_topk_keys(vs, min(k, (e0 - b0) * col), index_base=b0 * col))
+                        slabs.append(vs)
+                    else:
+                        lists.append(torch.zeros(32, dtype=torch.int64, device="cuda"))
+                rig.ctx.synchronize()
+                assert torch.equal(torch.cat(slabs).view(torch.int16), full.view(torch.int16)), (dims, world)
+                idx_m, v_m = rig.ctx.ia_merge_keys(torch.cat(lists), world, k)
+                rig.ctx.synchronize()
+                assert torch.equal(idx_m, idx_f) and torch.equal(v_m.view(torch.int16), v_f.view(torch.int16)), (dims, world)
+            # the single-process form of the whole split path
+            idx_s, v_s, _ = shard.split_vote_topk(rig.ctx, hd, ev.n_hits, LO, HI, dims, k)
+            rig.ctx.synchronize()
+            assert torch.equal(idx_s, idx_f)
+            vo = o.vote(rig.owires, oh, rig.oparams, LO, HI, dims)
+            eidx, evv = o.topk(full.cpu().numpy(), k)
+            assert (idx_f.cpu().numpy() == eidx).all() and (v_f.cpu().numpy() == evv).all()
+            assert (full.cpu().numpy() == vo).mean() >= 0.9999
+        # errors: a range outside the axis
+        with pytest.raises(b.IaError):
+            rig.ctx.ia_vote_slab(hd, ev.n_hits, LO, HI, (4, 4, 4, 4, 4), 2, 5)
+    finally:
+        rig.close()

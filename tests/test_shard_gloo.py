@@ -64,3 +64,42 @@ def test_two_ranks_gloo():
     assert t == 1.5                                      # max over ranks
     assert out.shape == (n_events, 2) and (out[:, 0] == np.arange(n_events)).all()
     assert out[:4, 1].tolist() == [0.0] * 4 and out[4:, 1].tolist() == [1.0] * 3
+
+
+def _keys_worker(rank, world, port, q):
+    import torch
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # stand-in for a rank's ia_topk_keys list: 32 int64 "keys" that name the rank
+        local = torch.arange(32, dtype=torch.int64) + 1000 * (rank + 1)
+        out = shard.gather_key_lists(local, dist)
+        if rank == 0:
+            q.put(out.numpy())
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_key_lists_are_gathered_in_rank_order_gloo():
+    """the one exchange of the split dense vote: every rank ends up with all lists, rank after rank"""
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_keys_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    out = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert out.shape == (64,)
+    assert (out[:32] == np.arange(32) + 1000).all() and (out[32:] == np.arange(32) + 2000).all()
+
+
+def test_slab_ranges_tile_the_axis():
+    for nx in (1, 3, 8, 64):
+        for world in (1, 2, 3, 8):
+            r = [shard.slab_range(nx, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == nx and all(r[i][1] == r[i + 1][0] for i in range(world - 1))
