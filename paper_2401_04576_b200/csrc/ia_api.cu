@@ -577,7 +577,7 @@ int ia_residual_fast(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const doub
 }
 
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev) {
-  if (!ctx || !a_dev || !out_dev || n < 0 || op < 0 || op > 17 || (prec != 64 && prec != 32)) return IA_ERR_ARG;
+  if (!ctx || !a_dev || !out_dev || n < 0 || op < 0 || op > 19 || (prec != 64 && prec != 32)) return IA_ERR_ARG;
   const bool binary = (op == 0 || op == 1 || op == 2 || op == 4 || op == 8 || op == 10 || op == 11 || op == 12 || op == 13);
   if (binary && !b_dev) return IA_ERR_ARG;
   DeviceGuard guard(ctx->device);

@@ -330,8 +330,36 @@ static __constant__ double IA_SIN_C[5] = {-2.5052108385441720e-08, 2.75573192239
 //                                        1/12!                   -1/10!                   1/8!                    -1/6!                    1/4!
 static __constant__ double IA_COS_C[6] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05, -1.3888888888888889e-03,
                                           4.1666666666666664e-02, -0.5};
+// Medium range, |x| < 1 (double only; round 2): terms to x^19 / x^20 - truncation x^21/21! < 2e-20 |x| and x^22/22! < 1e-21;
+// rounding, with u = 2^-53: sin = x + x^3 q: |error| <= 0.84 u |x| (x^3 q, |q| <= 1/6) + u |sin x| <= 2 u |sin x| as
+// sin x >= 0.84 |x|; cos = 1 + x^2 r: |error| <= 2.1 u (x^2 r with |r| <= 1/2, last two Horner steps, the final FMA)
+// <= 3.9 u cos x as cos x >= 0.54 - both inside the relative pad 2^-50 = 8 u.  On the 8^5 start grid of a refinement 11 %
+// of the warp-evaluations have a lane with |e| in [1/4, 1) and took the general form for it (library sin/cos and two
+// general products: 720 warp-instructions against 100 here; profiles/).
+//                                        -1/19!                  1/17!                   -1/15!                  1/13!
+static __constant__ double IA_SIN_M[9] = {-8.22063524662433e-18, 2.8114572543455206e-15, -7.647163731819816e-13, 1.6059043836821613e-10,
+//                                        -1/11!                  1/9!                    -1/7!                   1/5!                  -1/3!
+                                          -2.505210838544172e-08, 2.7557319223985893e-06, -0.0001984126984126984, 0.008333333333333333,
+                                          -0.16666666666666666};
+//                                         1/20!                  -1/18!                   1/16!                  -1/14!
+static __constant__ double IA_COS_M[10] = {4.110317623312165e-19, -1.5619206968586225e-16, 4.779477332387385e-14, -1.1470745597729725e-11,
+//                                         1/12!                 -1/10!                  1/8!                  -1/6!                   1/4!
+                                           2.08767569878681e-09, -2.755731922398589e-07, 2.48015873015873e-05, -0.001388888888888889,
+                                           0.041666666666666664, -0.5};
 template <class T> struct Trig;
 template <> struct Trig<double> {
+  static IA_DEV double sin_medium(double x, double s) {
+    double q = __fma_rn(IA_SIN_M[0], s, IA_SIN_M[1]);
+#pragma unroll
+    for (int k = 2; k < 9; ++k) q = __fma_rn(q, s, IA_SIN_M[k]);
+    return __fma_rn(__dmul_rn(x, s), q, x);
+  }
+  static IA_DEV double cos_medium(double s) {
+    double q = __fma_rn(IA_COS_M[0], s, IA_COS_M[1]);
+#pragma unroll
+    for (int k = 2; k < 10; ++k) q = __fma_rn(q, s, IA_COS_M[k]);
+    return __fma_rn(q, s, 1.0);
+  }
   static IA_DEV double sqr(double x) { return __dmul_rn(x, x); }
   static IA_DEV double sin_small(double x, double s) {
     double q = __fma_rn(IA_SIN_C[0], s, IA_SIN_C[1]);
@@ -377,6 +405,18 @@ template <class T> IA_DEV void trig_small(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
   const T chi = pad_up(c ? c1 : c0);
   ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? T(1) : chi};   // cos > 0.96
 }
+
+// the same over e inside (-1, 1), double only (prim op 18 / 19; the kernels use the quad form in ia_fastq.cuh)
+IA_DEV void trig_medium(Iv<double> e, Iv<double>& se, Iv<double>& ce) {
+  const double s0 = Trig<double>::sqr(e.lo), s1 = Trig<double>::sqr(e.hi);
+  se = {pad_dn(Trig<double>::sin_medium(e.lo, s0)), pad_up(Trig<double>::sin_medium(e.hi, s1))};
+  const double c0 = Trig<double>::cos_medium(s0), c1 = Trig<double>::cos_medium(s1);
+  const bool c = nn_gt(s0, s1);
+  const bool straddle = sgn(e.lo) != sgn(e.hi);
+  const double chi = pad_up(c ? c1 : c0);
+  ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? 1.0 : chi};
+}
+IA_DEV void trig_medium(Iv<float> e, Iv<float>& se, Iv<float>& ce) { se = isin(e); ce = icos(e); }   // not used in float
 
 // ---- the FP32 fast form as a floating-point filter ---------------------------------------------------
 // The sign-specialised form and the general form enclose the same function but round differently (fused FMAs, midpoint-

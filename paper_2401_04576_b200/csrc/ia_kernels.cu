@@ -156,6 +156,8 @@ __global__ void prim_kernel(int op, const double* __restrict__ a, const double* 
     case 15: { Iv<T> c; trig_small(x, r, c); break; }        // sin over x inside [-1/4, 1/4]
     case 16: { Iv<T> s; trig_small(x, s, r); break; }        // cos
     case 17: r = clamp_unit(x); break;
+    case 18: { Iv<T> c; trig_medium(x, r, c); break; }       // sin over x inside (-1, 1) (double)
+    case 19: { Iv<T> s; trig_medium(x, s, r); break; }       // cos
     default: break;
   }
   out[2 * i] = double(r.lo);

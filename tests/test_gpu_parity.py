@@ -433,7 +433,7 @@ def test_one_body_and_three_body_variants_identical(precision):
         rig.close()
 
 
-PROD_P, PROD_U, D_OVER_SQRT, SQR_U, SIN_SMALL, COS_SMALL, CLAMP_UNIT = 11, 12, 13, 14, 15, 16, 17
+PROD_P, PROD_U, D_OVER_SQRT, SQR_U, SIN_SMALL, COS_SMALL, CLAMP_UNIT, SIN_MEDIUM, COS_MEDIUM = 11, 12, 13, 14, 15, 16, 17, 18, 19
 
 
 @pytest.mark.parametrize("prec", [64, 32])
@@ -499,6 +499,30 @@ def test_fast_path_primitives(rig0, prec):
         cmax = mp.mpf(1) if lo <= 0 <= hi else mp.cos(min(abs(lo), abs(hi)))
         assert mp.mpf(cc[i, 0]) <= cmin and cmax <= mp.mpf(cc[i, 1]) and cc[i, 1] <= 1.0, (e[i], cc[i])
         assert cmin - mp.mpf(cc[i, 0]) <= 10 * eps and mp.mpf(cc[i, 1]) - cmax <= 10 * eps, (e[i], cc[i])
+    # the medium tier (double only): sin / cos inside (-1, 1) by the longer polynomials - contains the truth, and is at most
+    # 10 ulps of the result (sin) / of 1 (cos) wider: the relative pad 2^-50 = 8 half-ulps plus the polynomial's own error
+    if prec == 64:
+        c = rng.uniform(-1.0, 1.0, n)
+        w = rng.choice([0.0, 1e-12, 1e-6, 1e-3, 0.05, 0.5, 2.0], size=n) * rng.random(n)
+        lim = float(np.nextafter(1.0, 0.0))
+        e = np.clip(np.stack([c - w, c + w], 1), -lim, lim)
+        e[:10] = [[-lim, lim]] * 10
+        e[10:20] = np.stack([np.zeros(10), np.abs(e[10:20, 1])], 1)
+        e[20:30] = np.stack([-np.abs(e[20:30, 0]), -np.zeros(10)], 1)
+        e[30:40] = [[lim, lim]] * 10
+        s = ctx.ia_prim(SIN_MEDIUM, prec, rig0.dev(e)).cpu().numpy()
+        cc = ctx.ia_prim(COS_MEDIUM, prec, rig0.dev(e)).cpu().numpy()
+        for i in range(n):
+            lo, hi = mp.mpf(e[i, 0]), mp.mpf(e[i, 1])
+            assert mp.mpf(s[i, 0]) <= mp.sin(lo) and mp.sin(hi) <= mp.mpf(s[i, 1]), (e[i], s[i])
+            assert mp.sin(lo) - mp.mpf(s[i, 0]) <= 10 * eps * max(abs(mp.sin(lo)), mp.mpf(2) ** -1000), (e[i], s[i])
+            assert mp.mpf(s[i, 1]) - mp.sin(hi) <= 10 * eps * max(abs(mp.sin(hi)), mp.mpf(2) ** -1000), (e[i], s[i])
+            cmin = mp.cos(max(abs(lo), abs(hi)))
+            cmax = mp.mpf(1) if lo <= 0 <= hi else mp.cos(min(abs(lo), abs(hi)))
+            assert mp.mpf(cc[i, 0]) <= cmin and cmax <= mp.mpf(cc[i, 1]) and cc[i, 1] <= 1.0, (e[i], cc[i])
+            assert cmin - mp.mpf(cc[i, 0]) <= 10 * eps and mp.mpf(cc[i, 1]) - cmax <= 10 * eps, (e[i], cc[i])
+            # the polynomial alone stays well inside the pad: the padded endpoint is at least 2 half-ulps beyond the truth
+            assert mp.sin(hi) - mp.mpf(s[i, 1]) <= 0 and cmin - mp.mpf(cc[i, 0]) >= 2 * (eps / 2) * cmin, (e[i], cc[i])
 
 
 def test_refine_graph_replay_gives_the_same_boxes(rig1):
