@@ -287,7 +287,7 @@ int ia_residual_fast(ia_ctx* ctx, const ia_hit* hits_dev, int n_hits, const doub
  *     11 a*b with a >= 0 taken in midpoint-radius form  12 the same for a of any sign
  *     13 a / sqrt(b) for a >= 0 and b in [1/4, 4] (delta = d_St/u_d of S6, one fused enclosure)
  *     14 sqr(a) branch-free  15 sin(a), 16 cos(a) for a inside [-1/4, 1/4] (Taylor, padded)
- *     17 a intersected with [-1, 1]  18 sin(a), 19 cos(a) for a inside (-1, 1), prec 64 (longer Taylor forms, padded) */
+ *     17 a intersected with [-1, 1]  18 sin(a), 19 cos(a) for a inside (-1, 1) (longer Taylor forms, padded) */
 int ia_prim(ia_ctx* ctx, int op, int prec, const double* a_dev, const double* b_dev, int64_t n, double* out_dev);
 
 /* Roofline probe: enqueue a kernel of `blocks` x 256 threads, each running 8 independent FP64

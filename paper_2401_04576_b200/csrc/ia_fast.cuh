@@ -330,7 +330,7 @@ static __constant__ double IA_SIN_C[5] = {-2.5052108385441720e-08, 2.75573192239
 //                                        1/12!                   -1/10!                   1/8!                    -1/6!                    1/4!
 static __constant__ double IA_COS_C[6] = {2.0876756987868100e-09, -2.7557319223985888e-07, 2.4801587301587302e-05, -1.3888888888888889e-03,
                                           4.1666666666666664e-02, -0.5};
-// Medium range, |x| < 1 (double only; round 2): terms to x^19 / x^20 - truncation x^21/21! < 2e-20 |x| and x^22/22! < 1e-21;
+// Medium range, |x| < 1 (round 2; the float form is in Trig<float>): terms to x^19 / x^20 - truncation x^21/21! < 2e-20 |x| and x^22/22! < 1e-21;
 // rounding, with u = 2^-53: sin = x + x^3 q: |error| <= 0.84 u |x| (x^3 q, |q| <= 1/6) + u |sin x| <= 2 u |sin x| as
 // sin x >= 0.84 |x|; cos = 1 + x^2 r: |error| <= 2.1 u (x^2 r with |r| <= 1/2, last two Horner steps, the final FMA)
 // <= 3.9 u cos x as cos x >= 0.54 - both inside the relative pad 2^-50 = 8 u.  On the 8^5 start grid of a refinement 11 %
@@ -378,6 +378,22 @@ template <> struct Trig<double> {
   }
 };
 template <> struct Trig<float> {
+  // medium range in float: terms to x^11 / x^12 (truncation x^13/13! < 1.7e-10, x^14/14! < 1.2e-11 against 2^-24 = 6e-8); the
+  // rounding bound is the double one with u = 2^-24: 2 u |sin x|, 3.9 u cos x, inside the relative pad 2^-21 = 8 u
+  static IA_DEV float sm(int k) { const float c[5] = {-2.5052108e-08f, 2.7557319e-06f, -1.9841270e-04f, 8.3333338e-03f, -1.6666667e-01f}; return c[k]; }
+  static IA_DEV float cm(int k) { const float d[6] = {2.0876757e-09f, -2.7557319e-07f, 2.4801588e-05f, -1.3888889e-03f, 4.1666668e-02f, -0.5f}; return d[k]; }
+  static IA_DEV float sin_medium(float x, float s) {
+    float q = __fmaf_rn(sm(0), s, sm(1));
+#pragma unroll
+    for (int k = 2; k < 5; ++k) q = __fmaf_rn(q, s, sm(k));
+    return __fmaf_rn(__fmul_rn(x, s), q, x);
+  }
+  static IA_DEV float cos_medium(float s) {
+    float q = __fmaf_rn(cm(0), s, cm(1));
+#pragma unroll
+    for (int k = 2; k < 6; ++k) q = __fmaf_rn(q, s, cm(k));
+    return __fmaf_rn(q, s, 1.0f);
+  }
   static IA_DEV float sqr(float x) { return __fmul_rn(x, x); }
   static IA_DEV float sin_small(float x, float s) {
     float q = -1.9841270e-04f;
@@ -406,17 +422,16 @@ template <class T> IA_DEV void trig_small(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
   ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? T(1) : chi};   // cos > 0.96
 }
 
-// the same over e inside (-1, 1), double only (prim op 18 / 19; the kernels use the quad form in ia_fastq.cuh)
-IA_DEV void trig_medium(Iv<double> e, Iv<double>& se, Iv<double>& ce) {
-  const double s0 = Trig<double>::sqr(e.lo), s1 = Trig<double>::sqr(e.hi);
-  se = {pad_dn(Trig<double>::sin_medium(e.lo, s0)), pad_up(Trig<double>::sin_medium(e.hi, s1))};
-  const double c0 = Trig<double>::cos_medium(s0), c1 = Trig<double>::cos_medium(s1);
+// the same over e inside (-1, 1) (prim op 18 / 19; the kernels use the quad form in ia_fastq.cuh)
+template <class T> IA_DEV void trig_medium(Iv<T> e, Iv<T>& se, Iv<T>& ce) {
+  const T s0 = Trig<T>::sqr(e.lo), s1 = Trig<T>::sqr(e.hi);
+  se = {pad_dn(Trig<T>::sin_medium(e.lo, s0)), pad_up(Trig<T>::sin_medium(e.hi, s1))};
+  const T c0 = Trig<T>::cos_medium(s0), c1 = Trig<T>::cos_medium(s1);
   const bool c = nn_gt(s0, s1);
   const bool straddle = sgn(e.lo) != sgn(e.hi);
-  const double chi = pad_up(c ? c1 : c0);
-  ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? 1.0 : chi};
+  const T chi = pad_up(c ? c1 : c0);
+  ce = {pad_dn(c ? c0 : c1), (straddle || ge_one(chi)) ? T(1) : chi};
 }
-IA_DEV void trig_medium(Iv<float> e, Iv<float>& se, Iv<float>& ce) { se = isin(e); ce = icos(e); }   // not used in float
 
 // ---- the FP32 fast form as a floating-point filter ---------------------------------------------------
 // The sign-specialised form and the general form enclose the same function but round differently (fused FMAs, midpoint-

@@ -109,7 +109,7 @@ template <class T> IA_DEV void q_add(Iv<T> a0, Iv<T> a1, Iv<T> b0, Iv<T> b1, Iv<
 // largest magnitude among the four endpoints of e (both drift signs), read off the sign-magnitude bit patterns
 template <class T> struct EMag;
 template <> struct EMag<double> { static constexpr int quarter = 0x3fd00000, sixteenth = 0x3fb00000, one = 0x3ff00000; };
-template <> struct EMag<float> { static constexpr int quarter = 0x3e800000, sixteenth = 0x3d800000, one = 0; };   // no medium tier in float
+template <> struct EMag<float> { static constexpr int quarter = 0x3e800000, sixteenth = 0x3d800000, one = 0x3f800000; };
 template <class T> IA_DEV int e_mag(const Iv<T> (&e)[2]) {
   return max(__vimax3_s32(hiw(e[0].lo) & 0x7fffffff, hiw(e[0].hi) & 0x7fffffff, hiw(e[1].lo) & 0x7fffffff), hiw(e[1].hi) & 0x7fffffff);
 }
@@ -120,16 +120,22 @@ template <> struct TrigC<double> {
   static constexpr int NS = 5, NC = 6;
   static IA_DEV double s(int k) { return IA_SIN_C[k]; }
   static IA_DEV double c(int k) { return IA_COS_C[k]; }
+  static constexpr int NSM = 9, NCM = 10;            // medium tier (|e| < 1)
+  static IA_DEV double sm(int k) { return IA_SIN_M[k]; }
+  static IA_DEV double cm(int k) { return IA_COS_M[k]; }
 };
 template <> struct TrigC<float> {
   static constexpr int NS = 3, NC = 4;
   static IA_DEV float s(int k) { const float c[NS] = {-1.9841270e-04f, 8.3333338e-03f, -1.6666667e-01f}; return c[k]; }
   static IA_DEV float c(int k) { const float d[NC] = {2.4801588e-05f, -1.3888889e-03f, 4.1666668e-02f, -0.5f}; return d[k]; }
+  static constexpr int NSM = 5, NCM = 6;
+  static IA_DEV float sm(int k) { return Trig<float>::sm(k); }
+  static IA_DEV float cm(int k) { return Trig<float>::cm(k); }
 };
 // short (warp-uniform, double only): every |e| < 2^-4 - the leading coefficients 1/11! (sin) and 1/12!, 1/10! (cos) are
 // then below 2^-60 relative (x^10/11! < 2.3e-20; x^10/10! < 2.5e-19 against cos > 0.99) and their three Horner steps
 // per point are skipped: 12 FP64 instructions per evaluation.  Same bound as the long form (below 1 ulp, inside the pad).
-// medium (warp-uniform, double only): every |e| < 1 - the polynomials of IA_SIN_M / IA_COS_M (ia_fast.cuh), terms to x^19 / x^20
+// medium (warp-uniform): every |e| < 1 - the longer polynomials of ia_fast.cuh (double: terms to x^19 / x^20, float: x^11 / x^12)
 template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2], Iv<T> (&ce)[2], bool short_poly = false, bool medium = false) {
   using V = VR<T>;
   using C = TrigC<T>;
@@ -137,16 +143,16 @@ template <class T> IA_DEV void q_trig_small(const Iv<T> (&e)[2], Iv<T> (&se)[2],
   T s[4], xs[4], qs[4], qc[4], sn[4], cs[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) s[i] = V::mul_rn(x[i], x[i]);
-  if (sizeof(T) == 8 && medium) {
+  if (medium) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(T(IA_SIN_M[0]), s[i], T(IA_SIN_M[1])); qc[i] = V::fma_rn(T(IA_COS_M[0]), s[i], T(IA_COS_M[1])); }
+    for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(C::sm(0), s[i], C::sm(1)); qc[i] = V::fma_rn(C::cm(0), s[i], C::cm(1)); }
 #pragma unroll
-    for (int k = 2; k < 9; ++k) {
+    for (int k = 2; k < C::NSM; ++k) {
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(qs[i], s[i], T(IA_SIN_M[k])); qc[i] = V::fma_rn(qc[i], s[i], T(IA_COS_M[k])); }
+      for (int i = 0; i < 4; ++i) { qs[i] = V::fma_rn(qs[i], s[i], C::sm(k)); qc[i] = V::fma_rn(qc[i], s[i], C::cm(k)); }
     }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) { xs[i] = V::mul_rn(x[i], s[i]); qc[i] = V::fma_rn(qc[i], s[i], T(IA_COS_M[9])); }
+    for (int i = 0; i < 4; ++i) { xs[i] = V::mul_rn(x[i], s[i]); qc[i] = V::fma_rn(qc[i], s[i], C::cm(C::NCM - 1)); }
   } else if (sizeof(T) == 8) {
     // both forms start with an FMA on constants (no register initialisation) and meet after the 1/7! and 1/6! steps
     if (short_poly) {
@@ -354,7 +360,7 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
   // S5
   Iv<T> se[2], sce[2], cce[2];                                         // sin e, sigma sA cos e, cA cos e
   const bool all_small = __all_sync(0xffffffffu, small);
-  if (all_small || (sizeof(T) == 8 && __all_sync(0xffffffffu, emag < EMag<T>::one))) {
+  if (all_small || __all_sync(0xffffffffu, emag < EMag<T>::one)) {
     Iv<T> ce[2];
     q_trig_small(e, se, ce, all_small && __all_sync(0xffffffffu, emag < EMag<T>::sixteenth), !all_small);
     q_mulpos<SS>(ce[0], ce[1], SS < 0 ? ineg(h.sA(va)) : h.sA(va), sce[0], sce[1]);
@@ -546,7 +552,7 @@ IA_DEV unsigned pass_vote_qr(const H& h, int ss_in, int va, const Pass2<T>& pc, 
   const bool small = emag < EMag<T>::quarter;
   // S5
   const bool all_small = __all_sync(0xffffffffu, small);
-  if (all_small || (sizeof(T) == 8 && __all_sync(0xffffffffu, emag < EMag<T>::one))) {
+  if (all_small || __all_sync(0xffffffffu, emag < EMag<T>::one)) {
     Iv<T> ce[2];
     q_trig_small(e, se, ce, all_small && __all_sync(0xffffffffu, emag < EMag<T>::sixteenth), !all_small);
     if (ss != 0) {

@@ -499,13 +499,15 @@ def test_fast_path_primitives(rig0, prec):
         cmax = mp.mpf(1) if lo <= 0 <= hi else mp.cos(min(abs(lo), abs(hi)))
         assert mp.mpf(cc[i, 0]) <= cmin and cmax <= mp.mpf(cc[i, 1]) and cc[i, 1] <= 1.0, (e[i], cc[i])
         assert cmin - mp.mpf(cc[i, 0]) <= 10 * eps and mp.mpf(cc[i, 1]) - cmax <= 10 * eps, (e[i], cc[i])
-    # the medium tier (double only): sin / cos inside (-1, 1) by the longer polynomials - contains the truth, and is at most
-    # 10 ulps of the result (sin) / of 1 (cos) wider: the relative pad 2^-50 = 8 half-ulps plus the polynomial's own error
-    if prec == 64:
+    # the medium tier: sin / cos inside (-1, 1) by the longer polynomials - contains the truth, and is at most 10 ulps of
+    # the result (sin) / of 1 (cos) wider: the relative pad 2^-50 (2^-21) = 8 half-ulps plus the polynomial's own error
+    if True:
         c = rng.uniform(-1.0, 1.0, n)
         w = rng.choice([0.0, 1e-12, 1e-6, 1e-3, 0.05, 0.5, 2.0], size=n) * rng.random(n)
-        lim = float(np.nextafter(1.0, 0.0))
+        lim = float(np.nextafter(1.0, 0.0)) if prec == 64 else float(np.nextafter(np.float32(1.0), np.float32(0.0)))
         e = np.clip(np.stack([c - w, c + w], 1), -lim, lim)
+        if prec == 32:
+            e = np.clip(e.astype(np.float32).astype(np.float64), -lim, lim)
         e[:10] = [[-lim, lim]] * 10
         e[10:20] = np.stack([np.zeros(10), np.abs(e[10:20, 1])], 1)
         e[20:30] = np.stack([-np.abs(e[20:30, 0]), -np.zeros(10)], 1)
