@@ -751,7 +751,7 @@ def main():
         dt = (time.perf_counter() - t0) / n_e2e
         line["e2e"] = {"value": evals_per_step / dt, "unit": UNIT, "h2d_bytes_per_step": int(pinned_hits.nbytes),
                        "d2h_bytes_per_step": int(host_votes.nbytes), "ms_per_step": dt * 1e3,
-                       "call": "ia_vote_host (pinned host buffers, synchronous)"}
+                       "call": "ia_vote_host (pinned host buffers, synchronous; the votes leave in up to 8 slabs of xc cells, each copied while the next is voted)"}
 
         # ---- cpu_baseline: the oracle on a bounded sample of the same cells, and a parity spot check ----
         rate, cores, n_s, dt_o, vo, cells = oracle_sample_rate(ch, ev, dims, args.ref_cells)

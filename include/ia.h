@@ -258,7 +258,8 @@ int ia_refine_batch(ia_ctx* ctx, const ia_hit* hits_dev, const int32_t* hit_offs
 
 /* End-to-end variants: every pointer is HOST memory (pinned for full copy speed).  They validate
  * the hits, copy them to the device, run the call above and copy the result back, then
- * synchronise the stream. */
+ * synchronise the stream.  ia_vote_host sends an accumulator of 32 MB or more in up to 8 slabs of xc cells
+ * (the launches of ia_vote_slab), slab i copied on a second stream while slab i+1 is voted: same counts. */
 int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double box_lo[5], const double box_hi[5],
                  const int32_t grid_dims[5], uint16_t* votes_out_host);
 int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hit_offsets_host, int n_events,

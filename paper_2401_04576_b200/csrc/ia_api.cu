@@ -220,6 +220,8 @@ void ia_destroy(ia_ctx* ctx) {
   for (Scratch* s : all)
     if (s->p) cudaFree(s->p);
   if (ctx->rgraph.exec) cudaGraphExecDestroy(ctx->rgraph.exec);
+  if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+  if (ctx->slab_done) cudaEventDestroy(ctx->slab_done);
   if (ctx->wires) cudaFree(ctx->wires);
   if (ctx->status) cudaFree(ctx->status);
   delete ctx;
@@ -502,12 +504,42 @@ int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double 
   IA_CUDA(ctx, scratch_reserve(ctx->io_b, size_t(g.cells) * sizeof(uint16_t)));
   if (n_hits > 0)
     IA_CUDA(ctx, cudaMemcpyAsync(ctx->io_a.p, hits_host, size_t(n_hits) * sizeof(ia_hit), cudaMemcpyHostToDevice, ctx->stream));
-  rc = ia_vote(ctx, static_cast<const ia_hit*>(ctx->io_a.p), n_hits, box_lo, box_hi, grid_dims,
-               static_cast<uint16_t*>(ctx->io_b.p));
+  uint16_t* acc = static_cast<uint16_t*>(ctx->io_b.p);
+  const ia_hit* hits_dev = static_cast<const ia_hit*>(ctx->io_a.p);
+  // A large accumulator (C4: 2.1 GB, 38 ms of PCIe after 1.2 s of vote) goes out in slabs of xc cells: slab i is copied
+  // on a second stream while slab i+1 is voted (ia_vote_slab's launch: same edges, same counts), so only the last copy
+  // is exposed.  At most 8 slabs of at least 32 MB: more would add partial waves of blocks to every launch.
+  const int64_t slab_min = int64_t(16) << 20;            // cells
+  int n_slabs = int(std::min<int64_t>(std::min<int64_t>(8, g.n[0]), g.cells / slab_min));
+  if (n_slabs < 2) {
+    rc = ia_vote(ctx, hits_dev, n_hits, box_lo, box_hi, grid_dims, acc);
+    if (rc) return rc;
+    IA_CUDA(ctx, cudaMemcpyAsync(votes_out_host, acc, size_t(g.cells) * sizeof(uint16_t), cudaMemcpyDeviceToHost, ctx->stream));
+    IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return IA_OK;
+  }
+  rc = check_domain(ctx, box_lo, box_hi);
   if (rc) return rc;
-  IA_CUDA(ctx, cudaMemcpyAsync(votes_out_host, ctx->io_b.p, size_t(g.cells) * sizeof(uint16_t), cudaMemcpyDeviceToHost,
-                               ctx->stream));
+  if (n_hits > IA_MAX_HITS) return IA_ERR_CAPACITY;
+  if (!ctx->copy_stream) IA_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  if (!ctx->slab_done) IA_CUDA(ctx, cudaEventCreateWithFlags(&ctx->slab_done, cudaEventDisableTiming));
+  HitSpan sp = single_span(hits_dev, n_hits);
+  IA_CUDA(ctx, launch_stage_hits(ctx, sp));
+  const int64_t per_ix = g.cells / g.n[0];
+  for (int i = 0; i < n_slabs; ++i) {
+    const int b0 = int(int64_t(g.n[0]) * i / n_slabs), e0 = int(int64_t(g.n[0]) * (i + 1) / n_slabs);
+    GridDesc gs = g;
+    gs.ix0 = b0;
+    gs.nx_run = e0 - b0;
+    gs.cells = per_ix * gs.nx_run;
+    IA_CUDA(ctx, launch_vote_dense(ctx, sp, gs, acc + per_ix * b0));
+    IA_CUDA(ctx, cudaEventRecord(ctx->slab_done, ctx->stream));
+    IA_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_done, 0));
+    IA_CUDA(ctx, cudaMemcpyAsync(votes_out_host + per_ix * b0, acc + per_ix * b0, size_t(gs.cells) * sizeof(uint16_t),
+                                 cudaMemcpyDeviceToHost, ctx->copy_stream));
+  }
   IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  IA_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
   return IA_OK;
 }
 

@@ -74,6 +74,8 @@ struct ia_ctx {
   ia::Scratch misc;          // idx / votes of internal top-K, host-variant device buffers
   ia::Scratch io_a, io_b, io_c, io_d;   // *_host entry points: device mirrors of host buffers
   int* status = nullptr;     // device: sticky error flag
+  cudaStream_t copy_stream = nullptr;   // ia_vote_host: device->host copies of finished slabs, beside the vote
+  cudaEvent_t slab_done = nullptr;
   int64_t launches = 0;
   int64_t graph_replays = 0;  // refinement calls served by cudaGraphLaunch
   cudaError_t last_err = cudaSuccess;

@@ -387,6 +387,12 @@ def test_host_entry_point_matches_device_path(rig0):
     vh = rig0.ctx.ia_vote_host(b.hits_of(ev.wire, ev.drift), LO, HI, dims)
     assert (vd.cpu().numpy() == vh).all()
     assert rig0.ctx.ia_launch_count() > 0
+    # accumulators of 32 MB and more leave in slabs of xc cells, copied while the next slab is voted (2 and 3 uneven slabs)
+    for dims in ((37, 32, 32, 32, 32), (7, 64, 64, 64, 32)):
+        vd = rig0.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+        rig0.ctx.synchronize()
+        vh = rig0.ctx.ia_vote_host(b.hits_of(ev.wire, ev.drift), LO, HI, dims)
+        assert (vd.cpu().numpy() == vh).all(), dims
 
 
 @pytest.mark.parametrize("precision", [64, 32])
