@@ -807,3 +807,83 @@ def test_slab_votes_tile_the_accumulator_and_key_lists_merge_to_the_same_topk(pr
             rig.ctx.ia_vote_slab(hd, ev.n_hits, LO, HI, (4, 4, 4, 4, 4), 2, 5)
     finally:
         rig.close()
+
+
+def test_outputs_stay_inside_their_buffers(rig1):
+    """compute-sanitizer is closed on this GPU pool, so: every caller-provided output is a window inside a larger buffer
+    of canary bytes, on shapes chosen to end in partial warps, partial tiles and odd strides; after the calls the canaries
+    on both sides are intact and the window equals what the same call writes into a buffer of its own."""
+    import torch
+    ctx = rig1.ctx
+    ev = g.make_event(rig1.ch, 5, n_noise=7)
+    hd, _ = rig1.hits(ev.wire, ev.drift)
+    GUARD = 4096
+
+    def window(nbytes, dtype):
+        buf = torch.full((nbytes + 2 * GUARD,), 0xA5, dtype=torch.uint8, device="cuda")
+        return buf, buf[GUARD:GUARD + nbytes].view(dtype)
+
+    def intact(buf, nbytes):
+        return bool((buf[:GUARD] == 0xA5).all()) and bool((buf[GUARD + nbytes:] == 0xA5).all())
+
+    for prec in (64, 32):
+        ctx.ia_set_params(g.TOL, precision=prec)
+        # dense vote: ragged grids (partial pair tiles, partial z0 tiles, odd lambda count), the general kernel, a slab
+        for dims, flags in (((3, 2, 7, 5, 9), 0), ((2, 3, 33, 17, 10), 0), ((2, 2, 5, 19, 3), 1), ((1, 1, 1, 1, 1), 0)):
+            ctx.ia_set_params(g.TOL, precision=prec, flags=flags)
+            n = int(np.prod(dims))
+            buf, w = window(2 * n, torch.uint16)
+            ctx.ia_vote(hd, ev.n_hits, LO, HI, dims, votes_out=w)
+            ref = ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+            ctx.synchronize()
+            assert intact(buf, 2 * n) and torch.equal(w.view(torch.int16), ref.view(torch.int16)), (prec, dims, flags)
+        ctx.ia_set_params(g.TOL, precision=prec)
+        dims = (5, 3, 9, 7, 4)
+        col = int(np.prod(dims[1:]))
+        buf, w = window(2 * 2 * col, torch.uint16)
+        ctx.ia_vote_slab(hd, ev.n_hits, LO, HI, dims, 2, 4, votes_out=w)
+        full = ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+        ctx.synchronize()
+        assert intact(buf, 4 * col) and torch.equal(w.view(torch.int16), full[2 * col:4 * col].view(torch.int16))
+        # explicit boxes: a count that is not a multiple of the block
+        nb = 131
+        blo = np.tile(LO, (nb, 1)) + np.linspace(0, 1, nb)[:, None] * 0.3 * (HI - LO)
+        bhi = blo + 0.1 * (HI - LO)
+        buf, w = window(2 * nb, torch.uint16)
+        ctx.ia_vote_boxes(hd, ev.n_hits, rig1.dev(blo), rig1.dev(bhi), votes_out=w)
+        ref = ctx.ia_vote_boxes(hd, ev.n_hits, rig1.dev(blo), rig1.dev(bhi))
+        ctx.synchronize()
+        assert intact(buf, 2 * nb) and torch.equal(w.view(torch.int16), ref.view(torch.int16))
+        # refinement: boxes and parameters, single event and a batch with an empty event, K not a power of two
+        for levels, k in ((3, 5), (4, 16)):
+            nbx = levels * k * b.BOX_DT.itemsize
+            bb, wb = window(nbx, torch.uint8)
+            pb, wp = window(8 * b.IA_N_PARAMS, torch.float64)
+            ctx.ia_refine(hd, ev.n_hits, LO, HI, (4, 4, 4, 4, 4), levels, k, boxes=wb, params=wp)
+            rb_, rp_ = ctx.ia_refine(hd, ev.n_hits, LO, HI, (4, 4, 4, 4, 4), levels, k)
+            ctx.synchronize()
+            assert intact(bb, nbx) and intact(pb, 8 * b.IA_N_PARAMS) and torch.equal(wb, rb_) and torch.equal(wp, rp_)
+        evs = [g.make_event(rig1.ch, 40 + e, n_noise=3) for e in range(3)]
+        wire = np.concatenate([evs[0].wire, evs[2].wire]); drift = np.concatenate([evs[0].drift, evs[2].drift])
+        off = np.array([0, evs[0].n_hits, evs[0].n_hits, evs[0].n_hits + evs[2].n_hits], np.int32)
+        hb, _ = rig1.hits(wire, drift)
+        levels, k = 3, 7
+        nbx = 3 * levels * k * b.BOX_DT.itemsize
+        bb, wb = window(nbx, torch.uint8)
+        pb, wp = window(3 * 8 * b.IA_N_PARAMS, torch.float64)
+        mh = int(max(evs[0].n_hits, evs[2].n_hits))
+        ctx.ia_refine_batch(hb, rig1.dev(off), 3, mh, LO, HI, (4, 4, 4, 4, 4), levels, k, boxes=wb, params=wp)
+        rb_, rp_ = ctx.ia_refine_batch(hb, rig1.dev(off), 3, mh, LO, HI, (4, 4, 4, 4, 4), levels, k)
+        ctx.synchronize()
+        assert intact(bb, nbx) and intact(pb, 3 * 8 * b.IA_N_PARAMS) and torch.equal(wb, rb_) and torch.equal(wp, rp_)
+    # paper mode (double): two accumulators of an odd-shaped grid
+    ctx.ia_set_params(g.TOL)
+    xc, yc, R, z0, lam = ev.track.params
+    P = R * (1.0 + lam * lam) ** 0.5
+    d4 = (7, 5, 9, 3)
+    n4 = int(np.prod(d4))
+    buf, w = window(2 * 2 * n4, torch.uint16)
+    ctx.ia_vote_paper(hd, ev.n_hits, P, LO[:4], HI[:4], d4, votes_out=w)
+    ref = ctx.ia_vote_paper(hd, ev.n_hits, P, LO[:4], HI[:4], d4)
+    ctx.synchronize()
+    assert intact(buf, 4 * n4) and torch.equal(w.view(torch.int16), ref.reshape(-1).view(torch.int16))
