@@ -87,15 +87,17 @@ typedef struct {
  * point of the base circle closest to the axis, instead of the principal value in (-pi, pi]; bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
  * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
  * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; ia_vote runs it in the
- * sign-specialised dense kernel (about 6 x the series mode), the explicit-box and refinement kernels in the general
+ * sign-specialised dense and children kernels (about 6 x the series mode), the explicit-box kernel in the general
  * form; bit 5: ia_refine / ia_refine_batch always enqueue
  * their launches one by one (default: a call repeated with identical arguments and buffers is replayed as a
  * CUDA graph from its third occurrence on); bit 6 (sign-specialised dense kernel): prefilter - before the fine
  * evaluation of a hit a warp asks a crude enclosure of the same residual (magnitude bounds of every step of S4-S8, both
  * drift signs, all the z0 cells of its tile at once) whether 0 can be excluded for all its cells, and skips the hit if
  * so: the votes are identical (a wider enclosure that excludes 0 implies the finer one does, L80), the kernel no longer
- * evaluates every (cell, hit) in full - default off: north_star's metric is the brute-force evaluation; other bits
- * must be 0. */
+ * evaluates every (cell, hit) in full - default off: north_star's metric is the brute-force evaluation; bit 7: the
+ * kernels of the vote / top-K / refinement chain are launched without the programmatic-dependent-launch attribute
+ * (default: with it - each of them starts by waiting for the kernels in front, so that its launch overlaps their
+ * execution; same results either way); other bits must be 0. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;

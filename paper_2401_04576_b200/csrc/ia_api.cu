@@ -264,7 +264,7 @@ int ia_set_params(ia_ctx* ctx, const ia_params* p) {
       !std::isfinite(p->z_ref))
     return IA_ERR_ARG;
   if (p->precision != 64 && p->precision != 32) return IA_ERR_ARG;
-  if (p->flags & ~127u) return IA_ERR_ARG;
+  if (p->flags & ~255u) return IA_ERR_ARG;
   ctx->params = *p;
   return IA_OK;
 }

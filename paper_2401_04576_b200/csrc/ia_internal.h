@@ -84,6 +84,34 @@ struct ia_ctx {
 
 namespace ia {
 
+// ---- programmatic dependent launch (sm_90+) --------------------------------------------------------
+// A refinement is a chain of short dependent kernels (C2: 25 launches in 0.22 ms).  Launched with the
+// programmatic-stream-serialization attribute, kernel N+1 does not wait for kernel N to be retired before it is launched:
+// its blocks start as the last blocks of N leave and wait in griddepcontrol.wait - the first statement of every kernel
+// of the chain, pdl_wait() - until the grids in front have completed and their writes are visible (it returns at once
+// if there are none).  Nothing is read or written early, and completion stays transitive along the chain.  Only kernels
+// that begin with pdl_wait() may be launched through launch_k.  ia_params.flags bit 7 switches the attribute off.
+// Measured on C2: 0.2175 ms against 0.2249 replayed as a graph, 0.2187 against 0.2772 launched one by one.
+#ifdef __CUDACC__
+// (an early griddepcontrol.launch_dependents after the wait was tried: C2 0.222 ms against 0.2175 without it)
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+cudaError_t launch_k(ia_ctx* ctx, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = ctx->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (ctx->params.flags & 128u) ? 0 : 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // All launchers enqueue on ctx->stream, bump ctx->launches and return the launch's cudaError_t.
 // prec selects the endpoint type (64: double, 32: float).
 

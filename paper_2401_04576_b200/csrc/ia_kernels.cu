@@ -70,6 +70,7 @@ __device__ __forceinline__ void event_hits(const HitSpan& sp, int e, int& first,
 template <class T>
 __global__ void stage_hits_kernel(HitSpan sp, const double* __restrict__ wires, int n_wires, ia_params p,
                                   HitC<T>* __restrict__ staged, int* status) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   const int e = blockIdx.x;
   int first, count;
   event_hits(sp, e, first, count);
@@ -168,6 +169,7 @@ __global__ void prim_kernel(int op, const double* __restrict__ a, const double* 
 // dense cell index -> box (S9): linear index ((((ix*ny+iy)*nR+iR)*nz+iz)*nl+il), lambda fastest
 __global__ void gather_dense_kernel(GridDesc g, const int64_t* __restrict__ idx, const uint16_t* __restrict__ v,
                                     int k, int levels, ia_box* __restrict__ boxes) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   const int e = blockIdx.x, r = threadIdx.x;
   if (r >= k) return;
   int64_t c = idx[int64_t(e) * k + r];
@@ -198,6 +200,7 @@ template <class T>
 __global__ void __launch_bounds__(256)
 vote_children_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
                      int levels, int k, int per_split, uint16_t* __restrict__ partial) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   extern __shared__ __align__(16) unsigned char smem_raw[];
   HitC<T>* sh = reinterpret_cast<HitC<T>*>(smem_raw);
   const int e = blockIdx.y, split = blockIdx.x;
@@ -231,6 +234,7 @@ vote_children_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_bo
 __global__ void __launch_bounds__(1024)
 select_children_kernel(const uint16_t* __restrict__ partial, int n_splits, int lev, int levels, int k,
                        ia_box* __restrict__ boxes) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   __shared__ u64 smem_keys[32 * 32];
   const int e = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
   unsigned v = 0;
@@ -254,6 +258,7 @@ select_children_kernel(const uint16_t* __restrict__ partial, int n_splits, int l
 // the last pass that share rank 0's vote count (G19: the paper keeps every cell at the maximum, L94)
 __global__ void params_kernel(int n_events, int levels, int k, const ia_box* __restrict__ boxes,
                               double* __restrict__ params) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n_events) return;
   const ia_box* last = boxes + (int64_t(e) * levels + (levels - 1)) * k;
@@ -289,12 +294,12 @@ cudaError_t launch_stage_hits(ia_ctx* ctx, const HitSpan& sp) {
   if (err != cudaSuccess) return err;
   if (sp.n_events <= 0 || sp.max_hits <= 0) return cudaSuccess;
   IA_DISPATCH_PREC(ctx,
-    (stage_hits_kernel<double><<<sp.n_events, 64, 0, ctx->stream>>>(sp, ctx->wires, ctx->n_wires, ctx->params,
-                                                                    static_cast<HitC<double>*>(ctx->staged.p), ctx->status)),
-    (stage_hits_kernel<float><<<sp.n_events, 64, 0, ctx->stream>>>(sp, ctx->wires, ctx->n_wires, ctx->params,
-                                                                   static_cast<HitC<float>*>(ctx->staged.p), ctx->status)));
+    (err = launch_k(ctx, stage_hits_kernel<double>, dim3(sp.n_events), dim3(64), 0, sp, ctx->wires, ctx->n_wires, ctx->params,
+                    static_cast<HitC<double>*>(ctx->staged.p), ctx->status)),
+    (err = launch_k(ctx, stage_hits_kernel<float>, dim3(sp.n_events), dim3(64), 0, sp, ctx->wires, ctx->n_wires, ctx->params,
+                    static_cast<HitC<float>*>(ctx->staged.p), ctx->status)));
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 cudaError_t launch_vote_boxes(ia_ctx* ctx, const HitSpan& sp, const double* lo, const double* hi, int64_t n_boxes,
@@ -343,9 +348,9 @@ cudaError_t launch_prim(ia_ctx* ctx, int op, int prec, const double* a, const do
 
 cudaError_t launch_gather_dense(ia_ctx* ctx, const GridDesc& g, const int64_t* idx, const uint16_t* v, int n_events,
                                 int k, int levels, ia_box* boxes_out) {
-  gather_dense_kernel<<<n_events, 32, 0, ctx->stream>>>(g, idx, v, k, levels, boxes_out);
+  const cudaError_t err = launch_k(ctx, gather_dense_kernel, dim3(n_events), dim3(32), 0, g, idx, v, k, levels, boxes_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, ia_box* boxes_out) {
@@ -379,23 +384,22 @@ cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int lev
                                   int(per_split * sizeof(HitC<float>)))));
     if (err != cudaSuccess) return err;
     IA_DISPATCH_PREC(ctx,
-      (vote_children_kernel<double><<<grid, 256, per_split * sizeof(HitC<double>), ctx->stream>>>(
-          sp, static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),
-      (vote_children_kernel<float><<<grid, 256, per_split * sizeof(HitC<float>), ctx->stream>>>(
-          sp, static_cast<const HitC<float>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)));
+      (err = launch_k(ctx, vote_children_kernel<double>, grid, dim3(256), per_split * sizeof(HitC<double>), sp,
+                      static_cast<const HitC<double>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)),
+      (err = launch_k(ctx, vote_children_kernel<float>, grid, dim3(256), per_split * sizeof(HitC<float>), sp,
+                      static_cast<const HitC<float>*>(ctx->staged.p), boxes_out, lev, levels, k, per_split, partial)));
     ctx->launches++;
-    err = cudaGetLastError();
     if (err != cudaSuccess) return err;
   }
-  select_children_kernel<<<sp.n_events, threads, 0, ctx->stream>>>(partial, n_splits, lev, levels, k, boxes_out);
+  err = launch_k(ctx, select_children_kernel, dim3(sp.n_events), dim3(threads), 0, partial, n_splits, lev, levels, k, boxes_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 cudaError_t launch_params(ia_ctx* ctx, int n_events, int levels, int k, const ia_box* boxes, double* params_out) {
-  params_kernel<<<(n_events + 127) / 128, 128, 0, ctx->stream>>>(n_events, levels, k, boxes, params_out);
+  const cudaError_t err = launch_k(ctx, params_kernel, dim3((n_events + 127) / 128), dim3(128), 0, n_events, levels, k, boxes, params_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 }  // namespace ia

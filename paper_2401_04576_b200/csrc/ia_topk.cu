@@ -38,6 +38,7 @@ template <int U>
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, int64_t idx_base, u64* __restrict__ partial,
              int64_t* __restrict__ idx_out, uint16_t* __restrict__ votes_out, u64* __restrict__ keys_out, int write_final) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   __shared__ u64 smem_keys[(TOPK_THREADS / 32) * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int e = blockIdx.y;
@@ -95,6 +96,7 @@ topk_partial(const uint16_t* __restrict__ votes, int64_t n, int k, int64_t idx_b
 __global__ void __launch_bounds__(TOPK_THREADS)
 topk_final(const u64* __restrict__ partial, int n_lists, int k, int64_t* __restrict__ idx_out,
            uint16_t* __restrict__ votes_out, u64* __restrict__ keys_out) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   __shared__ u64 smem_keys[(TOPK_THREADS / 32) * 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int e = blockIdx.x;
@@ -138,22 +140,25 @@ cudaError_t launch_topk(ia_ctx* ctx, const uint16_t* votes, int64_t n, int n_eve
     partial = static_cast<u64*>(ctx->keys.p);
   }
   dim3 grid((unsigned)blocks, (unsigned)n_events);
-  if (unroll == 1) topk_partial<1><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, idx_base, partial, idx_out, votes_out, keys_out, write_final);
-  else topk_partial<TOPK_UNROLL><<<grid, TOPK_THREADS, 0, ctx->stream>>>(votes, n, k, idx_base, partial, idx_out, votes_out, keys_out, write_final);
+  cudaError_t err;
+  if (unroll == 1)
+    err = launch_k(ctx, topk_partial<1>, grid, dim3(TOPK_THREADS), 0, votes, n, k, idx_base, partial, idx_out, votes_out, keys_out, write_final);
+  else
+    err = launch_k(ctx, topk_partial<TOPK_UNROLL>, grid, dim3(TOPK_THREADS), 0, votes, n, k, idx_base, partial, idx_out, votes_out, keys_out,
+                   write_final);
   ctx->launches++;
-  cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess || write_final) return err;
-  topk_final<<<n_events, TOPK_THREADS, 0, ctx->stream>>>(partial, int(blocks), k, idx_out, votes_out, keys_out);
+  err = launch_k(ctx, topk_final, dim3(n_events), dim3(TOPK_THREADS), 0, partial, int(blocks), k, idx_out, votes_out, keys_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 // key lists of several accumulators (the slabs of a split vote, gathered from their GPUs) -> the k best of their union
 cudaError_t launch_merge_keys(ia_ctx* ctx, const unsigned long long* keys, int n_lists, int k, int64_t* idx_out,
                               uint16_t* votes_out) {
-  topk_final<<<1, TOPK_THREADS, 0, ctx->stream>>>(keys, n_lists, k, idx_out, votes_out, nullptr);
+  const cudaError_t err = launch_k(ctx, topk_final, dim3(1), dim3(TOPK_THREADS), 0, keys, n_lists, k, idx_out, votes_out, nullptr);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 }  // namespace ia

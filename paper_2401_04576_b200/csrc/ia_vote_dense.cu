@@ -30,6 +30,7 @@ template <class T>
 __global__ void __launch_bounds__(GEN_THREADS)
 vote_dense_general_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int chunks_per_col,
                           uint16_t* __restrict__ votes) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   extern __shared__ __align__(16) unsigned char smem_raw[];
   HitShared<T>* sh = reinterpret_cast<HitShared<T>*>(smem_raw);
   const int e = blockIdx.y;
@@ -177,6 +178,7 @@ template <class T, bool RT, bool SPLIT, bool RIG = false>
 __global__ void __launch_bounds__(FAST_THREADS, FAST_MIN_BLOCKS)
 vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc g, int tiles_p, int tiles_z, int zt,
                        int per_split, int prefilter, uint16_t* __restrict__ votes) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ZTab<T>* ztab = reinterpret_cast<ZTab<T>*>(smem_raw);
   HitF<T>* sh = reinterpret_cast<HitF<T>*>(smem_raw + sizeof(ZTab<T>));
@@ -297,6 +299,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
 
 // partial accumulators of a hit-split launch -> the accumulator (deterministic, no atomics)
 __global__ void sum_partial_votes_kernel(const uint16_t* __restrict__ partial, int n_splits, int64_t n, uint16_t* __restrict__ votes) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += int64_t(gridDim.x) * blockDim.x) {
     unsigned v = 0;
     for (int s = 0; s < n_splits; ++s) v += partial[int64_t(s) * n + i];
@@ -327,6 +330,7 @@ template <class T, bool RIG = false>
 __global__ void __launch_bounds__(512, 1)
 vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
                           int levels, int k, int per_split, uint16_t* __restrict__ partial) {
+  pdl_wait();                 // programmatic dependent launch: nothing before the kernels in front have completed
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ZTab2<T>* ztab = reinterpret_cast<ZTab2<T>*>(smem_raw);
   HitF<T>* rec = reinterpret_cast<HitF<T>*>(smem_raw + size_t(k) * sizeof(ZTab2<T>));
@@ -529,8 +533,8 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   do {                                                                                                                       \
     err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
     if (err != cudaSuccess) return err;                                                                                      \
-    vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_><<<grid, threads, smem, ctx->stream>>>(sp, staged, g, tiles_p, tiles_z, zt, per_split, \
-                                                                                  (ctx->params.flags & 64u) ? 1 : 0, target);   \
+    err = launch_k(ctx, vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_>, grid, dim3(threads), smem, sp, staged, g, tiles_p, tiles_z, zt, \
+                   per_split, (ctx->params.flags & 64u) ? 1 : 0, target);                                                     \
   } while (0)
   if (ctx->params.flags & 16u) {
     // rigorous Phi: the one-body variant carries the verification loop (any grid)
@@ -542,13 +546,12 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   }
 #undef IA_LAUNCH_FAST
   ctx->launches++;
-  err = cudaGetLastError();
   if (err != cudaSuccess || n_splits == 1) return err;
   int sum_blocks = int((n_acc + 1023) / 1024);
   if (sum_blocks > 8 * n_sm) sum_blocks = 8 * n_sm;
-  sum_partial_votes_kernel<<<sum_blocks, 256, 0, ctx->stream>>>(target, n_splits, n_acc, votes_out);
+  err = launch_k(ctx, sum_partial_votes_kernel, dim3(sum_blocks), dim3(256), 0, target, n_splits, n_acc, votes_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 template <class T>
@@ -560,10 +563,10 @@ static cudaError_t launch_general(ia_ctx* ctx, const HitSpan& sp, const GridDesc
   const size_t smem = size_t(sp.max_hits) * sizeof(HitShared<T>);
   cudaError_t err = cudaFuncSetAttribute(vote_dense_general_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
   if (err != cudaSuccess) return err;
-  vote_dense_general_kernel<T><<<grid, GEN_THREADS, smem, ctx->stream>>>(sp, static_cast<const HitC<T>*>(ctx->staged.p), g,
-                                                                        chunks, votes_out);
+  err = launch_k(ctx, vote_dense_general_kernel<T>, grid, dim3(GEN_THREADS), smem, sp, static_cast<const HitC<T>*>(ctx->staged.p), g, chunks,
+                 votes_out);
   ctx->launches++;
-  return cudaGetLastError();
+  return err;
 }
 
 template <class T>
@@ -590,16 +593,16 @@ static cudaError_t launch_children_fast_t(ia_ctx* ctx, const HitSpan& sp, int le
   if (ctx->params.flags & 16u) {
     err = cudaFuncSetAttribute(vote_children_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (err != cudaSuccess) return err;
-    vote_children_fast_kernel<T, true><<<grid, threads, smem, ctx->stream>>>(sp, staged, boxes, lev, levels, k, per_split, partial);
+    err = launch_k(ctx, vote_children_fast_kernel<T, true>, grid, dim3(threads), smem, sp, staged, boxes, lev, levels, k, per_split, partial);
   } else {
     err = cudaFuncSetAttribute(vote_children_fast_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (err != cudaSuccess) return err;
-    vote_children_fast_kernel<T, false><<<grid, threads, smem, ctx->stream>>>(sp, staged, boxes, lev, levels, k, per_split, partial);
+    err = launch_k(ctx, vote_children_fast_kernel<T, false>, grid, dim3(threads), smem, sp, staged, boxes, lev, levels, k, per_split, partial);
   }
   ctx->launches++;
   *n_splits_out = n_splits;
   *partial_out = partial;
-  return cudaGetLastError();
+  return err;
 }
 
 cudaError_t launch_vote_children_fast(ia_ctx* ctx, const HitSpan& sp, int lev, int levels, int k, int n_sm, ia_box* boxes,

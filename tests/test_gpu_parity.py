@@ -887,3 +887,27 @@ def test_outputs_stay_inside_their_buffers(rig1):
     ref = ctx.ia_vote_paper(hd, ev.n_hits, P, LO[:4], HI[:4], d4)
     ctx.synchronize()
     assert intact(buf, 4 * n4) and torch.equal(w.view(torch.int16), ref.reshape(-1).view(torch.int16))
+
+
+def test_programmatic_dependent_launch_changes_nothing(rig1):
+    """flags bit 7 launches the chain without the programmatic-dependent-launch attribute: same boxes and parameters,
+    replayed as a graph or not (bit 5), and the same dense votes and top-K."""
+    import torch
+    cfg = g.config(2)
+    ev = cfg.events[0]
+    hd, _ = rig1.hits(ev.wire, ev.drift)
+    ctx = rig1.ctx
+    ref = None
+    for flags in (0, 128, 32, 160):
+        ctx.ia_set_params(g.TOL, flags=flags)
+        for _ in range(3):                                   # third call: the graph replay where it applies
+            boxes, par = ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 6, cfg.k)
+        v = ctx.ia_vote(hd, ev.n_hits, LO, HI, (6, 5, 9, 7, 4))
+        idx, vv = ctx.ia_topk(v, 10)
+        ctx.synchronize()
+        got = (boxes.clone(), par.clone(), v.view(torch.int16).clone(), idx.clone())
+        if ref is None:
+            ref = got
+        else:
+            assert all(torch.equal(a, c) for a, c in zip(ref, got)), flags
+    ctx.ia_set_params(g.TOL)
