@@ -316,7 +316,11 @@ __global__ void sum_partial_votes_kernel(const uint16_t* __restrict__ partial, i
 // fit CHILD_SMEM bytes and a single event still fills the chip; partial[e][split][rank*32 + c].
 // A warp holds two parents and four xy sub-cells, so the class of a hit is a per-lane value: the warp
 // takes the body of the class all its lanes share, else the universal one (valid for every class).
-constexpr int CHILD_SMEM = 48 * 1024;
+// records per block (measured on C3, 1,024 events, K = 8: 20 KB 27.6 ms, 37 KB 27.03, 48 KB 27.02, 74 KB 27.25, 96 KB 27.8, 148 KB 29.5)
+#ifndef IA_CHILD_SMEM
+#define IA_CHILD_SMEM (48 * 1024)
+#endif
+constexpr int CHILD_SMEM = IA_CHILD_SMEM;
 template <class T> struct ZTab2 { Iv<T> z[2][2]; };           // [negated][z half]
 
 __device__ __forceinline__ void child_half(double lo, double hi, int upper, double& clo, double& chi) {
