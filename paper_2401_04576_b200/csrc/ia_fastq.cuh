@@ -343,16 +343,26 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
     const T l = V::mul_dn(p.LRm.m, zA.lo), u = V::mul_up(p.LRm.m, zA.hi);
     t1.lo = V::fma_dn(-p.LRm.r, fabs(zA.lo), l); t1.hi = V::fma_up(p.LRm.r, fabs(zA.hi), u);
   }
-  const Mag<T> gz = mag_of(zA);
   Iv<T> W[2], TY[2], in[2], zG[2], Vv[2], e[2];
   q_fma<QKind<SS>::add>(sAm, sAm, zA, zA, pc.LDcA, ineg(pc.LDcA), W[0], W[1]);              // lambda D cA + zA sA
   if (h.c2cls() == CLS_P) q_fma<QK_SUB_P>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);  // t1 - t2
   else if (h.c2cls() == CLS_N) q_fma<QK_ADD_P>(mr_neg(pc.Km[0]), mr_neg(pc.Km[1]), zA, zA, t1, t1, in[0], in[1]);
   else q_fma<QK_SUB_U>(pc.Km[0], pc.Km[1], zA, zA, t1, t1, in[0], in[1]);
   q_prod_p(h.TiQm(), W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
-  zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
-  zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
-  if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
+  // G + zA^2: with the pairs of a warp running along R the sign of zA is the same for every lane of most warps - decided
+  // per warp: no magnitude sort, no selects (same values: mnn = lo, mag = hi for zA >= 0, the other way round for zA <= 0)
+  if (__all_sync(0xffffffffu, !sgn(zA.lo))) {
+    zG[0].lo = V::fma_dn(zA.lo, zA.lo, pc.G[0].lo); zG[0].hi = V::fma_up(zA.hi, zA.hi, pc.G[0].hi);
+    zG[1].lo = V::fma_dn(zA.lo, zA.lo, pc.G[1].lo); zG[1].hi = V::fma_up(zA.hi, zA.hi, pc.G[1].hi);
+  } else if (__all_sync(0xffffffffu, sgn(zA.hi))) {
+    zG[0].lo = V::fma_dn(zA.hi, zA.hi, pc.G[0].lo); zG[0].hi = V::fma_up(zA.lo, zA.lo, pc.G[0].hi);
+    zG[1].lo = V::fma_dn(zA.hi, zA.hi, pc.G[1].lo); zG[1].hi = V::fma_up(zA.lo, zA.lo, pc.G[1].hi);
+  } else {
+    const Mag<T> gz = mag_of(zA);
+    zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
+    zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
+    if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
+  }
   q_fma<QKind<SS>::add>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);                // (t1 - t2) + t3
   q_fma<QK_ADD_P>(h.T2hiQm(), h.T2hiQm(), Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
   const int emag = e_mag(e);                 // largest |endpoint| of e over both signs, as the high word of the double
@@ -425,7 +435,13 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
   Iv<T> r1[2], r2[2], f[2];
 #pragma unroll
   for (int s = 0; s < 2; ++s) { r1[s].lo = V::fma_dn(Rd1[s].lo, Rd1[s].lo, -ct[s].hi); r1[s].hi = V::fma_up(Rd1[s].hi, Rd1[s].hi, -ct[s].lo); }
-  {
+  if (__all_sync(0xffffffffu, (hiw(Tz[0].lo) | hiw(Tz[1].lo)) >= 0)) {          // z >= 0 for both signs, every lane
+    r2[0].lo = V::fma_dn(-Tz[0].hi, Tz[0].hi, r1[0].lo); r2[1].lo = V::fma_dn(-Tz[1].hi, Tz[1].hi, r1[1].lo);
+    r2[0].hi = V::fma_up(-Tz[0].lo, Tz[0].lo, r1[0].hi); r2[1].hi = V::fma_up(-Tz[1].lo, Tz[1].lo, r1[1].hi);
+  } else if (__all_sync(0xffffffffu, (hiw(Tz[0].hi) & hiw(Tz[1].hi)) < 0)) {     // z <= 0
+    r2[0].lo = V::fma_dn(-Tz[0].lo, Tz[0].lo, r1[0].lo); r2[1].lo = V::fma_dn(-Tz[1].lo, Tz[1].lo, r1[1].lo);
+    r2[0].hi = V::fma_up(-Tz[0].hi, Tz[0].hi, r1[0].hi); r2[1].hi = V::fma_up(-Tz[1].hi, Tz[1].hi, r1[1].hi);
+  } else {
     const Mag<T> g0 = mag_of(Tz[0]), g1 = mag_of(Tz[1]);
     r2[0].lo = V::fma_dn(-g0.mag, g0.mag, r1[0].lo); r2[1].lo = V::fma_dn(-g1.mag, g1.mag, r1[1].lo);
     const T h0 = V::fma_up(-g0.mnn, g0.mnn, r1[0].hi), h1 = V::fma_up(-g1.mnn, g1.mnn, r1[1].hi);
