@@ -351,17 +351,18 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
   q_prod_p(h.TiQm(), W[0], W[1], TY[0], TY[1]);                                               // T Phi1 = -TY   (A.8b)
   // G + zA^2: with the pairs of a warp running along R the sign of zA is the same for every lane of most warps - decided
   // per warp: no magnitude sort, no selects (same values: mnn = lo, mag = hi for zA >= 0, the other way round for zA <= 0)
-  if (__all_sync(0xffffffffu, !sgn(zA.lo))) {
-    zG[0].lo = V::fma_dn(zA.lo, zA.lo, pc.G[0].lo); zG[0].hi = V::fma_up(zA.hi, zA.hi, pc.G[0].hi);
-    zG[1].lo = V::fma_dn(zA.lo, zA.lo, pc.G[1].lo); zG[1].hi = V::fma_up(zA.hi, zA.hi, pc.G[1].hi);
-  } else if (__all_sync(0xffffffffu, sgn(zA.hi))) {
-    zG[0].lo = V::fma_dn(zA.hi, zA.hi, pc.G[0].lo); zG[0].hi = V::fma_up(zA.lo, zA.lo, pc.G[0].hi);
-    zG[1].lo = V::fma_dn(zA.hi, zA.hi, pc.G[1].lo); zG[1].hi = V::fma_up(zA.lo, zA.lo, pc.G[1].hi);
-  } else {
-    const Mag<T> gz = mag_of(zA);
-    zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
-    zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
-    if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
+  {
+    const bool zpos = __all_sync(0xffffffffu, !sgn(zA.lo)), zneg = __all_sync(0xffffffffu, sgn(zA.hi));
+    if (zpos || zneg) {
+      const T a = zpos ? zA.lo : zA.hi, b = zpos ? zA.hi : zA.lo;        // smaller, larger magnitude (warp-uniform choice)
+      zG[0].lo = V::fma_dn(a, a, pc.G[0].lo); zG[0].hi = V::fma_up(b, b, pc.G[0].hi);
+      zG[1].lo = V::fma_dn(a, a, pc.G[1].lo); zG[1].hi = V::fma_up(b, b, pc.G[1].hi);
+    } else {
+      const Mag<T> gz = mag_of(zA);
+      zG[0].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[0].lo); zG[0].hi = V::fma_up(gz.mag, gz.mag, pc.G[0].hi);
+      zG[1].lo = V::fma_dn(gz.mnn, gz.mnn, pc.G[1].lo); zG[1].hi = V::fma_up(gz.mag, gz.mag, pc.G[1].hi);
+      if (gz.straddle) { zG[0].lo = pc.G[0].lo; zG[1].lo = pc.G[1].lo; }
+    }
   }
   q_fma<QKind<SS>::add>(s2m, s2m, zG[0], zG[1], in[0], in[1], Vv[0], Vv[1]);                // (t1 - t2) + t3
   q_fma<QK_ADD_P>(h.T2hiQm(), h.T2hiQm(), Vv[0], Vv[1], ineg(TY[0]), ineg(TY[1]), e[0], e[1]);  // T^2 Phi2 + T Phi1  (A.8a,c)
@@ -435,17 +436,20 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
   Iv<T> r1[2], r2[2], f[2];
 #pragma unroll
   for (int s = 0; s < 2; ++s) { r1[s].lo = V::fma_dn(Rd1[s].lo, Rd1[s].lo, -ct[s].hi); r1[s].hi = V::fma_up(Rd1[s].hi, Rd1[s].hi, -ct[s].lo); }
-  if (__all_sync(0xffffffffu, (hiw(Tz[0].lo) | hiw(Tz[1].lo)) >= 0)) {          // z >= 0 for both signs, every lane
-    r2[0].lo = V::fma_dn(-Tz[0].hi, Tz[0].hi, r1[0].lo); r2[1].lo = V::fma_dn(-Tz[1].hi, Tz[1].hi, r1[1].lo);
-    r2[0].hi = V::fma_up(-Tz[0].lo, Tz[0].lo, r1[0].hi); r2[1].hi = V::fma_up(-Tz[1].lo, Tz[1].lo, r1[1].hi);
-  } else if (__all_sync(0xffffffffu, (hiw(Tz[0].hi) & hiw(Tz[1].hi)) < 0)) {     // z <= 0
-    r2[0].lo = V::fma_dn(-Tz[0].lo, Tz[0].lo, r1[0].lo); r2[1].lo = V::fma_dn(-Tz[1].lo, Tz[1].lo, r1[1].lo);
-    r2[0].hi = V::fma_up(-Tz[0].hi, Tz[0].hi, r1[0].hi); r2[1].hi = V::fma_up(-Tz[1].hi, Tz[1].hi, r1[1].hi);
-  } else {
-    const Mag<T> g0 = mag_of(Tz[0]), g1 = mag_of(Tz[1]);
-    r2[0].lo = V::fma_dn(-g0.mag, g0.mag, r1[0].lo); r2[1].lo = V::fma_dn(-g1.mag, g1.mag, r1[1].lo);
-    const T h0 = V::fma_up(-g0.mnn, g0.mnn, r1[0].hi), h1 = V::fma_up(-g1.mnn, g1.mnn, r1[1].hi);
-    r2[0].hi = g0.straddle ? r1[0].hi : h0; r2[1].hi = g1.straddle ? r1[1].hi : h1;
+  {
+    const bool tpos = __all_sync(0xffffffffu, (hiw(Tz[0].lo) | hiw(Tz[1].lo)) >= 0);      // z >= 0 for both signs, every lane
+    const bool tneg = __all_sync(0xffffffffu, (hiw(Tz[0].hi) & hiw(Tz[1].hi)) < 0);       // z <= 0
+    if (tpos || tneg) {
+      const T a0 = tpos ? Tz[0].lo : Tz[0].hi, b0 = tpos ? Tz[0].hi : Tz[0].lo;
+      const T a1 = tpos ? Tz[1].lo : Tz[1].hi, b1 = tpos ? Tz[1].hi : Tz[1].lo;
+      r2[0].lo = V::fma_dn(-b0, b0, r1[0].lo); r2[1].lo = V::fma_dn(-b1, b1, r1[1].lo);
+      r2[0].hi = V::fma_up(-a0, a0, r1[0].hi); r2[1].hi = V::fma_up(-a1, a1, r1[1].hi);
+    } else {
+      const Mag<T> g0 = mag_of(Tz[0]), g1 = mag_of(Tz[1]);
+      r2[0].lo = V::fma_dn(-g0.mag, g0.mag, r1[0].lo); r2[1].lo = V::fma_dn(-g1.mag, g1.mag, r1[1].lo);
+      const T h0 = V::fma_up(-g0.mnn, g0.mnn, r1[0].hi), h1 = V::fma_up(-g1.mnn, g1.mnn, r1[1].hi);
+      r2[0].hi = g0.straddle ? r1[0].hi : h0; r2[1].hi = g1.straddle ? r1[1].hi : h1;
+    }
   }
 #pragma unroll
   for (int s = 0; s < 2; ++s) { r2[s].lo = V::fma_dn(-TLq[s].hi, TLq[s].hi, r2[s].lo); r2[s].hi = V::fma_up(-TLq[s].lo, TLq[s].lo, r2[s].hi); }
