@@ -23,8 +23,9 @@
  *     the hit is dropped (it never votes) and a sticky flag is raised that ia_device_status()
  *     reads (it synchronises).  The *_host entry points validate hits on the host instead.
  *   - The library allocates device memory only inside the context (geometry, staged hits, child
- *     boxes, partial top-K lists, vote scratch) and frees it in ia_destroy().  No global state,
- *     no CPU fallback: every step below runs in CUDA kernels compiled for sm_100a.
+ *     boxes, partial top-K lists, vote scratch) and frees it in ia_destroy().  No global state - with one
+ *     exception, the fixed device array of ia_topk_static, the entry point for callers that must not allocate -
+ *     and no CPU fallback: every step below runs in CUDA kernels compiled for sm_100a.
  *   - Units: cm and rad.  Order of the five axes everywhere: xc, yc, R, z0, lambda.
  */
 #ifndef IA_B200_H
@@ -239,6 +240,41 @@ int ia_topk(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int6
 #define IA_KEY_LIST 32
 int ia_topk_keys(ia_ctx* ctx, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t index_base, uint64_t* keys_out_dev);
 int ia_merge_keys(ia_ctx* ctx, const uint64_t* keys_dev, int n_lists, int k, int64_t* idx_out_dev, uint16_t* votes_out_dev);
+
+/* a7 again, for callers that must not allocate device memory.  ia_topk keeps the per-block candidate lists of its first
+ * pass in a buffer of the context that it cudaMalloc's the first time it is needed and grows when a larger launch comes
+ * along; ia_create allocates too.  That is a problem for three kinds of caller this library expects: an online event
+ * filter that has handed the whole device to its framework's memory pool (a raw cudaMalloc behind the pool's back can fail
+ * although memory is "free", and the pool's owner usually forbids it); a latency-bound loop (one event every few hundred
+ * microseconds) in which cudaMalloc's implicit device-wide synchronisation stalls every other stream; and code that runs
+ * while a stream is being captured, where cudaMalloc is not allowed at all.  ia_topk_static is the same selection (same
+ * two kernels, same keys, same order: votes descending, index ascending, L94 / G16) with those lists in a fixed array
+ * that is part of the library's device image: IA_TOPK_STATIC_BYTES = 256 KB per GPU, resident on every GPU that loads
+ * the library's device code, from that moment until the process exits.  It takes no context: the device and the stream
+ * are arguments, inputs and outputs stay the caller's (DEVICE pointers), and it calls no cudaMalloc, no cudaFree and no
+ * library routine that allocates.
+ *   - Limits: 1 <= k <= min(n_cells, IA_MAX_K); n_cells <= IA_TOPK_STATIC_MAX_CELLS (2^40, the accumulator bound of
+ *     ia_vote); the first pass never uses more than IA_TOPK_STATIC_LISTS lists (it takes two blocks per SM, fewer on a
+ *     small accumulator, and is cut to the array's capacity on a device that would want more).  Anything beyond these
+ *     returns IA_ERR_CAPACITY (IA_ERR_ARG for null pointers, n_cells <= 0, k <= 0, k > n_cells, a device that does
+ *     not exist) before anything is launched, and ia_topk_static_error() says which limit and by how much.
+ *   - First call per device: the entry point asks the runtime where the array lives on that device (with the device
+ *     current, return code checked) and remembers the answer; this is also what makes the driver load the library's
+ *     device code there if nothing has yet.  Make that first call during set-up, before any stream capture begins.
+ *   - The array is shared by every call on a device and keeps whatever the last call left in it.  Nothing in it has to
+ *     start at zero: the merge pass reads exactly the lists the first pass of the same call has just written.  But two
+ *     calls whose kernels can overlap on one GPU - different streams without an event between them, or two host threads -
+ *     write the same lists and race; order them (one stream, or an event dependency).
+ *   - Like the other calls it only enqueues: results are valid once the caller has synchronised cuda_stream
+ *     (a cudaStream_t cast to void*; NULL = the legacy default stream). */
+#define IA_TOPK_STATIC_LISTS 1024
+#define IA_TOPK_STATIC_BYTES (IA_TOPK_STATIC_LISTS * 32 * 8)
+#define IA_TOPK_STATIC_MAX_CELLS (((int64_t)1) << 40)
+int ia_topk_static(int device, void* cuda_stream, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t* idx_out_dev,
+                   uint16_t* votes_out_dev);
+/* Text describing why the calling thread's most recent ia_topk_static call failed ("" after a success).  The pointer
+ * stays valid until that thread calls ia_topk_static again. */
+const char* ia_topk_static_error(void);
 
 /* a8-a9 - adaptive refinement of one event, entirely on the device: vote the dense grid0, keep the
  * top k, then (levels-1) times: cut every kept box at its per-axis midpoints into 2^5 children

@@ -28,6 +28,7 @@ PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,))
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 112
 
 EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_slab", "ia_topk_keys", "ia_merge_keys", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
+           "ia_topk_static", "ia_topk_static_error",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_residual_fast", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_graph_replays", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
@@ -73,6 +74,9 @@ def load_library(path: str = LIB_PATH):
     lib.ia_track_paper.argtypes = [vp, vp, i32, dbl, dbl, dbl, vp, i32, vp, vp]
     lib.ia_find_hits_paper.argtypes = [vp, vp, i32, dbl, vp, dbl, vp]
     lib.ia_topk.argtypes = [vp, vp, i64, i32, vp, vp]
+    lib.ia_topk_static.argtypes = [i32, vp, vp, i64, i32, vp, vp]
+    lib.ia_topk_static_error.argtypes = []
+    lib.ia_topk_static_error.restype = C.c_char_p
     lib.ia_refine.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_refine_batch.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_vote_host.argtypes = [vp, vp, i32, vp, vp, vp, vp]
@@ -93,6 +97,32 @@ def load_library(path: str = LIB_PATH):
     lib.ia_pad_ulps.argtypes = []
     _lib = lib
     return lib
+
+
+TOPK_STATIC_LISTS = 1024                 # IA_TOPK_STATIC_LISTS
+TOPK_STATIC_MAX_CELLS = 1 << 40          # IA_TOPK_STATIC_MAX_CELLS
+
+
+def ia_topk_static(votes_dev, k, idx_out, votes_out, n_cells=None, stream=None):
+    """ia_topk for callers that must not allocate on the device (see include/ia.h): no context, no torch allocation -
+    the caller owns the accumulator and both outputs (idx_out: int64[k], votes_out: uint16[k], CUDA tensors on the
+    accumulator's device), the work is enqueued on `stream` (default: torch's current stream of that device) and the
+    candidate lists live in the library's fixed 256 KB device array.  Calls on one GPU must not overlap."""
+    import torch
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("libia_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+    dev = votes_dev.device.index
+    if idx_out.dtype != torch.int64 or votes_out.dtype != torch.uint16 or idx_out.numel() < k or votes_out.numel() < k:
+        raise ValueError("idx_out must be int64[k] and votes_out uint16[k]")
+    if idx_out.device != votes_dev.device or votes_out.device != votes_dev.device:
+        raise ValueError("outputs must live on the accumulator's device")
+    n = votes_dev.numel() if n_cells is None else int(n_cells)
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    rc = lib.ia_topk_static(dev, C.c_void_p(s.cuda_stream), _dp(votes_dev), n, int(k), _dp(idx_out), _dp(votes_out))
+    if rc != 0:
+        raise IaError(rc, "ia_topk_static", lib.ia_topk_static_error().decode())
+    return idx_out, votes_out
 
 
 def wires_of(chamber) -> np.ndarray:

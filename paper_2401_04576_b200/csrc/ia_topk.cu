@@ -6,6 +6,9 @@
 // maxima, one compare per lane and one warp vote - the pass is HBM-bound.  Warps are merged per
 // block through shared memory.  Pass 2 (topk_final): the per-block lists of an event are merged and
 // the first k entries written out.  Ties on votes are broken by index ascending, carried in the key.
+#include <cstdio>
+#include <mutex>
+
 #include "ia_internal.h"
 #include "ia_topk.cuh"
 
@@ -161,4 +164,123 @@ cudaError_t launch_merge_keys(ia_ctx* ctx, const unsigned long long* keys, int n
   return err;
 }
 
+// ---- ia_topk_static: the same two passes with the per-block lists in a fixed array of the device image -----------
+// (include/ia.h says who needs this and why).  Everything that concerns the array is in this file: its definition,
+// the one place that asks the runtime for its device address, and the launches that are given that address.
+namespace {
+
+// One sorted 32-key list per block of the first pass.  256 KB on every GPU that loads this module, until process exit.
+static __device__ __align__(256) u64 static_lists[size_t(IA_TOPK_STATIC_LISTS) * 32];
+
+// In host code `static_lists` is only the runtime's handle for the symbol - not an address a kernel could use.  The
+// address on a given device is what cudaGetSymbolAddress returns while that device is current; it is looked up once per
+// device and kept here.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex static_mu;
+u64* static_lists_on[STATIC_MAX_DEVICES] = {};
+thread_local char static_msg[320] = "";
+
+struct CurrentDevice {          // make `dev` current for the scope, restore the caller's device afterwards
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit CurrentDevice(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+  }
+  ~CurrentDevice() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+
+// set-up, once per device, with that device current
+cudaError_t static_lists_address(int device, u64** out) {
+  std::lock_guard<std::mutex> lock(static_mu);
+  if (!static_lists_on[device]) {
+    u64* p = nullptr;
+    const cudaError_t err = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), static_lists);
+    if (err != cudaSuccess) return err;
+    if (!p) return cudaErrorInvalidSymbol;
+    static_lists_on[device] = p;
+  }
+  *out = static_lists_on[device];
+  return cudaSuccess;
+}
+
+int static_fail(int code, const char* fmt, long long a = 0, long long b = 0) {
+  std::snprintf(static_msg, sizeof(static_msg), fmt, a, b);
+  return code;
+}
+
+int static_fail_cuda(const char* what, cudaError_t err) {
+  std::snprintf(static_msg, sizeof(static_msg), "ia_topk_static: %s failed: %s", what, cudaGetErrorString(err));
+  cudaGetLastError();           // a launch-configuration error is sticky until read
+  return IA_ERR_CUDA;
+}
+
+}  // namespace
+
 }  // namespace ia
+
+extern "C" {
+
+int ia_topk_static(int device, void* cuda_stream, const uint16_t* votes_dev, int64_t n_cells, int k, int64_t* idx_out_dev,
+                   uint16_t* votes_out_dev) {
+  using namespace ia;
+  static_msg[0] = 0;
+  if (!votes_dev || !idx_out_dev || !votes_out_dev)
+    return static_fail(IA_ERR_ARG, "ia_topk_static: votes_dev, idx_out_dev and votes_out_dev must be device pointers, not NULL");
+  if (n_cells <= 0 || k <= 0 || k > n_cells)
+    return static_fail(IA_ERR_ARG, "ia_topk_static: needs n_cells >= 1 and 1 <= k <= n_cells (got n_cells = %lld, k = %lld)",
+                       (long long)n_cells, (long long)k);
+  if (k > IA_MAX_K)
+    return static_fail(IA_ERR_CAPACITY, "ia_topk_static: k = %lld is beyond IA_MAX_K = %lld (one key per lane of a warp)",
+                       (long long)k, (long long)IA_MAX_K);
+  if (n_cells > IA_TOPK_STATIC_MAX_CELLS)
+    return static_fail(IA_ERR_CAPACITY, "ia_topk_static: n_cells = %lld is beyond IA_TOPK_STATIC_MAX_CELLS = %lld",
+                       (long long)n_cells, (long long)IA_TOPK_STATIC_MAX_CELLS);
+  int n_dev = 0;
+  cudaError_t err = cudaGetDeviceCount(&n_dev);
+  if (err != cudaSuccess) return static_fail_cuda("cudaGetDeviceCount", err);
+  if (device < 0 || device >= n_dev)
+    return static_fail(IA_ERR_ARG, "ia_topk_static: device %lld does not exist (%lld visible)", (long long)device, (long long)n_dev);
+  if (device >= STATIC_MAX_DEVICES)
+    return static_fail(IA_ERR_CAPACITY, "ia_topk_static: device %lld is beyond the %lld devices the address table holds",
+                       (long long)device, (long long)STATIC_MAX_DEVICES);
+  CurrentDevice cur(device);
+  if (cur.err != cudaSuccess) return static_fail_cuda("cudaSetDevice", cur.err);
+  u64* lists = nullptr;
+  if ((err = static_lists_address(device, &lists)) != cudaSuccess) return static_fail_cuda("cudaGetSymbolAddress(static_lists)", err);
+  // the grid of launch_topk for one accumulator: two blocks per SM, never more than there are groups of chunks -
+  // and never more lists than the array holds
+  int sm = 148;
+  if ((err = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess)
+    return static_fail_cuda("cudaDeviceGetAttribute", err);
+  const int64_t n_chunks = (n_cells + 255) / 256;
+  int64_t want_blocks = int64_t(sm) * IA_TOPK_BLOCKS_PER_SM;
+  if (want_blocks > IA_TOPK_STATIC_LISTS) want_blocks = IA_TOPK_STATIC_LISTS;
+  const int unroll = n_chunks >= want_blocks * (TOPK_THREADS / 32) * TOPK_UNROLL ? TOPK_UNROLL : 1;
+  const int64_t per_block = int64_t(256) * unroll * (TOPK_THREADS / 32);
+  const int64_t max_blocks = (n_cells + per_block - 1) / per_block;
+  int64_t blocks = want_blocks < max_blocks ? want_blocks : max_blocks;
+  if (blocks < 1) blocks = 1;              // 1 <= blocks <= IA_TOPK_STATIC_LISTS from here on
+  const int write_final = blocks == 1;      // one block: its list is the answer, the array is not touched
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const dim3 grid((unsigned)blocks, 1u);
+  u64* no_keys = nullptr;
+  if (unroll == 1)
+    topk_partial<1><<<grid, TOPK_THREADS, 0, stream>>>(votes_dev, n_cells, k, int64_t(0), lists, idx_out_dev, votes_out_dev, no_keys,
+                                                      write_final);
+  else
+    topk_partial<TOPK_UNROLL><<<grid, TOPK_THREADS, 0, stream>>>(votes_dev, n_cells, k, int64_t(0), lists, idx_out_dev, votes_out_dev,
+                                                                no_keys, write_final);
+  if ((err = cudaGetLastError()) != cudaSuccess) return static_fail_cuda("launch of the first pass", err);
+  if (write_final) return IA_OK;
+  topk_final<<<1, TOPK_THREADS, 0, stream>>>(lists, int(blocks), k, idx_out_dev, votes_out_dev, no_keys);
+  if ((err = cudaGetLastError()) != cudaSuccess) return static_fail_cuda("launch of the merge pass", err);
+  return IA_OK;
+}
+
+const char* ia_topk_static_error(void) { return ia::static_msg; }
+
+}  // extern "C"
