@@ -534,6 +534,29 @@ def main():
         run_reference(args, rank, world)
         return
 
+    # --gpus N is a promise about the number of ranks, one per GPU.  Started plainly (no launcher in the environment)
+    # with N > 1, the script starts itself again under torchrun; started under a launcher whose world size is not N,
+    # it stops: a line that says n_gpus = 1 for a run asked to use 8 would be read as a scaling point.
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} asked for, {have} CUDA device(s) visible: not running on fewer "
+                             "(the product path has no CPU fallback)")
+        import socket
+        with socket.socket() as sk:                      # a free port on the loopback interface for the rendezvous
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        sys.stdout.flush()
+        os.execv(sys.executable, cmd)
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE = {world} ranks; "
+                         f"launch with --nproc-per-node {args.gpus} (or plain `python bench.py --gpus {args.gpus}`)")
+
     import torch
     import torch.distributed as dist
     from paper_2401_04576_b200 import binding as b
