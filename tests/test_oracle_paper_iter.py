@@ -13,6 +13,7 @@ F2c  hit finding = condition (4) on one multidimensional interval: equals the (p
 from fractions import Fraction as Fr
 
 import numpy as np
+import pytest
 
 from paper_2401_04576_b200 import eventgen as g
 from oracle import oracle as o
@@ -333,3 +334,62 @@ def test_f2d_transport_of_z0_between_reference_points():
                         turn = 2.0 * np.pi * t.R * t.lam
                         want = want + turn * round((got - want) / turn)
                     assert abs(got - want) < 1e-9, (vertex, seed, unwrap, a, b_, got, want)
+
+
+def _helix_point(xc, yc, R, phi, z_e, lam, theta, r=None):
+    """Eq. (1a-c) L43-47 written out with the turning angle theta = rho s counted from the emission point (direction phi):
+    the helix point, or - r given - the point at distance r from the axis of the helix on the same radius, whose closest
+    point of the helix (in the transverse plane) is that helix point."""
+    rr = R if r is None else r
+    return xc + rr * np.sin(phi + theta), yc - rr * np.cos(phi + theta), z_e + lam * R * theta
+
+
+@pytest.mark.parametrize("vertex", [(0.0, 0.0), (5.0, 0.0), (0.0, 5.0)])
+def test_f2d_z0_against_the_helix_written_out(vertex):
+    """Independent of eventgen.Track.z0_at and of the oracle: for a reference point on the radius through the helix point
+    of turning angle theta, "z where the helix is closest to the reference point" (eq. (1d)) is z_e + lambda R theta
+    by eq. (1c).  Checked three ways for both lambda signs, with theta inside the margin below the emission
+    point (-0.3 < theta < 0), near a full turn, and for emission at the origin, (5, 0) and (0, 5) cm (L123):
+      (i)   Track.z0_at (the generator's statement of the truth the tests compare fits with),
+      (ii)  a brute-force scan of the helix for the point closest to the reference point,
+      (iii) orc_transport_z0 (reading F2d'): the difference between two reference points is lambda R (theta_b - theta_a)."""
+    rng = np.random.default_rng(int(10 * vertex[0] + vertex[1]) + 3)
+    p8 = o.make_params(0.0, flags=8)
+    for trial in range(12):
+        R = rng.uniform(30.0, 38.0)
+        phi = rng.uniform(-np.pi, np.pi)
+        lam = rng.uniform(0.2, 1.2) * (1 if trial % 2 else -1)
+        z_e = rng.uniform(-20.0, 20.0)
+        t = g.Track(R, phi, z_e, lam, vertex[0], vertex[1])
+        xc, yc = t.xc, t.yc
+        # the angle of the emission point in the convention of the unwrapped mode (from the circle point closest to the axis)
+        th_v = np.arctan2(np.sin(phi - np.arctan2(-xc, yc)), np.cos(phi - np.arctan2(-xc, yc)))
+        lo_th, hi_th = -0.3 - th_v, 2.0 * np.pi - 0.3 - th_v        # turning angles the convention can express
+        thetas = np.concatenate([[lo_th + 1e-3, lo_th + 0.15, -1e-3, 1e-3, hi_th - 1e-3, hi_th - 0.2], rng.uniform(0.0, 5.5, 6)])
+        prev = None
+        for theta in thetas:
+            r = R * rng.uniform(0.6, 1.5)                          # off the circle, on the same radius
+            px, py, z_want = _helix_point(xc, yc, R, phi, z_e, lam, theta, r)
+            # (i)
+            assert abs(t.z0_at(px, py, unwrap=True) - z_want) < 1e-9, (vertex, trial, theta)
+            # (ii) brute force over the expressible range of turning angles
+            scan = np.linspace(lo_th, hi_th, 400001)
+            hx, hy, hz = _helix_point(xc, yc, R, phi, z_e, lam, scan)
+            k = int(np.argmin((hx - px) ** 2 + (hy - py) ** 2))
+            assert abs(hz[k] - z_want) <= abs(lam) * R * (scan[1] - scan[0]) + 1e-9
+            # (iii)
+            if prev is not None:
+                f = _fit(xc, yc, R)
+                f["value"][3], f["lam"], f["x_ref"], f["y_ref"] = prev[2], lam, prev[0], prev[1]
+                got = o.transport_z0(p8, f, px, py)
+                assert abs(got - z_want) < 1e-9, (vertex, trial, theta, got, z_want)
+                assert abs((got - prev[2]) - lam * R * (theta - prev[3])) < 1e-9
+            prev = (px, py, z_want, theta)
+        # the principal-value convention (flags 0): two reference points less than half a turn apart
+        p0 = o.make_params(0.0, flags=0)
+        for theta_a, theta_b in ((0.2, 1.9), (2.5, 0.4), (-0.2, 0.3), (3.0, 5.9)):
+            ax, ay, za = _helix_point(xc, yc, R, phi, z_e, lam, theta_a, 1.2 * R)
+            bx, by, zb = _helix_point(xc, yc, R, phi, z_e, lam, theta_b, 0.8 * R)
+            f = _fit(xc, yc, R)
+            f["value"][3], f["lam"], f["x_ref"], f["y_ref"] = za, lam, ax, ay
+            assert abs(o.transport_z0(p0, f, bx, by) - zb) < 1e-9
