@@ -173,6 +173,35 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line))
 
 
+FP32_LANES_PER_SM = 128
+# f1 (paper mode): DADD + DMUL + DFMA thread-instructions the kernel EXECUTES per (voxel, hit) decision, read from the
+# committed capture profiles/r02_vote_paper_ncu.md (420 of 851 instructions).  An executed count, not an op-by-op count of
+# the DAG: it bounds the algorithmic count from above, so the fraction built on it is an upper bound.
+F1_EXECUTED_FP64_INST_PER_EVAL = 420.0
+
+
+def alu_roofline(kernel: str, evals: float, ms: float, local_rank: int, precision: int = 64,
+                 inst_per_eval: float = ALG_FP64_INST_PER_EVAL, count_kind: str = "algorithmic", note: str | None = None):
+    """roofline object of an ALU-bound leg: inst_per_eval x evals / time against SMs x lanes x maximum SM clock (the
+    derivation of DESIGN.md 6; FP32 intervals run the same DAG, instruction for instruction, on the 128-lane FP32 pipe)."""
+    import torch
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    try:
+        f_max_mhz = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("sm_max_mhz", 1965.0))
+    except Exception:
+        f_max_mhz = 1965.0
+    lanes = FP64_LANES_PER_SM if precision == 64 else FP32_LANES_PER_SM
+    peak = n_sm * lanes * f_max_mhz * 1e6
+    achieved = inst_per_eval * evals / (ms * 1e-3)
+    r = {"bound": "alu", "kernel": kernel, "achieved": achieved / 1e12, "peak": peak / 1e12,
+         "unit": f"T FP{precision} inst/s", "frac": achieved / peak, "traffic": None,
+         "alg_inst_per_eval": inst_per_eval, "count_kind": count_kind, "kernel_ms": ms,
+         "peak_source": f"derived: {n_sm} SMs x {lanes} FP{precision} lanes x {f_max_mhz:.0f} MHz (DESIGN.md 6)"}
+    if note:
+        r["note"] = note
+    return r
+
+
 def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
     """SURVEY 8(f) f1 on 50 x 50 x 40 x 20 voxels (iteration 1) x the C1 event's 40 hits; one
     evaluation = one (voxel, hit) decision = 2 lambda signs x 2 drift signs x 2 tolerance ends of the mid-voxel d_Ax."""
@@ -205,6 +234,10 @@ def paper_mode_leg(local_rank: int, steps: int, warmup: int = 1):
                         "momentum fixed, 2 lambda-sign accumulators, mid-voxel d_Ax, tol 0.045",
             "ms": ms, "voxel_hit_evals_per_s": nvox * ev1.n_hits / (ms * 1e-3), "evals_per_step": nvox * ev1.n_hits,
             "gpu_launches": int(launches),
+            "roofline": alu_roofline("vote_paper_kernel", nvox * ev1.n_hits, ms, local_rank,
+                                     inst_per_eval=F1_EXECUTED_FP64_INST_PER_EVAL, count_kind="executed (ncu), upper bound",
+                                     note="one evaluation = one (voxel, hit) decision: 2 lambda signs x 2 drift signs, "
+                                          "d_Ax at the voxel centre in rn double, condition (4) in intervals"),
             "context": "paper: about 1.2 s per track for 3 such passes of < 1 M voxels on 4 x K80 (L117)"}
 
 
@@ -218,7 +251,7 @@ def paper_track_leg(local_rank: int, n_tracks: int = 16, extra_passes: int = 0, 
     ch = g.chamber_paper()
     ctx = b.Context(local_rank)
     ctx.ia_load_geometry(b.wires_of(ch))
-    ctx.ia_set_params(tol, flags=8)
+    ctx.ia_set_params(tol, flags=b.FLAG_FULL_TURN)
     lo, hi = np.array(g.PAPER_BOX_LO), np.array(g.PAPER_BOX_HI)
     # beyond Table 1 (--f2-extra-passes): finer windows around the third pass's value - 0.2 mm voxels, then 0.05 mm
     extra = [((0.5, 0.5, 0.5, 8.0), (50, 50, 50, 16)), ((0.1, 0.1, 0.1, 2.0), (40, 40, 40, 16))][:extra_passes]
@@ -438,6 +471,10 @@ def run_c3(args, rank, world, local_rank, barrier):
                        "evals_per_step": evals, "l2": "vote scratch (64 KB per event) rewritten every step"},
             "events_per_s": n_ev * world / (ms_step * 1e-3), "gpu_launches": int(launches), "graph_replays": int(replays),
             "clocks": clocks,
+            "roofline": alu_roofline("ia_refine_batch: every launch of the call (the start-grid vote is about 90 % of it)",
+                                     evals, ms_step, local_rank, precision=args.precision,
+                                     note="evals = events x (8^5 + (passes-1) x K x 32) x hits; staging, top-K, gather and "
+                                          "parameter kernels are inside the time and add no counted instruction"),
             "cpu_baseline": {"value": n_s * evals / n_ev / dt_o, "unit": UNIT, "cores": o.max_threads(), "kind": "oracle",
                              "sample": f"orc_refine_batch on the first {n_s} event(s) ({dt_o:.2f} s)",
                              "events_per_s": n_s / dt_o, "boxes_identical": same},
@@ -518,7 +555,10 @@ def main():
     ap.add_argument("--f2-noise", type=int, default=0, help="workload F2: noise hits per event (the paper has none)")
     ap.add_argument("--f2-smear", type=float, default=0.0, help="workload F2: drift-distance smearing, cm (the paper has none)")
     ap.add_argument("--f2-tol", type=float, default=0.0, help="workload F2: vote tolerance, cm")
-    ap.add_argument("--f2-fixed-ref", action="store_true", help="workload F2: keep the reference point at (0,0) (no L98 update)")
+    ap.add_argument("--f2-move-ref", action="store_true",
+                    help="workload F2: vote passes 2 and 3 with the reference point of L98 (reading F2d').  Off by default: with "
+                         "the literal three passes the moved point recovers fewer tracks than the fixed one (DESIGN.md 14)")
+    ap.add_argument("--f2-fixed-ref", action="store_true", help="workload F2: the default, kept for old command lines")
     ap.add_argument("--f2-vertex", type=float, nargs=2, default=[0.0, 0.0], help="workload F2: emission point (x y) in cm (L123)")
     ap.add_argument("--flags", type=int, default=0, help="ia_params.flags for the dense workloads (1: general kernel, 16: rigorous Phi)")
     ap.add_argument("--split-event", action="store_true",
@@ -575,7 +615,7 @@ def main():
     if args.workload == "F2":
         barrier()
         r = paper_track_leg(local_rank, n_tracks=max(args.steps, 1), extra_passes=args.f2_extra_passes,
-                            n_noise=args.f2_noise, smear=args.f2_smear, tol=args.f2_tol, move_ref=not args.f2_fixed_ref,
+                            n_noise=args.f2_noise, smear=args.f2_smear, tol=args.f2_tol, move_ref=args.f2_move_ref and not args.f2_fixed_ref,
                             vertex=(args.f2_vertex[0], args.f2_vertex[1]))
         if rank == 0:
             print(json.dumps({"metric": "paper-scheme tracks/s", "value": r["tracks_per_s"] * world, "unit": "tracks/s",
@@ -606,7 +646,7 @@ def main():
                               "unit": "evals/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                               "ms_per_step": r["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                               "dtype": "f64", "data": "synthetic", "config": {"workload": r["workload"]},
-                              "gpu_launches": r["gpu_launches"]}))
+                              "gpu_launches": r["gpu_launches"], "roofline": r["roofline"]}))
         if world > 1:
             dist.destroy_process_group()
         return
@@ -737,11 +777,11 @@ def main():
         except Exception as exc:  # pragma: no cover
             line["roofline"]["probe_error"] = str(exc)
 
-        # ---- prefilter (ia_params.flags bit 6): the same grid with hits skipped that a crude enclosure excludes for a whole
+        # ---- prefilter (IA_FLAG_PREFILTER): the same grid with hits skipped that a crude enclosure excludes for a whole
         # warp and z0 tile; identical accumulator (checked here on the device), NOT the brute-force evaluation the headline
         # value and the roofline describe
         try:
-            ctx.ia_set_params(g.TOL, flags=args.flags | 64)
+            ctx.ia_set_params(g.TOL, flags=args.flags | b.FLAG_PREFILTER)
             votes_pf = torch.empty_like(votes)
             ctx.ia_vote(hd, ev.n_hits, g.BOX_LO, g.BOX_HI, dims, votes_out=votes_pf)
             torch.cuda.synchronize()
@@ -821,6 +861,8 @@ def main():
             eps[f"fp{prec}"] = {"events_per_s": n_ev / (ms * 1e-3), "ms": ms, "e2e_events_per_s": n_ev / dt_h,
                                 "graph_replays": ctx3.ia_graph_replays(),
                                 "evals_per_s": n_ev * (8 ** 5 + 7 * 8 * 32) * 30 / (ms * 1e-3),
+                                "roofline": alu_roofline("ia_refine_batch: every launch of the call", n_ev * (8 ** 5 + 7 * 8 * 32) * 30,
+                                                         ms, local_rank, precision=prec),
                                 "truth": refine_truth_stats(ctx3, hd3, off, evs, b.boxes_to_numpy(boxes, (n_ev, 8, 8)),
                                                             par.cpu().numpy().reshape(n_ev, -1), (8,) * 5, 8)}
         line["events_per_s"] = {"workload": "C3: BASELINE.json configs[3], 1024 events x 30 hits, 8^5 start, K=8, 8 passes",
@@ -832,7 +874,7 @@ def main():
             line["paper_mode"] = paper_mode_leg(local_rank, steps=5)
         except Exception as exc:  # pragma: no cover
             line["paper_mode"] = {"error": str(exc)}
-        # ---- f3: rigorous-Phi mode (flags bit 4) against the series mode, both in the general-form kernel ----------
+        # ---- f3: rigorous-Phi mode (IA_FLAG_RIGOROUS_PHI) against the series mode, both in the general-form kernel ----------
         try:
             ch1 = g.chamber_c1()
             ev1 = g.make_event(ch1, 1, n_noise=20)
@@ -843,7 +885,8 @@ def main():
             nr = int(np.prod(rdims))
             vr = torch.empty(nr, dtype=torch.uint16, device=f"cuda:{local_rank}")
             rr = {}
-            for name, fl in (("fast_series", 0), ("fast_rigorous", 16), ("general_series", 1), ("general_rigorous", 17)):
+            for name, fl in (("fast_series", 0), ("fast_rigorous", b.FLAG_RIGOROUS_PHI), ("general_series", b.FLAG_GENERAL),
+                             ("general_rigorous", b.FLAG_GENERAL | b.FLAG_RIGOROUS_PHI)):
                 ctxr.ia_set_params(g.TOL, flags=fl)
                 ctxr.ia_vote(hdr, ev1.n_hits, g.BOX_LO, g.BOX_HI, rdims, votes_out=vr)
                 torch.cuda.synchronize()
@@ -857,6 +900,12 @@ def main():
                 rr[name] = {"ms": ms, "evals_per_s": nr * ev1.n_hits / (ms * 1e-3), "sum_votes": int(vr.to(torch.int64).sum().item())}
             rr["workload"] = ("f3: dense 24^5 x 40 hits (C1 event): series (A.8) vs verified fixed point of (A.6), in the "
                               "sign-specialised kernels (flags 0 / 16) and in the general-form kernel (flags 1 / 17)")
+            for name in ("fast_series", "fast_rigorous"):
+                rr[name]["roofline"] = alu_roofline(
+                    "vote_dense_fast_kernel" + (" (rigorous Phi)" if name == "fast_rigorous" else ""), nr * ev1.n_hits,
+                    rr[name]["ms"], local_rank,
+                    note=None if name == "fast_series" else "counted with the series DAG's instructions: the verification "
+                    "rounds of (A.6) are overhead of this mode, not algorithmic work")
             rr["cost_ratio"] = rr["fast_rigorous"]["ms"] / rr["fast_series"]["ms"]
             rr["cost_ratio_general_form"] = rr["general_rigorous"]["ms"] / rr["general_series"]["ms"]
             rr["votes_fast_equal_general"] = rr["fast_rigorous"]["sum_votes"] == rr["general_rigorous"]["sum_votes"]
@@ -864,20 +913,12 @@ def main():
             ctxr.close()
         except Exception as exc:  # pragma: no cover
             line["rigorous_phi"] = {"error": str(exc)}
-        # f2: the paper's scheme with and without the reference-point update of L98, and with displaced emission (L123)
-        try:
-            chp = g.chamber_paper()
-            n_tr = 256
-            evs0 = [g.make_event_paper(chp, 500 + i) for i in range(n_tr)]
-            line["paper_track"] = paper_track_leg(local_rank, move_ref=True, evs=evs0)
-            line["paper_track_fixed_ref"] = paper_track_leg(local_rank, move_ref=False, evs=evs0)
-            for name, vx in (("paper_track_emitted_at_5_0", (5.0, 0.0)), ("paper_track_emitted_at_0_5", (0.0, 5.0))):
-                evsv = [g.make_event_paper(chp, 500 + i, vertex=vx) for i in range(n_tr // 2)]
-                line[name] = paper_track_leg(local_rank, move_ref=True, vertex=vx, evs=evsv)
-                line[name + "_fixed_ref"] = paper_track_leg(local_rank, move_ref=False, vertex=vx, evs=evsv)
-        except Exception as exc:  # pragma: no cover
-            line["paper_track"] = {"error": str(exc)}
+        # (the paper's three-pass scheme, f2, is a workload of its own: --workload F2)
 
+    # the contract's keys last: a reader of the tail of a long line sees the headline, not a side leg
+    last = ("topk", "roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches", "config", "metric", "value", "unit", "n_gpus",
+            "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline", "dtype", "data")
+    line = {**{k_: v_ for k_, v_ in line.items() if k_ not in last}, **{k_: line[k_] for k_ in last if k_ in line}}
     print(json.dumps(line))
     ctx.close()
     if world > 1:

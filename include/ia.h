@@ -77,28 +77,46 @@ typedef struct {
   double drift; /* cm */
 } ia_hit;
 
+/* Bits of ia_params.flags.  Every bit but IA_FLAG_FULL_TURN, IA_FLAG_RIGOROUS_PHI leaves the results unchanged. */
+enum {
+  /* dense vote: the general, sign-agnostic kernel (interval DAG S4-S8 as written, (A.5b) L183 / (A.8a-c) L211-216)
+   * instead of the sign-specialised one; same results, kept for cross-checks */
+  IA_FLAG_GENERAL = 1u << 0,
+  /* sign-specialised dense kernel: force the one-body variant (sign classes decided at run time; default for coarse
+   * xy cells) ... */
+  IA_FLAG_ONE_BODY = 1u << 1,
+  /* ... or the three-body variant (one body per sign class of the hit; default for fine xy cells).  Same results:
+   * the default is picked from the xy cell width for speed only */
+  IA_FLAG_THREE_BODY = 1u << 2,
+  /* paper-mode calls only: tracks of up to one turn emitted near the z axis (reading M6) - the
+   * turning angle phi_Ax - phi0 of (A.8d) L218 is theta(wire point) - theta(reference point), theta in
+   * [-0.3, 2 pi - 0.3) counted from the point of the base circle closest to the axis, instead of the principal value
+   * in (-pi, pi] */
+  IA_FLAG_FULL_TURN = 1u << 3,
+  /* 5-D interval calls: Phi - Phi_Ax is not the series (A.8a-c) L211-216 but a verified enclosure of the fixed point of
+   * the angular equation (A.6) L187 ("solved numerically", L220), obtained by inflation from the series enclosure
+   * (reading f3): restores the guarantee of L80 at tol -> 0.  ia_vote runs it in the sign-specialised dense and
+   * children kernels (several times the cost of the series mode), the explicit-box kernel in the general form */
+  IA_FLAG_RIGOROUS_PHI = 1u << 4,
+  /* ia_refine / ia_refine_batch always enqueue their launches one by one (default: a call repeated with identical
+   * arguments and buffers is replayed as a CUDA graph from its third occurrence on) */
+  IA_FLAG_NO_GRAPH = 1u << 5,
+  /* sign-specialised dense kernel: before the fine evaluation of a hit a warp asks a crude enclosure of the same
+   * residual (magnitude bounds of every step of S4-S8, both drift signs, all the z0 cells of its tile at once) whether
+   * 0 can be excluded for all its cells, and skips the hit if so.  The votes are identical (a wider enclosure that
+   * excludes 0 implies the finer one does, L80), but the kernel no longer evaluates every (cell, hit) in full -
+   * default off: north_star's metric is the brute-force evaluation of condition (4) L74-78 */
+  IA_FLAG_PREFILTER = 1u << 6,
+  /* the kernels of the vote / top-K / refinement chain are launched without the programmatic-dependent-launch
+   * attribute (default: with it - each of them starts by waiting for the kernels in front, so that its launch overlaps
+   * their execution) */
+  IA_FLAG_NO_PDL = 1u << 7,
+  IA_FLAG_ALL = (1u << 8) - 1 /* other bits must be 0 (IA_ERR_ARG) */
+};
+
 /* tol: vote tolerance on the drift distance, D = [max(d-tol,0), d+tol] (S1, G6).
  * (x_ref, y_ref): reference point of eq. (1d); z_ref: reference plane of (A.4c-e) L172-176.
- * precision: 64 or 32 = type of the interval endpoints (G22).  flags: bit 0 = vote the dense grid
- * with the general (sign-agnostic) kernel instead of the sign-specialised one (same results; for
- * cross-checks); bits 1 / 2 = force the one-body / three-body variant of the sign-specialised
- * dense kernel (same results; default: picked from the xy cell width); bit 3 (paper-mode calls only):
- * tracks of up to one turn emitted near the z axis (reading M6) - the turning angle
- * phi_Ax - phi0 of (A.8d) is theta(wire point) - theta(reference point), theta in [-0.3, 2 pi - 0.3) counted from the
- * point of the base circle closest to the axis, instead of the principal value in (-pi, pi]; bit 4 (the 5-D interval calls): Phi - Phi_Ax is not the
- * series (A.8) but a verified enclosure of the fixed point of the angular equation (A.6), obtained by
- * inflation from the series enclosure (reading f3): restores the guarantee of L80 at tol -> 0; ia_vote runs it in the
- * sign-specialised dense and children kernels (about 6 x the series mode), the explicit-box kernel in the general
- * form; bit 5: ia_refine / ia_refine_batch always enqueue
- * their launches one by one (default: a call repeated with identical arguments and buffers is replayed as a
- * CUDA graph from its third occurrence on); bit 6 (sign-specialised dense kernel): prefilter - before the fine
- * evaluation of a hit a warp asks a crude enclosure of the same residual (magnitude bounds of every step of S4-S8, both
- * drift signs, all the z0 cells of its tile at once) whether 0 can be excluded for all its cells, and skips the hit if
- * so: the votes are identical (a wider enclosure that excludes 0 implies the finer one does, L80), the kernel no longer
- * evaluates every (cell, hit) in full - default off: north_star's metric is the brute-force evaluation; bit 7: the
- * kernels of the vote / top-K / refinement chain are launched without the programmatic-dependent-launch attribute
- * (default: with it - each of them starts by waiting for the kernels in front, so that its launch overlaps their
- * execution; same results either way); other bits must be 0. */
+ * precision: 64 or 32 = type of the interval endpoints (G22).  flags: an OR of IA_FLAG_* bits. */
 typedef struct {
   double tol;
   double x_ref, y_ref, z_ref;
@@ -296,13 +314,20 @@ int ia_refine_batch(ia_ctx* ctx, const ia_hit* hits_dev, const int32_t* hit_offs
 
 /* End-to-end variants: every pointer is HOST memory (pinned for full copy speed).  They validate
  * the hits, copy them to the device, run the call above and copy the result back, then
- * synchronise the stream.  ia_vote_host sends an accumulator of 32 MB or more in up to 8 slabs of xc cells
- * (the launches of ia_vote_slab), slab i copied on a second stream while slab i+1 is voted: same counts. */
+ * synchronise the stream.  ia_vote_host sends a large accumulator in slabs of xc cells (the launches of
+ * ia_vote_slab), slab i copied on a second stream while slab i+1 is voted: same counts.  The number of slabs is
+ * min(8, grid_dims[0], cells / min_cells) with min_cells = 16 Mi cells (32 MB of counts) by default, and the split is
+ * taken from 2 slabs on - that is, for accumulators of 64 MB and more.  On any error both streams are synchronised
+ * before the call returns: nothing writes to votes_out_host afterwards. */
 int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double box_lo[5], const double box_hi[5],
                  const int32_t grid_dims[5], uint16_t* votes_out_host);
 int ia_refine_batch_host(ia_ctx* ctx, const ia_hit* hits_host, const int32_t* hit_offsets_host, int n_events,
                          const double box_lo[5], const double box_hi[5], const int32_t grid0[5], int levels, int k,
                          ia_box* boxes_out_host, double* params_out_host);
+/* Smallest slab of ia_vote_host, in cells (>= 1; default 16 Mi).  A tuning knob - smaller slabs start the first copy
+ * earlier but add partial waves of blocks to every launch - and the handle by which the tests drive the slab pipeline
+ * on small, ragged grids.  The counts do not depend on it. */
+int ia_set_host_slab_min(ia_ctx* ctx, int64_t min_cells);
 
 /* Diagnostics for parity tracing (G25): the enclosure f = R_Ax^2 - (R + d_Ax)^2 of every
  * (box, hit, drift sign): out_dev[((b*n_hits + h)*2 + s)*4 + {0,1,2,3}] = f.lo, f.hi,

@@ -28,11 +28,14 @@ PASS_DT = np.dtype([("lo", "f8", (4,)), ("hi", "f8", (4,)), ("dims", "i4", (4,))
 assert WIRE_DT.itemsize == 56 and HIT_DT.itemsize == 16 and BOX_DT.itemsize == 88 and FIT_DT.itemsize == 112
 
 EXPORTS = ("ia_create", "ia_destroy", "ia_load_geometry", "ia_set_params", "ia_vote", "ia_vote_slab", "ia_topk_keys", "ia_merge_keys", "ia_vote_boxes", "ia_vote_paper", "ia_select_max_paper", "ia_find_hits_paper", "ia_track_paper", "ia_topk",
-           "ia_topk_static", "ia_topk_static_error",
+           "ia_topk_static", "ia_topk_static_error", "ia_set_host_slab_min",
            "ia_refine", "ia_refine_batch", "ia_vote_host", "ia_refine_batch_host", "ia_residual", "ia_residual_fast", "ia_prim",
            "ia_probe_fp64", "ia_device_status", "ia_launch_count", "ia_graph_replays", "ia_strerror", "ia_last_cuda_error", "ia_pad_ulps")
 
 KEY_LIST = 32      # IA_KEY_LIST
+# IA_FLAG_* of include/ia.h (bits of ia_params.flags)
+FLAG_GENERAL, FLAG_ONE_BODY, FLAG_THREE_BODY, FLAG_FULL_TURN = 1, 2, 4, 8
+FLAG_RIGOROUS_PHI, FLAG_NO_GRAPH, FLAG_PREFILTER, FLAG_NO_PDL = 16, 32, 64, 128
 
 
 class IaParams(C.Structure):
@@ -81,6 +84,7 @@ def load_library(path: str = LIB_PATH):
     lib.ia_refine_batch.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, i32, i32, vp, vp]
     lib.ia_vote_host.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.ia_refine_batch_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, i32, vp, vp]
+    lib.ia_set_host_slab_min.argtypes = [vp, i64]
     lib.ia_residual.argtypes = [vp, vp, i32, vp, vp, i64, vp]
     lib.ia_residual_fast.argtypes = [vp, vp, i32, vp, vp, i64, vp]
     lib.ia_prim.argtypes = [vp, i32, i32, vp, vp, i64, vp]
@@ -360,6 +364,9 @@ class Context:
         self._chk(self.lib.ia_vote_host(self.h, _hp(hits), len(hits), _hp(lo), _hp(hi), _hp(dims), _hp(votes_out)),
                   "ia_vote_host")
         return votes_out
+
+    def ia_set_host_slab_min(self, min_cells: int):
+        self._chk(self.lib.ia_set_host_slab_min(self.h, int(min_cells)), "ia_set_host_slab_min")
 
     def ia_refine_batch_host(self, hits: np.ndarray, hit_offsets: np.ndarray, box_lo, box_hi, grid0, levels, k,
                              boxes: np.ndarray | None = None, params: np.ndarray | None = None):

@@ -109,7 +109,7 @@ int refine_impl(ia_ctx* ctx, const HitSpan& sp, const double lo[5], const double
   };
   fill_scratch(key);
   RefineGraph& rg = ctx->rgraph;
-  const bool use_graphs = !(ctx->params.flags & 32u);
+  const bool use_graphs = !(ctx->params.flags & IA_FLAG_NO_GRAPH);
   const bool same = rg.seen > 0 && std::memcmp(&rg.key, &key, sizeof(key)) == 0;
   if (use_graphs && same && rg.exec) {
     IA_CUDA(ctx, cudaGraphLaunch(rg.exec, ctx->stream));
@@ -264,7 +264,7 @@ int ia_set_params(ia_ctx* ctx, const ia_params* p) {
       !std::isfinite(p->z_ref))
     return IA_ERR_ARG;
   if (p->precision != 64 && p->precision != 32) return IA_ERR_ARG;
-  if (p->flags & ~255u) return IA_ERR_ARG;
+  if (p->flags & ~unsigned(IA_FLAG_ALL)) return IA_ERR_ARG;
   ctx->params = *p;
   return IA_OK;
 }
@@ -508,8 +508,9 @@ int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double 
   const ia_hit* hits_dev = static_cast<const ia_hit*>(ctx->io_a.p);
   // A large accumulator (C4: 2.1 GB, 38 ms of PCIe after 1.2 s of vote) goes out in slabs of xc cells: slab i is copied
   // on a second stream while slab i+1 is voted (ia_vote_slab's launch: same edges, same counts), so only the last copy
-  // is exposed.  At most 8 slabs of at least 32 MB: more would add partial waves of blocks to every launch.
-  const int64_t slab_min = int64_t(16) << 20;            // cells
+  // is exposed.  At most 8 slabs of at least host_slab_min cells (16 M = 32 MB unless ia_set_host_slab_min changed it):
+  // more would add partial waves of blocks to every launch.
+  const int64_t slab_min = ctx->host_slab_min;
   int n_slabs = int(std::min<int64_t>(std::min<int64_t>(8, g.n[0]), g.cells / slab_min));
   if (n_slabs < 2) {
     rc = ia_vote(ctx, hits_dev, n_hits, box_lo, box_hi, grid_dims, acc);
@@ -526,20 +527,36 @@ int ia_vote_host(ia_ctx* ctx, const ia_hit* hits_host, int n_hits, const double 
   HitSpan sp = single_span(hits_dev, n_hits);
   IA_CUDA(ctx, launch_stage_hits(ctx, sp));
   const int64_t per_ix = g.cells / g.n[0];
-  for (int i = 0; i < n_slabs; ++i) {
-    const int b0 = int(int64_t(g.n[0]) * i / n_slabs), e0 = int(int64_t(g.n[0]) * (i + 1) / n_slabs);
-    GridDesc gs = g;
-    gs.ix0 = b0;
-    gs.nx_run = e0 - b0;
-    gs.cells = per_ix * gs.nx_run;
-    IA_CUDA(ctx, launch_vote_dense(ctx, sp, gs, acc + per_ix * b0));
-    IA_CUDA(ctx, cudaEventRecord(ctx->slab_done, ctx->stream));
-    IA_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_done, 0));
-    IA_CUDA(ctx, cudaMemcpyAsync(votes_out_host + per_ix * b0, acc + per_ix * b0, size_t(gs.cells) * sizeof(uint16_t),
-                                 cudaMemcpyDeviceToHost, ctx->copy_stream));
-  }
-  IA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  IA_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
+  auto pipeline = [&]() -> cudaError_t {
+    cudaError_t e;
+    for (int i = 0; i < n_slabs; ++i) {
+      const int b0 = int(int64_t(g.n[0]) * i / n_slabs), e0 = int(int64_t(g.n[0]) * (i + 1) / n_slabs);
+      GridDesc gs = g;
+      gs.ix0 = b0;
+      gs.nx_run = e0 - b0;
+      gs.cells = per_ix * gs.nx_run;
+      if ((e = launch_vote_dense(ctx, sp, gs, acc + per_ix * b0)) != cudaSuccess) return e;
+      if ((e = cudaEventRecord(ctx->slab_done, ctx->stream)) != cudaSuccess) return e;
+      if ((e = cudaStreamWaitEvent(ctx->copy_stream, ctx->slab_done, 0)) != cudaSuccess) return e;
+      if ((e = cudaMemcpyAsync(votes_out_host + per_ix * b0, acc + per_ix * b0, size_t(gs.cells) * sizeof(uint16_t),
+                               cudaMemcpyDeviceToHost, ctx->copy_stream)) != cudaSuccess)
+        return e;
+    }
+    return cudaSuccess;
+  };
+  const cudaError_t pe = pipeline();
+  // success or not, nothing may still be writing into the caller's buffer when this call returns
+  const cudaError_t s1 = cudaStreamSynchronize(ctx->stream);
+  const cudaError_t s2 = cudaStreamSynchronize(ctx->copy_stream);
+  IA_CUDA(ctx, pe);
+  IA_CUDA(ctx, s1);
+  IA_CUDA(ctx, s2);
+  return IA_OK;
+}
+
+int ia_set_host_slab_min(ia_ctx* ctx, int64_t min_cells) {
+  if (!ctx || min_cells < 1) return IA_ERR_ARG;
+  ctx->host_slab_min = min_cells;
   return IA_OK;
 }
 

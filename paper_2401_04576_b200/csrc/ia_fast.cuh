@@ -2,7 +2,7 @@
 //
 // Same expression DAG as ia_residual.cuh and the same association order.  What changes is how each
 // interval product is formed.  The dense kernel is bound by the FP64 pipe and by the dependency
-// latency around it (profiles/r01_pipe_probe.md: a dependent FP64 instruction issues 8 cycles after
+// latency around it (profiles/r02_pipe_probe.md: a dependent FP64 instruction issues 8 cycles after
 // its producer; profiles/r01_vote_dense_fast_c1_ncu.md), and the textbook sign-case product - pick the
 // partner endpoint by the sign of x, then multiply (2 DMUL + 2 ISETP + 4 FSEL) - puts a compare and a
 // select between every pair of FP64 instructions.  The form below is 4 FP64 instructions and nothing else:
@@ -477,7 +477,7 @@ template <class T> struct __align__(16) HitF {
   Iv<T> iQ, iR, c2, s2[2];         // interval forms, general fallback only
   // scalars after the pairs: every Iv / MR above sits on a 16-byte (8-byte in float) boundary, which the vector
   // ld.shared of HitLds (ia_fastq.cuh) needs
-  T cAabs, sAabs, c2abs, s2abs, dphiabs, iQhi, RAhi, dm;   // magnitudes for the crude enclosure (prefilter, flags bit 6)
+  T cAabs, sAabs, c2abs, s2abs, dphiabs, iQhi, RAhi, dm;   // magnitudes for the crude enclosure (prefilter, IA_FLAG_PREFILTER)
   T twoT;                          // 2 |tan tau| (exact)
   T Tabs;                          // |tan tau|
   T Dlo, Dhi;
@@ -564,7 +564,7 @@ template <class T> struct PairC {
   MR<T> Lm, LRm;       // midpoint forms of lambda and lambda R
   Iv<T> L2;            // lambda^2
 };
-// ---- crude enclosure of f over a whole z0 tile (prefilter, flags bit 6) --------------------------------------------
+// ---- crude enclosure of f over a whole z0 tile (prefilter, IA_FLAG_PREFILTER) --------------------------------------------
 // Condition (4) asks whether 0 is in the interval extension F of f = R_Ax^2 - (R + d_Ax)^2.  Any enclosure G of F answers
 // "no" safely: 0 not in G implies 0 not in F ("if the condition is false the solution is not in the
 // voxel" holds for every valid enclosure; the paper's own disk pre-filter L64-72 is such a cheaper test).  G here bounds,
@@ -628,7 +628,7 @@ template <class T> IA_DEV HitP<T> hit_prepare(const HitF<T>& h, int va, const Pa
 // The two signs of one (cell, hit) are independent dependency chains that share zA, t1 and the
 // magnitude sort of zA.  Written side by side they give the FP64 pipe four independent instructions
 // per step (two endpoints x two signs), which covers its 8-cycle dependent-issue latency from inside
-// one warp (profiles/r01_pipe_probe.md).
+// one warp (profiles/r02_pipe_probe.md).
 // D- = -D+ exactly, hence lambda D- c_Ax = -(lambda D+ c_Ax) exactly (negation commutes with directed
 // rounding); G and K differ between the signs and are kept for both.
 template <class T> struct Pass2 {

@@ -1,6 +1,6 @@
 // ia_fastq.cuh - S4-S8 for both drift signs of one (cell, hit), scheduled for the FP64 pipe of sm_100a.
 //
-// Why this file exists (measured on B200, profiles/r01_pipe_probe.md and DESIGN.md section 6.1): a
+// Why this file exists (measured on B200, profiles/r02_pipe_probe.md and DESIGN.md section 6.1): a
 // sub-partition issues one FP64 warp instruction per 2 cycles, a dependent one 8 cycles after its
 // producer, and the dense kernel runs 4 warps per sub-partition (128 registers per thread), each of
 // which stalls on FP64 -> compare/select -> FP64 dependencies.  Four independent FP64 instructions in a
@@ -469,7 +469,7 @@ IA_DEV unsigned pass_vote_q(const H& h, int va, const Pass2<T>& pc, const PairC<
 // dependent quads are short uniform switches.  Same arithmetic as pass_vote_q<SS> for every class.
 IA_DEV int opaque_i(int x) { asm volatile("" : "+r"(x)); return x; }
 
-// ---- rigorous Phi in the sign-specialised form (ia_params.flags bit 4; reading f3) ------------------
+// ---- rigorous Phi in the sign-specialised form (ia_params.IA_FLAG_RIGOROUS_PHI; reading f3) ------------------
 // atan on [-1/16, 1/16]: odd Taylor polynomial, round-to-nearest Horner; truncation t^14/15 < 2^-59 relative (double,
 // terms to t^13) resp. t^8/9 < 2^-35 (float, terms to t^7), rounding below 1 ulp: inside the relative pad 2^-50 (2^-21).
 template <class T> struct AtanC;

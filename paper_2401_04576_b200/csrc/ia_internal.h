@@ -76,6 +76,7 @@ struct ia_ctx {
   int* status = nullptr;     // device: sticky error flag
   cudaStream_t copy_stream = nullptr;   // ia_vote_host: device->host copies of finished slabs, beside the vote
   cudaEvent_t slab_done = nullptr;
+  int64_t host_slab_min = int64_t(16) << 20;   // ia_vote_host: smallest slab, in cells (ia_set_host_slab_min)
   int64_t launches = 0;
   int64_t graph_replays = 0;  // refinement calls served by cudaGraphLaunch
   cudaError_t last_err = cudaSuccess;
@@ -90,7 +91,7 @@ namespace ia {
 // its blocks start as the last blocks of N leave and wait in griddepcontrol.wait - the first statement of every kernel
 // of the chain, pdl_wait() - until the grids in front have completed and their writes are visible (it returns at once
 // if there are none).  Nothing is read or written early, and completion stays transitive along the chain.  Only kernels
-// that begin with pdl_wait() may be launched through launch_k.  ia_params.flags bit 7 switches the attribute off.
+// that begin with pdl_wait() may be launched through launch_k.  IA_FLAG_NO_PDL switches the attribute off.
 // Measured on C2: 0.2175 ms against 0.2249 replayed as a graph, 0.2187 against 0.2772 launched one by one.
 #ifdef __CUDACC__
 // (an early griddepcontrol.launch_dependents after the wait was tried: C2 0.222 ms against 0.2175 without it)
@@ -107,7 +108,7 @@ cudaError_t launch_k(ia_ctx* ctx, void (*kernel)(KArgs...), dim3 grid, dim3 bloc
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = (ctx->params.flags & 128u) ? 0 : 1;
+  cfg.numAttrs = (ctx->params.flags & IA_FLAG_NO_PDL) ? 0 : 1;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 #endif

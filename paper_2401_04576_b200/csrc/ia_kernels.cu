@@ -51,7 +51,7 @@ __device__ HitC<T> make_hitc(const double* __restrict__ wires, int n_wires, ia_h
   c.Dlo = mx(R::add_dn(d, -tol), T(0));                          // S1 (G6)
   c.Dhi = R::add_up(d, tol);
   c.zref = zr;
-  c._pad = (p.flags & 16u) ? 1 : 0;        // rigorous-Phi mode travels with the staged hit (HitS::rig)
+  c._pad = (p.flags & IA_FLAG_RIGOROUS_PHI) ? 1 : 0;        // rigorous-Phi mode travels with the staged hit (HitS::rig)
   return c;
 }
 
@@ -360,13 +360,13 @@ cudaError_t launch_refine_level(ia_ctx* ctx, const HitSpan& sp, int lev, int lev
   int n_splits = 1;
   uint16_t* partial = nullptr;
   cudaError_t err;
-  if (!(ctx->params.flags & 1u)) {
-    // sign-specialised form, a4 shared by the children of an xy sub-cell (ia_vote_dense.cu); with flags bit 4 its
+  if (!(ctx->params.flags & IA_FLAG_GENERAL)) {
+    // sign-specialised form, a4 shared by the children of an xy sub-cell (ia_vote_dense.cu); with IA_FLAG_RIGOROUS_PHI its
     // rigorous-Phi instantiation
     err = launch_vote_children_fast(ctx, sp, lev, levels, k, sm, boxes_out, &n_splits, &partial);
     if (err != cudaSuccess) return err;
   } else {
-    // general form (flags bit 0, alone or with the rigorous-Phi mode of bit 4): split the hit range when there are too few events to fill the chip
+    // general form (IA_FLAG_GENERAL, alone or with the rigorous-Phi mode of IA_FLAG_RIGOROUS_PHI): split the hit range when there are too few events to fill the chip
     n_splits = (2 * sm + sp.n_events - 1) / sp.n_events;
     if (n_splits > sp.max_hits) n_splits = sp.max_hits;
     if (n_splits < 1) n_splits = 1;

@@ -31,7 +31,7 @@ template <class T> struct HitC {
 template <class T> struct HitS {
   T Tn, Dlo, Dhi;
   int valid;
-  int rig;           // params.flags bit 4: rigorous enclosure of Phi (reading f3), carried in HitC::_pad
+  int rig;           // params.IA_FLAG_RIGOROUS_PHI: rigorous enclosure of Phi (reading f3), carried in HitC::_pad
 };
 template <class T> IA_DEV HitS<T> hit_small(const HitC<T>& c) { return {c.Tn, c.Dlo, c.Dhi, c.valid, c._pad}; }
 

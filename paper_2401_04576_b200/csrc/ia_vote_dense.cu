@@ -142,7 +142,7 @@ IA_DEV unsigned settle(unsigned bits, const HitF<T>& h, int va, Iv<T> R, Iv<T> L
 }
 
 // the same with the sign class as a run-time value (one compiled body, ia_fastq.cuh)
-// RIG: rigorous-Phi mode (flags bit 4); cells whose evaluation leaves the fast form's domain there (bit 2 of the result)
+// RIG: rigorous-Phi mode (IA_FLAG_RIGOROUS_PHI); cells whose evaluation leaves the fast form's domain there (bit 2 of the result)
 // are re-taken in the general form at once
 template <class T, bool RIG = false>
 IA_DEV unsigned fast_hit_rt(const HitF<T>& h, unsigned h_addr, int ss, int va, const PairC<T>& p, const Iv<T>* zt, int nz_tile) {
@@ -232,7 +232,10 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     if (threadIdx.x == 0) ztab->zeta = zm;
   }
   __syncthreads();
-  const unsigned sh_addr = hit_address(sh);             // of record 0 (sh is already shifted by -h_begin in the SPLIT case)
+  // shared-window address of (virtual) record 0: the conversion is applied to a record that exists, sh[h_begin], and
+  // the shift is taken in unsigned arithmetic afterwards - in the SPLIT case sh itself may point below the window, where
+  // cvta.to.shared is undefined; every address formed from sh_addr is sh_addr + h*sizeof(HitF) with h >= h_begin
+  const unsigned sh_addr = hit_address(sh + h_begin) - unsigned(h_begin) * unsigned(sizeof(HitF<T>));
   // pair enumeration: R fastest, then the lambda index within its half, then the half - a warp's lambda cells share a
   // sign, and along R the sign of z_A = (z0 - z_ref) + lambda R dphi is the same for every lane of most warps, which
   // pass_vote_q uses (round 2: C4 1.2226 -> 1.2080 s; the stores of a warp are then strided, 2 bytes per cell in 1.2 s)
@@ -272,7 +275,7 @@ vote_dense_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, GridDesc 
     }
     const Iv<T>* zt = ztab->z[hf.zflip];
     if (kind != HIT_GENERAL && warp_fast) {
-      // flags bit 6: a crude enclosure over the whole z0 tile excludes this hit for every lane -> nobody votes
+      // IA_FLAG_PREFILTER: a crude enclosure over the whole z0 tile excludes this hit for every lane -> nobody votes
       // (not in the rigorous-Phi mode: the bound is built on the series value of Phi - Phi_Ax)
       if (!RIG && prefilter && __all_sync(0xffffffffu, crude_excludes(hf, pr, ztab->zeta))) continue;
       unsigned bits;
@@ -330,7 +333,7 @@ __device__ __forceinline__ void child_half(double lo, double hi, int upper, doub
   chi = upper ? hi : mid;
 }
 
-// RIG: rigorous-Phi mode (flags bit 4): the verification loop of pass_vote_qr, as in the dense kernel
+// RIG: rigorous-Phi mode (IA_FLAG_RIGOROUS_PHI): the verification loop of pass_vote_qr, as in the dense kernel
 template <class T, bool RIG = false>
 __global__ void __launch_bounds__(512, 1)
 vote_children_fast_kernel(HitSpan sp, const HitC<T>* __restrict__ staged, const ia_box* __restrict__ boxes, int lev,
@@ -531,7 +534,7 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
   // hit to hit inside every block (measured: C3's 8^5 start grid runs 28 % faster with the one-body form,
   // C1's 32^5 grid about the same, C4's 64^5 grid 0.7 % slower)
   const double wxy = std::fmin((g.hi[0] - g.lo[0]) / g.n[0], (g.hi[1] - g.lo[1]) / g.n[1]);
-  const bool coarse = (ctx->params.flags & 2u) ? true : ((ctx->params.flags & 4u) ? false : wxy > 0.5 * ctx->max_wire_r);
+  const bool coarse = (ctx->params.flags & IA_FLAG_ONE_BODY) ? true : ((ctx->params.flags & IA_FLAG_THREE_BODY) ? false : wxy > 0.5 * ctx->max_wire_r);
   dim3 grid((unsigned)blocks, (unsigned)sp.n_events, (unsigned)n_splits);
   const HitC<T>* staged = static_cast<const HitC<T>*>(ctx->staged.p);
 #define IA_LAUNCH_FAST(RT_, SPLIT_, RIG_)                                                                                    \
@@ -539,9 +542,9 @@ static cudaError_t launch_fast(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g
     err = cudaFuncSetAttribute(vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)); \
     if (err != cudaSuccess) return err;                                                                                      \
     err = launch_k(ctx, vote_dense_fast_kernel<T, RT_, SPLIT_, RIG_>, grid, dim3(threads), smem, sp, staged, g, tiles_p, tiles_z, zt, \
-                   per_split, (ctx->params.flags & 64u) ? 1 : 0, target);                                                     \
+                   per_split, (ctx->params.flags & IA_FLAG_PREFILTER) ? 1 : 0, target);                                                     \
   } while (0)
-  if (ctx->params.flags & 16u) {
+  if (ctx->params.flags & IA_FLAG_RIGOROUS_PHI) {
     // rigorous Phi: the one-body variant carries the verification loop (any grid)
     if (n_splits > 1) IA_LAUNCH_FAST(true, true, true); else IA_LAUNCH_FAST(true, false, true);
   } else if (n_splits > 1) {
@@ -595,7 +598,7 @@ static cudaError_t launch_children_fast_t(ia_ctx* ctx, const HitSpan& sp, int le
   const int threads = (k * 16 + 31) / 32 * 32;
   dim3 grid(n_splits, sp.n_events);
   const HitC<T>* staged = static_cast<const HitC<T>*>(ctx->staged.p);
-  if (ctx->params.flags & 16u) {
+  if (ctx->params.flags & IA_FLAG_RIGOROUS_PHI) {
     err = cudaFuncSetAttribute(vote_children_fast_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
     if (err != cudaSuccess) return err;
     err = launch_k(ctx, vote_children_fast_kernel<T, true>, grid, dim3(threads), smem, sp, staged, boxes, lev, levels, k, per_split, partial);
@@ -620,7 +623,7 @@ cudaError_t launch_vote_dense(ia_ctx* ctx, const HitSpan& sp, const GridDesc& g,
   // the fast form packs vote counts in bytes and keeps one HitF per hit in shared memory
   // bit 4 (rigorous Phi): sign-specialised too since round 2 (one-body variant with the verification loop); bits 0 + 4
   // together keep the general form
-  const bool fast = !(ctx->params.flags & 1u) && sp.max_hits <= 255;
+  const bool fast = !(ctx->params.flags & IA_FLAG_GENERAL) && sp.max_hits <= 255;
   if (ctx->params.precision == 32)
     return fast ? launch_fast<float>(ctx, sp, g, votes_out) : launch_general<float>(ctx, sp, g, votes_out);
   return fast ? launch_fast<double>(ctx, sp, g, votes_out) : launch_general<double>(ctx, sp, g, votes_out);

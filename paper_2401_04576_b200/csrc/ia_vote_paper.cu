@@ -71,12 +71,12 @@ __device__ void make_phit(const double* __restrict__ wires, int n_wires, ia_hit 
   const double dx = sub(xc, mx_), dy = sub(yc, my_);
   const double dt = sub(add(mul(dx, dx), mul(dy, dy)), h2);
   double dphi = atan2(cr, dt);
-  // reading M6 (flags bit 3): a counter-clockwise track of less than one turn emitted near the z axis has turned by
+  // reading M6 (IA_FLAG_FULL_TURN): a counter-clockwise track of less than one turn emitted near the z axis has turned by
   // theta in [-m, 2 pi - m), m = 0.3 rad, past the point of its base circle closest to the axis when it reaches a point
   // P of the circle; phi_Ax - phi0 of (A.8d) = theta(wire point) - theta(reference point), right wherever the
   // reference point lies along the track (it moves between passes, L98).  theta(P) = the S3 angle with the reference
   // at the axis and the wire point at P; same operations, same order as the oracle's.
-  if (p.flags & 8u) {
+  if (p.flags & IA_FLAG_FULL_TURN) {
     auto theta = [&](double px, double py) {
       const double hx_ = mul(0.5, px), hy_ = mul(0.5, py);
       const double cr0 = add(mul(sub(0.0, py), xc), mul(px, yc));
@@ -439,7 +439,7 @@ __global__ void paper_ref_kernel(const ia_hit* __restrict__ hits, int n_hits, co
     if (!(bx == x_old && by == y_old)) {
       const double xc = prev->value[0], yc = prev->value[1], two_pi = 6.283185307179586;
       double dth;
-      if (p.flags & 8u) {
+      if (p.flags & IA_FLAG_FULL_TURN) {
         auto theta = [&](double px, double py) {
           const double hx_ = mul(0.5, px), hy_ = mul(0.5, py);
           const double cr0 = add(mul(sub(0.0, py), xc), mul(px, yc));

@@ -74,8 +74,8 @@ def gather_key_lists(keys_local, dist=None):
 def split_vote_topk(ctx, hits_dev, n_hits, box_lo, box_hi, grid_dims, k, rank=0, world=1, dist=None, votes_out=None):
     """The K best cells of ONE event's dense vote computed by `world` GPUs: slab vote, local key list, all-gather, merge.
     Returns (idx[k], votes[k]) - identical on every rank and identical to ia_vote + ia_topk on one GPU - and the rank's
-    slab accumulator.  Every step is a call of the C ABI on ctx's stream; the all-gather runs on torch's current stream,
-    so the caller's streams must be ordered (bench.py and the tests use one stream for both)."""
+    slab accumulator.  Every step is a call of the C ABI on ctx's stream, and the all-gather is issued with that stream
+    current, so the three are ordered on one stream for any stream the context was built with."""
     import torch
     dims = [int(d) for d in grid_dims]
     b, e = slab_range(dims[0], rank, world)
@@ -88,6 +88,12 @@ def split_vote_topk(ctx, hits_dev, n_hits, box_lo, box_hi, grid_dims, k, rank=0,
     else:
         votes = None
         keys = torch.zeros(32, dtype=torch.int64, device=f"cuda:{ctx.device}")
-    all_keys = gather_key_lists(keys, dist)
+    # the collective is ordered against torch's CURRENT stream only; the C-ABI calls before and after it run on ctx's
+    # stream.  Making ctx's stream current for the gather puts all three on one stream, whatever stream the context has.
+    if keys.is_cuda and getattr(ctx, "stream", None) is not None:
+        with torch.cuda.stream(ctx.stream):
+            all_keys = gather_key_lists(keys, dist)
+    else:
+        all_keys = gather_key_lists(keys, dist)
     idx, v = ctx.ia_merge_keys(all_keys, all_keys.numel() // 32, k)
     return idx, v, votes

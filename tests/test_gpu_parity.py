@@ -291,7 +291,7 @@ def test_c3_refine_batch_identical(precision):
 @pytest.mark.parametrize("grid,levels,k", [((8,) * 5, 6, 8), ((4, 4, 4, 4, 5), 5, 3), ((6, 5, 4, 3, 2), 4, 32),
                                            ((3, 3, 3, 3, 3), 7, 1)])
 def test_children_fast_and_general_kernels_agree(precision, grid, levels, k):
-    """The sign-specialised children kernel against the general one (flags bit 0) and against the oracle:
+    """The sign-specialised children kernel against the general one (IA_FLAG_GENERAL) and against the oracle:
     K = 3 and 1 leave warps partly filled, an odd lambda grid makes parents whose children straddle 0,
     K = 32 is the largest list."""
     rig = Rig(g.chamber_c1(), precision=precision)
@@ -303,7 +303,7 @@ def test_children_fast_and_general_kernels_agree(precision, grid, levels, k):
         hd, oh = rig.hits(wire, drift)
         mh = max(e.n_hits for e in evs)
         out = []
-        for flags in (0, 1):
+        for flags in (0, b.FLAG_GENERAL):
             rig.ctx.ia_set_params(g.TOL, precision=precision, flags=flags)
             boxes, par = rig.ctx.ia_refine_batch(hd, rig.dev(off), len(evs), mh, LO, HI, grid, levels, k)
             rig.ctx.synchronize()
@@ -395,9 +395,42 @@ def test_host_entry_point_matches_device_path(rig0):
         assert (vd.cpu().numpy() == vh).all(), dims
 
 
+@pytest.mark.parametrize("nx,slab_min,n_slabs", [(5, 2000, 2), (7, 2200, 3), (7, 1, 7), (13, 700, 8), (11, 1, 8), (3, 1 << 40, 1)])
+def test_host_slab_pipeline_every_cell_on_ragged_grids(rig0, nx, slab_min, n_slabs):
+    """The slab pipeline of ia_vote_host (vote of slab i+1 beside the copy of slab i on a second stream) with the slab
+    size lowered so that small grids take it: 2, 3, 7 and 8 slabs of unequal width on an odd number of xc cells, every
+    cell compared with ia_vote; the buffer between canaries, a second call into the same buffer (the copies of the
+    first must be over), and the single-launch path of the same call."""
+    ev = g.make_event(rig0.ch, 5, n_noise=3)
+    hd, _ = rig0.hits(ev.wire, ev.drift)
+    hh = b.hits_of(ev.wire, ev.drift)
+    dims = (nx, 3, 6, 7, 9)
+    n = int(np.prod(dims))
+    assert min(8, nx, n // slab_min) == n_slabs or (n_slabs == 1 and n // slab_min < 2)
+    vd = rig0.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
+    rig0.ctx.synchronize()
+    vd = vd.cpu().numpy()
+    assert vd.max() > 0
+    launches0 = rig0.ctx.ia_launch_count()
+    try:
+        rig0.ctx.ia_set_host_slab_min(slab_min)
+        buf = np.full(n + 64, 0xA5A5, np.uint16)
+        for _ in range(2):
+            buf[32:32 + n] = 0xFFFF
+            rig0.ctx.ia_vote_host(hh, LO, HI, dims, votes_out=buf[32:32 + n])
+            assert (buf[32:32 + n] == vd).all(), (dims, slab_min)
+            assert (buf[:32] == 0xA5A5).all() and (buf[32 + n:] == 0xA5A5).all()
+        # one staging launch + one vote launch per slab and call (small grids may add a partial-sum launch per slab)
+        assert rig0.ctx.ia_launch_count() - launches0 >= 2 * (1 + n_slabs)
+    finally:
+        rig0.ctx.ia_set_host_slab_min(16 << 20)
+    with pytest.raises(b.IaError):
+        rig0.ctx.ia_set_host_slab_min(0)
+
+
 @pytest.mark.parametrize("precision", [64, 32])
 def test_fast_and_general_kernels_agree(precision):
-    """The sign-specialised dense kernel against the general one (flags bit 0) on a full 24^5 grid and
+    """The sign-specialised dense kernel against the general one (IA_FLAG_GENERAL) on a full 24^5 grid and
     on ragged shapes: same DAG, same roundings, so only the sin/cos pads may move a knife-edge cell."""
     rig = Rig(g.chamber_c1(), precision=precision)
     try:
@@ -406,7 +439,7 @@ def test_fast_and_general_kernels_agree(precision):
         for dims in ((24,) * 5, (5, 4, 10, 9, 12), (3, 3, 6, 20, 7), (2, 2, 64, 3, 64)):
             rig.ctx.ia_set_params(g.TOL, precision=precision, flags=0)
             vf = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
-            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=1)
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=b.FLAG_GENERAL)
             vg = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
             rig.ctx.synchronize()
             vf, vg = vf.cpu().numpy(), vg.cpu().numpy()
@@ -419,7 +452,7 @@ def test_fast_and_general_kernels_agree(precision):
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_one_body_and_three_body_variants_identical(precision):
-    """The two compiled forms of the sign-specialised dense kernel (flags bit 1: sign class as a run-time
+    """The two compiled forms of the sign-specialised dense kernel (IA_FLAG_ONE_BODY: sign class as a run-time
     value in one body; bit 2: three bodies) do the same arithmetic: votes identical bit for bit, on a
     coarse and on a fine grid, and whichever the library picks by itself equals both."""
     rig = Rig(g.chamber_c1(), precision=precision)
@@ -428,7 +461,7 @@ def test_one_body_and_three_body_variants_identical(precision):
         hd, oh = rig.hits(ev.wire, ev.drift)
         for dims in ((8,) * 5, (20, 20, 12, 9, 12), (3, 3, 6, 20, 7)):
             out = []
-            for flags in (2, 4, 0):
+            for flags in (b.FLAG_ONE_BODY, b.FLAG_THREE_BODY, 0):
                 rig.ctx.ia_set_params(g.TOL, precision=precision, flags=flags)
                 out.append(rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims))
             rig.ctx.synchronize()
@@ -535,13 +568,13 @@ def test_fast_path_primitives(rig0, prec):
 
 def test_refine_graph_replay_gives_the_same_boxes(rig1):
     """ia_refine repeated with identical arguments is replayed as a CUDA graph from the third call on: results
-    identical to the direct path (flags bit 5), also after the hits in the same buffer change, after another call
+    identical to the direct path (IA_FLAG_NO_GRAPH), also after the hits in the same buffer change, after another call
     in between, and with new output buffers."""
     cfg = g.config(2)
     ev = cfg.events[0]
     hd, oh = rig1.hits(ev.wire, ev.drift)
     ctx = rig1.ctx
-    ctx.ia_set_params(g.TOL, flags=32)
+    ctx.ia_set_params(g.TOL, flags=b.FLAG_NO_GRAPH)
     b0, p0 = ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 5, cfg.k)
     ctx.synchronize()
     ref = (b.boxes_to_numpy(b0, (5, cfg.k)).copy(), p0.cpu().numpy().copy())
@@ -662,7 +695,7 @@ def test_refine_with_no_hits(rig1):
     assert (gb["votes"] == 0).all() and (par.cpu().numpy() == opar).all()
     # a batch whose events are all empty, sign-specialised and general children kernels
     off = np.zeros(4, np.int32)
-    for flags in (0, 1):
+    for flags in (0, b.FLAG_GENERAL):
         rig1.ctx.ia_set_params(g.TOL, flags=flags)
         boxes, par = rig1.ctx.ia_refine_batch(None, rig1.dev(off), 3, 0, LO, HI, grid, levels, k)
         rig1.ctx.synchronize()
@@ -686,14 +719,14 @@ def test_many_hits_need_more_than_48k_of_shared_memory(rig1):
     vo = o.vote_boxes(rig1.owires, oh, rig1.oparams, blo, bhi)
     # 300 boxes x 600 hits = 180,000 decisions: up to three traced knife-edge boxes allowed
     compare_votes(rig1, hd, oh, vg.cpu().numpy(), vo, lambda idx: (blo[idx], bhi[idx]), min_equal=0.99, kind="boxes")
-    # general-form refinement (flags bit 0) of 300 events x 420 hits: one hit split per event, all hits in one block
+    # general-form refinement (IA_FLAG_GENERAL) of 300 events x 420 hits: one hit split per event, all hits in one block
     n_events, mh = 300, 420
     wire = rng.integers(0, rig1.ch.n_wires, n_events * mh).astype(np.int32)
     drift = rng.uniform(0.0, 1.5, n_events * mh)
     off = (np.arange(n_events + 1) * mh).astype(np.int32)
     hd, oh = rig1.hits(wire, drift)
     grid, levels, k = (3, 3, 3, 2, 2), 2, 4
-    rig1.ctx.ia_set_params(g.TOL, flags=1)
+    rig1.ctx.ia_set_params(g.TOL, flags=b.FLAG_GENERAL)
     try:
         boxes, par = rig1.ctx.ia_refine_batch(hd, rig1.dev(off), n_events, mh, LO, HI, grid, levels, k)
         rig1.ctx.synchronize()
@@ -736,7 +769,7 @@ def test_refine_graph_is_really_replayed_on_a_capturable_stream():
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_prefilter_gives_identical_votes(precision):
-    """flags bit 6: hits that a crude enclosure (magnitude bounds over a whole z0 tile) excludes for every lane of a warp
+    """IA_FLAG_PREFILTER: hits that a crude enclosure (magnitude bounds over a whole z0 tile) excludes for every lane of a warp
     are skipped.  A wider enclosure that excludes 0 implies the fine one does, so the accumulator must be identical bit for
     bit to the exhaustive kernel's - on a fine grid (where most hits are skipped), a coarse one, ragged shapes, a window
     around the truth (where few are), an odd lambda grid, and with the reference plane and point off zero."""
@@ -890,15 +923,15 @@ def test_outputs_stay_inside_their_buffers(rig1):
 
 
 def test_programmatic_dependent_launch_changes_nothing(rig1):
-    """flags bit 7 launches the chain without the programmatic-dependent-launch attribute: same boxes and parameters,
-    replayed as a graph or not (bit 5), and the same dense votes and top-K."""
+    """IA_FLAG_NO_PDL launches the chain without the programmatic-dependent-launch attribute: same boxes and parameters,
+    replayed as a graph or not (IA_FLAG_NO_GRAPH), and the same dense votes and top-K."""
     import torch
     cfg = g.config(2)
     ev = cfg.events[0]
     hd, _ = rig1.hits(ev.wire, ev.drift)
     ctx = rig1.ctx
     ref = None
-    for flags in (0, 128, 32, 160):
+    for flags in (0, b.FLAG_NO_PDL, b.FLAG_NO_GRAPH, b.FLAG_NO_PDL | b.FLAG_NO_GRAPH):
         ctx.ia_set_params(g.TOL, flags=flags)
         for _ in range(3):                                   # third call: the graph replay where it applies
             boxes, par = ctx.ia_refine(hd, ev.n_hits, LO, HI, cfg.grid, 6, cfg.k)

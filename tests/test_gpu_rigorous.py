@@ -1,4 +1,4 @@
-"""-m gpu parity of the rigorous-Phi mode (flags bit 4) against the oracle's.
+"""-m gpu parity of the rigorous-Phi mode (IA_FLAG_RIGOROUS_PHI) against the oracle's.
 
 Same algorithm on both sides (verification of the fixed point of (A.6) by inflation from the series enclosure, then
 S5-S8); they differ only in the padding of sin, cos and atan2, a few ulps per round of the verification.
@@ -13,7 +13,7 @@ from oracle import oracle as o
 from gpu_common import HI, LO, Rig, compare_votes
 
 pytestmark = pytest.mark.gpu
-RIG = 16
+RIG = b.FLAG_RIGOROUS_PHI
 
 
 @pytest.mark.parametrize("precision", [64, 32])
@@ -93,7 +93,7 @@ def test_rigorous_dense_vote_refine_and_truth_with_no_tolerance():
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_sign_specialised_rigorous_kernel_agrees_with_the_general_one(precision):
-    """flags bit 4 in the sign-specialised dense kernel (verification loop inside the one-body form, own atan2 on x > 0)
+    """IA_FLAG_RIGOROUS_PHI in the sign-specialised dense kernel (verification loop inside the one-body form, own atan2 on x > 0)
     against the general-form kernel (bits 0 + 4: library atan2 at four corners): same algorithm, roundings differ by the
     pads, so the accumulators agree except at knife edges - on a full 14^5 grid, ragged shapes and an odd lambda grid."""
     rig = Rig(g.chamber_c1(), precision=precision, flags=RIG)
@@ -103,7 +103,7 @@ def test_sign_specialised_rigorous_kernel_agrees_with_the_general_one(precision)
         for dims in ((14,) * 5, (5, 4, 10, 19, 12), (3, 3, 6, 20, 7)):
             rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG)
             vf = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
-            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | 1)
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | b.FLAG_GENERAL)
             vg = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, dims)
             rig.ctx.synchronize()
             vf, vg = vf.cpu().numpy(), vg.cpu().numpy()
@@ -116,7 +116,7 @@ def test_sign_specialised_rigorous_kernel_agrees_with_the_general_one(precision)
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_rigorous_refinement_children_kernel_matches_the_oracle(precision):
-    """flags bit 4 in the sign-specialised CHILDREN kernel (round 2; before, a rigorous refinement took the general-form
+    """IA_FLAG_RIGOROUS_PHI in the sign-specialised CHILDREN kernel (round 2; before, a rigorous refinement took the general-form
     children kernel): kept boxes, votes and parameters of a batch refinement identical to the oracle's rigorous mode at
     every level, and to the general-form kernels (bits 0 + 4)."""
     rig = Rig(g.chamber_c1(), precision=precision, flags=RIG)
@@ -134,7 +134,7 @@ def test_rigorous_refinement_children_kernel_matches_the_oracle(precision):
             ob, opar = o.refine_batch(rig.owires, oh, off, rig.oparams, LO, HI, (8,) * 5, levels, k)
             assert (gb["lo"] == ob["lo"]).all() and (gb["hi"] == ob["hi"]).all() and (gb["votes"] == ob["votes"]).all(), (levels, k)
             assert (par.cpu().numpy().reshape(opar.shape) == opar).all()
-            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | 1)
+            rig.ctx.ia_set_params(g.TOL, precision=precision, flags=RIG | b.FLAG_GENERAL)
             boxes2, par2 = rig.ctx.ia_refine_batch(hd, od, len(evs), 30, LO, HI, (8,) * 5, levels, k)
             rig.ctx.synchronize()
             g2 = b.boxes_to_numpy(boxes2, (len(evs), levels, k))
