@@ -80,6 +80,54 @@ def test_c4_stratified_sample():
     assert v_truth >= 38            # 40 genuine hits, 3-sigma tolerance on smeared drifts
 
 
+@pytest.mark.slow
+def test_c4_every_cell():
+    """"C4 full if <= 1 h": every one of the 64^5 = 1,073,741,824 cells x 60 hits of the configuration the
+    headline is quoted on (condition (4)), GPU accumulator against the oracle's, slab of xc cells by slab
+    (64 slabs of 2^24 cells; about 50 s of oracle time each on 16 cores).  Run once per round, not by default:
+
+        IA_RUN_SLOW=1 python -m pytest tests/test_gpu_fullsize.py -q -m gpu -k c4_every_cell
+
+    Progress and the final counts are written to gpurun_out/c4_full_parity.json after every slab (a run cut short still
+    leaves what it compared); BASELINE.md section 3 records the result."""
+    import json
+    import os
+    import time
+    cfg = g.config(4)
+    ev = cfg.events[0]
+    rig = Rig(cfg.chamber)
+    out_dir = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    os.makedirs(out_dir, exist_ok=True)
+    try:
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        votes = rig.ctx.ia_vote(hd, ev.n_hits, LO, HI, cfg.grid)
+        rig.ctx.synchronize()
+        vg = votes.cpu().numpy()
+        n = vg.size
+        nx = cfg.grid[0]
+        per = n // nx
+        done = {"config": "C4 64^5 x 60 hits, seed 4", "cells_total": n, "cells_compared": 0, "mismatches": 0, "traced": 0,
+                "slabs_done": 0, "oracle_seconds": 0.0, "complete": False}
+        for ix in range(nx):
+            cells = np.arange(ix * per, (ix + 1) * per, dtype=np.int64)
+            t0 = time.perf_counter()
+            vo = o.vote(rig.owires, oh, rig.oparams, LO, HI, cfg.grid, cell_idx=cells)
+            done["oracle_seconds"] += time.perf_counter() - t0
+            n_bad = compare_votes(rig, hd, oh, vg[ix * per:(ix + 1) * per], vo, lambda i: o.cell_boxes(LO, HI, cfg.grid, cells[i]))
+            done["cells_compared"] += per
+            done["mismatches"] += int(n_bad)
+            done["traced"] += int(min(n_bad, 200))          # compare_votes traces up to 200 per call and fails on an unexplained one
+            done["slabs_done"] = ix + 1
+            with open(os.path.join(out_dir, "c4_full_parity.json"), "w") as f:
+                json.dump(done, f)
+        done["complete"] = True
+        with open(os.path.join(out_dir, "c4_full_parity.json"), "w") as f:
+            json.dump(done, f)
+        assert done["cells_compared"] == n and done["mismatches"] <= n // 10000
+    finally:
+        rig.close()
+
+
 @pytest.mark.parametrize("precision", [64, 32])
 def test_c3_all_1024_events_identical(precision):
     n_events = 1024

@@ -209,7 +209,7 @@ def _fits_to_host(t, n_passes):
 
 def test_track_paper_matches_the_oracle_chain():
     """ia_track_paper against orc_track_paper on reduced grids (the oracle needs seconds per pass): every fit of every
-    pass and both chains identical, same final sign.  Tracks of more than half a turn (flags bit 3)."""
+    pass and both chains identical, same final sign.  Tracks of more than half a turn (IA_FLAG_FULL_TURN)."""
     ch = g.chamber_paper()
     rig = Rig(ch)
     try:
@@ -220,14 +220,23 @@ def test_track_paper_matches_the_oracle_chain():
                                    (300, True, (0.0, 0.0)), (301, True, (0.0, 0.0)), (303, True, (5.0, 0.0)), (304, True, (0.0, 5.0))):
             ev = g.make_event_paper(ch, seed, n_noise=3, vertex=vertex)
             hd, oh = rig.hits(ev.wire, ev.drift)
-            rig.ctx.ia_set_params(0.01, flags=8)
+            rig.ctx.ia_set_params(0.01, flags=b.FLAG_FULL_TURN)
             fits_dev, sign_dev = rig.ctx.ia_track_paper(hd, ev.n_hits, g.PAPER_P, _passes(spec, move), r_disk=10.0, factor=5.0)
             rig.ctx.synchronize()
             fg = _fits_to_host(fits_dev, len(spec))
             fo, so = o.track_paper(rig.owires, oh, o.make_params(0.01, flags=8), g.PAPER_P, 10.0, 5.0, o.make_passes(spec, move))
             assert int(sign_dev.cpu().numpy()[0]) == so
-            for name in ("lambda_sign", "vmax", "n_sel", "x_ref", "y_ref"):
+            for name in ("lambda_sign", "x_ref", "y_ref"):
                 assert (fg[name] == fo[name]).all(), (seed, move, name, fg[name], fo[name])
+            for name in ("vmax", "n_sel"):
+                # identical wherever the two sides vote the same grid.  The window of a pass whose reference point moved
+                # is centred on a z0 transported with atan2 (CUDA's against glibc's): where that centre differs in its
+                # last bits the voxel edges do too, and a knife-edge vote may flip - allowed there only, by one vote
+                same_grid = fg["z0_centre"] == fo["z0_centre"]
+                differ = fg[name] != fo[name]
+                assert not (differ & same_grid).any(), (seed, move, name, fg[name], fo[name])
+                assert not differ[:2].any(), (seed, move, name, fg[name], fo[name])
+            assert (np.abs(fg["vmax"].astype(np.int64) - fo["vmax"]) <= 1).all()
             assert np.allclose(fg["z0_centre"], fo["z0_centre"], rtol=0, atol=1e-9)      # transported with atan2: to rounding
             for name in ("value", "error", "lam"):
                 # the global passes bit for bit; the window after a moved reference point is centred on a z0 transported
@@ -244,6 +253,42 @@ def test_track_paper_matches_the_oracle_chain():
         rig.close()
 
 
+def test_table1_first_pass_every_voxel():
+    """The first pass of the paper's scheme at the size Table 1 gives it (L100-106: 50 x 50 x 40 x 20 voxels on the global
+    box), on a paper-shaped event with the disk pre-filter (3a,b) and tracks of up to one turn: both lambda-sign
+    accumulators of ia_vote_paper against orc_vote_paper, voxel for voxel (the reduced grids of the chain test above
+    keep the oracle's time down; this is the one pass at full size).  Then the selection on both sides."""
+    ch = g.chamber_paper()
+    rig = Rig(ch)
+    try:
+        ev = g.make_event_paper(ch, 500)
+        hd, oh = rig.hits(ev.wire, ev.drift)
+        dims = (50, 50, 40, 20)
+        rig.ctx.ia_set_params(0.0, flags=b.FLAG_FULL_TURN)
+        vg_dev = rig.ctx.ia_vote_paper(hd, ev.n_hits, g.PAPER_P, PLO, PHI, dims, r_disk=10.0)
+        fit_dev = rig.ctx.ia_select_max_paper(vg_dev.view(-1), g.PAPER_P, PLO, PHI, dims)
+        rig.ctx.synchronize()
+        vg = vg_dev.cpu().numpy()
+        op = o.make_params(0.0, flags=8)
+        vo = o.vote_paper(rig.owires, oh, op, g.PAPER_P, PLO, PHI, dims, r_disk=10.0)
+        assert vg.shape == vo.shape == (2, 2_000_000) and vo.max() >= 5
+        bad = np.argwhere(vg != vo)
+        assert len(bad) <= vo.size * 1e-4, len(bad)
+        if len(bad):
+            cells = np.unique(bad[:, 1])
+            blo, bhi = o.cell_boxes4(PLO, PHI, dims, cells)
+            r = o.residual_paper(rig.owires, oh, op, g.PAPER_P, blo, bhi)
+            for i in range(len(cells)):
+                knife = (r[i, ..., 3] > 0) & (np.minimum(np.abs(r[i, ..., 0]), np.abs(r[i, ..., 1])) <= 1e-12 * r[i, ..., 2])
+                assert knife.any(), f"unexplained paper-mode mismatch in voxel {cells[i]}"
+        # the selection is defined on the accumulators it is given: the oracle's on the GPU's own accumulators
+        fg, fo = _fit_to_host(fit_dev), o.select_max_paper(vg, PLO, PHI, dims, g.PAPER_P)
+        assert list(fg["value"]) == list(fo.value) and list(fg["error"]) == list(fo.error)
+        assert (fg["vmax"], fg["n_sel"], fg["lambda_sign"], fg["lam"]) == (fo.vmax, fo.n_sel, fo.lambda_sign, fo.lam)
+    finally:
+        rig.close()
+
+
 def test_track_paper_recovers_the_generated_helix():
     """Table 1 of the paper in cm (L100-106): two global passes (voxels 1.8 x 1.8 x 0.375 x 7.5 and 1.0 x 1.0 x 0.375 x 7.5
     cm) and a window of +/-2.5, 2.5, 2.5, 40 cm with voxels 0.1 x 0.1 x 0.1 x 4 cm, on noise-free paper-shaped events
@@ -253,7 +298,7 @@ def test_track_paper_recovers_the_generated_helix():
     try:
         spec = [("grid", PLO, PHI, (50, 50, 40, 20)), ("grid", PLO, PHI, (90, 90, 40, 20)),
                 ("window", (2.5, 2.5, 2.5, 40.0), (50, 50, 50, 20))]
-        rig.ctx.ia_set_params(0.0, flags=8)
+        rig.ctx.ia_set_params(0.0, flags=b.FLAG_FULL_TURN)
         for move, vertex in ((False, (0.0, 0.0)), (True, (0.0, 0.0)), (True, (5.0, 0.0))):
             ok_sign, dev = 0, []
             seeds = range(400, 424)
